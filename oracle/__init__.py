@@ -1,0 +1,134 @@
+"""CPU oracle for the all-pairs softened gravity path -- TEST INFRASTRUCTURE, NOT PRODUCT.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  The product
+(``paper_astro_ph_0703100_b200``) never imports it, and this package never imports the product.
+
+The arithmetic lives in ``nbody_oracle.c`` (plain C, double precision; see its header for the
+passages of PAPER.md each line follows).  This file only builds that C file with gcc and marshals
+numpy arrays into it through ctypes.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+from typing import Optional, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "nbody_oracle.c")
+_SO = os.path.join(_HERE, "libnbody_oracle.so")
+_lock = threading.Lock()
+_lib = None
+
+GCC_FLAGS = ["-O2", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared", "-std=c99", "-Wall"]
+
+
+def build(force: bool = False) -> str:
+    """Compile nbody_oracle.c -> libnbody_oracle.so (in-tree) if missing or stale."""
+    with _lock:
+        stale = (not os.path.exists(_SO)) or os.path.getmtime(_SO) < os.path.getmtime(_SRC)
+        if force or stale:
+            tmp = _SO + f".tmp{os.getpid()}"
+            subprocess.run(["gcc", *GCC_FLAGS, "-o", tmp, _SRC, "-lm"], check=True)
+            os.replace(tmp, _SO)
+    return _SO
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        i64, f32, f64 = ctypes.c_int64, ctypes.c_float, ctypes.c_double
+        p = ctypes.c_void_p
+        lib.oracle_force_f64.argtypes = [i64, p, i64, p, p, f64, p, p]
+        lib.oracle_force_f64.restype = ctypes.c_int
+        lib.oracle_force_f32.argtypes = [i64, p, i64, p, p, f32, p, p]
+        lib.oracle_force_f32.restype = ctypes.c_int
+        lib.oracle_energy_f32.argtypes = [i64, p, p, p, f32, p]
+        lib.oracle_energy_f32.restype = ctypes.c_int
+        lib.oracle_leapfrog_kdk_f64.argtypes = [i64, p, p, p, f64, f64, i64, p, p]
+        lib.oracle_leapfrog_kdk_f64.restype = ctypes.c_int
+        lib.oracle_num_threads.restype = ctypes.c_int
+        lib.oracle_set_num_threads.argtypes = [ctypes.c_int]
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _load().oracle_set_num_threads(int(n))
+
+
+def _c(a: np.ndarray, dtype) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def force(x_i: np.ndarray, x_j: np.ndarray, m_j: np.ndarray, eps2: float,
+          want_pot: bool = True) -> Tuple[np.ndarray, Optional[np.ndarray]]:
+    """Eq. (1) and phi in double.  float32 inputs are promoted exactly; float64 inputs are used as is.
+
+    Returns (acc float64 [n_i,3], pot float64 [n_i] or None).
+    """
+    f32 = (x_i.dtype == np.float32 and x_j.dtype == np.float32 and m_j.dtype == np.float32)
+    dt = np.float32 if f32 else np.float64
+    xi, xj, mj = _c(x_i, dt).reshape(-1, 3), _c(x_j, dt).reshape(-1, 3), _c(m_j, dt).reshape(-1)
+    n_i, n_j = xi.shape[0], xj.shape[0]
+    if mj.shape[0] != n_j:
+        raise ValueError("m_j length != n_j")
+    acc = np.zeros((n_i, 3), dtype=np.float64)
+    pot = np.zeros(n_i, dtype=np.float64) if want_pot else None
+    fn = _load().oracle_force_f32 if f32 else _load().oracle_force_f64
+    rc = fn(n_i, _ptr(xi), n_j, _ptr(xj), _ptr(mj), float(eps2), _ptr(acc), _ptr(pot))
+    if rc != 0:
+        raise ValueError(f"oracle_force returned {rc}")
+    return acc, pot
+
+
+def energy(x: np.ndarray, v: np.ndarray, m: np.ndarray, eps2: float) -> Tuple[float, float, float]:
+    """(T, W, E) in double from an FP32 state; W = 1/2 sum m_i phi_i with coincident pairs skipped."""
+    xx, vv, mm = _c(x, np.float32).reshape(-1, 3), _c(v, np.float32).reshape(-1, 3), _c(m, np.float32).reshape(-1)
+    out = np.zeros(3, dtype=np.float64)
+    rc = _load().oracle_energy_f32(xx.shape[0], _ptr(xx), _ptr(vv), _ptr(mm), float(eps2), _ptr(out))
+    if rc != 0:
+        raise ValueError(f"oracle_energy returned {rc}")
+    return float(out[0]), float(out[1]), float(out[2])
+
+
+def leapfrog_kdk(x: np.ndarray, v: np.ndarray, m: np.ndarray, eps2: float, dt: float, n_steps: int):
+    """Textbook KDK in double.  Returns (x, v, acc, pot) at the final time (inputs are not modified)."""
+    xx = np.array(x, dtype=np.float64, order="C").reshape(-1, 3)
+    vv = np.array(v, dtype=np.float64, order="C").reshape(-1, 3)
+    mm = _c(m, np.float64).reshape(-1)
+    n = xx.shape[0]
+    acc = np.zeros((n, 3), dtype=np.float64)
+    pot = np.zeros(n, dtype=np.float64)
+    rc = _load().oracle_leapfrog_kdk_f64(n, _ptr(xx), _ptr(vv), _ptr(mm), float(eps2), float(dt), int(n_steps),
+                                         _ptr(acc), _ptr(pot))
+    if rc != 0:
+        raise ValueError(f"oracle_leapfrog_kdk returned {rc}")
+    return xx, vv, acc, pot
+
+
+def error_metrics(acc_test: np.ndarray, acc_ref: np.ndarray, pot_test: Optional[np.ndarray] = None,
+                  pot_ref: Optional[np.ndarray] = None) -> dict:
+    """Eq. (3): e_i = |a_test,i - a_ref,i| / |a_ref,i|; max and RMS over i; same for phi."""
+    a_t = np.asarray(acc_test, dtype=np.float64)
+    a_r = np.asarray(acc_ref, dtype=np.float64)
+    e = np.linalg.norm(a_t - a_r, axis=1) / np.linalg.norm(a_r, axis=1)
+    out = {"acc_max": float(e.max()), "acc_rms": float(np.sqrt(np.mean(e * e)))}
+    if pot_test is not None and pot_ref is not None:
+        p = np.abs(np.asarray(pot_test, dtype=np.float64) - pot_ref) / np.abs(pot_ref)
+        out["pot_max"] = float(p.max())
+        out["pot_rms"] = float(np.sqrt(np.mean(p * p)))
+    return out

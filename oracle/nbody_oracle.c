@@ -1,0 +1,193 @@
+/*
+ * nbody_oracle.c -- the CPU ORACLE for the all-pairs softened gravity path.
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call anything in oracle/.  The CUDA
+ * path (paper_astro_ph_0703100_b200/csrc) shares no code, header, table or helper with this file
+ * and neither side includes or imports the other.
+ *
+ * What it is: the *definition* of the result, written out in double precision, plain loops, no
+ * blocking, no fusion, no reordering.  The method of the paper (the Chamomile Scheme) reaches
+ * exactly this sum, up to FP32 rounding order, just faster; so the oracle is Eq. (1) itself:
+ *
+ *     a_i = sum_j  m_j r_ij / (r_ij^2 + eps^2)^(3/2),     r_ij = r_j - r_i      PAPER.md:30-32, Eq. (1)
+ *     phi_i = - sum_j m_j / (r_ij^2 + eps^2)^(1/2)                              PAPER.md:509-516, 552 (Fig. A.4:
+ *                                                     mf = mj*r5i*r2, pot = mf*r2 = mj/sqrt(r2), OUTPUT[6] -= pot)
+ *
+ * with G = 1 (absent from Eq. (1)), the softening passed as eps^2 (PAPER.md:227, 235, 379:
+ * "eps2"), and per-pair steps in the order of the paper's pipeline description
+ * (Fig. A.3): d = r_j - r_i; r2 = d.d + eps2; r1i = 1/sqrt(r2); r2i, r3i;
+ * mr3i = m_j r3i; a += mr3i d.
+ *
+ * Reading taken where the paper is silent (reading R1): a pair whose three coordinate
+ * differences are all exactly zero ("coincident", which includes i == j when the i-set is the
+ * j-set) contributes nothing to a_i and nothing to phi_i.  Eq. (1) has no i != j test and the
+ * unmasked pipeline would add -m_i/eps to phi_i (and 0*inf = NaN when eps = 0).
+ *
+ * Accumulation: one double accumulator per component, j ascending.  With n_j <= 2^20 the rounding
+ * error of that sum is <~ n_j 2^-53 ~ 1e-10 of the summand scale, five orders below the FP32
+ * tolerances the CUDA path is held to, so no compensated summation is used.
+ *
+ * The leapfrog is the textbook kick-drift-kick scheme (not in the paper; BASELINE.json
+ * north_star bullet 4, configs[4]; reading R8):
+ *     a0 = force(x0);  per step:  v += a dt/2;  x += v dt;  a = force(x);  v += a dt/2.
+ *
+ * Pins (tests/test_oracle_pins.py): exact two-body rationals, coincident rule, momentum
+ * antisymmetry, translation / rotation / axis-permutation invariance, Plummer and uniform-sphere
+ * potential energies, brute force in exact rational arithmetic at N <= 8, large-eps limit, regular
+ * figures, softened circular binary, time reversal, dt^2 convergence.
+ * Parity unpinned: nothing in this file.  (The *value* of C4's energy drift is not pinned by the
+ * paper -- see DESIGN.md -- but that is a property of the FP32 path, not an oracle function.)
+ *
+ * Build: gcc -O2 -fopenmp -ffp-contract=off -fPIC -shared (oracle/__init__.py: build()).  No -ffast-math.
+ * OpenMP only parallelises the independent i-loop; the j-loop is sequential and ordered.
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* One i-particle against all j, Eq. (1) and phi, double precision.  out4 = (ax, ay, az, phi). */
+static void one_i(const double xi[3], int64_t n_j, const double *xj, const double *mj, double eps2,
+                  double out4[4])
+{
+    double ax = 0.0, ay = 0.0, az = 0.0, phi = 0.0;
+    for (int64_t j = 0; j < n_j; ++j) {
+        double dx = xj[3 * j + 0] - xi[0];            /* r_ij = r_j - r_i  */
+        double dy = xj[3 * j + 1] - xi[1];
+        double dz = xj[3 * j + 2] - xi[2];
+        if (dx == 0.0 && dy == 0.0 && dz == 0.0)      /* coincident pair: reading R1            */
+            continue;
+        double r2 = dx * dx + dy * dy + dz * dz + eps2; /* r_ij^2 + eps^2 */
+        double r1i = 1.0 / sqrt(r2);                  /* 1/sqrt(r2) */
+        double r2i = r1i * r1i;
+        double r3i = r2i * r1i;
+        double mr3i = mj[j] * r3i;
+        ax += mr3i * dx;                              /* OUTPUT[0..2] += mr3i * d */
+        ay += mr3i * dy;
+        az += mr3i * dz;
+        phi -= mj[j] * r1i;                           /* OUTPUT[6] -= pot */
+    }
+    out4[0] = ax; out4[1] = ay; out4[2] = az; out4[3] = phi;
+}
+
+/*
+ * Double-precision inputs.  x_i [n_i][3], x_j [n_j][3], m_j [n_j]; acc [n_i][3]; pot [n_i] or NULL.
+ * x_i may alias x_j.  Returns 0, or 1 on a bad argument.
+ */
+int oracle_force_f64(int64_t n_i, const double *x_i, int64_t n_j, const double *x_j, const double *m_j,
+                     double eps2, double *acc, double *pot)
+{
+    if (n_i < 0 || n_j < 0 || !(eps2 >= 0.0)) return 1;
+    if (n_i > 0 && (!x_i || !acc)) return 1;
+    if (n_j > 0 && (!x_j || !m_j)) return 1;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n_i; ++i) {
+        double out[4];
+        one_i(&x_i[3 * i], n_j, x_j, m_j, eps2, out);
+        acc[3 * i + 0] = out[0];
+        acc[3 * i + 1] = out[1];
+        acc[3 * i + 2] = out[2];
+        if (pot) pot[i] = out[3];
+    }
+    return 0;
+}
+
+/*
+ * FP32 inputs, each value converted exactly to double (the parity entry: the CUDA path receives
+ * the very same FP32 arrays, so input rounding never enters the comparison).  Outputs are double.
+ */
+int oracle_force_f32(int64_t n_i, const float *x_i, int64_t n_j, const float *x_j, const float *m_j,
+                     float eps2, double *acc, double *pot)
+{
+    if (n_i < 0 || n_j < 0 || !(eps2 >= 0.0f)) return 1;
+    if (n_i > 0 && (!x_i || !acc)) return 1;
+    if (n_j > 0 && (!x_j || !m_j)) return 1;
+    double *xj = (double *)malloc(sizeof(double) * 3 * (size_t)(n_j > 0 ? n_j : 1));
+    double *mj = (double *)malloc(sizeof(double) * (size_t)(n_j > 0 ? n_j : 1));
+    if (!xj || !mj) { free(xj); free(mj); return 2; }
+    for (int64_t j = 0; j < n_j; ++j) {
+        xj[3 * j + 0] = (double)x_j[3 * j + 0];
+        xj[3 * j + 1] = (double)x_j[3 * j + 1];
+        xj[3 * j + 2] = (double)x_j[3 * j + 2];
+        mj[j] = (double)m_j[j];
+    }
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n_i; ++i) {
+        double xi[3] = { (double)x_i[3 * i + 0], (double)x_i[3 * i + 1], (double)x_i[3 * i + 2] };
+        double out[4];
+        one_i(xi, n_j, xj, mj, (double)eps2, out);
+        acc[3 * i + 0] = out[0];
+        acc[3 * i + 1] = out[1];
+        acc[3 * i + 2] = out[2];
+        if (pot) pot[i] = out[3];
+    }
+    free(xj); free(mj);
+    return 0;
+}
+
+/*
+ * Total energy of a self-gravitating set: E = T + W, T = 1/2 sum m_i |v_i|^2,
+ * W = 1/2 sum m_i phi_i with the masked phi above (no self-energy).  FP32 state in (the GPU's own
+ * x, v at some step), double arithmetic.  out3 = (T, W, E).
+ */
+int oracle_energy_f32(int64_t n, const float *x, const float *v, const float *m, float eps2, double out3[3])
+{
+    if (n < 0 || !out3) return 1;
+    double *acc = (double *)malloc(sizeof(double) * 3 * (size_t)(n > 0 ? n : 1));
+    double *pot = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    if (!acc || !pot) { free(acc); free(pot); return 2; }
+    int rc = oracle_force_f32(n, x, n, x, m, eps2, acc, pot);
+    double T = 0.0, W = 0.0;
+    if (rc == 0) {
+        for (int64_t i = 0; i < n; ++i) {
+            double vx = (double)v[3 * i], vy = (double)v[3 * i + 1], vz = (double)v[3 * i + 2];
+            T += 0.5 * (double)m[i] * (vx * vx + vy * vy + vz * vz);
+            W += 0.5 * (double)m[i] * pot[i];
+        }
+        out3[0] = T; out3[1] = W; out3[2] = T + W;
+    }
+    free(acc); free(pot);
+    return rc;
+}
+
+/*
+ * Kick-drift-kick leapfrog in double precision, state updated in place.
+ * x, v [n][3]; m [n]; acc [n][3] and pot [n] receive a and phi at the final time.
+ */
+int oracle_leapfrog_kdk_f64(int64_t n, double *x, double *v, const double *m, double eps2, double dt,
+                            int64_t n_steps, double *acc, double *pot)
+{
+    if (n < 0 || n_steps < 0 || !(eps2 >= 0.0)) return 1;
+    if (n > 0 && (!x || !v || !m || !acc || !pot)) return 1;
+    int rc = oracle_force_f64(n, x, n, x, m, eps2, acc, pot);       /* a0 = force(x0) */
+    for (int64_t s = 0; s < n_steps && rc == 0; ++s) {
+        for (int64_t k = 0; k < 3 * n; ++k) v[k] += acc[k] * (0.5 * dt);   /* kick  dt/2 */
+        for (int64_t k = 0; k < 3 * n; ++k) x[k] += v[k] * dt;             /* drift dt   */
+        rc = oracle_force_f64(n, x, n, x, m, eps2, acc, pot);              /* a = force(x) */
+        for (int64_t k = 0; k < 3 * n; ++k) v[k] += acc[k] * (0.5 * dt);   /* kick  dt/2 */
+    }
+    return rc;
+}
