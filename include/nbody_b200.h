@@ -1,0 +1,135 @@
+/*
+ * nbody_b200.h -- C ABI of libnbody_b200.so: all-pairs softened gravity on one NVIDIA B200 (sm_100a).
+ *
+ * What is computed (arXiv astro-ph/0703100, Hamada & Iitaka, "The Chamomile Scheme"; citations are
+ * to /root/reference/PAPER.md by line):
+ *
+ *     a_i   =  sum_j m_j r_ij / (r_ij^2 + eps^2)^(3/2),   r_ij = r_j - r_i      Eq. (1)
+ *     phi_i = -sum_j m_j / (r_ij^2 + eps^2)^(1/2)                               Fig. A.4
+ *
+ * with G = 1, in FP32 arithmetic with an approximate reciprocal square root, as in the paper's
+ * pipeline description (Fig. A.3: all variables are float, r1i = 1/sqrt(r2)).
+ * A pair whose three coordinate differences are all exactly zero (in particular i == j when the
+ * i-set is the j-set) contributes nothing to a_i and nothing to phi_i (reading R1).
+ * The sum over j is formed as the paper's Eq. (2): partial sums over blocks of
+ * consecutive j-particles, each started from zero, added to a running total.
+ *
+ * The call shape follows the paper's only entry point, force(xj, mj, xi, eps2, a, ni, nj)
+ * (PAPER.md:235, 246, 376-382): separate i- and j-sets, so that the same call serves direct
+ * integration (i-set == j-set) and active subsets / tree interaction lists.
+ *
+ * Conventions for every function below
+ *   - plain C, no C++ types; safe to call through ctypes / dlopen.
+ *   - "device" pointers are CUDA global-memory pointers valid on the current device; "host"
+ *     pointers are ordinary process memory.  The library never takes ownership of any argument.
+ *   - counts are int64_t and must be in [0, 2^31 - 1].
+ *   - every function returns an nb_status (int); nothing throws, aborts or prints.
+ *   - functions that take a stream enqueue work on it and return without synchronising; results
+ *     are valid once the stream has reached that point.  `stream` is a cudaStream_t passed as
+ *     void*; NULL means the legacy default stream.
+ *   - results are bitwise reproducible for the same inputs, device and library build (no floating
+ *     point atomics; all reductions run in a fixed order).
+ *   - there is no CPU fallback and no other GPU architecture: a device whose compute capability
+ *     is not 10.x yields NB_ERR_UNSUPPORTED_DEVICE.
+ */
+#ifndef NBODY_B200_H
+#define NBODY_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum nb_status {
+    NB_OK = 0,
+    NB_ERR_INVALID_VALUE = 1,      /* negative / too large count, required pointer NULL, eps2 < 0 or not finite, ... */
+    NB_ERR_CUDA = 2,               /* a CUDA runtime call failed; see nb_last_cuda_error() */
+    NB_ERR_ALLOC = 3,              /* the internal workspace could not be allocated */
+    NB_ERR_UNSUPPORTED_DEVICE = 4  /* current device is not compute capability 10.x */
+} nb_status;
+
+/*
+ * nb_force -- Eq. (1) and phi for n_i i-particles against n_j j-particles.
+ *
+ *   n_i      number of i-particles (particles that receive a force)
+ *   x_i      device, const, float [n_i][3]   positions (x,y,z) of the i-particles, 4-byte aligned
+ *   n_j      number of j-particles (particles that exert a force)
+ *   x_j      device, const, float [n_j][3]   positions of the j-particles
+ *   m_j      device, const, float [n_j]      masses of the j-particles
+ *   eps2     softening length SQUARED ("eps2"), >= 0 and finite
+ *   acc_out  device, float [n_i][3]          receives a_i; required when n_i > 0
+ *   pot_out  device, float [n_i]             receives phi_i; may be NULL (phi is then not stored)
+ *   stream   cudaStream_t as void*
+ *
+ * x_i may alias x_j (i-set == j-set).  acc_out / pot_out must not overlap any input.
+ * n_i == 0: NB_OK, nothing is written.  n_j == 0: NB_OK, outputs are zero-filled.
+ * Inputs are not validated on the device: non-finite or |x| > ~1e18 inputs give undefined values.
+ * Uses an internal per-stream workspace (packed j records, j-split partial sums) that grows on
+ * demand with stream-ordered allocation; once warm the call is CUDA-graph capturable.
+ */
+int nb_force(int64_t n_i, const float *x_i,
+             int64_t n_j, const float *x_j, const float *m_j,
+             float eps2,
+             float *acc_out, float *pot_out,
+             void *stream);
+
+/*
+ * nb_force_host -- the same operation on HOST arrays: copies the inputs to the device, runs
+ * nb_force, copies a and phi back and waits for completion.  This is the paper's force() with its
+ * steps (a) and (l) -- host->device and device->host transfers -- inside the call
+ * (PAPER.md:151, 167, 233-237).  All pointers are host pointers with the layouts of nb_force.
+ * Blocking.  pot_out may be NULL.
+ */
+int nb_force_host(int64_t n_i, const float *x_i,
+                  int64_t n_j, const float *x_j, const float *m_j,
+                  float eps2,
+                  float *acc_out, float *pot_out);
+
+/*
+ * nb_leapfrog_kdk -- n_steps kick-drift-kick leapfrog steps with all state on the device.
+ * (Not in the paper; BASELINE.json north_star bullet 4 and configs[4]; reading R8.)
+ *
+ *     a = force(x)                      once, before the first step
+ *     repeat n_steps times:
+ *         v += a * (dt/2);  x += v * dt;  a = force(x);  v += a * (dt/2)
+ *
+ *   n        number of particles (i-set == j-set == all)
+ *   x, v     device, float [n][3], updated in place
+ *   m        device, const, float [n]
+ *   eps2     softening squared, >= 0, finite;   dt  finite;   n_steps >= 0
+ *   acc_io   device, float [n][3]: receives a at the final time (its content on entry is ignored)
+ *   pot_out  device, float [n]: receives phi at the final time; may be NULL
+ *
+ * n_steps == 0 only evaluates a and phi of the given state.
+ */
+int nb_leapfrog_kdk(int64_t n, float *x, float *v, const float *m,
+                    float eps2, float dt, int64_t n_steps,
+                    float *acc_io, float *pot_out,
+                    void *stream);
+
+/*
+ * nb_plan_query -- the decomposition the launch planner picks for (n_i, n_j) on a device with
+ * sm_count SMs (pure host function, no CUDA call; sm_count <= 0 means 148).
+ * out[0] = K  i-particles per thread        out[1] = WI warps per CTA along i
+ * out[2] = WJ warps per CTA along j         out[3] = S  j-chunks across CTAs (grid.y)
+ * out[4] = number of i-tiles (grid.x)       out[5] = i-particles per CTA tile (32*K*WI)
+ * out[6] = j-pairs per shared-memory stage  out[7] = pipeline stages
+ */
+int nb_plan_query(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]);
+
+/* Number of kernel launches the most recent nb_force / nb_leapfrog_kdk / nb_force_host call of this thread enqueued. */
+int64_t nb_last_launch_count(void);
+
+/* Frees every internal workspace of the current device (synchronises the device). */
+int nb_release_workspace(void);
+
+const char *nb_status_string(int status);   /* static storage */
+int nb_last_cuda_error(void);                /* cudaError_t behind this thread's last NB_ERR_CUDA / NB_ERR_ALLOC */
+int nb_version(void);                        /* major*10000 + minor*100 + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NBODY_B200_H */

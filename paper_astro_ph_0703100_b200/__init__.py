@@ -1,0 +1,17 @@
+"""B200-native all-pairs softened gravity (Hamada & Iitaka, arXiv astro-ph/0703100), sm_100a only.
+
+The product is ``libnbody_b200.so`` (C ABI, ``include/nbody_b200.h``); this package is the thin
+Python binding over it (argument marshalling only) plus the seeded workload generators.
+"""
+from .binding import (  # noqa: F401
+    NBError,
+    force,
+    force_host,
+    last_launch_count,
+    leapfrog_kdk,
+    lib,
+    plan_query,
+    release_workspace,
+    status_string,
+    version,
+)

@@ -1,0 +1,160 @@
+"""ctypes binding over libnbody_b200.so -- same names as the C ABI, argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; nothing here computes.  PyTorch
+tensors are used for device memory and streams only (``tensor.data_ptr()``,
+``torch.cuda.current_stream().cuda_stream``).  There is no CPU fallback: if the shared library
+is missing or no sm_100 device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Tuple
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libnbody_b200.so")
+
+NB_OK = 0
+_lib = None
+
+
+class NBError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        l = lib()
+        msg = l.nb_status_string(status).decode()
+        cuda = l.nb_last_cuda_error()
+        super().__init__(f"{where}: status {status} ({msg}); last cudaError_t = {cuda}")
+
+
+def lib() -> ctypes.CDLL:
+    """Loads the in-tree shared library (raises if it has not been built: no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_astro_ph_0703100_b200.build` "
+                "(or __graft_entry__.build()); there is no fallback path")
+        l = ctypes.CDLL(LIB_PATH)
+        i64, f32, p, ci = ctypes.c_int64, ctypes.c_float, ctypes.c_void_p, ctypes.c_int
+        l.nb_force.argtypes = [i64, p, i64, p, p, f32, p, p, p]
+        l.nb_force.restype = ci
+        l.nb_force_host.argtypes = [i64, p, i64, p, p, f32, p, p]
+        l.nb_force_host.restype = ci
+        l.nb_leapfrog_kdk.argtypes = [i64, p, p, p, f32, f32, i64, p, p, p]
+        l.nb_leapfrog_kdk.restype = ci
+        l.nb_plan_query.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
+        l.nb_plan_query.restype = ci
+        l.nb_last_launch_count.restype = i64
+        l.nb_release_workspace.restype = ci
+        l.nb_status_string.argtypes = [ci]
+        l.nb_status_string.restype = ctypes.c_char_p
+        l.nb_last_cuda_error.restype = ci
+        l.nb_version.restype = ci
+        _lib = l
+    return _lib
+
+
+def _check(status: int, where: str) -> None:
+    if status != NB_OK:
+        raise NBError(status, where)
+
+
+def _dev_f32(t, name: str, shape_tail: Tuple[int, ...]):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+        raise TypeError(f"{name} must be a contiguous float32 CUDA tensor")
+    if tuple(t.shape[1:]) != shape_tail:
+        raise ValueError(f"{name} must have shape [n{''.join(', %d' % s for s in shape_tail)}]")
+    return t
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def force(x_i, x_j, m_j, eps2: float, acc_out=None, pot_out=None, want_pot: bool = True, stream=None):
+    """nb_force on CUDA tensors.  Returns (acc [n_i,3], pot [n_i] or None); asynchronous on the stream."""
+    import torch
+    _dev_f32(x_i, "x_i", (3,)); _dev_f32(x_j, "x_j", (3,)); _dev_f32(m_j, "m_j", ())
+    n_i, n_j = x_i.shape[0], x_j.shape[0]
+    if m_j.shape[0] != n_j:
+        raise ValueError("m_j length != n_j")
+    if acc_out is None:
+        acc_out = torch.empty((n_i, 3), dtype=torch.float32, device=x_i.device)
+    if pot_out is None and want_pot:
+        pot_out = torch.empty((n_i,), dtype=torch.float32, device=x_i.device)
+    _dev_f32(acc_out, "acc_out", (3,))
+    if pot_out is not None:
+        _dev_f32(pot_out, "pot_out", ())
+    with torch.cuda.device(x_i.device):
+        st = lib().nb_force(n_i, x_i.data_ptr(), n_j, x_j.data_ptr(), m_j.data_ptr(), float(eps2),
+                            acc_out.data_ptr(), None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_force")
+    return acc_out, pot_out
+
+
+def force_host(x_i, x_j, m_j, eps2: float, want_pot: bool = True, acc_out=None, pot_out=None):
+    """nb_force_host on numpy float32 arrays (or pinned CPU tensors' numpy views).  Blocking."""
+    import numpy as np
+    xi = np.ascontiguousarray(x_i, dtype=np.float32).reshape(-1, 3) if x_i is not x_j else None
+    xj = np.ascontiguousarray(x_j, dtype=np.float32).reshape(-1, 3)
+    mj = np.ascontiguousarray(m_j, dtype=np.float32).reshape(-1)
+    if xi is None:
+        xi = xj
+    n_i, n_j = xi.shape[0], xj.shape[0]
+    if mj.shape[0] != n_j:
+        raise ValueError("m_j length != n_j")
+    if acc_out is None:
+        acc_out = np.empty((n_i, 3), dtype=np.float32)
+    if pot_out is None and want_pot:
+        pot_out = np.empty((n_i,), dtype=np.float32)
+    st = lib().nb_force_host(n_i, xi.ctypes.data, n_j, xj.ctypes.data, mj.ctypes.data, float(eps2),
+                             acc_out.ctypes.data, None if pot_out is None else pot_out.ctypes.data)
+    _check(st, "nb_force_host")
+    return acc_out, pot_out
+
+
+def leapfrog_kdk(x, v, m, eps2: float, dt: float, n_steps: int, acc_io=None, pot_out=None, want_pot: bool = True,
+                 stream=None):
+    """nb_leapfrog_kdk: x, v updated IN PLACE.  Returns (acc, pot) at the final time."""
+    import torch
+    _dev_f32(x, "x", (3,)); _dev_f32(v, "v", (3,)); _dev_f32(m, "m", ())
+    n = x.shape[0]
+    if v.shape[0] != n or m.shape[0] != n:
+        raise ValueError("x, v, m lengths differ")
+    if acc_io is None:
+        acc_io = torch.empty((n, 3), dtype=torch.float32, device=x.device)
+    if pot_out is None and want_pot:
+        pot_out = torch.empty((n,), dtype=torch.float32, device=x.device)
+    with torch.cuda.device(x.device):
+        st = lib().nb_leapfrog_kdk(n, x.data_ptr(), v.data_ptr(), m.data_ptr(), float(eps2), float(dt), int(n_steps),
+                                   acc_io.data_ptr(), None if pot_out is None else pot_out.data_ptr(),
+                                   _stream_ptr(stream))
+    _check(st, "nb_leapfrog_kdk")
+    return acc_io, pot_out
+
+
+def plan_query(n_i: int, n_j: int, sm_count: int = 148) -> dict:
+    out = (ctypes.c_int64 * 8)()
+    _check(lib().nb_plan_query(int(n_i), int(n_j), int(sm_count), out), "nb_plan_query")
+    keys = ("K", "WI", "WJ", "S", "tiles_i", "tile_i", "tile_pairs", "stages")
+    return dict(zip(keys, [int(v) for v in out]))
+
+
+def last_launch_count() -> int:
+    return int(lib().nb_last_launch_count())
+
+
+def release_workspace() -> None:
+    _check(lib().nb_release_workspace(), "nb_release_workspace")
+
+
+def status_string(status: int) -> str:
+    return lib().nb_status_string(int(status)).decode()
+
+
+def version() -> int:
+    return int(lib().nb_version())

@@ -1,0 +1,350 @@
+// nbody_b200.cu -- C-ABI shim, workspace and launch logic of libnbody_b200.so (include/nbody_b200.h).
+#include "../../include/nbody_b200.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <map>
+#include <mutex>
+#include <tuple>
+#include <unordered_map>
+
+#include "nb_kernels.cuh"
+#include "nb_plan.h"
+
+#define NB_VERSION 100
+
+namespace {
+
+thread_local int t_last_cuda_error = 0;
+thread_local int64_t t_launches = 0;
+
+#define NB_CUDA(call)                                  \
+    do {                                               \
+        cudaError_t e__ = (call);                      \
+        if (e__ != cudaSuccess) {                      \
+            t_last_cuda_error = (int)e__;              \
+            (void)cudaGetLastError();                  \
+            return NB_ERR_CUDA;                        \
+        }                                              \
+    } while (0)
+
+struct DeviceInfo {
+    bool known = false;
+    bool supported = false;
+    int sm_count = 0;
+};
+
+struct Workspace {
+    void* jp = nullptr;        size_t jp_bytes = 0;        // packed pair records
+    void* partial = nullptr;   size_t partial_bytes = 0;   // [S][n_i] double4
+    void* stage = nullptr;     size_t stage_bytes = 0;     // device copies for nb_force_host
+};
+
+std::mutex g_mutex;
+DeviceInfo g_dev[64];
+std::map<std::pair<int, cudaStream_t>, Workspace> g_ws;
+std::map<std::tuple<int64_t, int64_t, int>, nb::Plan> g_plans;
+
+int device_info(int* dev_out, DeviceInfo* out) {
+    int dev = 0;
+    NB_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return NB_ERR_UNSUPPORTED_DEVICE;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    DeviceInfo& d = g_dev[dev];
+    if (!d.known) {
+        int major = 0;
+        NB_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        NB_CUDA(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
+        d.supported = (major == 10);
+        d.known = true;
+    }
+    *dev_out = dev;
+    *out = d;
+    return d.supported ? NB_OK : NB_ERR_UNSUPPORTED_DEVICE;
+}
+
+// grow-only, stream-ordered
+int ensure(void** ptr, size_t* have, size_t need, cudaStream_t stream) {
+    if (need <= *have) return NB_OK;
+    size_t want = need + need / 4 + 256;
+    void* fresh = nullptr;
+    cudaError_t e = cudaMallocAsync(&fresh, want, stream);
+    if (e != cudaSuccess) {
+        t_last_cuda_error = (int)e;
+        (void)cudaGetLastError();
+        return NB_ERR_ALLOC;
+    }
+    if (*ptr) NB_CUDA(cudaFreeAsync(*ptr, stream));
+    *ptr = fresh;
+    *have = want;
+    return NB_OK;
+}
+
+nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count) {
+    std::lock_guard<std::mutex> lock(g_mutex);
+    auto key = std::make_tuple(n_i, n_j, sm_count);
+    auto it = g_plans.find(key);
+    if (it != g_plans.end() && !std::getenv("NB_PLAN")) return it->second;
+    nb::Plan p = nb::make_plan(n_i, n_j, sm_count);
+    if (g_plans.size() > 4096) g_plans.clear();
+    g_plans[key] = p;
+    return p;
+}
+
+bool exact_mask_enabled() {
+    // debugging aid: NB_MASK=approx selects the 2-instruction (r2 == eps2) coincidence test
+    static int v = -1;
+    if (v < 0) {
+        const char* e = std::getenv("NB_MASK");
+        v = (e && e[0] == 'a') ? 0 : 1;
+    }
+    return v == 1;
+}
+
+template <int K, int WI, int WJ, int TP, int STAGES, bool EXACT>
+int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
+    constexpr size_t ring = (size_t)WJ * STAGES * TP * 32;
+    constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
+    constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
+    auto kern = nb::nb_force_kernel<K, WI, WJ, TP, STAGES, EXACT>;
+    static bool configured[64] = {};
+    int dev = 0;
+    NB_CUDA(cudaGetDevice(&dev));
+    if (!configured[dev & 63]) {
+        NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured[dev & 63] = true;
+    }
+    dim3 grid((unsigned)plan.tiles_i, (unsigned)plan.S, 1);
+    kern<<<grid, 32 * WI * WJ, smem, stream>>>(args);
+    NB_CUDA(cudaGetLastError());
+    ++t_launches;
+    return NB_OK;
+}
+
+template <int K, bool EXACT>
+int launch_force_k(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
+    switch (plan.WJ) {
+        case 1: return launch_force_inst<K, 8, 1, 256, 4, EXACT>(args, plan, stream);
+        case 2: return launch_force_inst<K, 4, 2, 256, 4, EXACT>(args, plan, stream);
+        case 4: return launch_force_inst<K, 2, 4, 128, 4, EXACT>(args, plan, stream);
+        default: return launch_force_inst<K, 1, 8, 128, 3, EXACT>(args, plan, stream);
+    }
+}
+
+template <bool EXACT>
+int launch_force(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
+    switch (plan.K) {
+        case 1: return launch_force_k<1, EXACT>(args, plan, stream);
+        case 2: return launch_force_k<2, EXACT>(args, plan, stream);
+        default: return launch_force_k<4, EXACT>(args, plan, stream);
+    }
+}
+
+bool bad_count(int64_t n) { return n < 0 || n > (int64_t)INT32_MAX; }
+
+// pack (a1) when repack is true, then force (+ reduce).  The packed array lives in the workspace.
+int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
+               float* acc_out, float* pot_out, cudaStream_t stream) {
+    if (bad_count(n_i) || bad_count(n_j)) return NB_ERR_INVALID_VALUE;
+    if (!(eps2 >= 0.0f) || !std::isfinite(eps2)) return NB_ERR_INVALID_VALUE;
+    if (n_i > 0 && (!x_i || !acc_out)) return NB_ERR_INVALID_VALUE;
+    if (n_j > 0 && (!x_j || !m_j)) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n_i == 0) return NB_OK;
+    if (n_j == 0) {
+        NB_CUDA(cudaMemsetAsync(acc_out, 0, sizeof(float) * 3 * (size_t)n_i, stream));
+        if (pot_out) NB_CUDA(cudaMemsetAsync(pot_out, 0, sizeof(float) * (size_t)n_i, stream));
+        return NB_OK;
+    }
+    const nb::Plan plan = cached_plan(n_i, n_j, info.sm_count);
+
+    Workspace* ws;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        ws = &g_ws[std::make_pair(dev, stream)];
+    }
+    rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)plan.n_pairs_padded * 32, stream);
+    if (rc != NB_OK) return rc;
+    if (plan.S > 1) {
+        rc = ensure(&ws->partial, &ws->partial_bytes, (size_t)plan.S * (size_t)n_i * sizeof(double4), stream);
+        if (rc != NB_OK) return rc;
+    }
+
+    {   // a1: j-pack
+        const int threads = 256;
+        const int blocks = (int)((plan.n_pairs_padded + threads - 1) / threads);
+        nb::nb_pack_pairs_kernel<<<blocks, threads, 0, stream>>>(x_j, m_j, (int)n_j, (int)plan.n_pairs_padded,
+                                                                 reinterpret_cast<float4*>(ws->jp));
+        NB_CUDA(cudaGetLastError());
+        ++t_launches;
+    }
+
+    nb::ForceArgs args;
+    args.x_i = x_i;
+    args.jp = reinterpret_cast<const ulonglong2*>(ws->jp);
+    args.acc = acc_out;
+    args.pot = pot_out;
+    args.partial = reinterpret_cast<double4*>(ws->partial);
+    args.n_i = (int)n_i;
+    args.n_units = (int)(plan.n_pairs_padded / nb::kUnitPairs);
+    args.S = plan.S;
+    args.eps2 = eps2;
+    rc = exact_mask_enabled() ? launch_force<true>(args, plan, stream) : launch_force<false>(args, plan, stream);
+    if (rc != NB_OK) return rc;
+
+    if (plan.S > 1) {
+        const int threads = 128;
+        const int blocks = (int)((n_i + threads - 1) / threads);
+        nb::nb_reduce_kernel<<<blocks, threads, 0, stream>>>(reinterpret_cast<const double4*>(ws->partial), (int)n_i,
+                                                             plan.S, acc_out, pot_out);
+        NB_CUDA(cudaGetLastError());
+        ++t_launches;
+    }
+    return NB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int nb_force(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
+             float* acc_out, float* pot_out, void* stream) {
+    t_launches = 0;
+    return force_impl(n_i, x_i, n_j, x_j, m_j, eps2, acc_out, pot_out, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int nb_force_host(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
+                  float* acc_out, float* pot_out) {
+    t_launches = 0;
+    if (bad_count(n_i) || bad_count(n_j)) return NB_ERR_INVALID_VALUE;
+    if (!(eps2 >= 0.0f) || !std::isfinite(eps2)) return NB_ERR_INVALID_VALUE;
+    if (n_i > 0 && (!x_i || !acc_out)) return NB_ERR_INVALID_VALUE;
+    if (n_j > 0 && (!x_j || !m_j)) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n_i == 0) return NB_OK;
+    cudaStream_t stream = nullptr;   // legacy default stream
+    Workspace* ws;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        ws = &g_ws[std::make_pair(dev, stream)];
+    }
+    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
+    const bool aliased = (x_i == x_j && n_i <= n_j);
+    const size_t b_xj = up(sizeof(float) * 3 * (size_t)n_j), b_mj = up(sizeof(float) * (size_t)n_j);
+    const size_t b_xi = aliased ? 0 : up(sizeof(float) * 3 * (size_t)n_i);
+    const size_t b_acc = up(sizeof(float) * 3 * (size_t)n_i), b_pot = up(sizeof(float) * (size_t)n_i);
+    rc = ensure(&ws->stage, &ws->stage_bytes, b_xj + b_mj + b_xi + b_acc + b_pot + 256, stream);
+    if (rc != NB_OK) return rc;
+    char* base = reinterpret_cast<char*>(ws->stage);
+    float* d_xj = reinterpret_cast<float*>(base);
+    float* d_mj = reinterpret_cast<float*>(base + b_xj);
+    float* d_xi = aliased ? d_xj : reinterpret_cast<float*>(base + b_xj + b_mj);
+    float* d_acc = reinterpret_cast<float*>(base + b_xj + b_mj + b_xi);
+    float* d_pot = reinterpret_cast<float*>(base + b_xj + b_mj + b_xi + b_acc);
+    // step (a): host -> device
+    if (n_j > 0) {
+        NB_CUDA(cudaMemcpyAsync(d_xj, x_j, sizeof(float) * 3 * (size_t)n_j, cudaMemcpyHostToDevice, stream));
+        NB_CUDA(cudaMemcpyAsync(d_mj, m_j, sizeof(float) * (size_t)n_j, cudaMemcpyHostToDevice, stream));
+    }
+    if (!aliased) NB_CUDA(cudaMemcpyAsync(d_xi, x_i, sizeof(float) * 3 * (size_t)n_i, cudaMemcpyHostToDevice, stream));
+    rc = force_impl(n_i, d_xi, n_j, d_xj, d_mj, eps2, d_acc, pot_out ? d_pot : nullptr, stream);
+    if (rc != NB_OK) return rc;
+    // step (l): device -> host
+    NB_CUDA(cudaMemcpyAsync(acc_out, d_acc, sizeof(float) * 3 * (size_t)n_i, cudaMemcpyDeviceToHost, stream));
+    if (pot_out) NB_CUDA(cudaMemcpyAsync(pot_out, d_pot, sizeof(float) * (size_t)n_i, cudaMemcpyDeviceToHost, stream));
+    NB_CUDA(cudaStreamSynchronize(stream));
+    return NB_OK;
+}
+
+int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, float dt, int64_t n_steps,
+                    float* acc_io, float* pot_out, void* stream_) {
+    t_launches = 0;
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (bad_count(n) || n_steps < 0) return NB_ERR_INVALID_VALUE;
+    if (!(eps2 >= 0.0f) || !std::isfinite(eps2) || !std::isfinite(dt)) return NB_ERR_INVALID_VALUE;
+    if (n > 0 && (!x || !v || !m || !acc_io)) return NB_ERR_INVALID_VALUE;
+    if (3 * n > (int64_t)INT32_MAX) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n == 0) return NB_OK;
+    const int n3 = (int)(3 * n);
+    const int threads = 256, blocks = (n3 + threads - 1) / threads;
+    const float h = 0.5f * dt;
+    // a0 = force(x0)
+    rc = force_impl(n, x, n, x, m, eps2, acc_io, pot_out, stream);
+    if (rc != NB_OK) return rc;
+    for (int64_t s = 0; s < n_steps; ++s) {
+        // opening half-kick + drift; from the second step on it also carries the previous step's
+        // closing half-kick (two separately rounded kicks, identical to the unfused sequence)
+        if (s == 0)
+            nb::nb_kick_drift_kernel<false><<<blocks, threads, 0, stream>>>(x, v, acc_io, n3, h, dt);
+        else
+            nb::nb_kick_drift_kernel<true><<<blocks, threads, 0, stream>>>(x, v, acc_io, n3, h, dt);
+        NB_CUDA(cudaGetLastError());
+        ++t_launches;
+        rc = force_impl(n, x, n, x, m, eps2, acc_io, pot_out, stream);
+        if (rc != NB_OK) return rc;
+    }
+    if (n_steps > 0) {
+        nb::nb_kick_kernel<<<blocks, threads, 0, stream>>>(v, acc_io, n3, h);   // closing half-kick of the last step
+        NB_CUDA(cudaGetLastError());
+        ++t_launches;
+    }
+    return NB_OK;
+}
+
+int nb_plan_query(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]) {
+    if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
+    const nb::Plan p = nb::make_plan(n_i, n_j, sm_count);
+    out[0] = p.K; out[1] = p.WI; out[2] = p.WJ; out[3] = p.S;
+    out[4] = p.tiles_i; out[5] = p.tile_i; out[6] = p.tile_pairs; out[7] = p.stages;
+    return NB_OK;
+}
+
+int64_t nb_last_launch_count(void) { return t_launches; }
+
+int nb_release_workspace(void) {
+    int dev = 0;
+    NB_CUDA(cudaGetDevice(&dev));
+    NB_CUDA(cudaDeviceSynchronize());
+    std::lock_guard<std::mutex> lock(g_mutex);
+    for (auto it = g_ws.begin(); it != g_ws.end();) {
+        if (it->first.first == dev) {
+            if (it->second.jp) (void)cudaFree(it->second.jp);
+            if (it->second.partial) (void)cudaFree(it->second.partial);
+            if (it->second.stage) (void)cudaFree(it->second.stage);
+            it = g_ws.erase(it);
+        } else {
+            ++it;
+        }
+    }
+    return NB_OK;
+}
+
+const char* nb_status_string(int status) {
+    switch (status) {
+        case NB_OK: return "NB_OK";
+        case NB_ERR_INVALID_VALUE: return "NB_ERR_INVALID_VALUE: bad count, NULL required pointer, or eps2/dt out of range";
+        case NB_ERR_CUDA: return "NB_ERR_CUDA: a CUDA runtime call failed (see nb_last_cuda_error)";
+        case NB_ERR_ALLOC: return "NB_ERR_ALLOC: workspace allocation failed";
+        case NB_ERR_UNSUPPORTED_DEVICE: return "NB_ERR_UNSUPPORTED_DEVICE: compute capability 10.x (B200, sm_100a) required";
+        default: return "unknown nb_status";
+    }
+}
+
+int nb_last_cuda_error(void) { return t_last_cuda_error; }
+
+int nb_version(void) { return NB_VERSION; }
+
+}  // extern "C"

@@ -1,0 +1,244 @@
+"""Parity of the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle.
+
+Tolerances are BASELINE.json north_star's: per-particle relative acceleration error
+|a_gpu - a_ref| / |a_ref| (Eq. (3)): RMS <= 1e-5 and max <= 1e-4; relative potential
+error <= 1e-5 RMS.  All inputs are seeded and synthetic (paper_astro_ph_0703100_b200/workloads.py).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_astro_ph_0703100_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+ACC_RMS_TOL = 1e-5
+ACC_MAX_TOL = 1e-4
+POT_RMS_TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def nb():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    import paper_astro_ph_0703100_b200 as nb_
+    nb_.lib()
+    return nb_
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_force(nb, x_i, x_j, m_j, eps2, want_pot=True, alias=False):
+    import torch
+    d_xj = dev(x_j)
+    d_xi = d_xj if alias else dev(x_i)
+    acc, pot = nb.force(d_xi, d_xj, dev(m_j), eps2, want_pot=want_pot)
+    torch.cuda.synchronize()
+    return acc.cpu().numpy(), (None if pot is None else pot.cpu().numpy())
+
+
+def check_parity(acc, pot, ref_acc, ref_pot, label=""):
+    e = oracle.error_metrics(acc, ref_acc, pot, ref_pot)
+    assert e["acc_rms"] <= ACC_RMS_TOL, (label, e)
+    assert e["acc_max"] <= ACC_MAX_TOL, (label, e)
+    if pot is not None:
+        assert e["pot_rms"] <= POT_RMS_TOL, (label, e)
+    return e
+
+
+# ------------------------------------------------------------------ element-by-element, small
+def test_c0_full_parity(nb):
+    w = wl.config(0)
+    acc, pot = gpu_force(nb, w.xi, w.x_j, w.m_j, w.eps2, alias=True)
+    ref_acc, ref_pot = oracle.force(w.xi, w.x_j, w.m_j, w.eps2)
+    e = check_parity(acc, pot, ref_acc, ref_pot, "C0")
+    # paper's Table 2: blocked FP32 sums give E_max ~ 3e-7 ... 1.5e-6; same order here
+    assert e["acc_max"] < 2e-5
+
+
+@pytest.mark.parametrize("n_i,n_j", [(1500, 4999), (31, 1000), (1, 777), (129, 8), (1025, 2051), (4096, 513)])
+def test_ragged_shapes_separate_sets(nb, n_i, n_j):
+    rng = np.random.default_rng(n_i * 7919 + n_j)
+    pos_j, _ = wl.plummer_positions(n_j, rng)
+    pos_i, _ = wl.plummer_positions(n_i, rng)
+    m = rng.uniform(0.5, 1.5, n_j) / n_j
+    x_i, x_j, m_j = pos_i.astype(np.float32), pos_j.astype(np.float32), m.astype(np.float32)
+    eps2 = np.float32(2.0 ** -12)
+    acc, pot = gpu_force(nb, x_i, x_j, m_j, eps2)
+    ref_acc, ref_pot = oracle.force(x_i, x_j, m_j, eps2)
+    check_parity(acc, pot, ref_acc, ref_pot, f"{n_i}x{n_j}")
+
+
+PLANS = [(k, 8 // wj, wj, s) for k in (1, 2, 4) for wj in (1, 2, 4, 8) for s in (1, 3)]
+
+
+@pytest.mark.parametrize("plan", PLANS, ids=lambda p: "K%d_WI%d_WJ%d_S%d" % p)
+def test_every_decomposition_matches_oracle(nb, plan, monkeypatch):
+    """Each kernel instantiation (K x WJ) with and without the second-pass reduce (S)."""
+    monkeypatch.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
+    w = wl.subset_workload(3001, 777, 1.0 / 128, seed=21)
+    acc, pot = gpu_force(nb, w.x_i, w.x_j, w.m_j, w.eps2)
+    ref_acc, ref_pot = oracle.force(w.x_i, w.x_j, w.m_j, w.eps2)
+    check_parity(acc, pot, ref_acc, ref_pot, str(plan))
+
+
+def test_approximate_mask_variant(nb, monkeypatch):
+    # NB_MASK is read once per process; this only checks the default (exact) path is the one running
+    w = wl.config(0)
+    acc, pot = gpu_force(nb, w.xi, w.x_j, w.m_j, w.eps2, alias=True)
+    ref_acc, ref_pot = oracle.force(w.xi, w.x_j, w.m_j, w.eps2)
+    # the self term would shift phi by m/eps = 64/2048 = 3e-2 absolute (~3 % relative): far outside tolerance
+    check_parity(acc, pot, ref_acc, ref_pot, "C0 mask")
+
+
+# ------------------------------------------------------------------ edge cases
+def test_coincident_and_eps0(nb):
+    # same point: a = 0, phi = 0, for eps2 = 0 too (no NaN)
+    x = np.array([[1.5, -2.0, 0.25]], dtype=np.float32)
+    m = np.array([3.0], dtype=np.float32)
+    for eps2 in (0.0, 1e-4):
+        acc, pot = gpu_force(nb, x, x, m, eps2)
+        assert np.all(acc == 0.0) and pot[0] == 0.0
+    # duplicates in the j-set, eps2 = 0, distinct third particle
+    xj = np.array([[1, 1, 1], [1, 1, 1], [4, 1, 1]], dtype=np.float32)
+    mj = np.array([5.0, 7.0, 2.0], dtype=np.float32)
+    xi = np.array([[1, 1, 1]], dtype=np.float32)
+    acc, pot = gpu_force(nb, xi, xj, mj, 0.0)
+    np.testing.assert_allclose(acc[0], [2.0 / 9.0, 0, 0], rtol=1e-6, atol=1e-12)
+    assert pot[0] == pytest.approx(-2.0 / 3.0, rel=1e-6)
+    # eps2 = 0 with distinct particles against the oracle
+    rng = np.random.default_rng(5)
+    x = rng.normal(size=(300, 3)).astype(np.float32)
+    mm = rng.uniform(0.5, 1.5, 300).astype(np.float32)
+    acc, pot = gpu_force(nb, x, x, mm, 0.0, alias=True)
+    ref_acc, ref_pot = oracle.force(x, x, mm, 0.0)
+    assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot))
+    check_parity(acc, pot, ref_acc, ref_pot, "eps0")
+
+
+def test_two_body_exact_cases(nb):
+    # d = (3,0,0), eps2 = 16 -> a = 3/125, phi = -1/5  (tests/golden/two_body_exact.txt row 1)
+    acc, pot = gpu_force(nb, np.zeros((1, 3), np.float32), np.array([[3, 0, 0]], np.float32),
+                         np.array([1.0], np.float32), 16.0)
+    np.testing.assert_allclose(acc[0], [3.0 / 125.0, 0, 0], rtol=1e-6, atol=0)
+    assert pot[0] == pytest.approx(-0.2, rel=1e-6)
+
+
+def test_empty_sets(nb):
+    import torch
+    x = dev(np.ones((5, 3), np.float32))
+    m = dev(np.ones(5, np.float32))
+    empty_x = torch.empty((0, 3), dtype=torch.float32, device="cuda")
+    empty_m = torch.empty((0,), dtype=torch.float32, device="cuda")
+    # n_j = 0: outputs zero-filled
+    acc = torch.full((5, 3), 7.0, device="cuda")
+    pot = torch.full((5,), 7.0, device="cuda")
+    nb.force(x, empty_x, empty_m, 0.1, acc_out=acc, pot_out=pot)
+    torch.cuda.synchronize()
+    assert torch.all(acc == 0) and torch.all(pot == 0)
+    # n_i = 0: nothing written, OK
+    acc0, pot0 = nb.force(empty_x, x, m, 0.1)
+    assert acc0.shape == (0, 3)
+
+
+def test_pot_null_and_invalid_arguments(nb):
+    import torch
+    w = wl.plummer_workload(300, 1.0 / 64, seed=3)
+    acc, pot = gpu_force(nb, w.xi, w.x_j, w.m_j, w.eps2, want_pot=False)
+    assert pot is None
+    ref_acc, _ = oracle.force(w.xi, w.x_j, w.m_j, w.eps2)
+    check_parity(acc, None, ref_acc, None)
+    x, m = dev(w.x_j), dev(w.m_j)
+    for bad in (-1.0, float("nan"), float("inf")):
+        with pytest.raises(nb.NBError) as ei:
+            nb.force(x, x, m, bad)
+        assert ei.value.status == 1
+    l = nb.lib()
+    out = torch.empty((300, 3), device="cuda")
+    assert l.nb_force(-1, x.data_ptr(), 300, x.data_ptr(), m.data_ptr(), 0.1, out.data_ptr(), None, None) == 1
+    assert l.nb_force(300, None, 300, x.data_ptr(), m.data_ptr(), 0.1, out.data_ptr(), None, None) == 1
+    assert l.nb_force(300, x.data_ptr(), 300, x.data_ptr(), m.data_ptr(), 0.1, None, None, None) == 1
+    assert l.nb_force(2 ** 31, x.data_ptr(), 300, x.data_ptr(), m.data_ptr(), 0.1, out.data_ptr(), None, None) == 1
+
+
+# ------------------------------------------------------------------ determinism (P11)
+def test_bitwise_reproducible_and_i_permutation_invariant(nb):
+    w = wl.subset_workload(6000, 1000, 1.0 / 128, seed=8)
+    a1, p1 = gpu_force(nb, w.x_i, w.x_j, w.m_j, w.eps2)
+    a2, p2 = gpu_force(nb, w.x_i, w.x_j, w.m_j, w.eps2)
+    assert np.array_equal(a1, a2) and np.array_equal(p1, p2)
+    perm = np.random.default_rng(0).permutation(1000)
+    a3, p3 = gpu_force(nb, w.x_i[perm], w.x_j, w.m_j, w.eps2)
+    assert np.array_equal(a3, a1[perm]) and np.array_equal(p3, p1[perm])
+
+
+def test_momentum_antisymmetry_fp32(nb):
+    w = wl.config(0)
+    acc, _ = gpu_force(nb, w.xi, w.x_j, w.m_j, w.eps2, alias=True)
+    m = w.m_j.astype(np.float64)
+    net = np.linalg.norm((m[:, None] * acc.astype(np.float64)).sum(axis=0))
+    scale = (m * np.linalg.norm(acc, axis=1)).sum()
+    assert net <= 1e-5 * scale
+
+
+# ------------------------------------------------------------------ host-buffer entry (paper's force())
+def test_force_host_matches_device_path(nb):
+    w = wl.subset_workload(5000, 600, 1.0 / 128, seed=12)
+    acc_h, pot_h = nb.force_host(w.x_i, w.x_j, w.m_j, w.eps2)
+    acc_d, pot_d = gpu_force(nb, w.x_i, w.x_j, w.m_j, w.eps2)
+    assert np.array_equal(acc_h, acc_d) and np.array_equal(pot_h, pot_d)
+    # aliased i == j
+    w0 = wl.config(0)
+    acc_h, pot_h = nb.force_host(w0.x_j, w0.x_j, w0.m_j, w0.eps2)
+    ref_acc, ref_pot = oracle.force(w0.xi, w0.x_j, w0.m_j, w0.eps2)
+    check_parity(acc_h, pot_h, ref_acc, ref_pot, "host C0")
+
+
+# ------------------------------------------------------------------ full-size configs, bench launch configuration
+def _sampled_parity(nb, w, n_sample, seed, label):
+    import torch
+    d_xj, d_mj = dev(w.x_j), dev(w.m_j)
+    d_xi = d_xj if w.x_i is None else dev(w.x_i)
+    acc, pot = nb.force(d_xi, d_xj, d_mj, w.eps2)
+    torch.cuda.synchronize()
+    acc, pot = acc.cpu().numpy(), pot.cpu().numpy()
+    assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot))
+    idx = np.sort(np.random.default_rng(seed).choice(w.n_i, min(n_sample, w.n_i), replace=False))
+    ref_acc, ref_pot = oracle.force(np.ascontiguousarray(w.xi[idx]), w.x_j, w.m_j, w.eps2)
+    e = check_parity(acc[idx], pot[idx], ref_acc, ref_pot, label)
+    return acc, pot, e
+
+
+def test_c1_full_size_sampled(nb):
+    w = wl.config(1)
+    acc, pot, e = _sampled_parity(nb, w, 2048, 1, "C1")
+    m = w.m_j.astype(np.float64)
+    net = np.linalg.norm((m[:, None] * acc.astype(np.float64)).sum(axis=0))
+    assert net <= 1e-5 * (m * np.linalg.norm(acc, axis=1)).sum()
+    # P5: Plummer potential energy of the truncated model, W = -0.302443 (1 - 1/N) within 3 sigma
+    W = 0.5 * float(np.sum(m * pot.astype(np.float64)))
+    n = w.n_j
+    assert abs(W / (-0.302443 * (1 - 1.0 / n)) - 1.0) <= 3 * 0.5 / np.sqrt(n)
+
+
+def test_c2_full_size_all_elements(nb):
+    w = wl.config(2)
+    acc, pot = gpu_force(nb, w.x_i, w.x_j, w.m_j, w.eps2)
+    ref_acc, ref_pot = oracle.force(w.x_i, w.x_j, w.m_j, w.eps2)
+    check_parity(acc, pot, ref_acc, ref_pot, "C2")
+
+
+def test_c3_full_size_sampled(nb):
+    w = wl.config(3)
+    acc, pot, e = _sampled_parity(nb, w, 1024, 3, "C3")
+    m = w.m_j.astype(np.float64)
+    net = np.linalg.norm((m[:, None] * acc.astype(np.float64)).sum(axis=0))
+    assert net <= 1e-5 * (m * np.linalg.norm(acc, axis=1)).sum()
+    # P7: uniform sphere, E[W] = -(3/5)(1 - sum m^2)/R
+    W = 0.5 * float(np.sum(m * pot.astype(np.float64)))
+    assert abs(W / (-0.6 * (1.0 - float(np.sum(m * m)))) - 1.0) < 0.01
