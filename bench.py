@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the all-pairs softened-gravity hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C1] [--impl reference]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input: one nb_force call
+(j-pack + pair-interaction kernel + j-split reduce) on BASELINE.json configs[1] -- the N = 131072
+equal-mass Plummer sphere, i-set = j-set, eps = 1/256, seed 1 (the paper's largest N).
+Metric: interactions/s = n_i * n_j / t (the paper's N^2 of Eq. (4)), with Gflop/s at
+20 and 38 flop per interaction alongside.
+
+Prints ONE JSON line on rank 0.  Multi-GPU (N > 1, under torchrun): the path does not shard in this
+build (BASELINE.json: "Everything runs on one GPU"), so N ranks run N independent replicas with no
+data-path collective ("replicas only"); value = total interactions of all ranks / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "interactions/s"
+FP32_INST_PER_PAIR = 13          # FMA-pipe instructions per interaction (acc + phi), DESIGN.md "Roofline"
+FP32_LANES_PER_SM_CLK = 128
+CONFIG_INDEX = {"C0": 0, "C1": 1, "C2": 2, "C3": 3, "C4": 4}
+L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"sm_max_mhz": 1965.0, "hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as exc:  # NVML missing: report that, never fake numbers
+            self.nv, self.h, self.err = None, None, repr(exc)
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, bit in names.items():
+                    if mask & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.02)
+
+    def start(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "note": "NVML unavailable"}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def physical_gpu_index(local_rank: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+def oracle_rate(w, target_seconds: float, rng_seed: int = 0):
+    """Times the CPU oracle, as it stands, on a bounded i-sample of workload w.  Returns (pairs/s, cores, sample)."""
+    import oracle
+    cores = oracle.num_threads()
+    rng = np.random.default_rng(rng_seed)
+
+    def run(n_i):
+        idx = np.sort(rng.choice(w.n_i, n_i, replace=False))
+        xi = np.ascontiguousarray(w.xi[idx])
+        t0 = time.perf_counter()
+        oracle.force(xi, w.x_j, w.m_j, w.eps2)
+        return time.perf_counter() - t0
+
+    n_probe = min(w.n_i, max(64, 8 * cores))
+    run(min(n_probe, 64))                                   # page in, spin up the OpenMP team
+    t_probe = run(n_probe)
+    rate = n_probe * w.n_j / t_probe
+    n_i = int(min(w.n_i, max(n_probe, target_seconds * rate / w.n_j)))
+    t = run(n_i)
+    return n_i * w.n_j / t, cores, f"{n_i} of {w.n_i} i-particles (seeded, sorted) x all {w.n_j} j-particles, {t:.2f} s"
+
+
+def reference_arm(args, w, cfg_name):
+    """--impl reference: the CPU oracle (this tier has no reference implementation), rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    per_step = max(0.5, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_rate(w, per_step / 4)
+    rates, sample = [], ""
+    t0 = time.perf_counter()
+    for s in range(args.steps):
+        r, cores, sample = oracle_rate(w, per_step, rng_seed=s)
+        rates.append(r)
+    wall = time.perf_counter() - t0
+    value = float(np.mean(rates))
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg_name, w)},
+        "gflops_20": 20e-9 * value, "gflops_38": 38e-9 * value,
+        "cpu_baseline": {"value": value, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out), flush=True)
+
+
+def workload_name(cfg_name, w):
+    return (f"BASELINE.json configs[{CONFIG_INDEX[cfg_name]}] ({cfg_name}): {w.meta.get('model', '')}, "
+            f"n_i={w.n_i}, n_j={w.n_j}, eps2={w.eps2:.6g}, seed={w.seed}, one nb_force call with phi")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+
+    from paper_astro_ph_0703100_b200 import workloads as wl
+    w = wl.config(CONFIG_INDEX[args.config])
+
+    if args.impl == "reference":
+        reference_arm(args, w, args.config)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_astro_ph_0703100_b200 as nb
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    nb.lib()
+    peaks, peaks_kind = load_peaks()
+
+    # inputs resident in HBM before the timed region
+    d_xj = torch.from_numpy(w.x_j).cuda()
+    d_mj = torch.from_numpy(w.m_j).cuda()
+    d_xi = d_xj if w.x_i is None else torch.from_numpy(w.x_i).cuda()
+    acc = torch.empty((w.n_i, 3), dtype=torch.float32, device="cuda")
+    pot = torch.empty((w.n_i,), dtype=torch.float32, device="cuda")
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        flush.fill_(1)
+        nb.force(d_xi, d_xj, d_mj, w.eps2, acc_out=acc, pot_out=pot)
+    torch.cuda.synchronize()
+    launches_per_step = nb.last_launch_count()
+
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    nb.profile_enable(True)
+    barrier()
+    sampler.start()
+    t_wall0 = time.perf_counter()
+    for s in range(args.steps):
+        flush.fill_(s & 0xff)                      # L2 flush between timed iterations (outside the events)
+        ev[s][0].record(stream)
+        nb.force(d_xi, d_xj, d_mj, w.eps2, acc_out=acc, pot_out=pot)
+        ev[s][1].record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    nb.profile_enable(False)
+    n_k, k_ms = nb.profile_read()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+
+    # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    h_xj = torch.from_numpy(w.x_j).pin_memory()
+    h_mj = torch.from_numpy(w.m_j).pin_memory()
+    h_xi = h_xj if w.x_i is None else torch.from_numpy(w.x_i).pin_memory()
+    h_acc = torch.empty((w.n_i, 3), dtype=torch.float32).pin_memory()
+    h_pot = torch.empty((w.n_i,), dtype=torch.float32).pin_memory()
+    e2e_steps = max(3, min(args.steps, 10))
+    for _ in range(2):
+        nb.force_host(h_xi.numpy(), h_xj.numpy(), h_mj.numpy(), w.eps2, acc_out=h_acc.numpy(), pot_out=h_pot.numpy())
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        nb.force_host(h_xi.numpy(), h_xj.numpy(), h_mj.numpy(), w.eps2, acc_out=h_acc.numpy(), pot_out=h_pot.numpy())
+    torch.cuda.synchronize()
+    e2e_ms = 1e3 * (time.perf_counter() - t0)
+    h2d = w.x_j.nbytes + w.m_j.nbytes + (0 if w.x_i is None else w.x_i.nbytes)
+    d2h = h_acc.numel() * 4 + h_pot.numel() * 4
+
+    # max over ranks
+    if world > 1:
+        t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, e2e_ms = float(t[0]), float(t[1])
+
+    if rank == 0:
+        pairs = float(w.pairs)
+        value = world * pairs * args.steps / (total_ms * 1e-3)
+        e2e_value = world * pairs * e2e_steps / (e2e_ms * 1e-3)
+        f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+        sm_count = torch.cuda.get_device_properties(0).multi_processor_count
+        peak_inst = sm_count * FP32_LANES_PER_SM_CLK * f_max                 # FP32-pipe lane-instructions / s
+        k_rate = pairs * n_k / (k_ms * 1e-3) if n_k else 0.0
+        achieved = FP32_INST_PER_PAIR * k_rate
+        roofline = {
+            "bound": "alu", "kernel": "nb_force_kernel (pair interaction, rows a2-a7)",
+            "achieved": achieved / 1e12, "peak": peak_inst / 1e12, "unit": "FP32-pipe Tinst/s",
+            "frac": achieved / peak_inst, "traffic": None,
+            "kernel_ms": k_ms / max(1, n_k), "kernel_launches_timed": n_k,
+            "kernel_interactions_per_s": k_rate, "roofline_interactions_per_s": peak_inst / FP32_INST_PER_PAIR,
+            "peak_source": f"{sm_count} SMs x {FP32_LANES_PER_SM_CLK} FP32 lanes x sm_max_mhz {f_max / 1e6:.0f} MHz "
+                           f"({peaks_kind} MEASURED_PEAKS.json clock), {FP32_INST_PER_PAIR} FMA-pipe instr/interaction",
+        }
+        if clocks.get("sm_mhz"):
+            roofline["frac_at_observed_clock"] = achieved / (sm_count * FP32_LANES_PER_SM_CLK * clocks["sm_mhz"] * 1e6)
+        out = {
+            "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(args.config, w), "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "l2": f"flushed between timed iterations ({L2_FLUSH_BYTES >> 20} MiB write, outside the events)",
+                       "plan": nb.plan_query(w.n_i, w.n_j, sm_count)},
+            "gflops_20": 20e-9 * value, "gflops_38": 38e-9 * value,
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps, "api": "nb_force_host (pinned host buffers)"},
+            "gpu_launches": int(launches_per_step * args.steps),
+            "roofline": roofline,
+            "wall_s_timed_region": t_wall,
+            "paper_context": {"gflops_38_8800gtx_n131072": 256, "interactions_per_s_8800gtx_n131072": 6.74e9,
+                              "note": "PAPER.md:314, includes PCIe copies; context, not target"},
+        }
+        if not args.no_cpu_baseline:
+            v, cores, sample = oracle_rate(w, args.cpu_seconds)
+            out["cpu_baseline"] = {"value": v, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample}
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

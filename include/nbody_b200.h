@@ -115,12 +115,22 @@ int nb_leapfrog_kdk(int64_t n, float *x, float *v, const float *m,
  * out[0] = K  i-particles per thread        out[1] = WI warps per CTA along i
  * out[2] = WJ warps per CTA along j         out[3] = S  j-chunks across CTAs (grid.y)
  * out[4] = number of i-tiles (grid.x)       out[5] = i-particles per CTA tile (32*K*WI)
- * out[6] = j-pairs per shared-memory stage  out[7] = pipeline stages
+ * out[6] = j-particles per shared-memory stage  out[7] = pipeline stages
  */
 int nb_plan_query(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]);
 
 /* Number of kernel launches the most recent nb_force / nb_leapfrog_kdk / nb_force_host call of this thread enqueued. */
 int64_t nb_last_launch_count(void);
+
+/*
+ * nb_profile_enable / nb_profile_read -- optional timing of the dominant kernel (the pair-interaction
+ * kernel, rows a2..a7) for the roofline report.  While enabled, every force-kernel launch of this
+ * thread is bracketed by two CUDA events recorded on the launching stream.  nb_profile_read waits
+ * for the recorded events, returns the number of bracketed launches and the sum of their durations in
+ * milliseconds, and clears the record.  Disabled by default; when disabled nothing is recorded.
+ */
+int nb_profile_enable(int on);
+int nb_profile_read(int64_t *n_launches, double *total_ms);
 
 /* Frees every internal workspace of the current device (synchronises the device). */
 int nb_release_workspace(void);

@@ -11,6 +11,8 @@ from .binding import (  # noqa: F401
     leapfrog_kdk,
     lib,
     plan_query,
+    profile_enable,
+    profile_read,
     release_workspace,
     status_string,
     version,

@@ -47,6 +47,10 @@ def lib() -> ctypes.CDLL:
         l.nb_plan_query.restype = ci
         l.nb_last_launch_count.restype = i64
         l.nb_release_workspace.restype = ci
+        l.nb_profile_enable.argtypes = [ci]
+        l.nb_profile_enable.restype = ci
+        l.nb_profile_read.argtypes = [ctypes.POINTER(i64), ctypes.POINTER(ctypes.c_double)]
+        l.nb_profile_read.restype = ci
         l.nb_status_string.argtypes = [ci]
         l.nb_status_string.restype = ctypes.c_char_p
         l.nb_last_cuda_error.restype = ci
@@ -140,12 +144,23 @@ def leapfrog_kdk(x, v, m, eps2: float, dt: float, n_steps: int, acc_io=None, pot
 def plan_query(n_i: int, n_j: int, sm_count: int = 148) -> dict:
     out = (ctypes.c_int64 * 8)()
     _check(lib().nb_plan_query(int(n_i), int(n_j), int(sm_count), out), "nb_plan_query")
-    keys = ("K", "WI", "WJ", "S", "tiles_i", "tile_i", "tile_pairs", "stages")
+    keys = ("K", "WI", "WJ", "S", "tiles_i", "tile_i", "tile_j", "stages")
     return dict(zip(keys, [int(v) for v in out]))
 
 
 def last_launch_count() -> int:
     return int(lib().nb_last_launch_count())
+
+
+def profile_enable(on: bool) -> None:
+    _check(lib().nb_profile_enable(1 if on else 0), "nb_profile_enable")
+
+
+def profile_read() -> Tuple[int, float]:
+    """(number of force-kernel launches bracketed since the last read, sum of their durations in ms)."""
+    n, ms = ctypes.c_int64(0), ctypes.c_double(0.0)
+    _check(lib().nb_profile_read(ctypes.byref(n), ctypes.byref(ms)), "nb_profile_read")
+    return int(n.value), float(ms.value)
 
 
 def release_workspace() -> None:

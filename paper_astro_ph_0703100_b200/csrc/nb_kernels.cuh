@@ -1,7 +1,7 @@
 // nb_kernels.cuh -- sm_100a device code for the all-pairs softened gravity path.
 //
 // Rows of SURVEY.md section 8(a) implemented here (citations: PAPER.md by line):
-//   a1  j-pack            nb_pack_pairs_kernel     Fig. A.1 packing loop
+//   a1  j-pack            nb_pack_j_kernel         Fig. A.1 packing loop
 //   a2  j-tile staging    TMA bulk copy + mbarrier ring in nb_force_kernel   step (d) J-PACKING
 //   a3  i-load            prologue of nb_force_kernel                        step (e)
 //   a4  pair interaction  pair_body()                                        step (h); Eq. (1); Fig. A.3 PAPER.md:458-471;
@@ -10,11 +10,16 @@
 //   a6  epilogue          end of nb_force_kernel / nb_reduce_kernel          step (i)
 //   a7  j-split + reduce  WJ (warps) and S (CTAs) split, fixed-order sums    (paper analogue: force-memory round trips)
 //
-// Layout of the packed j-array ("pair records", 32 B each, 128-B aligned array):
-//     record p = { x[2p], x[2p+1], y[2p], y[2p+1],   z[2p], z[2p+1], m[2p], m[2p+1] }
-// so that one LDS.128 yields two 64-bit operands for the packed FP32 instructions
-// (add/mul/fma.f32x2 -> SASS FADD2/FMUL2/FFMA2): the two halves of every packed operand are two
-// consecutive j-particles interacting with the same i-particle.
+// Layout of the packed j-array: one 16-byte record (x, y, z, m) per j-particle -- the paper's own
+// [n_j][JDIM = 4] rows -- in a 128-byte aligned array, so that a tile is one
+// contiguous 1-D TMA bulk copy and one broadcast LDS.128 yields a whole j-particle.
+//
+// Register layout of the i-particles: each thread owns K i-particles as K/2 PAIRS held in 64-bit
+// registers, so that the packed FP32 instructions (add/mul/fma.f32x2 -> SASS FADD2/FMUL2/FFMA2)
+// process two i-particles against one j-particle per instruction; the j operand is the 32-bit
+// broadcast form of those instructions.  Why: on sm_100 the loop is bound
+// by register-file read bandwidth and issue slots, not by the FMA pipe alone; the packed forms halve
+// the issue slots and the scalar j operand saves a register read per instruction.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -91,28 +96,30 @@ __device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint3
 }
 
 // ---------------------------------------------------------------- a1: j-pack
-// One thread per pair record.  Particles beyond n_j (padding up to a multiple of 8) take the
-// position of the last real particle and mass 0, so they contribute exactly nothing.
-__global__ void __launch_bounds__(256) nb_pack_pairs_kernel(const float* __restrict__ x_j, const float* __restrict__ m_j,
-                                                            int n_j, int n_pairs_padded, float4* __restrict__ jp) {
-    int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n_pairs_padded) return;
-    int j0 = 2 * p, j1 = 2 * p + 1;
-    int c0 = min(j0, n_j - 1), c1 = min(j1, n_j - 1);
-    float x0 = x_j[3 * c0 + 0], y0 = x_j[3 * c0 + 1], z0 = x_j[3 * c0 + 2];
-    float x1 = x_j[3 * c1 + 0], y1 = x_j[3 * c1 + 1], z1 = x_j[3 * c1 + 2];
-    float m0 = (j0 < n_j) ? m_j[c0] : 0.0f;
-    float m1 = (j1 < n_j) ? m_j[c1] : 0.0f;
-    jp[2 * p + 0] = make_float4(x0, x1, y0, y1);
-    jp[2 * p + 1] = make_float4(z0, z1, m0, m1);
+// One thread per j-particle: (x, y, z) || m -> float4.
+__global__ void __launch_bounds__(256) nb_pack_j_kernel(const float* __restrict__ x_j, const float* __restrict__ m_j,
+                                                        int n_j, float4* __restrict__ jp) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_j) return;
+    jp[j] = make_float4(x_j[3 * j + 0], x_j[3 * j + 1], x_j[3 * j + 2], m_j[j]);
 }
 
-// ---------------------------------------------------------------- a4: one i-particle x one j-pair
-// 13 packed FP32-pipe instructions (3 FADD2, 3 FFMA2, 3 FMUL2, 3 FFMA2, 1 FADD2) + 2 MUFU.RSQ
-// + the coincidence mask on the ALU pipe.  nxi = (-x_i, -x_i) etc., so d = r_j - r_i.
-template <bool EXACT_MASK>
+// ---------------------------------------------------------------- a4: two i-particles x one j-particle
+// 13 packed FP32-pipe instructions (3 FADD2, 3 FFMA2, 3 FMUL2, 3 FFMA2, 1 FADD2) + 2 MUFU.RSQ.
+// nxi = (-x_i0, -x_i1) etc., so d = r_j - r_i.  xj, yj, zj, mj hold the j value in both halves.
+//
+// Coincident pairs (reading R1: all three differences exactly zero => the pair adds nothing).
+//   MASK_EXACT : test (dx | dy | dz) == 0 bitwise and send r2 to +inf, so rsqrt gives +0 and every
+//                term of the pair vanishes; 2 ALU-pipe instructions with 4 register reads per pair.
+//   MASK_SPEC  : no masking; only records whether r2 == eps2 occurred (a necessary condition for
+//                coincidence, since fma(0, 0, eps2) == eps2): 1 ALU instruction, 1 register read per
+//                pair.  The caller recomputes the whole tile with MASK_EXACT when the flag is set, so
+//                the stored result is always the MASK_EXACT one.  Requires eps2 > 0.
+enum { MASK_EXACT = 0, MASK_SPEC = 1 };
+
+template <int MASK>
 __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nxi, u64 nyi, u64 nzi, u64 eps2_2,
-                                          float eps2, u64& ax, u64& ay, u64& az, u64& ph) {
+                                          float eps2, u64& ax, u64& ay, u64& az, u64& ph, bool& hit) {
     const u64 dx = add2(xj, nxi);                    // dx = xj - xi
     const u64 dy = add2(yj, nyi);
     const u64 dz = add2(zj, nzi);
@@ -121,9 +128,9 @@ __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nx
     r2 = fma2(dz, dz, r2);
     float r2a, r2b;
     unpack2(r2, r2a, r2b);
-    const float inf = __int_as_float(0x7f800000);
-    if (EXACT_MASK) {
+    if (MASK == MASK_EXACT) {
         // coincident <=> all three differences are exactly +0 (x - x rounds to +0)
+        const float inf = __int_as_float(0x7f800000);
         float dxa, dxb, dya, dyb, dza, dzb;
         unpack2(dx, dxa, dxb); unpack2(dy, dya, dyb); unpack2(dz, dza, dzb);
         const uint32_t ta = __float_as_uint(dxa) | __float_as_uint(dya) | __float_as_uint(dza);
@@ -131,8 +138,8 @@ __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nx
         r2a = (ta == 0u) ? inf : r2a;                // rsqrt(+inf) = +0 -> the pair adds exactly 0
         r2b = (tb == 0u) ? inf : r2b;
     } else {
-        r2a = (r2a == eps2) ? inf : r2a;
-        r2b = (r2b == eps2) ? inf : r2b;
+        hit |= (r2a == eps2);
+        hit |= (r2b == eps2);
     }
     const u64 u = pack2(rsqrt_approx(r2a), rsqrt_approx(r2b));   // r1i = 1/sqrt(r2)
     const u64 u2 = mul2(u, u);                       // r2i
@@ -144,14 +151,33 @@ __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nx
     ph = add2(ph, mu);                               // OUTPUT[6] -= pot (sign applied at the end) PAPER.md:552
 }
 
+// One tile: K/2 i-pairs of this thread against np j-particles in shared memory; partial sums start from zero (Eq. (2)).
+template <int K, int MASK>
+__device__ __forceinline__ bool tile_sweep(const float4* __restrict__ sp, int np, const u64 (&nxi)[K / 2], const u64 (&nyi)[K / 2],
+                                           const u64 (&nzi)[K / 2], u64 eps2_2, float eps2, u64 (&pax)[K / 2], u64 (&pay)[K / 2],
+                                           u64 (&paz)[K / 2], u64 (&pph)[K / 2]) {
+    bool hit = false;
+#pragma unroll
+    for (int k = 0; k < K / 2; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
+#pragma unroll 4
+    for (int j = 0; j < np; ++j) {
+        const float4 J = sp[j];                                        // broadcast LDS.128: x y z m
+        const u64 xj = pack2(J.x, J.x), yj = pack2(J.y, J.y), zj = pack2(J.z, J.z), mj = pack2(J.w, J.w);
+#pragma unroll
+        for (int k = 0; k < K / 2; ++k)
+            pair_body<MASK>(xj, yj, zj, mj, nxi[k], nyi[k], nzi[k], eps2_2, eps2, pax[k], pay[k], paz[k], pph[k], hit);
+    }
+    return hit;
+}
+
 struct ForceArgs {
     const float* x_i;      // [n_i][3]
-    const ulonglong2* jp;  // packed pair records, 2 x 16 B per pair
+    const float4* jp;      // packed j records (x, y, z, m)
     float* acc;            // [n_i][3]
     float* pot;            // [n_i] or nullptr
     double4* partial;      // [S][n_i] when S > 1
     int n_i;
-    int n_units;           // padded pairs / 4
+    int n_j;
     int S;
     float eps2;
 };
@@ -162,11 +188,12 @@ struct ForceArgs {
 // Each sub-range is streamed through its own shared-memory ring by 1-D TMA bulk copies issued by
 // lane 0 of the group's first warp; "full" mbarriers count bytes, "empty" mbarriers count the WI
 // consuming warps.
-template <int K, int WI, int WJ, int TP, int STAGES, bool EXACT_MASK>
+template <int K, int WI, int WJ, int TJ, int STAGES, bool SPEC>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceArgs a) {
+    static_assert(K % 2 == 0, "i-particles are held in pairs");
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    constexpr int RING_BYTES = STAGES * TP * 32;
-    unsigned char* rings = smem_raw;                                   // [WJ][STAGES][TP*32]
+    constexpr int RING_BYTES = STAGES * TJ * 16;
+    unsigned char* rings = smem_raw;                                   // [WJ][STAGES][TJ] float4
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + WJ * RING_BYTES);   // full[WJ][STAGES], empty[WJ][STAGES]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -185,23 +212,25 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
         mbar_fence_init();
     }
 
-    // j sub-range of this warp group, in units of 4 pairs
+    // j sub-range of this warp group
     const long long G = (long long)a.S * WJ;
     const long long g = (long long)blockIdx.y * WJ + wj;
-    const int u_begin = (int)((long long)a.n_units * g / G);
-    const int u_end = (int)((long long)a.n_units * (g + 1) / G);
-    const int n_sub = (u_end - u_begin) * 4;                           // pairs
-    const int n_tiles = (n_sub + TP - 1) / TP;
-    const unsigned char* src = reinterpret_cast<const unsigned char*>(a.jp) + (size_t)u_begin * 128;
+    const int j_begin = (int)((long long)a.n_j * g / G);
+    const int j_end = (int)((long long)a.n_j * (g + 1) / G);
+    const int n_sub = j_end - j_begin;
+    const int n_tiles = (n_sub + TJ - 1) / TJ;
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(a.jp + j_begin);
 
-    // a3: i-particles of this thread (clamped loads; stores are guarded)
+    // a3: i-particles of this thread (clamped loads; stores are guarded), pair k2 = (k = 2 k2, 2 k2 + 1)
     const int i_base = blockIdx.x * (32 * K * WI) + wi * 32 + lane;
-    u64 nxi[K], nyi[K], nzi[K];
+    u64 nxi[K / 2], nyi[K / 2], nzi[K / 2];
 #pragma unroll
-    for (int k = 0; k < K; ++k) {
-        const int i = min(i_base + k * 32 * WI, a.n_i - 1);
-        const float x = a.x_i[3 * i + 0], y = a.x_i[3 * i + 1], z = a.x_i[3 * i + 2];
-        nxi[k] = pack2(-x, -x); nyi[k] = pack2(-y, -y); nzi[k] = pack2(-z, -z);
+    for (int k2 = 0; k2 < K / 2; ++k2) {
+        const int i0 = min(i_base + (2 * k2) * 32 * WI, a.n_i - 1);
+        const int i1 = min(i_base + (2 * k2 + 1) * 32 * WI, a.n_i - 1);
+        nxi[k2] = pack2(-a.x_i[3 * i0 + 0], -a.x_i[3 * i1 + 0]);
+        nyi[k2] = pack2(-a.x_i[3 * i0 + 1], -a.x_i[3 * i1 + 1]);
+        nzi[k2] = pack2(-a.x_i[3 * i0 + 2], -a.x_i[3 * i1 + 2]);
     }
     const float eps2 = a.eps2;
     const u64 eps2_2 = pack2(eps2, eps2);
@@ -211,9 +240,9 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
     if (producer) {
         const int pre = n_tiles < STAGES ? n_tiles : STAGES;
         for (int t = 0; t < pre; ++t) {
-            const uint32_t bytes = (uint32_t)min(TP, n_sub - t * TP) * 32u;
+            const uint32_t bytes = (uint32_t)min(TJ, n_sub - t * TJ) * 16u;
             mbar_expect_tx(full0 + 8 * t, bytes);
-            tma_load_1d(ring + t * TP * 32, src + (size_t)t * TP * 32, bytes, full0 + 8 * t);
+            tma_load_1d(ring + t * TJ * 16, src + (size_t)t * TJ * 16, bytes, full0 + 8 * t);
         }
     }
 
@@ -226,30 +255,26 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
         const uint32_t parity = (uint32_t)(t / STAGES) & 1u;
         mbar_wait(full0 + 8 * slot, parity);
 
-        const int np = min(TP, n_sub - t * TP);                        // multiple of 4
-        const ulonglong2* sp = reinterpret_cast<const ulonglong2*>(rings + wj * RING_BYTES + slot * TP * 32);
+        const int np = min(TJ, n_sub - t * TJ);
+        const float4* sp = reinterpret_cast<const float4*>(rings + wj * RING_BYTES + slot * TJ * 16);
 
-        u64 pax[K], pay[K], paz[K], pph[K];                            // tile partial sums, started from zero (Eq. (2))
-#pragma unroll
-        for (int k = 0; k < K; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
-
-#pragma unroll 4
-        for (int p = 0; p < np; ++p) {
-            const ulonglong2 A = sp[2 * p + 0];                        // broadcast LDS.128: x0 x1 | y0 y1
-            const ulonglong2 B = sp[2 * p + 1];                        //                    z0 z1 | m0 m1
-#pragma unroll
-            for (int k = 0; k < K; ++k)
-                pair_body<EXACT_MASK>(A.x, A.y, B.x, B.y, nxi[k], nyi[k], nzi[k], eps2_2, eps2, pax[k], pay[k], paz[k], pph[k]);
+        u64 pax[K / 2], pay[K / 2], paz[K / 2], pph[K / 2];            // tile partial sums (Eq. (2))
+        if (SPEC) {
+            const bool hit = tile_sweep<K, MASK_SPEC>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+            if (__any_sync(0xffffffffu, hit))                          // rare: some pair of this warp may be coincident
+                (void)tile_sweep<K, MASK_EXACT>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+        } else {
+            (void)tile_sweep<K, MASK_EXACT>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
         }
 
         // a5: tile partial -> running total
 #pragma unroll
-        for (int k = 0; k < K; ++k) {
+        for (int k2 = 0; k2 < K / 2; ++k2) {
             float lo, hi;
-            unpack2(pax[k], lo, hi); run[k][0] += (double)(lo + hi);
-            unpack2(pay[k], lo, hi); run[k][1] += (double)(lo + hi);
-            unpack2(paz[k], lo, hi); run[k][2] += (double)(lo + hi);
-            unpack2(pph[k], lo, hi); run[k][3] += (double)(lo + hi);
+            unpack2(pax[k2], lo, hi); run[2 * k2][0] += (double)lo; run[2 * k2 + 1][0] += (double)hi;
+            unpack2(pay[k2], lo, hi); run[2 * k2][1] += (double)lo; run[2 * k2 + 1][1] += (double)hi;
+            unpack2(paz[k2], lo, hi); run[2 * k2][2] += (double)lo; run[2 * k2 + 1][2] += (double)hi;
+            unpack2(pph[k2], lo, hi); run[2 * k2][3] += (double)lo; run[2 * k2 + 1][3] += (double)hi;
         }
 
         // release the slot; the producer refills it with tile t' + STAGES.  With several consumer
@@ -262,9 +287,9 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
                 const int rs = tt % STAGES;
                 mbar_wait(empty0 + 8 * rs, (uint32_t)(tt / STAGES) & 1u);
                 const int tn = tt + STAGES;
-                const uint32_t bytes = (uint32_t)min(TP, n_sub - tn * TP) * 32u;
+                const uint32_t bytes = (uint32_t)min(TJ, n_sub - tn * TJ) * 16u;
                 mbar_expect_tx(full0 + 8 * rs, bytes);
-                tma_load_1d(ring + rs * TP * 32, src + (size_t)tn * TP * 32, bytes, full0 + 8 * rs);
+                tma_load_1d(ring + rs * TJ * 16, src + (size_t)tn * TJ * 16, bytes, full0 + 8 * rs);
             }
         }
         __syncwarp();

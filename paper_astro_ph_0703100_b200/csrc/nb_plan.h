@@ -16,50 +16,43 @@
 
 namespace nb {
 
-constexpr int kUnitPairs = 4;          // j-ranges are cut in units of 4 pairs = 8 particles = 128 bytes
 constexpr int kWarpsPerCta = 8;        // every force CTA has 8 warps = WI * WJ
 constexpr int kMaxS = 2048;
 
 struct Plan {
-    int K;            // i-particles per thread (1, 2 or 4)
+    int K;            // i-particles per thread (2, 4 or 8; held as K/2 packed pairs)
     int WI;           // warps per CTA along i
     int WJ;           // warps per CTA along j (WI * WJ == 8)
     int S;            // j-chunks across CTAs (grid.y); S > 1 needs the second-pass reduce
     int tiles_i;      // grid.x
     int tile_i;       // i-particles per CTA = 32 * K * WI
-    int tile_pairs;   // j-pairs per shared-memory stage
+    int tile_j;       // j-particles per shared-memory stage
     int stages;       // ring depth
-    int64_t n_pairs_padded;   // padded j-pair count (multiple of kUnitPairs)
 };
 
-inline int64_t padded_pairs(int64_t n_j) {
-    int64_t pairs = (n_j + 1) / 2;
-    return (pairs + kUnitPairs - 1) / kUnitPairs * kUnitPairs;
-}
-
-inline void ring_shape(int WJ, int* tile_pairs, int* stages) {
-    // shared memory: WJ rings x stages x tile_pairs x 32 B
+inline void ring_shape(int WJ, int* tile_j, int* stages) {
+    // shared memory: WJ rings x stages x tile_j x 16 B
     switch (WJ) {
-        case 1: *tile_pairs = 256; *stages = 4; break;   //  32 KB
-        case 2: *tile_pairs = 256; *stages = 4; break;   //  64 KB
-        case 4: *tile_pairs = 128; *stages = 4; break;   //  64 KB
-        default: *tile_pairs = 128; *stages = 3; break;  //  96 KB (WJ = 8)
+        case 1: *tile_j = 512; *stages = 4; break;   //  32 KB
+        case 2: *tile_j = 512; *stages = 4; break;   //  64 KB
+        case 4: *tile_j = 256; *stages = 4; break;   //  64 KB
+        default: *tile_j = 256; *stages = 3; break;  //  96 KB (WJ = 8)
     }
 }
 
 // Cost model in SM clock cycles.  pair_cycles: 13 FP32-pipe lane-ops per pair over 128 lanes per
-// clock per SM at an assumed 80 % pipe efficiency.
+// clock per SM at the measured ~84 % pipe efficiency of the K = 8 inner loop (profiles/).
 inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, int WJ, int S) {
     const double c_fixed = 6000.0;                    // CTA start + first TMA round trip + epilogue
     const double c_reduce_launch = 8000.0;            // second kernel
-    const double pair_cycles = 13.0 / (128.0 * 0.80);
+    const double pair_cycles = 13.0 / (128.0 * 0.84);
     const int tile_i = 32 * K * WI;
     const int64_t tiles_i = (n_i + tile_i - 1) / tile_i;
     const double ctas = double(tiles_i) * S;
     const double waves = double((int64_t)((ctas + sm_count - 1) / sm_count));
-    const double j_per_cta = double(padded_pairs(n_j)) * 2.0 / S;
-    // a CTA alone on an SM with lanes idle (K < 4 costs more shared-memory traffic: penalise mildly)
-    const double k_pen = (K == 4) ? 1.0 : (K == 2 ? 1.08 : 1.3);
+    const double j_per_cta = double(n_j) / S;
+    // fewer i-particles per thread: more shared-memory reads and loop overhead per pair
+    const double k_pen = (K == 8) ? 1.0 : (K == 4 ? 1.03 : 1.12);
     double cta_cycles = c_fixed + double(tile_i) * j_per_cta * pair_cycles * k_pen;
     if (WJ > 1) cta_cycles += 1500.0;                 // cross-warp reduction through shared memory
     double cost = waves * cta_cycles;
@@ -70,37 +63,39 @@ inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, i
 inline Plan make_plan(int64_t n_i, int64_t n_j, int sm_count) {
     if (sm_count <= 0) sm_count = 148;
     Plan best{};
-    const int64_t units = padded_pairs(n_j) / kUnitPairs;
-    const int K = (n_i > 64) ? 4 : (n_i > 32 ? 2 : 1);
     double best_cost = -1.0;
+    static const int k_opts[3] = {8, 4, 2};
     static const int wj_opts[4] = {1, 2, 4, 8};
-    for (int wi_idx = 0; wi_idx < 4; ++wi_idx) {
-        const int WJ = wj_opts[wi_idx];
-        const int WI = kWarpsPerCta / WJ;
-        int64_t s_max = units / WJ;                   // every warp-level sub-range gets >= 1 unit
-        if (s_max < 1) s_max = 1;
-        if (s_max > kMaxS) s_max = kMaxS;
-        for (int S = 1; S <= s_max; ++S) {
-            const double c = plan_cost(n_i, n_j, sm_count, K, WI, WJ, S);
-            // strict '<' keeps the first (smallest WJ, then smallest S) among equal costs
-            if (best_cost < 0.0 || c < best_cost * (1.0 - 1e-9)) {
-                best_cost = c;
-                best.K = K; best.WI = WI; best.WJ = WJ; best.S = S;
+    for (int k_idx = 0; k_idx < 3; ++k_idx) {
+        const int K = k_opts[k_idx];
+        if (K > 2 && n_i <= 32 * (K / 2)) continue;   // a smaller K already covers all i with one warp
+        for (int wj_idx = 0; wj_idx < 4; ++wj_idx) {
+            const int WJ = wj_opts[wj_idx];
+            const int WI = kWarpsPerCta / WJ;
+            int64_t s_max = n_j / (8 * WJ);               // every warp-level sub-range gets >= 8 particles
+            if (s_max < 1) s_max = 1;
+            if (s_max > kMaxS) s_max = kMaxS;
+            for (int S = 1; S <= s_max; ++S) {
+                const double c = plan_cost(n_i, n_j, sm_count, K, WI, WJ, S);
+                // strict '<' keeps the first (largest K, smallest WJ, smallest S) among equal costs
+                if (best_cost < 0.0 || c < best_cost * (1.0 - 1e-9)) {
+                    best_cost = c;
+                    best.K = K; best.WI = WI; best.WJ = WJ; best.S = S;
+                }
             }
         }
     }
     // debugging aid, not part of the ABI: NB_PLAN="K,WI,WJ,S" overrides the choice
     if (const char* env = std::getenv("NB_PLAN")) {
         int k, wi, wj, s;
-        if (std::sscanf(env, "%d,%d,%d,%d", &k, &wi, &wj, &s) == 4 && (k == 1 || k == 2 || k == 4) &&
+        if (std::sscanf(env, "%d,%d,%d,%d", &k, &wi, &wj, &s) == 4 && (k == 2 || k == 4 || k == 8) &&
             wi * wj == kWarpsPerCta && (wj == 1 || wj == 2 || wj == 4 || wj == 8) && s >= 1 && s <= kMaxS) {
             best.K = k; best.WI = wi; best.WJ = wj; best.S = s;
         }
     }
     best.tile_i = 32 * best.K * best.WI;
     best.tiles_i = (int)((n_i + best.tile_i - 1) / best.tile_i);
-    ring_shape(best.WJ, &best.tile_pairs, &best.stages);
-    best.n_pairs_padded = padded_pairs(n_j);
+    ring_shape(best.WJ, &best.tile_j, &best.stages);
     return best;
 }
 

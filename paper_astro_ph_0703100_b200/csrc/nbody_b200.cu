@@ -10,6 +10,8 @@
 #include <mutex>
 #include <tuple>
 #include <unordered_map>
+#include <utility>
+#include <vector>
 
 #include "nb_kernels.cuh"
 #include "nb_plan.h"
@@ -20,6 +22,8 @@ namespace {
 
 thread_local int t_last_cuda_error = 0;
 thread_local int64_t t_launches = 0;
+thread_local bool t_profile = false;
+thread_local std::vector<std::pair<cudaEvent_t, cudaEvent_t>> t_events;
 
 #define NB_CUDA(call)                                  \
     do {                                               \
@@ -94,22 +98,23 @@ nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count) {
     return p;
 }
 
-bool exact_mask_enabled() {
-    // debugging aid: NB_MASK=approx selects the 2-instruction (r2 == eps2) coincidence test
-    static int v = -1;
-    if (v < 0) {
-        const char* e = std::getenv("NB_MASK");
-        v = (e && e[0] == 'a') ? 0 : 1;
-    }
-    return v == 1;
+// The speculative-mask kernel (nb_kernels.cuh, MASK_SPEC) needs eps2 > 0 and a finite
+// m * rsqrt(eps2)^3 for the unmasked coincident pair; below this threshold (and for eps2 == 0)
+// the always-masked kernel runs.  2^-40: rsqrt(eps2)^3 = 2^60.
+constexpr float kSpecMinEps2 = 9.094947017729282e-13f;
+
+bool spec_allowed() {
+    // debugging aid: NB_MASK=exact forces the always-masked kernel
+    const char* e = std::getenv("NB_MASK");
+    return !(e && e[0] == 'e');
 }
 
-template <int K, int WI, int WJ, int TP, int STAGES, bool EXACT>
+template <int K, int WI, int WJ, int TJ, int STAGES, bool SPEC>
 int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
-    constexpr size_t ring = (size_t)WJ * STAGES * TP * 32;
+    constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
     constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_force_kernel<K, WI, WJ, TP, STAGES, EXACT>;
+    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, SPEC>;
     static bool configured[64] = {};
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
@@ -118,28 +123,39 @@ int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStrea
         configured[dev & 63] = true;
     }
     dim3 grid((unsigned)plan.tiles_i, (unsigned)plan.S, 1);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (t_profile) {
+        NB_CUDA(cudaEventCreate(&e0));
+        NB_CUDA(cudaEventCreate(&e1));
+        NB_CUDA(cudaEventRecord(e0, stream));
+    }
     kern<<<grid, 32 * WI * WJ, smem, stream>>>(args);
     NB_CUDA(cudaGetLastError());
+    if (t_profile) {
+        NB_CUDA(cudaEventRecord(e1, stream));
+        t_events.emplace_back(e0, e1);
+    }
     ++t_launches;
     return NB_OK;
 }
 
-template <int K, bool EXACT>
+// tile_j / stages per WJ must match nb::ring_shape (nb_plan.h)
+template <int K, bool SPEC>
 int launch_force_k(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     switch (plan.WJ) {
-        case 1: return launch_force_inst<K, 8, 1, 256, 4, EXACT>(args, plan, stream);
-        case 2: return launch_force_inst<K, 4, 2, 256, 4, EXACT>(args, plan, stream);
-        case 4: return launch_force_inst<K, 2, 4, 128, 4, EXACT>(args, plan, stream);
-        default: return launch_force_inst<K, 1, 8, 128, 3, EXACT>(args, plan, stream);
+        case 1: return launch_force_inst<K, 8, 1, 512, 4, SPEC>(args, plan, stream);
+        case 2: return launch_force_inst<K, 4, 2, 512, 4, SPEC>(args, plan, stream);
+        case 4: return launch_force_inst<K, 2, 4, 256, 4, SPEC>(args, plan, stream);
+        default: return launch_force_inst<K, 1, 8, 256, 3, SPEC>(args, plan, stream);
     }
 }
 
-template <bool EXACT>
+template <bool SPEC>
 int launch_force(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     switch (plan.K) {
-        case 1: return launch_force_k<1, EXACT>(args, plan, stream);
-        case 2: return launch_force_k<2, EXACT>(args, plan, stream);
-        default: return launch_force_k<4, EXACT>(args, plan, stream);
+        case 2: return launch_force_k<2, SPEC>(args, plan, stream);
+        case 4: return launch_force_k<4, SPEC>(args, plan, stream);
+        default: return launch_force_k<8, SPEC>(args, plan, stream);
     }
 }
 
@@ -169,7 +185,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         std::lock_guard<std::mutex> lock(g_mutex);
         ws = &g_ws[std::make_pair(dev, stream)];
     }
-    rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)plan.n_pairs_padded * 32, stream);
+    rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)n_j * sizeof(float4), stream);
     if (rc != NB_OK) return rc;
     if (plan.S > 1) {
         rc = ensure(&ws->partial, &ws->partial_bytes, (size_t)plan.S * (size_t)n_i * sizeof(double4), stream);
@@ -178,24 +194,23 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
 
     {   // a1: j-pack
         const int threads = 256;
-        const int blocks = (int)((plan.n_pairs_padded + threads - 1) / threads);
-        nb::nb_pack_pairs_kernel<<<blocks, threads, 0, stream>>>(x_j, m_j, (int)n_j, (int)plan.n_pairs_padded,
-                                                                 reinterpret_cast<float4*>(ws->jp));
+        const int blocks = (int)((n_j + threads - 1) / threads);
+        nb::nb_pack_j_kernel<<<blocks, threads, 0, stream>>>(x_j, m_j, (int)n_j, reinterpret_cast<float4*>(ws->jp));
         NB_CUDA(cudaGetLastError());
         ++t_launches;
     }
 
     nb::ForceArgs args;
     args.x_i = x_i;
-    args.jp = reinterpret_cast<const ulonglong2*>(ws->jp);
+    args.jp = reinterpret_cast<const float4*>(ws->jp);
     args.acc = acc_out;
     args.pot = pot_out;
     args.partial = reinterpret_cast<double4*>(ws->partial);
     args.n_i = (int)n_i;
-    args.n_units = (int)(plan.n_pairs_padded / nb::kUnitPairs);
+    args.n_j = (int)n_j;
     args.S = plan.S;
     args.eps2 = eps2;
-    rc = exact_mask_enabled() ? launch_force<true>(args, plan, stream) : launch_force<false>(args, plan, stream);
+    rc = (spec_allowed() && eps2 >= kSpecMinEps2) ? launch_force<true>(args, plan, stream) : launch_force<false>(args, plan, stream);
     if (rc != NB_OK) return rc;
 
     if (plan.S > 1) {
@@ -308,11 +323,42 @@ int nb_plan_query(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]) {
     if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
     const nb::Plan p = nb::make_plan(n_i, n_j, sm_count);
     out[0] = p.K; out[1] = p.WI; out[2] = p.WJ; out[3] = p.S;
-    out[4] = p.tiles_i; out[5] = p.tile_i; out[6] = p.tile_pairs; out[7] = p.stages;
+    out[4] = p.tiles_i; out[5] = p.tile_i; out[6] = p.tile_j; out[7] = p.stages;
     return NB_OK;
 }
 
 int64_t nb_last_launch_count(void) { return t_launches; }
+
+int nb_profile_enable(int on) {
+    t_profile = (on != 0);
+    return NB_OK;
+}
+
+int nb_profile_read(int64_t* n_launches, double* total_ms) {
+    if (!n_launches || !total_ms) return NB_ERR_INVALID_VALUE;
+    double sum = 0.0;
+    int64_t n = 0;
+    int rc = NB_OK;
+    for (auto& ev : t_events) {
+        float ms = 0.0f;
+        cudaError_t e = cudaEventSynchronize(ev.second);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, ev.first, ev.second);
+        if (e != cudaSuccess) {
+            t_last_cuda_error = (int)e;
+            (void)cudaGetLastError();
+            rc = NB_ERR_CUDA;
+        } else {
+            sum += ms;
+            ++n;
+        }
+        (void)cudaEventDestroy(ev.first);
+        (void)cudaEventDestroy(ev.second);
+    }
+    t_events.clear();
+    *n_launches = n;
+    *total_ms = sum;
+    return rc;
+}
 
 int nb_release_workspace(void) {
     int dev = 0;

@@ -74,7 +74,7 @@ def test_ragged_shapes_separate_sets(nb, n_i, n_j):
     check_parity(acc, pot, ref_acc, ref_pot, f"{n_i}x{n_j}")
 
 
-PLANS = [(k, 8 // wj, wj, s) for k in (1, 2, 4) for wj in (1, 2, 4, 8) for s in (1, 3)]
+PLANS = [(k, 8 // wj, wj, s) for k in (2, 4, 8) for wj in (1, 2, 4, 8) for s in (1, 3)]
 
 
 @pytest.mark.parametrize("plan", PLANS, ids=lambda p: "K%d_WI%d_WJ%d_S%d" % p)
@@ -87,13 +87,39 @@ def test_every_decomposition_matches_oracle(nb, plan, monkeypatch):
     check_parity(acc, pot, ref_acc, ref_pot, str(plan))
 
 
-def test_approximate_mask_variant(nb, monkeypatch):
-    # NB_MASK is read once per process; this only checks the default (exact) path is the one running
+def test_speculative_and_always_masked_kernels_agree_bitwise(nb, monkeypatch):
+    """The speculative-mask kernel redoes a tile with the exact mask when r2 == eps2 occurred, so its output is
+    the always-masked kernel's, bit for bit -- with self pairs (aliased sets), duplicates and near-coincident pairs."""
     w = wl.config(0)
-    acc, pot = gpu_force(nb, w.xi, w.x_j, w.m_j, w.eps2, alias=True)
-    ref_acc, ref_pot = oracle.force(w.xi, w.x_j, w.m_j, w.eps2)
+    x = w.x_j.copy()
+    x[100] = x[7]                                  # exact duplicates
+    x[101] = x[7]
+    x[300] = x[8] + np.float32(1e-7)               # closer than eps * 2.4e-4: r2 rounds to eps2 without coincidence
+    ref_acc, ref_pot = oracle.force(x, x, w.m_j, w.eps2)
+    monkeypatch.setenv("NB_MASK", "exact")
+    a_e, p_e = gpu_force(nb, x, x, w.m_j, w.eps2, alias=True)
+    monkeypatch.delenv("NB_MASK")
+    a_s, p_s = gpu_force(nb, x, x, w.m_j, w.eps2, alias=True)
+    assert np.array_equal(a_e, a_s) and np.array_equal(p_e, p_s)
     # the self term would shift phi by m/eps = 64/2048 = 3e-2 absolute (~3 % relative): far outside tolerance
-    check_parity(acc, pot, ref_acc, ref_pot, "C0 mask")
+    check_parity(a_s, p_s, ref_acc, ref_pot, "C0 + duplicates")
+    # separate i-set drawn from the j-set (C2 shape): each i coincides with exactly one j
+    w2 = wl.subset_workload(5000, 700, 1.0 / 128, seed=9)
+    monkeypatch.setenv("NB_MASK", "exact")
+    a_e, p_e = gpu_force(nb, w2.x_i, w2.x_j, w2.m_j, w2.eps2)
+    monkeypatch.delenv("NB_MASK")
+    a_s, p_s = gpu_force(nb, w2.x_i, w2.x_j, w2.m_j, w2.eps2)
+    assert np.array_equal(a_e, a_s) and np.array_equal(p_e, p_s)
+
+
+def test_tiny_eps2_uses_masked_kernel(nb):
+    # eps2 below the speculative kernel's threshold (and denormal-small): still finite and within tolerance
+    w = wl.plummer_workload(700, 1.0 / 64, seed=6)
+    for eps2 in (1e-13, 1e-30):
+        acc, pot = gpu_force(nb, w.xi, w.x_j, w.m_j, eps2, alias=True)
+        ref_acc, ref_pot = oracle.force(w.xi, w.x_j, w.m_j, np.float32(eps2))
+        assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot))
+        check_parity(acc, pot, ref_acc, ref_pot, f"eps2={eps2}")
 
 
 # ------------------------------------------------------------------ edge cases
