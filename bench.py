@@ -126,6 +126,23 @@ def oracle_rate(w, target_seconds: float, rng_seed: int = 0):
     return n_i * w.n_j / t, cores, f"{n_i} of {w.n_i} i-particles (seeded, sorted) x all {w.n_j} j-particles, {t:.2f} s"
 
 
+def reduce_max(values, world):
+    """Max over ranks of a list of floats (device timings): NCCL on the GPU, gloo on the CPU tests."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor(list(values), dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def replica_throughput(pairs_per_rank_step, world, steps, total_ms):
+    """Whole-job interactions/s of `world` independent replicas: all ranks' units / the slowest rank's time."""
+    return world * pairs_per_rank_step * steps / (total_ms * 1e-3)
+
+
 def reference_arm(args, w, cfg_name):
     """--impl reference: the CPU oracle (this tier has no reference implementation), rank 0 only."""
     rank = int(os.environ.get("RANK", "0"))
@@ -253,15 +270,12 @@ def main():
     d2h = h_acc.numel() * 4 + h_pot.numel() * 4
 
     # max over ranks
-    if world > 1:
-        t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, e2e_ms = float(t[0]), float(t[1])
+    total_ms, e2e_ms = reduce_max([total_ms, e2e_ms], world)
 
     if rank == 0:
         pairs = float(w.pairs)
-        value = world * pairs * args.steps / (total_ms * 1e-3)
-        e2e_value = world * pairs * e2e_steps / (e2e_ms * 1e-3)
+        value = replica_throughput(pairs, world, args.steps, total_ms)
+        e2e_value = replica_throughput(pairs, world, e2e_steps, e2e_ms)
         f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
         sm_count = torch.cuda.get_device_properties(0).multi_processor_count
         peak_inst = sm_count * FP32_LANES_PER_SM_CLK * f_max                 # FP32-pipe lane-instructions / s

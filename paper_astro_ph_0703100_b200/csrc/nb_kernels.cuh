@@ -188,7 +188,7 @@ struct ForceArgs {
 // Each sub-range is streamed through its own shared-memory ring by 1-D TMA bulk copies issued by
 // lane 0 of the group's first warp; "full" mbarriers count bytes, "empty" mbarriers count the WI
 // consuming warps.
-template <int K, int WI, int WJ, int TJ, int STAGES, bool SPEC>
+template <int K, int WI, int WJ, int TJ, int STAGES, bool SPEC, int SUB = 256>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -222,12 +222,13 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
     const unsigned char* src = reinterpret_cast<const unsigned char*>(a.jp + j_begin);
 
     // a3: i-particles of this thread (clamped loads; stores are guarded), pair k2 = (k = 2 k2, 2 k2 + 1)
-    const int i_base = blockIdx.x * (32 * K * WI) + wi * 32 + lane;
+    // a warp owns 32*K consecutive i-particles, so that an aliased i-set meets its own copies in few j-tiles
+    const int i_base = blockIdx.x * (32 * K * WI) + wi * (32 * K) + lane;
     u64 nxi[K / 2], nyi[K / 2], nzi[K / 2];
 #pragma unroll
     for (int k2 = 0; k2 < K / 2; ++k2) {
-        const int i0 = min(i_base + (2 * k2) * 32 * WI, a.n_i - 1);
-        const int i1 = min(i_base + (2 * k2 + 1) * 32 * WI, a.n_i - 1);
+        const int i0 = min(i_base + (2 * k2) * 32, a.n_i - 1);
+        const int i1 = min(i_base + (2 * k2 + 1) * 32, a.n_i - 1);
         nxi[k2] = pack2(-a.x_i[3 * i0 + 0], -a.x_i[3 * i1 + 0]);
         nyi[k2] = pack2(-a.x_i[3 * i0 + 1], -a.x_i[3 * i1 + 1]);
         nzi[k2] = pack2(-a.x_i[3 * i0 + 2], -a.x_i[3 * i1 + 2]);
@@ -258,23 +259,26 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
         const int np = min(TJ, n_sub - t * TJ);
         const float4* sp = reinterpret_cast<const float4*>(rings + wj * RING_BYTES + slot * TJ * 16);
 
-        u64 pax[K / 2], pay[K / 2], paz[K / 2], pph[K / 2];            // tile partial sums (Eq. (2))
-        if (SPEC) {
-            const bool hit = tile_sweep<K, MASK_SPEC>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
-            if (__any_sync(0xffffffffu, hit))                          // rare: some pair of this warp may be coincident
-                (void)tile_sweep<K, MASK_EXACT>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
-        } else {
-            (void)tile_sweep<K, MASK_EXACT>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
-        }
-
-        // a5: tile partial -> running total
+        // Eq. (2) blocks of at most SUB consecutive j: partial sums from zero, then added to the running total
+        for (int c = 0; c < np; c += SUB) {
+            const int nc = min(SUB, np - c);
+            u64 pax[K / 2], pay[K / 2], paz[K / 2], pph[K / 2];
+            if (SPEC) {
+                const bool hit = tile_sweep<K, MASK_SPEC>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+                if (__any_sync(0xffffffffu, hit))                      // rare: some pair of this warp may be coincident
+                    (void)tile_sweep<K, MASK_EXACT>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+            } else {
+                (void)tile_sweep<K, MASK_EXACT>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+            }
+            // a5: block partial -> running total
 #pragma unroll
-        for (int k2 = 0; k2 < K / 2; ++k2) {
-            float lo, hi;
-            unpack2(pax[k2], lo, hi); run[2 * k2][0] += (double)lo; run[2 * k2 + 1][0] += (double)hi;
-            unpack2(pay[k2], lo, hi); run[2 * k2][1] += (double)lo; run[2 * k2 + 1][1] += (double)hi;
-            unpack2(paz[k2], lo, hi); run[2 * k2][2] += (double)lo; run[2 * k2 + 1][2] += (double)hi;
-            unpack2(pph[k2], lo, hi); run[2 * k2][3] += (double)lo; run[2 * k2 + 1][3] += (double)hi;
+            for (int k2 = 0; k2 < K / 2; ++k2) {
+                float lo, hi;
+                unpack2(pax[k2], lo, hi); run[2 * k2][0] += (double)lo; run[2 * k2 + 1][0] += (double)hi;
+                unpack2(pay[k2], lo, hi); run[2 * k2][1] += (double)lo; run[2 * k2 + 1][1] += (double)hi;
+                unpack2(paz[k2], lo, hi); run[2 * k2][2] += (double)lo; run[2 * k2 + 1][2] += (double)hi;
+                unpack2(pph[k2], lo, hi); run[2 * k2][3] += (double)lo; run[2 * k2 + 1][3] += (double)hi;
+            }
         }
 
         // release the slot; the producer refills it with tile t' + STAGES.  With several consumer
@@ -320,7 +324,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
     // a6: epilogue
 #pragma unroll
     for (int k = 0; k < K; ++k) {
-        const int i = i_base + k * 32 * WI;
+        const int i = i_base + k * 32;
         if (i >= a.n_i) continue;
         if (a.S == 1) {
             a.acc[3 * i + 0] = (float)run[k][0];

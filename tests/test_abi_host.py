@@ -1,0 +1,84 @@
+"""CPU-only checks of the C-ABI library and its host logic: the shared library loads, exports every symbol
+include/nbody_b200.h declares, validates arguments before touching CUDA, fails loudly (never silently succeeds)
+without a device, and the launch planner is a sane pure function.  No compute calls are made here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_astro_ph_0703100_b200 as nb
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "nbody_b200.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(nb_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    names = declared_functions()
+    assert {"nb_force", "nb_force_host", "nb_leapfrog_kdk", "nb_plan_query", "nb_status_string", "nb_version"} <= set(names)
+    lib = nb.lib()
+    for name in names:
+        assert hasattr(lib, name), f"{name} is declared in include/nbody_b200.h but not exported"
+    assert nb.version() >= 100
+
+
+def test_status_strings():
+    for code, word in ((0, "NB_OK"), (1, "INVALID"), (2, "CUDA"), (3, "ALLOC"), (4, "UNSUPPORTED")):
+        assert word in nb.status_string(code)
+    assert "unknown" in nb.status_string(99)
+
+
+def test_argument_validation_happens_before_any_cuda_call():
+    lib = nb.lib()
+    buf = (ctypes.c_float * 12)()
+    p = ctypes.addressof(buf)
+    assert lib.nb_force(-1, p, 1, p, p, 0.1, p, None, None) == 1
+    assert lib.nb_force(1, p, 2 ** 31, p, p, 0.1, p, None, None) == 1
+    assert lib.nb_force(1, None, 1, p, p, 0.1, p, None, None) == 1
+    assert lib.nb_force(1, p, 1, p, None, 0.1, p, None, None) == 1
+    assert lib.nb_force(1, p, 1, p, p, -0.5, p, None, None) == 1
+    assert lib.nb_force(1, p, 1, p, p, float("nan"), p, None, None) == 1
+    assert lib.nb_force_host(1, p, 1, p, p, float("inf"), p, None) == 1
+    assert lib.nb_leapfrog_kdk(4, p, p, p, 0.1, float("nan"), 1, p, None, None) == 1
+    assert lib.nb_leapfrog_kdk(4, p, p, p, 0.1, 0.1, -1, p, None, None) == 1
+    assert lib.nb_leapfrog_kdk(4, None, p, p, 0.1, 0.1, 1, p, None, None) == 1
+    out = (ctypes.c_int64 * 8)()
+    assert lib.nb_plan_query(0, 5, 148, out) == 1
+    assert lib.nb_plan_query(5, 5, 148, None) == 1
+
+
+def test_no_cpu_fallback_without_a_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    lib = nb.lib()
+    buf = (ctypes.c_float * 12)()
+    p = ctypes.addressof(buf)
+    st = lib.nb_force_host(1, p, 1, p, p, 0.1, p, None)
+    assert st in (2, 4), "without a B200 the library must report an error, not compute on the CPU"
+
+
+@pytest.mark.parametrize("n_i,n_j", [(1, 1), (1, 777), (31, 1000), (512, 65536), (2048, 2048), (65536, 65536),
+                                      (131072, 131072), (1048576, 1048576), (2 ** 31 - 1, 9)])
+def test_planner_invariants(n_i, n_j):
+    p = nb.plan_query(n_i, n_j, 148)
+    assert p["K"] in (2, 4, 8) and p["WI"] * p["WJ"] == 8 and p["WJ"] in (1, 2, 4, 8)
+    assert p["tile_i"] == 32 * p["K"] * p["WI"]
+    assert p["tiles_i"] * p["tile_i"] >= n_i > (p["tiles_i"] - 1) * p["tile_i"]
+    assert 1 <= p["S"] <= 2048 and p["S"] * p["WJ"] <= max(1, n_j)
+    assert p["tile_j"] * 16 * p["stages"] * p["WJ"] <= 200 * 1024            # fits shared memory
+    assert p == nb.plan_query(n_i, n_j, 148)                                  # pure function
+    assert nb.plan_query(n_i, n_j, 0) == p                                    # sm_count <= 0 means 148
+
+
+def test_planner_fills_the_machine_for_the_bench_config():
+    p = nb.plan_query(131072, 131072, 148)
+    ctas = p["tiles_i"] * p["S"]
+    assert ctas >= 148 and p["K"] == 8
+    waves = ctas / 148.0
+    assert waves / -(-ctas // 148) > 0.9                                       # < 10 % wave-quantisation loss
