@@ -33,6 +33,9 @@ FP32_INST_PER_PAIR = 13          # FMA-pipe instructions per interaction (acc + 
 FP32_LANES_PER_SM_CLK = 128
 CONFIG_INDEX = {"C0": 0, "C1": 1, "C2": 2, "C3": 3, "C4": 4}
 L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
+# dram__bytes_read.sum + dram__bytes_write.sum of one nb_force_kernel launch, from the committed
+# `ncu --set full` captures (profiles/r01_force_c1_ncu_full.md); null for configs without a capture
+NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 8.63e6}
 
 
 def load_peaks():
@@ -284,7 +287,8 @@ def main():
         roofline = {
             "bound": "alu", "kernel": "nb_force_kernel (pair interaction, rows a2-a7)",
             "achieved": achieved / 1e12, "peak": peak_inst / 1e12, "unit": "FP32-pipe Tinst/s",
-            "frac": achieved / peak_inst, "traffic": None,
+            "frac": achieved / peak_inst, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config),
+            "traffic_unit": "DRAM bytes per launch (ncu --set full, profiles/r01_force_c1_ncu_full.md)",
             "kernel_ms": k_ms / max(1, n_k), "kernel_launches_timed": n_k,
             "kernel_interactions_per_s": k_rate, "roofline_interactions_per_s": peak_inst / FP32_INST_PER_PAIR,
             "peak_source": f"{sm_count} SMs x {FP32_LANES_PER_SM_CLK} FP32 lanes x sm_max_mhz {f_max / 1e6:.0f} MHz "
