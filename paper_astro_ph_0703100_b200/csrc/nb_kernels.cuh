@@ -115,7 +115,10 @@ __global__ void __launch_bounds__(256) nb_pack_j_kernel(const float* __restrict_
 //                coincidence, since fma(0, 0, eps2) == eps2): 1 ALU instruction, 1 register read per
 //                pair.  The caller recomputes the whole tile with MASK_EXACT when the flag is set, so
 //                the stored result is always the MASK_EXACT one.  Requires eps2 > 0.
-enum { MASK_EXACT = 0, MASK_SPEC = 1 };
+//   MASK_NONE  : no masking and no flag; only valid for a block of j-particles that is known (from the
+//                coincidence lists built by nb_coin_probe_kernel) to hold no partner of this warp's
+//                i-particles, where it gives bit for bit what MASK_EXACT gives.  13 + 1 instructions.
+enum { MASK_EXACT = 0, MASK_SPEC = 1, MASK_NONE = 2 };
 
 template <int MASK>
 __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nxi, u64 nyi, u64 nzi, u64 eps2_2,
@@ -137,7 +140,7 @@ __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nx
         const uint32_t tb = __float_as_uint(dxb) | __float_as_uint(dyb) | __float_as_uint(dzb);
         r2a = (ta == 0u) ? inf : r2a;                // rsqrt(+inf) = +0 -> the pair adds exactly 0
         r2b = (tb == 0u) ? inf : r2b;
-    } else {
+    } else if (MASK == MASK_SPEC) {
         hit |= (r2a == eps2);
         hit |= (r2b == eps2);
     }
@@ -170,17 +173,124 @@ __device__ __forceinline__ bool tile_sweep(const float4* __restrict__ sp, int np
     return hit;
 }
 
+// ---------------------------------------------------------------- coincidence lists (reading R1, large calls)
+// For large calls the coincident pairs (reading R1) are located BEFORE the force kernel by
+// a hash join on the positions, so that the hot loop carries no test at all (MASK_NONE) and only the
+// few (i-group, j-segment) combinations that do hold a coincident pair run the masked loop:
+//   nb_coin_insert_kernel : every j-particle is entered in an open-addressing table keyed by its
+//                           canonical position bits (subnormals and -0 -> +0, as add.ftz sees them);
+//   nb_coin_probe_kernel  : one CTA per i-group (the 32*K i-particles one warp of the force kernel
+//                           owns) looks its i-particles up and writes the sorted list of j-SEGMENTS
+//                           (kCoinSeg consecutive j, global index / kCoinSeg) that hold a partner.
+// List layout: int [n_groups][1 + kCoinCap] = (count, segment ids ascending); count = -1 means "too
+// many, mask every block".  *flag != 0 means the table degenerated (very many identical positions):
+// the force kernel then masks everywhere.  Either way the stored result equals the always-masked one.
+constexpr int kCoinSeg = 256;         // j-particles per segment (= SUB of the force kernel)
+constexpr int kCoinSegShift = 8;
+constexpr int kCoinCap = 8;           // segments kept per i-group
+constexpr int kCoinRaw = 32;          // distinct segments collected per i-group before giving up (set of 64 slots)
+constexpr int kCoinMaxProbe = 2048;   // probe steps before giving up
+
+__device__ __forceinline__ uint32_t coin_canon(float v) {
+    return (fabsf(v) < 1.17549435e-38f) ? 0u : __float_as_uint(v);
+}
+__device__ __forceinline__ uint32_t coin_hash(uint32_t a, uint32_t b, uint32_t c) {
+    uint64_t h = (uint64_t)a * 0x9E3779B97F4A7C15ull;
+    h ^= (uint64_t)b * 0xC2B2AE3D27D4EB4Full + (h >> 29);
+    h ^= (uint64_t)c * 0x165667B19E3779F9ull + (h << 17);
+    h ^= h >> 32;
+    h *= 0xD6E8FEB86659FD93ull;
+    return (uint32_t)(h >> 32);
+}
+
+// table entries: 0 = empty, else j + 1
+__global__ void __launch_bounds__(256) nb_coin_insert_kernel(const float4* __restrict__ jp, int n_j,
+                                                             uint32_t* __restrict__ table, uint32_t mask,
+                                                             int* __restrict__ flag) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_j) return;
+    const float4 J = jp[j];
+    uint32_t slot = coin_hash(coin_canon(J.x), coin_canon(J.y), coin_canon(J.z)) & mask;
+    for (int step = 0; step < kCoinMaxProbe; ++step) {
+        if (table[slot] == 0u && atomicCAS(table + slot, 0u, (uint32_t)j + 1u) == 0u) return;
+        slot = (slot + 1u) & mask;
+    }
+    *flag = 1;                                                         // degenerate input: mask everywhere
+}
+
+__global__ void __launch_bounds__(256) nb_coin_probe_kernel(const float* __restrict__ x_i, int n_i,
+                                                            const float4* __restrict__ jp,
+                                                            const uint32_t* __restrict__ table, uint32_t mask,
+                                                            int* __restrict__ lists) {
+    __shared__ int set[2 * kCoinRaw];                                  // open-addressing set of segment ids, -1 = empty
+    __shared__ int n_set;
+    __shared__ int overflow;
+    if (threadIdx.x < 2 * kCoinRaw) set[threadIdx.x] = -1;
+    if (threadIdx.x == 0) { n_set = 0; overflow = 0; }
+    __syncthreads();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;               // blockDim.x = 32 * K = one i-group
+    if (i < n_i) {
+        const uint32_t cx = coin_canon(x_i[3 * i + 0]), cy = coin_canon(x_i[3 * i + 1]), cz = coin_canon(x_i[3 * i + 2]);
+        uint32_t slot = coin_hash(cx, cy, cz) & mask;
+        int step = 0;
+        for (; step < kCoinMaxProbe; ++step) {
+            const uint32_t e = table[slot];
+            if (e == 0u) break;
+            const float4 J = jp[e - 1u];
+            if (coin_canon(J.x) == cx && coin_canon(J.y) == cy && coin_canon(J.z) == cz) {
+                const int seg = (int)((e - 1u) >> kCoinSegShift);
+                uint32_t h = ((uint32_t)seg * 2654435761u) >> 26;      // 64 slots
+                bool placed = false;
+                for (int q = 0; q < 2 * kCoinRaw && !placed; ++q) {
+                    const int old = atomicCAS(&set[h], -1, seg);
+                    if (old == seg) placed = true;
+                    else if (old == -1) { placed = true; if (atomicAdd(&n_set, 1) >= kCoinRaw) overflow = 1; }
+                    h = (h + 1u) & (2 * kCoinRaw - 1);
+                }
+                if (!placed) overflow = 1;
+                if (*(volatile int*)&overflow) break;
+            }
+            slot = (slot + 1u) & mask;
+        }
+        if (step == kCoinMaxProbe) overflow = 1;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int* out = lists + (size_t)blockIdx.x * (1 + kCoinCap);
+        int n = 0, cnt = 0;
+        int seg[2 * kCoinRaw];
+        for (int q = 0; q < 2 * kCoinRaw; ++q)
+            if (set[q] >= 0) seg[n++] = set[q];
+        for (int a = 1; a < n; ++a) {                                  // insertion sort of <= 64 distinct entries
+            const int v = seg[a];
+            int b = a - 1;
+            while (b >= 0 && seg[b] > v) { seg[b + 1] = seg[b]; --b; }
+            seg[b + 1] = v;
+        }
+        const bool too_many = (overflow != 0) || n > kCoinCap;
+        for (int q = 0; q < n && !too_many; ++q) out[1 + cnt++] = seg[q];
+        out[0] = too_many ? -1 : cnt;
+    }
+}
+
 struct ForceArgs {
     const float* x_i;      // [n_i][3]
     const float4* jp;      // packed j records (x, y, z, m)
     float* acc;            // [n_i][3]
     float* pot;            // [n_i] or nullptr
     double4* partial;      // [S][n_i] when S > 1
+    const int* coin_lists; // MODE_LIST: [n_groups][1 + kCoinCap]
+    const int* coin_flag;  // MODE_LIST: != 0 -> mask everywhere
     int n_i;
     int n_j;
     int S;
     float eps2;
 };
+
+// how the force kernel honours the coincident-pair rule
+enum { MODE_EXACT = 0,     // masked loop everywhere (eps2 == 0 or tiny)
+       MODE_SPEC = 1,      // unmasked loop + flag, masked redo of a flagged block (small calls)
+       MODE_LIST = 2 };    // coincidence lists from the pre-pass, no test in the hot loop (large calls)
 
 // ---------------------------------------------------------------- a2..a7: the force kernel
 // CTA = 8 warps = WI (along i) x WJ (along j).  A CTA owns 32*K*WI i-particles (K per thread, in
@@ -188,9 +298,10 @@ struct ForceArgs {
 // Each sub-range is streamed through its own shared-memory ring by 1-D TMA bulk copies issued by
 // lane 0 of the group's first warp; "full" mbarriers count bytes, "empty" mbarriers count the WI
 // consuming warps.
-template <int K, int WI, int WJ, int TJ, int STAGES, bool SPEC, int SUB = 256>
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, int SUB = 256>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
+    static_assert(SUB == kCoinSeg, "coincidence segments are SUB j-particles");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int RING_BYTES = STAGES * TJ * 16;
     unsigned char* rings = smem_raw;                                   // [WJ][STAGES][TJ] float4
@@ -251,6 +362,15 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
 #pragma unroll
     for (int k = 0; k < K; ++k) { run[k][0] = run[k][1] = run[k][2] = run[k][3] = 0.0; }
 
+    // MODE_LIST: ascending j-segments that hold a partner of this warp's i-particles (warp-uniform)
+    const int* coin = nullptr;
+    int coin_cnt = 0, coin_pos = 0, coin_next = 0x7fffffff;
+    if (MODE == MODE_LIST) {
+        coin = a.coin_lists + (size_t)(blockIdx.x * WI + wi) * (1 + kCoinCap);
+        coin_cnt = (*a.coin_flag != 0) ? -1 : coin[0];
+        if (coin_cnt > 0) coin_next = coin[1];
+    }
+
     for (int t = 0; t < n_tiles; ++t) {
         const int slot = t % STAGES;
         const uint32_t parity = (uint32_t)(t / STAGES) & 1u;
@@ -263,10 +383,21 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
         for (int c = 0; c < np; c += SUB) {
             const int nc = min(SUB, np - c);
             u64 pax[K / 2], pay[K / 2], paz[K / 2], pph[K / 2];
-            if (SPEC) {
+            if (MODE == MODE_SPEC) {
                 const bool hit = tile_sweep<K, MASK_SPEC>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
                 if (__any_sync(0xffffffffu, hit))                      // rare: some pair of this warp may be coincident
                     (void)tile_sweep<K, MASK_EXACT>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+            } else if (MODE == MODE_LIST) {
+                const int j0 = j_begin + t * TJ + c;                   // global index of the block's first j
+                const int seg_lo = j0 >> kCoinSegShift, seg_hi = (j0 + nc - 1) >> kCoinSegShift;
+                while (coin_next < seg_lo) {
+                    ++coin_pos;
+                    coin_next = (coin_pos < coin_cnt) ? coin[1 + coin_pos] : 0x7fffffff;
+                }
+                if (coin_cnt < 0 || coin_next <= seg_hi)               // rare: the block holds a coincident pair
+                    (void)tile_sweep<K, MASK_EXACT>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+                else
+                    (void)tile_sweep<K, MASK_NONE>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
             } else {
                 (void)tile_sweep<K, MASK_EXACT>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
             }

@@ -53,7 +53,10 @@ inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, i
     const double j_per_cta = double(n_j) / S;
     // fewer i-particles per thread: more shared-memory reads and loop overhead per pair
     const double k_pen = (K == 8) ? 1.0 : (K == 4 ? 1.03 : 1.12);
-    double cta_cycles = c_fixed + double(tile_i) * j_per_cta * pair_cycles * k_pen;
+    // measured on B200 at full occupancy (one wave of 148 CTAs, K = 8): WJ = 1 / 2 / 4 / 8 reach
+    // 82.8 / 77.9 / 81.7 / 81.6 % of the FP32 roofline
+    const double wj_pen = (WJ == 1) ? 1.0 : (WJ == 2 ? 1.06 : 1.014);
+    double cta_cycles = c_fixed + double(tile_i) * j_per_cta * pair_cycles * k_pen * wj_pen;
     if (WJ > 1) cta_cycles += 1500.0;                 // cross-warp reduction through shared memory
     double cost = waves * cta_cycles;
     if (S > 1) cost += c_reduce_launch + double(n_i) * S * 32.0 / 2500.0;  // ~5 TB/s at ~2 GHz

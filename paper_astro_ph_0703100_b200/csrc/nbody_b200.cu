@@ -45,6 +45,7 @@ struct Workspace {
     void* jp = nullptr;        size_t jp_bytes = 0;        // packed pair records
     void* partial = nullptr;   size_t partial_bytes = 0;   // [S][n_i] double4
     void* stage = nullptr;     size_t stage_bytes = 0;     // device copies for nb_force_host
+    void* coin = nullptr;      size_t coin_bytes = 0;      // coincidence pre-pass: flag | lists | hash table
 };
 
 std::mutex g_mutex;
@@ -103,18 +104,26 @@ nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count) {
 // the always-masked kernel runs.  2^-40: rsqrt(eps2)^3 = 2^60.
 constexpr float kSpecMinEps2 = 9.094947017729282e-13f;
 
-bool spec_allowed() {
-    // debugging aid: NB_MASK=exact forces the always-masked kernel
+// Calls with at least this many pairs locate their coincident pairs with the hash-join pre-pass
+// (MODE_LIST: three extra O(n) launches, no test in the hot loop); smaller ones use MODE_SPEC.
+constexpr double kListMinPairs = 1073741824.0;   // 2^30
+
+int pick_mode(int64_t n_i, int64_t n_j, float eps2) {
+    // debugging aid: NB_MASK=exact|spec|list forces a mode (spec/list still need eps2 >= 2^-40)
     const char* e = std::getenv("NB_MASK");
-    return !(e && e[0] == 'e');
+    if (e && e[0] == 'e') return nb::MODE_EXACT;
+    if (eps2 < kSpecMinEps2) return nb::MODE_EXACT;
+    if (e && e[0] == 's') return nb::MODE_SPEC;
+    if (e && e[0] == 'l') return nb::MODE_LIST;
+    return ((double)n_i * (double)n_j >= kListMinPairs) ? nb::MODE_LIST : nb::MODE_SPEC;
 }
 
-template <int K, int WI, int WJ, int TJ, int STAGES, bool SPEC>
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE>
 int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
     constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, SPEC>;
+    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE>;
     static bool configured[64] = {};
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
@@ -140,22 +149,22 @@ int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStrea
 }
 
 // tile_j / stages per WJ must match nb::ring_shape (nb_plan.h)
-template <int K, bool SPEC>
+template <int K, int MODE>
 int launch_force_k(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     switch (plan.WJ) {
-        case 1: return launch_force_inst<K, 8, 1, 512, 4, SPEC>(args, plan, stream);
-        case 2: return launch_force_inst<K, 4, 2, 512, 4, SPEC>(args, plan, stream);
-        case 4: return launch_force_inst<K, 2, 4, 256, 4, SPEC>(args, plan, stream);
-        default: return launch_force_inst<K, 1, 8, 256, 3, SPEC>(args, plan, stream);
+        case 1: return launch_force_inst<K, 8, 1, 512, 4, MODE>(args, plan, stream);
+        case 2: return launch_force_inst<K, 4, 2, 512, 4, MODE>(args, plan, stream);
+        case 4: return launch_force_inst<K, 2, 4, 256, 4, MODE>(args, plan, stream);
+        default: return launch_force_inst<K, 1, 8, 256, 3, MODE>(args, plan, stream);
     }
 }
 
-template <bool SPEC>
+template <int MODE>
 int launch_force(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     switch (plan.K) {
-        case 2: return launch_force_k<2, SPEC>(args, plan, stream);
-        case 4: return launch_force_k<4, SPEC>(args, plan, stream);
-        default: return launch_force_k<8, SPEC>(args, plan, stream);
+        case 2: return launch_force_k<2, MODE>(args, plan, stream);
+        case 4: return launch_force_k<4, MODE>(args, plan, stream);
+        default: return launch_force_k<8, MODE>(args, plan, stream);
     }
 }
 
@@ -210,7 +219,37 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.n_j = (int)n_j;
     args.S = plan.S;
     args.eps2 = eps2;
-    rc = (spec_allowed() && eps2 >= kSpecMinEps2) ? launch_force<true>(args, plan, stream) : launch_force<false>(args, plan, stream);
+    args.coin_lists = nullptr;
+    args.coin_flag = nullptr;
+    const int mode = pick_mode(n_i, n_j, eps2);
+    if (mode == nb::MODE_LIST) {
+        // coincidence pre-pass: hash table over the j-positions, one sorted j-segment list per i-group
+        const int group = 32 * plan.K;
+        const int64_t n_groups = (int64_t)plan.tiles_i * plan.WI;    // every warp slot of the grid has a list
+        uint32_t slots = 1024;
+        while ((int64_t)slots < 2 * n_j) slots <<= 1;
+        const size_t b_lists = ((size_t)(1 + n_groups * (1 + nb::kCoinCap)) * sizeof(int) + 255) / 256 * 256;
+        rc = ensure(&ws->coin, &ws->coin_bytes, b_lists + (size_t)slots * sizeof(uint32_t), stream);
+        if (rc != NB_OK) return rc;
+        int* flag = reinterpret_cast<int*>(ws->coin);
+        int* lists = flag + 1;
+        uint32_t* table = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(ws->coin) + b_lists);
+        NB_CUDA(cudaMemsetAsync(ws->coin, 0, b_lists + (size_t)slots * sizeof(uint32_t), stream));
+        nb::nb_coin_insert_kernel<<<(unsigned)((n_j + 255) / 256), 256, 0, stream>>>(
+            reinterpret_cast<const float4*>(ws->jp), (int)n_j, table, slots - 1, flag);
+        NB_CUDA(cudaGetLastError());
+        nb::nb_coin_probe_kernel<<<(unsigned)n_groups, group, 0, stream>>>(
+            x_i, (int)n_i, reinterpret_cast<const float4*>(ws->jp), table, slots - 1, lists);
+        NB_CUDA(cudaGetLastError());
+        t_launches += 2;
+        args.coin_lists = lists;
+        args.coin_flag = flag;
+        rc = launch_force<nb::MODE_LIST>(args, plan, stream);
+    } else if (mode == nb::MODE_SPEC) {
+        rc = launch_force<nb::MODE_SPEC>(args, plan, stream);
+    } else {
+        rc = launch_force<nb::MODE_EXACT>(args, plan, stream);
+    }
     if (rc != NB_OK) return rc;
 
     if (plan.S > 1) {
@@ -370,6 +409,7 @@ int nb_release_workspace(void) {
             if (it->second.jp) (void)cudaFree(it->second.jp);
             if (it->second.partial) (void)cudaFree(it->second.partial);
             if (it->second.stage) (void)cudaFree(it->second.stage);
+            if (it->second.coin) (void)cudaFree(it->second.coin);
             it = g_ws.erase(it);
         } else {
             ++it;

@@ -112,6 +112,64 @@ def test_speculative_and_always_masked_kernels_agree_bitwise(nb, monkeypatch):
     assert np.array_equal(a_e, a_s) and np.array_equal(p_e, p_s)
 
 
+def _three_modes(nb, monkeypatch, x_i, x_j, m_j, eps2, alias=False):
+    out = {}
+    for mode in ("exact", "spec", "list"):
+        monkeypatch.setenv("NB_MASK", mode)
+        out[mode] = gpu_force(nb, x_i, x_j, m_j, eps2, alias=alias)
+    monkeypatch.delenv("NB_MASK")
+    return out
+
+
+@pytest.mark.parametrize("plan", [(8, 8, 1, 3), (8, 4, 2, 1), (4, 2, 4, 5), (2, 1, 8, 2), (4, 8, 1, 1), (2, 4, 2, 7)],
+                         ids=lambda p: "K%d_WI%d_WJ%d_S%d" % p)
+def test_list_mode_agrees_bitwise_with_masked_kernel(nb, plan, monkeypatch):
+    """MODE_LIST (hash-join pre-pass, untested hot loop, masked loop only on listed j-segments) stores what the
+    always-masked kernel stores, bit for bit: self pairs, duplicates across segments, -0 vs +0, subnormals."""
+    monkeypatch.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
+    w = wl.plummer_workload(3000, 1.0 / 64, seed=12)
+    x = w.x_j.copy()
+    x[2999] = x[5]                                 # duplicate far away in j (another segment)
+    x[1500] = x[5]
+    x[700] = (0.0, 0.0, 0.0)
+    x[2100] = (-0.0, 1e-41, 0.0)                   # canonically equal to particle 700 (add.ftz flushes subnormals)
+    x[300] = x[8] + np.float32(1e-7)               # near, not coincident
+    out = _three_modes(nb, monkeypatch, x, x, w.m_j, w.eps2, alias=True)
+    for mode in ("spec", "list"):
+        assert np.array_equal(out["exact"][0], out[mode][0]), mode
+        assert np.array_equal(out["exact"][1], out[mode][1]), mode
+    ref_acc, ref_pot = oracle.force(x, x, w.m_j, w.eps2)
+    keep = np.ones(3000, bool); keep[[700, 2100]] = False      # the oracle does not flush 1e-41: that pair differs by design
+    check_parity(out["list"][0][keep], out["list"][1][keep], ref_acc[keep], ref_pot[keep], "list " + str(plan))
+    # separate i-set drawn from the j-set (C2 shape)
+    w2 = wl.subset_workload(5000, 700, 1.0 / 128, seed=9)
+    out = _three_modes(nb, monkeypatch, w2.x_i, w2.x_j, w2.m_j, w2.eps2)
+    assert np.array_equal(out["exact"][0], out["list"][0]) and np.array_equal(out["exact"][1], out["list"][1])
+    ref_acc, ref_pot = oracle.force(w2.x_i, w2.x_j, w2.m_j, w2.eps2)
+    check_parity(out["list"][0], out["list"][1], ref_acc, ref_pot, "list subset " + str(plan))
+
+
+def test_list_mode_degenerate_inputs(nb, monkeypatch):
+    """Overflowing lists (> 8 partner segments per i-group) and a degenerate table (thousands of identical
+    positions) fall back to masking everywhere: still the always-masked result."""
+    rng = np.random.default_rng(3)
+    n = 6000
+    x = rng.normal(size=(n, 3)).astype(np.float32)
+    m = rng.uniform(0.5, 1.5, n).astype(np.float32) / n
+    x[::300] = x[0]                                # 20 copies spread over 20 segments: list overflow for group 0
+    out = _three_modes(nb, monkeypatch, x, x, m, 1e-3, alias=True)
+    assert np.array_equal(out["exact"][0], out["list"][0]) and np.array_equal(out["exact"][1], out["list"][1])
+    ref_acc, ref_pot = oracle.force(x, x, m, 1e-3)
+    check_parity(out["list"][0], out["list"][1], ref_acc, ref_pot, "overflow")
+    x[:5000] = (1.0, 2.0, 3.0)                     # 5000 identical positions: probe chains exceed the cap
+    out = _three_modes(nb, monkeypatch, x, x, m, 1e-3, alias=True)
+    assert np.array_equal(out["exact"][0], out["list"][0]) and np.array_equal(out["exact"][1], out["list"][1])
+    ref_acc, ref_pot = oracle.force(x, x, m, 1e-3)
+    sel = slice(5000, n)                           # the 5000 coincident ones have a ~ 0: compare the others relatively
+    check_parity(out["list"][0][sel], out["list"][1][sel], ref_acc[sel], ref_pot[sel], "degenerate")
+    assert np.abs(out["list"][1][:5000] - ref_pot[:5000]).max() <= 1e-5 * np.abs(ref_pot[:5000]).max()
+
+
 def test_tiny_eps2_uses_masked_kernel(nb):
     # eps2 below the speculative kernel's threshold (and denormal-small): still finite and within tolerance
     w = wl.plummer_workload(700, 1.0 / 64, seed=6)
