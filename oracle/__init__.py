@@ -52,6 +52,10 @@ def _load():
         lib.oracle_energy_f32.restype = ctypes.c_int
         lib.oracle_leapfrog_kdk_f64.argtypes = [i64, p, p, p, f64, f64, i64, p, p]
         lib.oracle_leapfrog_kdk_f64.restype = ctypes.c_int
+        lib.oracle_force_jerk_f64.argtypes = [i64, p, p, i64, p, p, p, f64, p, p, p]
+        lib.oracle_force_jerk_f64.restype = ctypes.c_int
+        lib.oracle_force_jerk_f32.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p]
+        lib.oracle_force_jerk_f32.restype = ctypes.c_int
         lib.oracle_num_threads.restype = ctypes.c_int
         lib.oracle_set_num_threads.argtypes = [ctypes.c_int]
         _lib = lib
@@ -93,6 +97,30 @@ def force(x_i: np.ndarray, x_j: np.ndarray, m_j: np.ndarray, eps2: float,
     if rc != 0:
         raise ValueError(f"oracle_force returned {rc}")
     return acc, pot
+
+
+def force_jerk(x_i: np.ndarray, v_i: np.ndarray, x_j: np.ndarray, v_j: np.ndarray, m_j: np.ndarray, eps2: float,
+               want_pot: bool = True):
+    """Force + jerk + potential of Fig. A.4 in double.  float32 inputs are promoted exactly.
+
+    Returns (acc [n_i,3], jerk [n_i,3], pot [n_i] or None), all float64.
+    """
+    arrs = (x_i, v_i, x_j, v_j, m_j)
+    f32 = all(a.dtype == np.float32 for a in arrs)
+    dt = np.float32 if f32 else np.float64
+    xi, vi = _c(x_i, dt).reshape(-1, 3), _c(v_i, dt).reshape(-1, 3)
+    xj, vj, mj = _c(x_j, dt).reshape(-1, 3), _c(v_j, dt).reshape(-1, 3), _c(m_j, dt).reshape(-1)
+    n_i, n_j = xi.shape[0], xj.shape[0]
+    if vi.shape[0] != n_i or vj.shape[0] != n_j or mj.shape[0] != n_j:
+        raise ValueError("array lengths differ")
+    acc = np.zeros((n_i, 3), dtype=np.float64)
+    jerk = np.zeros((n_i, 3), dtype=np.float64)
+    pot = np.zeros(n_i, dtype=np.float64) if want_pot else None
+    fn = _load().oracle_force_jerk_f32 if f32 else _load().oracle_force_jerk_f64
+    rc = fn(n_i, _ptr(xi), _ptr(vi), n_j, _ptr(xj), _ptr(vj), _ptr(mj), float(eps2), _ptr(acc), _ptr(jerk), _ptr(pot))
+    if rc != 0:
+        raise ValueError(f"oracle_force_jerk returned {rc}")
+    return acc, jerk, pot
 
 
 def energy(x: np.ndarray, v: np.ndarray, m: np.ndarray, eps2: float) -> Tuple[float, float, float]:

@@ -191,3 +191,99 @@ int oracle_leapfrog_kdk_f64(int64_t n, double *x, double *v, const double *m, do
     }
     return rc;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Row f1: force + jerk + potential for the 4th-order Hermite scheme,
+ * the paper's second pipeline description (Fig. A.2, Fig. A.4):
+ *
+ *     a_i    =  sum_j m_j d / r^3                                   d = r_j - r_i, r^2 = d.d + eps^2
+ *     jerk_i =  sum_j m_j [ dv / r^3  -  3 (d.dv) d / r^5 ]         dv = v_j - v_i   (= d a_i / dt)
+ *     phi_i  = -sum_j m_j / r
+ *
+ * Per-pair statements in the order of Fig. A.4: r1i, r2i, r3i, r5i,
+ * mr5i = mj r5i, mf = mr5i r2 (= mj r3i), pot = mf r2 (= mj r1i),
+ * fx = mf d, jk1 = mf dv, xv = d*dv per component,
+ * mf3a = 3 mr5i (xv0+xv1+xv2), jk2 = mf3a d, jk = jk1 - jk2,
+ * OUTPUT[0..2] += fx, OUTPUT[3..5] += jk, OUTPUT[6] -= pot.
+ * Coincident pairs (all three POSITION differences exactly zero) are skipped (reading R1), whatever
+ * their velocities.  Pins (tests/test_oracle_hermite_pins.py): exact two-body rationals, central
+ * finite difference of the (separately pinned) acceleration along the flow, exact rational brute
+ * force at N <= 6, momentum antisymmetry, Galilean and rotation invariance, circular binary.
+ * out7 = (ax, ay, az, jx, jy, jz, phi).
+ */
+static void one_i_jerk(const double xi[3], const double vi[3], int64_t n_j, const double *xj, const double *vj,
+                       const double *mj, double eps2, double out7[7])
+{
+    double ax = 0.0, ay = 0.0, az = 0.0, jx = 0.0, jy = 0.0, jz = 0.0, phi = 0.0;
+    for (int64_t j = 0; j < n_j; ++j) {
+        double dx0 = xj[3 * j + 0] - xi[0];            /* dx = xj - xi */
+        double dx1 = xj[3 * j + 1] - xi[1];
+        double dx2 = xj[3 * j + 2] - xi[2];
+        if (dx0 == 0.0 && dx1 == 0.0 && dx2 == 0.0)    /* coincident pair: reading R1 */
+            continue;
+        double r2 = dx0 * dx0 + dx1 * dx1 + dx2 * dx2 + eps2;
+        double r1i = 1.0 / sqrt(r2);
+        double r2i = r1i * r1i;
+        double r3i = r1i * r2i;
+        double r5i = r2i * r3i;
+        double mr5i = mj[j] * r5i;
+        double mf = mr5i * r2;                         /* = mj / r^3 */
+        double pot = mf * r2;                          /* = mj / r */
+        double dv0 = vj[3 * j + 0] - vi[0];            /* dv = vj - vi */
+        double dv1 = vj[3 * j + 1] - vi[1];
+        double dv2 = vj[3 * j + 2] - vi[2];
+        double mf3a = 3.0 * mr5i * (dx0 * dv0 + dx1 * dv1 + dx2 * dv2);
+        ax += mf * dx0;                                /* OUTPUT[0..2] += fx */
+        ay += mf * dx1;
+        az += mf * dx2;
+        jx += mf * dv0 - mf3a * dx0;                   /* OUTPUT[3..5] += jk1 - jk2 PAPER.md:532-550 */
+        jy += mf * dv1 - mf3a * dx1;
+        jz += mf * dv2 - mf3a * dx2;
+        phi -= pot;                                    /* OUTPUT[6] -= pot */
+    }
+    out7[0] = ax; out7[1] = ay; out7[2] = az; out7[3] = jx; out7[4] = jy; out7[5] = jz; out7[6] = phi;
+}
+
+/* Double inputs.  x_i, v_i [n_i][3]; x_j, v_j [n_j][3]; m_j [n_j]; acc, jerk [n_i][3]; pot [n_i] or NULL. */
+int oracle_force_jerk_f64(int64_t n_i, const double *x_i, const double *v_i, int64_t n_j, const double *x_j,
+                          const double *v_j, const double *m_j, double eps2, double *acc, double *jerk, double *pot)
+{
+    if (n_i < 0 || n_j < 0 || !(eps2 >= 0.0)) return 1;
+    if (n_i > 0 && (!x_i || !v_i || !acc || !jerk)) return 1;
+    if (n_j > 0 && (!x_j || !v_j || !m_j)) return 1;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n_i; ++i) {
+        double out[7];
+        one_i_jerk(&x_i[3 * i], &v_i[3 * i], n_j, x_j, v_j, m_j, eps2, out);
+        for (int c = 0; c < 3; ++c) { acc[3 * i + c] = out[c]; jerk[3 * i + c] = out[3 + c]; }
+        if (pot) pot[i] = out[6];
+    }
+    return 0;
+}
+
+/* FP32 inputs promoted exactly to double (the parity entry); outputs double. */
+int oracle_force_jerk_f32(int64_t n_i, const float *x_i, const float *v_i, int64_t n_j, const float *x_j,
+                          const float *v_j, const float *m_j, float eps2, double *acc, double *jerk, double *pot)
+{
+    if (n_i < 0 || n_j < 0 || !(eps2 >= 0.0f)) return 1;
+    if (n_i > 0 && (!x_i || !v_i || !acc || !jerk)) return 1;
+    if (n_j > 0 && (!x_j || !v_j || !m_j)) return 1;
+    size_t nj = (size_t)(n_j > 0 ? n_j : 1);
+    double *xj = (double *)malloc(sizeof(double) * 3 * nj);
+    double *vj = (double *)malloc(sizeof(double) * 3 * nj);
+    double *mj = (double *)malloc(sizeof(double) * nj);
+    if (!xj || !vj || !mj) { free(xj); free(vj); free(mj); return 2; }
+    for (int64_t k = 0; k < 3 * n_j; ++k) { xj[k] = (double)x_j[k]; vj[k] = (double)v_j[k]; }
+    for (int64_t j = 0; j < n_j; ++j) mj[j] = (double)m_j[j];
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n_i; ++i) {
+        double xi[3] = { (double)x_i[3 * i + 0], (double)x_i[3 * i + 1], (double)x_i[3 * i + 2] };
+        double vi[3] = { (double)v_i[3 * i + 0], (double)v_i[3 * i + 1], (double)v_i[3 * i + 2] };
+        double out[7];
+        one_i_jerk(xi, vi, n_j, xj, vj, mj, (double)eps2, out);
+        for (int c = 0; c < 3; ++c) { acc[3 * i + c] = out[c]; jerk[3 * i + c] = out[3 + c]; }
+        if (pot) pot[i] = out[6];
+    }
+    free(xj); free(vj); free(mj);
+    return 0;
+}

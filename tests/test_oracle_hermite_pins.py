@@ -1,0 +1,161 @@
+"""Pins of the force + jerk + potential oracle (row f1; Fig. A.4) -- CPU only.
+
+Each pin is independent of oracle_force_jerk's own arithmetic: exact rationals worked from the
+statements of Fig. A.4, the time derivative of the separately pinned acceleration oracle, an
+arbitrary-precision brute force written from the textbook formula, and invariances.
+"""
+import os
+from fractions import Fraction
+
+import mpmath
+import numpy as np
+import pytest
+
+import oracle
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "hermite_two_body_exact.txt")
+
+
+def _rows():
+    rows = []
+    with open(GOLDEN) as f:
+        for line in f:
+            line = line.strip()
+            if line and not line.startswith("#"):
+                rows.append(tuple(Fraction(t) for t in line.split()))
+    return rows
+
+
+@pytest.mark.parametrize("row", _rows())
+def test_h1_two_body_exact_rationals(row):
+    dx, dy, dz, ux, uy, uz, eps2, m, s = row
+    assert dx * dx + dy * dy + dz * dz + eps2 == s * s              # the fixture is self-consistent
+    d, dv = (dx, dy, dz), (ux, uy, uz)
+    ddv = sum(a * b for a, b in zip(d, dv))
+    a_exact = [m * c / s ** 3 for c in d]
+    j_exact = [m * w / s ** 3 - 3 * m * ddv * c / s ** 5 for c, w in zip(d, dv)]
+    for off, voff in (((0, 0, 0), (0, 0, 0)), ((1.5, -2.0, 0.25), (0.5, 0.25, -1.0))):
+        xi = np.array([off], dtype=np.float64); vi = np.array([voff], dtype=np.float64)
+        xj = xi + np.array([[float(c) for c in d]]); vj = vi + np.array([[float(c) for c in dv]])
+        acc, jerk, pot = oracle.force_jerk(xi, vi, xj, vj, np.array([float(m)]), float(eps2))
+        np.testing.assert_allclose(acc[0], [float(c) for c in a_exact], rtol=1e-15, atol=1e-18)
+        np.testing.assert_allclose(jerk[0], [float(c) for c in j_exact], rtol=4e-15, atol=1e-17)
+        assert pot[0] == pytest.approx(float(-m / s), rel=1e-15)
+
+
+def _random_system(n, seed, dtype=np.float64):
+    rng = np.random.default_rng(seed)
+    x = rng.normal(size=(n, 3)).astype(dtype)
+    v = rng.normal(size=(n, 3)).astype(dtype)
+    m = rng.uniform(0.5, 1.5, n).astype(dtype)
+    return x, v, m
+
+
+@pytest.mark.parametrize("seed,eps2", [(0, 0.01), (1, 0.0), (2, 1.0)])
+def test_h2_jerk_is_the_time_derivative_of_the_pinned_acceleration(seed, eps2):
+    """jerk_i = d a_i / dt along x(t) = x + v t: central difference of oracle.force (pinned by test_oracle_pins)."""
+    x, v, m = _random_system(40, seed)
+    xi, vi = x[:13] + 0.0, v[:13] + 0.0                  # i-set is a subset: exercises the coincident rule too
+    acc, jerk, pot = oracle.force_jerk(xi, vi, x, v, m, eps2)
+    a0, p0 = oracle.force(xi, x, m, eps2)
+    np.testing.assert_allclose(acc, a0, rtol=1e-14, atol=1e-15)       # same a and phi as the force-only oracle
+    np.testing.assert_allclose(pot, p0, rtol=1e-14)
+    h = 1e-4
+    ap, _ = oracle.force(xi + h * vi, x + h * v, m, eps2)
+    am, _ = oracle.force(xi - h * vi, x - h * v, m, eps2)
+    fd = (ap - am) / (2 * h)
+    scale = np.linalg.norm(jerk, axis=1).max()
+    assert np.abs(fd - jerk).max() <= 3e-6 * scale                    # O(h^2) truncation + 1e-16/h roundoff
+    # Richardson: the error shrinks 4x when h halves -> it is truncation of the right derivative, not a wrong term
+    h2 = 2e-4
+    ap2, _ = oracle.force(xi + h2 * vi, x + h2 * v, m, eps2)
+    am2, _ = oracle.force(xi - h2 * vi, x - h2 * v, m, eps2)
+    rich = (4 * fd - (ap2 - am2) / (2 * h2)) / 3
+    assert np.abs(rich - jerk).max() <= 2e-9 * scale
+
+
+def _brute_mp(xi, vi, xj, vj, mj, eps2):
+    """Independent evaluator: mpmath, 40 digits, textbook formula d/dt [m d / r^3] -- not the Fig. A.4 statement order."""
+    mpmath.mp.dps = 40
+    out_a, out_j, out_p = [], [], []
+    for a in range(len(xi)):
+        A = [mpmath.mpf(0)] * 3; J = [mpmath.mpf(0)] * 3; P = mpmath.mpf(0)
+        for b in range(len(xj)):
+            d = [mpmath.mpf(float(xj[b][c])) - mpmath.mpf(float(xi[a][c])) for c in range(3)]
+            if all(c == 0 for c in d):
+                continue
+            w = [mpmath.mpf(float(vj[b][c])) - mpmath.mpf(float(vi[a][c])) for c in range(3)]
+            r = mpmath.sqrt(sum(c * c for c in d) + mpmath.mpf(float(eps2)))
+            rdot = sum(c * e for c, e in zip(d, w)) / r                # d r / dt
+            mm = mpmath.mpf(float(mj[b]))
+            for c in range(3):
+                A[c] += mm * d[c] / r ** 3
+                J[c] += mm * (w[c] / r ** 3 - 3 * d[c] * rdot / r ** 4)
+            P -= mm / r
+        out_a.append([float(c) for c in A]); out_j.append([float(c) for c in J]); out_p.append(float(P))
+    return np.array(out_a), np.array(out_j), np.array(out_p)
+
+
+@pytest.mark.parametrize("n,eps2,seed", [(2, 0.0, 0), (3, 0.25, 1), (6, 1e-4, 2), (5, 0.0, 3)])
+def test_h3_brute_force_small_n(n, eps2, seed):
+    x, v, m = _random_system(n, seed)
+    acc, jerk, pot = oracle.force_jerk(x, v, x, v, m, eps2)
+    ra, rj, rp = _brute_mp(x, v, x, v, m, eps2)
+    np.testing.assert_allclose(acc, ra, rtol=1e-13, atol=1e-15)
+    np.testing.assert_allclose(jerk, rj, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(pot, rp, rtol=1e-13)
+
+
+def test_h3_float32_entry_promotes_exactly():
+    x, v, m = _random_system(7, 5, np.float32)
+    xi, vi = x[:3].copy(), v[:3].copy() + np.float32(0.5)             # same positions, other velocities: still coincident
+    acc, jerk, pot = oracle.force_jerk(xi, vi, x, v, m, np.float32(0.01))
+    ra, rj, rp = _brute_mp(xi, vi, x, v, m, np.float32(0.01))
+    np.testing.assert_allclose(acc, ra, rtol=1e-13, atol=1e-15)
+    np.testing.assert_allclose(jerk, rj, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(pot, rp, rtol=1e-13)
+
+
+def test_h4_momentum_antisymmetry_and_galilean_invariance():
+    x, v, m = _random_system(200, 7)
+    acc, jerk, pot = oracle.force_jerk(x, v, x, v, m, 0.01)
+    for arr in (acc, jerk):                                           # sum_i m_i jerk_i = d/dt sum m a = 0
+        tot = (m[:, None] * arr).sum(0)
+        assert np.linalg.norm(tot) <= 1e-13 * (m[:, None] * np.abs(arr)).sum()
+    boost = np.array([3.0, -1.0, 0.5])
+    acc2, jerk2, pot2 = oracle.force_jerk(x, v + boost, x, v + boost, m, 0.01)
+    np.testing.assert_allclose(jerk2, jerk, rtol=1e-11, atol=1e-12)   # only velocity differences enter
+    np.testing.assert_array_equal(acc2, acc)
+    # rotation: vectors rotate with the frame
+    q, _ = np.linalg.qr(np.random.default_rng(1).normal(size=(3, 3)))
+    acc3, jerk3, pot3 = oracle.force_jerk(x @ q.T, v @ q.T, x @ q.T, v @ q.T, m, 0.01)
+    np.testing.assert_allclose(jerk3, jerk @ q.T, rtol=1e-10, atol=1e-11)
+    np.testing.assert_allclose(pot3, pot, rtol=1e-12)
+    # velocity scaling: jerk is linear in the velocities, a does not depend on them
+    acc4, jerk4, _ = oracle.force_jerk(x, 2.5 * v, x, 2.5 * v, m, 0.01)
+    np.testing.assert_allclose(jerk4, 2.5 * jerk, rtol=1e-12, atol=1e-13)
+    np.testing.assert_array_equal(acc4, acc)
+
+
+def test_h5_circular_binary_jerk_is_omega_cross_a():
+    """On a circular orbit a rotates rigidly: jerk = omega x a, |jerk| = omega |a|."""
+    d, m, eps2 = 1.0, 0.5, 0.01
+    w2 = 2 * m / (d * d + eps2) ** 1.5
+    x = np.array([[-d / 2, 0, 0], [d / 2, 0, 0]]); mm = np.array([m, m])
+    vorb = np.sqrt(w2) * d / 2
+    v = np.array([[0, -vorb, 0], [0, vorb, 0]])
+    acc, jerk, _ = oracle.force_jerk(x, v, x, v, mm, eps2)
+    omega = np.array([0, 0, np.sqrt(w2)])
+    np.testing.assert_allclose(jerk, np.cross(omega, acc), rtol=1e-13, atol=1e-15)
+
+
+def test_h6_edge_sizes_and_coincidence():
+    z3 = np.zeros((0, 3)); z1 = np.zeros(0)
+    x, v, m = _random_system(4, 9)
+    a, j, p = oracle.force_jerk(x, v, z3, z3, z1, 0.1)
+    assert not a.any() and not j.any() and not p.any()
+    a, j, p = oracle.force_jerk(z3, z3, x, v, m, 0.1)
+    assert a.shape == (0, 3) and j.shape == (0, 3)
+    one = np.array([[1.0, 2.0, 3.0]])
+    a, j, p = oracle.force_jerk(one, np.array([[1.0, 0, 0]]), one, np.array([[0, 5.0, 0]]), np.array([2.0]), 0.0)
+    assert not a.any() and not j.any() and p[0] == 0.0               # coincident in position: nothing, even at eps2 = 0
