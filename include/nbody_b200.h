@@ -110,6 +110,33 @@ int nb_leapfrog_kdk(int64_t n, float *x, float *v, const float *m,
                     void *stream);
 
 /*
+ * nb_force_jerk -- force + jerk + potential for the 4th-order Hermite scheme: the paper's second
+ * pipeline description (Fig. A.2, Fig. A.4; used by the authors'
+ * Hermite code):
+ *
+ *     a_i    =  sum_j m_j d / r^3                          d = r_j - r_i,  r^2 = d.d + eps2
+ *     jerk_i =  sum_j m_j [ dv / r^3 - 3 (d.dv) d / r^5 ]  dv = v_j - v_i      (= d a_i / dt)
+ *     phi_i  = -sum_j m_j / r
+ *
+ *   x_i, v_i  device, const, float [n_i][3]   positions and velocities of the i-particles
+ *   x_j, v_j  device, const, float [n_j][3]   positions and velocities of the j-particles
+ *   m_j       device, const, float [n_j]
+ *   acc_out, jerk_out   device, float [n_i][3], required when n_i > 0
+ *   pot_out   device, float [n_i], may be NULL
+ *
+ * Everything else (aliasing, edge sizes, coincident-pair rule -- decided on the POSITIONS only --,
+ * asynchrony, errors, reproducibility) is as for nb_force.
+ */
+int nb_force_jerk(int64_t n_i, const float *x_i, const float *v_i,
+                  int64_t n_j, const float *x_j, const float *v_j, const float *m_j,
+                  float eps2,
+                  float *acc_out, float *jerk_out, float *pot_out,
+                  void *stream);
+
+/* nb_plan_query for nb_force_jerk (same out[] layout; K <= 4, 256 j-particles of 32 bytes per stage). */
+int nb_plan_query_jerk(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]);
+
+/*
  * nb_plan_query -- the decomposition the launch planner picks for (n_i, n_j) on a device with
  * sm_count SMs (pure host function, no CUDA call; sm_count <= 0 means 148).
  * out[0] = K  i-particles per thread        out[1] = WI warps per CTA along i

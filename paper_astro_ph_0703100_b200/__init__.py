@@ -7,10 +7,12 @@ from .binding import (  # noqa: F401
     NBError,
     force,
     force_host,
+    force_jerk,
     last_launch_count,
     leapfrog_kdk,
     lib,
     plan_query,
+    plan_query_jerk,
     profile_enable,
     profile_read,
     release_workspace,

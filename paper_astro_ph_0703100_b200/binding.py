@@ -43,6 +43,10 @@ def lib() -> ctypes.CDLL:
         l.nb_force_host.restype = ci
         l.nb_leapfrog_kdk.argtypes = [i64, p, p, p, f32, f32, i64, p, p, p]
         l.nb_leapfrog_kdk.restype = ci
+        l.nb_force_jerk.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p, p]
+        l.nb_force_jerk.restype = ci
+        l.nb_plan_query_jerk.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
+        l.nb_plan_query_jerk.restype = ci
         l.nb_plan_query.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
         l.nb_plan_query.restype = ci
         l.nb_last_launch_count.restype = i64
@@ -100,6 +104,33 @@ def force(x_i, x_j, m_j, eps2: float, acc_out=None, pot_out=None, want_pot: bool
     return acc_out, pot_out
 
 
+def force_jerk(x_i, v_i, x_j, v_j, m_j, eps2: float, acc_out=None, jerk_out=None, pot_out=None, want_pot: bool = True,
+               stream=None):
+    """nb_force_jerk on CUDA tensors.  Returns (acc [n_i,3], jerk [n_i,3], pot [n_i] or None); asynchronous."""
+    import torch
+    for t, name in ((x_i, "x_i"), (v_i, "v_i"), (x_j, "x_j"), (v_j, "v_j")):
+        _dev_f32(t, name, (3,))
+    _dev_f32(m_j, "m_j", ())
+    n_i, n_j = x_i.shape[0], x_j.shape[0]
+    if v_i.shape[0] != n_i or v_j.shape[0] != n_j or m_j.shape[0] != n_j:
+        raise ValueError("array lengths differ")
+    if acc_out is None:
+        acc_out = torch.empty((n_i, 3), dtype=torch.float32, device=x_i.device)
+    if jerk_out is None:
+        jerk_out = torch.empty((n_i, 3), dtype=torch.float32, device=x_i.device)
+    if pot_out is None and want_pot:
+        pot_out = torch.empty((n_i,), dtype=torch.float32, device=x_i.device)
+    _dev_f32(acc_out, "acc_out", (3,)); _dev_f32(jerk_out, "jerk_out", (3,))
+    if pot_out is not None:
+        _dev_f32(pot_out, "pot_out", ())
+    with torch.cuda.device(x_i.device):
+        st = lib().nb_force_jerk(n_i, x_i.data_ptr(), v_i.data_ptr(), n_j, x_j.data_ptr(), v_j.data_ptr(), m_j.data_ptr(),
+                                 float(eps2), acc_out.data_ptr(), jerk_out.data_ptr(),
+                                 None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_force_jerk")
+    return acc_out, jerk_out, pot_out
+
+
 def force_host(x_i, x_j, m_j, eps2: float, want_pot: bool = True, acc_out=None, pot_out=None):
     """nb_force_host on numpy float32 arrays (or pinned CPU tensors' numpy views).  Blocking."""
     import numpy as np
@@ -144,6 +175,13 @@ def leapfrog_kdk(x, v, m, eps2: float, dt: float, n_steps: int, acc_io=None, pot
 def plan_query(n_i: int, n_j: int, sm_count: int = 148) -> dict:
     out = (ctypes.c_int64 * 8)()
     _check(lib().nb_plan_query(int(n_i), int(n_j), int(sm_count), out), "nb_plan_query")
+    keys = ("K", "WI", "WJ", "S", "tiles_i", "tile_i", "tile_j", "stages")
+    return dict(zip(keys, [int(v) for v in out]))
+
+
+def plan_query_jerk(n_i: int, n_j: int, sm_count: int = 148) -> dict:
+    out = (ctypes.c_int64 * 8)()
+    _check(lib().nb_plan_query_jerk(int(n_i), int(n_j), int(sm_count), out), "nb_plan_query_jerk")
     keys = ("K", "WI", "WJ", "S", "tiles_i", "tile_i", "tile_j", "stages")
     return dict(zip(keys, [int(v) for v in out]))
 

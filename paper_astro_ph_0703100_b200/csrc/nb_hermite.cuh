@@ -1,0 +1,300 @@
+// nb_hermite.cuh -- sm_100a device code for row f1: force + jerk + potential for the 4th-order
+// Hermite scheme, the paper's second pipeline description (Fig. A.2 PAPER.md:397-428,
+// Fig. A.4):
+//
+//     a_i    =  sum_j m_j d / r^3                          d = r_j - r_i,  r^2 = d.d + eps^2
+//     jerk_i =  sum_j m_j [ dv / r^3 - 3 (d.dv) d / r^5 ]  dv = v_j - v_i
+//     phi_i  = -sum_j m_j / r
+//
+// Same structure as nb_force_kernel (nb_kernels.cuh): i stationary in registers as packed pairs,
+// j streamed through a TMA + mbarrier ring, Eq. (2) two-level sums (FP32 partials over <= 256 j,
+// FP64 running totals), WJ x S j-split with fixed-order reductions.  Differences:
+//   - j record = 32 bytes (x, y, z, m | vx, vy, vz, 0): the paper's [n_j][JDIM = 7] row
+//     padded to two LDS.128;
+//   - 10 accumulators per i-particle: a (3), J1 = sum mf dv (3), J2 = sum mr5i (d.dv) d (3), phi;
+//     jerk = J1 - 3 J2 is formed once, in FP64, in the epilogue (jk = jk1 - jk2 with
+//     mf3a = 3 mr5i (xv0+xv1+xv2)) -- the factor 3 leaves the hot loop;
+//   - per pair 27 FP32-pipe instructions + 1 MUFU.RSQ:
+//       3 FADD (d)  3 FFMA (r2)  3 FMUL (u2, m u, m u^3)  3 FADD (dv)  1 FMUL + 2 FFMA (d.dv)
+//       2 FMUL (u2 (d.dv), m u^5 (d.dv))  3 FFMA (a)  3 FFMA (J1)  3 FFMA (J2)  1 FADD (phi).
+// Coincident pairs (all three POSITION differences exactly zero, reading R1) add nothing:
+// MODE_EXACT masks every pair; MODE_LIST uses the coincidence lists of the pre-pass (nb_kernels.cuh)
+// and masks only the listed j-segments.  An unmasked coincident pair would add m dv / eps^3 to the
+// jerk, so unlike the plain force there is no speculative mode here.
+#pragma once
+#include "nb_kernels.cuh"
+
+namespace nb {
+
+constexpr int kHermiteAcc = 10;   // ax ay az | j1x j1y j1z | j2x j2y j2z | phi
+
+// (x, y, z) || m || (vx, vy, vz) -> two float4 per j-particle
+__global__ void __launch_bounds__(256) nb_pack_jv_kernel(const float* __restrict__ x_j, const float* __restrict__ v_j,
+                                                         const float* __restrict__ m_j, int n_j, float4* __restrict__ jp) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_j) return;
+    jp[2 * j + 0] = make_float4(x_j[3 * j + 0], x_j[3 * j + 1], x_j[3 * j + 2], m_j[j]);
+    jp[2 * j + 1] = make_float4(v_j[3 * j + 0], v_j[3 * j + 1], v_j[3 * j + 2], 0.0f);
+}
+
+struct HermiteArgs {
+    const float* x_i;      // [n_i][3]
+    const float* v_i;      // [n_i][3]
+    const float4* jp;      // [n_j][2] packed records
+    float* acc;            // [n_i][3]
+    float* jerk;           // [n_i][3]
+    float* pot;            // [n_i] or nullptr
+    double* partial;       // [S][n_i][10] when S > 1
+    const int* coin_lists;
+    const int* coin_flag;
+    int n_i;
+    int n_j;
+    int S;
+    float eps2;
+};
+
+template <bool MASKED>
+__device__ __forceinline__ void hermite_pair(u64 xj, u64 yj, u64 zj, u64 mj, u64 vxj, u64 vyj, u64 vzj,
+                                             u64 nxi, u64 nyi, u64 nzi, u64 nvxi, u64 nvyi, u64 nvzi, u64 eps2_2,
+                                             u64 (&s)[kHermiteAcc]) {
+    const u64 dx = add2(xj, nxi);                    // dx = xj - xi
+    const u64 dy = add2(yj, nyi);
+    const u64 dz = add2(zj, nzi);
+    u64 r2 = fma2(dx, dx, eps2_2);                   // r2 = dx.dx + eps2
+    r2 = fma2(dy, dy, r2);
+    r2 = fma2(dz, dz, r2);
+    float r2a, r2b;
+    unpack2(r2, r2a, r2b);
+    if (MASKED) {
+        const float inf = __int_as_float(0x7f800000);
+        float dxa, dxb, dya, dyb, dza, dzb;
+        unpack2(dx, dxa, dxb); unpack2(dy, dya, dyb); unpack2(dz, dza, dzb);
+        const uint32_t ta = __float_as_uint(dxa) | __float_as_uint(dya) | __float_as_uint(dza);
+        const uint32_t tb = __float_as_uint(dxb) | __float_as_uint(dyb) | __float_as_uint(dzb);
+        r2a = (ta == 0u) ? inf : r2a;                // rsqrt(+inf) = +0 -> every term of the pair is exactly 0
+        r2b = (tb == 0u) ? inf : r2b;
+    }
+    const u64 u = pack2(rsqrt_approx(r2a), rsqrt_approx(r2b));   // r1i
+    const u64 u2 = mul2(u, u);                       // r2i
+    const u64 mu = mul2(mj, u);                      // pot = mj r1i
+    const u64 mu3 = mul2(mu, u2);                    // mf  = mj r3i
+    const u64 dvx = add2(vxj, nvxi);                 // dv = vj - vi
+    const u64 dvy = add2(vyj, nvyi);
+    const u64 dvz = add2(vzj, nvzi);
+    u64 xv = mul2(dx, dvx);                          // xv0 + xv1 + xv2
+    xv = fma2(dy, dvy, xv);
+    xv = fma2(dz, dvz, xv);
+    const u64 q = mul2(u2, xv);
+    const u64 w = mul2(mu3, q);                      // mr5i (d.dv)   (mf3a / 3)
+    s[0] = fma2(mu3, dx, s[0]);                      // OUTPUT[0..2] += fx
+    s[1] = fma2(mu3, dy, s[1]);
+    s[2] = fma2(mu3, dz, s[2]);
+    s[3] = fma2(mu3, dvx, s[3]);                     // jk1 = mf dv
+    s[4] = fma2(mu3, dvy, s[4]);
+    s[5] = fma2(mu3, dvz, s[5]);
+    s[6] = fma2(w, dx, s[6]);                        // jk2 / 3 = mr5i (d.dv) d
+    s[7] = fma2(w, dy, s[7]);
+    s[8] = fma2(w, dz, s[8]);
+    s[9] = add2(s[9], mu);                           // OUTPUT[6] -= pot (sign at the end)
+}
+
+template <int K, bool MASKED>
+__device__ __forceinline__ void hermite_sweep(const float4* __restrict__ sp, int np, const u64 (&ni)[K / 2][6], u64 eps2_2,
+                                              u64 (&part)[K / 2][kHermiteAcc]) {
+#pragma unroll
+    for (int k = 0; k < K / 2; ++k)
+#pragma unroll
+        for (int c = 0; c < kHermiteAcc; ++c) part[k][c] = 0ull;
+#pragma unroll 2
+    for (int j = 0; j < np; ++j) {
+        const float4 P = sp[2 * j], V = sp[2 * j + 1];                 // two broadcast LDS.128
+        const u64 xj = pack2(P.x, P.x), yj = pack2(P.y, P.y), zj = pack2(P.z, P.z), mj = pack2(P.w, P.w);
+        const u64 vx = pack2(V.x, V.x), vy = pack2(V.y, V.y), vz = pack2(V.z, V.z);
+#pragma unroll
+        for (int k = 0; k < K / 2; ++k)
+            hermite_pair<MASKED>(xj, yj, zj, mj, vx, vy, vz, ni[k][0], ni[k][1], ni[k][2], ni[k][3], ni[k][4], ni[k][5],
+                                 eps2_2, part[k]);
+    }
+}
+
+// CTA = 8 warps = WI x WJ, as nb_force_kernel.  TJ j-particles (32 B each) per ring stage.
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, int SUB = 256>
+__global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const HermiteArgs a) {
+    static_assert(K % 2 == 0, "i-particles are held in pairs");
+    static_assert(SUB == kCoinSeg, "coincidence segments are SUB j-particles");
+    static_assert(MODE == MODE_EXACT || MODE == MODE_LIST, "no speculative mode for the jerk");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int REC = 32;
+    constexpr int RING_BYTES = STAGES * TJ * REC;
+    unsigned char* rings = smem_raw;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + WJ * RING_BYTES);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wi = warp % WI, wj = warp / WI;
+    const bool producer = (wi == 0) && (lane == 0);
+    const uint32_t ring = smem_u32(rings + wj * RING_BYTES);
+    const uint32_t full0 = smem_u32(bars + wj * STAGES);
+    const uint32_t empty0 = smem_u32(bars + (WJ + wj) * STAGES);
+    if (producer) {
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, WI);
+        }
+        mbar_fence_init();
+    }
+
+    const long long G = (long long)a.S * WJ;
+    const long long g = (long long)blockIdx.y * WJ + wj;
+    const int j_begin = (int)((long long)a.n_j * g / G);
+    const int j_end = (int)((long long)a.n_j * (g + 1) / G);
+    const int n_sub = j_end - j_begin;
+    const int n_tiles = (n_sub + TJ - 1) / TJ;
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(a.jp) + (size_t)j_begin * REC;
+
+    const int i_base = blockIdx.x * (32 * K * WI) + wi * (32 * K) + lane;
+    u64 ni[K / 2][6];                                                  // (-x, -y, -z, -vx, -vy, -vz) of each i-pair
+#pragma unroll
+    for (int k2 = 0; k2 < K / 2; ++k2) {
+        const int i0 = min(i_base + (2 * k2) * 32, a.n_i - 1);
+        const int i1 = min(i_base + (2 * k2 + 1) * 32, a.n_i - 1);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            ni[k2][c] = pack2(-a.x_i[3 * i0 + c], -a.x_i[3 * i1 + c]);
+            ni[k2][3 + c] = pack2(-a.v_i[3 * i0 + c], -a.v_i[3 * i1 + c]);
+        }
+    }
+    const u64 eps2_2 = pack2(a.eps2, a.eps2);
+    __syncthreads();
+
+    if (producer) {
+        const int pre = n_tiles < STAGES ? n_tiles : STAGES;
+        for (int t = 0; t < pre; ++t) {
+            const uint32_t bytes = (uint32_t)min(TJ, n_sub - t * TJ) * REC;
+            mbar_expect_tx(full0 + 8 * t, bytes);
+            tma_load_1d(ring + t * TJ * REC, src + (size_t)t * TJ * REC, bytes, full0 + 8 * t);
+        }
+    }
+
+    double run[K][kHermiteAcc];
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+#pragma unroll
+        for (int c = 0; c < kHermiteAcc; ++c) run[k][c] = 0.0;
+
+    const int* coin = nullptr;
+    int coin_cnt = 0, coin_pos = 0, coin_next = 0x7fffffff;
+    if (MODE == MODE_LIST) {
+        coin = a.coin_lists + (size_t)(blockIdx.x * WI + wi) * (1 + kCoinCap);
+        coin_cnt = (*a.coin_flag != 0) ? -1 : coin[0];
+        if (coin_cnt > 0) coin_next = coin[1];
+    }
+
+    for (int t = 0; t < n_tiles; ++t) {
+        const int slot = t % STAGES;
+        mbar_wait(full0 + 8 * slot, (uint32_t)(t / STAGES) & 1u);
+        const int np = min(TJ, n_sub - t * TJ);
+        const float4* sp = reinterpret_cast<const float4*>(rings + wj * RING_BYTES + slot * TJ * REC);
+        for (int c = 0; c < np; c += SUB) {
+            const int nc = min(SUB, np - c);
+            u64 part[K / 2][kHermiteAcc];
+            bool masked = true;
+            if (MODE == MODE_LIST) {
+                const int j0 = j_begin + t * TJ + c;
+                const int seg_lo = j0 >> kCoinSegShift, seg_hi = (j0 + nc - 1) >> kCoinSegShift;
+                while (coin_next < seg_lo) {
+                    ++coin_pos;
+                    coin_next = (coin_pos < coin_cnt) ? coin[1 + coin_pos] : 0x7fffffff;
+                }
+                masked = (coin_cnt < 0 || coin_next <= seg_hi);
+            }
+            if (masked) hermite_sweep<K, true>(sp + 2 * c, nc, ni, eps2_2, part);
+            else hermite_sweep<K, false>(sp + 2 * c, nc, ni, eps2_2, part);
+#pragma unroll
+            for (int k2 = 0; k2 < K / 2; ++k2)
+#pragma unroll
+                for (int q = 0; q < kHermiteAcc; ++q) {
+                    float lo, hi;
+                    unpack2(part[k2][q], lo, hi);
+                    run[2 * k2][q] += (double)lo;
+                    run[2 * k2 + 1][q] += (double)hi;
+                }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty0 + 8 * slot);
+        if (producer) {
+            const int tt = (WI > 1) ? t - 1 : t;
+            if (tt >= 0 && tt + STAGES < n_tiles) {
+                const int rs = tt % STAGES;
+                mbar_wait(empty0 + 8 * rs, (uint32_t)(tt / STAGES) & 1u);
+                const int tn = tt + STAGES;
+                const uint32_t bytes = (uint32_t)min(TJ, n_sub - tn * TJ) * REC;
+                mbar_expect_tx(full0 + 8 * rs, bytes);
+                tma_load_1d(ring + rs * TJ * REC, src + (size_t)tn * TJ * REC, bytes, full0 + 8 * rs);
+            }
+        }
+        __syncwarp();
+    }
+
+    if (WJ > 1) {
+        __syncthreads();
+        double* red = reinterpret_cast<double*>(smem_raw);             // [WJ][K][10][WI*32]
+        const int tig = wi * 32 + lane;
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+#pragma unroll
+            for (int c = 0; c < kHermiteAcc; ++c) red[((wj * K + k) * kHermiteAcc + c) * (WI * 32) + tig] = run[k][c];
+        __syncthreads();
+        if (wj != 0) return;
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+#pragma unroll
+            for (int c = 0; c < kHermiteAcc; ++c) {
+                double s = red[((0 * K + k) * kHermiteAcc + c) * (WI * 32) + tig];
+#pragma unroll
+                for (int w = 1; w < WJ; ++w) s += red[((w * K + k) * kHermiteAcc + c) * (WI * 32) + tig];
+                run[k][c] = s;
+            }
+    }
+
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const int i = i_base + k * 32;
+        if (i >= a.n_i) continue;
+        if (a.S == 1) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                a.acc[3 * i + c] = (float)run[k][c];
+                a.jerk[3 * i + c] = (float)(run[k][3 + c] - 3.0 * run[k][6 + c]);   // jk = jk1 - jk2
+            }
+            if (a.pot) a.pot[i] = -(float)run[k][9];
+        } else {
+            double* dst = a.partial + ((size_t)blockIdx.y * a.n_i + i) * kHermiteAcc;
+#pragma unroll
+            for (int c = 0; c < kHermiteAcc; c += 2) *reinterpret_cast<double2*>(dst + c) = make_double2(run[k][c], run[k][c + 1]);
+        }
+    }
+}
+
+// second pass over the S chunk partials, fixed order
+__global__ void __launch_bounds__(128) nb_hermite_reduce_kernel(const double* __restrict__ partial, int n_i, int S,
+                                                                float* __restrict__ acc, float* __restrict__ jerk,
+                                                                float* __restrict__ pot) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_i) return;
+    double s[kHermiteAcc];
+#pragma unroll
+    for (int c = 0; c < kHermiteAcc; ++c) s[c] = partial[(size_t)i * kHermiteAcc + c];
+    for (int q = 1; q < S; ++q) {
+        const double* p = partial + ((size_t)q * n_i + i) * kHermiteAcc;
+#pragma unroll
+        for (int c = 0; c < kHermiteAcc; ++c) s[c] += p[c];
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        acc[3 * i + c] = (float)s[c];
+        jerk[3 * i + c] = (float)(s[3 + c] - 3.0 * s[6 + c]);
+    }
+    if (pot) pot[i] = -(float)s[9];
+}
+
+}  // namespace nb

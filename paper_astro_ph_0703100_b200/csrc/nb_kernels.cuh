@@ -204,12 +204,13 @@ __device__ __forceinline__ uint32_t coin_hash(uint32_t a, uint32_t b, uint32_t c
 }
 
 // table entries: 0 = empty, else j + 1
-__global__ void __launch_bounds__(256) nb_coin_insert_kernel(const float4* __restrict__ jp, int n_j,
+// stride = float4 per j record (1 for the force path, 2 for the force + jerk path)
+__global__ void __launch_bounds__(256) nb_coin_insert_kernel(const float4* __restrict__ jp, int stride, int n_j,
                                                              uint32_t* __restrict__ table, uint32_t mask,
                                                              int* __restrict__ flag) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_j) return;
-    const float4 J = jp[j];
+    const float4 J = jp[(size_t)j * stride];
     uint32_t slot = coin_hash(coin_canon(J.x), coin_canon(J.y), coin_canon(J.z)) & mask;
     for (int step = 0; step < kCoinMaxProbe; ++step) {
         if (table[slot] == 0u && atomicCAS(table + slot, 0u, (uint32_t)j + 1u) == 0u) return;
@@ -219,7 +220,7 @@ __global__ void __launch_bounds__(256) nb_coin_insert_kernel(const float4* __res
 }
 
 __global__ void __launch_bounds__(256) nb_coin_probe_kernel(const float* __restrict__ x_i, int n_i,
-                                                            const float4* __restrict__ jp,
+                                                            const float4* __restrict__ jp, int stride,
                                                             const uint32_t* __restrict__ table, uint32_t mask,
                                                             int* __restrict__ lists) {
     __shared__ int set[2 * kCoinRaw];                                  // open-addressing set of segment ids, -1 = empty
@@ -236,7 +237,7 @@ __global__ void __launch_bounds__(256) nb_coin_probe_kernel(const float* __restr
         for (; step < kCoinMaxProbe; ++step) {
             const uint32_t e = table[slot];
             if (e == 0u) break;
-            const float4 J = jp[e - 1u];
+            const float4 J = jp[(size_t)(e - 1u) * stride];
             if (coin_canon(J.x) == cx && coin_canon(J.y) == cy && coin_canon(J.z) == cz) {
                 const int seg = (int)((e - 1u) >> kCoinSegShift);
                 uint32_t h = ((uint32_t)seg * 2654435761u) >> 26;      // 64 slots

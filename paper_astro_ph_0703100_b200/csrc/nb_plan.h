@@ -42,10 +42,11 @@ inline void ring_shape(int WJ, int* tile_j, int* stages) {
 
 // Cost model in SM clock cycles.  pair_cycles: 13 FP32-pipe lane-ops per pair over 128 lanes per
 // clock per SM at the measured ~84 % pipe efficiency of the K = 8 inner loop (profiles/).
-inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, int WJ, int S) {
+inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, int WJ, int S,
+                        double pair_inst = 13.0, double partial_bytes = 32.0) {
     const double c_fixed = 6000.0;                    // CTA start + first TMA round trip + epilogue
     const double c_reduce_launch = 8000.0;            // second kernel
-    const double pair_cycles = 13.0 / (128.0 * 0.84);
+    const double pair_cycles = pair_inst / (128.0 * 0.84);
     const int tile_i = 32 * K * WI;
     const int64_t tiles_i = (n_i + tile_i - 1) / tile_i;
     const double ctas = double(tiles_i) * S;
@@ -59,11 +60,14 @@ inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, i
     double cta_cycles = c_fixed + double(tile_i) * j_per_cta * pair_cycles * k_pen * wj_pen;
     if (WJ > 1) cta_cycles += 1500.0;                 // cross-warp reduction through shared memory
     double cost = waves * cta_cycles;
-    if (S > 1) cost += c_reduce_launch + double(n_i) * S * 32.0 / 2500.0;  // ~5 TB/s at ~2 GHz
+    if (S > 1) cost += c_reduce_launch + double(n_i) * S * partial_bytes / 2500.0;  // ~5 TB/s at ~2 GHz
     return cost;
 }
 
-inline Plan make_plan(int64_t n_i, int64_t n_j, int sm_count) {
+// k_max: largest K the kernel family is instantiated for; pair_inst: FP32-pipe instructions per pair;
+// partial_bytes: bytes per (chunk, i) of the second-pass partials; rec_bytes: bytes per j record.
+inline Plan make_plan(int64_t n_i, int64_t n_j, int sm_count, int k_max = 8, double pair_inst = 13.0,
+                      double partial_bytes = 32.0) {
     if (sm_count <= 0) sm_count = 148;
     Plan best{};
     double best_cost = -1.0;
@@ -71,6 +75,7 @@ inline Plan make_plan(int64_t n_i, int64_t n_j, int sm_count) {
     static const int wj_opts[4] = {1, 2, 4, 8};
     for (int k_idx = 0; k_idx < 3; ++k_idx) {
         const int K = k_opts[k_idx];
+        if (K > k_max) continue;
         if (K > 2 && n_i <= 32 * (K / 2)) continue;   // a smaller K already covers all i with one warp
         for (int wj_idx = 0; wj_idx < 4; ++wj_idx) {
             const int WJ = wj_opts[wj_idx];
@@ -79,7 +84,7 @@ inline Plan make_plan(int64_t n_i, int64_t n_j, int sm_count) {
             if (s_max < 1) s_max = 1;
             if (s_max > kMaxS) s_max = kMaxS;
             for (int S = 1; S <= s_max; ++S) {
-                const double c = plan_cost(n_i, n_j, sm_count, K, WI, WJ, S);
+                const double c = plan_cost(n_i, n_j, sm_count, K, WI, WJ, S, pair_inst, partial_bytes);
                 // strict '<' keeps the first (largest K, smallest WJ, smallest S) among equal costs
                 if (best_cost < 0.0 || c < best_cost * (1.0 - 1e-9)) {
                     best_cost = c;
@@ -91,7 +96,7 @@ inline Plan make_plan(int64_t n_i, int64_t n_j, int sm_count) {
     // debugging aid, not part of the ABI: NB_PLAN="K,WI,WJ,S" overrides the choice
     if (const char* env = std::getenv("NB_PLAN")) {
         int k, wi, wj, s;
-        if (std::sscanf(env, "%d,%d,%d,%d", &k, &wi, &wj, &s) == 4 && (k == 2 || k == 4 || k == 8) &&
+        if (std::sscanf(env, "%d,%d,%d,%d", &k, &wi, &wj, &s) == 4 && (k == 2 || k == 4 || k == 8) && k <= k_max &&
             wi * wj == kWarpsPerCta && (wj == 1 || wj == 2 || wj == 4 || wj == 8) && s >= 1 && s <= kMaxS) {
             best.K = k; best.WI = wi; best.WJ = wj; best.S = s;
         }

@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "nb_kernels.cuh"
+#include "nb_hermite.cuh"
 #include "nb_plan.h"
 
 #define NB_VERSION 100
@@ -46,12 +47,15 @@ struct Workspace {
     void* partial = nullptr;   size_t partial_bytes = 0;   // [S][n_i] double4
     void* stage = nullptr;     size_t stage_bytes = 0;     // device copies for nb_force_host
     void* coin = nullptr;      size_t coin_bytes = 0;      // coincidence pre-pass: flag | lists | hash table
+    void* jp2 = nullptr;       size_t jp2_bytes = 0;       // force + jerk: 32-byte j records
+    void* hpartial = nullptr;  size_t hpartial_bytes = 0;  // force + jerk: [S][n_i][10] double
 };
 
 std::mutex g_mutex;
 DeviceInfo g_dev[64];
 std::map<std::pair<int, cudaStream_t>, Workspace> g_ws;
 std::map<std::tuple<int64_t, int64_t, int>, nb::Plan> g_plans;
+std::map<std::tuple<int64_t, int64_t, int>, nb::Plan> g_hplans;
 
 int device_info(int* dev_out, DeviceInfo* out) {
     int dev = 0;
@@ -170,6 +174,31 @@ int launch_force(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t s
 
 bool bad_count(int64_t n) { return n < 0 || n > (int64_t)INT32_MAX; }
 
+// Coincidence pre-pass (MODE_LIST): hash table over the j-positions, one sorted j-segment list per
+// i-group of 32*K i-particles.  jp = packed j records, stride float4 each.  Three launches.
+int coin_prepass(Workspace* ws, const nb::Plan& plan, int64_t n_i, const float* x_i, int64_t n_j, const float4* jp,
+                 int stride, cudaStream_t stream, const int** lists_out, const int** flag_out) {
+    const int group = 32 * plan.K;
+    const int64_t n_groups = (int64_t)plan.tiles_i * plan.WI;        // every warp slot of the grid has a list
+    uint32_t slots = 1024;
+    while ((int64_t)slots < 2 * n_j) slots <<= 1;
+    const size_t b_lists = ((size_t)(1 + n_groups * (1 + nb::kCoinCap)) * sizeof(int) + 255) / 256 * 256;
+    int rc = ensure(&ws->coin, &ws->coin_bytes, b_lists + (size_t)slots * sizeof(uint32_t), stream);
+    if (rc != NB_OK) return rc;
+    int* flag = reinterpret_cast<int*>(ws->coin);
+    int* lists = flag + 1;
+    uint32_t* table = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(ws->coin) + b_lists);
+    NB_CUDA(cudaMemsetAsync(ws->coin, 0, b_lists + (size_t)slots * sizeof(uint32_t), stream));
+    nb::nb_coin_insert_kernel<<<(unsigned)((n_j + 255) / 256), 256, 0, stream>>>(jp, stride, (int)n_j, table, slots - 1, flag);
+    NB_CUDA(cudaGetLastError());
+    nb::nb_coin_probe_kernel<<<(unsigned)n_groups, group, 0, stream>>>(x_i, (int)n_i, jp, stride, table, slots - 1, lists);
+    NB_CUDA(cudaGetLastError());
+    t_launches += 2;
+    *lists_out = lists;
+    *flag_out = flag;
+    return NB_OK;
+}
+
 // pack (a1) when repack is true, then force (+ reduce).  The packed array lives in the workspace.
 int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
                float* acc_out, float* pot_out, cudaStream_t stream) {
@@ -223,27 +252,9 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.coin_flag = nullptr;
     const int mode = pick_mode(n_i, n_j, eps2);
     if (mode == nb::MODE_LIST) {
-        // coincidence pre-pass: hash table over the j-positions, one sorted j-segment list per i-group
-        const int group = 32 * plan.K;
-        const int64_t n_groups = (int64_t)plan.tiles_i * plan.WI;    // every warp slot of the grid has a list
-        uint32_t slots = 1024;
-        while ((int64_t)slots < 2 * n_j) slots <<= 1;
-        const size_t b_lists = ((size_t)(1 + n_groups * (1 + nb::kCoinCap)) * sizeof(int) + 255) / 256 * 256;
-        rc = ensure(&ws->coin, &ws->coin_bytes, b_lists + (size_t)slots * sizeof(uint32_t), stream);
+        rc = coin_prepass(ws, plan, n_i, x_i, n_j, reinterpret_cast<const float4*>(ws->jp), 1, stream,
+                          &args.coin_lists, &args.coin_flag);
         if (rc != NB_OK) return rc;
-        int* flag = reinterpret_cast<int*>(ws->coin);
-        int* lists = flag + 1;
-        uint32_t* table = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(ws->coin) + b_lists);
-        NB_CUDA(cudaMemsetAsync(ws->coin, 0, b_lists + (size_t)slots * sizeof(uint32_t), stream));
-        nb::nb_coin_insert_kernel<<<(unsigned)((n_j + 255) / 256), 256, 0, stream>>>(
-            reinterpret_cast<const float4*>(ws->jp), (int)n_j, table, slots - 1, flag);
-        NB_CUDA(cudaGetLastError());
-        nb::nb_coin_probe_kernel<<<(unsigned)n_groups, group, 0, stream>>>(
-            x_i, (int)n_i, reinterpret_cast<const float4*>(ws->jp), table, slots - 1, lists);
-        NB_CUDA(cudaGetLastError());
-        t_launches += 2;
-        args.coin_lists = lists;
-        args.coin_flag = flag;
         rc = launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (mode == nb::MODE_SPEC) {
         rc = launch_force<nb::MODE_SPEC>(args, plan, stream);
@@ -263,9 +274,159 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     return NB_OK;
 }
 
+
+// ------------------------------------------------------------------ row f1: force + jerk + potential
+constexpr double kHermiteInstPerPair = 27.0;
+constexpr double kHermitePartialBytes = 80.0;
+
+nb::Plan hermite_plan(int64_t n_i, int64_t n_j, int sm_count) {
+    return nb::make_plan(n_i, n_j, sm_count, 4, kHermiteInstPerPair, kHermitePartialBytes);
+}
+
+template <int K, int WI, int WJ, int STAGES, int MODE>
+int launch_hermite_inst(const nb::HermiteArgs& args, const nb::Plan& plan, cudaStream_t stream) {
+    constexpr int TJ = 256;
+    constexpr size_t ring = (size_t)WJ * STAGES * TJ * 32;
+    constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * nb::kHermiteAcc * (WI * 32) * sizeof(double) : 0;
+    constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
+    auto kern = nb::nb_hermite_kernel<K, WI, WJ, TJ, STAGES, MODE>;
+    static bool configured[64] = {};
+    int dev = 0;
+    NB_CUDA(cudaGetDevice(&dev));
+    if (!configured[dev & 63]) {
+        NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured[dev & 63] = true;
+    }
+    dim3 grid((unsigned)plan.tiles_i, (unsigned)plan.S, 1);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (t_profile) {
+        NB_CUDA(cudaEventCreate(&e0));
+        NB_CUDA(cudaEventCreate(&e1));
+        NB_CUDA(cudaEventRecord(e0, stream));
+    }
+    kern<<<grid, 32 * WI * WJ, smem, stream>>>(args);
+    NB_CUDA(cudaGetLastError());
+    if (t_profile) {
+        NB_CUDA(cudaEventRecord(e1, stream));
+        t_events.emplace_back(e0, e1);
+    }
+    ++t_launches;
+    return NB_OK;
+}
+
+template <int K, int MODE>
+int launch_hermite_k(const nb::HermiteArgs& args, const nb::Plan& plan, cudaStream_t stream) {
+    switch (plan.WJ) {
+        case 1: return launch_hermite_inst<K, 8, 1, 4, MODE>(args, plan, stream);
+        case 2: return launch_hermite_inst<K, 4, 2, 4, MODE>(args, plan, stream);
+        case 4: return launch_hermite_inst<K, 2, 4, 3, MODE>(args, plan, stream);
+        default: return launch_hermite_inst<K, 1, 8, 3, MODE>(args, plan, stream);
+    }
+}
+
+template <int MODE>
+int launch_hermite(const nb::HermiteArgs& args, const nb::Plan& plan, cudaStream_t stream) {
+    return plan.K == 2 ? launch_hermite_k<2, MODE>(args, plan, stream) : launch_hermite_k<4, MODE>(args, plan, stream);
+}
+
+int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j, const float* x_j, const float* v_j,
+                    const float* m_j, float eps2, float* acc_out, float* jerk_out, float* pot_out, cudaStream_t stream) {
+    if (bad_count(n_i) || bad_count(n_j)) return NB_ERR_INVALID_VALUE;
+    if (!(eps2 >= 0.0f) || !std::isfinite(eps2)) return NB_ERR_INVALID_VALUE;
+    if (n_i > 0 && (!x_i || !v_i || !acc_out || !jerk_out)) return NB_ERR_INVALID_VALUE;
+    if (n_j > 0 && (!x_j || !v_j || !m_j)) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n_i == 0) return NB_OK;
+    if (n_j == 0) {
+        NB_CUDA(cudaMemsetAsync(acc_out, 0, sizeof(float) * 3 * (size_t)n_i, stream));
+        NB_CUDA(cudaMemsetAsync(jerk_out, 0, sizeof(float) * 3 * (size_t)n_i, stream));
+        if (pot_out) NB_CUDA(cudaMemsetAsync(pot_out, 0, sizeof(float) * (size_t)n_i, stream));
+        return NB_OK;
+    }
+    nb::Plan plan;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        auto key = std::make_tuple(n_i, n_j, info.sm_count);
+        auto it = g_hplans.find(key);
+        if (it != g_hplans.end() && !std::getenv("NB_PLAN")) {
+            plan = it->second;
+        } else {
+            plan = hermite_plan(n_i, n_j, info.sm_count);
+            if (g_hplans.size() > 4096) g_hplans.clear();
+            g_hplans[key] = plan;
+        }
+    }
+    Workspace* ws;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        ws = &g_ws[std::make_pair(dev, stream)];
+    }
+    rc = ensure(&ws->jp2, &ws->jp2_bytes, (size_t)n_j * 2 * sizeof(float4), stream);
+    if (rc != NB_OK) return rc;
+    if (plan.S > 1) {
+        rc = ensure(&ws->hpartial, &ws->hpartial_bytes, (size_t)plan.S * (size_t)n_i * nb::kHermiteAcc * sizeof(double), stream);
+        if (rc != NB_OK) return rc;
+    }
+    nb::nb_pack_jv_kernel<<<(unsigned)((n_j + 255) / 256), 256, 0, stream>>>(x_j, v_j, m_j, (int)n_j,
+                                                                              reinterpret_cast<float4*>(ws->jp2));
+    NB_CUDA(cudaGetLastError());
+    ++t_launches;
+
+    nb::HermiteArgs args;
+    args.x_i = x_i;
+    args.v_i = v_i;
+    args.jp = reinterpret_cast<const float4*>(ws->jp2);
+    args.acc = acc_out;
+    args.jerk = jerk_out;
+    args.pot = pot_out;
+    args.partial = reinterpret_cast<double*>(ws->hpartial);
+    args.coin_lists = nullptr;
+    args.coin_flag = nullptr;
+    args.n_i = (int)n_i;
+    args.n_j = (int)n_j;
+    args.S = plan.S;
+    args.eps2 = eps2;
+    // the jerk has no speculative mode: small calls mask every pair, large ones use the coincidence lists
+    int mode = pick_mode(n_i, n_j, eps2);
+    if (mode == nb::MODE_SPEC) mode = nb::MODE_EXACT;
+    if (mode == nb::MODE_LIST) {
+        rc = coin_prepass(ws, plan, n_i, x_i, n_j, args.jp, 2, stream, &args.coin_lists, &args.coin_flag);
+        if (rc != NB_OK) return rc;
+        rc = launch_hermite<nb::MODE_LIST>(args, plan, stream);
+    } else {
+        rc = launch_hermite<nb::MODE_EXACT>(args, plan, stream);
+    }
+    if (rc != NB_OK) return rc;
+    if (plan.S > 1) {
+        nb::nb_hermite_reduce_kernel<<<(unsigned)((n_i + 127) / 128), 128, 0, stream>>>(
+            reinterpret_cast<const double*>(ws->hpartial), (int)n_i, plan.S, acc_out, jerk_out, pot_out);
+        NB_CUDA(cudaGetLastError());
+        ++t_launches;
+    }
+    return NB_OK;
+}
+
 }  // namespace
 
 extern "C" {
+
+int nb_force_jerk(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j, const float* x_j, const float* v_j,
+                  const float* m_j, float eps2, float* acc_out, float* jerk_out, float* pot_out, void* stream) {
+    t_launches = 0;
+    return force_jerk_impl(n_i, x_i, v_i, n_j, x_j, v_j, m_j, eps2, acc_out, jerk_out, pot_out,
+                           reinterpret_cast<cudaStream_t>(stream));
+}
+
+int nb_plan_query_jerk(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]) {
+    if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
+    const nb::Plan p = hermite_plan(n_i, n_j, sm_count);
+    out[0] = p.K; out[1] = p.WI; out[2] = p.WJ; out[3] = p.S;
+    out[4] = p.tiles_i; out[5] = p.tile_i; out[6] = 256; out[7] = (p.WJ <= 2) ? 4 : 3;
+    return NB_OK;
+}
 
 int nb_force(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
              float* acc_out, float* pot_out, void* stream) {
@@ -410,6 +571,8 @@ int nb_release_workspace(void) {
             if (it->second.partial) (void)cudaFree(it->second.partial);
             if (it->second.stage) (void)cudaFree(it->second.stage);
             if (it->second.coin) (void)cudaFree(it->second.coin);
+            if (it->second.jp2) (void)cudaFree(it->second.jp2);
+            if (it->second.hpartial) (void)cudaFree(it->second.hpartial);
             it = g_ws.erase(it);
         } else {
             ++it;
