@@ -133,6 +133,34 @@ int nb_force_jerk(int64_t n_i, const float *x_i, const float *v_i,
                   float *acc_out, float *jerk_out, float *pot_out,
                   void *stream);
 
+/*
+ * nb_force_batched -- many independent small (i-set, j-set) sub-problems of nb_force in ONE launch:
+ * the use the paper shapes its interface for, a host tree code calling the force routine on
+ * interaction lists of "several thousands" particles per group (PAPER.md:246 last sentence, section
+ * 4.4 PAPER.md:355-359).  Sub-problem b = i-particles [i_offsets[b], i_offsets[b+1]) of x_i against
+ * j-particles [j_offsets[b], j_offsets[b+1]) of x_j / m_j (CSR-style concatenation):
+ *
+ *     for b in 0 .. n_batch-1:   nb_force(n_i(b), x_i + 3 i_offsets[b], n_j(b), x_j + 3 j_offsets[b],
+ *                                         m_j + j_offsets[b], eps2, acc_out + 3 i_offsets[b], pot_out + i_offsets[b])
+ *
+ *   n_batch    number of sub-problems
+ *   i_offsets  device, const, int32 [n_batch + 1], non-decreasing, i_offsets[n_batch] <= n_i_total
+ *   j_offsets  device, const, int32 [n_batch + 1], non-decreasing, j_offsets[n_batch] <= n_j_total
+ *   n_i_total, n_j_total   lengths of the concatenated arrays (host values; the offsets are NOT read on the host)
+ *   x_i [n_i_total][3], x_j [n_j_total][3], m_j [n_j_total], acc_out [n_i_total][3], pot_out [n_i_total] or NULL: device
+ *
+ * Each sub-problem is handled by ceil(n_i(b) / tile) CTAs (tile = 64 .. 512, chosen from the mean
+ * n_i_total / n_batch) whose 8 warps split its j-range; no partial sums leave a CTA.  A sub-problem with
+ * n_j(b) == 0 gets zeros; i-particles outside every sub-problem are not written.  The offsets are not
+ * validated.  Same coincident-pair rule, determinism and error conventions as nb_force.
+ */
+int nb_force_batched(int64_t n_batch, const int32_t *i_offsets, const int32_t *j_offsets,
+                     int64_t n_i_total, const float *x_i,
+                     int64_t n_j_total, const float *x_j, const float *m_j,
+                     float eps2,
+                     float *acc_out, float *pot_out,
+                     void *stream);
+
 /* nb_plan_query for nb_force_jerk (same out[] layout; K <= 4, 256 j-particles of 32 bytes per stage). */
 int nb_plan_query_jerk(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]);
 

@@ -123,6 +123,22 @@ def force_jerk(x_i: np.ndarray, v_i: np.ndarray, x_j: np.ndarray, v_j: np.ndarra
     return acc, jerk, pot
 
 
+def force_batched(i_offsets: np.ndarray, j_offsets: np.ndarray, x_i: np.ndarray, x_j: np.ndarray, m_j: np.ndarray,
+                  eps2: float):
+    """Row f2: Eq. (1) and phi for independent sub-problems b = (i in [i_offsets[b], i_offsets[b+1]),
+    j in [j_offsets[b], j_offsets[b+1])) -- literally one ``force`` call per sub-problem (PAPER.md:246, 355-359:
+    the host tree code calls the force routine once per interaction list).  i-particles outside every
+    sub-problem keep a = 0, phi = 0."""
+    n_i = np.asarray(x_i).reshape(-1, 3).shape[0]
+    acc = np.zeros((n_i, 3), dtype=np.float64)
+    pot = np.zeros(n_i, dtype=np.float64)
+    for b in range(len(i_offsets) - 1):
+        i0, i1, j0, j1 = int(i_offsets[b]), int(i_offsets[b + 1]), int(j_offsets[b]), int(j_offsets[b + 1])
+        if i1 > i0:
+            acc[i0:i1], pot[i0:i1] = force(x_i[i0:i1], x_j[j0:j1], m_j[j0:j1], eps2)
+    return acc, pot
+
+
 def energy(x: np.ndarray, v: np.ndarray, m: np.ndarray, eps2: float) -> Tuple[float, float, float]:
     """(T, W, E) in double from an FP32 state; W = 1/2 sum m_i phi_i with coincident pairs skipped."""
     xx, vv, mm = _c(x, np.float32).reshape(-1, 3), _c(v, np.float32).reshape(-1, 3), _c(m, np.float32).reshape(-1)

@@ -6,6 +6,7 @@ Python binding over it (argument marshalling only) plus the seeded workload gene
 from .binding import (  # noqa: F401
     NBError,
     force,
+    force_batched,
     force_host,
     force_jerk,
     last_launch_count,

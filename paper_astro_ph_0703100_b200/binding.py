@@ -45,6 +45,8 @@ def lib() -> ctypes.CDLL:
         l.nb_leapfrog_kdk.restype = ci
         l.nb_force_jerk.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p, p]
         l.nb_force_jerk.restype = ci
+        l.nb_force_batched.argtypes = [i64, p, p, i64, p, i64, p, p, f32, p, p, p]
+        l.nb_force_batched.restype = ci
         l.nb_plan_query_jerk.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
         l.nb_plan_query_jerk.restype = ci
         l.nb_plan_query.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
@@ -129,6 +131,31 @@ def force_jerk(x_i, v_i, x_j, v_j, m_j, eps2: float, acc_out=None, jerk_out=None
                                  None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
     _check(st, "nb_force_jerk")
     return acc_out, jerk_out, pot_out
+
+
+def force_batched(i_offsets, j_offsets, x_i, x_j, m_j, eps2: float, acc_out=None, pot_out=None, want_pot: bool = True,
+                  stream=None):
+    """nb_force_batched on CUDA tensors; i_offsets / j_offsets are int32 CUDA tensors of length n_batch + 1."""
+    import torch
+    _dev_f32(x_i, "x_i", (3,)); _dev_f32(x_j, "x_j", (3,)); _dev_f32(m_j, "m_j", ())
+    for t, name in ((i_offsets, "i_offsets"), (j_offsets, "j_offsets")):
+        if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.int32 or not t.is_contiguous() or t.dim() != 1:
+            raise TypeError(f"{name} must be a contiguous 1-D int32 CUDA tensor")
+    if i_offsets.shape[0] != j_offsets.shape[0] or i_offsets.shape[0] < 1:
+        raise ValueError("i_offsets and j_offsets must both have n_batch + 1 entries")
+    n_batch, n_i, n_j = i_offsets.shape[0] - 1, x_i.shape[0], x_j.shape[0]
+    if m_j.shape[0] != n_j:
+        raise ValueError("m_j length != n_j")
+    if acc_out is None:
+        acc_out = torch.zeros((n_i, 3), dtype=torch.float32, device=x_i.device)
+    if pot_out is None and want_pot:
+        pot_out = torch.zeros((n_i,), dtype=torch.float32, device=x_i.device)
+    with torch.cuda.device(x_i.device):
+        st = lib().nb_force_batched(n_batch, i_offsets.data_ptr(), j_offsets.data_ptr(), n_i, x_i.data_ptr(), n_j,
+                                    x_j.data_ptr(), m_j.data_ptr(), float(eps2), acc_out.data_ptr(),
+                                    None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_force_batched")
+    return acc_out, pot_out
 
 
 def force_host(x_i, x_j, m_j, eps2: float, want_pot: bool = True, acc_out=None, pot_out=None):

@@ -282,6 +282,11 @@ struct ForceArgs {
     double4* partial;      // [S][n_i] when S > 1
     const int* coin_lists; // MODE_LIST: [n_groups][1 + kCoinCap]
     const int* coin_flag;  // MODE_LIST: != 0 -> mask everywhere
+    const int* i_off;      // BATCHED: [n_batch + 1] first i of every sub-problem
+    const int* j_off;      // BATCHED: [n_batch + 1] first j of every sub-problem
+    const int* tile_start; // BATCHED: [n_batch + 1] first CTA of every sub-problem (exclusive scan of its i-tiles)
+    const int* cta_batch;  // BATCHED: [number of CTAs] sub-problem of every CTA
+    int n_batch;
     int n_i;
     int n_j;
     int S;
@@ -299,11 +304,27 @@ enum { MODE_EXACT = 0,     // masked loop everywhere (eps2 == 0 or tiny)
 // Each sub-range is streamed through its own shared-memory ring by 1-D TMA bulk copies issued by
 // lane 0 of the group's first warp; "full" mbarriers count bytes, "empty" mbarriers count the WI
 // consuming warps.
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, int SUB = 256>
+//
+// BATCHED (row f2, nb_force_batched): the grid is one row of CTAs; CTA blockIdx.x finds the
+// sub-problem b it belongs to in cta_batch[] (written by nb_batch_scan_kernel) and works on i in
+// [i_off[b], i_off[b+1]) against j in [j_off[b], j_off[b+1]); no split across CTAs (S = 1).
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool BATCHED = false, int SUB = 256>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
     static_assert(SUB == kCoinSeg, "coincidence segments are SUB j-particles");
+    static_assert(!(BATCHED && MODE == MODE_LIST), "no coincidence lists for batched calls");
     extern __shared__ __align__(128) unsigned char smem_raw[];
+
+    // i-range [i_lo, i_hi) this CTA draws its tile from, j-range [jr_lo, jr_lo + jr_n) it sums over
+    int i_lo = blockIdx.x * (32 * K * WI), i_hi = a.n_i, jr_lo = 0, jr_n = a.n_j;
+    if (BATCHED) {
+        if ((int)blockIdx.x >= a.tile_start[a.n_batch]) return;        // the grid is an upper bound
+        const int lo = a.cta_batch[blockIdx.x];
+        i_lo = a.i_off[lo] + ((int)blockIdx.x - a.tile_start[lo]) * (32 * K * WI);
+        i_hi = a.i_off[lo + 1];
+        jr_lo = a.j_off[lo];
+        jr_n = a.j_off[lo + 1] - jr_lo;
+    }
     constexpr int RING_BYTES = STAGES * TJ * 16;
     unsigned char* rings = smem_raw;                                   // [WJ][STAGES][TJ] float4
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + WJ * RING_BYTES);   // full[WJ][STAGES], empty[WJ][STAGES]
@@ -327,20 +348,20 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
     // j sub-range of this warp group
     const long long G = (long long)a.S * WJ;
     const long long g = (long long)blockIdx.y * WJ + wj;
-    const int j_begin = (int)((long long)a.n_j * g / G);
-    const int j_end = (int)((long long)a.n_j * (g + 1) / G);
+    const int j_begin = jr_lo + (int)((long long)jr_n * g / G);
+    const int j_end = jr_lo + (int)((long long)jr_n * (g + 1) / G);
     const int n_sub = j_end - j_begin;
     const int n_tiles = (n_sub + TJ - 1) / TJ;
     const unsigned char* src = reinterpret_cast<const unsigned char*>(a.jp + j_begin);
 
     // a3: i-particles of this thread (clamped loads; stores are guarded), pair k2 = (k = 2 k2, 2 k2 + 1)
     // a warp owns 32*K consecutive i-particles, so that an aliased i-set meets its own copies in few j-tiles
-    const int i_base = blockIdx.x * (32 * K * WI) + wi * (32 * K) + lane;
+    const int i_base = i_lo + wi * (32 * K) + lane;
     u64 nxi[K / 2], nyi[K / 2], nzi[K / 2];
 #pragma unroll
     for (int k2 = 0; k2 < K / 2; ++k2) {
-        const int i0 = min(i_base + (2 * k2) * 32, a.n_i - 1);
-        const int i1 = min(i_base + (2 * k2 + 1) * 32, a.n_i - 1);
+        const int i0 = min(i_base + (2 * k2) * 32, i_hi - 1);
+        const int i1 = min(i_base + (2 * k2 + 1) * 32, i_hi - 1);
         nxi[k2] = pack2(-a.x_i[3 * i0 + 0], -a.x_i[3 * i1 + 0]);
         nyi[k2] = pack2(-a.x_i[3 * i0 + 1], -a.x_i[3 * i1 + 1]);
         nzi[k2] = pack2(-a.x_i[3 * i0 + 2], -a.x_i[3 * i1 + 2]);
@@ -457,7 +478,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const int i = i_base + k * 32;
-        if (i >= a.n_i) continue;
+        if (i >= i_hi) continue;
         if (a.S == 1) {
             a.acc[3 * i + 0] = (float)run[k][0];
             a.acc[3 * i + 1] = (float)run[k][1];
@@ -467,6 +488,47 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
             a.partial[(size_t)blockIdx.y * a.n_i + i] = make_double4(run[k][0], run[k][1], run[k][2], run[k][3]);
         }
     }
+}
+
+// f2: exclusive scan of the i-tiles per sub-problem -> first CTA of every sub-problem (one CTA, n_batch + 1 outputs)
+__global__ void __launch_bounds__(1024) nb_batch_scan_kernel(const int* __restrict__ i_off, int n_batch, int tile_i,
+                                                             int* __restrict__ tile_start, int* __restrict__ cta_batch) {
+    __shared__ int warp_sum[32];
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int base = 0; base < n_batch; base += 1024) {
+        const int b = base + threadIdx.x;
+        const int tiles = (b < n_batch) ? (max(i_off[b + 1] - i_off[b], 0) + tile_i - 1) / tile_i : 0;
+        int incl = tiles;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += v;
+        }
+        if (lane == 31) warp_sum[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            int w = warp_sum[lane];
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, w, d);
+                if (lane >= d) w += v;
+            }
+            warp_sum[lane] = w;                                        // inclusive over warps
+        }
+        __syncthreads();
+        const int before = carry + (warp > 0 ? warp_sum[warp - 1] : 0) + incl - tiles;
+        if (b < n_batch) {
+            tile_start[b] = before;
+            for (int t = 0; t < tiles; ++t) cta_batch[before + t] = b;
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) carry = before + tiles;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) tile_start[n_batch] = carry;
 }
 
 // a7 (inter-CTA): second pass, fixed-order sum over the S chunk partials

@@ -47,6 +47,7 @@ struct Workspace {
     void* partial = nullptr;   size_t partial_bytes = 0;   // [S][n_i] double4
     void* stage = nullptr;     size_t stage_bytes = 0;     // device copies for nb_force_host
     void* coin = nullptr;      size_t coin_bytes = 0;      // coincidence pre-pass: flag | lists | hash table
+    void* tiles = nullptr;     size_t tiles_bytes = 0;     // batched calls: first CTA of every sub-problem
     void* jp2 = nullptr;       size_t jp2_bytes = 0;       // force + jerk: 32-byte j records
     void* hpartial = nullptr;  size_t hpartial_bytes = 0;  // force + jerk: [S][n_i][10] double
 };
@@ -250,6 +251,8 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.eps2 = eps2;
     args.coin_lists = nullptr;
     args.coin_flag = nullptr;
+    args.i_off = args.j_off = args.tile_start = args.cta_batch = nullptr;
+    args.n_batch = 0;
     const int mode = pick_mode(n_i, n_j, eps2);
     if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, reinterpret_cast<const float4*>(ws->jp), 1, stream,
@@ -409,9 +412,130 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     return NB_OK;
 }
 
+
+// ------------------------------------------------------------------ row f2: many small sub-problems in one launch
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE>
+int launch_batched_inst(const nb::ForceArgs& args, unsigned max_ctas, cudaStream_t stream) {
+    constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
+    constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
+    constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
+    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, true>;
+    static bool configured[64] = {};
+    int dev = 0;
+    NB_CUDA(cudaGetDevice(&dev));
+    if (!configured[dev & 63]) {
+        NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured[dev & 63] = true;
+    }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (t_profile) {
+        NB_CUDA(cudaEventCreate(&e0));
+        NB_CUDA(cudaEventCreate(&e1));
+        NB_CUDA(cudaEventRecord(e0, stream));
+    }
+    kern<<<max_ctas, 32 * WI * WJ, smem, stream>>>(args);
+    NB_CUDA(cudaGetLastError());
+    if (t_profile) {
+        NB_CUDA(cudaEventRecord(e1, stream));
+        t_events.emplace_back(e0, e1);
+    }
+    ++t_launches;
+    return NB_OK;
+}
+
+// i-tile of a batched call.  Measured on tree lists (groups of 32..256, lists of 2000..6000): the padding of
+// the last tile of every sub-problem costs more than the smaller K loses, and smaller CTAs overlap their
+// prologues, so the tile stays well below the mean sub-problem size.
+int batched_tile(int64_t n_i_total, int64_t n_batch) {
+    const double mean = (double)n_i_total / (double)(n_batch > 0 ? n_batch : 1);
+    if (const char* e = std::getenv("NB_BATCH_TILE")) {
+        const int t = std::atoi(e);
+        if (t == 64 || t == 128 || t == 256 || t == 512) return t;
+    }
+    if (mean <= 384.0) return 64;
+    if (mean <= 768.0) return 128;
+    if (mean <= 2048.0) return 256;
+    return 512;
+}
+
+template <int MODE>
+int launch_batched(const nb::ForceArgs& args, int tile, unsigned max_ctas, cudaStream_t stream) {
+    switch (tile) {
+        case 64: return launch_batched_inst<2, 1, 8, 256, 3, MODE>(args, max_ctas, stream);
+        case 128: return launch_batched_inst<4, 1, 8, 256, 3, MODE>(args, max_ctas, stream);
+        case 256: return launch_batched_inst<8, 1, 8, 256, 3, MODE>(args, max_ctas, stream);
+        default: return launch_batched_inst<8, 2, 4, 256, 4, MODE>(args, max_ctas, stream);
+    }
+}
+
 }  // namespace
 
 extern "C" {
+
+int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j_offsets, int64_t n_i_total,
+                     const float* x_i, int64_t n_j_total, const float* x_j, const float* m_j, float eps2,
+                     float* acc_out, float* pot_out, void* stream_) {
+    t_launches = 0;
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (bad_count(n_batch) || bad_count(n_i_total) || bad_count(n_j_total)) return NB_ERR_INVALID_VALUE;
+    if (!(eps2 >= 0.0f) || !std::isfinite(eps2)) return NB_ERR_INVALID_VALUE;
+    if (n_batch > 0 && (!i_offsets || !j_offsets)) return NB_ERR_INVALID_VALUE;
+    if (n_i_total > 0 && (!x_i || !acc_out)) return NB_ERR_INVALID_VALUE;
+    if (n_j_total > 0 && (!x_j || !m_j)) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n_batch == 0 || n_i_total == 0) return NB_OK;
+    Workspace* ws;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        ws = &g_ws[std::make_pair(dev, stream)];
+    }
+    rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)(n_j_total > 0 ? n_j_total : 1) * sizeof(float4), stream);
+    if (rc != NB_OK) return rc;
+    const int tile = batched_tile(n_i_total, n_batch);
+    // sum_b ceil(n_i(b) / tile) <= n_i_total / tile + n_batch
+    const int64_t max_ctas = n_i_total / tile + n_batch;
+    if (max_ctas > (int64_t)INT32_MAX) return NB_ERR_INVALID_VALUE;
+    rc = ensure(&ws->tiles, &ws->tiles_bytes, (size_t)(n_batch + 1 + max_ctas) * sizeof(int), stream);
+    if (rc != NB_OK) return rc;
+    if (n_j_total > 0) {
+        nb::nb_pack_j_kernel<<<(unsigned)((n_j_total + 255) / 256), 256, 0, stream>>>(x_j, m_j, (int)n_j_total,
+                                                                                      reinterpret_cast<float4*>(ws->jp));
+        NB_CUDA(cudaGetLastError());
+        ++t_launches;
+    }
+    int* tile_start = reinterpret_cast<int*>(ws->tiles);
+    int* cta_batch = tile_start + n_batch + 1;
+    nb::nb_batch_scan_kernel<<<1, 1024, 0, stream>>>(i_offsets, (int)n_batch, tile, tile_start, cta_batch);
+    NB_CUDA(cudaGetLastError());
+    ++t_launches;
+
+    nb::ForceArgs args;
+    args.x_i = x_i;
+    args.jp = reinterpret_cast<const float4*>(ws->jp);
+    args.acc = acc_out;
+    args.pot = pot_out;
+    args.partial = nullptr;
+    args.coin_lists = nullptr;
+    args.coin_flag = nullptr;
+    args.i_off = i_offsets;
+    args.j_off = j_offsets;
+    args.tile_start = tile_start;
+    args.cta_batch = cta_batch;
+    args.n_batch = (int)n_batch;
+    args.n_i = (int)n_i_total;
+    args.n_j = (int)n_j_total;
+    args.S = 1;
+    args.eps2 = eps2;
+    // Interaction lists start with the group's own members (coincident pairs in every sub-problem), and the
+    // speculative mode's redo would fall on one warp of the CTA, so batched calls mask every pair by default.
+    const char* e = std::getenv("NB_MASK");
+    const bool spec = eps2 >= kSpecMinEps2 && (e && e[0] == 's');
+    return spec ? launch_batched<nb::MODE_SPEC>(args, tile, (unsigned)max_ctas, stream)
+                : launch_batched<nb::MODE_EXACT>(args, tile, (unsigned)max_ctas, stream);
+}
 
 int nb_force_jerk(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j, const float* x_j, const float* v_j,
                   const float* m_j, float eps2, float* acc_out, float* jerk_out, float* pot_out, void* stream) {
@@ -572,6 +696,7 @@ int nb_release_workspace(void) {
             if (it->second.stage) (void)cudaFree(it->second.stage);
             if (it->second.coin) (void)cudaFree(it->second.coin);
             if (it->second.jp2) (void)cudaFree(it->second.jp2);
+            if (it->second.tiles) (void)cudaFree(it->second.tiles);
             if (it->second.hpartial) (void)cudaFree(it->second.hpartial);
             it = g_ws.erase(it);
         } else {

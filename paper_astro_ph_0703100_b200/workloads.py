@@ -174,3 +174,77 @@ def config(k: int, scale: float = 1.0) -> Workload:
         return plummer_workload(s(65536), 1.0 / 128, seed=4, name="C4", with_velocities=True,
                                 dt=1.0 / 512, n_steps=1000)
     raise ValueError(f"no config {k}")
+
+
+# ---------------------------------------------------------------------------------------------
+# Row f2: interaction lists of a host tree code (section
+# 4.4: "the force calculation on several thousands particles", Barnes' modified tree algorithm).
+# The paper gives no tree and no list statistics beyond "several thousands"; the recipe below only
+# reproduces the SHAPE of such a call sequence -- many groups of a few tens to a few hundred
+# i-particles, each with its own list of a few thousand j-particles (its own members, near
+# neighbours taken directly, and heavier pseudo-particles standing for far cells).
+@dataclass
+class BatchedWorkload:
+    name: str
+    i_offsets: np.ndarray           # int32 [n_batch + 1]
+    j_offsets: np.ndarray           # int32 [n_batch + 1]
+    x_i: np.ndarray                 # float32 [n_i_total, 3]
+    x_j: np.ndarray                 # float32 [n_j_total, 3]
+    m_j: np.ndarray                 # float32 [n_j_total]
+    eps2: float
+    seed: int = 0
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def n_batch(self) -> int:
+        return int(self.i_offsets.shape[0] - 1)
+
+    @property
+    def pairs(self) -> int:
+        ni = np.diff(self.i_offsets).astype(np.int64)
+        nj = np.diff(self.j_offsets).astype(np.int64)
+        return int((ni * nj).sum())
+
+
+def tree_list_workload(n_particles: int, group_min: int, group_max: int, list_min: int, list_max: int, eps: float,
+                       seed: int, name: str = "tree-lists", max_groups: Optional[int] = None) -> BatchedWorkload:
+    """Groups = runs of consecutive particles of a Plummer sphere sorted along a 3-D grid order.
+
+    Draw order: Plummer positions (X1, X2, X3); group sizes (uniform integers, cut to cover the
+    sorted particles); then per group: list length (uniform integer), the indices of the direct
+    neighbours (``rng.choice`` over all particles, without replacement), the cell positions
+    (a fresh Plummer draw) and the cell occupation numbers (uniform integers 2..64; a cell's mass
+    is that many particle masses).  One third of a list (rounded down) are cells.
+    """
+    rng = _rng(seed)
+    pos, _ = plummer_positions(n_particles, rng)
+    cell = np.floor((pos + 10.0) * (64.0 / 20.0)).astype(np.int64).clip(0, 63)
+    order = np.lexsort((cell[:, 2], cell[:, 1], cell[:, 0]))
+    pos = pos[order]
+    m = 1.0 / n_particles
+    sizes = []
+    left = n_particles
+    while left > 0 and (max_groups is None or len(sizes) < max_groups):
+        g = int(min(left, rng.integers(group_min, group_max + 1)))
+        sizes.append(g)
+        left -= g
+    i_off = np.concatenate([[0], np.cumsum(sizes)])
+    xi_parts, xj_parts, mj_parts, lens = [], [], [], []
+    for b, g in enumerate(sizes):
+        own = np.arange(i_off[b], i_off[b + 1])
+        n_list = int(rng.integers(list_min, list_max + 1))
+        n_cells = n_list // 3
+        n_near = max(0, n_list - n_cells - g)
+        near = rng.choice(n_particles, n_near, replace=False)
+        cells, _ = plummer_positions(n_cells, rng)
+        occ = rng.integers(2, 65, n_cells)
+        xi_parts.append(pos[own])
+        xj_parts.append(np.concatenate([pos[own], pos[near], cells]))
+        mj_parts.append(np.concatenate([np.full(g + n_near, m), occ * m]))
+        lens.append(g + n_near + n_cells)
+    j_off = np.concatenate([[0], np.cumsum(lens)])
+    return BatchedWorkload(name=name, i_offsets=i_off.astype(np.int32), j_offsets=j_off.astype(np.int32),
+                           x_i=_f32(np.concatenate(xi_parts)), x_j=_f32(np.concatenate(xj_parts)),
+                           m_j=_f32(np.concatenate(mj_parts)), eps2=float(np.float32(eps * eps)), seed=seed,
+                           meta={"model": "plummer a=1 truncated at 10a, grid-sorted groups with own + near + cell lists",
+                                 "eps": eps, "groups": len(sizes)})

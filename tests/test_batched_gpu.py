@@ -1,0 +1,127 @@
+"""Parity of nb_force_batched (row f2: tree-code interaction lists) against the oracle.
+
+Same tolerances as nb_force (BASELINE.json north_star): acc RMS <= 1e-5, max <= 1e-4; phi RMS <= 1e-5.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_astro_ph_0703100_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def nb():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    import paper_astro_ph_0703100_b200 as nb_
+    nb_.lib()
+    return nb_
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_batched(nb, w, want_pot=True, fill=None):
+    import torch
+    acc = pot = None
+    if fill is not None:
+        acc = torch.full((w.x_i.shape[0], 3), fill, dtype=torch.float32, device="cuda")
+        pot = torch.full((w.x_i.shape[0],), fill, dtype=torch.float32, device="cuda")
+    acc, pot = nb.force_batched(dev(w.i_offsets), dev(w.j_offsets), dev(w.x_i), dev(w.x_j), dev(w.m_j), w.eps2,
+                                acc_out=acc, pot_out=pot, want_pot=want_pot)
+    torch.cuda.synchronize()
+    return acc.cpu().numpy(), (None if pot is None else pot.cpu().numpy())
+
+
+def check(acc, pot, ra, rp, label=""):
+    e = oracle.error_metrics(acc, ra, pot, rp)
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4, (label, e)
+    if pot is not None:
+        assert e["pot_rms"] <= 1e-5, (label, e)
+
+
+@pytest.mark.parametrize("tile", ["64", "128", "256", "512", ""])
+def test_tree_lists_every_tile_shape(nb, tile, monkeypatch):
+    if tile:
+        monkeypatch.setenv("NB_BATCH_TILE", tile)
+    w = wl.tree_list_workload(6000, 20, 300, 900, 2500, 1.0 / 128, seed=5)
+    acc, pot = gpu_batched(nb, w)
+    ra, rp = oracle.force_batched(w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j, w.eps2)
+    check(acc, pot, ra, rp, "tile " + tile)
+
+
+def test_equals_separate_nb_force_calls_within_tolerance_and_masks_own_members(nb):
+    w = wl.tree_list_workload(3000, 50, 120, 500, 900, 1.0 / 64, seed=8)
+    acc, pot = gpu_batched(nb, w)
+    # each group's list starts with its own members: the self term m/eps would shift phi by ~ 0.02 (2 % of |phi|)
+    ra, rp = oracle.force_batched(w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j, w.eps2)
+    check(acc, pot, ra, rp, "own members")
+    import torch
+    b = 3
+    i0, i1, j0, j1 = (int(v) for v in (w.i_offsets[b], w.i_offsets[b + 1], w.j_offsets[b], w.j_offsets[b + 1]))
+    a1, p1 = nb.force(dev(w.x_i[i0:i1]), dev(w.x_j[j0:j1]), dev(w.m_j[j0:j1]), w.eps2)
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(acc[i0:i1], a1.cpu().numpy(), rtol=2e-5, atol=1e-7)
+    np.testing.assert_allclose(pot[i0:i1], p1.cpu().numpy(), rtol=2e-6)
+
+
+def test_edge_cases_empty_groups_empty_lists_gaps(nb):
+    rng = np.random.default_rng(2)
+    x_i = rng.normal(size=(700, 3)).astype(np.float32)
+    x_j = rng.normal(size=(5000, 3)).astype(np.float32)
+    m_j = rng.uniform(0.5, 1.5, 5000).astype(np.float32)
+    # sub-problems: normal, empty i-range, empty j-list, 1 x 1, ragged tail; i in [650, 700) belongs to nobody
+    i_off = np.array([0, 100, 100, 163, 164, 650], dtype=np.int32)
+    j_off = np.array([0, 3000, 3100, 3100, 3101, 4999], dtype=np.int32)
+    w = wl.BatchedWorkload("edge", i_off, j_off, x_i, x_j, m_j, 1e-3)
+    acc, pot = gpu_batched(nb, w, fill=7.0)
+    ra, rp = oracle.force_batched(i_off, j_off, x_i, x_j, m_j, 1e-3)
+    assert np.all(acc[100:163] == 0.0) and np.all(pot[100:163] == 0.0)          # empty list -> zeros
+    assert np.all(acc[650:] == 7.0) and np.all(pot[650:] == 7.0)                # nobody's particles: untouched
+    sel = np.r_[0:100, 163:650]
+    check(acc[sel], pot[sel], ra[sel], rp[sel], "edge")
+    # n_batch = 0 and invalid arguments
+    import torch
+    z = torch.zeros((1,), dtype=torch.int32, device="cuda")
+    a0, p0 = nb.force_batched(z, z, dev(x_i), dev(x_j), dev(m_j), 1e-3)
+    assert nb.lib().nb_force_batched(3, None, None, 10, None, 10, None, None, 0.1, None, None, None) == 1
+    with pytest.raises(nb.NBError):
+        nb.force_batched(dev(i_off), dev(j_off), dev(x_i), dev(x_j), dev(m_j), -1.0)
+
+
+def test_eps0_and_masked_mode_agree(nb, monkeypatch):
+    w = wl.tree_list_workload(2000, 30, 90, 300, 700, 1.0 / 64, seed=3)
+    a_e, p_e = gpu_batched(nb, w)                     # default: every pair masked
+    monkeypatch.setenv("NB_MASK", "spec")
+    a_s, p_s = gpu_batched(nb, w)                     # speculative mode with masked redo: same bits
+    assert np.array_equal(a_s, a_e) and np.array_equal(p_s, p_e)
+    monkeypatch.delenv("NB_MASK")
+    w0 = wl.BatchedWorkload("eps0", w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j, 0.0)
+    acc, pot = gpu_batched(nb, w0)
+    ra, rp = oracle.force_batched(w0.i_offsets, w0.j_offsets, w0.x_i, w0.x_j, w0.m_j, 0.0)
+    assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot))
+    check(acc, pot, ra, rp, "eps0")
+
+
+def test_reproducible_and_pot_null(nb):
+    w = wl.tree_list_workload(4000, 32, 256, 1000, 3000, 1.0 / 128, seed=6)
+    a1, p1 = gpu_batched(nb, w)
+    a2, p2 = gpu_batched(nb, w)
+    assert np.array_equal(a1, a2) and np.array_equal(p1, p2)
+    a3, p3 = gpu_batched(nb, w, want_pot=False)
+    assert p3 is None and np.array_equal(a1, a3)
+
+
+def test_bench_size_sampled(nb):
+    """The size bench.py --op batched times (65536 particles, groups 32..256, lists 2000..6000): sampled groups."""
+    w = wl.tree_list_workload(65536, 32, 256, 2000, 6000, 1.0 / 128, seed=7)
+    acc, pot = gpu_batched(nb, w)
+    rng = np.random.default_rng(0)
+    for b in rng.choice(w.n_batch, 24, replace=False):
+        i0, i1, j0, j1 = (int(v) for v in (w.i_offsets[b], w.i_offsets[b + 1], w.j_offsets[b], w.j_offsets[b + 1]))
+        ra, rp = oracle.force(w.x_i[i0:i1], w.x_j[j0:j1], w.m_j[j0:j1], w.eps2)
+        check(acc[i0:i1], pot[i0:i1], ra, rp, f"group {b}")

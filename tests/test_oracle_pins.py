@@ -416,3 +416,19 @@ def test_error_metric_eq3():
     assert e["acc_max"] == pytest.approx(0.1)
     assert e["acc_rms"] == pytest.approx(0.1 / math.sqrt(2))
     assert e["pot_max"] == pytest.approx(0.1)
+
+
+def test_f2_batched_entry_is_one_force_call_per_sub_problem():
+    """oracle.force_batched against the mpmath brute force, sub-problem by sub-problem (tiny), incl. empty ones."""
+    rng = np.random.default_rng(4)
+    x_i = rng.normal(size=(7, 3)); x_j = rng.normal(size=(12, 3)); m_j = rng.uniform(0.5, 1.5, 12)
+    x_j[2] = x_i[1]                                   # a coincident pair inside sub-problem 0
+    i_off = np.array([0, 3, 3, 6]); j_off = np.array([0, 5, 9, 12])
+    acc, pot = oracle.force_batched(i_off, j_off, x_i, x_j, m_j, 0.01)
+    for b in range(3):
+        i0, i1, j0, j1 = i_off[b], i_off[b + 1], j_off[b], j_off[b + 1]
+        if i1 > i0:
+            ra, rp = _brute_force_mp(x_i[i0:i1], x_j[j0:j1], m_j[j0:j1], 0.01)
+            np.testing.assert_allclose(acc[i0:i1], ra, rtol=1e-13, atol=1e-15)
+            np.testing.assert_allclose(pot[i0:i1], rp, rtol=1e-13)
+    assert not acc[6].any() and pot[6] == 0.0         # outside every sub-problem
