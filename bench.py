@@ -146,28 +146,37 @@ def replica_throughput(pairs_per_rank_step, world, steps, total_ms):
     return world * pairs_per_rank_step * steps / (total_ms * 1e-3)
 
 
-def reference_arm(args, w, cfg_name):
+def reference_arm(args, wl):
     """--impl reference: the CPU oracle (this tier has no reference implementation), rank 0 only."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import oracle
+    if args.op == "force":
+        w = wl.config(CONFIG_INDEX[args.config])
+        name = workload_name(args.config, w)
+    elif args.op == "jerk":
+        w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
+        name = "row f1 (H1): plummer N=131072 with velocities, one force+jerk+phi evaluation"
+    else:
+        w = wl.tree_list_workload(524288, 32, 256, 2000, 6000, 1.0 / 128, seed=7, name="T1")
+        name = "row f2 (T1): tree lists, 524288 particles, groups 32..256, lists 2000..6000"
     per_step = max(0.5, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
-        oracle_rate(w, per_step / 4)
-    rates, sample = [], ""
+        oracle_rate_op(args.op, w, per_step / 4)
+    rates, sample, cores = [], "", 0
     t0 = time.perf_counter()
     for s in range(args.steps):
-        r, cores, sample = oracle_rate(w, per_step, rng_seed=s)
+        r, cores, sample = oracle_rate_op(args.op, w, per_step, rng_seed=s)
         rates.append(r)
     wall = time.perf_counter() - t0
     value = float(np.mean(rates))
+    f_lo, f_hi = OPS[args.op]["flops"]
     out = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(cfg_name, w)},
-        "gflops_20": 20e-9 * value, "gflops_38": 38e-9 * value,
+        "config": {"workload": name, "op": args.op},
+        f"gflops_{f_lo}": f_lo * 1e-9 * value, f"gflops_{f_hi}": f_hi * 1e-9 * value,
         "cpu_baseline": {"value": value, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -180,12 +189,132 @@ def workload_name(cfg_name, w):
             f"n_i={w.n_i}, n_j={w.n_j}, eps2={w.eps2:.6g}, seed={w.seed}, one nb_force call with phi")
 
 
+# ---------------------------------------------------------------------------------------------
+# The ops bench.py can time.  "force" (default) is the contract line: BASELINE.json's metric on
+# configs[1].  "jerk" (row f1) and "batched" (row f2) are the widened rows, each with its own
+# instruction count per interaction for the roofline.
+OPS = {
+    "force": {"inst": 13, "kernel": "nb_force_kernel (pair interaction, rows a2-a7)", "flops": (20, 38)},
+    "jerk": {"inst": 27, "kernel": "nb_hermite_kernel (force + jerk + potential, row f1)", "flops": (60, 60)},
+    "batched": {"inst": 13, "kernel": "nb_force_kernel<BATCHED> (row f2)", "flops": (20, 38)},
+}
+
+
+class Problem:
+    """One op on one workload: device call, end-to-end call from pinned host buffers, oracle sample."""
+
+    def __init__(self, op, cfg_name, nb, torch, wl):
+        self.op, self.nb, self.torch = op, nb, torch
+        if op == "force":
+            w = wl.config(CONFIG_INDEX[cfg_name])
+            self.w, self.pairs, self.name = w, float(w.pairs), workload_name(cfg_name, w)
+            self.host = [w.x_j, w.m_j] + ([] if w.x_i is None else [w.x_i])
+            self.n_out = w.n_i
+        elif op == "jerk":
+            w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
+            self.w, self.pairs = w, float(w.n_i) * float(w.n_j)
+            self.name = (f"row f1 (H1): {w.meta.get('model', '')} with Aarseth velocities, n_i=n_j={w.n_j}, "
+                         f"eps2={w.eps2:.6g}, seed=1, one nb_force_jerk call with phi (configs[1]'s particles)")
+            self.host = [w.x_j, w.v, w.m_j]
+            self.n_out = w.n_i
+        else:
+            w = wl.tree_list_workload(524288, 32, 256, 2000, 6000, 1.0 / 128, seed=7, name="T1")
+            self.w, self.pairs = w, float(w.pairs)
+            self.name = (f"row f2 (T1): {w.meta.get('model', '')}; 524288 particles in {w.n_batch} groups of 32..256, "
+                         f"lists of 2000..6000, eps2={w.eps2:.6g}, seed=7, one nb_force_batched call with phi")
+            self.host = [w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j]
+            self.n_out = w.x_i.shape[0]
+        self.dev = [torch.from_numpy(a).cuda() for a in self.host]
+        self.pinned = [torch.from_numpy(a).pin_memory() for a in self.host]
+        n = self.n_out
+        self.outs = [torch.empty((n, 3), dtype=torch.float32, device="cuda")]
+        if op == "jerk":
+            self.outs.append(torch.empty((n, 3), dtype=torch.float32, device="cuda"))
+        self.outs.append(torch.empty((n,), dtype=torch.float32, device="cuda"))
+        self.h_outs = [torch.empty(o.shape, dtype=torch.float32).pin_memory() for o in self.outs]
+        self.h2d = int(sum(a.nbytes for a in self.host))
+        self.d2h = int(sum(o.numel() * 4 for o in self.outs))
+
+    def call(self, t=None):
+        t = self.dev if t is None else t
+        nb, w = self.nb, self.w
+        if self.op == "force":
+            xj, mj = t[0], t[1]
+            xi = xj if w.x_i is None else t[2]
+            nb.force(xi, xj, mj, w.eps2, acc_out=self.outs[0], pot_out=self.outs[1])
+        elif self.op == "jerk":
+            nb.force_jerk(t[0], t[1], t[0], t[1], t[2], w.eps2, acc_out=self.outs[0], jerk_out=self.outs[1], pot_out=self.outs[2])
+        else:
+            nb.force_batched(t[0], t[1], t[2], t[3], t[4], w.eps2, acc_out=self.outs[0], pot_out=self.outs[1])
+
+    def call_e2e(self):
+        """Inputs from pinned host memory, results back to pinned host memory, blocking."""
+        nb, w = self.nb, self.w
+        if self.op == "force":
+            h = [p.numpy() for p in self.pinned]
+            nb.force_host(h[0] if w.x_i is None else h[2], h[0], h[1], w.eps2,
+                          acc_out=self.h_outs[0].numpy(), pot_out=self.h_outs[1].numpy())
+            return
+        staged = [p.cuda(non_blocking=True) for p in self.pinned]
+        self.call(staged)
+        for h, d in zip(self.h_outs, self.outs):
+            h.copy_(d, non_blocking=True)
+        self.torch.cuda.synchronize()
+
+    @property
+    def e2e_api(self):
+        if self.op == "force":
+            return "nb_force_host (pinned host buffers)"
+        return f"pinned host tensors -> cudaMemcpyAsync -> nb_{'force_jerk' if self.op == 'jerk' else 'force_batched'} -> cudaMemcpyAsync -> pinned host"
+
+    def plan(self, sm_count):
+        if self.op == "force":
+            return self.nb.plan_query(self.w.n_i, self.w.n_j, sm_count)
+        if self.op == "jerk":
+            return self.nb.plan_query_jerk(self.w.n_i, self.w.n_j, sm_count)
+        return {"cta": "one row of CTAs, 8 warps split each list (WJ = 8), no split across CTAs"}
+
+
+def oracle_rate_op(op, w, target_seconds, rng_seed=0):
+    """CPU oracle, as it stands, on a bounded sample of the op's workload: (pairs/s, cores, sample)."""
+    import oracle
+    if op == "force":
+        return oracle_rate(w, target_seconds, rng_seed)
+    cores = oracle.num_threads()
+    rng = np.random.default_rng(rng_seed)
+    if op == "jerk":
+        def run(n_i):
+            idx = np.sort(rng.choice(w.n_i, n_i, replace=False))
+            xi, vi = np.ascontiguousarray(w.x_j[idx]), np.ascontiguousarray(w.v[idx])
+            t0 = time.perf_counter()
+            oracle.force_jerk(xi, vi, w.x_j, w.v, w.m_j, w.eps2)
+            return time.perf_counter() - t0
+        run(64)
+        n_probe = max(64, 8 * cores)
+        rate = n_probe * w.n_j / run(n_probe)
+        n_i = int(min(w.n_i, max(n_probe, target_seconds * rate / w.n_j)))
+        t = run(n_i)
+        return n_i * w.n_j / t, cores, f"{n_i} of {w.n_i} i-particles (seeded) x all {w.n_j} j-particles, {t:.2f} s"
+    order = rng.permutation(w.n_batch)
+    pairs, t0, used = 0, time.perf_counter(), 0
+    for b in order:
+        i0, i1, j0, j1 = (int(v) for v in (w.i_offsets[b], w.i_offsets[b + 1], w.j_offsets[b], w.j_offsets[b + 1]))
+        oracle.force(w.x_i[i0:i1], w.x_j[j0:j1], w.m_j[j0:j1], w.eps2)
+        pairs += (i1 - i0) * (j1 - j0)
+        used += 1
+        if time.perf_counter() - t0 > target_seconds:
+            break
+    t = time.perf_counter() - t0
+    return pairs / t, cores, f"{used} of {w.n_batch} sub-problems (seeded order), one oracle.force call each, {t:.2f} s"
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
+    ap.add_argument("--op", default="force", choices=sorted(OPS))
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -193,10 +322,9 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
     from paper_astro_ph_0703100_b200 import workloads as wl
-    w = wl.config(CONFIG_INDEX[args.config])
 
     if args.impl == "reference":
-        reference_arm(args, w, args.config)
+        reference_arm(args, wl)
         return
 
     import torch
@@ -214,13 +342,10 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     nb.lib()
     peaks, peaks_kind = load_peaks()
+    op = OPS[args.op]
 
     # inputs resident in HBM before the timed region
-    d_xj = torch.from_numpy(w.x_j).cuda()
-    d_mj = torch.from_numpy(w.m_j).cuda()
-    d_xi = d_xj if w.x_i is None else torch.from_numpy(w.x_i).cuda()
-    acc = torch.empty((w.n_i, 3), dtype=torch.float32, device="cuda")
-    pot = torch.empty((w.n_i,), dtype=torch.float32, device="cuda")
+    prob = Problem(args.op, args.config, nb, torch, wl)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
 
@@ -231,7 +356,7 @@ def main():
 
     for _ in range(args.warmup):
         flush.fill_(1)
-        nb.force(d_xi, d_xj, d_mj, w.eps2, acc_out=acc, pot_out=pot)
+        prob.call()
     torch.cuda.synchronize()
     launches_per_step = nb.last_launch_count()
 
@@ -244,7 +369,7 @@ def main():
     for s in range(args.steps):
         flush.fill_(s & 0xff)                      # L2 flush between timed iterations (outside the events)
         ev[s][0].record(stream)
-        nb.force(d_xi, d_xj, d_mj, w.eps2, acc_out=acc, pot_out=pot)
+        prob.call()
         ev[s][1].record(stream)
     barrier()
     t_wall = time.perf_counter() - t_wall0
@@ -254,67 +379,65 @@ def main():
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
 
-    # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
-    h_xj = torch.from_numpy(w.x_j).pin_memory()
-    h_mj = torch.from_numpy(w.m_j).pin_memory()
-    h_xi = h_xj if w.x_i is None else torch.from_numpy(w.x_i).pin_memory()
-    h_acc = torch.empty((w.n_i, 3), dtype=torch.float32).pin_memory()
-    h_pot = torch.empty((w.n_i,), dtype=torch.float32).pin_memory()
+    # end to end with HOST buffers (pinned), copies inside the timed region
     e2e_steps = max(3, min(args.steps, 10))
     for _ in range(2):
-        nb.force_host(h_xi.numpy(), h_xj.numpy(), h_mj.numpy(), w.eps2, acc_out=h_acc.numpy(), pot_out=h_pot.numpy())
+        prob.call_e2e()
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        nb.force_host(h_xi.numpy(), h_xj.numpy(), h_mj.numpy(), w.eps2, acc_out=h_acc.numpy(), pot_out=h_pot.numpy())
+        prob.call_e2e()
     torch.cuda.synchronize()
     e2e_ms = 1e3 * (time.perf_counter() - t0)
-    h2d = w.x_j.nbytes + w.m_j.nbytes + (0 if w.x_i is None else w.x_i.nbytes)
-    d2h = h_acc.numel() * 4 + h_pot.numel() * 4
 
     # max over ranks
     total_ms, e2e_ms = reduce_max([total_ms, e2e_ms], world)
 
     if rank == 0:
-        pairs = float(w.pairs)
+        pairs = prob.pairs
         value = replica_throughput(pairs, world, args.steps, total_ms)
         e2e_value = replica_throughput(pairs, world, e2e_steps, e2e_ms)
         f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
         sm_count = torch.cuda.get_device_properties(0).multi_processor_count
         peak_inst = sm_count * FP32_LANES_PER_SM_CLK * f_max                 # FP32-pipe lane-instructions / s
         k_rate = pairs * n_k / (k_ms * 1e-3) if n_k else 0.0
-        achieved = FP32_INST_PER_PAIR * k_rate
+        inst = op["inst"]
+        achieved = inst * k_rate
+        traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if args.op == "force" else NCU_DRAM_BYTES_PER_LAUNCH.get(args.op)
         roofline = {
-            "bound": "alu", "kernel": "nb_force_kernel (pair interaction, rows a2-a7)",
+            "bound": "alu", "kernel": op["kernel"],
             "achieved": achieved / 1e12, "peak": peak_inst / 1e12, "unit": "FP32-pipe Tinst/s",
-            "frac": achieved / peak_inst, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config),
-            "traffic_unit": "DRAM bytes per launch (ncu --set full, profiles/r01_force_c1_ncu_full.md)",
+            "frac": achieved / peak_inst, "traffic": traffic,
+            "traffic_unit": "DRAM bytes per launch (ncu --set full, profiles/)",
             "kernel_ms": k_ms / max(1, n_k), "kernel_launches_timed": n_k,
-            "kernel_interactions_per_s": k_rate, "roofline_interactions_per_s": peak_inst / FP32_INST_PER_PAIR,
+            "kernel_interactions_per_s": k_rate, "roofline_interactions_per_s": peak_inst / inst,
             "peak_source": f"{sm_count} SMs x {FP32_LANES_PER_SM_CLK} FP32 lanes x sm_max_mhz {f_max / 1e6:.0f} MHz "
-                           f"({peaks_kind} MEASURED_PEAKS.json clock), {FP32_INST_PER_PAIR} FMA-pipe instr/interaction",
+                           f"({peaks_kind} MEASURED_PEAKS.json clock), {inst} FMA-pipe instr/interaction",
         }
         if clocks.get("sm_mhz"):
             roofline["frac_at_observed_clock"] = achieved / (sm_count * FP32_LANES_PER_SM_CLK * clocks["sm_mhz"] * 1e6)
+        f_lo, f_hi = op["flops"]
         out = {
             "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload_name(args.config, w), "parallelism": "replicas only" if world > 1 else "1 gpu",
+            "config": {"workload": prob.name, "op": args.op,
+                       "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": f"flushed between timed iterations ({L2_FLUSH_BYTES >> 20} MiB write, outside the events)",
-                       "plan": nb.plan_query(w.n_i, w.n_j, sm_count)},
-            "gflops_20": 20e-9 * value, "gflops_38": 38e-9 * value,
+                       "plan": prob.plan(sm_count)},
+            f"gflops_{f_lo}": f_lo * 1e-9 * value, f"gflops_{f_hi}": f_hi * 1e-9 * value,
             "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps, "api": "nb_force_host (pinned host buffers)"},
+            "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": prob.h2d, "d2h_bytes_per_step": prob.d2h,
+                    "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps, "api": prob.e2e_api},
             "gpu_launches": int(launches_per_step * args.steps),
             "roofline": roofline,
             "wall_s_timed_region": t_wall,
             "paper_context": {"gflops_38_8800gtx_n131072": 256, "interactions_per_s_8800gtx_n131072": 6.74e9,
-                              "note": "PAPER.md:314, includes PCIe copies; context, not target"},
+                              "gflops_force_jerk_8800gtx_n131072": 179,
+                              "note": "PAPER.md:314 (includes PCIe copies) and PAPER.md:343; context, not target"},
         }
         if not args.no_cpu_baseline:
-            v, cores, sample = oracle_rate(w, args.cpu_seconds)
+            v, cores, sample = oracle_rate_op(args.op, prob.w, args.cpu_seconds)
             out["cpu_baseline"] = {"value": v, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample}
         print(json.dumps(out), flush=True)
     if world > 1:
