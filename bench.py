@@ -33,9 +33,9 @@ FP32_INST_PER_PAIR = 13          # FMA-pipe instructions per interaction (acc + 
 FP32_LANES_PER_SM_CLK = 128
 CONFIG_INDEX = {"C0": 0, "C1": 1, "C2": 2, "C3": 3, "C4": 4}
 L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
-# dram__bytes_read.sum + dram__bytes_write.sum of one nb_force_kernel launch, from the committed
-# `ncu --set full` captures (profiles/r01_force_c1_ncu_full.md); null for configs without a capture
-NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 8.63e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/r01_ncu_full.md); null for configs / ops without a capture
+NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 71.1e6, "jerk": 105.4e6}
 
 
 def load_peaks():
