@@ -56,6 +56,8 @@ def _load():
         lib.oracle_force_jerk_f64.restype = ctypes.c_int
         lib.oracle_force_jerk_f32.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p]
         lib.oracle_force_jerk_f32.restype = ctypes.c_int
+        lib.oracle_force_eps_i_f64.argtypes = [i64, p, p, i64, p, p, p, p]
+        lib.oracle_force_eps_i_f64.restype = ctypes.c_int
         lib.oracle_num_threads.restype = ctypes.c_int
         lib.oracle_set_num_threads.argtypes = [ctypes.c_int]
         _lib = lib
@@ -121,6 +123,22 @@ def force_jerk(x_i: np.ndarray, v_i: np.ndarray, x_j: np.ndarray, v_j: np.ndarra
     if rc != 0:
         raise ValueError(f"oracle_force_jerk returned {rc}")
     return acc, jerk, pot
+
+
+def force_eps_i(x_i: np.ndarray, eps2_i: np.ndarray, x_j: np.ndarray, m_j: np.ndarray, want_pot: bool = True):
+    """Row f3: Eq. (1) and phi with one eps^2 per i-particle (Fig. A.1).  Inputs (float32 or
+    float64) are promoted exactly to double.  Returns (acc [n_i,3], pot [n_i] or None) in float64."""
+    xi, xj = _c(x_i, np.float64).reshape(-1, 3), _c(x_j, np.float64).reshape(-1, 3)
+    e2, mj = _c(eps2_i, np.float64).reshape(-1), _c(m_j, np.float64).reshape(-1)
+    n_i, n_j = xi.shape[0], xj.shape[0]
+    if e2.shape[0] != n_i or mj.shape[0] != n_j:
+        raise ValueError("array lengths differ")
+    acc = np.zeros((n_i, 3), dtype=np.float64)
+    pot = np.zeros(n_i, dtype=np.float64) if want_pot else None
+    rc = _load().oracle_force_eps_i_f64(n_i, _ptr(xi), _ptr(e2), n_j, _ptr(xj), _ptr(mj), _ptr(acc), _ptr(pot))
+    if rc != 0:
+        raise ValueError(f"oracle_force_eps_i returned {rc}")
+    return acc, pot
 
 
 def force_batched(i_offsets: np.ndarray, j_offsets: np.ndarray, x_i: np.ndarray, x_j: np.ndarray, m_j: np.ndarray,

@@ -287,3 +287,30 @@ int oracle_force_jerk_f32(int64_t n_i, const float *x_i, const float *v_i, int64
     free(xj); free(vj); free(mj);
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Row f3: the softening travels PER i-PARTICLE, as in the paper's own driver,
+ * where slot 3 of every i-record is eps2 (Fig. A.1: p_xi[i][3] = eps2;
+ * Fig. A.3: eps2 = INPUT_I[3]).  Same sum as one_i() with eps2 -> eps2_i[i].
+ * Pins (tests/test_oracle_pins.py, "f3"): a constant array reproduces oracle_force_f64 bit for bit;
+ * exact two-body rationals with a different eps2 per i; mpmath brute force.
+ */
+int oracle_force_eps_i_f64(int64_t n_i, const double *x_i, const double *eps2_i, int64_t n_j, const double *x_j,
+                           const double *m_j, double *acc, double *pot)
+{
+    if (n_i < 0 || n_j < 0) return 1;
+    if (n_i > 0 && (!x_i || !eps2_i || !acc)) return 1;
+    if (n_j > 0 && (!x_j || !m_j)) return 1;
+    for (int64_t i = 0; i < n_i; ++i)
+        if (!(eps2_i[i] >= 0.0)) return 1;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n_i; ++i) {
+        double out[4];
+        one_i(&x_i[3 * i], n_j, x_j, m_j, eps2_i[i], out);     /* eps2 = INPUT_I[3] */
+        acc[3 * i + 0] = out[0];
+        acc[3 * i + 1] = out[1];
+        acc[3 * i + 2] = out[2];
+        if (pot) pot[i] = out[3];
+    }
+    return 0;
+}

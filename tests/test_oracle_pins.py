@@ -432,3 +432,40 @@ def test_f2_batched_entry_is_one_force_call_per_sub_problem():
             np.testing.assert_allclose(acc[i0:i1], ra, rtol=1e-13, atol=1e-15)
             np.testing.assert_allclose(pot[i0:i1], rp, rtol=1e-13)
     assert not acc[6].any() and pot[6] == 0.0         # outside every sub-problem
+
+
+# ----------------------------------------------------------------------------- row f3: eps2 per i-particle
+def test_f3_constant_array_reproduces_the_scalar_entry_bitwise():
+    rng = np.random.default_rng(11)
+    x = rng.normal(size=(60, 3)); m = rng.uniform(0.5, 1.5, 60)
+    a0, p0 = oracle.force(x[:17], x, m, 0.03)
+    a1, p1 = oracle.force_eps_i(x[:17], np.full(17, 0.03), x, m)
+    assert np.array_equal(a0, a1) and np.array_equal(p0, p1)
+
+
+def test_f3_two_body_exact_with_a_different_eps2_per_i():
+    """Golden rows (d, eps2, m, s) of two_body_exact.txt, all i-particles in ONE call, each with its own eps2."""
+    rows = _golden_rows()
+    xj = np.array([[10.0, -20.0, 5.0]])                       # one j-particle; i-particle k sits at xj - d_k
+    xi = np.array([[10.0 - float(r[0]), -20.0 - float(r[1]), 5.0 - float(r[2])] for r in rows])
+    e2 = np.array([float(r[3]) for r in rows])
+    m = float(rows[0][4])
+    acc, pot = oracle.force_eps_i(xi, e2, xj, np.array([m]))
+    for k, r in enumerate(rows):
+        d, s = r[:3], r[5]
+        exact = [float(Fraction(m) * c / s ** 3) for c in d]
+        np.testing.assert_allclose(acc[k], exact, rtol=1e-14, atol=1e-17)
+        assert pot[k] == pytest.approx(float(-Fraction(m) / s), rel=1e-14)
+
+
+def test_f3_brute_force_random_eps2_per_i():
+    rng = np.random.default_rng(12)
+    x = rng.normal(size=(7, 3)); m = rng.uniform(0.5, 1.5, 7)
+    e2 = np.array([0.0, 1e-4, 0.01, 0.25, 1.0, 0.0, 3.0])
+    acc, pot = oracle.force_eps_i(x, e2, x, m)
+    for i in range(7):
+        ra, rp = _brute_force_mp(x[i:i + 1], x, m, e2[i])
+        np.testing.assert_allclose(acc[i], ra[0], rtol=1e-13, atol=1e-15)
+        np.testing.assert_allclose(pot[i], rp[0], rtol=1e-13)
+    with pytest.raises(ValueError):
+        oracle.force_eps_i(x, -e2 - 1.0, x, m)
