@@ -134,6 +134,21 @@ int nb_force_jerk(int64_t n_i, const float *x_i, const float *v_i,
                   void *stream);
 
 /*
+ * nb_force_eps_i -- nb_force with the softening carried PER i-PARTICLE, as in the paper's own driver, where slot 3
+ * of every i-record is eps2 (Fig. A.1: p_xi[i][3] = eps2; Fig. A.3 PAPER.md:446-450:
+ * eps2 = INPUT_I[3]) -- the first step of the generalised CUNBODY-1 kernel of section 4.5:
+ *
+ *     a_i = sum_j m_j d / (d.d + eps2_i[i])^(3/2),   phi_i = -sum_j m_j / (d.d + eps2_i[i])^(1/2)
+ *
+ *   eps2_i   device, const, float [n_i], every value >= 0 and finite (not validated: device data)
+ * Everything else as for nb_force.  Coincident pairs add nothing whatever eps2_i is (0 included).
+ */
+int nb_force_eps_i(int64_t n_i, const float *x_i, const float *eps2_i,
+                   int64_t n_j, const float *x_j, const float *m_j,
+                   float *acc_out, float *pot_out,
+                   void *stream);
+
+/*
  * nb_force_batched -- many independent small (i-set, j-set) sub-problems of nb_force in ONE launch:
  * the use the paper shapes its interface for, a host tree code calling the force routine on
  * interaction lists of "several thousands" particles per group (PAPER.md:246 last sentence, section

@@ -7,6 +7,7 @@ from .binding import (  # noqa: F401
     NBError,
     force,
     force_batched,
+    force_eps_i,
     force_host,
     force_jerk,
     last_launch_count,

@@ -45,6 +45,8 @@ def lib() -> ctypes.CDLL:
         l.nb_leapfrog_kdk.restype = ci
         l.nb_force_jerk.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p, p]
         l.nb_force_jerk.restype = ci
+        l.nb_force_eps_i.argtypes = [i64, p, p, i64, p, p, p, p, p]
+        l.nb_force_eps_i.restype = ci
         l.nb_force_batched.argtypes = [i64, p, p, i64, p, i64, p, p, f32, p, p, p]
         l.nb_force_batched.restype = ci
         l.nb_plan_query_jerk.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
@@ -131,6 +133,24 @@ def force_jerk(x_i, v_i, x_j, v_j, m_j, eps2: float, acc_out=None, jerk_out=None
                                  None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
     _check(st, "nb_force_jerk")
     return acc_out, jerk_out, pot_out
+
+
+def force_eps_i(x_i, eps2_i, x_j, m_j, acc_out=None, pot_out=None, want_pot: bool = True, stream=None):
+    """nb_force_eps_i on CUDA tensors: one softening (squared) per i-particle."""
+    import torch
+    _dev_f32(x_i, "x_i", (3,)); _dev_f32(eps2_i, "eps2_i", ()); _dev_f32(x_j, "x_j", (3,)); _dev_f32(m_j, "m_j", ())
+    n_i, n_j = x_i.shape[0], x_j.shape[0]
+    if eps2_i.shape[0] != n_i or m_j.shape[0] != n_j:
+        raise ValueError("array lengths differ")
+    if acc_out is None:
+        acc_out = torch.empty((n_i, 3), dtype=torch.float32, device=x_i.device)
+    if pot_out is None and want_pot:
+        pot_out = torch.empty((n_i,), dtype=torch.float32, device=x_i.device)
+    with torch.cuda.device(x_i.device):
+        st = lib().nb_force_eps_i(n_i, x_i.data_ptr(), eps2_i.data_ptr(), n_j, x_j.data_ptr(), m_j.data_ptr(),
+                                  acc_out.data_ptr(), None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_force_eps_i")
+    return acc_out, pot_out
 
 
 def force_batched(i_offsets, j_offsets, x_i, x_j, m_j, eps2: float, acc_out=None, pot_out=None, want_pot: bool = True,

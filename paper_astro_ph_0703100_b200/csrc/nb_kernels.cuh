@@ -155,10 +155,11 @@ __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nx
 }
 
 // One tile: K/2 i-pairs of this thread against np j-particles in shared memory; partial sums start from zero (Eq. (2)).
-template <int K, int MASK>
+// EPS_I (row f3): the softening is a property of the i-particle (Fig. A.1) and sits, packed, in e2[].
+template <int K, int MASK, bool EPS_I = false>
 __device__ __forceinline__ bool tile_sweep(const float4* __restrict__ sp, int np, const u64 (&nxi)[K / 2], const u64 (&nyi)[K / 2],
                                            const u64 (&nzi)[K / 2], u64 eps2_2, float eps2, u64 (&pax)[K / 2], u64 (&pay)[K / 2],
-                                           u64 (&paz)[K / 2], u64 (&pph)[K / 2]) {
+                                           u64 (&paz)[K / 2], u64 (&pph)[K / 2], const u64 (&e2)[K / 2]) {
     bool hit = false;
 #pragma unroll
     for (int k = 0; k < K / 2; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
@@ -168,7 +169,7 @@ __device__ __forceinline__ bool tile_sweep(const float4* __restrict__ sp, int np
         const u64 xj = pack2(J.x, J.x), yj = pack2(J.y, J.y), zj = pack2(J.z, J.z), mj = pack2(J.w, J.w);
 #pragma unroll
         for (int k = 0; k < K / 2; ++k)
-            pair_body<MASK>(xj, yj, zj, mj, nxi[k], nyi[k], nzi[k], eps2_2, eps2, pax[k], pay[k], paz[k], pph[k], hit);
+            pair_body<MASK>(xj, yj, zj, mj, nxi[k], nyi[k], nzi[k], EPS_I ? e2[k] : eps2_2, eps2, pax[k], pay[k], paz[k], pph[k], hit);
     }
     return hit;
 }
@@ -276,6 +277,7 @@ __global__ void __launch_bounds__(256) nb_coin_probe_kernel(const float* __restr
 
 struct ForceArgs {
     const float* x_i;      // [n_i][3]
+    const float* eps2_i;   // EPS_I: [n_i] softening squared of every i-particle
     const float4* jp;      // packed j records (x, y, z, m)
     float* acc;            // [n_i][3]
     float* pot;            // [n_i] or nullptr
@@ -308,9 +310,10 @@ enum { MODE_EXACT = 0,     // masked loop everywhere (eps2 == 0 or tiny)
 // BATCHED (row f2, nb_force_batched): the grid is one row of CTAs; CTA blockIdx.x finds the
 // sub-problem b it belongs to in cta_batch[] (written by nb_batch_scan_kernel) and works on i in
 // [i_off[b], i_off[b+1]) against j in [j_off[b], j_off[b+1]); no split across CTAs (S = 1).
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool BATCHED = false, int SUB = 256>
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool BATCHED = false, bool EPS_I = false, int SUB = 256>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
+    static_assert(!(EPS_I && MODE == MODE_SPEC), "per-i softening: masked or list mode only");
     static_assert(SUB == kCoinSeg, "coincidence segments are SUB j-particles");
     static_assert(!(BATCHED && MODE == MODE_LIST), "no coincidence lists for batched calls");
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -368,6 +371,17 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
     }
     const float eps2 = a.eps2;
     const u64 eps2_2 = pack2(eps2, eps2);
+    u64 e2[K / 2];
+#pragma unroll
+    for (int k2 = 0; k2 < K / 2; ++k2) {
+        if (EPS_I) {
+            const int i0 = min(i_base + (2 * k2) * 32, i_hi - 1);
+            const int i1 = min(i_base + (2 * k2 + 1) * 32, i_hi - 1);
+            e2[k2] = pack2(a.eps2_i[i0], a.eps2_i[i1]);
+        } else {
+            e2[k2] = eps2_2;
+        }
+    }
 
     __syncthreads();                                                   // barriers initialised
 
@@ -406,9 +420,9 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
             const int nc = min(SUB, np - c);
             u64 pax[K / 2], pay[K / 2], paz[K / 2], pph[K / 2];
             if (MODE == MODE_SPEC) {
-                const bool hit = tile_sweep<K, MASK_SPEC>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+                const bool hit = tile_sweep<K, MASK_SPEC, EPS_I>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
                 if (__any_sync(0xffffffffu, hit))                      // rare: some pair of this warp may be coincident
-                    (void)tile_sweep<K, MASK_EXACT>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+                    (void)tile_sweep<K, MASK_EXACT, EPS_I>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
             } else if (MODE == MODE_LIST) {
                 const int j0 = j_begin + t * TJ + c;                   // global index of the block's first j
                 const int seg_lo = j0 >> kCoinSegShift, seg_hi = (j0 + nc - 1) >> kCoinSegShift;
@@ -417,11 +431,11 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
                     coin_next = (coin_pos < coin_cnt) ? coin[1 + coin_pos] : 0x7fffffff;
                 }
                 if (coin_cnt < 0 || coin_next <= seg_hi)               // rare: the block holds a coincident pair
-                    (void)tile_sweep<K, MASK_EXACT>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+                    (void)tile_sweep<K, MASK_EXACT, EPS_I>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
                 else
-                    (void)tile_sweep<K, MASK_NONE>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+                    (void)tile_sweep<K, MASK_NONE, EPS_I>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
             } else {
-                (void)tile_sweep<K, MASK_EXACT>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+                (void)tile_sweep<K, MASK_EXACT, EPS_I>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
             }
             // a5: block partial -> running total
 #pragma unroll

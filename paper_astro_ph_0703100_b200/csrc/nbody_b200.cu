@@ -123,12 +123,12 @@ int pick_mode(int64_t n_i, int64_t n_j, float eps2) {
     return ((double)n_i * (double)n_j >= kListMinPairs) ? nb::MODE_LIST : nb::MODE_SPEC;
 }
 
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE>
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I>
 int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
     constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE>;
+    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, false, EPS_I>;
     static bool configured[64] = {};
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
@@ -154,22 +154,22 @@ int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStrea
 }
 
 // tile_j / stages per WJ must match nb::ring_shape (nb_plan.h)
-template <int K, int MODE>
+template <int K, int MODE, bool EPS_I>
 int launch_force_k(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     switch (plan.WJ) {
-        case 1: return launch_force_inst<K, 8, 1, 512, 4, MODE>(args, plan, stream);
-        case 2: return launch_force_inst<K, 4, 2, 512, 4, MODE>(args, plan, stream);
-        case 4: return launch_force_inst<K, 2, 4, 256, 4, MODE>(args, plan, stream);
-        default: return launch_force_inst<K, 1, 8, 256, 3, MODE>(args, plan, stream);
+        case 1: return launch_force_inst<K, 8, 1, 512, 4, MODE, EPS_I>(args, plan, stream);
+        case 2: return launch_force_inst<K, 4, 2, 512, 4, MODE, EPS_I>(args, plan, stream);
+        case 4: return launch_force_inst<K, 2, 4, 256, 4, MODE, EPS_I>(args, plan, stream);
+        default: return launch_force_inst<K, 1, 8, 256, 3, MODE, EPS_I>(args, plan, stream);
     }
 }
 
-template <int MODE>
+template <int MODE, bool EPS_I = false>
 int launch_force(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     switch (plan.K) {
-        case 2: return launch_force_k<2, MODE>(args, plan, stream);
-        case 4: return launch_force_k<4, MODE>(args, plan, stream);
-        default: return launch_force_k<8, MODE>(args, plan, stream);
+        case 2: return launch_force_k<2, MODE, EPS_I>(args, plan, stream);
+        case 4: return launch_force_k<4, MODE, EPS_I>(args, plan, stream);
+        default: return launch_force_k<8, MODE, EPS_I>(args, plan, stream);
     }
 }
 
@@ -201,10 +201,11 @@ int coin_prepass(Workspace* ws, const nb::Plan& plan, int64_t n_i, const float* 
 }
 
 // pack (a1) when repack is true, then force (+ reduce).  The packed array lives in the workspace.
+// eps2_i != nullptr: row f3, the softening of every i-particle comes from that device array and eps2 is ignored.
 int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
-               float* acc_out, float* pot_out, cudaStream_t stream) {
+               float* acc_out, float* pot_out, cudaStream_t stream, const float* eps2_i = nullptr) {
     if (bad_count(n_i) || bad_count(n_j)) return NB_ERR_INVALID_VALUE;
-    if (!(eps2 >= 0.0f) || !std::isfinite(eps2)) return NB_ERR_INVALID_VALUE;
+    if (!eps2_i && (!(eps2 >= 0.0f) || !std::isfinite(eps2))) return NB_ERR_INVALID_VALUE;
     if (n_i > 0 && (!x_i || !acc_out)) return NB_ERR_INVALID_VALUE;
     if (n_j > 0 && (!x_j || !m_j)) return NB_ERR_INVALID_VALUE;
     int dev = 0;
@@ -241,6 +242,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
 
     nb::ForceArgs args;
     args.x_i = x_i;
+    args.eps2_i = eps2_i;
     args.jp = reinterpret_cast<const float4*>(ws->jp);
     args.acc = acc_out;
     args.pot = pot_out;
@@ -253,12 +255,15 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.coin_flag = nullptr;
     args.i_off = args.j_off = args.tile_start = args.cta_batch = nullptr;
     args.n_batch = 0;
-    const int mode = pick_mode(n_i, n_j, eps2);
+    int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2);
+    if (eps2_i && mode == nb::MODE_SPEC) mode = nb::MODE_EXACT;      // the values are on the device: no threshold test
     if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, reinterpret_cast<const float4*>(ws->jp), 1, stream,
                           &args.coin_lists, &args.coin_flag);
         if (rc != NB_OK) return rc;
-        rc = launch_force<nb::MODE_LIST>(args, plan, stream);
+        rc = eps2_i ? launch_force<nb::MODE_LIST, true>(args, plan, stream) : launch_force<nb::MODE_LIST>(args, plan, stream);
+    } else if (eps2_i) {
+        rc = launch_force<nb::MODE_EXACT, true>(args, plan, stream);
     } else if (mode == nb::MODE_SPEC) {
         rc = launch_force<nb::MODE_SPEC>(args, plan, stream);
     } else {
@@ -514,6 +519,7 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
 
     nb::ForceArgs args;
     args.x_i = x_i;
+    args.eps2_i = nullptr;
     args.jp = reinterpret_cast<const float4*>(ws->jp);
     args.acc = acc_out;
     args.pot = pot_out;
@@ -556,6 +562,15 @@ int nb_force(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const
              float* acc_out, float* pot_out, void* stream) {
     t_launches = 0;
     return force_impl(n_i, x_i, n_j, x_j, m_j, eps2, acc_out, pot_out, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int nb_force_eps_i(int64_t n_i, const float* x_i, const float* eps2_i, int64_t n_j, const float* x_j, const float* m_j,
+                   float* acc_out, float* pot_out, void* stream) {
+    t_launches = 0;
+    if (n_i > 0 && !eps2_i) return NB_ERR_INVALID_VALUE;
+    static const float dummy = 0.0f;
+    return force_impl(n_i, x_i, n_j, x_j, m_j, 0.0f, acc_out, pot_out, reinterpret_cast<cudaStream_t>(stream),
+                      eps2_i ? eps2_i : &dummy);
 }
 
 int nb_force_host(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
