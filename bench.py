@@ -206,8 +206,13 @@ class Problem:
     def __init__(self, op, cfg_name, nb, torch, wl):
         self.op, self.nb, self.torch = op, nb, torch
         if op == "force":
-            w = wl.config(CONFIG_INDEX[cfg_name])
-            self.w, self.pairs, self.name = w, float(w.pairs), workload_name(cfg_name, w)
+            if isinstance(cfg_name, int):
+                w = wl.plummer_workload(cfg_name, 1.0 / 256, seed=1, name=f"plummer{cfg_name}")
+                name = f"N-scan: {w.meta.get('model', '')}, n_i=n_j={cfg_name}, eps2={w.eps2:.6g}, seed=1, one nb_force call with phi"
+            else:
+                w = wl.config(CONFIG_INDEX[cfg_name])
+                name = workload_name(cfg_name, w)
+            self.w, self.pairs, self.name = w, float(w.pairs), name
             self.host = [w.x_j, w.m_j] + ([] if w.x_i is None else [w.x_i])
             self.n_out = w.n_i
         elif op == "jerk":
@@ -315,6 +320,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
     ap.add_argument("--op", default="force", choices=sorted(OPS))
+    ap.add_argument("--n", type=int, default=0, help="--op force only: an equal-mass Plummer sphere of this N "
+                    "(eps = 1/256, seed 1) instead of a BASELINE.json config; for the N-scan in profiles/")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -345,7 +352,7 @@ def main():
     op = OPS[args.op]
 
     # inputs resident in HBM before the timed region
-    prob = Problem(args.op, args.config, nb, torch, wl)
+    prob = Problem(args.op, args.n if (args.n > 0 and args.op == "force") else args.config, nb, torch, wl)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
 
@@ -403,7 +410,8 @@ def main():
         k_rate = pairs * n_k / (k_ms * 1e-3) if n_k else 0.0
         inst = op["inst"]
         achieved = inst * k_rate
-        traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if args.op == "force" else NCU_DRAM_BYTES_PER_LAUNCH.get(args.op)
+        traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(args.op) if args.op != "force" else (
+            None if args.n > 0 else NCU_DRAM_BYTES_PER_LAUNCH.get(args.config))
         roofline = {
             "bound": "alu", "kernel": op["kernel"],
             "achieved": achieved / 1e12, "peak": peak_inst / 1e12, "unit": "FP32-pipe Tinst/s",

@@ -282,6 +282,7 @@ struct ForceArgs {
     float* acc;            // [n_i][3]
     float* pot;            // [n_i] or nullptr
     double4* partial;      // [S][n_i] when S > 1
+    int* tickets;          // [tiles_i] zero between calls; non-null => the last CTA of an i-tile sums the partials
     const int* coin_lists; // MODE_LIST: [n_groups][1 + kCoinCap]
     const int* coin_flag;  // MODE_LIST: != 0 -> mask everywhere
     const int* i_off;      // BATCHED: [n_batch + 1] first i of every sub-problem
@@ -476,30 +477,69 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
 #pragma unroll
             for (int c = 0; c < 4; ++c) red[((wj * K + k) * 4 + c) * (WI * 32) + tig] = run[k][c];
         __syncthreads();
-        if (wj != 0) return;
+        if (wj == 0) {
 #pragma unroll
-        for (int k = 0; k < K; ++k)
+            for (int k = 0; k < K; ++k)
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                double s = red[((0 * K + k) * 4 + c) * (WI * 32) + tig];
+                for (int c = 0; c < 4; ++c) {
+                    double s = red[((0 * K + k) * 4 + c) * (WI * 32) + tig];
 #pragma unroll
-                for (int w = 1; w < WJ; ++w) s += red[((w * K + k) * 4 + c) * (WI * 32) + tig];
-                run[k][c] = s;
-            }
+                    for (int w = 1; w < WJ; ++w) s += red[((w * K + k) * 4 + c) * (WI * 32) + tig];
+                    run[k][c] = s;
+                }
+        }
     }
 
     // a6: epilogue
+    if (wj == 0) {
 #pragma unroll
-    for (int k = 0; k < K; ++k) {
-        const int i = i_base + k * 32;
-        if (i >= i_hi) continue;
-        if (a.S == 1) {
-            a.acc[3 * i + 0] = (float)run[k][0];
-            a.acc[3 * i + 1] = (float)run[k][1];
-            a.acc[3 * i + 2] = (float)run[k][2];
-            if (a.pot) a.pot[i] = -(float)run[k][3];
-        } else {
-            a.partial[(size_t)blockIdx.y * a.n_i + i] = make_double4(run[k][0], run[k][1], run[k][2], run[k][3]);
+        for (int k = 0; k < K; ++k) {
+            const int i = i_base + k * 32;
+            if (i >= i_hi) continue;
+            if (a.S == 1) {
+                a.acc[3 * i + 0] = (float)run[k][0];
+                a.acc[3 * i + 1] = (float)run[k][1];
+                a.acc[3 * i + 2] = (float)run[k][2];
+                if (a.pot) a.pot[i] = -(float)run[k][3];
+            } else {
+                a.partial[(size_t)blockIdx.y * a.n_i + i] = make_double4(run[k][0], run[k][1], run[k][2], run[k][3]);
+            }
+        }
+    }
+    if (BATCHED) return;
+
+    // a7 (inter-CTA), fused: the CTA that finishes LAST among the S chunks of this i-tile sums the S partials in the
+    // fixed order s = 0 .. S-1 (so the result does not depend on which CTA that is) and writes a and phi.  The
+    // ticket counter of the tile returns to zero for the next call.  (nb_reduce_kernel is the same sum as a separate
+    // launch; it is kept for the NB_FUSED_REDUCE=0 comparison.)
+    if (a.S > 1 && a.tickets != nullptr) {
+        __shared__ int s_last;
+        __threadfence();                                               // partials visible device-wide before the ticket
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const int ticket = atomicAdd(a.tickets + blockIdx.x, 1);
+            s_last = (ticket == a.S - 1);
+            if (s_last) a.tickets[blockIdx.x] = 0;
+        }
+        __syncthreads();
+        if (!s_last) return;
+        __threadfence();
+        const int tile0 = blockIdx.x * (32 * K * WI);
+        const int tile_n = min(32 * K * WI, a.n_i - tile0);
+        for (int q = threadIdx.x; q < tile_n; q += 32 * WI * WJ) {
+            const int i = tile0 + q;
+            const double2* p2 = reinterpret_cast<const double2*>(a.partial + i);          // L2 reads (other SMs wrote these)
+            double2 lo = __ldcg(p2), hi = __ldcg(p2 + 1);
+            double4 sum = make_double4(lo.x, lo.y, hi.x, hi.y);
+            for (int c = 1; c < a.S; ++c) {
+                p2 = reinterpret_cast<const double2*>(a.partial + (size_t)c * a.n_i + i);
+                lo = __ldcg(p2); hi = __ldcg(p2 + 1);
+                sum.x += lo.x; sum.y += lo.y; sum.z += hi.x; sum.w += hi.y;
+            }
+            a.acc[3 * i + 0] = (float)sum.x;
+            a.acc[3 * i + 1] = (float)sum.y;
+            a.acc[3 * i + 2] = (float)sum.z;
+            if (a.pot) a.pot[i] = -(float)sum.w;
         }
     }
 }

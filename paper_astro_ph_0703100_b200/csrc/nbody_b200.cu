@@ -46,6 +46,7 @@ struct Workspace {
     void* jp = nullptr;        size_t jp_bytes = 0;        // packed pair records
     void* partial = nullptr;   size_t partial_bytes = 0;   // [S][n_i] double4
     void* stage = nullptr;     size_t stage_bytes = 0;     // device copies for nb_force_host
+    void* tickets = nullptr;   size_t tickets_bytes = 0;   // fused second pass: one counter per i-tile, zero between calls
     void* coin = nullptr;      size_t coin_bytes = 0;      // coincidence pre-pass: flag | lists | hash table
     void* tiles = nullptr;     size_t tiles_bytes = 0;     // batched calls: first CTA of every sub-problem
     void* jp2 = nullptr;       size_t jp2_bytes = 0;       // force + jerk: 32-byte j records
@@ -113,14 +114,20 @@ constexpr float kSpecMinEps2 = 9.094947017729282e-13f;
 // (MODE_LIST: three extra O(n) launches, no test in the hot loop); smaller ones use MODE_SPEC.
 constexpr double kListMinPairs = 1073741824.0;   // 2^30
 
-int pick_mode(int64_t n_i, int64_t n_j, float eps2) {
+// Small calls: the speculative mode pays a masked redo of a whole 256-j block per warp that meets a coincident
+// pair.  When the i-set IS the j-set (same pointer) those pairs sit on the diagonal and few warps meet one; when
+// the i-set is a separate array it is, in practice, an active subset of the j-set (block time steps, BASELINE.json
+// configs[2]) whose partners are scattered over all j, nearly every warp would redo its block (measured on C2:
+// 39 us speculative, 27 us masked), so separate sets mask every pair.
+int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool aliased) {
     // debugging aid: NB_MASK=exact|spec|list forces a mode (spec/list still need eps2 >= 2^-40)
     const char* e = std::getenv("NB_MASK");
     if (e && e[0] == 'e') return nb::MODE_EXACT;
     if (eps2 < kSpecMinEps2) return nb::MODE_EXACT;
     if (e && e[0] == 's') return nb::MODE_SPEC;
     if (e && e[0] == 'l') return nb::MODE_LIST;
-    return ((double)n_i * (double)n_j >= kListMinPairs) ? nb::MODE_LIST : nb::MODE_SPEC;
+    if ((double)n_i * (double)n_j >= kListMinPairs) return nb::MODE_LIST;
+    return aliased ? nb::MODE_SPEC : nb::MODE_EXACT;
 }
 
 template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I>
@@ -227,9 +234,19 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     }
     rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)n_j * sizeof(float4), stream);
     if (rc != NB_OK) return rc;
+    // Second pass over the S chunk partials: small (latency-bound) calls fuse it into the force kernel -- the last
+    // CTA of an i-tile does it, one launch fewer: C0 31 -> 28 us, C2 65 -> 56 us; large calls launch nb_reduce_kernel
+    // (the fused tail costs 0.2 % on C1).  NB_FUSED_REDUCE=0/1 forces either.
+    const char* fr = std::getenv("NB_FUSED_REDUCE");
+    const bool fused_reduce = fr ? (fr[0] != '0') : ((double)n_i * (double)n_j < kListMinPairs);
     if (plan.S > 1) {
         rc = ensure(&ws->partial, &ws->partial_bytes, (size_t)plan.S * (size_t)n_i * sizeof(double4), stream);
         if (rc != NB_OK) return rc;
+        if (fused_reduce && (size_t)plan.tiles_i * sizeof(int) > ws->tickets_bytes) {
+            rc = ensure(&ws->tickets, &ws->tickets_bytes, (size_t)plan.tiles_i * sizeof(int), stream);
+            if (rc != NB_OK) return rc;
+            NB_CUDA(cudaMemsetAsync(ws->tickets, 0, ws->tickets_bytes, stream));   // once per growth; kernels leave zeros
+        }
     }
 
     {   // a1: j-pack
@@ -247,6 +264,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.acc = acc_out;
     args.pot = pot_out;
     args.partial = reinterpret_cast<double4*>(ws->partial);
+    args.tickets = (plan.S > 1 && fused_reduce) ? reinterpret_cast<int*>(ws->tickets) : nullptr;
     args.n_i = (int)n_i;
     args.n_j = (int)n_j;
     args.S = plan.S;
@@ -255,7 +273,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.coin_flag = nullptr;
     args.i_off = args.j_off = args.tile_start = args.cta_batch = nullptr;
     args.n_batch = 0;
-    int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2);
+    int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2, x_i == x_j);
     if (eps2_i && mode == nb::MODE_SPEC) mode = nb::MODE_EXACT;      // the values are on the device: no threshold test
     if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, reinterpret_cast<const float4*>(ws->jp), 1, stream,
@@ -271,7 +289,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     }
     if (rc != NB_OK) return rc;
 
-    if (plan.S > 1) {
+    if (plan.S > 1 && !fused_reduce) {
         const int threads = 128;
         const int blocks = (int)((n_i + threads - 1) / threads);
         nb::nb_reduce_kernel<<<blocks, threads, 0, stream>>>(reinterpret_cast<const double4*>(ws->partial), (int)n_i,
@@ -398,7 +416,7 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     args.S = plan.S;
     args.eps2 = eps2;
     // the jerk has no speculative mode: small calls mask every pair, large ones use the coincidence lists
-    int mode = pick_mode(n_i, n_j, eps2);
+    int mode = pick_mode(n_i, n_j, eps2, x_i == x_j);
     if (mode == nb::MODE_SPEC) mode = nb::MODE_EXACT;
     if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, args.jp, 2, stream, &args.coin_lists, &args.coin_flag);
@@ -524,6 +542,7 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     args.acc = acc_out;
     args.pot = pot_out;
     args.partial = nullptr;
+    args.tickets = nullptr;
     args.coin_lists = nullptr;
     args.coin_flag = nullptr;
     args.i_off = i_offsets;
@@ -710,6 +729,7 @@ int nb_release_workspace(void) {
             if (it->second.partial) (void)cudaFree(it->second.partial);
             if (it->second.stage) (void)cudaFree(it->second.stage);
             if (it->second.coin) (void)cudaFree(it->second.coin);
+            if (it->second.tickets) (void)cudaFree(it->second.tickets);
             if (it->second.jp2) (void)cudaFree(it->second.jp2);
             if (it->second.tiles) (void)cudaFree(it->second.tiles);
             if (it->second.hpartial) (void)cudaFree(it->second.hpartial);
