@@ -531,7 +531,8 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
             const double2* p2 = reinterpret_cast<const double2*>(a.partial + i);          // L2 reads (other SMs wrote these)
             double2 lo = __ldcg(p2), hi = __ldcg(p2 + 1);
             double4 sum = make_double4(lo.x, lo.y, hi.x, hi.y);
-            for (int c = 1; c < a.S; ++c) {
+#pragma unroll 8
+            for (int c = 1; c < a.S; ++c) {                            // loads run ahead, the adds keep the order s = 0 .. S-1
                 p2 = reinterpret_cast<const double2*>(a.partial + (size_t)c * a.n_i + i);
                 lo = __ldcg(p2); hi = __ldcg(p2 + 1);
                 sum.x += lo.x; sum.y += lo.y; sum.z += hi.x; sum.w += hi.y;
@@ -591,7 +592,8 @@ __global__ void __launch_bounds__(128) nb_reduce_kernel(const double4* __restric
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_i) return;
     double4 s = partial[i];
-    for (int c = 1; c < S; ++c) {
+#pragma unroll 8
+    for (int c = 1; c < S; ++c) {                                      // loads run ahead, the adds keep the order
         const double4 v = partial[(size_t)c * n_i + i];
         s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
     }

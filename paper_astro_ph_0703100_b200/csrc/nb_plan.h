@@ -18,6 +18,11 @@ namespace nb {
 
 constexpr int kWarpsPerCta = 8;        // every force CTA has 8 warps = WI * WJ
 constexpr int kMaxS = 2048;
+// Second pass over the S chunk partials of an i-tile: done inside the force kernel by the tile's last CTA when
+// the tile's partials are small (one launch fewer: C0 31 -> 24 us, C2 65 -> 38 us per call), else by a separate
+// nb_reduce_kernel launch (a 2048-particle tile with S = 18..30 would keep one CTA busy for ~10 us at the tail).
+constexpr int64_t kFusedReduceBytes = 1048576;
+inline bool fused_second_pass(int tile_i, int S) { return S > 1 && (int64_t)tile_i * S * 32 <= kFusedReduceBytes; }
 
 struct Plan {
     int K;            // i-particles per thread (2, 4 or 8; held as K/2 packed pairs)
@@ -60,7 +65,14 @@ inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, i
     double cta_cycles = c_fixed + double(tile_i) * j_per_cta * pair_cycles * k_pen * wj_pen;
     if (WJ > 1) cta_cycles += 1500.0;                 // cross-warp reduction through shared memory
     double cost = waves * cta_cycles;
-    if (S > 1) cost += c_reduce_launch + double(n_i) * S * partial_bytes / 2500.0;  // ~5 TB/s at ~2 GHz
+    if (S > 1) {
+        if (fused_second_pass(tile_i, S))
+            cost += 1500.0 + 200.0 * S;               // the last CTA of a tile walks S partials
+        else {                                        // separate launch: ~5 TB/s at ~2 GHz, or the latency of S loads in a row
+            const double bw = double(n_i) * S * partial_bytes / 2500.0, lat = 200.0 * S;
+            cost += c_reduce_launch + (bw > lat ? bw : lat);
+        }
+    }
     return cost;
 }
 

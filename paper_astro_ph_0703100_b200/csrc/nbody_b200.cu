@@ -234,11 +234,9 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     }
     rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)n_j * sizeof(float4), stream);
     if (rc != NB_OK) return rc;
-    // Second pass over the S chunk partials: small (latency-bound) calls fuse it into the force kernel -- the last
-    // CTA of an i-tile does it, one launch fewer: C0 31 -> 28 us, C2 65 -> 56 us; large calls launch nb_reduce_kernel
-    // (the fused tail costs 0.2 % on C1).  NB_FUSED_REDUCE=0/1 forces either.
+    // second pass: fused into the force kernel or a separate launch (nb_plan.h: fused_second_pass); NB_FUSED_REDUCE=0/1 forces
     const char* fr = std::getenv("NB_FUSED_REDUCE");
-    const bool fused_reduce = fr ? (fr[0] != '0') : ((double)n_i * (double)n_j < kListMinPairs);
+    const bool fused_reduce = fr ? (fr[0] != '0') : nb::fused_second_pass(plan.tile_i, plan.S);
     if (plan.S > 1) {
         rc = ensure(&ws->partial, &ws->partial_bytes, (size_t)plan.S * (size_t)n_i * sizeof(double4), stream);
         if (rc != NB_OK) return rc;
