@@ -157,6 +157,9 @@ def reference_arm(args, wl):
     elif args.op == "jerk":
         w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
         name = "row f1 (H1): plummer N=131072 with velocities, one force+jerk+phi evaluation"
+    elif args.op == "leapfrog":
+        w = wl.config(4)
+        name = "BASELINE.json configs[4] (C4): force evaluations of the KDK integration, N=65536 (oracle force on a sample)"
     else:
         w = wl.tree_list_workload(524288, 32, 256, 2000, 6000, 1.0 / 128, seed=7, name="T1")
         name = "row f2 (T1): tree lists, 524288 particles, groups 32..256, lists 2000..6000"
@@ -197,7 +200,11 @@ OPS = {
     "force": {"inst": 13, "kernel": "nb_force_kernel (pair interaction, rows a2-a7)", "flops": (20, 38)},
     "jerk": {"inst": 27, "kernel": "nb_hermite_kernel (force + jerk + potential, row f1)", "flops": (60, 60)},
     "batched": {"inst": 13, "kernel": "nb_force_kernel<BATCHED> (row f2)", "flops": (20, 38)},
+    # BASELINE.json configs[4]: one bench "step" = one nb_leapfrog_kdk call of LEAPFROG_KDK_PER_CALL KDK steps that
+    # continues the integration (the first call also pays the initial force evaluation)
+    "leapfrog": {"inst": 13, "kernel": "nb_force_kernel inside nb_leapfrog_kdk (row a8)", "flops": (20, 38)},
 }
+LEAPFROG_KDK_PER_CALL = 100
 
 
 class Problem:
@@ -215,6 +222,16 @@ class Problem:
             self.w, self.pairs, self.name = w, float(w.pairs), name
             self.host = [w.x_j, w.m_j] + ([] if w.x_i is None else [w.x_i])
             self.n_out = w.n_i
+        elif op == "leapfrog":
+            w = wl.config(4)
+            self.w = w
+            self.pairs = float(w.n_j) ** 2 * (LEAPFROG_KDK_PER_CALL + 1)     # force evaluations per call x N^2
+            self.name = (f"BASELINE.json configs[4] (C4): {w.meta.get('model', '')} with Aarseth velocities, N={w.n_j}, "
+                         f"eps2={w.eps2:.6g}, dt=1/512, seed=4; one step = one nb_leapfrog_kdk call of "
+                         f"{LEAPFROG_KDK_PER_CALL} KDK steps (the config's 1000 steps = 10 such calls)")
+            self.host = [w.x_j, w.v, w.m_j]
+            self.n_out = w.n_j
+            self.kdk_done = 0
         elif op == "jerk":
             w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
             self.w, self.pairs = w, float(w.n_i) * float(w.n_j)
@@ -247,6 +264,10 @@ class Problem:
             xj, mj = t[0], t[1]
             xi = xj if w.x_i is None else t[2]
             nb.force(xi, xj, mj, w.eps2, acc_out=self.outs[0], pot_out=self.outs[1])
+        elif self.op == "leapfrog":
+            nb.leapfrog_kdk(t[0], t[1], t[2], w.eps2, w.dt, LEAPFROG_KDK_PER_CALL, acc_io=self.outs[0], pot_out=self.outs[1])
+            if t is self.dev:
+                self.kdk_done += LEAPFROG_KDK_PER_CALL
         elif self.op == "jerk":
             nb.force_jerk(t[0], t[1], t[0], t[1], t[2], w.eps2, acc_out=self.outs[0], jerk_out=self.outs[1], pot_out=self.outs[2])
         else:
@@ -270,11 +291,15 @@ class Problem:
     def e2e_api(self):
         if self.op == "force":
             return "nb_force_host (pinned host buffers)"
+        if self.op == "leapfrog":
+            return "pinned host (x, v, m) -> cudaMemcpyAsync -> nb_leapfrog_kdk (100 KDK steps) -> cudaMemcpyAsync of a, phi -> pinned host"
         return f"pinned host tensors -> cudaMemcpyAsync -> nb_{'force_jerk' if self.op == 'jerk' else 'force_batched'} -> cudaMemcpyAsync -> pinned host"
 
     def plan(self, sm_count):
         if self.op == "force":
             return self.nb.plan_query(self.w.n_i, self.w.n_j, sm_count)
+        if self.op == "leapfrog":
+            return self.nb.plan_query(self.w.n_j, self.w.n_j, sm_count)
         if self.op == "jerk":
             return self.nb.plan_query_jerk(self.w.n_i, self.w.n_j, sm_count)
         return {"cta": "one row of CTAs, 8 warps split each list (WJ = 8), no split across CTAs"}
@@ -283,7 +308,7 @@ class Problem:
 def oracle_rate_op(op, w, target_seconds, rng_seed=0):
     """CPU oracle, as it stands, on a bounded sample of the op's workload: (pairs/s, cores, sample)."""
     import oracle
-    if op == "force":
+    if op in ("force", "leapfrog"):
         return oracle_rate(w, target_seconds, rng_seed)
     cores = oracle.num_threads()
     rng = np.random.default_rng(rng_seed)
@@ -407,7 +432,9 @@ def main():
         f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
         sm_count = torch.cuda.get_device_properties(0).multi_processor_count
         peak_inst = sm_count * FP32_LANES_PER_SM_CLK * f_max                 # FP32-pipe lane-instructions / s
-        k_rate = pairs * n_k / (k_ms * 1e-3) if n_k else 0.0
+        # interactions per launch of the dominant kernel (a leapfrog call launches it once per force evaluation)
+        pairs_k = float(prob.w.n_j) ** 2 if args.op == "leapfrog" else pairs
+        k_rate = pairs_k * n_k / (k_ms * 1e-3) if n_k else 0.0
         inst = op["inst"]
         achieved = inst * k_rate
         traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(args.op) if args.op != "force" else (
@@ -444,6 +471,17 @@ def main():
                               "gflops_force_jerk_8800gtx_n131072": 179,
                               "note": "PAPER.md:314 (includes PCIe copies) and PAPER.md:343; context, not target"},
         }
+        if args.op == "leapfrog":
+            out["kdk_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
+            if not args.no_cpu_baseline:
+                # BASELINE.json configs[4]: relative total-energy drift against oracle-force energies (double) evaluated
+                # on the GPU's own FP32 state: initial conditions vs the state after every warm-up + timed KDK step
+                import oracle
+                w = prob.w
+                _, _, e_start = oracle.energy(w.x_j, w.v, w.m_j, w.eps2)
+                _, _, e_end = oracle.energy(prob.dev[0].cpu().numpy(), prob.dev[1].cpu().numpy(), w.m_j, w.eps2)
+                out["energy"] = {"kdk_steps": prob.kdk_done, "E_start": e_start, "E_end": e_end,
+                                 "rel_drift": abs(e_end - e_start) / abs(e_start), "by": "oracle.energy (FP64) on the GPU's FP32 (x, v)"}
         if not args.no_cpu_baseline:
             v, cores, sample = oracle_rate_op(args.op, prob.w, args.cpu_seconds)
             out["cpu_baseline"] = {"value": v, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample}
