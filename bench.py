@@ -347,6 +347,9 @@ def main():
     ap.add_argument("--op", default="force", choices=sorted(OPS))
     ap.add_argument("--n", type=int, default=0, help="--op force only: an equal-mass Plummer sphere of this N "
                     "(eps = 1/256, seed 1) instead of a BASELINE.json config; for the N-scan in profiles/")
+    ap.add_argument("--shard", action="store_true", help="--op force only: i-shard ONE problem over the ranks (row f4: "
+                    "all-gather of the packed j records over NCCL, then nb_force_packed on the local i-slice; strong "
+                    "scaling) instead of N independent replicas")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -380,6 +383,21 @@ def main():
     prob = Problem(args.op, args.n if (args.n > 0 and args.op == "force") else args.config, nb, torch, wl)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
+    if args.shard:
+        if args.op != "force" or prob.w.x_i is not None:
+            raise SystemExit("--shard needs --op force on a config whose i-set is its j-set (C0, C1, C3, --n)")
+        from paper_astro_ph_0703100_b200 import sharded
+        n_all = prob.w.n_j
+        lo, hi = sharded.shard_range(n_all, rank, world)
+        x_loc, m_loc = prob.dev[0][lo:hi].contiguous(), prob.dev[1][lo:hi].contiguous()
+        acc_loc, pot_loc = prob.outs[0][lo:hi], prob.outs[1][lo:hi]
+
+        def sharded_call(t=None):
+            xm_all = sharded.gather_packed(x_loc, m_loc, n_all)          # the one exchange step: 16 B x N over NCCL
+            nb.force_packed(x_loc, xm_all, prob.w.eps2, acc_out=acc_loc, pot_out=pot_loc)
+        prob.call = sharded_call
+        prob.call_e2e = sharded_call                                     # no host leg in the sharded mode
+        prob.pairs = float(n_all) * float(n_all) / world                 # per rank; replica_throughput multiplies by world
 
     def barrier():
         if world > 1:
@@ -433,7 +451,7 @@ def main():
         sm_count = torch.cuda.get_device_properties(0).multi_processor_count
         peak_inst = sm_count * FP32_LANES_PER_SM_CLK * f_max                 # FP32-pipe lane-instructions / s
         # interactions per launch of the dominant kernel (a leapfrog call launches it once per force evaluation)
-        pairs_k = float(prob.w.n_j) ** 2 if args.op == "leapfrog" else pairs
+        pairs_k = float(prob.w.n_j) ** 2 if args.op == "leapfrog" else pairs   # (sharded: this rank's slice x all j)
         k_rate = pairs_k * n_k / (k_ms * 1e-3) if n_k else 0.0
         inst = op["inst"]
         achieved = inst * k_rate
@@ -455,9 +473,10 @@ def main():
         out = {
             "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "scaling": "strong" if args.shard else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": prob.name, "op": args.op,
-                       "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "parallelism": (f"i-sharded over {world} rank(s): all-gather of packed j + nb_force_packed" if args.shard
+                                       else ("replicas only" if world > 1 else "1 gpu")),
                        "l2": f"flushed between timed iterations ({L2_FLUSH_BYTES >> 20} MiB write, outside the events)",
                        "plan": prob.plan(sm_count)},
             f"gflops_{f_lo}": f_lo * 1e-9 * value, f"gflops_{f_hi}": f_hi * 1e-9 * value,

@@ -134,6 +134,24 @@ int nb_force_jerk(int64_t n_i, const float *x_i, const float *v_i,
                   void *stream);
 
 /*
+ * nb_force_packed -- nb_force for a caller that already holds the j-particles as packed 16-byte records
+ * (x, y, z, m): the paper's own internal layout, p_xj[j][0..3] = (x, y, z, m) (Fig. A.1), so the
+ * packing pass (row a1) is skipped.  This is the entry the multi-GPU i-sharding uses: every rank all-gathers the
+ * packed records of all ranks' particles and evaluates its own i-slice against them.
+ *
+ *   xm_j   device, const, float [n_j][4] = (x, y, z, m) per j-particle, 16-byte aligned
+ * Everything else as for nb_force.  A record with m = 0 adds nothing (padding of a ragged shard).
+ */
+/* nb_pack_j -- row a1 on its own: (x, y, z) || m -> xm_out [n_j][4], device, 16-byte aligned (Fig. A.1). */
+int nb_pack_j(int64_t n_j, const float *x_j, const float *m_j, float *xm_out, void *stream);
+
+int nb_force_packed(int64_t n_i, const float *x_i,
+                    int64_t n_j, const float *xm_j,
+                    float eps2,
+                    float *acc_out, float *pot_out,
+                    void *stream);
+
+/*
  * nb_force_eps_i -- nb_force with the softening carried PER i-PARTICLE, as in the paper's own driver, where slot 3
  * of every i-record is eps2 (Fig. A.1: p_xi[i][3] = eps2; Fig. A.3 PAPER.md:446-450:
  * eps2 = INPUT_I[3]) -- the first step of the generalised CUNBODY-1 kernel of section 4.5:

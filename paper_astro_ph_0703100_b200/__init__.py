@@ -10,8 +10,10 @@ from .binding import (  # noqa: F401
     force_eps_i,
     force_host,
     force_jerk,
+    force_packed,
     last_launch_count,
     leapfrog_kdk,
+    pack_j,
     lib,
     plan_query,
     plan_query_jerk,

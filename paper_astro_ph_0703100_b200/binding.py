@@ -45,6 +45,10 @@ def lib() -> ctypes.CDLL:
         l.nb_leapfrog_kdk.restype = ci
         l.nb_force_jerk.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p, p]
         l.nb_force_jerk.restype = ci
+        l.nb_pack_j.argtypes = [i64, p, p, p, p]
+        l.nb_pack_j.restype = ci
+        l.nb_force_packed.argtypes = [i64, p, i64, p, f32, p, p, p]
+        l.nb_force_packed.restype = ci
         l.nb_force_eps_i.argtypes = [i64, p, p, i64, p, p, p, p, p]
         l.nb_force_eps_i.restype = ci
         l.nb_force_batched.argtypes = [i64, p, p, i64, p, i64, p, p, f32, p, p, p]
@@ -133,6 +137,35 @@ def force_jerk(x_i, v_i, x_j, v_j, m_j, eps2: float, acc_out=None, jerk_out=None
                                  None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
     _check(st, "nb_force_jerk")
     return acc_out, jerk_out, pot_out
+
+
+def pack_j(x_j, m_j, xm_out, stream=None):
+    """nb_pack_j: writes (x, y, z, m) records of x_j / m_j into the first n_j rows of xm_out [>= n_j, 4]."""
+    _dev_f32(x_j, "x_j", (3,)); _dev_f32(m_j, "m_j", ()); _dev_f32(xm_out, "xm_out", (4,))
+    n_j = x_j.shape[0]
+    if m_j.shape[0] != n_j or xm_out.shape[0] < n_j:
+        raise ValueError("array lengths differ")
+    import torch
+    with torch.cuda.device(x_j.device):
+        st = lib().nb_pack_j(n_j, x_j.data_ptr(), m_j.data_ptr(), xm_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_pack_j")
+    return xm_out
+
+
+def force_packed(x_i, xm_j, eps2: float, acc_out=None, pot_out=None, want_pot: bool = True, stream=None):
+    """nb_force_packed on CUDA tensors: xm_j is [n_j, 4] = (x, y, z, m) per j-particle."""
+    import torch
+    _dev_f32(x_i, "x_i", (3,)); _dev_f32(xm_j, "xm_j", (4,))
+    n_i, n_j = x_i.shape[0], xm_j.shape[0]
+    if acc_out is None:
+        acc_out = torch.empty((n_i, 3), dtype=torch.float32, device=x_i.device)
+    if pot_out is None and want_pot:
+        pot_out = torch.empty((n_i,), dtype=torch.float32, device=x_i.device)
+    with torch.cuda.device(x_i.device):
+        st = lib().nb_force_packed(n_i, x_i.data_ptr(), n_j, xm_j.data_ptr(), float(eps2), acc_out.data_ptr(),
+                                   None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_force_packed")
+    return acc_out, pot_out
 
 
 def force_eps_i(x_i, eps2_i, x_j, m_j, acc_out=None, pot_out=None, want_pot: bool = True, stream=None):

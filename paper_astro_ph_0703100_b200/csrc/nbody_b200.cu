@@ -210,11 +210,14 @@ int coin_prepass(Workspace* ws, const nb::Plan& plan, int64_t n_i, const float* 
 // pack (a1) when repack is true, then force (+ reduce).  The packed array lives in the workspace.
 // eps2_i != nullptr: row f3, the softening of every i-particle comes from that device array and eps2 is ignored.
 int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
-               float* acc_out, float* pot_out, cudaStream_t stream, const float* eps2_i = nullptr) {
+               float* acc_out, float* pot_out, cudaStream_t stream, const float* eps2_i = nullptr,
+               const float4* packed_j = nullptr) {
+    // packed_j != nullptr: the caller already holds the 16-byte (x, y, z, m) records (nb_force_packed); x_j, m_j unused
     if (bad_count(n_i) || bad_count(n_j)) return NB_ERR_INVALID_VALUE;
     if (!eps2_i && (!(eps2 >= 0.0f) || !std::isfinite(eps2))) return NB_ERR_INVALID_VALUE;
     if (n_i > 0 && (!x_i || !acc_out)) return NB_ERR_INVALID_VALUE;
-    if (n_j > 0 && (!x_j || !m_j)) return NB_ERR_INVALID_VALUE;
+    if (n_j > 0 && !packed_j && (!x_j || !m_j)) return NB_ERR_INVALID_VALUE;
+    if (packed_j && (reinterpret_cast<uintptr_t>(packed_j) & 15u)) return NB_ERR_INVALID_VALUE;
     int dev = 0;
     DeviceInfo info;
     int rc = device_info(&dev, &info);
@@ -247,7 +250,8 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         }
     }
 
-    {   // a1: j-pack
+    const float4* jp = packed_j ? packed_j : reinterpret_cast<const float4*>(ws->jp);
+    if (!packed_j) {   // a1: j-pack
         const int threads = 256;
         const int blocks = (int)((n_j + threads - 1) / threads);
         nb::nb_pack_j_kernel<<<blocks, threads, 0, stream>>>(x_j, m_j, (int)n_j, reinterpret_cast<float4*>(ws->jp));
@@ -258,7 +262,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     nb::ForceArgs args;
     args.x_i = x_i;
     args.eps2_i = eps2_i;
-    args.jp = reinterpret_cast<const float4*>(ws->jp);
+    args.jp = jp;
     args.acc = acc_out;
     args.pot = pot_out;
     args.partial = reinterpret_cast<double4*>(ws->partial);
@@ -271,11 +275,10 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.coin_flag = nullptr;
     args.i_off = args.j_off = args.tile_start = args.cta_batch = nullptr;
     args.n_batch = 0;
-    int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2, x_i == x_j);
+    int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2, !packed_j && x_i == x_j);
     if (eps2_i && mode == nb::MODE_SPEC) mode = nb::MODE_EXACT;      // the values are on the device: no threshold test
     if (mode == nb::MODE_LIST) {
-        rc = coin_prepass(ws, plan, n_i, x_i, n_j, reinterpret_cast<const float4*>(ws->jp), 1, stream,
-                          &args.coin_lists, &args.coin_flag);
+        rc = coin_prepass(ws, plan, n_i, x_i, n_j, jp, 1, stream, &args.coin_lists, &args.coin_flag);
         if (rc != NB_OK) return rc;
         rc = eps2_i ? launch_force<nb::MODE_LIST, true>(args, plan, stream) : launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (eps2_i) {
@@ -588,6 +591,32 @@ int nb_force_eps_i(int64_t n_i, const float* x_i, const float* eps2_i, int64_t n
     static const float dummy = 0.0f;
     return force_impl(n_i, x_i, n_j, x_j, m_j, 0.0f, acc_out, pot_out, reinterpret_cast<cudaStream_t>(stream),
                       eps2_i ? eps2_i : &dummy);
+}
+
+int nb_pack_j(int64_t n_j, const float* x_j, const float* m_j, float* xm_out, void* stream) {
+    t_launches = 0;
+    if (bad_count(n_j)) return NB_ERR_INVALID_VALUE;
+    if (n_j > 0 && (!x_j || !m_j || !xm_out)) return NB_ERR_INVALID_VALUE;
+    if (reinterpret_cast<uintptr_t>(xm_out) & 15u) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n_j == 0) return NB_OK;
+    nb::nb_pack_j_kernel<<<(unsigned)((n_j + 255) / 256), 256, 0, reinterpret_cast<cudaStream_t>(stream)>>>(
+        x_j, m_j, (int)n_j, reinterpret_cast<float4*>(xm_out));
+    NB_CUDA(cudaGetLastError());
+    ++t_launches;
+    return NB_OK;
+}
+
+int nb_force_packed(int64_t n_i, const float* x_i, int64_t n_j, const float* xm_j, float eps2, float* acc_out,
+                    float* pot_out, void* stream) {
+    t_launches = 0;
+    if (n_j > 0 && !xm_j) return NB_ERR_INVALID_VALUE;
+    static const float4 dummy = {0.f, 0.f, 0.f, 0.f};
+    return force_impl(n_i, x_i, n_j, nullptr, nullptr, eps2, acc_out, pot_out, reinterpret_cast<cudaStream_t>(stream),
+                      nullptr, xm_j ? reinterpret_cast<const float4*>(xm_j) : &dummy);
 }
 
 int nb_force_host(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
