@@ -1,0 +1,222 @@
+// nb_batched.cuh -- sm_100a kernel of row f2: many small (i-set, j-set) sub-problems of Eq. (1) in ONE launch,
+// the call pattern of a host tree code with interaction lists of "several thousands" particles
+// (PAPER.md:246 last sentence; section 4.4).
+//
+// One CTA = 8 warps works on up to 64 G i-particles of ONE sub-problem (G = 1, 2 or 4 packed groups of 64, a
+// template parameter).  Unlike nb_force_kernel every warp holds the SAME i-particles (in registers) and the 8 warps
+// split the j-list, each streaming its part through its own TMA + mbarrier ring; nothing leaves the CTA but a_i, phi_i.
+//   - K per CTA at run time: a tile that holds n_i <= 64 / 128 / 192 / 256 particles runs 1 / 2 / 3 / 4 packed groups
+//     (tile_sweep<2 KG>), so the padding of a sub-problem is at most 63 idle lanes;
+//   - coincident pairs (reading R1): interaction lists contain the group's own members, so EVERY
+//     sub-problem has them, bunched in a few 256-j blocks of ONE warp.  MODE_SPEC runs the flag-only loop
+//     (MASK_SPEC); a block that raised the flag is not added but DEFERRED, and after the main loop all 8 warps redo
+//     the deferred blocks together with the exact mask, 32 j-particles each, reading them from global memory.
+//     The deferred list is sorted, so the summation order -- and the result, bit for bit -- does not depend on
+//     which warp finished first.  MODE_EXACT masks every pair in the main loop.
+// Measured on the T1 tree lists: G = 1 with MODE_EXACT is the fastest combination (57 % of roofline:
+// 83 % lane use x 69 % loop efficiency, the masked loop's ceiling being 72 %); with one packed group per warp the
+// flag-only loop is latency-bound, not ALU-bound, so MODE_SPEC + deferred redo (55 %) does not pay and is kept as
+// NB_MASK=spec only; G = 2 / 4 reach 53 / 51 %.
+#pragma once
+#include "nb_kernels.cuh"
+
+namespace nb {
+
+constexpr int kBatchDefer = 64;      // deferred blocks per CTA before a warp redoes its block on its own
+
+template <int KG, int G>
+__device__ __forceinline__ const u64 (&first_groups(const u64 (&arr)[G]))[KG] {
+    return *reinterpret_cast<const u64(*)[KG]>(&arr[0]);
+}
+template <int KG, int G>
+__device__ __forceinline__ u64 (&first_groups(u64 (&arr)[G]))[KG] {
+    return *reinterpret_cast<u64(*)[KG]>(&arr[0]);
+}
+
+template <int KG, int MASK, int G>
+__device__ __forceinline__ bool sweep_groups(const float4* __restrict__ sp, int np, const u64 (&nxi)[G], const u64 (&nyi)[G],
+                                             const u64 (&nzi)[G], u64 eps2_2, float eps2, u64 (&pax)[G], u64 (&pay)[G],
+                                             u64 (&paz)[G], u64 (&pph)[G]) {
+    return tile_sweep<2 * KG, MASK, false>(sp, np, first_groups<KG, G>(nxi), first_groups<KG, G>(nyi), first_groups<KG, G>(nzi),
+                                           eps2_2, eps2, first_groups<KG, G>(pax), first_groups<KG, G>(pay),
+                                           first_groups<KG, G>(paz), first_groups<KG, G>(pph),
+                                           first_groups<KG, G>(nxi) /* e2: unused */);
+}
+
+// kg (1..G) active packed groups, uniform over the CTA; the inactive groups' partial sums stay zero
+template <int MASK, int G>
+__device__ __forceinline__ bool sweep_dyn(int kg, const float4* __restrict__ sp, int np, const u64 (&nxi)[G], const u64 (&nyi)[G],
+                                          const u64 (&nzi)[G], u64 eps2_2, float eps2, u64 (&pax)[G], u64 (&pay)[G],
+                                          u64 (&paz)[G], u64 (&pph)[G]) {
+#pragma unroll
+    for (int k = 0; k < G; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
+    if (G >= 4 && kg >= 4) return sweep_groups<(G >= 4 ? 4 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+    if (G >= 3 && kg == 3) return sweep_groups<(G >= 3 ? 3 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+    if (G >= 2 && kg == 2) return sweep_groups<(G >= 2 ? 2 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+    return sweep_groups<1, MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+}
+
+template <int G>
+__device__ __forceinline__ void add_partials(double (&run)[2 * G][4], const u64 (&pax)[G], const u64 (&pay)[G], const u64 (&paz)[G],
+                                             const u64 (&pph)[G]) {
+#pragma unroll
+    for (int k2 = 0; k2 < G; ++k2) {
+        float lo, hi;
+        unpack2(pax[k2], lo, hi); run[2 * k2][0] += (double)lo; run[2 * k2 + 1][0] += (double)hi;
+        unpack2(pay[k2], lo, hi); run[2 * k2][1] += (double)lo; run[2 * k2 + 1][1] += (double)hi;
+        unpack2(paz[k2], lo, hi); run[2 * k2][2] += (double)lo; run[2 * k2 + 1][2] += (double)hi;
+        unpack2(pph[k2], lo, hi); run[2 * k2][3] += (double)lo; run[2 * k2 + 1][3] += (double)hi;
+    }
+}
+
+// G = packed groups of 64 i-particles a CTA can hold (tile = 64 G); STAGES = ring depth per warp.
+template <int MODE, int G, int STAGES>
+__global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const ForceArgs a) {
+    static_assert(MODE == MODE_SPEC || MODE == MODE_EXACT, "batched calls: speculative with deferred redo, or masked");
+    static_assert(G >= 1 && G <= 4, "1 .. 4 packed groups");
+    constexpr int K = 2 * G, WJ = 8, TJ = 256, SUB = 256, kBatchTile = 64 * G;
+    constexpr int RING_BYTES = STAGES * TJ * 16;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    unsigned char* rings = smem_raw;                                   // [WJ][STAGES][TJ] float4
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + WJ * RING_BYTES);   // full[WJ][STAGES]
+    __shared__ int2 s_def[kBatchDefer];                                // deferred blocks: (first global j, count)
+    __shared__ int s_ndef;
+
+    if ((int)blockIdx.x >= a.tile_start[a.n_batch]) return;            // the grid is an upper bound
+    const int b = a.cta_batch[blockIdx.x];
+    const int i_lo = a.i_off[b] + ((int)blockIdx.x - a.tile_start[b]) * kBatchTile;
+    const int i_hi = a.i_off[b + 1];
+    const int jr_lo = a.j_off[b], jr_n = a.j_off[b + 1] - jr_lo;
+    const int kg = (min(kBatchTile, i_hi - i_lo) + 63) >> 6;           // packed groups that hold particles (1..G)
+
+    const int wj = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t ring = smem_u32(rings + wj * RING_BYTES);
+    const uint32_t full0 = smem_u32(bars + wj * STAGES);
+    if (lane == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(full0 + 8 * s, 1);
+        mbar_fence_init();
+    }
+    if (threadIdx.x == 0) s_ndef = 0;
+
+    const int j_begin = jr_lo + (int)((long long)jr_n * wj / WJ);
+    const int j_end = jr_lo + (int)((long long)jr_n * (wj + 1) / WJ);
+    const int n_sub = j_end - j_begin;
+    const int n_tiles = (n_sub + TJ - 1) / TJ;
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(a.jp + j_begin);
+
+    const int i_base = i_lo + lane;
+    u64 nxi[G], nyi[G], nzi[G];
+#pragma unroll
+    for (int k2 = 0; k2 < G; ++k2) {
+        const int i0 = min(i_base + (2 * k2) * 32, i_hi - 1);
+        const int i1 = min(i_base + (2 * k2 + 1) * 32, i_hi - 1);
+        nxi[k2] = pack2(-a.x_i[3 * i0 + 0], -a.x_i[3 * i1 + 0]);
+        nyi[k2] = pack2(-a.x_i[3 * i0 + 1], -a.x_i[3 * i1 + 1]);
+        nzi[k2] = pack2(-a.x_i[3 * i0 + 2], -a.x_i[3 * i1 + 2]);
+    }
+    const float eps2 = a.eps2;
+    const u64 eps2_2 = pack2(eps2, eps2);
+    __syncthreads();                                                   // barriers and s_ndef initialised
+
+    // each warp is its own producer; a ring slot is refilled by the warp that has just finished reading it
+    if (lane == 0) {
+        const int pre = n_tiles < STAGES ? n_tiles : STAGES;
+        for (int t = 0; t < pre; ++t) {
+            const uint32_t bytes = (uint32_t)min(TJ, n_sub - t * TJ) * 16u;
+            mbar_expect_tx(full0 + 8 * t, bytes);
+            tma_load_1d(ring + t * TJ * 16, src + (size_t)t * TJ * 16, bytes, full0 + 8 * t);
+        }
+    }
+
+    double run[K][4];
+#pragma unroll
+    for (int k = 0; k < K; ++k) { run[k][0] = run[k][1] = run[k][2] = run[k][3] = 0.0; }
+
+    for (int t = 0; t < n_tiles; ++t) {
+        const int slot = t % STAGES;
+        mbar_wait(full0 + 8 * slot, (uint32_t)(t / STAGES) & 1u);
+        const int nc = min(TJ, n_sub - t * TJ);                        // TJ == SUB: one Eq. (2) block per tile
+        const float4* sp = reinterpret_cast<const float4*>(rings + wj * RING_BYTES + slot * TJ * 16);
+        u64 pax[G], pay[G], paz[G], pph[G];
+        bool add = true;
+        if (MODE == MODE_SPEC) {
+            const bool hit = sweep_dyn<MASK_SPEC, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+            if (__any_sync(0xffffffffu, hit)) {                        // this block may hold a coincident pair
+                int idx = 0;
+                if (lane == 0) idx = atomicAdd(&s_ndef, 1);
+                idx = __shfl_sync(0xffffffffu, idx, 0);
+                if (idx < kBatchDefer) {
+                    if (lane == 0) s_def[idx] = make_int2(j_begin + t * TJ, nc);
+                    add = false;                                       // redone by all warps after the main loop
+                } else {
+                    (void)sweep_dyn<MASK_EXACT, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+                }
+            }
+        } else {
+            (void)sweep_dyn<MASK_EXACT, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+        }
+        if (add) add_partials<G>(run, pax, pay, paz, pph);
+        __syncwarp();                                                  // every lane is done with the slot
+        if (lane == 0 && t + STAGES < n_tiles) {
+            const int tn = t + STAGES;
+            const uint32_t bytes = (uint32_t)min(TJ, n_sub - tn * TJ) * 16u;
+            mbar_expect_tx(full0 + 8 * slot, bytes);
+            tma_load_1d(ring + slot * TJ * 16, src + (size_t)tn * TJ * 16, bytes, full0 + 8 * slot);
+        }
+    }
+
+    __syncthreads();                                                   // main loops done: rings are free, s_def complete
+    if (MODE == MODE_SPEC) {
+        const int n_def = min(s_ndef, kBatchDefer);
+        if (n_def > 1) {                                               // fixed order whatever the arrival order was
+            if (threadIdx.x == 0) {
+                for (int p = 1; p < n_def; ++p) {
+                    const int2 v = s_def[p];
+                    int q = p - 1;
+                    while (q >= 0 && s_def[q].x > v.x) { s_def[q + 1] = s_def[q]; --q; }
+                    s_def[q + 1] = v;
+                }
+            }
+            __syncthreads();
+        }
+        for (int d = 0; d < n_def; ++d) {
+            const int2 blk = s_def[d];
+            const int p0 = wj * (SUB / WJ);                            // this warp's 32 j-particles of the block
+            const int pn = min(SUB / WJ, blk.y - p0);
+            if (pn > 0) {
+                u64 pax[G], pay[G], paz[G], pph[G];
+                (void)sweep_dyn<MASK_EXACT, G>(kg, a.jp + blk.x + p0, pn, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+                add_partials<G>(run, pax, pay, paz, pph);
+            }
+        }
+        __syncthreads();
+    }
+
+    // fixed-order sum over the 8 warps through shared memory (the rings are free)
+    double* red = reinterpret_cast<double*>(smem_raw);                 // [WJ][K][4][32]
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) red[((wj * K + k) * 4 + c) * 32 + lane] = run[k][c];
+    __syncthreads();
+    // warp w finishes particle slot k = w (K <= 8 slots, 8 warps)
+    if (wj < K) {
+        const int k = wj;
+        const int i = i_base + k * 32;
+        if (i < i_hi) {
+            double s[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                s[c] = red[((0 * K + k) * 4 + c) * 32 + lane];
+#pragma unroll
+                for (int w = 1; w < WJ; ++w) s[c] += red[((w * K + k) * 4 + c) * 32 + lane];
+            }
+            a.acc[3 * i + 0] = (float)s[0];
+            a.acc[3 * i + 1] = (float)s[1];
+            a.acc[3 * i + 2] = (float)s[2];
+            if (a.pot) a.pot[i] = -(float)s[3];
+        }
+    }
+}
+
+}  // namespace nb

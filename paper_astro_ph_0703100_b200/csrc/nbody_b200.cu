@@ -15,6 +15,7 @@
 
 #include "nb_kernels.cuh"
 #include "nb_hermite.cuh"
+#include "nb_batched.cuh"
 #include "nb_plan.h"
 
 #define NB_VERSION 100
@@ -438,12 +439,25 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
 
 
 // ------------------------------------------------------------------ row f2: many small sub-problems in one launch
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE>
+// i-tile of a batched call: 64 G particles per CTA.  Measured on tree lists (groups of 32..256, lists of 2000..6000):
+// small tiles win -- less padding in every group's last tile, and several CTAs per SM overlap their prologues.
+int batched_groups(int64_t n_i_total, int64_t n_batch) {
+    const double mean = (double)n_i_total / (double)(n_batch > 0 ? n_batch : 1);
+    if (const char* e = std::getenv("NB_BATCH_TILE")) {
+        const int t = std::atoi(e);
+        if (t == 64 || t == 128 || t == 256) return t / 64;
+    }
+    if (mean <= 384.0) return 1;
+    if (mean <= 1024.0) return 2;
+    return 4;
+}
+
+template <int MODE, int G, int STAGES>
 int launch_batched_inst(const nb::ForceArgs& args, unsigned max_ctas, cudaStream_t stream) {
-    constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
-    constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
-    constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, true>;
+    constexpr size_t ring = (size_t)8 * STAGES * 256 * 16;
+    constexpr size_t red = (size_t)8 * (2 * G) * 4 * 32 * sizeof(double);
+    constexpr size_t smem = (ring > red ? ring : red) + 8 * STAGES * sizeof(uint64_t) + 128;
+    auto kern = nb::nb_batched_kernel<MODE, G, STAGES>;
     static bool configured[64] = {};
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
@@ -457,7 +471,7 @@ int launch_batched_inst(const nb::ForceArgs& args, unsigned max_ctas, cudaStream
         NB_CUDA(cudaEventCreate(&e1));
         NB_CUDA(cudaEventRecord(e0, stream));
     }
-    kern<<<max_ctas, 32 * WI * WJ, smem, stream>>>(args);
+    kern<<<max_ctas, 256, smem, stream>>>(args);
     NB_CUDA(cudaGetLastError());
     if (t_profile) {
         NB_CUDA(cudaEventRecord(e1, stream));
@@ -467,28 +481,12 @@ int launch_batched_inst(const nb::ForceArgs& args, unsigned max_ctas, cudaStream
     return NB_OK;
 }
 
-// i-tile of a batched call.  Measured on tree lists (groups of 32..256, lists of 2000..6000): the padding of
-// the last tile of every sub-problem costs more than the smaller K loses, and smaller CTAs overlap their
-// prologues, so the tile stays well below the mean sub-problem size.
-int batched_tile(int64_t n_i_total, int64_t n_batch) {
-    const double mean = (double)n_i_total / (double)(n_batch > 0 ? n_batch : 1);
-    if (const char* e = std::getenv("NB_BATCH_TILE")) {
-        const int t = std::atoi(e);
-        if (t == 64 || t == 128 || t == 256 || t == 512) return t;
-    }
-    if (mean <= 384.0) return 64;
-    if (mean <= 768.0) return 128;
-    if (mean <= 2048.0) return 256;
-    return 512;
-}
-
 template <int MODE>
-int launch_batched(const nb::ForceArgs& args, int tile, unsigned max_ctas, cudaStream_t stream) {
-    switch (tile) {
-        case 64: return launch_batched_inst<2, 1, 8, 256, 3, MODE>(args, max_ctas, stream);
-        case 128: return launch_batched_inst<4, 1, 8, 256, 3, MODE>(args, max_ctas, stream);
-        case 256: return launch_batched_inst<8, 1, 8, 256, 3, MODE>(args, max_ctas, stream);
-        default: return launch_batched_inst<8, 2, 4, 256, 4, MODE>(args, max_ctas, stream);
+int launch_batched(const nb::ForceArgs& args, int groups, unsigned max_ctas, cudaStream_t stream) {
+    switch (groups) {
+        case 1: return launch_batched_inst<MODE, 1, 2>(args, max_ctas, stream);    // 64 KB of rings: 3 CTAs per SM
+        case 2: return launch_batched_inst<MODE, 2, 3>(args, max_ctas, stream);
+        default: return launch_batched_inst<MODE, 4, 3>(args, max_ctas, stream);
     }
 }
 
@@ -518,7 +516,8 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     }
     rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)(n_j_total > 0 ? n_j_total : 1) * sizeof(float4), stream);
     if (rc != NB_OK) return rc;
-    const int tile = batched_tile(n_i_total, n_batch);
+    const int groups = batched_groups(n_i_total, n_batch);
+    const int tile = 64 * groups;
     // sum_b ceil(n_i(b) / tile) <= n_i_total / tile + n_batch
     const int64_t max_ctas = n_i_total / tile + n_batch;
     if (max_ctas > (int64_t)INT32_MAX) return NB_ERR_INVALID_VALUE;
@@ -555,12 +554,12 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     args.n_j = (int)n_j_total;
     args.S = 1;
     args.eps2 = eps2;
-    // Interaction lists start with the group's own members (coincident pairs in every sub-problem), and the
-    // speculative mode's redo would fall on one warp of the CTA, so batched calls mask every pair by default.
+    // masked loop by default (measured faster on tree lists, nb_batched.cuh); NB_MASK=spec: flag-only loop with the
+    // flagged blocks redone by all 8 warps together (needs eps2 >= 2^-40)
     const char* e = std::getenv("NB_MASK");
     const bool spec = eps2 >= kSpecMinEps2 && (e && e[0] == 's');
-    return spec ? launch_batched<nb::MODE_SPEC>(args, tile, (unsigned)max_ctas, stream)
-                : launch_batched<nb::MODE_EXACT>(args, tile, (unsigned)max_ctas, stream);
+    return spec ? launch_batched<nb::MODE_SPEC>(args, groups, (unsigned)max_ctas, stream)
+                : launch_batched<nb::MODE_EXACT>(args, groups, (unsigned)max_ctas, stream);
 }
 
 int nb_force_jerk(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j, const float* x_j, const float* v_j,
