@@ -285,10 +285,10 @@ struct ForceArgs {
     int* tickets;          // [tiles_i] zero between calls; non-null => the last CTA of an i-tile sums the partials
     const int* coin_lists; // MODE_LIST: [n_groups][1 + kCoinCap]
     const int* coin_flag;  // MODE_LIST: != 0 -> mask everywhere
-    const int* i_off;      // BATCHED: [n_batch + 1] first i of every sub-problem
-    const int* j_off;      // BATCHED: [n_batch + 1] first j of every sub-problem
-    const int* tile_start; // BATCHED: [n_batch + 1] first CTA of every sub-problem (exclusive scan of its i-tiles)
-    const int* cta_batch;  // BATCHED: [number of CTAs] sub-problem of every CTA
+    const int* i_off;      // nb_batched_kernel: [n_batch + 1] first i of every sub-problem
+    const int* j_off;      // nb_batched_kernel: [n_batch + 1] first j of every sub-problem
+    const int* tile_start; // nb_batched_kernel: [n_batch + 1] first CTA of every sub-problem (exclusive scan of its i-tiles)
+    const int* cta_batch;  // nb_batched_kernel: [number of CTAs] sub-problem of every CTA
     int n_batch;
     int n_i;
     int n_j;
@@ -307,28 +307,15 @@ enum { MODE_EXACT = 0,     // masked loop everywhere (eps2 == 0 or tiny)
 // Each sub-range is streamed through its own shared-memory ring by 1-D TMA bulk copies issued by
 // lane 0 of the group's first warp; "full" mbarriers count bytes, "empty" mbarriers count the WI
 // consuming warps.
-//
-// BATCHED (row f2, nb_force_batched): the grid is one row of CTAs; CTA blockIdx.x finds the
-// sub-problem b it belongs to in cta_batch[] (written by nb_batch_scan_kernel) and works on i in
-// [i_off[b], i_off[b+1]) against j in [j_off[b], j_off[b+1]); no split across CTAs (S = 1).
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool BATCHED = false, bool EPS_I = false, int SUB = 256>
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I = false, int SUB = 256>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
     static_assert(!(EPS_I && MODE == MODE_SPEC), "per-i softening: masked or list mode only");
     static_assert(SUB == kCoinSeg, "coincidence segments are SUB j-particles");
-    static_assert(!(BATCHED && MODE == MODE_LIST), "no coincidence lists for batched calls");
     extern __shared__ __align__(128) unsigned char smem_raw[];
 
     // i-range [i_lo, i_hi) this CTA draws its tile from, j-range [jr_lo, jr_lo + jr_n) it sums over
-    int i_lo = blockIdx.x * (32 * K * WI), i_hi = a.n_i, jr_lo = 0, jr_n = a.n_j;
-    if (BATCHED) {
-        if ((int)blockIdx.x >= a.tile_start[a.n_batch]) return;        // the grid is an upper bound
-        const int lo = a.cta_batch[blockIdx.x];
-        i_lo = a.i_off[lo] + ((int)blockIdx.x - a.tile_start[lo]) * (32 * K * WI);
-        i_hi = a.i_off[lo + 1];
-        jr_lo = a.j_off[lo];
-        jr_n = a.j_off[lo + 1] - jr_lo;
-    }
+    const int i_lo = blockIdx.x * (32 * K * WI), i_hi = a.n_i, jr_lo = 0, jr_n = a.n_j;
     constexpr int RING_BYTES = STAGES * TJ * 16;
     unsigned char* rings = smem_raw;                                   // [WJ][STAGES][TJ] float4
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + WJ * RING_BYTES);   // full[WJ][STAGES], empty[WJ][STAGES]
@@ -506,7 +493,6 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
             }
         }
     }
-    if (BATCHED) return;
 
     // a7 (inter-CTA), fused: the CTA that finishes LAST among the S chunks of this i-tile sums the S partials in the
     // fixed order s = 0 .. S-1 (so the result does not depend on which CTA that is) and writes a and phi.  The

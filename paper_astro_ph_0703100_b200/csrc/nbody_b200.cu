@@ -136,7 +136,7 @@ int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStrea
     constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
     constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, false, EPS_I>;
+    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, EPS_I>;
     static bool configured[64] = {};
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
