@@ -120,7 +120,8 @@ __global__ void __launch_bounds__(256) nb_pack_j_kernel(const float* __restrict_
 //                i-particles, where it gives bit for bit what MASK_EXACT gives.  13 + 1 instructions.
 enum { MASK_EXACT = 0, MASK_SPEC = 1, MASK_NONE = 2 };
 
-template <int MASK>
+// PHI = false: the caller does not want the potential (pot_out == NULL): 12 FP32-pipe instructions per pair.
+template <int MASK, bool PHI = true>
 __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nxi, u64 nyi, u64 nzi, u64 eps2_2,
                                           float eps2, u64& ax, u64& ay, u64& az, u64& ph, bool& hit) {
     const u64 dx = add2(xj, nxi);                    // dx = xj - xi
@@ -151,12 +152,12 @@ __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nx
     ax = fma2(mu3, dx, ax);                          // OUTPUT[0..2] += mr3i*d PAPER.md:469-471
     ay = fma2(mu3, dy, ay);
     az = fma2(mu3, dz, az);
-    ph = add2(ph, mu);                               // OUTPUT[6] -= pot (sign applied at the end) PAPER.md:552
+    if (PHI) ph = add2(ph, mu);                      // OUTPUT[6] -= pot (sign applied at the end) PAPER.md:552
 }
 
 // One tile: K/2 i-pairs of this thread against np j-particles in shared memory; partial sums start from zero (Eq. (2)).
 // EPS_I (row f3): the softening is a property of the i-particle (Fig. A.1) and sits, packed, in e2[].
-template <int K, int MASK, bool EPS_I = false>
+template <int K, int MASK, bool EPS_I = false, bool PHI = true>
 __device__ __forceinline__ bool tile_sweep(const float4* __restrict__ sp, int np, const u64 (&nxi)[K / 2], const u64 (&nyi)[K / 2],
                                            const u64 (&nzi)[K / 2], u64 eps2_2, float eps2, u64 (&pax)[K / 2], u64 (&pay)[K / 2],
                                            u64 (&paz)[K / 2], u64 (&pph)[K / 2], const u64 (&e2)[K / 2]) {
@@ -169,7 +170,7 @@ __device__ __forceinline__ bool tile_sweep(const float4* __restrict__ sp, int np
         const u64 xj = pack2(J.x, J.x), yj = pack2(J.y, J.y), zj = pack2(J.z, J.z), mj = pack2(J.w, J.w);
 #pragma unroll
         for (int k = 0; k < K / 2; ++k)
-            pair_body<MASK>(xj, yj, zj, mj, nxi[k], nyi[k], nzi[k], EPS_I ? e2[k] : eps2_2, eps2, pax[k], pay[k], paz[k], pph[k], hit);
+            pair_body<MASK, PHI>(xj, yj, zj, mj, nxi[k], nyi[k], nzi[k], EPS_I ? e2[k] : eps2_2, eps2, pax[k], pay[k], paz[k], pph[k], hit);
     }
     return hit;
 }
@@ -307,7 +308,7 @@ enum { MODE_EXACT = 0,     // masked loop everywhere (eps2 == 0 or tiny)
 // Each sub-range is streamed through its own shared-memory ring by 1-D TMA bulk copies issued by
 // lane 0 of the group's first warp; "full" mbarriers count bytes, "empty" mbarriers count the WI
 // consuming warps.
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I = false, int SUB = 256>
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I = false, bool PHI = true, int SUB = 256>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
     static_assert(!(EPS_I && MODE == MODE_SPEC), "per-i softening: masked or list mode only");
@@ -408,9 +409,9 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
             const int nc = min(SUB, np - c);
             u64 pax[K / 2], pay[K / 2], paz[K / 2], pph[K / 2];
             if (MODE == MODE_SPEC) {
-                const bool hit = tile_sweep<K, MASK_SPEC, EPS_I>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
+                const bool hit = tile_sweep<K, MASK_SPEC, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
                 if (__any_sync(0xffffffffu, hit))                      // rare: some pair of this warp may be coincident
-                    (void)tile_sweep<K, MASK_EXACT, EPS_I>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
+                    (void)tile_sweep<K, MASK_EXACT, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
             } else if (MODE == MODE_LIST) {
                 const int j0 = j_begin + t * TJ + c;                   // global index of the block's first j
                 const int seg_lo = j0 >> kCoinSegShift, seg_hi = (j0 + nc - 1) >> kCoinSegShift;
@@ -419,11 +420,11 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
                     coin_next = (coin_pos < coin_cnt) ? coin[1 + coin_pos] : 0x7fffffff;
                 }
                 if (coin_cnt < 0 || coin_next <= seg_hi)               // rare: the block holds a coincident pair
-                    (void)tile_sweep<K, MASK_EXACT, EPS_I>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
+                    (void)tile_sweep<K, MASK_EXACT, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
                 else
-                    (void)tile_sweep<K, MASK_NONE, EPS_I>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
+                    (void)tile_sweep<K, MASK_NONE, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
             } else {
-                (void)tile_sweep<K, MASK_EXACT, EPS_I>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
+                (void)tile_sweep<K, MASK_EXACT, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
             }
             // a5: block partial -> running total
 #pragma unroll
@@ -432,7 +433,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
                 unpack2(pax[k2], lo, hi); run[2 * k2][0] += (double)lo; run[2 * k2 + 1][0] += (double)hi;
                 unpack2(pay[k2], lo, hi); run[2 * k2][1] += (double)lo; run[2 * k2 + 1][1] += (double)hi;
                 unpack2(paz[k2], lo, hi); run[2 * k2][2] += (double)lo; run[2 * k2 + 1][2] += (double)hi;
-                unpack2(pph[k2], lo, hi); run[2 * k2][3] += (double)lo; run[2 * k2 + 1][3] += (double)hi;
+                if (PHI) { unpack2(pph[k2], lo, hi); run[2 * k2][3] += (double)lo; run[2 * k2 + 1][3] += (double)hi; }
             }
         }
 

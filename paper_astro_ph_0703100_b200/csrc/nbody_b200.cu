@@ -131,12 +131,12 @@ int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool aliased) {
     return aliased ? nb::MODE_SPEC : nb::MODE_EXACT;
 }
 
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I>
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I, bool PHI = true>
 int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
     constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, EPS_I>;
+    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, EPS_I, PHI>;
     static bool configured[64] = {};
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
@@ -169,6 +169,16 @@ int launch_force_k(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t
         case 2: return launch_force_inst<K, 4, 2, 512, 4, MODE, EPS_I>(args, plan, stream);
         case 4: return launch_force_inst<K, 2, 4, 256, 4, MODE, EPS_I>(args, plan, stream);
         default: return launch_force_inst<K, 1, 8, 256, 3, MODE, EPS_I>(args, plan, stream);
+    }
+}
+
+// pot_out == NULL on a large call: the 12-instruction loop without the potential (K = 8, list mode only)
+int launch_force_nophi(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
+    switch (plan.WJ) {
+        case 1: return launch_force_inst<8, 8, 1, 512, 4, nb::MODE_LIST, false, false>(args, plan, stream);
+        case 2: return launch_force_inst<8, 4, 2, 512, 4, nb::MODE_LIST, false, false>(args, plan, stream);
+        case 4: return launch_force_inst<8, 2, 4, 256, 4, nb::MODE_LIST, false, false>(args, plan, stream);
+        default: return launch_force_inst<8, 1, 8, 256, 3, nb::MODE_LIST, false, false>(args, plan, stream);
     }
 }
 
@@ -281,7 +291,9 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, jp, 1, stream, &args.coin_lists, &args.coin_flag);
         if (rc != NB_OK) return rc;
-        rc = eps2_i ? launch_force<nb::MODE_LIST, true>(args, plan, stream) : launch_force<nb::MODE_LIST>(args, plan, stream);
+        if (eps2_i) rc = launch_force<nb::MODE_LIST, true>(args, plan, stream);
+        else if (!pot_out && plan.K == 8) rc = launch_force_nophi(args, plan, stream);
+        else rc = launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (eps2_i) {
         rc = launch_force<nb::MODE_EXACT, true>(args, plan, stream);
     } else if (mode == nb::MODE_SPEC) {
@@ -681,7 +693,8 @@ int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, f
     const int threads = 256, blocks = (n3 + threads - 1) / threads;
     const float h = 0.5f * dt;
     // a0 = force(x0)
-    rc = force_impl(n, x, n, x, m, eps2, acc_io, pot_out, stream);
+    // phi is only wanted at the final time: the evaluations before it run the 12-instruction loop without it
+    rc = force_impl(n, x, n, x, m, eps2, acc_io, n_steps == 0 ? pot_out : nullptr, stream);
     if (rc != NB_OK) return rc;
     for (int64_t s = 0; s < n_steps; ++s) {
         // opening half-kick + drift; from the second step on it also carries the previous step's
@@ -692,7 +705,7 @@ int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, f
             nb::nb_kick_drift_kernel<true><<<blocks, threads, 0, stream>>>(x, v, acc_io, n3, h, dt);
         NB_CUDA(cudaGetLastError());
         ++t_launches;
-        rc = force_impl(n, x, n, x, m, eps2, acc_io, pot_out, stream);
+        rc = force_impl(n, x, n, x, m, eps2, acc_io, s + 1 == n_steps ? pot_out : nullptr, stream);
         if (rc != NB_OK) return rc;
     }
     if (n_steps > 0) {

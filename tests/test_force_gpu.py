@@ -326,3 +326,14 @@ def test_c3_full_size_sampled(nb):
     # P7: uniform sphere, E[W] = -(3/5)(1 - sum m^2)/R
     W = 0.5 * float(np.sum(m * pot.astype(np.float64)))
     assert abs(W / (-0.6 * (1.0 - float(np.sum(m * m)))) - 1.0) < 0.01
+
+
+def test_no_potential_variant_gives_the_same_acceleration_bitwise(nb, monkeypatch):
+    """pot_out = NULL on a large call runs the 12-instruction loop (no phi): a_i is the same, bit for bit."""
+    monkeypatch.setenv("NB_MASK", "list")
+    for plan in ("8,8,1,3", "8,4,2,1", "8,2,4,2", "8,1,8,5"):
+        monkeypatch.setenv("NB_PLAN", plan)
+        w = wl.plummer_workload(3000, 1.0 / 64, seed=17)
+        a1, p1 = gpu_force(nb, w.x_j, w.x_j, w.m_j, w.eps2, alias=True)
+        a2, p2 = gpu_force(nb, w.x_j, w.x_j, w.m_j, w.eps2, want_pot=False, alias=True)
+        assert p2 is None and np.array_equal(a1, a2), plan
