@@ -431,6 +431,28 @@ def main():
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
 
+    # small calls are launch-bound: also report the same call replayed from a CUDA graph (no L2 flush between replays)
+    graph_ms = None
+    if args.op == "force" and not args.shard and prob.pairs < 2.0 ** 30:
+        gs = torch.cuda.Stream()
+        with torch.cuda.stream(gs):
+            for _ in range(3):
+                prob.call()                                # warm this stream's workspace
+            gs.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=gs):
+                prob.call()
+            g.replay()
+            gs.synchronize()
+            reps = 200
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record(gs)
+            for _ in range(reps):
+                g.replay()
+            g1.record(gs)
+            gs.synchronize()
+        graph_ms = g0.elapsed_time(g1) / reps
+
     # end to end with HOST buffers (pinned), copies inside the timed region
     e2e_steps = max(3, min(args.steps, 10))
     for _ in range(2):
@@ -492,6 +514,9 @@ def main():
                               "gflops_force_jerk_8800gtx_n131072": 179,
                               "note": "PAPER.md:314 (includes PCIe copies) and PAPER.md:343; context, not target"},
         }
+        if graph_ms is not None:
+            out["graph_replay"] = {"ms_per_call": graph_ms, "value": pairs / (graph_ms * 1e-3), "unit": METRIC,
+                                   "note": "one captured nb_force call replayed 200x back to back, L2 warm"}
         if args.op == "leapfrog":
             out["kdk_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
             if not args.no_cpu_baseline:

@@ -337,3 +337,33 @@ def test_no_potential_variant_gives_the_same_acceleration_bitwise(nb, monkeypatc
         a1, p1 = gpu_force(nb, w.x_j, w.x_j, w.m_j, w.eps2, alias=True)
         a2, p2 = gpu_force(nb, w.x_j, w.x_j, w.m_j, w.eps2, want_pot=False, alias=True)
         assert p2 is None and np.array_equal(a1, a2), plan
+
+
+@pytest.mark.parametrize("n,mode", [(2048, ""), (3000, "list"), (3000, "exact")])
+def test_cuda_graph_capture_and_replay(nb, n, mode, monkeypatch):
+    """include/nbody_b200.h: "once warm the call is CUDA-graph capturable" -- capture nb_force (small-call path with the
+    fused second pass; large-call path with the coincidence pre-pass and its memset), replay on new inputs."""
+    import torch
+    if mode:
+        monkeypatch.setenv("NB_MASK", mode)
+    w = wl.plummer_workload(n, 1.0 / 64, seed=23)
+    x, m = dev(w.x_j), dev(w.m_j)
+    acc = torch.empty((n, 3), device="cuda"); pot = torch.empty((n,), device="cuda")
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        for _ in range(2):                                             # warm: workspace allocated on this stream
+            nb.force(x, x, m, w.eps2, acc_out=acc, pot_out=pot)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            nb.force(x, x, m, w.eps2, acc_out=acc, pot_out=pot)
+    ref = (acc.clone(), pot.clone())
+    # new positions in the same buffers, replay twice
+    w2 = wl.plummer_workload(n, 1.0 / 64, seed=24)
+    x.copy_(dev(w2.x_j))
+    acc.zero_(); pot.zero_()
+    g.replay(); g.replay()
+    torch.cuda.synchronize()
+    ra, rp = oracle.force(w2.x_j, w2.x_j, w2.m_j, w2.eps2)
+    check_parity(acc.cpu().numpy(), pot.cpu().numpy(), ra, rp, f"graph replay {n} {mode}")
+    assert not torch.equal(ref[0], acc)
