@@ -283,6 +283,11 @@ class Problem:
             nb.force_host(h[0] if w.x_i is None else h[2], h[0], h[1], w.eps2,
                           acc_out=self.h_outs[0].numpy(), pot_out=self.h_outs[1].numpy())
             return
+        if self.op == "jerk":
+            h = [p.numpy() for p in self.pinned]
+            nb.force_jerk_host(h[0], h[1], h[0], h[1], h[2], w.eps2, acc_out=self.h_outs[0].numpy(),
+                               jerk_out=self.h_outs[1].numpy(), pot_out=self.h_outs[2].numpy())
+            return
         staged = [p.cuda(non_blocking=True) for p in self.pinned]
         self.call(staged)
         for h, d in zip(self.h_outs, self.outs):
@@ -293,6 +298,8 @@ class Problem:
     def e2e_api(self):
         if self.op == "force":
             return "nb_force_host (pinned host buffers)"
+        if self.op == "jerk":
+            return "nb_force_jerk_host (pinned host buffers)"
         if self.op == "leapfrog":
             return "pinned host (x, v, m) -> cudaMemcpyAsync -> nb_leapfrog_kdk (100 KDK steps) -> cudaMemcpyAsync of a, phi -> pinned host"
         return f"pinned host tensors -> cudaMemcpyAsync -> nb_{'force_jerk' if self.op == 'jerk' else 'force_batched'} -> cudaMemcpyAsync -> pinned host"

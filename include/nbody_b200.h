@@ -194,6 +194,15 @@ int nb_force_batched(int64_t n_batch, const int32_t *i_offsets, const int32_t *j
                      float *acc_out, float *pot_out,
                      void *stream);
 
+/*
+ * nb_force_jerk_host -- nb_force_jerk on HOST arrays: the paper's force() of Fig. A.2 with its
+ * host->device and device->host copies (steps (a) and (l)) inside the call.  Blocking.
+ */
+int nb_force_jerk_host(int64_t n_i, const float *x_i, const float *v_i,
+                       int64_t n_j, const float *x_j, const float *v_j, const float *m_j,
+                       float eps2,
+                       float *acc_out, float *jerk_out, float *pot_out);
+
 /* nb_plan_query for nb_force_jerk (same out[] layout; K <= 4, 256 j-particles of 32 bytes per stage). */
 int nb_plan_query_jerk(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]);
 

@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     force_eps_i,
     force_host,
     force_jerk,
+    force_jerk_host,
     force_packed,
     last_launch_count,
     leapfrog_kdk,

@@ -53,6 +53,8 @@ def lib() -> ctypes.CDLL:
         l.nb_force_eps_i.restype = ci
         l.nb_force_batched.argtypes = [i64, p, p, i64, p, i64, p, p, f32, p, p, p]
         l.nb_force_batched.restype = ci
+        l.nb_force_jerk_host.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p]
+        l.nb_force_jerk_host.restype = ci
         l.nb_plan_query_jerk.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
         l.nb_plan_query_jerk.restype = ci
         l.nb_plan_query.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
@@ -209,6 +211,31 @@ def force_batched(i_offsets, j_offsets, x_i, x_j, m_j, eps2: float, acc_out=None
                                     None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
     _check(st, "nb_force_batched")
     return acc_out, pot_out
+
+
+def force_jerk_host(x_i, v_i, x_j, v_j, m_j, eps2: float, acc_out=None, jerk_out=None, pot_out=None, want_pot: bool = True):
+    """nb_force_jerk_host on numpy float32 arrays (or pinned CPU tensors' numpy views).  Blocking."""
+    import numpy as np
+    same = x_i is x_j and v_i is v_j
+    xj = np.ascontiguousarray(x_j, dtype=np.float32).reshape(-1, 3)
+    vj = np.ascontiguousarray(v_j, dtype=np.float32).reshape(-1, 3)
+    mj = np.ascontiguousarray(m_j, dtype=np.float32).reshape(-1)
+    xi = xj if same else np.ascontiguousarray(x_i, dtype=np.float32).reshape(-1, 3)
+    vi = vj if same else np.ascontiguousarray(v_i, dtype=np.float32).reshape(-1, 3)
+    n_i, n_j = xi.shape[0], xj.shape[0]
+    if vi.shape[0] != n_i or vj.shape[0] != n_j or mj.shape[0] != n_j:
+        raise ValueError("array lengths differ")
+    if acc_out is None:
+        acc_out = np.empty((n_i, 3), dtype=np.float32)
+    if jerk_out is None:
+        jerk_out = np.empty((n_i, 3), dtype=np.float32)
+    if pot_out is None and want_pot:
+        pot_out = np.empty((n_i,), dtype=np.float32)
+    st = lib().nb_force_jerk_host(n_i, xi.ctypes.data, vi.ctypes.data, n_j, xj.ctypes.data, vj.ctypes.data, mj.ctypes.data,
+                                  float(eps2), acc_out.ctypes.data, jerk_out.ctypes.data,
+                                  None if pot_out is None else pot_out.ctypes.data)
+    _check(st, "nb_force_jerk_host")
+    return acc_out, jerk_out, pot_out
 
 
 def force_host(x_i, x_j, m_j, eps2: float, want_pot: bool = True, acc_out=None, pot_out=None):

@@ -581,6 +581,58 @@ int nb_force_jerk(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j, 
                            reinterpret_cast<cudaStream_t>(stream));
 }
 
+int nb_force_jerk_host(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j, const float* x_j, const float* v_j,
+                       const float* m_j, float eps2, float* acc_out, float* jerk_out, float* pot_out) {
+    t_launches = 0;
+    if (bad_count(n_i) || bad_count(n_j)) return NB_ERR_INVALID_VALUE;
+    if (!(eps2 >= 0.0f) || !std::isfinite(eps2)) return NB_ERR_INVALID_VALUE;
+    if (n_i > 0 && (!x_i || !v_i || !acc_out || !jerk_out)) return NB_ERR_INVALID_VALUE;
+    if (n_j > 0 && (!x_j || !v_j || !m_j)) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n_i == 0) return NB_OK;
+    cudaStream_t stream = nullptr;   // legacy default stream
+    Workspace* ws;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        ws = &g_ws[std::make_pair(dev, stream)];
+    }
+    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
+    const bool aliased = (x_i == x_j && v_i == v_j && n_i <= n_j);
+    const size_t b_j3 = up(sizeof(float) * 3 * (size_t)n_j), b_mj = up(sizeof(float) * (size_t)n_j);
+    const size_t b_i3 = up(sizeof(float) * 3 * (size_t)n_i), b_pot = up(sizeof(float) * (size_t)n_i);
+    const size_t total = 2 * b_j3 + b_mj + (aliased ? 0 : 2 * b_i3) + 2 * b_i3 + b_pot + 256;
+    rc = ensure(&ws->stage, &ws->stage_bytes, total, stream);
+    if (rc != NB_OK) return rc;
+    char* p = reinterpret_cast<char*>(ws->stage);
+    float* d_xj = reinterpret_cast<float*>(p); p += b_j3;
+    float* d_vj = reinterpret_cast<float*>(p); p += b_j3;
+    float* d_mj = reinterpret_cast<float*>(p); p += b_mj;
+    float* d_xi = d_xj; float* d_vi = d_vj;
+    if (!aliased) { d_xi = reinterpret_cast<float*>(p); p += b_i3; d_vi = reinterpret_cast<float*>(p); p += b_i3; }
+    float* d_acc = reinterpret_cast<float*>(p); p += b_i3;
+    float* d_jerk = reinterpret_cast<float*>(p); p += b_i3;
+    float* d_pot = reinterpret_cast<float*>(p);
+    if (n_j > 0) {                                                             // step (a): host -> device
+        NB_CUDA(cudaMemcpyAsync(d_xj, x_j, sizeof(float) * 3 * (size_t)n_j, cudaMemcpyHostToDevice, stream));
+        NB_CUDA(cudaMemcpyAsync(d_vj, v_j, sizeof(float) * 3 * (size_t)n_j, cudaMemcpyHostToDevice, stream));
+        NB_CUDA(cudaMemcpyAsync(d_mj, m_j, sizeof(float) * (size_t)n_j, cudaMemcpyHostToDevice, stream));
+    }
+    if (!aliased) {
+        NB_CUDA(cudaMemcpyAsync(d_xi, x_i, sizeof(float) * 3 * (size_t)n_i, cudaMemcpyHostToDevice, stream));
+        NB_CUDA(cudaMemcpyAsync(d_vi, v_i, sizeof(float) * 3 * (size_t)n_i, cudaMemcpyHostToDevice, stream));
+    }
+    rc = force_jerk_impl(n_i, d_xi, d_vi, n_j, d_xj, d_vj, d_mj, eps2, d_acc, d_jerk, pot_out ? d_pot : nullptr, stream);
+    if (rc != NB_OK) return rc;
+    NB_CUDA(cudaMemcpyAsync(acc_out, d_acc, sizeof(float) * 3 * (size_t)n_i, cudaMemcpyDeviceToHost, stream));   // step (l)
+    NB_CUDA(cudaMemcpyAsync(jerk_out, d_jerk, sizeof(float) * 3 * (size_t)n_i, cudaMemcpyDeviceToHost, stream));
+    if (pot_out) NB_CUDA(cudaMemcpyAsync(pot_out, d_pot, sizeof(float) * (size_t)n_i, cudaMemcpyDeviceToHost, stream));
+    NB_CUDA(cudaStreamSynchronize(stream));
+    return NB_OK;
+}
+
 int nb_plan_query_jerk(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]) {
     if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
     const nb::Plan p = hermite_plan(n_i, n_j, sm_count);

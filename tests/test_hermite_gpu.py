@@ -182,3 +182,15 @@ def test_c1_shape_full_size_sampled(nb):
     check(acc[idx], jerk[idx], pot[idx], ra, rj, rp, "C1 shape sampled")
     tot = np.linalg.norm((m[:, None].astype(np.float64) * jerk).sum(0))
     assert tot <= 1e-5 * (m[:, None] * np.linalg.norm(jerk, axis=1)[:, None]).sum()
+
+
+def test_force_jerk_host_matches_device_path(nb):
+    x, v, m, eps2 = plummer_xv(3000, 1.0 / 64, 15)
+    a_d, j_d, p_d = gpu_fj(nb, x, v, x, v, m, eps2, alias=True)
+    a_h, j_h, p_h = nb.force_jerk_host(x, v, x, v, m, eps2)
+    assert np.array_equal(a_d, a_h) and np.array_equal(j_d, j_h) and np.array_equal(p_d, p_h)
+    xi, vi = x[:100].copy(), v[:100].copy()
+    a_h, j_h, p_h = nb.force_jerk_host(xi, vi, x, v, m, eps2, want_pot=False)
+    ra, rj, _ = oracle.force_jerk(xi, vi, x, v, m, eps2)
+    assert p_h is None
+    check(a_h, j_h, None, ra, rj, None, "host subset")
