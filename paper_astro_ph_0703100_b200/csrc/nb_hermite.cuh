@@ -26,6 +26,10 @@
 
 namespace nb {
 
+#ifndef NB_HERMITE_UNROLL
+#define NB_HERMITE_UNROLL 2
+#endif
+constexpr int kHermiteUnroll = NB_HERMITE_UNROLL;   // j-particles per loop iteration (measured: 1 / 2 / 4)
 constexpr int kHermiteAcc = 10;   // ax ay az | j1x j1y j1z | j2x j2y j2z | phi
 
 // (x, y, z) || m || (vx, vy, vz) -> two float4 per j-particle
@@ -105,7 +109,7 @@ __device__ __forceinline__ void hermite_sweep(const float4* __restrict__ sp, int
     for (int k = 0; k < K / 2; ++k)
 #pragma unroll
         for (int c = 0; c < kHermiteAcc; ++c) part[k][c] = 0ull;
-#pragma unroll 2
+#pragma unroll kHermiteUnroll
     for (int j = 0; j < np; ++j) {
         const float4 P = sp[2 * j], V = sp[2 * j + 1];                 // two broadcast LDS.128
         const u64 xj = pack2(P.x, P.x), yj = pack2(P.y, P.y), zj = pack2(P.z, P.z), mj = pack2(P.w, P.w);
