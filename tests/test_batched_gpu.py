@@ -123,9 +123,11 @@ def test_reproducible_and_pot_null(nb):
 
 
 def test_bench_size_sampled(nb):
-    """The size bench.py --op batched times (65536 particles, groups 32..256, lists 2000..6000): sampled groups."""
-    w = wl.tree_list_workload(65536, 32, 256, 2000, 6000, 1.0 / 128, seed=7)
-    acc, pot = gpu_batched(nb, w)
+    """The workload bench.py --op batched times (T1: 524288 particles, 3624 groups of 32..256, lists of 2000..6000),
+    same launch configuration: 24 sampled groups against the oracle, and no group left unwritten."""
+    w = wl.tree_list_workload(524288, 32, 256, 2000, 6000, 1.0 / 128, seed=7)
+    acc, pot = gpu_batched(nb, w, fill=float("nan"))
+    assert np.all(np.isfinite(acc)) and np.all(pot < 0.0)
     rng = np.random.default_rng(0)
     for b in rng.choice(w.n_batch, 24, replace=False):
         i0, i1, j0, j1 = (int(v) for v in (w.i_offsets[b], w.i_offsets[b + 1], w.j_offsets[b], w.j_offsets[b + 1]))
