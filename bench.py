@@ -360,6 +360,8 @@ def main():
                     "all-gather of the packed j records over NCCL, then nb_force_packed on the local i-slice; strong "
                     "scaling) instead of N independent replicas")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--check", action="store_true", help="--op force / jerk: add a 'parity' object -- the timed call's "
+                    "output against the CPU oracle on up to 2048 sampled i-particles (Eq. (3), PAPER.md:278)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()
@@ -535,6 +537,24 @@ def main():
                 _, _, e_end = oracle.energy(prob.dev[0].cpu().numpy(), prob.dev[1].cpu().numpy(), w.m_j, w.eps2)
                 out["energy"] = {"kdk_steps": prob.kdk_done, "E_start": e_start, "E_end": e_end,
                                  "rel_drift": abs(e_end - e_start) / abs(e_start), "by": "oracle.energy (FP64) on the GPU's FP32 (x, v)"}
+        if args.check and args.op in ("force", "jerk") and not args.shard:
+            import oracle
+            w = prob.w
+            prob.call()
+            torch.cuda.synchronize()
+            idx = np.sort(np.random.default_rng(0).choice(w.n_i, min(2048, w.n_i), replace=False))
+            got = [o.cpu().numpy()[idx] for o in prob.outs]
+            if args.op == "force":
+                ra, rp = oracle.force(w.xi[idx], w.x_j, w.m_j, w.eps2)
+                par = oracle.error_metrics(got[0], ra, got[1], rp)
+            else:
+                ra, rj, rp = oracle.force_jerk(w.x_j[idx], w.v[idx], w.x_j, w.v, w.m_j, w.eps2)
+                par = oracle.error_metrics(got[0], ra, got[2], rp)
+                ej = oracle.error_metrics(got[1], rj)
+                par["jerk_max"], par["jerk_rms"] = ej["acc_max"], ej["acc_rms"]
+            par["sample"] = f"{len(idx)} seeded i-particles x all {w.n_j} j-particles, oracle in FP64"
+            par["tolerance"] = "acc (jerk) RMS <= 1e-5, max <= 1e-4; phi RMS <= 1e-5 (BASELINE.json north_star)"
+            out["parity"] = par
         if not args.no_cpu_baseline:
             v, cores, sample = oracle_rate_op(args.op, prob.w, args.cpu_seconds)
             out["cpu_baseline"] = {"value": v, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample}

@@ -112,14 +112,14 @@ nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count) {
 constexpr float kSpecMinEps2 = 9.094947017729282e-13f;
 
 // Calls with at least this many pairs locate their coincident pairs with the hash-join pre-pass
-// (MODE_LIST: three extra O(n) launches, no test in the hot loop); smaller ones use MODE_SPEC.
-constexpr double kListMinPairs = 1073741824.0;   // 2^30
+// (MODE_LIST: three extra O(n) launches, ~35 us, no test in the hot loop); smaller ones mask every pair.
+constexpr double kListMinPairs = 536870912.0;    // 2^29
 
-// Small calls: the speculative mode pays a masked redo of a whole 256-j block per warp that meets a coincident
-// pair.  When the i-set IS the j-set (same pointer) those pairs sit on the diagonal and few warps meet one; when
-// the i-set is a separate array it is, in practice, an active subset of the j-set (block time steps, BASELINE.json
-// configs[2]) whose partners are scattered over all j, nearly every warp would redo its block (measured on C2:
-// 39 us speculative, 27 us masked), so separate sets mask every pair.
+// Small calls mask every pair (MODE_EXACT).  The speculative mode (flag-only loop, masked redo of a flagged 256-j
+// block) is faster per pair but a small call is a single wave of CTAs, so the call lasts as long as its slowest
+// CTA -- one that redoes blocks: measured on aliased sets N = 4096 / 8192 / 16384: 34 / 67 / 186 us speculative
+// against 27 / 52 / 165 us masked; on an active subset (C2) 39 against 27 us.  MODE_SPEC stays available as
+// NB_MASK=spec (tests keep it bit-identical to the masked kernel).
 int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool aliased) {
     // debugging aid: NB_MASK=exact|spec|list forces a mode (spec/list still need eps2 >= 2^-40)
     const char* e = std::getenv("NB_MASK");
@@ -127,8 +127,8 @@ int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool aliased) {
     if (eps2 < kSpecMinEps2) return nb::MODE_EXACT;
     if (e && e[0] == 's') return nb::MODE_SPEC;
     if (e && e[0] == 'l') return nb::MODE_LIST;
-    if ((double)n_i * (double)n_j >= kListMinPairs) return nb::MODE_LIST;
-    return aliased ? nb::MODE_SPEC : nb::MODE_EXACT;
+    (void)aliased;
+    return ((double)n_i * (double)n_j >= kListMinPairs) ? nb::MODE_LIST : nb::MODE_EXACT;
 }
 
 template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I, bool PHI = true>
