@@ -22,7 +22,7 @@
  *   - plain C, no C++ types; safe to call through ctypes / dlopen.
  *   - "device" pointers are CUDA global-memory pointers valid on the current device; "host"
  *     pointers are ordinary process memory.  The library never takes ownership of any argument.
- *   - counts are int64_t and must be in [0, 2^31 - 1].
+ *   - counts are int64_t and must be in [0, 2^31 - 4097] (32-bit particle indices inside the kernels).
  *   - every function returns an nb_status (int); nothing throws, aborts or prints.
  *   - functions that take a stream enqueue work on it and return without synchronising; results
  *     are valid once the stream has reached that point.  `stream` is a cudaStream_t passed as

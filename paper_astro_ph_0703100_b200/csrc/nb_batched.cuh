@@ -110,9 +110,9 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
     for (int k2 = 0; k2 < G; ++k2) {
         const int i0 = min(i_base + (2 * k2) * 32, i_hi - 1);
         const int i1 = min(i_base + (2 * k2 + 1) * 32, i_hi - 1);
-        nxi[k2] = pack2(-a.x_i[3 * i0 + 0], -a.x_i[3 * i1 + 0]);
-        nyi[k2] = pack2(-a.x_i[3 * i0 + 1], -a.x_i[3 * i1 + 1]);
-        nzi[k2] = pack2(-a.x_i[3 * i0 + 2], -a.x_i[3 * i1 + 2]);
+        nxi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 0], -a.x_i[3 * (size_t)i1 + 0]);
+        nyi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 1], -a.x_i[3 * (size_t)i1 + 1]);
+        nzi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 2], -a.x_i[3 * (size_t)i1 + 2]);
     }
     const float eps2 = a.eps2;
     const u64 eps2_2 = pack2(eps2, eps2);
@@ -211,9 +211,9 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
 #pragma unroll
                 for (int w = 1; w < WJ; ++w) s[c] += red[((w * K + k) * 4 + c) * 32 + lane];
             }
-            a.acc[3 * i + 0] = (float)s[0];
-            a.acc[3 * i + 1] = (float)s[1];
-            a.acc[3 * i + 2] = (float)s[2];
+            a.acc[3 * (size_t)i + 0] = (float)s[0];
+            a.acc[3 * (size_t)i + 1] = (float)s[1];
+            a.acc[3 * (size_t)i + 2] = (float)s[2];
             if (a.pot) a.pot[i] = -(float)s[3];
         }
     }

@@ -37,8 +37,8 @@ __global__ void __launch_bounds__(256) nb_pack_jv_kernel(const float* __restrict
                                                          const float* __restrict__ m_j, int n_j, float4* __restrict__ jp) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_j) return;
-    jp[2 * j + 0] = make_float4(x_j[3 * j + 0], x_j[3 * j + 1], x_j[3 * j + 2], m_j[j]);
-    jp[2 * j + 1] = make_float4(v_j[3 * j + 0], v_j[3 * j + 1], v_j[3 * j + 2], 0.0f);
+    jp[2 * (size_t)j + 0] = make_float4(x_j[3 * (size_t)j + 0], x_j[3 * (size_t)j + 1], x_j[3 * (size_t)j + 2], m_j[j]);
+    jp[2 * (size_t)j + 1] = make_float4(v_j[3 * (size_t)j + 0], v_j[3 * (size_t)j + 1], v_j[3 * (size_t)j + 2], 0.0f);
 }
 
 struct HermiteArgs {
@@ -163,8 +163,8 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
         const int i1 = min(i_base + (2 * k2 + 1) * 32, a.n_i - 1);
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            ni[k2][c] = pack2(-a.x_i[3 * i0 + c], -a.x_i[3 * i1 + c]);
-            ni[k2][3 + c] = pack2(-a.v_i[3 * i0 + c], -a.v_i[3 * i1 + c]);
+            ni[k2][c] = pack2(-a.x_i[3 * (size_t)i0 + c], -a.x_i[3 * (size_t)i1 + c]);
+            ni[k2][3 + c] = pack2(-a.v_i[3 * (size_t)i0 + c], -a.v_i[3 * (size_t)i1 + c]);
         }
     }
     const u64 eps2_2 = pack2(a.eps2, a.eps2);
@@ -267,8 +267,8 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
         if (a.S == 1) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                a.acc[3 * i + c] = (float)run[k][c];
-                a.jerk[3 * i + c] = (float)(run[k][3 + c] - 3.0 * run[k][6 + c]);   // jk = jk1 - jk2
+                a.acc[3 * (size_t)i + c] = (float)run[k][c];
+                a.jerk[3 * (size_t)i + c] = (float)(run[k][3 + c] - 3.0 * run[k][6 + c]);   // jk = jk1 - jk2
             }
             if (a.pot) a.pot[i] = -(float)run[k][9];
         } else {
@@ -295,8 +295,8 @@ __global__ void __launch_bounds__(128) nb_hermite_reduce_kernel(const double* __
     }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        acc[3 * i + c] = (float)s[c];
-        jerk[3 * i + c] = (float)(s[3 + c] - 3.0 * s[6 + c]);
+        acc[3 * (size_t)i + c] = (float)s[c];
+        jerk[3 * (size_t)i + c] = (float)(s[3 + c] - 3.0 * s[6 + c]);
     }
     if (pot) pot[i] = -(float)s[9];
 }

@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(256) nb_pack_j_kernel(const float* __restrict_
                                                         int n_j, float4* __restrict__ jp) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_j) return;
-    jp[j] = make_float4(x_j[3 * j + 0], x_j[3 * j + 1], x_j[3 * j + 2], m_j[j]);
+    jp[j] = make_float4(x_j[3 * (size_t)j + 0], x_j[3 * (size_t)j + 1], x_j[3 * (size_t)j + 2], m_j[j]);
 }
 
 // ---------------------------------------------------------------- a4: two i-particles x one j-particle
@@ -233,7 +233,7 @@ __global__ void __launch_bounds__(256) nb_coin_probe_kernel(const float* __restr
     __syncthreads();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;               // blockDim.x = 32 * K = one i-group
     if (i < n_i) {
-        const uint32_t cx = coin_canon(x_i[3 * i + 0]), cy = coin_canon(x_i[3 * i + 1]), cz = coin_canon(x_i[3 * i + 2]);
+        const uint32_t cx = coin_canon(x_i[3 * (size_t)i + 0]), cy = coin_canon(x_i[3 * (size_t)i + 1]), cz = coin_canon(x_i[3 * (size_t)i + 2]);
         uint32_t slot = coin_hash(cx, cy, cz) & mask;
         int step = 0;
         for (; step < kCoinMaxProbe; ++step) {
@@ -354,9 +354,9 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
     for (int k2 = 0; k2 < K / 2; ++k2) {
         const int i0 = min(i_base + (2 * k2) * 32, i_hi - 1);
         const int i1 = min(i_base + (2 * k2 + 1) * 32, i_hi - 1);
-        nxi[k2] = pack2(-a.x_i[3 * i0 + 0], -a.x_i[3 * i1 + 0]);
-        nyi[k2] = pack2(-a.x_i[3 * i0 + 1], -a.x_i[3 * i1 + 1]);
-        nzi[k2] = pack2(-a.x_i[3 * i0 + 2], -a.x_i[3 * i1 + 2]);
+        nxi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 0], -a.x_i[3 * (size_t)i1 + 0]);
+        nyi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 1], -a.x_i[3 * (size_t)i1 + 1]);
+        nzi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 2], -a.x_i[3 * (size_t)i1 + 2]);
     }
     const float eps2 = a.eps2;
     const u64 eps2_2 = pack2(eps2, eps2);
@@ -485,9 +485,9 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
             const int i = i_base + k * 32;
             if (i >= i_hi) continue;
             if (a.S == 1) {
-                a.acc[3 * i + 0] = (float)run[k][0];
-                a.acc[3 * i + 1] = (float)run[k][1];
-                a.acc[3 * i + 2] = (float)run[k][2];
+                a.acc[3 * (size_t)i + 0] = (float)run[k][0];
+                a.acc[3 * (size_t)i + 1] = (float)run[k][1];
+                a.acc[3 * (size_t)i + 2] = (float)run[k][2];
                 if (a.pot) a.pot[i] = -(float)run[k][3];
             } else {
                 a.partial[(size_t)blockIdx.y * a.n_i + i] = make_double4(run[k][0], run[k][1], run[k][2], run[k][3]);
@@ -524,9 +524,9 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
                 lo = __ldcg(p2); hi = __ldcg(p2 + 1);
                 sum.x += lo.x; sum.y += lo.y; sum.z += hi.x; sum.w += hi.y;
             }
-            a.acc[3 * i + 0] = (float)sum.x;
-            a.acc[3 * i + 1] = (float)sum.y;
-            a.acc[3 * i + 2] = (float)sum.z;
+            a.acc[3 * (size_t)i + 0] = (float)sum.x;
+            a.acc[3 * (size_t)i + 1] = (float)sum.y;
+            a.acc[3 * (size_t)i + 2] = (float)sum.z;
             if (a.pot) a.pot[i] = -(float)sum.w;
         }
     }
@@ -584,9 +584,9 @@ __global__ void __launch_bounds__(128) nb_reduce_kernel(const double4* __restric
         const double4 v = partial[(size_t)c * n_i + i];
         s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
     }
-    acc[3 * i + 0] = (float)s.x;
-    acc[3 * i + 1] = (float)s.y;
-    acc[3 * i + 2] = (float)s.z;
+    acc[3 * (size_t)i + 0] = (float)s.x;
+    acc[3 * (size_t)i + 1] = (float)s.y;
+    acc[3 * (size_t)i + 2] = (float)s.z;
     if (pot) pot[i] = -(float)s.w;
 }
 

@@ -126,8 +126,9 @@ int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool aliased) {
     if (e && e[0] == 'e') return nb::MODE_EXACT;
     if (eps2 < kSpecMinEps2) return nb::MODE_EXACT;
     if (e && e[0] == 's') return nb::MODE_SPEC;
-    if (e && e[0] == 'l') return nb::MODE_LIST;
+    if (e && e[0] == 'l' && n_j <= ((int64_t)1 << 29)) return nb::MODE_LIST;
     (void)aliased;
+    if (n_j > ((int64_t)1 << 29)) return nb::MODE_EXACT;           // the 32-bit hash table holds 2 n_j <= 2^30 slots
     return ((double)n_i * (double)n_j >= kListMinPairs) ? nb::MODE_LIST : nb::MODE_EXACT;
 }
 
@@ -191,7 +192,9 @@ int launch_force(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t s
     }
 }
 
-bool bad_count(int64_t n) { return n < 0 || n > (int64_t)INT32_MAX; }
+// counts stay 4096 below 2^31 so that tile-padded 32-bit particle indices cannot wrap inside the kernels
+constexpr int64_t kMaxCount = (int64_t)INT32_MAX - 4096;
+bool bad_count(int64_t n) { return n < 0 || n > kMaxCount; }
 
 // Coincidence pre-pass (MODE_LIST): hash table over the j-positions, one sorted j-segment list per
 // i-group of 32*K i-particles.  jp = packed j records, stride float4 each.  Three launches.

@@ -39,6 +39,7 @@ def test_argument_validation_happens_before_any_cuda_call():
     p = ctypes.addressof(buf)
     assert lib.nb_force(-1, p, 1, p, p, 0.1, p, None, None) == 1
     assert lib.nb_force(1, p, 2 ** 31, p, p, 0.1, p, None, None) == 1
+    assert lib.nb_force(2 ** 31 - 4096, p, 1, p, p, 0.1, p, None, None) == 1      # largest count is 2^31 - 4097
     assert lib.nb_force(1, None, 1, p, p, 0.1, p, None, None) == 1
     assert lib.nb_force(1, p, 1, p, None, 0.1, p, None, None) == 1
     assert lib.nb_force(1, p, 1, p, p, -0.5, p, None, None) == 1
@@ -64,7 +65,7 @@ def test_no_cpu_fallback_without_a_device():
 
 
 @pytest.mark.parametrize("n_i,n_j", [(1, 1), (1, 777), (31, 1000), (512, 65536), (2048, 2048), (65536, 65536),
-                                      (131072, 131072), (1048576, 1048576), (2 ** 31 - 1, 9)])
+                                      (131072, 131072), (1048576, 1048576), (2 ** 31 - 4097, 9)])
 def test_planner_invariants(n_i, n_j):
     p = nb.plan_query(n_i, n_j, 148)
     assert p["K"] in (2, 4, 8) and p["WI"] * p["WJ"] == 8 and p["WJ"] in (1, 2, 4, 8)
