@@ -167,6 +167,24 @@ int nb_force_eps_i(int64_t n_i, const float *x_i, const float *eps2_i,
                    void *stream);
 
 /*
+ * nb_cunbody_force / nb_cunbody_force_jerk_pot -- the paper's own library call, cunbody_api(p_xj, p_xi, p_fi, ni, nj)
+ * (PAPER.md:389, 420), for its two pipeline descriptions, run by the generalised pair kernel of section 4.5
+ * (include/nb_pipeline.cuh, where users instantiate their own pipelines the same way):
+ *
+ *   nb_cunbody_force           Fig. A.1 / A.3
+ *        p_xj [nj][4] = (x, y, z, m)       p_xi [ni][4] = (x, y, z, eps2)       p_fi [ni][3] = (ax, ay, az)
+ *   nb_cunbody_force_jerk_pot  Fig. A.2 / A.4; eps2 is the listing's constant 1/256^2
+ *        p_xj [nj][7] = (x, v, m)          p_xi [ni][6] = (x, v)                p_fi [ni][7] = (a, jerk, pot)
+ *
+ * All rows are DEVICE float arrays (the paper passes host doubles and copies inside; here the caller owns device
+ * memory, as for nb_force).  p_fi is overwritten, not accumulated into.  Coincident pairs add nothing (reading R1).
+ * These entry points run the listings as written (scalar FP32, any pipeline); nb_force / nb_force_eps_i /
+ * nb_force_jerk compute the same sums with the specialised kernels and are 2.2 - 2.4x faster (N = 131072).
+ */
+int nb_cunbody_force(const float *p_xj, const float *p_xi, float *p_fi, int64_t ni, int64_t nj, void *stream);
+int nb_cunbody_force_jerk_pot(const float *p_xj, const float *p_xi, float *p_fi, int64_t ni, int64_t nj, void *stream);
+
+/*
  * nb_force_batched -- many independent small (i-set, j-set) sub-problems of nb_force in ONE launch:
  * the use the paper shapes its interface for, a host tree code calling the force routine on
  * interaction lists of "several thousands" particles per group (PAPER.md:246 last sentence, section

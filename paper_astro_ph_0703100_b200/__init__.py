@@ -5,6 +5,8 @@ Python binding over it (argument marshalling only) plus the seeded workload gene
 """
 from .binding import (  # noqa: F401
     NBError,
+    cunbody_force,
+    cunbody_force_jerk_pot,
     force,
     force_batched,
     force_eps_i,

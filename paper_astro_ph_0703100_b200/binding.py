@@ -45,6 +45,9 @@ def lib() -> ctypes.CDLL:
         l.nb_leapfrog_kdk.restype = ci
         l.nb_force_jerk.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p, p]
         l.nb_force_jerk.restype = ci
+        for fn in (l.nb_cunbody_force, l.nb_cunbody_force_jerk_pot):
+            fn.argtypes = [p, p, p, i64, i64, p]
+            fn.restype = ci
         l.nb_pack_j.argtypes = [i64, p, p, p, p]
         l.nb_pack_j.restype = ci
         l.nb_force_packed.argtypes = [i64, p, i64, p, f32, p, p, p]
@@ -139,6 +142,29 @@ def force_jerk(x_i, v_i, x_j, v_j, m_j, eps2: float, acc_out=None, jerk_out=None
                                  None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
     _check(st, "nb_force_jerk")
     return acc_out, jerk_out, pot_out
+
+
+def _cunbody(fn_name: str, p_xj, p_xi, idim: int, jdim: int, fdim: int, p_fi, stream):
+    import torch
+    _dev_f32(p_xj, "p_xj", (jdim,)); _dev_f32(p_xi, "p_xi", (idim,))
+    ni, nj = p_xi.shape[0], p_xj.shape[0]
+    if p_fi is None:
+        p_fi = torch.empty((ni, fdim), dtype=torch.float32, device=p_xi.device)
+    _dev_f32(p_fi, "p_fi", (fdim,))
+    with torch.cuda.device(p_xi.device):
+        st = getattr(lib(), fn_name)(p_xj.data_ptr(), p_xi.data_ptr(), p_fi.data_ptr(), ni, nj, _stream_ptr(stream))
+    _check(st, fn_name)
+    return p_fi
+
+
+def cunbody_force(p_xj, p_xi, p_fi=None, stream=None):
+    """nb_cunbody_force: the paper's cunbody_api call for the Fig. A.3 pipeline.  p_xj [nj,4], p_xi [ni,4] -> p_fi [ni,3]."""
+    return _cunbody("nb_cunbody_force", p_xj, p_xi, 4, 4, 3, p_fi, stream)
+
+
+def cunbody_force_jerk_pot(p_xj, p_xi, p_fi=None, stream=None):
+    """nb_cunbody_force_jerk_pot: the Fig. A.4 pipeline.  p_xj [nj,7], p_xi [ni,6] -> p_fi [ni,7]."""
+    return _cunbody("nb_cunbody_force_jerk_pot", p_xj, p_xi, 6, 7, 7, p_fi, stream)
 
 
 def pack_j(x_j, m_j, xm_out, stream=None):

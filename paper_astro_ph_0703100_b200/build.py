@@ -10,7 +10,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnbody_b200.so")
 SOURCES = ["nbody_b200.cu"]
-DEPS = ["nbody_b200.cu", "nb_kernels.cuh", "nb_hermite.cuh", "nb_batched.cuh", "nb_plan.h", os.path.join(ROOT, "include", "nbody_b200.h")]
+DEPS = ["nbody_b200.cu", "nb_kernels.cuh", "nb_hermite.cuh", "nb_batched.cuh", "nb_pipelines.cuh", os.path.join(ROOT, "include", "nb_pipeline.cuh"), "nb_plan.h", os.path.join(ROOT, "include", "nbody_b200.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -1,0 +1,54 @@
+// nb_pipelines.cuh -- the paper's two pipeline descriptions, statement by statement, as pipelines of the
+// generalised kernel (include/nb_pipeline.cuh).  The only addition to the listings is the coincident-pair rule
+// (reading R1): a pair whose three position differences are exactly zero adds nothing.
+#pragma once
+#include "../../include/nb_pipeline.cuh"
+
+namespace nb {
+
+// Fig. A.1 / A.3: IDIM 4 = (x, y, z, eps2), JDIM 4 = (x, y, z, m), FDIM 3 = (ax, ay, az)
+struct PipelineForceA3 {
+    static constexpr int IDIM = 4, JDIM = 4, FDIM = 3;
+    static __device__ __forceinline__ void pair(const float* INPUT_I, const float* INPUT_J, float* OUTPUT) {
+        const float xi = INPUT_I[0], yi = INPUT_I[1], zi = INPUT_I[2], eps2 = INPUT_I[3];
+        const float xj = INPUT_J[0], yj = INPUT_J[1], zj = INPUT_J[2], mj = INPUT_J[3];
+        const float dx = xj - xi, dy = yj - yi, dz = zj - zi;
+        if (dx == 0.0f && dy == 0.0f && dz == 0.0f) return;                                 // reading R1
+        const float dx2 = dx * dx, dy2 = dy * dy, dz2 = dz * dz;
+        const float r2 = (dx2 + dy2) + (dz2 + eps2);
+        const float r1i = rsqrtf(r2);
+        const float r2i = r1i * r1i;
+        const float r3i = r2i * r1i;
+        const float mr3i = mj * r3i;
+        OUTPUT[0] += mr3i * dx;
+        OUTPUT[1] += mr3i * dy;
+        OUTPUT[2] += mr3i * dz;
+    }
+};
+
+// Fig. A.2 / A.4: IDIM 6 = (x, v), JDIM 7 = (x, v, m), FDIM 7 = (a, jerk, pot);
+// eps2 is the listing's constant 1/(256*256).
+struct PipelineForceJerkPotA4 {
+    static constexpr int IDIM = 6, JDIM = 7, FDIM = 7;
+    static __device__ __forceinline__ void pair(const float* INPUT_I, const float* INPUT_J, float* OUTPUT) {
+        const float eps2 = 1.0f / (256.0f * 256.0f);
+        const float dx_0 = INPUT_J[0] - INPUT_I[0], dx_1 = INPUT_J[1] - INPUT_I[1], dx_2 = INPUT_J[2] - INPUT_I[2];
+        if (dx_0 == 0.0f && dx_1 == 0.0f && dx_2 == 0.0f) return;                           // reading R1
+        const float mj = INPUT_J[6];
+        const float r2 = dx_0 * dx_0 + dx_1 * dx_1 + dx_2 * dx_2 + eps2;
+        const float r1i = rsqrtf(r2);
+        const float r2i = r1i * r1i, r3i = r1i * r2i, r5i = r2i * r3i;
+        const float mr5i = mj * r5i, mf = mr5i * r2, pot = mf * r2;
+        const float dv_0 = INPUT_J[3] - INPUT_I[3], dv_1 = INPUT_J[4] - INPUT_I[4], dv_2 = INPUT_J[5] - INPUT_I[5];
+        const float mf3a = 3.0f * mr5i * (dx_0 * dv_0 + dx_1 * dv_1 + dx_2 * dv_2);
+        OUTPUT[0] += mf * dx_0;
+        OUTPUT[1] += mf * dx_1;
+        OUTPUT[2] += mf * dx_2;
+        OUTPUT[3] += mf * dv_0 - mf3a * dx_0;
+        OUTPUT[4] += mf * dv_1 - mf3a * dx_1;
+        OUTPUT[5] += mf * dv_2 - mf3a * dx_2;
+        OUTPUT[6] -= pot;
+    }
+};
+
+}  // namespace nb

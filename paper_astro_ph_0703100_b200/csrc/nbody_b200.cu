@@ -16,6 +16,7 @@
 #include "nb_kernels.cuh"
 #include "nb_hermite.cuh"
 #include "nb_batched.cuh"
+#include "nb_pipelines.cuh"
 #include "nb_plan.h"
 
 #define NB_VERSION 100
@@ -50,6 +51,7 @@ struct Workspace {
     void* tickets = nullptr;   size_t tickets_bytes = 0;   // fused second pass: one counter per i-tile, zero between calls
     void* coin = nullptr;      size_t coin_bytes = 0;      // coincidence pre-pass: flag | lists | hash table
     void* tiles = nullptr;     size_t tiles_bytes = 0;     // batched calls: first CTA of every sub-problem
+    void* pipe = nullptr;      size_t pipe_bytes = 0;      // generalised kernel: [S][n_i][FDIM] double
     void* jp2 = nullptr;       size_t jp2_bytes = 0;       // force + jerk: 32-byte j records
     void* hpartial = nullptr;  size_t hpartial_bytes = 0;  // force + jerk: [S][n_i][10] double
 };
@@ -659,6 +661,47 @@ int nb_force_eps_i(int64_t n_i, const float* x_i, const float* eps2_i, int64_t n
                       eps2_i ? eps2_i : &dummy);
 }
 
+}  // extern "C"
+
+namespace {
+// the cunbody_api call for a pipeline P on device rows
+template <class P>
+int cunbody_call(const float* p_xj, const float* p_xi, float* p_fi, int64_t ni, int64_t nj, cudaStream_t stream) {
+    t_launches = 0;
+    if (bad_count(ni) || bad_count(nj)) return NB_ERR_INVALID_VALUE;
+    if (ni > 0 && (!p_xi || !p_fi)) return NB_ERR_INVALID_VALUE;
+    if (nj > 0 && !p_xj) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (ni == 0) return NB_OK;
+    Workspace* ws;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        ws = &g_ws[std::make_pair(dev, stream)];
+    }
+    const size_t need = nj > 0 ? nb::pipeline_workspace_bytes<P>(ni, nj, info.sm_count) : 0;
+    if (need) {
+        rc = ensure(&ws->pipe, &ws->pipe_bytes, need, stream);
+        if (rc != NB_OK) return rc;
+    }
+    NB_CUDA(nb::pipeline_run<P>(p_xj, p_xi, p_fi, ni, nj, ws->pipe, info.sm_count, stream));
+    t_launches = (nj > 0) ? (nb::pipeline_chunks(ni, nj, info.sm_count) > 1 ? 2 : 1) : 0;
+    return NB_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int nb_cunbody_force(const float* p_xj, const float* p_xi, float* p_fi, int64_t ni, int64_t nj, void* stream) {
+    return cunbody_call<nb::PipelineForceA3>(p_xj, p_xi, p_fi, ni, nj, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int nb_cunbody_force_jerk_pot(const float* p_xj, const float* p_xi, float* p_fi, int64_t ni, int64_t nj, void* stream) {
+    return cunbody_call<nb::PipelineForceJerkPotA4>(p_xj, p_xi, p_fi, ni, nj, reinterpret_cast<cudaStream_t>(stream));
+}
+
 int nb_pack_j(int64_t n_j, const float* x_j, const float* m_j, float* xm_out, void* stream) {
     t_launches = 0;
     if (bad_count(n_j)) return NB_ERR_INVALID_VALUE;
@@ -826,6 +869,7 @@ int nb_release_workspace(void) {
             if (it->second.tickets) (void)cudaFree(it->second.tickets);
             if (it->second.jp2) (void)cudaFree(it->second.jp2);
             if (it->second.tiles) (void)cudaFree(it->second.tiles);
+            if (it->second.pipe) (void)cudaFree(it->second.pipe);
             if (it->second.hpartial) (void)cudaFree(it->second.hpartial);
             it = g_ws.erase(it);
         } else {

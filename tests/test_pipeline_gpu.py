@@ -1,0 +1,85 @@
+"""The generalised pair kernel (section 4.5; include/nb_pipeline.cuh) running the paper's two
+pipeline descriptions through the paper's own call shape cunbody_api(p_xj, p_xi, p_fi, ni, nj),
+against the CPU oracle.  Same tolerances as the specialised kernels."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_astro_ph_0703100_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def nb():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    import paper_astro_ph_0703100_b200 as nb_
+    nb_.lib()
+    return nb_
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def rows_a3(x_i, eps2_i, x_j, m_j):
+    """Fig. A.1 packing loops: p_xi[i] = (x, y, z, eps2), p_xj[j] = (x, y, z, m)."""
+    return np.concatenate([x_i, eps2_i[:, None]], 1), np.concatenate([x_j, m_j[:, None]], 1)
+
+
+def rows_a4(x_i, v_i, x_j, v_j, m_j):
+    """Fig. A.2 packing loop: p_xi[i] = (x, v), p_xj[j] = (x, v, m)."""
+    return np.concatenate([x_i, v_i], 1), np.concatenate([x_j, v_j, m_j[:, None]], 1)
+
+
+@pytest.mark.parametrize("n_i,n_j", [(3000, 3000), (1, 777), (31, 1000), (1025, 2051), (70000, 300), (513, 40000)])
+def test_fig_a3_pipeline_matches_oracle(nb, n_i, n_j):
+    import torch
+    w = wl.plummer_workload(max(n_i, n_j), 1.0 / 64, seed=41)
+    rng = np.random.default_rng(n_i)
+    x_j, m_j = w.x_j[:n_j], (w.m_j[:n_j] * rng.uniform(0.5, 2.0, n_j)).astype(np.float32)
+    x_i = w.x_j[:n_i] if n_i <= n_j else rng.normal(size=(n_i, 3)).astype(np.float32)   # subsets coincide with their j
+    e2 = (2.0 ** rng.integers(-18, -6, n_i)).astype(np.float32)
+    p_xi, p_xj = rows_a3(x_i, e2, x_j, m_j)
+    p_fi = nb.cunbody_force(dev(p_xj), dev(p_xi))
+    torch.cuda.synchronize()
+    ra, _ = oracle.force_eps_i(x_i, e2, x_j, m_j)
+    e = oracle.error_metrics(p_fi.cpu().numpy(), ra)
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4, e
+
+
+@pytest.mark.parametrize("n_i,n_j", [(2048, 2048), (100, 5000), (4097, 777)])
+def test_fig_a4_pipeline_matches_oracle(nb, n_i, n_j):
+    import torch
+    w = wl.plummer_workload(max(n_i, n_j), 1.0 / 256, seed=42, with_velocities=True)
+    x_j, v_j, m_j = w.x_j[:n_j], w.v[:n_j], w.m_j[:n_j]
+    x_i, v_i = w.x_j[:n_i], w.v[:n_i] * np.float32(1.5)
+    p_xi, p_xj = rows_a4(x_i, v_i, x_j, v_j, m_j)
+    p_fi = nb.cunbody_force_jerk_pot(dev(p_xj), dev(p_xi)).cpu().numpy()
+    torch.cuda.synchronize()
+    ra, rj, rp = oracle.force_jerk(x_i, v_i, x_j, v_j, m_j, np.float32(1.0 / 65536.0))     # the listing's eps2
+    e = oracle.error_metrics(p_fi[:, 0:3], ra, p_fi[:, 6], rp)
+    ej = oracle.error_metrics(p_fi[:, 3:6], rj)
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and e["pot_rms"] <= 1e-5, e
+    assert ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-4, ej
+
+
+def test_agrees_with_the_specialised_kernels_and_edge_sizes(nb):
+    import torch
+    w = wl.plummer_workload(5000, 1.0 / 64, seed=43)
+    e2 = np.full(5000, w.eps2, np.float32)
+    p_xi, p_xj = rows_a3(w.x_j, e2, w.x_j, w.m_j)
+    a_gen = nb.cunbody_force(dev(p_xj), dev(p_xi))
+    a_gen2 = nb.cunbody_force(dev(p_xj), dev(p_xi))
+    a_spec, _ = nb.force(dev(w.x_j), dev(w.x_j), dev(w.m_j), w.eps2)
+    torch.cuda.synchronize()
+    assert torch.equal(a_gen, a_gen2)                                           # reproducible
+    assert torch.allclose(a_gen, a_spec, rtol=2e-5, atol=1e-6)
+    z = torch.zeros((0, 4), device="cuda")
+    out = nb.cunbody_force(z, dev(p_xi))                                        # nj = 0: zero-filled
+    torch.cuda.synchronize()
+    assert out.shape == (5000, 3) and not out.any()
+    assert nb.cunbody_force(dev(p_xj), z).shape == (0, 3)                       # ni = 0
+    assert nb.lib().nb_cunbody_force(None, None, None, 5, 5, None) == 1
