@@ -390,7 +390,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
     // MODE_LIST: ascending j-segments that hold a partner of this warp's i-particles (warp-uniform)
     const int* coin = nullptr;
     int coin_cnt = 0, coin_pos = 0, coin_next = 0x7fffffff;
-    if (MODE == MODE_LIST) {
+    if (MODE == MODE_LIST && a.coin_lists != nullptr) {               // nullptr: no block needs the mask (see nbody_b200.cu)
         coin = a.coin_lists + (size_t)(blockIdx.x * WI + wi) * (1 + kCoinCap);
         coin_cnt = (*a.coin_flag != 0) ? -1 : coin[0];
         if (coin_cnt > 0) coin_next = coin[1];

@@ -293,7 +293,13 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.n_batch = 0;
     int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2, !packed_j && x_i == x_j);
     if (eps2_i && mode == nb::MODE_SPEC) mode = nb::MODE_EXACT;      // the values are on the device: no threshold test
-    if (mode == nb::MODE_LIST) {
+    // Without phi no pair needs a mask when eps2 >= 2^-40: an unmasked coincident pair adds m u^3 * (+-0) = +-0 to a
+    // (only phi would get m / eps), so a_i is bit for bit the masked loop's.  The list-mode kernel then runs with an
+    // empty list: no pre-pass, the untested loop everywhere (nb_leapfrog_kdk: every evaluation but the last).
+    const bool a_only = !pot_out && !eps2_i && eps2 >= kSpecMinEps2 && !std::getenv("NB_MASK");
+    if (a_only) {
+        rc = (plan.K == 8) ? launch_force_nophi(args, plan, stream) : launch_force<nb::MODE_LIST>(args, plan, stream);
+    } else if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, jp, 1, stream, &args.coin_lists, &args.coin_flag);
         if (rc != NB_OK) return rc;
         if (eps2_i) rc = launch_force<nb::MODE_LIST, true>(args, plan, stream);

@@ -367,3 +367,17 @@ def test_cuda_graph_capture_and_replay(nb, n, mode, monkeypatch):
     ra, rp = oracle.force(w2.x_j, w2.x_j, w2.m_j, w2.eps2)
     check_parity(acc.cpu().numpy(), pot.cpu().numpy(), ra, rp, f"graph replay {n} {mode}")
     assert not torch.equal(ref[0], acc)
+
+
+@pytest.mark.parametrize("n", [700, 3000, 40000])
+def test_acceleration_only_calls_need_no_mask(nb, n, monkeypatch):
+    """pot_out = NULL, eps2 >= 2^-40: the untested loop runs everywhere (no pre-pass); an unmasked coincident pair adds
+    +-0 to a, so the result is the masked kernel's bit for bit -- self pairs, duplicates, -0 / subnormal coordinates."""
+    w = wl.plummer_workload(n, 1.0 / 64, seed=27)
+    x = w.x_j.copy()
+    x[5] = x[n - 1]; x[n // 2] = x[5]
+    x[7] = (0.0, 0.0, 0.0); x[9] = (-0.0, 1e-41, 0.0)
+    a_free, p_free = gpu_force(nb, x, x, w.m_j, w.eps2, want_pot=False, alias=True)
+    monkeypatch.setenv("NB_MASK", "exact")
+    a_mask, _ = gpu_force(nb, x, x, w.m_j, w.eps2, alias=True)
+    assert p_free is None and np.array_equal(a_free, a_mask)
