@@ -157,6 +157,9 @@ def reference_arm(args, wl):
     elif args.op == "jerk":
         w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
         name = "row f1 (H1): plummer N=131072 with velocities, one force+jerk+phi evaluation"
+    elif args.op == "cunbody":
+        w = wl.config(1)
+        name = "row f3 (G1): configs[1]'s particles, Fig. A.3 pipeline (oracle force on a sample)"
     elif args.op == "leapfrog":
         w = wl.config(4)
         name = "BASELINE.json configs[4] (C4): force evaluations of the KDK integration, N=65536 (oracle force on a sample)"
@@ -204,6 +207,9 @@ OPS = {
     # continues the integration (the first call also pays the initial force evaluation)
     # (the integration needs phi only at the final time: 100 of the 101 evaluations of a call run the 12-instruction
     #  loop without it, so the algorithmic count for the roofline is 12 per interaction here)
+    # row f3: the paper's cunbody_api call for its Fig. A.3 pipeline through the generalised kernel (scalar FP32;
+    # the listing has no potential: 12 FP32-pipe instructions per interaction)
+    "cunbody": {"inst": 12, "kernel": "pipeline_kernel<PipelineForceA3> (generalised kernel, row f3)", "flops": (20, 38)},
     "leapfrog": {"inst": 12, "kernel": "nb_force_kernel<PHI=false> inside nb_leapfrog_kdk (row a8)", "flops": (20, 38)},
 }
 LEAPFROG_KDK_PER_CALL = 100
@@ -234,6 +240,15 @@ class Problem:
             self.host = [w.x_j, w.v, w.m_j]
             self.n_out = w.n_j
             self.kdk_done = 0
+        elif op == "cunbody":
+            w = wl.config(1)
+            self.w, self.pairs = w, float(w.pairs)
+            self.name = (f"row f3 (G1): configs[1]'s particles as the paper's rows p_xi[n][4] = (x,y,z,eps2), p_xj[n][4] = "
+                         f"(x,y,z,m) (Fig. A.1), n={w.n_j}, eps2={w.eps2:.6g}; one nb_cunbody_force call (Fig. A.3 pipeline, no phi)")
+            p_xi = np.concatenate([w.x_j, np.full((w.n_j, 1), w.eps2, np.float32)], axis=1).astype(np.float32)
+            p_xj = np.concatenate([w.x_j, w.m_j[:, None]], axis=1).astype(np.float32)
+            self.host = [np.ascontiguousarray(p_xj), np.ascontiguousarray(p_xi)]
+            self.n_out = w.n_j
         elif op == "jerk":
             w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
             self.w, self.pairs = w, float(w.n_i) * float(w.n_j)
@@ -254,7 +269,8 @@ class Problem:
         self.outs = [torch.empty((n, 3), dtype=torch.float32, device="cuda")]
         if op == "jerk":
             self.outs.append(torch.empty((n, 3), dtype=torch.float32, device="cuda"))
-        self.outs.append(torch.empty((n,), dtype=torch.float32, device="cuda"))
+        if op != "cunbody":
+            self.outs.append(torch.empty((n,), dtype=torch.float32, device="cuda"))
         self.h_outs = [torch.empty(o.shape, dtype=torch.float32).pin_memory() for o in self.outs]
         self.h2d = int(sum(a.nbytes for a in self.host))
         self.d2h = int(sum(o.numel() * 4 for o in self.outs))
@@ -266,6 +282,8 @@ class Problem:
             xj, mj = t[0], t[1]
             xi = xj if w.x_i is None else t[2]
             nb.force(xi, xj, mj, w.eps2, acc_out=self.outs[0], pot_out=self.outs[1])
+        elif self.op == "cunbody":
+            nb.cunbody_force(t[0], t[1], self.outs[0])
         elif self.op == "leapfrog":
             nb.leapfrog_kdk(t[0], t[1], t[2], w.eps2, w.dt, LEAPFROG_KDK_PER_CALL, acc_io=self.outs[0], pot_out=self.outs[1])
             if t is self.dev:
@@ -300,6 +318,8 @@ class Problem:
             return "nb_force_host (pinned host buffers)"
         if self.op == "jerk":
             return "nb_force_jerk_host (pinned host buffers)"
+        if self.op == "cunbody":
+            return "pinned host rows -> cudaMemcpyAsync -> nb_cunbody_force -> cudaMemcpyAsync -> pinned host"
         if self.op == "leapfrog":
             return "pinned host (x, v, m) -> cudaMemcpyAsync -> nb_leapfrog_kdk (100 KDK steps) -> cudaMemcpyAsync of a, phi -> pinned host"
         return f"pinned host tensors -> cudaMemcpyAsync -> nb_{'force_jerk' if self.op == 'jerk' else 'force_batched'} -> cudaMemcpyAsync -> pinned host"
@@ -307,6 +327,8 @@ class Problem:
     def plan(self, sm_count):
         if self.op == "force":
             return self.nb.plan_query(self.w.n_i, self.w.n_j, sm_count)
+        if self.op == "cunbody":
+            return {"cta": "256 threads x 2 i-records, 128-record j tiles, j-range split over S CTAs + second pass"}
         if self.op == "leapfrog":
             return self.nb.plan_query(self.w.n_j, self.w.n_j, sm_count)
         if self.op == "jerk":
@@ -317,7 +339,7 @@ class Problem:
 def oracle_rate_op(op, w, target_seconds, rng_seed=0):
     """CPU oracle, as it stands, on a bounded sample of the op's workload: (pairs/s, cores, sample)."""
     import oracle
-    if op in ("force", "leapfrog"):
+    if op in ("force", "leapfrog", "cunbody"):
         return oracle_rate(w, target_seconds, rng_seed)
     cores = oracle.num_threads()
     rng = np.random.default_rng(rng_seed)

@@ -692,7 +692,17 @@ int cunbody_call(const float* p_xj, const float* p_xi, float* p_fi, int64_t ni, 
         rc = ensure(&ws->pipe, &ws->pipe_bytes, need, stream);
         if (rc != NB_OK) return rc;
     }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (t_profile) {                                                   // brackets the pair kernel and its second pass
+        NB_CUDA(cudaEventCreate(&e0));
+        NB_CUDA(cudaEventCreate(&e1));
+        NB_CUDA(cudaEventRecord(e0, stream));
+    }
     NB_CUDA(nb::pipeline_run<P>(p_xj, p_xi, p_fi, ni, nj, ws->pipe, info.sm_count, stream));
+    if (t_profile) {
+        NB_CUDA(cudaEventRecord(e1, stream));
+        t_events.emplace_back(e0, e1);
+    }
     t_launches = (nj > 0) ? (nb::pipeline_chunks(ni, nj, info.sm_count) > 1 ? 2 : 1) : 0;
     return NB_OK;
 }
