@@ -8,21 +8,16 @@
 //   - K per CTA at run time: a tile that holds n_i <= 64 / 128 / 192 / 256 particles runs 1 / 2 / 3 / 4 packed groups
 //     (tile_sweep<2 KG>), so the padding of a sub-problem is at most 63 idle lanes;
 //   - coincident pairs (reading R1): interaction lists contain the group's own members, so EVERY
-//     sub-problem has them, bunched in a few 256-j blocks of ONE warp.  MODE_SPEC runs the flag-only loop
-//     (MASK_SPEC); a block that raised the flag is not added but DEFERRED, and after the main loop all 8 warps redo
-//     the deferred blocks together with the exact mask, 32 j-particles each, reading them from global memory.
-//     The deferred list is sorted, so the summation order -- and the result, bit for bit -- does not depend on
-//     which warp finished first.  MODE_EXACT masks every pair in the main loop.
-// Measured on the T1 tree lists: G = 1 with MODE_EXACT is the fastest combination (57 % of roofline:
-// 83 % lane use x 69 % loop efficiency, the masked loop's ceiling being 72 %); with one packed group per warp the
-// flag-only loop is latency-bound, not ALU-bound, so MODE_SPEC + deferred redo (55 %) does not pay and is kept as
-// NB_MASK=spec only; G = 2 / 4 reach 53 / 51 %.
+//     sub-problem has them; MASKED = true masks every pair in the loop.  MASKED = false (phi not wanted and
+//     eps2 >= 2^-40: an unmasked coincident pair adds +-0 to a) runs the untested loop.
+// Measured on the T1 tree lists: G = 1 is the fastest shape (57 % of roofline: 83 % lane use x 69 % loop
+// efficiency, the masked loop's ceiling being 72 %); G = 2 / 4 reach 53 / 51 %.  A flag-only loop with the flagged
+// blocks redone by all 8 warps together was tried and removed (55 %: with one packed group per warp the loop is
+// latency-bound, so not paying for the mask buys nothing).
 #pragma once
 #include "nb_kernels.cuh"
 
 namespace nb {
-
-constexpr int kBatchDefer = 64;      // deferred blocks per CTA before a warp redoes its block on its own
 
 template <int KG, int G>
 __device__ __forceinline__ const u64 (&first_groups(const u64 (&arr)[G]))[KG] {
@@ -34,26 +29,26 @@ __device__ __forceinline__ u64 (&first_groups(u64 (&arr)[G]))[KG] {
 }
 
 template <int KG, int MASK, int G>
-__device__ __forceinline__ bool sweep_groups(const float4* __restrict__ sp, int np, const u64 (&nxi)[G], const u64 (&nyi)[G],
-                                             const u64 (&nzi)[G], u64 eps2_2, float eps2, u64 (&pax)[G], u64 (&pay)[G],
+__device__ __forceinline__ void sweep_groups(const float4* __restrict__ sp, int np, const u64 (&nxi)[G], const u64 (&nyi)[G],
+                                             const u64 (&nzi)[G], u64 eps2_2, u64 (&pax)[G], u64 (&pay)[G],
                                              u64 (&paz)[G], u64 (&pph)[G]) {
-    return tile_sweep<2 * KG, MASK, false>(sp, np, first_groups<KG, G>(nxi), first_groups<KG, G>(nyi), first_groups<KG, G>(nzi),
-                                           eps2_2, eps2, first_groups<KG, G>(pax), first_groups<KG, G>(pay),
-                                           first_groups<KG, G>(paz), first_groups<KG, G>(pph),
-                                           first_groups<KG, G>(nxi) /* e2: unused */);
+    tile_sweep<2 * KG, MASK, false, MASK == MASK_EXACT>(sp, np, first_groups<KG, G>(nxi), first_groups<KG, G>(nyi),
+                                                        first_groups<KG, G>(nzi), eps2_2, first_groups<KG, G>(pax),
+                                                        first_groups<KG, G>(pay), first_groups<KG, G>(paz),
+                                                        first_groups<KG, G>(pph), first_groups<KG, G>(nxi) /* e2: unused */);
 }
 
 // kg (1..G) active packed groups, uniform over the CTA; the inactive groups' partial sums stay zero
 template <int MASK, int G>
-__device__ __forceinline__ bool sweep_dyn(int kg, const float4* __restrict__ sp, int np, const u64 (&nxi)[G], const u64 (&nyi)[G],
-                                          const u64 (&nzi)[G], u64 eps2_2, float eps2, u64 (&pax)[G], u64 (&pay)[G],
+__device__ __forceinline__ void sweep_dyn(int kg, const float4* __restrict__ sp, int np, const u64 (&nxi)[G], const u64 (&nyi)[G],
+                                          const u64 (&nzi)[G], u64 eps2_2, u64 (&pax)[G], u64 (&pay)[G],
                                           u64 (&paz)[G], u64 (&pph)[G]) {
 #pragma unroll
     for (int k = 0; k < G; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
-    if (G >= 4 && kg >= 4) return sweep_groups<(G >= 4 ? 4 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
-    if (G >= 3 && kg == 3) return sweep_groups<(G >= 3 ? 3 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
-    if (G >= 2 && kg == 2) return sweep_groups<(G >= 2 ? 2 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
-    return sweep_groups<1, MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
+    if (G >= 4 && kg >= 4) sweep_groups<(G >= 4 ? 4 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+    else if (G >= 3 && kg == 3) sweep_groups<(G >= 3 ? 3 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+    else if (G >= 2 && kg == 2) sweep_groups<(G >= 2 ? 2 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+    else sweep_groups<1, MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
 }
 
 template <int G>
@@ -70,17 +65,14 @@ __device__ __forceinline__ void add_partials(double (&run)[2 * G][4], const u64 
 }
 
 // G = packed groups of 64 i-particles a CTA can hold (tile = 64 G); STAGES = ring depth per warp.
-template <int MODE, int G, int STAGES>
+template <bool MASKED, int G, int STAGES>
 __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const ForceArgs a) {
-    static_assert(MODE == MODE_SPEC || MODE == MODE_EXACT, "batched calls: speculative with deferred redo, or masked");
     static_assert(G >= 1 && G <= 4, "1 .. 4 packed groups");
-    constexpr int K = 2 * G, WJ = 8, TJ = 256, SUB = 256, kBatchTile = 64 * G;
+    constexpr int K = 2 * G, WJ = 8, TJ = 256, kBatchTile = 64 * G;
     constexpr int RING_BYTES = STAGES * TJ * 16;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     unsigned char* rings = smem_raw;                                   // [WJ][STAGES][TJ] float4
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + WJ * RING_BYTES);   // full[WJ][STAGES]
-    __shared__ int2 s_def[kBatchDefer];                                // deferred blocks: (first global j, count)
-    __shared__ int s_ndef;
 
     if ((int)blockIdx.x >= a.tile_start[a.n_batch]) return;            // the grid is an upper bound
     const int b = a.cta_batch[blockIdx.x];
@@ -96,7 +88,6 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
         for (int s = 0; s < STAGES; ++s) mbar_init(full0 + 8 * s, 1);
         mbar_fence_init();
     }
-    if (threadIdx.x == 0) s_ndef = 0;
 
     const int j_begin = jr_lo + (int)((long long)jr_n * wj / WJ);
     const int j_end = jr_lo + (int)((long long)jr_n * (wj + 1) / WJ);
@@ -114,9 +105,8 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
         nyi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 1], -a.x_i[3 * (size_t)i1 + 1]);
         nzi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 2], -a.x_i[3 * (size_t)i1 + 2]);
     }
-    const float eps2 = a.eps2;
-    const u64 eps2_2 = pack2(eps2, eps2);
-    __syncthreads();                                                   // barriers and s_ndef initialised
+    const u64 eps2_2 = pack2(a.eps2, a.eps2);
+    __syncthreads();                                                   // barriers initialised
 
     // each warp is its own producer; a ring slot is refilled by the warp that has just finished reading it
     if (lane == 0) {
@@ -138,24 +128,8 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
         const int nc = min(TJ, n_sub - t * TJ);                        // TJ == SUB: one Eq. (2) block per tile
         const float4* sp = reinterpret_cast<const float4*>(rings + wj * RING_BYTES + slot * TJ * 16);
         u64 pax[G], pay[G], paz[G], pph[G];
-        bool add = true;
-        if (MODE == MODE_SPEC) {
-            const bool hit = sweep_dyn<MASK_SPEC, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
-            if (__any_sync(0xffffffffu, hit)) {                        // this block may hold a coincident pair
-                int idx = 0;
-                if (lane == 0) idx = atomicAdd(&s_ndef, 1);
-                idx = __shfl_sync(0xffffffffu, idx, 0);
-                if (idx < kBatchDefer) {
-                    if (lane == 0) s_def[idx] = make_int2(j_begin + t * TJ, nc);
-                    add = false;                                       // redone by all warps after the main loop
-                } else {
-                    (void)sweep_dyn<MASK_EXACT, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
-                }
-            }
-        } else {
-            (void)sweep_dyn<MASK_EXACT, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
-        }
-        if (add) add_partials<G>(run, pax, pay, paz, pph);
+        sweep_dyn<MASKED ? MASK_EXACT : MASK_NONE, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+        add_partials<G>(run, pax, pay, paz, pph);
         __syncwarp();                                                  // every lane is done with the slot
         if (lane == 0 && t + STAGES < n_tiles) {
             const int tn = t + STAGES;
@@ -165,32 +139,7 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
         }
     }
 
-    __syncthreads();                                                   // main loops done: rings are free, s_def complete
-    if (MODE == MODE_SPEC) {
-        const int n_def = min(s_ndef, kBatchDefer);
-        if (n_def > 1) {                                               // fixed order whatever the arrival order was
-            if (threadIdx.x == 0) {
-                for (int p = 1; p < n_def; ++p) {
-                    const int2 v = s_def[p];
-                    int q = p - 1;
-                    while (q >= 0 && s_def[q].x > v.x) { s_def[q + 1] = s_def[q]; --q; }
-                    s_def[q + 1] = v;
-                }
-            }
-            __syncthreads();
-        }
-        for (int d = 0; d < n_def; ++d) {
-            const int2 blk = s_def[d];
-            const int p0 = wj * (SUB / WJ);                            // this warp's 32 j-particles of the block
-            const int pn = min(SUB / WJ, blk.y - p0);
-            if (pn > 0) {
-                u64 pax[G], pay[G], paz[G], pph[G];
-                (void)sweep_dyn<MASK_EXACT, G>(kg, a.jp + blk.x + p0, pn, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph);
-                add_partials<G>(run, pax, pay, paz, pph);
-            }
-        }
-        __syncthreads();
-    }
+    __syncthreads();                                                   // main loops done: the rings are free
 
     // fixed-order sum over the 8 warps through shared memory (the rings are free)
     double* red = reinterpret_cast<double*>(smem_raw);                 // [WJ][K][4][32]

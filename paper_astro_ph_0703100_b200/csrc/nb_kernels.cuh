@@ -111,19 +111,18 @@ __global__ void __launch_bounds__(256) nb_pack_j_kernel(const float* __restrict_
 // Coincident pairs (reading R1: all three differences exactly zero => the pair adds nothing).
 //   MASK_EXACT : test (dx | dy | dz) == 0 bitwise and send r2 to +inf, so rsqrt gives +0 and every
 //                term of the pair vanishes; 2 ALU-pipe instructions with 4 register reads per pair.
-//   MASK_SPEC  : no masking; only records whether r2 == eps2 occurred (a necessary condition for
-//                coincidence, since fma(0, 0, eps2) == eps2): 1 ALU instruction, 1 register read per
-//                pair.  The caller recomputes the whole tile with MASK_EXACT when the flag is set, so
-//                the stored result is always the MASK_EXACT one.  Requires eps2 > 0.
-//   MASK_NONE  : no masking and no flag; only valid for a block of j-particles that is known (from the
-//                coincidence lists built by nb_coin_probe_kernel) to hold no partner of this warp's
-//                i-particles, where it gives bit for bit what MASK_EXACT gives.  13 + 1 instructions.
-enum { MASK_EXACT = 0, MASK_SPEC = 1, MASK_NONE = 2 };
+//   MASK_NONE  : no masking; valid for a block of j-particles that is known (from the coincidence lists built
+//                by nb_coin_probe_kernel) to hold no partner of this warp's i-particles, where it gives bit for
+//                bit what MASK_EXACT gives -- and everywhere when phi is not wanted and eps2 >= 2^-40, because an
+//                unmasked coincident pair adds m u^3 * (+-0) = +-0 to a.  13 + 1 instructions.
+// (A third, speculative variant -- flag r2 == eps2 in the loop, redo a flagged 256-j block with the mask -- was the
+//  default earlier in this round and was removed: DESIGN.md section 10.)
+enum { MASK_EXACT = 0, MASK_NONE = 2 };
 
 // PHI = false: the caller does not want the potential (pot_out == NULL): 12 FP32-pipe instructions per pair.
 template <int MASK, bool PHI = true>
 __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nxi, u64 nyi, u64 nzi, u64 eps2_2,
-                                          float eps2, u64& ax, u64& ay, u64& az, u64& ph, bool& hit) {
+                                          u64& ax, u64& ay, u64& az, u64& ph) {
     const u64 dx = add2(xj, nxi);                    // dx = xj - xi
     const u64 dy = add2(yj, nyi);
     const u64 dz = add2(zj, nzi);
@@ -141,9 +140,6 @@ __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nx
         const uint32_t tb = __float_as_uint(dxb) | __float_as_uint(dyb) | __float_as_uint(dzb);
         r2a = (ta == 0u) ? inf : r2a;                // rsqrt(+inf) = +0 -> the pair adds exactly 0
         r2b = (tb == 0u) ? inf : r2b;
-    } else if (MASK == MASK_SPEC) {
-        hit |= (r2a == eps2);
-        hit |= (r2b == eps2);
     }
     const u64 u = pack2(rsqrt_approx(r2a), rsqrt_approx(r2b));   // r1i = 1/sqrt(r2)
     const u64 u2 = mul2(u, u);                       // r2i
@@ -158,10 +154,9 @@ __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nx
 // One tile: K/2 i-pairs of this thread against np j-particles in shared memory; partial sums start from zero (Eq. (2)).
 // EPS_I (row f3): the softening is a property of the i-particle (Fig. A.1) and sits, packed, in e2[].
 template <int K, int MASK, bool EPS_I = false, bool PHI = true>
-__device__ __forceinline__ bool tile_sweep(const float4* __restrict__ sp, int np, const u64 (&nxi)[K / 2], const u64 (&nyi)[K / 2],
-                                           const u64 (&nzi)[K / 2], u64 eps2_2, float eps2, u64 (&pax)[K / 2], u64 (&pay)[K / 2],
+__device__ __forceinline__ void tile_sweep(const float4* __restrict__ sp, int np, const u64 (&nxi)[K / 2], const u64 (&nyi)[K / 2],
+                                           const u64 (&nzi)[K / 2], u64 eps2_2, u64 (&pax)[K / 2], u64 (&pay)[K / 2],
                                            u64 (&paz)[K / 2], u64 (&pph)[K / 2], const u64 (&e2)[K / 2]) {
-    bool hit = false;
 #pragma unroll
     for (int k = 0; k < K / 2; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
 #pragma unroll 4
@@ -170,9 +165,8 @@ __device__ __forceinline__ bool tile_sweep(const float4* __restrict__ sp, int np
         const u64 xj = pack2(J.x, J.x), yj = pack2(J.y, J.y), zj = pack2(J.z, J.z), mj = pack2(J.w, J.w);
 #pragma unroll
         for (int k = 0; k < K / 2; ++k)
-            pair_body<MASK, PHI>(xj, yj, zj, mj, nxi[k], nyi[k], nzi[k], EPS_I ? e2[k] : eps2_2, eps2, pax[k], pay[k], paz[k], pph[k], hit);
+            pair_body<MASK, PHI>(xj, yj, zj, mj, nxi[k], nyi[k], nzi[k], EPS_I ? e2[k] : eps2_2, pax[k], pay[k], paz[k], pph[k]);
     }
-    return hit;
 }
 
 // ---------------------------------------------------------------- coincidence lists (reading R1, large calls)
@@ -298,9 +292,8 @@ struct ForceArgs {
 };
 
 // how the force kernel honours the coincident-pair rule
-enum { MODE_EXACT = 0,     // masked loop everywhere (eps2 == 0 or tiny)
-       MODE_SPEC = 1,      // unmasked loop + flag, masked redo of a flagged block (small calls)
-       MODE_LIST = 2 };    // coincidence lists from the pre-pass, no test in the hot loop (large calls)
+enum { MODE_EXACT = 0,     // masked loop everywhere (small calls; eps2 == 0 or tiny)
+       MODE_LIST = 2 };    // coincidence lists from the pre-pass, no test in the hot loop (large calls; a-only calls)
 
 // ---------------------------------------------------------------- a2..a7: the force kernel
 // CTA = 8 warps = WI (along i) x WJ (along j).  A CTA owns 32*K*WI i-particles (K per thread, in
@@ -311,7 +304,7 @@ enum { MODE_EXACT = 0,     // masked loop everywhere (eps2 == 0 or tiny)
 template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I = false, bool PHI = true, int SUB = 256>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
-    static_assert(!(EPS_I && MODE == MODE_SPEC), "per-i softening: masked or list mode only");
+    static_assert(MODE == MODE_EXACT || MODE == MODE_LIST, "masked everywhere, or coincidence lists");
     static_assert(SUB == kCoinSeg, "coincidence segments are SUB j-particles");
     extern __shared__ __align__(128) unsigned char smem_raw[];
 
@@ -358,8 +351,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
         nyi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 1], -a.x_i[3 * (size_t)i1 + 1]);
         nzi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 2], -a.x_i[3 * (size_t)i1 + 2]);
     }
-    const float eps2 = a.eps2;
-    const u64 eps2_2 = pack2(eps2, eps2);
+    const u64 eps2_2 = pack2(a.eps2, a.eps2);
     u64 e2[K / 2];
 #pragma unroll
     for (int k2 = 0; k2 < K / 2; ++k2) {
@@ -408,11 +400,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
         for (int c = 0; c < np; c += SUB) {
             const int nc = min(SUB, np - c);
             u64 pax[K / 2], pay[K / 2], paz[K / 2], pph[K / 2];
-            if (MODE == MODE_SPEC) {
-                const bool hit = tile_sweep<K, MASK_SPEC, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
-                if (__any_sync(0xffffffffu, hit))                      // rare: some pair of this warp may be coincident
-                    (void)tile_sweep<K, MASK_EXACT, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
-            } else if (MODE == MODE_LIST) {
+            if (MODE == MODE_LIST) {
                 const int j0 = j_begin + t * TJ + c;                   // global index of the block's first j
                 const int seg_lo = j0 >> kCoinSegShift, seg_hi = (j0 + nc - 1) >> kCoinSegShift;
                 while (coin_next < seg_lo) {
@@ -420,11 +408,11 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
                     coin_next = (coin_pos < coin_cnt) ? coin[1 + coin_pos] : 0x7fffffff;
                 }
                 if (coin_cnt < 0 || coin_next <= seg_hi)               // rare: the block holds a coincident pair
-                    (void)tile_sweep<K, MASK_EXACT, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
+                    tile_sweep<K, MASK_EXACT, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph, e2);
                 else
-                    (void)tile_sweep<K, MASK_NONE, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
+                    tile_sweep<K, MASK_NONE, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph, e2);
             } else {
-                (void)tile_sweep<K, MASK_EXACT, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, eps2, pax, pay, paz, pph, e2);
+                tile_sweep<K, MASK_EXACT, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph, e2);
             }
             // a5: block partial -> running total
 #pragma unroll

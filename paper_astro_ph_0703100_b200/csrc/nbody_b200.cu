@@ -108,29 +108,22 @@ nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count) {
     return p;
 }
 
-// The speculative-mask kernel (nb_kernels.cuh, MASK_SPEC) needs eps2 > 0 and a finite
-// m * rsqrt(eps2)^3 for the unmasked coincident pair; below this threshold (and for eps2 == 0)
-// the always-masked kernel runs.  2^-40: rsqrt(eps2)^3 = 2^60.
-constexpr float kSpecMinEps2 = 9.094947017729282e-13f;
+// An UNMASKED coincident pair must stay finite (m * rsqrt(eps2)^3 = m * 2^60 at the threshold): the list mode and
+// the acceleration-only path need eps2 >= 2^-40; below that (and for eps2 == 0) every pair is masked.
+constexpr float kUnmaskedMinEps2 = 9.094947017729282e-13f;
 
 // Calls with at least this many pairs locate their coincident pairs with the hash-join pre-pass
-// (MODE_LIST: three extra O(n) launches, ~35 us, no test in the hot loop); smaller ones mask every pair.
+// (MODE_LIST: three extra O(n) launches, ~35 us, no test in the hot loop); smaller ones mask every pair
+// (MODE_EXACT: a small call is a single wave of CTAs, and 35 us of pre-pass would cost more than the mask).
 constexpr double kListMinPairs = 536870912.0;    // 2^29
 
-// Small calls mask every pair (MODE_EXACT).  The speculative mode (flag-only loop, masked redo of a flagged 256-j
-// block) is faster per pair but a small call is a single wave of CTAs, so the call lasts as long as its slowest
-// CTA -- one that redoes blocks: measured on aliased sets N = 4096 / 8192 / 16384: 34 / 67 / 186 us speculative
-// against 27 / 52 / 165 us masked; on an active subset (C2) 39 against 27 us.  MODE_SPEC stays available as
-// NB_MASK=spec (tests keep it bit-identical to the masked kernel).
-int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool aliased) {
-    // debugging aid: NB_MASK=exact|spec|list forces a mode (spec/list still need eps2 >= 2^-40)
+int pick_mode(int64_t n_i, int64_t n_j, float eps2) {
+    // debugging aid: NB_MASK=exact|list forces a mode (list still needs eps2 >= 2^-40 and n_j <= 2^29)
     const char* e = std::getenv("NB_MASK");
     if (e && e[0] == 'e') return nb::MODE_EXACT;
-    if (eps2 < kSpecMinEps2) return nb::MODE_EXACT;
-    if (e && e[0] == 's') return nb::MODE_SPEC;
-    if (e && e[0] == 'l' && n_j <= ((int64_t)1 << 29)) return nb::MODE_LIST;
-    (void)aliased;
-    if (n_j > ((int64_t)1 << 29)) return nb::MODE_EXACT;           // the 32-bit hash table holds 2 n_j <= 2^30 slots
+    if (eps2 < kUnmaskedMinEps2) return nb::MODE_EXACT;
+    if (n_j > ((int64_t)1 << 29)) return nb::MODE_EXACT;             // the 32-bit hash table holds 2 n_j <= 2^30 slots
+    if (e && e[0] == 'l') return nb::MODE_LIST;
     return ((double)n_i * (double)n_j >= kListMinPairs) ? nb::MODE_LIST : nb::MODE_EXACT;
 }
 
@@ -291,12 +284,11 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.coin_flag = nullptr;
     args.i_off = args.j_off = args.tile_start = args.cta_batch = nullptr;
     args.n_batch = 0;
-    int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2, !packed_j && x_i == x_j);
-    if (eps2_i && mode == nb::MODE_SPEC) mode = nb::MODE_EXACT;      // the values are on the device: no threshold test
+    const int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2);
     // Without phi no pair needs a mask when eps2 >= 2^-40: an unmasked coincident pair adds m u^3 * (+-0) = +-0 to a
     // (only phi would get m / eps), so a_i is bit for bit the masked loop's.  The list-mode kernel then runs with an
     // empty list: no pre-pass, the untested loop everywhere (nb_leapfrog_kdk: every evaluation but the last).
-    const bool a_only = !pot_out && !eps2_i && eps2 >= kSpecMinEps2 && !std::getenv("NB_MASK");
+    const bool a_only = !pot_out && !eps2_i && eps2 >= kUnmaskedMinEps2 && !std::getenv("NB_MASK");
     if (a_only) {
         rc = (plan.K == 8) ? launch_force_nophi(args, plan, stream) : launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (mode == nb::MODE_LIST) {
@@ -307,8 +299,6 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         else rc = launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (eps2_i) {
         rc = launch_force<nb::MODE_EXACT, true>(args, plan, stream);
-    } else if (mode == nb::MODE_SPEC) {
-        rc = launch_force<nb::MODE_SPEC>(args, plan, stream);
     } else {
         rc = launch_force<nb::MODE_EXACT>(args, plan, stream);
     }
@@ -440,9 +430,8 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     args.n_j = (int)n_j;
     args.S = plan.S;
     args.eps2 = eps2;
-    // the jerk has no speculative mode: small calls mask every pair, large ones use the coincidence lists
-    int mode = pick_mode(n_i, n_j, eps2, x_i == x_j);
-    if (mode == nb::MODE_SPEC) mode = nb::MODE_EXACT;
+    // small calls mask every pair, large ones use the coincidence lists
+    const int mode = pick_mode(n_i, n_j, eps2);
     if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, args.jp, 2, stream, &args.coin_lists, &args.coin_flag);
         if (rc != NB_OK) return rc;
@@ -475,12 +464,12 @@ int batched_groups(int64_t n_i_total, int64_t n_batch) {
     return 4;
 }
 
-template <int MODE, int G, int STAGES>
+template <bool MASKED, int G, int STAGES>
 int launch_batched_inst(const nb::ForceArgs& args, unsigned max_ctas, cudaStream_t stream) {
     constexpr size_t ring = (size_t)8 * STAGES * 256 * 16;
     constexpr size_t red = (size_t)8 * (2 * G) * 4 * 32 * sizeof(double);
     constexpr size_t smem = (ring > red ? ring : red) + 8 * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_batched_kernel<MODE, G, STAGES>;
+    auto kern = nb::nb_batched_kernel<MASKED, G, STAGES>;
     static bool configured[64] = {};
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
@@ -504,12 +493,12 @@ int launch_batched_inst(const nb::ForceArgs& args, unsigned max_ctas, cudaStream
     return NB_OK;
 }
 
-template <int MODE>
+template <bool MASKED>
 int launch_batched(const nb::ForceArgs& args, int groups, unsigned max_ctas, cudaStream_t stream) {
     switch (groups) {
-        case 1: return launch_batched_inst<MODE, 1, 2>(args, max_ctas, stream);    // 64 KB of rings: 3 CTAs per SM
-        case 2: return launch_batched_inst<MODE, 2, 3>(args, max_ctas, stream);
-        default: return launch_batched_inst<MODE, 4, 3>(args, max_ctas, stream);
+        case 1: return launch_batched_inst<MASKED, 1, 2>(args, max_ctas, stream);  // 64 KB of rings, 2 CTAs per SM
+        case 2: return launch_batched_inst<MASKED, 2, 3>(args, max_ctas, stream);
+        default: return launch_batched_inst<MASKED, 4, 3>(args, max_ctas, stream);
     }
 }
 
@@ -577,12 +566,10 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     args.n_j = (int)n_j_total;
     args.S = 1;
     args.eps2 = eps2;
-    // masked loop by default (measured faster on tree lists, nb_batched.cuh); NB_MASK=spec: flag-only loop with the
-    // flagged blocks redone by all 8 warps together (needs eps2 >= 2^-40)
-    const char* e = std::getenv("NB_MASK");
-    const bool spec = eps2 >= kSpecMinEps2 && (e && e[0] == 's');
-    return spec ? launch_batched<nb::MODE_SPEC>(args, groups, (unsigned)max_ctas, stream)
-                : launch_batched<nb::MODE_EXACT>(args, groups, (unsigned)max_ctas, stream);
+    // every pair masked -- unless phi is not wanted and eps2 >= 2^-40, where no pair needs the mask (see force_impl)
+    const bool a_only = !pot_out && eps2 >= kUnmaskedMinEps2 && !std::getenv("NB_MASK");
+    return a_only ? launch_batched<false>(args, groups, (unsigned)max_ctas, stream)
+                  : launch_batched<true>(args, groups, (unsigned)max_ctas, stream);
 }
 
 int nb_force_jerk(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j, const float* x_j, const float* v_j,

@@ -44,17 +44,16 @@ def check(acc, pot, ra, rp, label=""):
         assert e["pot_rms"] <= 1e-5, (label, e)
 
 
-@pytest.mark.parametrize("mode", ["", "spec"])
 @pytest.mark.parametrize("tile", ["64", "128", "256", ""])
-def test_tree_lists_every_tile_shape(nb, tile, mode, monkeypatch):
+def test_tree_lists_every_tile_shape(nb, tile, monkeypatch):
     if tile:
         monkeypatch.setenv("NB_BATCH_TILE", tile)
-    if mode:
-        monkeypatch.setenv("NB_MASK", mode)
     w = wl.tree_list_workload(6000, 20, 300, 900, 2500, 1.0 / 128, seed=5)
     acc, pot = gpu_batched(nb, w)
     ra, rp = oracle.force_batched(w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j, w.eps2)
-    check(acc, pot, ra, rp, "tile " + tile + mode)
+    check(acc, pot, ra, rp, "tile " + tile)
+    a_only, none = gpu_batched(nb, w, want_pot=False)         # acceleration only: the untested loop, same bits
+    assert none is None and np.array_equal(acc, a_only)
 
 
 def test_equals_separate_nb_force_calls_within_tolerance_and_masks_own_members(nb):
@@ -96,16 +95,8 @@ def test_edge_cases_empty_groups_empty_lists_gaps(nb):
         nb.force_batched(dev(i_off), dev(j_off), dev(x_i), dev(x_j), dev(m_j), -1.0)
 
 
-def test_eps0_and_masked_mode_agree(nb, monkeypatch):
+def test_eps0(nb):
     w = wl.tree_list_workload(2000, 30, 90, 300, 700, 1.0 / 64, seed=3)
-    a_e, p_e = gpu_batched(nb, w)                     # default: every pair masked
-    monkeypatch.setenv("NB_MASK", "spec")
-    a_s, p_s = gpu_batched(nb, w)                     # flag-only loop + deferred masked redo by all warps: in tolerance
-    a_s2, p_s2 = gpu_batched(nb, w)
-    assert np.array_equal(a_s, a_s2) and np.array_equal(p_s, p_s2)          # reproducible whatever warp finishes first
-    np.testing.assert_allclose(a_s, a_e, rtol=2e-5, atol=1e-7)              # (the redo sums a flagged block in 8 pieces)
-    np.testing.assert_allclose(p_s, p_e, rtol=2e-6)
-    monkeypatch.delenv("NB_MASK")
     w0 = wl.BatchedWorkload("eps0", w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j, 0.0)
     acc, pot = gpu_batched(nb, w0)
     ra, rp = oracle.force_batched(w0.i_offsets, w0.j_offsets, w0.x_i, w0.x_j, w0.m_j, 0.0)

@@ -87,9 +87,9 @@ def test_every_decomposition_matches_oracle(nb, plan, monkeypatch):
     check_parity(acc, pot, ref_acc, ref_pot, str(plan))
 
 
-def test_speculative_and_always_masked_kernels_agree_bitwise(nb, monkeypatch):
-    """The speculative-mask kernel redoes a tile with the exact mask when r2 == eps2 occurred, so its output is
-    the always-masked kernel's, bit for bit -- with self pairs (aliased sets), duplicates and near-coincident pairs."""
+def test_masked_list_and_acceleration_only_paths_agree_bitwise(nb, monkeypatch):
+    """Masked kernel, list-mode kernel and the acceleration-only path (untested loop everywhere) store the same bits --
+    with self pairs (aliased sets), duplicates, and a near-coincident pair whose r2 rounds to eps2."""
     w = wl.config(0)
     x = w.x_j.copy()
     x[100] = x[7]                                  # exact duplicates
@@ -98,23 +98,27 @@ def test_speculative_and_always_masked_kernels_agree_bitwise(nb, monkeypatch):
     ref_acc, ref_pot = oracle.force(x, x, w.m_j, w.eps2)
     monkeypatch.setenv("NB_MASK", "exact")
     a_e, p_e = gpu_force(nb, x, x, w.m_j, w.eps2, alias=True)
+    monkeypatch.setenv("NB_MASK", "list")
+    a_l, p_l = gpu_force(nb, x, x, w.m_j, w.eps2, alias=True)
     monkeypatch.delenv("NB_MASK")
-    a_s, p_s = gpu_force(nb, x, x, w.m_j, w.eps2, alias=True)
-    assert np.array_equal(a_e, a_s) and np.array_equal(p_e, p_s)
+    a_d, p_d = gpu_force(nb, x, x, w.m_j, w.eps2, alias=True)                  # default (small call: masked)
+    a_o, _ = gpu_force(nb, x, x, w.m_j, w.eps2, want_pot=False, alias=True)    # acceleration only: no mask at all
+    assert np.array_equal(a_e, a_l) and np.array_equal(p_e, p_l)
+    assert np.array_equal(a_e, a_d) and np.array_equal(p_e, p_d) and np.array_equal(a_e, a_o)
     # the self term would shift phi by m/eps = 64/2048 = 3e-2 absolute (~3 % relative): far outside tolerance
-    check_parity(a_s, p_s, ref_acc, ref_pot, "C0 + duplicates")
+    check_parity(a_d, p_d, ref_acc, ref_pot, "C0 + duplicates")
     # separate i-set drawn from the j-set (C2 shape): each i coincides with exactly one j
     w2 = wl.subset_workload(5000, 700, 1.0 / 128, seed=9)
     monkeypatch.setenv("NB_MASK", "exact")
     a_e, p_e = gpu_force(nb, w2.x_i, w2.x_j, w2.m_j, w2.eps2)
-    monkeypatch.delenv("NB_MASK")
-    a_s, p_s = gpu_force(nb, w2.x_i, w2.x_j, w2.m_j, w2.eps2)
-    assert np.array_equal(a_e, a_s) and np.array_equal(p_e, p_s)
+    monkeypatch.setenv("NB_MASK", "list")
+    a_l, p_l = gpu_force(nb, w2.x_i, w2.x_j, w2.m_j, w2.eps2)
+    assert np.array_equal(a_e, a_l) and np.array_equal(p_e, p_l)
 
 
-def _three_modes(nb, monkeypatch, x_i, x_j, m_j, eps2, alias=False):
+def _both_modes(nb, monkeypatch, x_i, x_j, m_j, eps2, alias=False):
     out = {}
-    for mode in ("exact", "spec", "list"):
+    for mode in ("exact", "list"):
         monkeypatch.setenv("NB_MASK", mode)
         out[mode] = gpu_force(nb, x_i, x_j, m_j, eps2, alias=alias)
     monkeypatch.delenv("NB_MASK")
@@ -134,16 +138,14 @@ def test_list_mode_agrees_bitwise_with_masked_kernel(nb, plan, monkeypatch):
     x[700] = (0.0, 0.0, 0.0)
     x[2100] = (-0.0, 1e-41, 0.0)                   # canonically equal to particle 700 (add.ftz flushes subnormals)
     x[300] = x[8] + np.float32(1e-7)               # near, not coincident
-    out = _three_modes(nb, monkeypatch, x, x, w.m_j, w.eps2, alias=True)
-    for mode in ("spec", "list"):
-        assert np.array_equal(out["exact"][0], out[mode][0]), mode
-        assert np.array_equal(out["exact"][1], out[mode][1]), mode
+    out = _both_modes(nb, monkeypatch, x, x, w.m_j, w.eps2, alias=True)
+    assert np.array_equal(out["exact"][0], out["list"][0]) and np.array_equal(out["exact"][1], out["list"][1])
     ref_acc, ref_pot = oracle.force(x, x, w.m_j, w.eps2)
     keep = np.ones(3000, bool); keep[[700, 2100]] = False      # the oracle does not flush 1e-41: that pair differs by design
     check_parity(out["list"][0][keep], out["list"][1][keep], ref_acc[keep], ref_pot[keep], "list " + str(plan))
     # separate i-set drawn from the j-set (C2 shape)
     w2 = wl.subset_workload(5000, 700, 1.0 / 128, seed=9)
-    out = _three_modes(nb, monkeypatch, w2.x_i, w2.x_j, w2.m_j, w2.eps2)
+    out = _both_modes(nb, monkeypatch, w2.x_i, w2.x_j, w2.m_j, w2.eps2)
     assert np.array_equal(out["exact"][0], out["list"][0]) and np.array_equal(out["exact"][1], out["list"][1])
     ref_acc, ref_pot = oracle.force(w2.x_i, w2.x_j, w2.m_j, w2.eps2)
     check_parity(out["list"][0], out["list"][1], ref_acc, ref_pot, "list subset " + str(plan))
@@ -157,12 +159,12 @@ def test_list_mode_degenerate_inputs(nb, monkeypatch):
     x = rng.normal(size=(n, 3)).astype(np.float32)
     m = rng.uniform(0.5, 1.5, n).astype(np.float32) / n
     x[::300] = x[0]                                # 20 copies spread over 20 segments: list overflow for group 0
-    out = _three_modes(nb, monkeypatch, x, x, m, 1e-3, alias=True)
+    out = _both_modes(nb, monkeypatch, x, x, m, 1e-3, alias=True)
     assert np.array_equal(out["exact"][0], out["list"][0]) and np.array_equal(out["exact"][1], out["list"][1])
     ref_acc, ref_pot = oracle.force(x, x, m, 1e-3)
     check_parity(out["list"][0], out["list"][1], ref_acc, ref_pot, "overflow")
     x[:5000] = (1.0, 2.0, 3.0)                     # 5000 identical positions: probe chains exceed the cap
-    out = _three_modes(nb, monkeypatch, x, x, m, 1e-3, alias=True)
+    out = _both_modes(nb, monkeypatch, x, x, m, 1e-3, alias=True)
     assert np.array_equal(out["exact"][0], out["list"][0]) and np.array_equal(out["exact"][1], out["list"][1])
     ref_acc, ref_pot = oracle.force(x, x, m, 1e-3)
     sel = slice(5000, n)                           # the 5000 coincident ones have a ~ 0: compare the others relatively
@@ -171,7 +173,7 @@ def test_list_mode_degenerate_inputs(nb, monkeypatch):
 
 
 def test_tiny_eps2_uses_masked_kernel(nb):
-    # eps2 below the speculative kernel's threshold (and denormal-small): still finite and within tolerance
+    # eps2 below the threshold of the unmasked loops (and denormal-small): still finite and within tolerance
     w = wl.plummer_workload(700, 1.0 / 64, seed=6)
     for eps2 in (1e-13, 1e-30):
         acc, pot = gpu_force(nb, w.xi, w.x_j, w.m_j, eps2, alias=True)
