@@ -274,6 +274,8 @@ struct ForceArgs {
     const float* x_i;      // [n_i][3]
     const float* eps2_i;   // EPS_I: [n_i] softening squared of every i-particle
     const float4* jp;      // packed j records (x, y, z, m)
+    const float* xj_raw;   // non-null (with mj_raw): small call, every warp group packs its own j sub-range straight
+    const float* mj_raw;   //   from x_j / m_j into its ring (it fits whole) -- no nb_pack_j_kernel launch, no TMA
     float* acc;            // [n_i][3]
     float* pot;            // [n_i] or nullptr
     double4* partial;      // [S][n_i] when S > 1
@@ -301,7 +303,8 @@ enum { MODE_EXACT = 0,     // masked loop everywhere (small calls; eps2 == 0 or 
 // Each sub-range is streamed through its own shared-memory ring by 1-D TMA bulk copies issued by
 // lane 0 of the group's first warp; "full" mbarriers count bytes, "empty" mbarriers count the WI
 // consuming warps.
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I = false, bool PHI = true, int SUB = 256>
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I = false, bool PHI = true, bool DIRECT = false,
+          int SUB = 256>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
     static_assert(MODE == MODE_EXACT || MODE == MODE_LIST, "masked everywhere, or coincidence lists");
@@ -366,7 +369,18 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
 
     __syncthreads();                                                   // barriers initialised
 
-    if (producer) {
+    // Small calls (nbody_b200.cu: the whole sub-range fits the ring): rows a1 + a2 in one step -- the WI warps of the
+    // group pack their sub-range from x_j / m_j into the ring themselves (Fig. A.1 packing loop);
+    // tile t then sits in slot t, exactly where the TMA path would have put it.
+    constexpr bool direct = DIRECT;                                    // a template parameter: the large-call kernels carry none of this
+    if (direct) {
+        float4* rp = reinterpret_cast<float4*>(rings + wj * RING_BYTES);
+        for (int q = wi * 32 + lane; q < n_sub; q += WI * 32) {
+            const size_t j = (size_t)(j_begin + q);
+            rp[q] = make_float4(a.xj_raw[3 * j + 0], a.xj_raw[3 * j + 1], a.xj_raw[3 * j + 2], a.mj_raw[j]);
+        }
+        __syncthreads();
+    } else if (producer) {
         const int pre = n_tiles < STAGES ? n_tiles : STAGES;
         for (int t = 0; t < pre; ++t) {
             const uint32_t bytes = (uint32_t)min(TJ, n_sub - t * TJ) * 16u;
@@ -391,7 +405,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
     for (int t = 0; t < n_tiles; ++t) {
         const int slot = t % STAGES;
         const uint32_t parity = (uint32_t)(t / STAGES) & 1u;
-        mbar_wait(full0 + 8 * slot, parity);
+        if (!direct) mbar_wait(full0 + 8 * slot, parity);
 
         const int np = min(TJ, n_sub - t * TJ);
         const float4* sp = reinterpret_cast<const float4*>(rings + wj * RING_BYTES + slot * TJ * 16);
@@ -428,6 +442,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
         // release the slot; the producer refills it with tile t' + STAGES.  With several consumer
         // warps the refill trails by one tile so that the producer rarely waits for a slower warp.
         __syncwarp();
+        if (direct) continue;
         if (lane == 0) mbar_arrive(empty0 + 8 * slot);
         if (producer) {
             const int tt = (WI > 1) ? t - 1 : t;

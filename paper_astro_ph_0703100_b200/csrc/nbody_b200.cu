@@ -127,12 +127,12 @@ int pick_mode(int64_t n_i, int64_t n_j, float eps2) {
     return ((double)n_i * (double)n_j >= kListMinPairs) ? nb::MODE_LIST : nb::MODE_EXACT;
 }
 
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I, bool PHI = true>
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I, bool PHI = true, bool DIRECT = false>
 int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
     constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, EPS_I, PHI>;
+    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, EPS_I, PHI, DIRECT>;
     static bool configured[64] = {};
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
@@ -158,13 +158,13 @@ int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStrea
 }
 
 // tile_j / stages per WJ must match nb::ring_shape (nb_plan.h)
-template <int K, int MODE, bool EPS_I>
+template <int K, int MODE, bool EPS_I, bool DIRECT = false>
 int launch_force_k(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     switch (plan.WJ) {
-        case 1: return launch_force_inst<K, 8, 1, 512, 4, MODE, EPS_I>(args, plan, stream);
-        case 2: return launch_force_inst<K, 4, 2, 512, 4, MODE, EPS_I>(args, plan, stream);
-        case 4: return launch_force_inst<K, 2, 4, 256, 4, MODE, EPS_I>(args, plan, stream);
-        default: return launch_force_inst<K, 1, 8, 256, 3, MODE, EPS_I>(args, plan, stream);
+        case 1: return launch_force_inst<K, 8, 1, 512, 4, MODE, EPS_I, true, DIRECT>(args, plan, stream);
+        case 2: return launch_force_inst<K, 4, 2, 512, 4, MODE, EPS_I, true, DIRECT>(args, plan, stream);
+        case 4: return launch_force_inst<K, 2, 4, 256, 4, MODE, EPS_I, true, DIRECT>(args, plan, stream);
+        default: return launch_force_inst<K, 1, 8, 256, 3, MODE, EPS_I, true, DIRECT>(args, plan, stream);
     }
 }
 
@@ -178,12 +178,12 @@ int launch_force_nophi(const nb::ForceArgs& args, const nb::Plan& plan, cudaStre
     }
 }
 
-template <int MODE, bool EPS_I = false>
+template <int MODE, bool EPS_I = false, bool DIRECT = false>
 int launch_force(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     switch (plan.K) {
-        case 2: return launch_force_k<2, MODE, EPS_I>(args, plan, stream);
-        case 4: return launch_force_k<4, MODE, EPS_I>(args, plan, stream);
-        default: return launch_force_k<8, MODE, EPS_I>(args, plan, stream);
+        case 2: return launch_force_k<2, MODE, EPS_I, DIRECT>(args, plan, stream);
+        case 4: return launch_force_k<4, MODE, EPS_I, DIRECT>(args, plan, stream);
+        default: return launch_force_k<8, MODE, EPS_I, DIRECT>(args, plan, stream);
     }
 }
 
@@ -259,8 +259,19 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         }
     }
 
+    const int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2);
+    // Without phi no pair needs a mask when eps2 >= 2^-40: an unmasked coincident pair adds m u^3 * (+-0) = +-0 to a
+    // (only phi would get m / eps), so a_i is bit for bit the masked loop's.  The list-mode kernel then runs with an
+    // empty list: no pre-pass, the untested loop everywhere (nb_leapfrog_kdk: every evaluation but the last).
+    const bool a_only = !pot_out && !eps2_i && eps2 >= kUnmaskedMinEps2 && !std::getenv("NB_MASK");
+    // Small calls whose per-warp-group j sub-range fits its shared-memory ring whole: the force kernel packs the
+    // sub-range itself, one launch fewer (C0: 21 -> 16 us per call).  NB_DIRECT=0 disables it (tests compare).
+    const int64_t sub_max = (n_j + (int64_t)plan.S * plan.WJ - 1) / ((int64_t)plan.S * plan.WJ);
+    const char* dr = std::getenv("NB_DIRECT");
+    const bool direct = !packed_j && !eps2_i && !a_only && mode == nb::MODE_EXACT && sub_max <= (int64_t)plan.tile_j * plan.stages &&
+                        !(dr && dr[0] == '0');
     const float4* jp = packed_j ? packed_j : reinterpret_cast<const float4*>(ws->jp);
-    if (!packed_j) {   // a1: j-pack
+    if (!packed_j && !direct) {   // a1: j-pack
         const int threads = 256;
         const int blocks = (int)((n_j + threads - 1) / threads);
         nb::nb_pack_j_kernel<<<blocks, threads, 0, stream>>>(x_j, m_j, (int)n_j, reinterpret_cast<float4*>(ws->jp));
@@ -272,6 +283,8 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.x_i = x_i;
     args.eps2_i = eps2_i;
     args.jp = jp;
+    args.xj_raw = direct ? x_j : nullptr;
+    args.mj_raw = direct ? m_j : nullptr;
     args.acc = acc_out;
     args.pot = pot_out;
     args.partial = reinterpret_cast<double4*>(ws->partial);
@@ -284,11 +297,6 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.coin_flag = nullptr;
     args.i_off = args.j_off = args.tile_start = args.cta_batch = nullptr;
     args.n_batch = 0;
-    const int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2);
-    // Without phi no pair needs a mask when eps2 >= 2^-40: an unmasked coincident pair adds m u^3 * (+-0) = +-0 to a
-    // (only phi would get m / eps), so a_i is bit for bit the masked loop's.  The list-mode kernel then runs with an
-    // empty list: no pre-pass, the untested loop everywhere (nb_leapfrog_kdk: every evaluation but the last).
-    const bool a_only = !pot_out && !eps2_i && eps2 >= kUnmaskedMinEps2 && !std::getenv("NB_MASK");
     if (a_only) {
         rc = (plan.K == 8) ? launch_force_nophi(args, plan, stream) : launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (mode == nb::MODE_LIST) {
@@ -299,6 +307,8 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         else rc = launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (eps2_i) {
         rc = launch_force<nb::MODE_EXACT, true>(args, plan, stream);
+    } else if (direct) {
+        rc = launch_force<nb::MODE_EXACT, false, true>(args, plan, stream);
     } else {
         rc = launch_force<nb::MODE_EXACT>(args, plan, stream);
     }
@@ -551,6 +561,7 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     args.x_i = x_i;
     args.eps2_i = nullptr;
     args.jp = reinterpret_cast<const float4*>(ws->jp);
+    args.xj_raw = args.mj_raw = nullptr;
     args.acc = acc_out;
     args.pot = pot_out;
     args.partial = nullptr;

@@ -383,3 +383,20 @@ def test_acceleration_only_calls_need_no_mask(nb, n, monkeypatch):
     monkeypatch.setenv("NB_MASK", "exact")
     a_mask, _ = gpu_force(nb, x, x, w.m_j, w.eps2, alias=True)
     assert p_free is None and np.array_equal(a_free, a_mask)
+
+
+@pytest.mark.parametrize("n_i,n_j", [(2048, 2048), (512, 8192), (1, 5), (700, 3001), (4096, 4096)])
+def test_small_call_direct_pack_path_agrees_bitwise(nb, n_i, n_j, monkeypatch):
+    """Small calls pack their j sub-ranges inside the force kernel (no nb_pack_j_kernel launch, no TMA): same bits as
+    the pack + TMA path (NB_DIRECT=0), one launch fewer."""
+    w = wl.plummer_workload(max(n_i, n_j), 1.0 / 64, seed=33)
+    x_j, m_j, x_i = w.x_j[:n_j], w.m_j[:n_j], w.x_j[:n_i]
+    a1, p1 = gpu_force(nb, x_i, x_j, m_j, w.eps2)
+    launches_direct = nb.last_launch_count()
+    monkeypatch.setenv("NB_DIRECT", "0")
+    a0, p0 = gpu_force(nb, x_i, x_j, m_j, w.eps2)
+    assert nb.last_launch_count() == launches_direct + 1
+    assert np.array_equal(a0, a1) and np.array_equal(p0, p1)
+    ref_acc, ref_pot = oracle.force(x_i, x_j, m_j, w.eps2)
+    if n_i > 1:
+        check_parity(a1, p1, ref_acc, ref_pot, f"direct {n_i}x{n_j}")
