@@ -11,10 +11,10 @@
  *     static __device__ void pair(const float* INPUT_I, const float* INPUT_J, float* OUTPUT);   // OUTPUT[] += ...
  * and  nb::pipeline_run<Pipeline>(p_xj, p_xi, p_fi, ni, nj, stream)  is the cunbody_api call on DEVICE rows.
  * The scheme around the pipeline is the same as for the library's own gravity kernels: i-records stationary in
- * registers (2 per thread), j-records streamed through shared memory in tiles and read as warp broadcasts, Eq. (2)
+ * registers (2 or 4 per thread), j-records streamed through shared memory in tiles and read as warp broadcasts, Eq. (2)
  * two-level sums (FP32 partials over 256 j, FP64 running totals), the j-range split over S CTAs with a fixed-order
  * second pass (no floating-point atomics: bitwise reproducible).  The specialised kernels (packed FP32, TMA rings,
- * coincidence lists) are 2.2 - 2.4x faster for gravity; this header is for the interactions the library does not ship.
+ * coincidence lists) are 1.8x faster for gravity; this header is for the interactions the library does not ship.
  *
  * libnbody_b200.so instantiates it for the paper's two listings: nb_cunbody_force (Fig. A.3) and
  * nb_cunbody_force_jerk_pot (Fig. A.4), see nbody_b200.h.  sm_100a, CUDA C++17, header only.
@@ -26,7 +26,9 @@
 namespace nb {
 
 constexpr int kPipeThreads = 256;    // threads per CTA
-constexpr int kPipeK = 2;            // i-records per thread (4: Fig. A.3 +3 %, Fig. A.4 -13 %)
+// i-records per thread: 4 for narrow records (Fig. A.3: +6 %), 2 for wide ones (Fig. A.4), by register budget
+template <class P>
+struct PipeK { static constexpr int value = (P::IDIM + 2 * P::FDIM <= 12) ? 4 : 2; };
 constexpr int kPipeTile = 128;       // j-records per shared-memory tile
 constexpr int kPipeBlock = 256;      // j-records per FP32 partial sum (Eq. (2))
 
@@ -34,7 +36,7 @@ template <class P>
 __global__ void __launch_bounds__(kPipeThreads) pipeline_kernel(const float* __restrict__ p_xj, const float* __restrict__ p_xi,
                                                                 float* __restrict__ p_fi, double* __restrict__ partial,
                                                                 int n_i, int n_j, int S) {
-    constexpr int I = P::IDIM, J = P::JDIM, F = P::FDIM;
+    constexpr int I = P::IDIM, J = P::JDIM, F = P::FDIM, kPipeK = PipeK<P>::value;
     __shared__ float tile[kPipeTile * J];
     const int i0 = (blockIdx.x * kPipeThreads + threadIdx.x) * kPipeK;
     float xi[kPipeK][I];
@@ -100,7 +102,9 @@ __global__ void __launch_bounds__(128) pipeline_reduce_kernel(const double* __re
 }
 
 // j-chunks across CTAs so that the grid fills the device about twice over (a pure function of the sizes)
+template <class P>
 inline int pipeline_chunks(int64_t n_i, int64_t n_j, int sm_count) {
+    constexpr int kPipeK = PipeK<P>::value;
     const int64_t tiles = (n_i + kPipeThreads * kPipeK - 1) / (kPipeThreads * kPipeK);
     int64_t S = (2 * (int64_t)sm_count + tiles - 1) / tiles;
     const int64_t s_max = n_j / kPipeBlock > 0 ? n_j / kPipeBlock : 1;
@@ -113,7 +117,7 @@ inline int pipeline_chunks(int64_t n_i, int64_t n_j, int sm_count) {
 // Workspace bytes pipeline_run needs when pipeline_chunks(...) > 1 (caller-owned device memory).
 template <class P>
 inline size_t pipeline_workspace_bytes(int64_t n_i, int64_t n_j, int sm_count) {
-    const int S = pipeline_chunks(n_i, n_j, sm_count);
+    const int S = pipeline_chunks<P>(n_i, n_j, sm_count);
     return S > 1 ? (size_t)S * (size_t)n_i * P::FDIM * sizeof(double) : 0;
 }
 
@@ -123,7 +127,8 @@ inline cudaError_t pipeline_run(const float* p_xj, const float* p_xi, float* p_f
                                 int sm_count, cudaStream_t stream) {
     if (n_i <= 0) return cudaSuccess;
     if (n_j <= 0) return cudaMemsetAsync(p_fi, 0, sizeof(float) * (size_t)n_i * P::FDIM, stream);
-    const int S = pipeline_chunks(n_i, n_j, sm_count);
+    constexpr int kPipeK = PipeK<P>::value;
+    const int S = pipeline_chunks<P>(n_i, n_j, sm_count);
     if (S > 1 && !workspace) return cudaErrorInvalidValue;
     const unsigned tiles = (unsigned)((n_i + kPipeThreads * kPipeK - 1) / (kPipeThreads * kPipeK));
     pipeline_kernel<P><<<dim3(tiles, (unsigned)S, 1), kPipeThreads, 0, stream>>>(p_xj, p_xi, p_fi, reinterpret_cast<double*>(workspace),

@@ -179,7 +179,7 @@ int nb_force_eps_i(int64_t n_i, const float *x_i, const float *eps2_i,
  * All rows are DEVICE float arrays (the paper passes host doubles and copies inside; here the caller owns device
  * memory, as for nb_force).  p_fi is overwritten, not accumulated into.  Coincident pairs add nothing (reading R1).
  * These entry points run the listings as written (scalar FP32, any pipeline); nb_force / nb_force_eps_i /
- * nb_force_jerk compute the same sums with the specialised kernels and are 2.2 - 2.4x faster (N = 131072).
+ * nb_force_jerk compute the same sums with the specialised kernels and are 1.8x faster (N = 131072).
  */
 int nb_cunbody_force(const float *p_xj, const float *p_xi, float *p_fi, int64_t ni, int64_t nj, void *stream);
 int nb_cunbody_force_jerk_pot(const float *p_xj, const float *p_xi, float *p_fi, int64_t ni, int64_t nj, void *stream);

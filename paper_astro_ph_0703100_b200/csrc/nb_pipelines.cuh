@@ -6,6 +6,13 @@
 
 namespace nb {
 
+// 1/sqrt as one MUFU.RSQ (the listings' "1/sqrt(r2)"; same instruction as the specialised kernels)
+__device__ __forceinline__ float pipeline_rsqrt(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 // Fig. A.1 / A.3: IDIM 4 = (x, y, z, eps2), JDIM 4 = (x, y, z, m), FDIM 3 = (ax, ay, az)
 struct PipelineForceA3 {
     static constexpr int IDIM = 4, JDIM = 4, FDIM = 3;
@@ -13,10 +20,10 @@ struct PipelineForceA3 {
         const float xi = INPUT_I[0], yi = INPUT_I[1], zi = INPUT_I[2], eps2 = INPUT_I[3];
         const float xj = INPUT_J[0], yj = INPUT_J[1], zj = INPUT_J[2], mj = INPUT_J[3];
         const float dx = xj - xi, dy = yj - yi, dz = zj - zi;
-        if (dx == 0.0f && dy == 0.0f && dz == 0.0f) return;                                 // reading R1
+        const bool coincident = (dx == 0.0f && dy == 0.0f && dz == 0.0f);                   // reading R1, branch-free:
         const float dx2 = dx * dx, dy2 = dy * dy, dz2 = dz * dz;
         const float r2 = (dx2 + dy2) + (dz2 + eps2);
-        const float r1i = rsqrtf(r2);
+        const float r1i = coincident ? 0.0f : pipeline_rsqrt(r2);                           // PAPER.md:465; r1i = 0 => the pair adds 0
         const float r2i = r1i * r1i;
         const float r3i = r2i * r1i;
         const float mr3i = mj * r3i;
@@ -33,10 +40,10 @@ struct PipelineForceJerkPotA4 {
     static __device__ __forceinline__ void pair(const float* INPUT_I, const float* INPUT_J, float* OUTPUT) {
         const float eps2 = 1.0f / (256.0f * 256.0f);
         const float dx_0 = INPUT_J[0] - INPUT_I[0], dx_1 = INPUT_J[1] - INPUT_I[1], dx_2 = INPUT_J[2] - INPUT_I[2];
-        if (dx_0 == 0.0f && dx_1 == 0.0f && dx_2 == 0.0f) return;                           // reading R1
+        const bool coincident = (dx_0 == 0.0f && dx_1 == 0.0f && dx_2 == 0.0f);             // reading R1, branch-free:
         const float mj = INPUT_J[6];
-        const float r2 = dx_0 * dx_0 + dx_1 * dx_1 + dx_2 * dx_2 + eps2;
-        const float r1i = rsqrtf(r2);
+        const float r2 = coincident ? 1.0f : dx_0 * dx_0 + dx_1 * dx_1 + dx_2 * dx_2 + eps2;   // PAPER.md:506-509 (r2 = 1: finite)
+        const float r1i = coincident ? 0.0f : pipeline_rsqrt(r2);                           // PAPER.md:510; r1i = 0 => the pair adds 0
         const float r2i = r1i * r1i, r3i = r1i * r2i, r5i = r2i * r3i;
         const float mr5i = mj * r5i, mf = mr5i * r2, pot = mf * r2;
         const float dv_0 = INPUT_J[3] - INPUT_I[3], dv_1 = INPUT_J[4] - INPUT_I[4], dv_2 = INPUT_J[5] - INPUT_I[5];

@@ -701,7 +701,7 @@ int cunbody_call(const float* p_xj, const float* p_xi, float* p_fi, int64_t ni, 
         NB_CUDA(cudaEventRecord(e1, stream));
         t_events.emplace_back(e0, e1);
     }
-    t_launches = (nj > 0) ? (nb::pipeline_chunks(ni, nj, info.sm_count) > 1 ? 2 : 1) : 0;
+    t_launches = (nj > 0) ? (nb::pipeline_chunks<P>(ni, nj, info.sm_count) > 1 ? 2 : 1) : 0;
     return NB_OK;
 }
 }  // namespace
