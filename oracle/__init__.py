@@ -58,6 +58,8 @@ def _load():
         lib.oracle_force_jerk_f32.restype = ctypes.c_int
         lib.oracle_force_eps_i_f64.argtypes = [i64, p, p, i64, p, p, p, p]
         lib.oracle_force_eps_i_f64.restype = ctypes.c_int
+        lib.oracle_hermite4_f64.argtypes = [i64, p, p, p, f64, f64, i64, p, p, p]
+        lib.oracle_hermite4_f64.restype = ctypes.c_int
         lib.oracle_num_threads.restype = ctypes.c_int
         lib.oracle_set_num_threads.argtypes = [ctypes.c_int]
         _lib = lib
@@ -180,6 +182,21 @@ def leapfrog_kdk(x: np.ndarray, v: np.ndarray, m: np.ndarray, eps2: float, dt: f
     if rc != 0:
         raise ValueError(f"oracle_leapfrog_kdk returned {rc}")
     return xx, vv, acc, pot
+
+
+def hermite4(x: np.ndarray, v: np.ndarray, m: np.ndarray, eps2: float, dt: float, n_steps: int):
+    """Shared-time-step 4th-order Hermite (predict-evaluate-correct) in double.  Returns (x, v, acc, jerk, pot);
+    inputs are not modified."""
+    xx = np.array(x, dtype=np.float64, order="C").reshape(-1, 3)
+    vv = np.array(v, dtype=np.float64, order="C").reshape(-1, 3)
+    mm = _c(m, np.float64).reshape(-1)
+    n = xx.shape[0]
+    acc = np.zeros((n, 3)); jerk = np.zeros((n, 3)); pot = np.zeros(n)
+    rc = _load().oracle_hermite4_f64(n, _ptr(xx), _ptr(vv), _ptr(mm), float(eps2), float(dt), int(n_steps),
+                                     _ptr(acc), _ptr(jerk), _ptr(pot))
+    if rc != 0:
+        raise ValueError(f"oracle_hermite4 returned {rc}")
+    return xx, vv, acc, jerk, pot
 
 
 def error_metrics(acc_test: np.ndarray, acc_ref: np.ndarray, pot_test: Optional[np.ndarray] = None,

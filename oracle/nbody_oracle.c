@@ -314,3 +314,48 @@ int oracle_force_eps_i_f64(int64_t n_i, const double *x_i, const double *eps2_i,
     }
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Fourth-order Hermite integration with a shared, constant time step -- the scheme the paper names as the user
+ * of its force + jerk pipeline ("Hermite scheme"), not described in the paper itself.
+ * Textbook predict - evaluate - correct form (Makino & Aarseth 1992), one evaluation per step:
+ *
+ *     a0, j0 = force_jerk(x, v)                                   once, before the first step
+ *     xp = x + v dt + a0 dt^2/2 + j0 dt^3/6      vp = v + a0 dt + j0 dt^2/2            (predict)
+ *     a1, j1 = force_jerk(xp, vp)                                                       (evaluate)
+ *     v' = v + (a0 + a1) dt/2 + (j0 - j1) dt^2/12                                       (correct)
+ *     x' = x + (v + v') dt/2 + (a0 - a1) dt^2/12
+ *     a0, j0 <- a1, j1            (the values at the predicted state are carried to the next step)
+ *
+ * Pins (tests/test_oracle_hermite_pins.py, "h7"): agreement with an adaptive high-order ODE solver (scipy DOP853)
+ * on a three-body problem, error ratio ~16 when dt halves (4th order), energy error far below the leapfrog's.
+ * x, v [n][3] updated in place; acc, jerk [n][3] and pot [n] receive the values carried out of the last step.
+ */
+int oracle_hermite4_f64(int64_t n, double *x, double *v, const double *m, double eps2, double dt, int64_t n_steps,
+                        double *acc, double *jerk, double *pot)
+{
+    if (n < 0 || n_steps < 0 || !(eps2 >= 0.0)) return 1;
+    if (n > 0 && (!x || !v || !m || !acc || !jerk || !pot)) return 1;
+    size_t n3 = 3 * (size_t)(n > 0 ? n : 1);
+    double *xp = (double *)malloc(sizeof(double) * n3), *vp = (double *)malloc(sizeof(double) * n3);
+    double *a1 = (double *)malloc(sizeof(double) * n3), *j1 = (double *)malloc(sizeof(double) * n3);
+    if (!xp || !vp || !a1 || !j1) { free(xp); free(vp); free(a1); free(j1); return 2; }
+    int rc = oracle_force_jerk_f64(n, x, v, n, x, v, m, eps2, acc, jerk, pot);
+    const double h = dt, h2 = dt * dt, h3 = dt * dt * dt;
+    for (int64_t s = 0; s < n_steps && rc == 0; ++s) {
+        for (int64_t k = 0; k < 3 * n; ++k) {                                   /* predict */
+            xp[k] = x[k] + v[k] * h + acc[k] * (h2 / 2.0) + jerk[k] * (h3 / 6.0);
+            vp[k] = v[k] + acc[k] * h + jerk[k] * (h2 / 2.0);
+        }
+        rc = oracle_force_jerk_f64(n, xp, vp, n, xp, vp, m, eps2, a1, j1, pot);   /* evaluate */
+        for (int64_t k = 0; k < 3 * n; ++k) {                                   /* correct */
+            double vn = v[k] + (acc[k] + a1[k]) * (h / 2.0) + (jerk[k] - j1[k]) * (h2 / 12.0);
+            x[k] = x[k] + (v[k] + vn) * (h / 2.0) + (acc[k] - a1[k]) * (h2 / 12.0);
+            v[k] = vn;
+            acc[k] = a1[k];
+            jerk[k] = j1[k];
+        }
+    }
+    free(xp); free(vp); free(a1); free(j1);
+    return rc;
+}

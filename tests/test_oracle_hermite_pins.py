@@ -159,3 +159,61 @@ def test_h6_edge_sizes_and_coincidence():
     one = np.array([[1.0, 2.0, 3.0]])
     a, j, p = oracle.force_jerk(one, np.array([[1.0, 0, 0]]), one, np.array([[0, 5.0, 0]]), np.array([2.0]), 0.0)
     assert not a.any() and not j.any() and p[0] == 0.0               # coincident in position: nothing, even at eps2 = 0
+
+
+# ----------------------------------------------------------------------------- h7: the Hermite integrator
+def _three_body():
+    x = np.array([[1.0, 0.0, 0.0], [-0.5, 0.8, 0.1], [-0.4, -0.9, -0.2]])
+    v = np.array([[0.0, 0.4, 0.1], [-0.35, -0.2, 0.0], [0.3, -0.15, -0.1]])
+    m = np.array([1.0, 0.8, 1.2])
+    return x, v, m
+
+
+def _energy3(x, v, m, eps2):
+    t = 0.5 * (m * (v * v).sum(1)).sum()
+    w = 0.0
+    for a in range(len(m)):
+        for b in range(a + 1, len(m)):
+            w -= m[a] * m[b] / np.sqrt(((x[a] - x[b]) ** 2).sum() + eps2)
+    return t + w
+
+
+def test_h7_hermite_matches_an_adaptive_high_order_solver_and_is_fourth_order():
+    from scipy.integrate import solve_ivp
+    x0, v0, m = _three_body()
+    eps2, T = 0.01, 1.0
+
+    def rhs(t, y):
+        x, v = y[:9].reshape(3, 3), y[9:].reshape(3, 3)
+        a = np.zeros((3, 3))
+        for p in range(3):
+            for q in range(3):
+                if p != q:
+                    d = x[q] - x[p]
+                    a[p] += m[q] * d / (d @ d + eps2) ** 1.5
+        return np.concatenate([v.ravel(), a.ravel()])
+
+    sol = solve_ivp(rhs, (0.0, T), np.concatenate([x0.ravel(), v0.ravel()]), method="DOP853", rtol=1e-13, atol=1e-14)
+    x_ref, v_ref = sol.y[:9, -1].reshape(3, 3), sol.y[9:, -1].reshape(3, 3)
+    errs = []
+    for steps in (32, 64, 128):
+        x, v, _, _, _ = oracle.hermite4(x0, v0, m, eps2, T / steps, steps)
+        errs.append(max(np.abs(x - x_ref).max(), np.abs(v - v_ref).max()))
+    assert errs[2] < 2e-7
+    assert 11.0 < errs[0] / errs[1] < 22.0 and 11.0 < errs[1] / errs[2] < 22.0       # error ~ dt^4
+
+
+def test_h7_hermite_energy_error_far_below_leapfrog_and_outputs_are_the_carried_values():
+    x0, v0, m = _three_body()
+    eps2, dt, steps = 0.01, 1.0 / 64, 64
+    e0 = _energy3(x0, v0, m, eps2)
+    xh, vh, ah, jh, ph = oracle.hermite4(x0, v0, m, eps2, dt, steps)
+    xl, vl, _, _ = oracle.leapfrog_kdk(x0, v0, m, eps2, dt, steps)
+    err_h, err_l = abs(_energy3(xh, vh, m, eps2) - e0), abs(_energy3(xl, vl, m, eps2) - e0)
+    assert err_h < 1e-7 and err_h < 0.02 * err_l
+    tot = (m[:, None] * vh).sum(0) - (m[:, None] * v0).sum(0)
+    assert np.abs(tot).max() < 1e-14                                              # momentum
+    # zero steps: just the evaluation
+    x, v, a, j, p = oracle.hermite4(x0, v0, m, eps2, dt, 0)
+    ra, rj, rp = oracle.force_jerk(x0, v0, x0, v0, m, eps2)
+    assert np.array_equal(x, x0) and np.array_equal(a, ra) and np.array_equal(j, rj) and np.array_equal(p, rp)
