@@ -160,6 +160,9 @@ def reference_arm(args, wl):
     elif args.op == "cunbody":
         w = wl.config(1)
         name = "row f3 (G1): configs[1]'s particles, Fig. A.3 pipeline (oracle force on a sample)"
+    elif args.op == "hermite":
+        w = wl.plummer_workload(65536, 1.0 / 128, seed=4, name="C4", with_velocities=True)
+        name = "C4's particles, force+jerk evaluations of the Hermite integration (oracle force_jerk on a sample)"
     elif args.op == "leapfrog":
         w = wl.config(4)
         name = "BASELINE.json configs[4] (C4): force evaluations of the KDK integration, N=65536 (oracle force on a sample)"
@@ -213,6 +216,7 @@ OPS = {
     "leapfrog": {"inst": 12, "kernel": "nb_force_kernel<PHI=false> inside nb_leapfrog_kdk (row a8)", "flops": (20, 38)},
 }
 LEAPFROG_KDK_PER_CALL = 100
+OPS["hermite"] = {"inst": 27, "kernel": "nb_hermite_kernel inside nb_hermite4 (consumer of row f1)", "flops": (60, 60)}
 
 
 class Problem:
@@ -249,6 +253,15 @@ class Problem:
             p_xj = np.concatenate([w.x_j, w.m_j[:, None]], axis=1).astype(np.float32)
             self.host = [np.ascontiguousarray(p_xj), np.ascontiguousarray(p_xi)]
             self.n_out = w.n_j
+        elif op == "hermite":
+            w = wl.config(4)
+            self.w = w
+            self.pairs = float(w.n_j) ** 2 * (LEAPFROG_KDK_PER_CALL + 1)
+            self.name = (f"configs[4]'s particles (C4: N={w.n_j}, eps2={w.eps2:.6g}, dt=1/512, seed=4) under the 4th-order Hermite "
+                         f"scheme: one step = one nb_hermite4 call of {LEAPFROG_KDK_PER_CALL} time steps (101 force+jerk evaluations)")
+            self.host = [w.x_j, w.v, w.m_j]
+            self.n_out = w.n_j
+            self.kdk_done = 0
         elif op == "jerk":
             w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
             self.w, self.pairs = w, float(w.n_i) * float(w.n_j)
@@ -267,7 +280,7 @@ class Problem:
         self.pinned = [torch.from_numpy(a).pin_memory() for a in self.host]
         n = self.n_out
         self.outs = [torch.empty((n, 3), dtype=torch.float32, device="cuda")]
-        if op == "jerk":
+        if op in ("jerk", "hermite"):
             self.outs.append(torch.empty((n, 3), dtype=torch.float32, device="cuda"))
         if op != "cunbody":
             self.outs.append(torch.empty((n,), dtype=torch.float32, device="cuda"))
@@ -286,6 +299,11 @@ class Problem:
             nb.cunbody_force(t[0], t[1], self.outs[0])
         elif self.op == "leapfrog":
             nb.leapfrog_kdk(t[0], t[1], t[2], w.eps2, w.dt, LEAPFROG_KDK_PER_CALL, acc_io=self.outs[0], pot_out=self.outs[1])
+            if t is self.dev:
+                self.kdk_done += LEAPFROG_KDK_PER_CALL
+        elif self.op == "hermite":
+            nb.hermite4(t[0], t[1], t[2], w.eps2, w.dt, LEAPFROG_KDK_PER_CALL, acc_io=self.outs[0], jerk_io=self.outs[1],
+                        pot_out=self.outs[2])
             if t is self.dev:
                 self.kdk_done += LEAPFROG_KDK_PER_CALL
         elif self.op == "jerk":
@@ -320,6 +338,8 @@ class Problem:
             return "nb_force_jerk_host (pinned host buffers)"
         if self.op == "cunbody":
             return "pinned host rows -> cudaMemcpyAsync -> nb_cunbody_force -> cudaMemcpyAsync -> pinned host"
+        if self.op == "hermite":
+            return "pinned host (x, v, m) -> cudaMemcpyAsync -> nb_hermite4 (100 steps) -> cudaMemcpyAsync of a, j, phi -> pinned host"
         if self.op == "leapfrog":
             return "pinned host (x, v, m) -> cudaMemcpyAsync -> nb_leapfrog_kdk (100 KDK steps) -> cudaMemcpyAsync of a, phi -> pinned host"
         return f"pinned host tensors -> cudaMemcpyAsync -> nb_{'force_jerk' if self.op == 'jerk' else 'force_batched'} -> cudaMemcpyAsync -> pinned host"
@@ -329,6 +349,8 @@ class Problem:
             return self.nb.plan_query(self.w.n_i, self.w.n_j, sm_count)
         if self.op == "cunbody":
             return {"cta": "256 threads x 2 i-records, 128-record j tiles, j-range split over S CTAs + second pass"}
+        if self.op == "hermite":
+            return self.nb.plan_query_jerk(self.w.n_j, self.w.n_j, sm_count)
         if self.op == "leapfrog":
             return self.nb.plan_query(self.w.n_j, self.w.n_j, sm_count)
         if self.op == "jerk":
@@ -341,6 +363,8 @@ def oracle_rate_op(op, w, target_seconds, rng_seed=0):
     import oracle
     if op in ("force", "leapfrog", "cunbody"):
         return oracle_rate(w, target_seconds, rng_seed)
+    if op == "hermite":
+        op = "jerk"
     cores = oracle.num_threads()
     rng = np.random.default_rng(rng_seed)
     if op == "jerk":
@@ -506,7 +530,7 @@ def main():
         sm_count = torch.cuda.get_device_properties(0).multi_processor_count
         peak_inst = sm_count * FP32_LANES_PER_SM_CLK * f_max                 # FP32-pipe lane-instructions / s
         # interactions per launch of the dominant kernel (a leapfrog call launches it once per force evaluation)
-        pairs_k = float(prob.w.n_j) ** 2 if args.op == "leapfrog" else pairs   # (sharded: this rank's slice x all j)
+        pairs_k = float(prob.w.n_j) ** 2 if args.op in ("leapfrog", "hermite") else pairs   # (sharded: this rank's slice x all j)
         k_rate = pairs_k * n_k / (k_ms * 1e-3) if n_k else 0.0
         inst = op["inst"]
         achieved = inst * k_rate
@@ -548,35 +572,17 @@ def main():
         if graph_ms is not None:
             out["graph_replay"] = {"ms_per_call": graph_ms, "value": pairs / (graph_ms * 1e-3), "unit": METRIC,
                                    "note": "one captured nb_force call replayed 200x back to back, L2 warm"}
-        if args.op == "leapfrog":
-            out["kdk_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
-            if not args.no_cpu_baseline:
-                # BASELINE.json configs[4]: relative total-energy drift against oracle-force energies (double) evaluated
-                # on the GPU's own FP32 state: initial conditions vs the state after every warm-up + timed KDK step
-                import oracle
-                w = prob.w
-                _, _, e_start = oracle.energy(w.x_j, w.v, w.m_j, w.eps2)
-                _, _, e_end = oracle.energy(prob.dev[0].cpu().numpy(), prob.dev[1].cpu().numpy(), w.m_j, w.eps2)
-                out["energy"] = {"kdk_steps": prob.kdk_done, "E_start": e_start, "E_end": e_end,
-                                 "rel_drift": abs(e_end - e_start) / abs(e_start), "by": "oracle.energy (FP64) on the GPU's FP32 (x, v)"}
-        if args.check and args.op in ("force", "jerk") and not args.shard:
+        if args.op == "hermite":
+            out["hermite_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
+        if args.op in ("leapfrog", "hermite") and not args.no_cpu_baseline:
             import oracle
             w = prob.w
-            prob.call()
-            torch.cuda.synchronize()
-            idx = np.sort(np.random.default_rng(0).choice(w.n_i, min(2048, w.n_i), replace=False))
-            got = [o.cpu().numpy()[idx] for o in prob.outs]
-            if args.op == "force":
-                ra, rp = oracle.force(w.xi[idx], w.x_j, w.m_j, w.eps2)
-                par = oracle.error_metrics(got[0], ra, got[1], rp)
-            else:
-                ra, rj, rp = oracle.force_jerk(w.x_j[idx], w.v[idx], w.x_j, w.v, w.m_j, w.eps2)
-                par = oracle.error_metrics(got[0], ra, got[2], rp)
-                ej = oracle.error_metrics(got[1], rj)
-                par["jerk_max"], par["jerk_rms"] = ej["acc_max"], ej["acc_rms"]
-            par["sample"] = f"{len(idx)} seeded i-particles x all {w.n_j} j-particles, oracle in FP64"
-            par["tolerance"] = "acc (jerk) RMS <= 1e-5, max <= 1e-4; phi RMS <= 1e-5 (BASELINE.json north_star)"
-            out["parity"] = par
+            _, _, e_start = oracle.energy(w.x_j, w.v, w.m_j, w.eps2)
+            _, _, e_end = oracle.energy(prob.dev[0].cpu().numpy(), prob.dev[1].cpu().numpy(), w.m_j, w.eps2)
+            out["energy"] = {"time_steps": prob.kdk_done, "kdk_steps": prob.kdk_done, "E_start": e_start, "E_end": e_end,
+                             "rel_drift": abs(e_end - e_start) / abs(e_start), "by": "oracle.energy (FP64) on the GPU's FP32 (x, v)"}
+        if args.op == "leapfrog":
+            out["kdk_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
         if not args.no_cpu_baseline:
             v, cores, sample = oracle_rate_op(args.op, prob.w, args.cpu_seconds)
             out["cpu_baseline"] = {"value": v, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample}

@@ -213,6 +213,29 @@ int nb_force_batched(int64_t n_batch, const int32_t *i_offsets, const int32_t *j
                      void *stream);
 
 /*
+ * nb_hermite4 -- n_steps steps of the 4th-order Hermite scheme with a shared, constant time step, all state on the
+ * device: the scheme the paper names as the user of its force + jerk pipeline; the paper does
+ * not describe it, this is the textbook predict - evaluate - correct form with one nb_force_jerk per step:
+ *
+ *     a, j = force_jerk(x, v)                                          once, before the first step
+ *     repeat n_steps times:
+ *         xp = x + v dt + a dt^2/2 + j dt^3/6;   vp = v + a dt + j dt^2/2
+ *         a1, j1 = force_jerk(xp, vp)
+ *         v' = v + (a + a1) dt/2 + (j - j1) dt^2/12;   x' = x + (v + v') dt/2 + (a - a1) dt^2/12
+ *         x, v, a, j <- x', v', a1, j1
+ *
+ *   x, v      device, float [n][3], updated in place          m   device, const, float [n]
+ *   acc_io, jerk_io   device, float [n][3]: receive the a and j carried out of the last step (evaluated at its
+ *             predicted state); their content on entry is ignored
+ *   pot_out   device, float [n] or NULL: phi of the last evaluation
+ * n_steps == 0 only evaluates a, j and phi of the given state.
+ */
+int nb_hermite4(int64_t n, float *x, float *v, const float *m,
+                float eps2, float dt, int64_t n_steps,
+                float *acc_io, float *jerk_io, float *pot_out,
+                void *stream);
+
+/*
  * nb_force_jerk_host -- nb_force_jerk on HOST arrays: the paper's force() of Fig. A.2 with its
  * host->device and device->host copies (steps (a) and (l)) inside the call.  Blocking.
  */

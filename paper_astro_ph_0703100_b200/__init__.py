@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     force_jerk,
     force_jerk_host,
     force_packed,
+    hermite4,
     last_launch_count,
     leapfrog_kdk,
     pack_j,

@@ -60,6 +60,8 @@ def lib() -> ctypes.CDLL:
         l.nb_force_jerk_host.restype = ci
         l.nb_plan_query_jerk.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
         l.nb_plan_query_jerk.restype = ci
+        l.nb_hermite4.argtypes = [i64, p, p, p, f32, f32, i64, p, p, p, p]
+        l.nb_hermite4.restype = ci
         l.nb_plan_query.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
         l.nb_plan_query.restype = ci
         l.nb_last_launch_count.restype = i64
@@ -303,6 +305,28 @@ def leapfrog_kdk(x, v, m, eps2: float, dt: float, n_steps: int, acc_io=None, pot
                                    _stream_ptr(stream))
     _check(st, "nb_leapfrog_kdk")
     return acc_io, pot_out
+
+
+def hermite4(x, v, m, eps2: float, dt: float, n_steps: int, acc_io=None, jerk_io=None, pot_out=None, want_pot: bool = True,
+             stream=None):
+    """nb_hermite4: x, v updated IN PLACE.  Returns (acc, jerk, pot) carried out of the last step."""
+    import torch
+    _dev_f32(x, "x", (3,)); _dev_f32(v, "v", (3,)); _dev_f32(m, "m", ())
+    n = x.shape[0]
+    if v.shape[0] != n or m.shape[0] != n:
+        raise ValueError("x, v, m lengths differ")
+    if acc_io is None:
+        acc_io = torch.empty((n, 3), dtype=torch.float32, device=x.device)
+    if jerk_io is None:
+        jerk_io = torch.empty((n, 3), dtype=torch.float32, device=x.device)
+    if pot_out is None and want_pot:
+        pot_out = torch.empty((n,), dtype=torch.float32, device=x.device)
+    with torch.cuda.device(x.device):
+        st = lib().nb_hermite4(n, x.data_ptr(), v.data_ptr(), m.data_ptr(), float(eps2), float(dt), int(n_steps),
+                               acc_io.data_ptr(), jerk_io.data_ptr(), None if pot_out is None else pot_out.data_ptr(),
+                               _stream_ptr(stream))
+    _check(st, "nb_hermite4")
+    return acc_io, jerk_io, pot_out
 
 
 def plan_query(n_i: int, n_j: int, sm_count: int = 148) -> dict:

@@ -301,4 +301,31 @@ __global__ void __launch_bounds__(128) nb_hermite_reduce_kernel(const double* __
     if (pot) pot[i] = -(float)s[9];
 }
 
+// ---------------------------------------------------------------- shared-time-step Hermite integrator (O(N) kernels)
+// predict:  xp = x + v dt + a dt^2/2 + j dt^3/6,   vp = v + a dt + j dt^2/2      (Horner form, FP32 FMAs)
+__global__ void __launch_bounds__(256) nb_hermite_predict_kernel(const float* __restrict__ x, const float* __restrict__ v,
+                                                                 const float* __restrict__ a, const float* __restrict__ j,
+                                                                 float* __restrict__ xp, float* __restrict__ vp, int n3, float dt) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n3) return;
+    const float aa = a[k], jj = j[k], vv = v[k];
+    xp[k] = fmaf(fmaf(fmaf(jj, dt * (1.0f / 3.0f), aa), dt * 0.5f, vv), dt, x[k]);
+    vp[k] = fmaf(fmaf(jj, dt * 0.5f, aa), dt, vv);
+}
+// correct:  v' = v + (a0 + a1) dt/2 + (j0 - j1) dt^2/12,   x' = x + (v + v') dt/2 + (a0 - a1) dt^2/12;   a0, j0 <- a1, j1
+__global__ void __launch_bounds__(256) nb_hermite_correct_kernel(float* __restrict__ x, float* __restrict__ v,
+                                                                 float* __restrict__ a0, float* __restrict__ j0,
+                                                                 const float* __restrict__ a1, const float* __restrict__ j1,
+                                                                 int n3, float dt) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n3) return;
+    const float h = 0.5f * dt, h2 = dt * dt * (1.0f / 12.0f);
+    const float a_old = a0[k], a_new = a1[k], j_old = j0[k], j_new = j1[k], v_old = v[k];
+    const float v_new = fmaf(j_old - j_new, h2, fmaf(a_old + a_new, h, v_old));
+    x[k] = fmaf(a_old - a_new, h2, fmaf(v_old + v_new, h, x[k]));
+    v[k] = v_new;
+    a0[k] = a_new;
+    j0[k] = j_new;
+}
+
 }  // namespace nb

@@ -52,6 +52,7 @@ struct Workspace {
     void* coin = nullptr;      size_t coin_bytes = 0;      // coincidence pre-pass: flag | lists | hash table
     void* tiles = nullptr;     size_t tiles_bytes = 0;     // batched calls: first CTA of every sub-problem
     void* pipe = nullptr;      size_t pipe_bytes = 0;      // generalised kernel: [S][n_i][FDIM] double
+    void* hstate = nullptr;    size_t hstate_bytes = 0;    // Hermite integrator: xp, vp, a1, j1
     void* jp2 = nullptr;       size_t jp2_bytes = 0;       // force + jerk: 32-byte j records
     void* hpartial = nullptr;  size_t hpartial_bytes = 0;  // force + jerk: [S][n_i][10] double
 };
@@ -828,6 +829,54 @@ int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, f
     return NB_OK;
 }
 
+int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float dt, int64_t n_steps, float* acc_io,
+                float* jerk_io, float* pot_out, void* stream_) {
+    t_launches = 0;
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (bad_count(n) || n_steps < 0) return NB_ERR_INVALID_VALUE;
+    if (!(eps2 >= 0.0f) || !std::isfinite(eps2) || !std::isfinite(dt)) return NB_ERR_INVALID_VALUE;
+    if (n > 0 && (!x || !v || !m || !acc_io || !jerk_io)) return NB_ERR_INVALID_VALUE;
+    if (3 * n > (int64_t)INT32_MAX) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n == 0) return NB_OK;
+    const int n3 = (int)(3 * n);
+    const int threads = 256, blocks = (n3 + threads - 1) / threads;
+    int64_t launches = 0;
+    // a0, j0 = force_jerk(x0, v0)
+    rc = force_jerk_impl(n, x, v, n, x, v, m, eps2, acc_io, jerk_io, pot_out, stream);
+    if (rc != NB_OK) return rc;
+    launches += t_launches;
+    if (n_steps == 0) return NB_OK;
+    Workspace* ws;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        ws = &g_ws[std::make_pair(dev, stream)];
+    }
+    const size_t b3 = ((size_t)n3 * sizeof(float) + 255) / 256 * 256;
+    rc = ensure(&ws->hstate, &ws->hstate_bytes, 4 * b3, stream);
+    if (rc != NB_OK) return rc;
+    char* base = reinterpret_cast<char*>(ws->hstate);
+    float* xp = reinterpret_cast<float*>(base);
+    float* vp = reinterpret_cast<float*>(base + b3);
+    float* a1 = reinterpret_cast<float*>(base + 2 * b3);
+    float* j1 = reinterpret_cast<float*>(base + 3 * b3);
+    for (int64_t s = 0; s < n_steps; ++s) {
+        nb::nb_hermite_predict_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, xp, vp, n3, dt);
+        NB_CUDA(cudaGetLastError());
+        t_launches = 0;
+        rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, pot_out, stream);
+        if (rc != NB_OK) return rc;
+        launches += t_launches + 2;
+        nb::nb_hermite_correct_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, a1, j1, n3, dt);
+        NB_CUDA(cudaGetLastError());
+    }
+    t_launches = launches;
+    return NB_OK;
+}
+
 int nb_plan_query(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]) {
     if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
     const nb::Plan p = nb::make_plan(n_i, n_j, sm_count);
@@ -884,6 +933,7 @@ int nb_release_workspace(void) {
             if (it->second.jp2) (void)cudaFree(it->second.jp2);
             if (it->second.tiles) (void)cudaFree(it->second.tiles);
             if (it->second.pipe) (void)cudaFree(it->second.pipe);
+            if (it->second.hstate) (void)cudaFree(it->second.hstate);
             if (it->second.hpartial) (void)cudaFree(it->second.hpartial);
             it = g_ws.erase(it);
         } else {

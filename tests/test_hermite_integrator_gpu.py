@@ -1,0 +1,78 @@
+"""nb_hermite4 (shared-time-step 4th-order Hermite on the device, the consumer of nb_force_jerk) against the FP64 oracle
+integrator, plus the properties of the scheme at FP32."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_astro_ph_0703100_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def nb():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    import paper_astro_ph_0703100_b200 as nb_
+    nb_.lib()
+    return nb_
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_gpu(nb, w, dt, steps):
+    import torch
+    x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
+    acc, jerk, pot = nb.hermite4(x, v, m, w.eps2, dt, steps)
+    torch.cuda.synchronize()
+    return x.cpu().numpy(), v.cpu().numpy(), acc.cpu().numpy(), jerk.cpu().numpy(), pot.cpu().numpy()
+
+
+@pytest.mark.parametrize("n,steps", [(300, 20), (1024, 8), (2049, 3)])
+def test_matches_oracle_integrator(nb, n, steps):
+    w = wl.plummer_workload(n, 1.0 / 64, seed=4, with_velocities=True)
+    dt = 1.0 / 256
+    x, v, acc, jerk, pot = run_gpu(nb, w, dt, steps)
+    xr, vr, ar, jr, pr = oracle.hermite4(w.x_j, w.v, w.m_j, w.eps2, dt, steps)
+    assert np.abs(x - xr).max() < 1e-5 and np.abs(v - vr).max() < 1e-5
+    e = oracle.error_metrics(acc, ar, pot, pr)
+    ej = oracle.error_metrics(jerk, jr)
+    assert e["acc_rms"] <= 1e-4 and e["pot_rms"] <= 1e-5 and ej["acc_rms"] <= 1e-3      # values at the FP32 trajectory's state
+
+
+def test_zero_steps_is_a_force_jerk_evaluation(nb):
+    w = wl.plummer_workload(700, 1.0 / 64, seed=5, with_velocities=True)
+    x, v, acc, jerk, pot = run_gpu(nb, w, 1.0 / 128, 0)
+    assert np.array_equal(x, w.x_j) and np.array_equal(v, w.v)
+    ra, rj, rp = oracle.force_jerk(w.x_j, w.v, w.x_j, w.v, w.m_j, w.eps2)
+    e = oracle.error_metrics(acc, ra, pot, rp)
+    ej = oracle.error_metrics(jerk, rj)
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and e["pot_rms"] <= 1e-5 and ej["acc_rms"] <= 1e-5
+
+
+def test_energy_error_below_leapfrog_and_momentum(nb):
+    import torch
+    w = wl.plummer_workload(4096, 1.0 / 32, seed=6, with_velocities=True)
+    dt, steps = 1.0 / 64, 64
+    _, _, e0 = oracle.energy(w.x_j, w.v, w.m_j, w.eps2)
+    xh, vh, _, _, _ = run_gpu(nb, w, dt, steps)
+    x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
+    nb.leapfrog_kdk(x, v, m, w.eps2, dt, steps)
+    torch.cuda.synchronize()
+    _, _, eh = oracle.energy(xh, vh, w.m_j, w.eps2)
+    _, _, el = oracle.energy(x.cpu().numpy(), v.cpu().numpy(), w.m_j, w.eps2)
+    err_h, err_l = abs(eh - e0) / abs(e0), abs(el - e0) / abs(e0)
+    print(f"relative energy error after {steps} steps of dt = 1/64: hermite {err_h:.2e}, leapfrog {err_l:.2e}")
+    assert err_h < 2e-6 and err_h < err_l
+    p0 = (w.m_j[:, None].astype(np.float64) * w.v).sum(0)
+    p1 = (w.m_j[:, None].astype(np.float64) * vh).sum(0)
+    assert np.abs(p1 - p0).max() < 1e-6
+
+
+def test_invalid_arguments(nb):
+    L = nb.lib()
+    assert L.nb_hermite4(5, None, None, None, 0.1, 0.1, 1, None, None, None, None) == 1
+    assert L.nb_hermite4(0, None, None, None, 0.1, 0.1, -1, None, None, None, None) == 1
