@@ -469,3 +469,54 @@ def test_f3_brute_force_random_eps2_per_i():
         np.testing.assert_allclose(pot[i], rp[0], rtol=1e-13)
     with pytest.raises(ValueError):
         oracle.force_eps_i(x, -e2 - 1.0, x, m)
+
+
+# ----------------------------------------------------------------------------- P13: a = -grad(phi), Gauss, Newton
+def test_p13_acceleration_is_minus_the_gradient_of_the_potential():
+    """Eq. (1) and the potential of Fig. A.4 must be consistent: a_i = -d phi / d r_i for a probe (an i-particle that
+    is not in the j-set).  Central differences of the oracle's OWN phi, Richardson-extrapolated."""
+    rng = np.random.default_rng(21)
+    xj = rng.normal(size=(50, 3)); mj = rng.uniform(0.5, 1.5, 50)
+    probes = rng.normal(size=(6, 3)) * 1.5
+    for eps2 in (0.0, 0.05):
+        acc, _ = oracle.force(probes, xj, mj, eps2)
+        grad = np.zeros_like(acc)
+        for c in range(3):
+            for h, wgt in ((1e-3, 4.0 / 3.0), (2e-3, -1.0 / 3.0)):
+                e = np.zeros(3); e[c] = h
+                _, pp = oracle.force(probes + e, xj, mj, eps2)
+                _, pm = oracle.force(probes - e, xj, mj, eps2)
+                grad[:, c] += wgt * (pp - pm) / (2 * h)
+        np.testing.assert_allclose(acc, -grad, rtol=2e-7, atol=1e-9)
+
+
+def test_p13_newton_shell_theorem_and_gauss_flux():
+    """A thin spherical shell of mass M (many equal points on a sphere of radius R, eps = 0): no force inside,
+    M / r^2 toward the centre outside; phi = -M / R inside (Newton's theorems, to the sampling error of the shell)."""
+    n, R, M = 20000, 1.0, 1.0
+    k = np.arange(n) + 0.5                                   # Fibonacci sphere: quasi-uniform points
+    z = 1 - 2 * k / n; phi = np.pi * (1 + 5 ** 0.5) * k
+    shell = R * np.stack([np.sqrt(1 - z * z) * np.cos(phi), np.sqrt(1 - z * z) * np.sin(phi), z], 1)
+    m = np.full(n, M / n)
+    inside = np.array([[0.0, 0.0, 0.0], [0.3, -0.2, 0.1], [0.0, 0.5, 0.0]])
+    outside = np.array([[2.0, 0.0, 0.0], [0.0, -3.0, 4.0]])
+    a_in, p_in = oracle.force(inside, shell, m, 0.0)
+    a_out, p_out = oracle.force(outside, shell, m, 0.0)
+    assert np.abs(a_in).max() < 2e-4 and np.abs(p_in + M / R).max() < 1e-5
+    r = np.linalg.norm(outside, axis=1)
+    np.testing.assert_allclose(a_out, -M * outside / r[:, None] ** 3, rtol=1e-5, atol=1e-6)
+    np.testing.assert_allclose(p_out, -M / r, rtol=1e-6)
+
+
+def test_p13_mass_linearity_and_superposition():
+    rng = np.random.default_rng(22)
+    xi = rng.normal(size=(9, 3)); xj = rng.normal(size=(40, 3)); mj = rng.uniform(0.5, 1.5, 40)
+    a, p = oracle.force(xi, xj, mj, 0.02)
+    a2, p2 = oracle.force(xi, xj, 3.5 * mj, 0.02)
+    np.testing.assert_allclose(a2, 3.5 * a, rtol=1e-14); np.testing.assert_allclose(p2, 3.5 * p, rtol=1e-14)
+    aa, pa = oracle.force(xi, xj[:17], mj[:17], 0.02)
+    ab, pb = oracle.force(xi, xj[17:], mj[17:], 0.02)
+    np.testing.assert_allclose(aa + ab, a, rtol=1e-13, atol=1e-15); np.testing.assert_allclose(pa + pb, p, rtol=1e-13)
+    perm = rng.permutation(40)                               # the order of the j-particles does not matter (to rounding)
+    a3, p3 = oracle.force(xi, xj[perm], mj[perm], 0.02)
+    np.testing.assert_allclose(a3, a, rtol=1e-13, atol=1e-15); np.testing.assert_allclose(p3, p, rtol=1e-13)
