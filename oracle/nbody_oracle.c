@@ -35,7 +35,8 @@
  * Pins (tests/test_oracle_pins.py): exact two-body rationals, coincident rule, momentum
  * antisymmetry, translation / rotation / axis-permutation invariance, Plummer and uniform-sphere
  * potential energies, brute force in exact rational arithmetic at N <= 8, large-eps limit, regular
- * figures, softened circular binary, time reversal, dt^2 convergence.
+ * figures, softened circular binary, time reversal, dt^2 convergence, a = -grad(phi), Newton's shell theorems,
+ * superposition.
  * Parity unpinned: nothing in this file.  (The *value* of C4's energy drift is not pinned by the
  * paper -- see DESIGN.md -- but that is a property of the FP32 path, not an oracle function.)
  *
