@@ -400,3 +400,51 @@ def test_small_call_direct_pack_path_agrees_bitwise(nb, n_i, n_j, monkeypatch):
     ref_acc, ref_pot = oracle.force(x_i, x_j, m_j, w.eps2)
     if n_i > 1:
         check_parity(a1, p1, ref_acc, ref_pot, f"direct {n_i}x{n_j}")
+
+
+# ------------------------------------------------------------------ stress cases for the FP32 arithmetic
+def test_far_from_the_origin_large_mass_contrast_and_tight_cluster(nb):
+    rng = np.random.default_rng(40)
+    w = wl.plummer_workload(4000, 1.0 / 64, seed=41)
+    # (i) the whole system shifted by ~1000 length units: d = r_j - r_i is still formed exactly from the FP32 inputs
+    xs = (w.x_j.astype(np.float64) + np.array([1000.0, -2000.0, 512.0])).astype(np.float32)
+    acc, pot = gpu_force(nb, xs, xs, w.m_j, w.eps2, alias=True)
+    ra, rp = oracle.force(xs, xs, w.m_j, w.eps2)
+    check_parity(acc, pot, ra, rp, "shifted")
+    # (ii) masses spread over six decades (a few particles dominate every sum)
+    m = (10.0 ** rng.uniform(-6, 0, 4000)).astype(np.float32)
+    acc, pot = gpu_force(nb, w.x_j, w.x_j, m, w.eps2, alias=True)
+    ra, rp = oracle.force(w.x_j, w.x_j, m, w.eps2)
+    check_parity(acc, pot, ra, rp, "mass contrast")
+    # (iii) everything inside 1e-3 of a point far from the origin, softening of the same order
+    xt = (np.array([3.0, 4.0, 5.0]) + 1e-3 * rng.normal(size=(3000, 3))).astype(np.float32)
+    mt = np.full(3000, 1.0 / 3000, np.float32)
+    acc, pot = gpu_force(nb, xt, xt, mt, np.float32(1e-6), alias=True)
+    ra, rp = oracle.force(xt, xt, mt, np.float32(1e-6))
+    check_parity(acc, pot, ra, rp, "tight cluster")
+
+
+@pytest.mark.parametrize("n_i,n_j", [(200000, 1), (200000, 7), (3, 200000), (1, 1)])
+def test_extreme_aspect_ratios(nb, n_i, n_j):
+    rng = np.random.default_rng(n_i + n_j)
+    xi = rng.normal(size=(n_i, 3)).astype(np.float32)
+    xj = rng.normal(size=(n_j, 3)).astype(np.float32)
+    mj = rng.uniform(0.5, 1.5, n_j).astype(np.float32)
+    acc, pot = gpu_force(nb, xi, xj, mj, 0.01)
+    ra, rp = oracle.force(xi, xj, mj, 0.01)
+    check_parity(acc, pot, ra, rp, f"{n_i}x{n_j}")
+
+
+def test_newton_shell_theorem_on_the_gpu(nb):
+    """P13 on the CUDA path: a quasi-uniform shell exerts no force inside and M / r^2 outside (eps = 0: masked kernel)."""
+    n = 20000
+    k = np.arange(n) + 0.5
+    z = 1 - 2 * k / n; ph = np.pi * (1 + 5 ** 0.5) * k
+    shell = np.stack([np.sqrt(1 - z * z) * np.cos(ph), np.sqrt(1 - z * z) * np.sin(ph), z], 1).astype(np.float32)
+    m = np.full(n, 1.0 / n, np.float32)
+    probes = np.array([[0, 0, 0], [0.3, -0.2, 0.1], [2, 0, 0], [0, -3, 4]], np.float32)
+    acc, pot = gpu_force(nb, probes, shell, m, 0.0)
+    assert np.abs(acc[:2]).max() < 1e-4 and np.abs(pot[:2] + 1.0).max() < 1e-5
+    r = np.linalg.norm(probes[2:], axis=1)
+    np.testing.assert_allclose(acc[2:], -probes[2:] / r[:, None] ** 3, rtol=1e-4, atol=1e-6)
+    np.testing.assert_allclose(pot[2:], -1.0 / r, rtol=1e-5)
