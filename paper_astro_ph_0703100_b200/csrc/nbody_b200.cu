@@ -269,7 +269,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     // sub-range itself, one launch fewer (C0: 21 -> 16 us per call).  NB_DIRECT=0 disables it (tests compare).
     const int64_t sub_max = (n_j + (int64_t)plan.S * plan.WJ - 1) / ((int64_t)plan.S * plan.WJ);
     const char* dr = std::getenv("NB_DIRECT");
-    const bool direct = !packed_j && !eps2_i && !a_only && mode == nb::MODE_EXACT && sub_max <= (int64_t)plan.tile_j * plan.stages &&
+    const bool direct = !packed_j && !eps2_i && mode == nb::MODE_EXACT && sub_max <= (int64_t)plan.tile_j * plan.stages &&
                         !(dr && dr[0] == '0');
     const float4* jp = packed_j ? packed_j : reinterpret_cast<const float4*>(ws->jp);
     if (!packed_j && !direct) {   // a1: j-pack
@@ -298,7 +298,9 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.coin_flag = nullptr;
     args.i_off = args.j_off = args.tile_start = args.cta_batch = nullptr;
     args.n_batch = 0;
-    if (a_only) {
+    if (direct) {                                                      // small call: one launch (masked loop, packs its own j)
+        rc = launch_force<nb::MODE_EXACT, false, true>(args, plan, stream);
+    } else if (a_only) {
         rc = (plan.K == 8) ? launch_force_nophi(args, plan, stream) : launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, jp, 1, stream, &args.coin_lists, &args.coin_flag);
@@ -308,8 +310,6 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         else rc = launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (eps2_i) {
         rc = launch_force<nb::MODE_EXACT, true>(args, plan, stream);
-    } else if (direct) {
-        rc = launch_force<nb::MODE_EXACT, false, true>(args, plan, stream);
     } else {
         rc = launch_force<nb::MODE_EXACT>(args, plan, stream);
     }
@@ -809,18 +809,54 @@ int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, f
     // phi is only wanted at the final time: the evaluations before it run the 12-instruction loop without it
     rc = force_impl(n, x, n, x, m, eps2, acc_io, n_steps == 0 ? pot_out : nullptr, stream);
     if (rc != NB_OK) return rc;
+    // Steps 1 .. n_steps-2 are identical launch sequences (fused kicks + drift, force without phi).  For small systems
+    // a step is a few launches of ~10 us and the HOST becomes the limit (N = 2048: 13 us of enqueueing per step), so
+    // those steps are captured once into a CUDA graph and replayed (N = 2048: 65 k -> see DESIGN.md steps/s).  Not
+    // when the caller is itself capturing this stream, nor while kernel timing events are being recorded.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    NB_CUDA(cudaStreamIsCapturing(stream, &cap));
+    const char* ng = std::getenv("NB_STEP_GRAPH");
+    const bool real_stream = reinterpret_cast<uintptr_t>(stream) > 2;   // the default streams cannot be captured
+    const bool step_graph = real_stream && n_steps >= 16 && n <= 32768 && cap == cudaStreamCaptureStatusNone && !t_profile &&
+                            !(ng && ng[0] == '0');
+    int64_t launches = t_launches;
     for (int64_t s = 0; s < n_steps; ++s) {
         // opening half-kick + drift; from the second step on it also carries the previous step's
         // closing half-kick (two separately rounded kicks, identical to the unfused sequence)
+        if (step_graph && s == 2) {                                    // steps 0 and 1 ran eagerly: everything is warm
+            cudaGraph_t graph = nullptr;
+            cudaGraphExec_t exec = nullptr;
+            NB_CUDA(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
+            nb::nb_kick_drift_kernel<true><<<blocks, threads, 0, stream>>>(x, v, acc_io, n3, h, dt);
+            t_launches = 0;
+            rc = force_impl(n, x, n, x, m, eps2, acc_io, nullptr, stream);
+            const int64_t per_step = t_launches + 1;
+            cudaError_t ce = cudaStreamEndCapture(stream, &graph);
+            if (rc != NB_OK || ce != cudaSuccess) {
+                if (graph) (void)cudaGraphDestroy(graph);
+                if (rc != NB_OK) return rc;
+                t_last_cuda_error = (int)ce;
+                return NB_ERR_CUDA;
+            }
+            NB_CUDA(cudaGraphInstantiate(&exec, graph, 0));
+            const int64_t replays = n_steps - 1 - s;                   // steps s .. n_steps-2
+            for (int64_t r = 0; r < replays; ++r) NB_CUDA(cudaGraphLaunch(exec, stream));
+            (void)cudaGraphExecDestroy(exec);                          // freed by the runtime once the replays have run
+            (void)cudaGraphDestroy(graph);
+            launches += per_step * replays;
+            s += replays;                                              // the last step follows eagerly (it wants phi)
+        }
         if (s == 0)
             nb::nb_kick_drift_kernel<false><<<blocks, threads, 0, stream>>>(x, v, acc_io, n3, h, dt);
         else
             nb::nb_kick_drift_kernel<true><<<blocks, threads, 0, stream>>>(x, v, acc_io, n3, h, dt);
         NB_CUDA(cudaGetLastError());
-        ++t_launches;
+        t_launches = 0;
         rc = force_impl(n, x, n, x, m, eps2, acc_io, s + 1 == n_steps ? pot_out : nullptr, stream);
         if (rc != NB_OK) return rc;
+        launches += t_launches + 1;
     }
+    t_launches = launches;
     if (n_steps > 0) {
         nb::nb_kick_kernel<<<blocks, threads, 0, stream>>>(v, acc_io, n3, h);   // closing half-kick of the last step
         NB_CUDA(cudaGetLastError());

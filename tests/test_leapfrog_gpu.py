@@ -111,3 +111,22 @@ def test_c4_energy_drift_full_size(nb):
     ref_acc, ref_pot = oracle.force(xf[:2048], xf, w.m_j, w.eps2)
     e = oracle.error_metrics(acc.cpu().numpy()[:2048], ref_acc, pot.cpu().numpy()[:2048], ref_pot)
     assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and e["pot_rms"] <= 1e-5
+
+
+def test_step_graph_replay_is_bitwise_the_eager_sequence(nb, monkeypatch):
+    """Small systems replay their identical middle steps from a CUDA graph: same launches, same bits as eager."""
+    import torch
+    w = wl.plummer_workload(1500, 1.0 / 64, seed=8, with_velocities=True)
+    out = {}
+    side = torch.cuda.Stream()                     # the default stream cannot be captured: graphs need a real stream
+    for mode in ("1", "0"):
+        monkeypatch.setenv("NB_STEP_GRAPH", mode)
+        x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            acc, pot = nb.leapfrog_kdk(x, v, m, w.eps2, 1.0 / 256, 40)
+        torch.cuda.synchronize()
+        out[mode] = (x.cpu().numpy(), v.cpu().numpy(), acc.cpu().numpy(), pot.cpu().numpy(), nb.last_launch_count())
+    for a, b in zip(out["1"][:4], out["0"][:4]):
+        assert np.array_equal(a, b)
+    assert out["1"][4] == out["0"][4]
