@@ -64,6 +64,26 @@ __device__ __forceinline__ void add_partials(double (&run)[2 * G][4], const u64 
     }
 }
 
+// A tile that holds at most 32 particles (the ragged tail of a group) would leave one half of every packed
+// instruction idle.  It packs over j instead: both halves carry the SAME i-particle, the two halves of the j operand
+// are two consecutive j-particles, and the two half-sums are added at the end -- the tile takes half the time.
+template <int MASK, bool PHI>
+__device__ __forceinline__ void half_sweep(const float4* __restrict__ sp, int np, u64 nx, u64 ny, u64 nz, u64 eps2_2, u64& ax,
+                                           u64& ay, u64& az, u64& ph) {
+    ax = 0ull; ay = 0ull; az = 0ull; ph = 0ull;
+    int j = 0;
+#pragma unroll 4
+    for (; j + 2 <= np; j += 2) {
+        const float4 A = sp[j], B = sp[j + 1];
+        pair_body<MASK, PHI>(pack2(A.x, B.x), pack2(A.y, B.y), pack2(A.z, B.z), pack2(A.w, B.w), nx, ny, nz, eps2_2, ax, ay, az, ph);
+    }
+    if (j < np) {                                                      // odd tail: the partner is a massless particle far away
+        const float4 A = sp[j];
+        const float far = 3.0e18f;
+        pair_body<MASK, PHI>(pack2(A.x, far), pack2(A.y, far), pack2(A.z, far), pack2(A.w, 0.0f), nx, ny, nz, eps2_2, ax, ay, az, ph);
+    }
+}
+
 // G = packed groups of 64 i-particles a CTA can hold (tile = 64 G); STAGES = ring depth per warp.
 template <bool MASKED, int G, int STAGES>
 __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const ForceArgs a) {
@@ -106,6 +126,14 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
         nzi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 2], -a.x_i[3 * (size_t)i1 + 2]);
     }
     const u64 eps2_2 = pack2(a.eps2, a.eps2);
+    const bool half = (G == 1) && (i_hi - i_lo <= 32);                 // ragged tail tile: pack over j (half_sweep)
+    u64 hx = 0ull, hy = 0ull, hz = 0ull;
+    if (half) {
+        const int i0 = min(i_base, i_hi - 1);
+        hx = pack2(-a.x_i[3 * (size_t)i0 + 0], -a.x_i[3 * (size_t)i0 + 0]);
+        hy = pack2(-a.x_i[3 * (size_t)i0 + 1], -a.x_i[3 * (size_t)i0 + 1]);
+        hz = pack2(-a.x_i[3 * (size_t)i0 + 2], -a.x_i[3 * (size_t)i0 + 2]);
+    }
     __syncthreads();                                                   // barriers initialised
 
     // each warp is its own producer; a ring slot is refilled by the warp that has just finished reading it
@@ -128,8 +156,17 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
         const int nc = min(TJ, n_sub - t * TJ);                        // TJ == SUB: one Eq. (2) block per tile
         const float4* sp = reinterpret_cast<const float4*>(rings + wj * RING_BYTES + slot * TJ * 16);
         u64 pax[G], pay[G], paz[G], pph[G];
-        sweep_dyn<MASKED ? MASK_EXACT : MASK_NONE, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
-        add_partials<G>(run, pax, pay, paz, pph);
+        if (half) {
+            half_sweep<MASKED ? MASK_EXACT : MASK_NONE, MASKED>(sp, nc, hx, hy, hz, eps2_2, pax[0], pay[0], paz[0], pph[0]);
+            float lo, hi;                                              // both halves belong to particle slot 0
+            unpack2(pax[0], lo, hi); run[0][0] += (double)lo + (double)hi;
+            unpack2(pay[0], lo, hi); run[0][1] += (double)lo + (double)hi;
+            unpack2(paz[0], lo, hi); run[0][2] += (double)lo + (double)hi;
+            unpack2(pph[0], lo, hi); run[0][3] += (double)lo + (double)hi;
+        } else {
+            sweep_dyn<MASKED ? MASK_EXACT : MASK_NONE, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+            add_partials<G>(run, pax, pay, paz, pph);
+        }
         __syncwarp();                                                  // every lane is done with the slot
         if (lane == 0 && t + STAGES < n_tiles) {
             const int tn = t + STAGES;
