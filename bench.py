@@ -35,7 +35,7 @@ CONFIG_INDEX = {"C0": 0, "C1": 1, "C2": 2, "C3": 3, "C4": 4}
 L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/r01_ncu_full.md); null for configs / ops without a capture
-NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 71.0e6, "jerk": 105.4e6, "batched": 249.6e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 71.0e6, "jerk": 105.4e6, "batched": 251.5e6}
 
 
 def load_peaks():
@@ -583,6 +583,24 @@ def main():
                              "rel_drift": abs(e_end - e_start) / abs(e_start), "by": "oracle.energy (FP64) on the GPU's FP32 (x, v)"}
         if args.op == "leapfrog":
             out["kdk_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
+        if args.check and args.op in ("force", "jerk") and not args.shard:
+            import oracle
+            w = prob.w
+            prob.call()
+            torch.cuda.synchronize()
+            idx = np.sort(np.random.default_rng(0).choice(w.n_i, min(2048, w.n_i), replace=False))
+            got = [o.cpu().numpy()[idx] for o in prob.outs]
+            if args.op == "force":
+                ra, rp = oracle.force(w.xi[idx], w.x_j, w.m_j, w.eps2)
+                par = oracle.error_metrics(got[0], ra, got[1], rp)
+            else:
+                ra, rj, rp = oracle.force_jerk(w.x_j[idx], w.v[idx], w.x_j, w.v, w.m_j, w.eps2)
+                par = oracle.error_metrics(got[0], ra, got[2], rp)
+                ej = oracle.error_metrics(got[1], rj)
+                par["jerk_max"], par["jerk_rms"] = ej["acc_max"], ej["acc_rms"]
+            par["sample"] = f"{len(idx)} seeded i-particles x all {w.n_j} j-particles, oracle in FP64"
+            par["tolerance"] = "acc (jerk) RMS <= 1e-5, max <= 1e-4; phi RMS <= 1e-5 (BASELINE.json north_star)"
+            out["parity"] = par
         if not args.no_cpu_baseline:
             v, cores, sample = oracle_rate_op(args.op, prob.w, args.cpu_seconds)
             out["cpu_baseline"] = {"value": v, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample}
