@@ -57,7 +57,8 @@ struct HermiteArgs {
     float eps2;
 };
 
-template <bool MASKED>
+// PHI = false: the caller does not want the potential: 26 FP32-pipe instructions per pair.
+template <bool MASKED, bool PHI = true>
 __device__ __forceinline__ void hermite_pair(u64 xj, u64 yj, u64 zj, u64 mj, u64 vxj, u64 vyj, u64 vzj,
                                              u64 nxi, u64 nyi, u64 nzi, u64 nvxi, u64 nvyi, u64 nvzi, u64 eps2_2,
                                              u64 (&s)[kHermiteAcc]) {
@@ -99,10 +100,10 @@ __device__ __forceinline__ void hermite_pair(u64 xj, u64 yj, u64 zj, u64 mj, u64
     s[6] = fma2(w, dx, s[6]);                        // jk2 / 3 = mr5i (d.dv) d
     s[7] = fma2(w, dy, s[7]);
     s[8] = fma2(w, dz, s[8]);
-    s[9] = add2(s[9], mu);                           // OUTPUT[6] -= pot (sign at the end)
+    if (PHI) s[9] = add2(s[9], mu);                  // OUTPUT[6] -= pot (sign at the end)
 }
 
-template <int K, bool MASKED>
+template <int K, bool MASKED, bool PHI = true>
 __device__ __forceinline__ void hermite_sweep(const float4* __restrict__ sp, int np, const u64 (&ni)[K / 2][6], u64 eps2_2,
                                               u64 (&part)[K / 2][kHermiteAcc]) {
 #pragma unroll
@@ -116,13 +117,13 @@ __device__ __forceinline__ void hermite_sweep(const float4* __restrict__ sp, int
         const u64 vx = pack2(V.x, V.x), vy = pack2(V.y, V.y), vz = pack2(V.z, V.z);
 #pragma unroll
         for (int k = 0; k < K / 2; ++k)
-            hermite_pair<MASKED>(xj, yj, zj, mj, vx, vy, vz, ni[k][0], ni[k][1], ni[k][2], ni[k][3], ni[k][4], ni[k][5],
+            hermite_pair<MASKED, PHI>(xj, yj, zj, mj, vx, vy, vz, ni[k][0], ni[k][1], ni[k][2], ni[k][3], ni[k][4], ni[k][5],
                                  eps2_2, part[k]);
     }
 }
 
 // CTA = 8 warps = WI x WJ, as nb_force_kernel.  TJ j-particles (32 B each) per ring stage.
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, int SUB = 256>
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool PHI = true, int SUB = 256>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const HermiteArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
     static_assert(SUB == kCoinSeg, "coincidence segments are SUB j-particles");
@@ -211,8 +212,8 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
                 }
                 masked = (coin_cnt < 0 || coin_next <= seg_hi);
             }
-            if (masked) hermite_sweep<K, true>(sp + 2 * c, nc, ni, eps2_2, part);
-            else hermite_sweep<K, false>(sp + 2 * c, nc, ni, eps2_2, part);
+            if (masked) hermite_sweep<K, true, PHI>(sp + 2 * c, nc, ni, eps2_2, part);
+            else hermite_sweep<K, false, PHI>(sp + 2 * c, nc, ni, eps2_2, part);
 #pragma unroll
             for (int k2 = 0; k2 < K / 2; ++k2)
 #pragma unroll

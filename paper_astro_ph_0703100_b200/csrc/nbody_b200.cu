@@ -335,13 +335,13 @@ nb::Plan hermite_plan(int64_t n_i, int64_t n_j, int sm_count) {
     return nb::make_plan(n_i, n_j, sm_count, 4, kHermiteInstPerPair, kHermitePartialBytes);
 }
 
-template <int K, int WI, int WJ, int STAGES, int MODE>
+template <int K, int WI, int WJ, int STAGES, int MODE, bool PHI = true>
 int launch_hermite_inst(const nb::HermiteArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     constexpr int TJ = 256;
     constexpr size_t ring = (size_t)WJ * STAGES * TJ * 32;
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * nb::kHermiteAcc * (WI * 32) * sizeof(double) : 0;
     constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_hermite_kernel<K, WI, WJ, TJ, STAGES, MODE>;
+    auto kern = nb::nb_hermite_kernel<K, WI, WJ, TJ, STAGES, MODE, PHI>;
     static bool configured[64] = {};
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
@@ -373,6 +373,16 @@ int launch_hermite_k(const nb::HermiteArgs& args, const nb::Plan& plan, cudaStre
         case 2: return launch_hermite_inst<K, 4, 2, 4, MODE>(args, plan, stream);
         case 4: return launch_hermite_inst<K, 2, 4, 3, MODE>(args, plan, stream);
         default: return launch_hermite_inst<K, 1, 8, 3, MODE>(args, plan, stream);
+    }
+}
+
+// pot_out == NULL on a large call (nb_hermite4: every evaluation but the last): 26 instructions per pair, K = 4 only
+int launch_hermite_nophi(const nb::HermiteArgs& args, const nb::Plan& plan, cudaStream_t stream) {
+    switch (plan.WJ) {
+        case 1: return launch_hermite_inst<4, 8, 1, 4, nb::MODE_LIST, false>(args, plan, stream);
+        case 2: return launch_hermite_inst<4, 4, 2, 4, nb::MODE_LIST, false>(args, plan, stream);
+        case 4: return launch_hermite_inst<4, 2, 4, 3, nb::MODE_LIST, false>(args, plan, stream);
+        default: return launch_hermite_inst<4, 1, 8, 3, nb::MODE_LIST, false>(args, plan, stream);
     }
 }
 
@@ -446,7 +456,7 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, args.jp, 2, stream, &args.coin_lists, &args.coin_flag);
         if (rc != NB_OK) return rc;
-        rc = launch_hermite<nb::MODE_LIST>(args, plan, stream);
+        rc = (!pot_out && plan.K == 4) ? launch_hermite_nophi(args, plan, stream) : launch_hermite<nb::MODE_LIST>(args, plan, stream);
     } else {
         rc = launch_hermite<nb::MODE_EXACT>(args, plan, stream);
     }
@@ -882,7 +892,7 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
     const int threads = 256, blocks = (n3 + threads - 1) / threads;
     int64_t launches = 0;
     // a0, j0 = force_jerk(x0, v0)
-    rc = force_jerk_impl(n, x, v, n, x, v, m, eps2, acc_io, jerk_io, pot_out, stream);
+    rc = force_jerk_impl(n, x, v, n, x, v, m, eps2, acc_io, jerk_io, n_steps == 0 ? pot_out : nullptr, stream);
     if (rc != NB_OK) return rc;
     launches += t_launches;
     if (n_steps == 0) return NB_OK;
@@ -903,7 +913,7 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
         nb::nb_hermite_predict_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, xp, vp, n3, dt);
         NB_CUDA(cudaGetLastError());
         t_launches = 0;
-        rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, pot_out, stream);
+        rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, s + 1 == n_steps ? pot_out : nullptr, stream);
         if (rc != NB_OK) return rc;
         launches += t_launches + 2;
         nb::nb_hermite_correct_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, a1, j1, n3, dt);
