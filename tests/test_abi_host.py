@@ -51,6 +51,41 @@ def test_argument_validation_happens_before_any_cuda_call():
     out = (ctypes.c_int64 * 8)()
     assert lib.nb_plan_query(0, 5, 148, out) == 1
     assert lib.nb_plan_query(5, 5, 148, None) == 1
+    # the widened entry points validate the same way
+    assert lib.nb_force_jerk(1, p, None, 1, p, p, p, 0.1, p, p, None, None) == 1
+    assert lib.nb_force_jerk(1, p, p, 1, p, p, p, -1.0, p, p, None, None) == 1
+    assert lib.nb_force_jerk_host(1, p, p, 1, p, p, p, 0.1, p, None, None) == 1
+    assert lib.nb_hermite4(4, p, p, p, 0.1, float("inf"), 1, p, p, None, None) == 1
+    assert lib.nb_hermite4(4, p, p, p, 0.1, 0.1, 1, p, None, None, None) == 1
+    assert lib.nb_force_batched(-1, p, p, 1, p, 1, p, p, 0.1, p, None, None) == 1
+    assert lib.nb_force_batched(2, None, p, 1, p, 1, p, p, 0.1, p, None, None) == 1
+    assert lib.nb_force_eps_i(1, p, None, 1, p, p, p, None, None) == 1
+    assert lib.nb_force_packed(1, p, 1, None, 0.1, p, None, None) == 1
+    assert lib.nb_force_packed(1, p, 1, p + 4, 0.1, p, None, None) == 1          # xm_j must be 16-byte aligned
+    assert lib.nb_pack_j(1, p, None, p, None) == 1
+    assert lib.nb_cunbody_force(p, None, p, 1, 1, None) == 1
+    assert lib.nb_cunbody_force_jerk_pot(None, p, p, 1, 1, None) == 1
+    assert lib.nb_plan_query_jerk(5, -5, 148, out) == 1
+
+
+def test_without_a_device_every_compute_entry_reports_an_error():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    lib = nb.lib()
+    buf = (ctypes.c_float * 64)()
+    p = ctypes.addressof(buf)
+    off = (ctypes.c_int32 * 2)(0, 1)
+    po = ctypes.addressof(off)
+    for st in (lib.nb_force(1, p, 1, p, p, 0.1, p, None, None),
+               lib.nb_force_jerk(1, p, p, 1, p, p, p, 0.1, p, p, None, None),
+               lib.nb_force_batched(1, po, po, 1, p, 1, p, p, 0.1, p, None, None),
+               lib.nb_force_eps_i(1, p, p, 1, p, p, p, None, None),
+               lib.nb_force_packed(1, p, 1, p, 0.1, p, None, None),
+               lib.nb_leapfrog_kdk(1, p, p, p, 0.1, 0.1, 1, p, None, None),
+               lib.nb_hermite4(1, p, p, p, 0.1, 0.1, 1, p, p, None, None),
+               lib.nb_cunbody_force(p, p, p, 1, 1, None)):
+        assert st in (2, 4), "without a B200 the library must report an error, not compute on the CPU"
 
 
 def test_no_cpu_fallback_without_a_device():
