@@ -448,3 +448,37 @@ def test_newton_shell_theorem_on_the_gpu(nb):
     r = np.linalg.norm(probes[2:], axis=1)
     np.testing.assert_allclose(acc[2:], -probes[2:] / r[:, None] ** 3, rtol=1e-4, atol=1e-6)
     np.testing.assert_allclose(pot[2:], -1.0 / r, rtol=1e-5)
+
+
+def test_randomised_shapes_plans_and_modes(nb, monkeypatch):
+    """40 seeded random cases: ragged sizes, every decomposition the planner could pick, both coincidence modes, with
+    and without aliasing, duplicates and phi -- each against the oracle."""
+    rng = np.random.default_rng(2024)
+    for case in range(40):
+        n_j = int(rng.integers(1, 6000))
+        alias = bool(rng.integers(0, 2))
+        n_i = n_j if alias else int(rng.integers(1, 3000))
+        k = int(rng.choice([2, 4, 8])); wj = int(rng.choice([1, 2, 4, 8])); s = int(rng.integers(1, 7))
+        mode = str(rng.choice(["exact", "list", ""]))
+        want_pot = bool(rng.integers(0, 4))
+        eps2 = float(np.float32(2.0 ** rng.integers(-16, -2)))
+        x_j = rng.normal(size=(n_j, 3)).astype(np.float32)
+        m_j = rng.uniform(0.1, 2.0, n_j).astype(np.float32)
+        if n_j > 10:
+            x_j[rng.integers(0, n_j, 3)] = x_j[0]                      # a few duplicates
+        x_i = x_j if alias else np.concatenate([x_j[: min(n_i, n_j) // 2],
+                                                rng.normal(size=(n_i - min(n_i, n_j) // 2, 3)).astype(np.float32)])
+        monkeypatch.setenv("NB_PLAN", f"{k},{8 // wj},{wj},{s}")
+        if mode:
+            monkeypatch.setenv("NB_MASK", mode)
+        else:
+            monkeypatch.delenv("NB_MASK", raising=False)
+        acc, pot = gpu_force(nb, x_i, x_j, m_j, eps2, want_pot=want_pot, alias=alias)
+        ra, rp = oracle.force(x_i, x_j, m_j, eps2)
+        label = f"case {case}: {n_i}x{n_j} plan {k},{8 // wj},{wj},{s} mode '{mode}' alias {alias} pot {want_pot}"
+        scale = np.linalg.norm(ra, axis=1)
+        ok = scale > 1e-3 * np.median(scale)                           # a particle whose field cancels has no relative error
+        e = oracle.error_metrics(acc[ok], ra[ok], None if pot is None else pot[ok], None if pot is None else rp[ok])
+        assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4, (label, e)
+        if pot is not None:
+            assert e["pot_rms"] <= 1e-5, (label, e)
