@@ -128,27 +128,24 @@ int pick_mode(int64_t n_i, int64_t n_j, float eps2) {
     return ((double)n_i * (double)n_j >= kListMinPairs) ? nb::MODE_LIST : nb::MODE_EXACT;
 }
 
-template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I, bool PHI = true, bool DIRECT = false>
-int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
-    constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
-    constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
-    constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, EPS_I, PHI, DIRECT>;
-    static bool configured[64] = {};
+// One launch of a dominant kernel: raises the kernel's dynamic shared-memory limit once per device, brackets the
+// launch with two events on the launching stream while nb_profile_enable is on, counts it.
+template <class Kernel, class Args>
+int launch_dominant(Kernel kern, bool* configured, dim3 grid, unsigned threads, size_t smem, cudaStream_t stream,
+                    const Args& args) {
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
     if (!configured[dev & 63]) {
         NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured[dev & 63] = true;
     }
-    dim3 grid((unsigned)plan.tiles_i, (unsigned)plan.S, 1);
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (t_profile) {
         NB_CUDA(cudaEventCreate(&e0));
         NB_CUDA(cudaEventCreate(&e1));
         NB_CUDA(cudaEventRecord(e0, stream));
     }
-    kern<<<grid, 32 * WI * WJ, smem, stream>>>(args);
+    kern<<<grid, threads, smem, stream>>>(args);
     NB_CUDA(cudaGetLastError());
     if (t_profile) {
         NB_CUDA(cudaEventRecord(e1, stream));
@@ -156,6 +153,16 @@ int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStrea
     }
     ++t_launches;
     return NB_OK;
+}
+
+template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I, bool PHI = true, bool DIRECT = false>
+int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
+    constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
+    constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
+    constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
+    static bool configured[64] = {};
+    return launch_dominant(nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, EPS_I, PHI, DIRECT>, configured,
+                           dim3((unsigned)plan.tiles_i, (unsigned)plan.S, 1), 32 * WI * WJ, smem, stream, args);
 }
 
 // tile_j / stages per WJ must match nb::ring_shape (nb_plan.h)
@@ -341,29 +348,9 @@ int launch_hermite_inst(const nb::HermiteArgs& args, const nb::Plan& plan, cudaS
     constexpr size_t ring = (size_t)WJ * STAGES * TJ * 32;
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * nb::kHermiteAcc * (WI * 32) * sizeof(double) : 0;
     constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_hermite_kernel<K, WI, WJ, TJ, STAGES, MODE, PHI>;
     static bool configured[64] = {};
-    int dev = 0;
-    NB_CUDA(cudaGetDevice(&dev));
-    if (!configured[dev & 63]) {
-        NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured[dev & 63] = true;
-    }
-    dim3 grid((unsigned)plan.tiles_i, (unsigned)plan.S, 1);
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (t_profile) {
-        NB_CUDA(cudaEventCreate(&e0));
-        NB_CUDA(cudaEventCreate(&e1));
-        NB_CUDA(cudaEventRecord(e0, stream));
-    }
-    kern<<<grid, 32 * WI * WJ, smem, stream>>>(args);
-    NB_CUDA(cudaGetLastError());
-    if (t_profile) {
-        NB_CUDA(cudaEventRecord(e1, stream));
-        t_events.emplace_back(e0, e1);
-    }
-    ++t_launches;
-    return NB_OK;
+    return launch_dominant(nb::nb_hermite_kernel<K, WI, WJ, TJ, STAGES, MODE, PHI>, configured,
+                           dim3((unsigned)plan.tiles_i, (unsigned)plan.S, 1), 32 * WI * WJ, smem, stream, args);
 }
 
 template <int K, int MODE>
@@ -490,28 +477,8 @@ int launch_batched_inst(const nb::ForceArgs& args, unsigned max_ctas, cudaStream
     constexpr size_t ring = (size_t)8 * STAGES * 256 * 16;
     constexpr size_t red = (size_t)8 * (2 * G) * 4 * 32 * sizeof(double);
     constexpr size_t smem = (ring > red ? ring : red) + 8 * STAGES * sizeof(uint64_t) + 128;
-    auto kern = nb::nb_batched_kernel<MASKED, G, STAGES>;
     static bool configured[64] = {};
-    int dev = 0;
-    NB_CUDA(cudaGetDevice(&dev));
-    if (!configured[dev & 63]) {
-        NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured[dev & 63] = true;
-    }
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (t_profile) {
-        NB_CUDA(cudaEventCreate(&e0));
-        NB_CUDA(cudaEventCreate(&e1));
-        NB_CUDA(cudaEventRecord(e0, stream));
-    }
-    kern<<<max_ctas, 256, smem, stream>>>(args);
-    NB_CUDA(cudaGetLastError());
-    if (t_profile) {
-        NB_CUDA(cudaEventRecord(e1, stream));
-        t_events.emplace_back(e0, e1);
-    }
-    ++t_launches;
-    return NB_OK;
+    return launch_dominant(nb::nb_batched_kernel<MASKED, G, STAGES>, configured, dim3(max_ctas, 1, 1), 256, smem, stream, args);
 }
 
 template <bool MASKED>
