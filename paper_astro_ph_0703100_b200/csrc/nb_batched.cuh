@@ -8,16 +8,19 @@
 //   - K per CTA at run time: a tile that holds n_i <= 64 / 128 / 192 / 256 particles runs 1 / 2 / 3 / 4 packed groups
 //     (tile_sweep<2 KG>), so the padding of a sub-problem is at most 63 idle lanes;
 //   - coincident pairs (reading R1): interaction lists contain the group's own members, so EVERY
-//     sub-problem has them; MASKED = true masks every pair in the loop.  MASKED = false (phi not wanted and
-//     eps2 >= 2^-40: an unmasked coincident pair adds +-0 to a) runs the untested loop.
-// Measured on the T1 tree lists: G = 1 is the fastest shape (57 % of roofline: 83 % lane use x 69 % loop
-// efficiency, the masked loop's ceiling being 72 %); G = 2 / 4 reach 53 / 51 %.  A flag-only loop with the flagged
-// blocks redone by all 8 warps together was tried and removed (55 %: with one packed group per warp the loop is
-// latency-bound, so not paying for the mask buys nothing).
+//     sub-problem has them -- but only where a j-particle lies inside the bounding box of the tile's i-particles.
+//     MASKED = true tests the list kBatchSub j at a time against that box: a part with a j inside runs the masked
+//     loop, the others the untested loop (bit for bit the same there).  MASKED = false (phi not wanted and
+//     eps2 >= 2^-40: an unmasked coincident pair adds +-0 to a) runs the untested loop everywhere, no test.
+// Measured on the T1 tree lists: G = 1 is the fastest shape (66 % of roofline: 83 % lane use x 80 % loop
+// efficiency; 60 % with every pair masked).  A flag-only loop with the flagged blocks redone by all 8 warps together
+// was tried and removed (55 %: the redo serialises the CTA).
 #pragma once
 #include "nb_kernels.cuh"
 
 namespace nb {
+
+constexpr int kBatchSub = 64;        // j-particles per bounding-box test (a multiple of 32, divides the 256-j tile)
 
 template <int KG, int G>
 __device__ __forceinline__ const u64 (&first_groups(const u64 (&arr)[G]))[KG] {
@@ -28,27 +31,26 @@ __device__ __forceinline__ u64 (&first_groups(u64 (&arr)[G]))[KG] {
     return *reinterpret_cast<u64(*)[KG]>(&arr[0]);
 }
 
-template <int KG, int MASK, int G>
+// the first KG packed groups against np j-particles; the partial sums CONTINUE (the caller zeroes them per Eq. (2) block)
+template <int KG, int MASK, bool PHI, int G>
 __device__ __forceinline__ void sweep_groups(const float4* __restrict__ sp, int np, const u64 (&nxi)[G], const u64 (&nyi)[G],
                                              const u64 (&nzi)[G], u64 eps2_2, u64 (&pax)[G], u64 (&pay)[G],
                                              u64 (&paz)[G], u64 (&pph)[G]) {
-    tile_sweep<2 * KG, MASK, false, MASK == MASK_EXACT>(sp, np, first_groups<KG, G>(nxi), first_groups<KG, G>(nyi),
-                                                        first_groups<KG, G>(nzi), eps2_2, first_groups<KG, G>(pax),
-                                                        first_groups<KG, G>(pay), first_groups<KG, G>(paz),
-                                                        first_groups<KG, G>(pph), first_groups<KG, G>(nxi) /* e2: unused */);
+    tile_sweep<2 * KG, MASK, false, PHI, true>(sp, np, first_groups<KG, G>(nxi), first_groups<KG, G>(nyi),
+                                               first_groups<KG, G>(nzi), eps2_2, first_groups<KG, G>(pax),
+                                               first_groups<KG, G>(pay), first_groups<KG, G>(paz),
+                                               first_groups<KG, G>(pph), first_groups<KG, G>(nxi) /* e2: unused */);
 }
 
 // kg (1..G) active packed groups, uniform over the CTA; the inactive groups' partial sums stay zero
-template <int MASK, int G>
+template <int MASK, bool PHI, int G>
 __device__ __forceinline__ void sweep_dyn(int kg, const float4* __restrict__ sp, int np, const u64 (&nxi)[G], const u64 (&nyi)[G],
                                           const u64 (&nzi)[G], u64 eps2_2, u64 (&pax)[G], u64 (&pay)[G],
                                           u64 (&paz)[G], u64 (&pph)[G]) {
-#pragma unroll
-    for (int k = 0; k < G; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
-    if (G >= 4 && kg >= 4) sweep_groups<(G >= 4 ? 4 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
-    else if (G >= 3 && kg == 3) sweep_groups<(G >= 3 ? 3 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
-    else if (G >= 2 && kg == 2) sweep_groups<(G >= 2 ? 2 : 1), MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
-    else sweep_groups<1, MASK, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+    if (G >= 4 && kg >= 4) sweep_groups<(G >= 4 ? 4 : 1), MASK, PHI, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+    else if (G >= 3 && kg == 3) sweep_groups<(G >= 3 ? 3 : 1), MASK, PHI, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+    else if (G >= 2 && kg == 2) sweep_groups<(G >= 2 ? 2 : 1), MASK, PHI, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+    else sweep_groups<1, MASK, PHI, G>(sp, np, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
 }
 
 template <int G>
@@ -67,10 +69,10 @@ __device__ __forceinline__ void add_partials(double (&run)[2 * G][4], const u64 
 // A tile that holds at most 32 particles (the ragged tail of a group) would leave one half of every packed
 // instruction idle.  It packs over j instead: both halves carry the SAME i-particle, the two halves of the j operand
 // are two consecutive j-particles, and the two half-sums are added at the end -- the tile takes half the time.
+// The sums CONTINUE (the caller zeroes them per Eq. (2) block); np is even except for the last part of a list.
 template <int MASK, bool PHI>
 __device__ __forceinline__ void half_sweep(const float4* __restrict__ sp, int np, u64 nx, u64 ny, u64 nz, u64 eps2_2, u64& ax,
                                            u64& ay, u64& az, u64& ph) {
-    ax = 0ull; ay = 0ull; az = 0ull; ph = 0ull;
     int j = 0;
 #pragma unroll 4
     for (; j + 2 <= np; j += 2) {
@@ -134,6 +136,24 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
         hy = pack2(-a.x_i[3 * (size_t)i0 + 1], -a.x_i[3 * (size_t)i0 + 1]);
         hz = pack2(-a.x_i[3 * (size_t)i0 + 2], -a.x_i[3 * (size_t)i0 + 2]);
     }
+    // bounding box of the tile's i-particles (every warp holds the same ones; NaN coordinates drop out of min / max
+    // and never coincide with anything)
+    float bx0 = __int_as_float(0x7f800000), by0 = bx0, bz0 = bx0, bx1 = -bx0, by1 = -bx0, bz1 = -bx0;
+    if (MASKED) {
+#pragma unroll
+        for (int k2 = 0; k2 < G; ++k2) {
+            float lo, hi;
+            unpack2(nxi[k2], lo, hi); bx0 = fminf(bx0, fminf(-lo, -hi)); bx1 = fmaxf(bx1, fmaxf(-lo, -hi));
+            unpack2(nyi[k2], lo, hi); by0 = fminf(by0, fminf(-lo, -hi)); by1 = fmaxf(by1, fmaxf(-lo, -hi));
+            unpack2(nzi[k2], lo, hi); bz0 = fminf(bz0, fminf(-lo, -hi)); bz1 = fmaxf(bz1, fmaxf(-lo, -hi));
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            bx0 = fminf(bx0, __shfl_xor_sync(0xffffffffu, bx0, o)); bx1 = fmaxf(bx1, __shfl_xor_sync(0xffffffffu, bx1, o));
+            by0 = fminf(by0, __shfl_xor_sync(0xffffffffu, by0, o)); by1 = fmaxf(by1, __shfl_xor_sync(0xffffffffu, by1, o));
+            bz0 = fminf(bz0, __shfl_xor_sync(0xffffffffu, bz0, o)); bz1 = fmaxf(bz1, __shfl_xor_sync(0xffffffffu, bz1, o));
+        }
+    }
     __syncthreads();                                                   // barriers initialised
 
     // each warp is its own producer; a ring slot is refilled by the warp that has just finished reading it
@@ -156,15 +176,40 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
         const int nc = min(TJ, n_sub - t * TJ);                        // TJ == SUB: one Eq. (2) block per tile
         const float4* sp = reinterpret_cast<const float4*>(rings + wj * RING_BYTES + slot * TJ * 16);
         u64 pax[G], pay[G], paz[G], pph[G];
+#pragma unroll
+        for (int k = 0; k < G; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
+        if (MASKED) {
+            // kBatchSub j at a time: a part with no j inside the bounding box of the tile's i-particles cannot hold
+            // a coincident pair and runs the untested loop (bit for bit what the masked loop gives there)
+            for (int c = 0; c < nc; c += kBatchSub) {
+                const int ncc = min(kBatchSub, nc - c);
+                bool inside = false;
+#pragma unroll
+                for (int q = 0; q < kBatchSub; q += 32) {
+                    if (q + lane < ncc) {
+                        const float4 J = sp[c + q + lane];
+                        inside |= (J.x >= bx0) & (J.x <= bx1) & (J.y >= by0) & (J.y <= by1) & (J.z >= bz0) & (J.z <= bz1);
+                    }
+                }
+                if (__any_sync(0xffffffffu, inside)) {
+                    if (half) half_sweep<MASK_EXACT, true>(sp + c, ncc, hx, hy, hz, eps2_2, pax[0], pay[0], paz[0], pph[0]);
+                    else sweep_dyn<MASK_EXACT, true, G>(kg, sp + c, ncc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+                } else {
+                    if (half) half_sweep<MASK_NONE, true>(sp + c, ncc, hx, hy, hz, eps2_2, pax[0], pay[0], paz[0], pph[0]);
+                    else sweep_dyn<MASK_NONE, true, G>(kg, sp + c, ncc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+                }
+            }
+        } else {
+            if (half) half_sweep<MASK_NONE, false>(sp, nc, hx, hy, hz, eps2_2, pax[0], pay[0], paz[0], pph[0]);
+            else sweep_dyn<MASK_NONE, false, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
+        }
         if (half) {
-            half_sweep<MASKED ? MASK_EXACT : MASK_NONE, MASKED>(sp, nc, hx, hy, hz, eps2_2, pax[0], pay[0], paz[0], pph[0]);
             float lo, hi;                                              // both halves belong to particle slot 0
             unpack2(pax[0], lo, hi); run[0][0] += (double)lo + (double)hi;
             unpack2(pay[0], lo, hi); run[0][1] += (double)lo + (double)hi;
             unpack2(paz[0], lo, hi); run[0][2] += (double)lo + (double)hi;
             unpack2(pph[0], lo, hi); run[0][3] += (double)lo + (double)hi;
         } else {
-            sweep_dyn<MASKED ? MASK_EXACT : MASK_NONE, G>(kg, sp, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph);
             add_partials<G>(run, pax, pay, paz, pph);
         }
         __syncwarp();                                                  // every lane is done with the slot

@@ -153,12 +153,15 @@ __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nx
 
 // One tile: K/2 i-pairs of this thread against np j-particles in shared memory; partial sums start from zero (Eq. (2)).
 // EPS_I (row f3): the softening is a property of the i-particle (Fig. A.1) and sits, packed, in e2[].
-template <int K, int MASK, bool EPS_I = false, bool PHI = true>
+// ACC = true: the partial sums continue (the caller zeroed them; row f2 sweeps one Eq. (2) block in several parts).
+template <int K, int MASK, bool EPS_I = false, bool PHI = true, bool ACC = false>
 __device__ __forceinline__ void tile_sweep(const float4* __restrict__ sp, int np, const u64 (&nxi)[K / 2], const u64 (&nyi)[K / 2],
                                            const u64 (&nzi)[K / 2], u64 eps2_2, u64 (&pax)[K / 2], u64 (&pay)[K / 2],
                                            u64 (&paz)[K / 2], u64 (&pph)[K / 2], const u64 (&e2)[K / 2]) {
+    if (!ACC) {
 #pragma unroll
-    for (int k = 0; k < K / 2; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
+        for (int k = 0; k < K / 2; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
+    }
 #pragma unroll 4
     for (int j = 0; j < np; ++j) {
         const float4 J = sp[j];                                        // broadcast LDS.128: x y z m
