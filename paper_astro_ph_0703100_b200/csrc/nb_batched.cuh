@@ -123,18 +123,18 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
     for (int k2 = 0; k2 < G; ++k2) {
         const int i0 = min(i_base + (2 * k2) * 32, i_hi - 1);
         const int i1 = min(i_base + (2 * k2 + 1) * 32, i_hi - 1);
-        nxi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 0], -a.x_i[3 * (size_t)i1 + 0]);
-        nyi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 1], -a.x_i[3 * (size_t)i1 + 1]);
-        nzi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 2], -a.x_i[3 * (size_t)i1 + 2]);
+        nxi[k2] = pack2(neg_canon(a.x_i[3 * (size_t)i0 + 0]), neg_canon(a.x_i[3 * (size_t)i1 + 0]));
+        nyi[k2] = pack2(neg_canon(a.x_i[3 * (size_t)i0 + 1]), neg_canon(a.x_i[3 * (size_t)i1 + 1]));
+        nzi[k2] = pack2(neg_canon(a.x_i[3 * (size_t)i0 + 2]), neg_canon(a.x_i[3 * (size_t)i1 + 2]));
     }
     const u64 eps2_2 = pack2(a.eps2, a.eps2);
     const bool half = (G == 1) && (i_hi - i_lo <= 32);                 // ragged tail tile: pack over j (half_sweep)
     u64 hx = 0ull, hy = 0ull, hz = 0ull;
     if (half) {
         const int i0 = min(i_base, i_hi - 1);
-        hx = pack2(-a.x_i[3 * (size_t)i0 + 0], -a.x_i[3 * (size_t)i0 + 0]);
-        hy = pack2(-a.x_i[3 * (size_t)i0 + 1], -a.x_i[3 * (size_t)i0 + 1]);
-        hz = pack2(-a.x_i[3 * (size_t)i0 + 2], -a.x_i[3 * (size_t)i0 + 2]);
+        hx = pack2(neg_canon(a.x_i[3 * (size_t)i0 + 0]), neg_canon(a.x_i[3 * (size_t)i0 + 0]));
+        hy = pack2(neg_canon(a.x_i[3 * (size_t)i0 + 1]), neg_canon(a.x_i[3 * (size_t)i0 + 1]));
+        hz = pack2(neg_canon(a.x_i[3 * (size_t)i0 + 2]), neg_canon(a.x_i[3 * (size_t)i0 + 2]));
     }
     // bounding box of the tile's i-particles (every warp holds the same ones; NaN coordinates drop out of min / max
     // and never coincide with anything)
@@ -153,6 +153,9 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
             by0 = fminf(by0, __shfl_xor_sync(0xffffffffu, by0, o)); by1 = fmaxf(by1, __shfl_xor_sync(0xffffffffu, by1, o));
             bz0 = fminf(bz0, __shfl_xor_sync(0xffffffffu, bz0, o)); bz1 = fmaxf(bz1, __shfl_xor_sync(0xffffffffu, bz1, o));
         }
+        // a subnormal coordinate counts as zero in the loop (add.ftz): widen the box by the smallest normal number
+        const float tiny = 1.17549435e-38f;
+        bx0 -= tiny; by0 -= tiny; bz0 -= tiny; bx1 += tiny; by1 += tiny; bz1 += tiny;
     }
     __syncthreads();                                                   // barriers initialised
 

@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
         const int i1 = min(i_base + (2 * k2 + 1) * 32, a.n_i - 1);
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            ni[k2][c] = pack2(-a.x_i[3 * (size_t)i0 + c], -a.x_i[3 * (size_t)i1 + c]);
+            ni[k2][c] = pack2(neg_canon(a.x_i[3 * (size_t)i0 + c]), neg_canon(a.x_i[3 * (size_t)i1 + c]));
             ni[k2][3 + c] = pack2(-a.v_i[3 * (size_t)i0 + c], -a.v_i[3 * (size_t)i1 + c]);
         }
     }

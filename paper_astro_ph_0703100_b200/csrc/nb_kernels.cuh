@@ -119,6 +119,11 @@ __global__ void __launch_bounds__(256) nb_pack_j_kernel(const float* __restrict_
 //  default earlier in this round and was removed: DESIGN.md section 10.)
 enum { MASK_EXACT = 0, MASK_NONE = 2 };
 
+// -x_i as the kernels hold it: +0 for a zero or subnormal coordinate (add.ftz reads a subnormal as zero), so that a
+// difference x_j + (-x_i) that is zero is always +0 -- (-0) + (-0) = -0 cannot arise -- and the bitwise test of
+// MASK_EXACT sees every coincident pair, whatever the signs of the zeros involved.
+__device__ __forceinline__ float neg_canon(float x) { return (fabsf(x) < 1.17549435e-38f) ? 0.0f : -x; }
+
 // PHI = false: the caller does not want the potential (pot_out == NULL): 12 FP32-pipe instructions per pair.
 template <int MASK, bool PHI = true>
 __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nxi, u64 nyi, u64 nzi, u64 eps2_2,
@@ -353,9 +358,9 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
     for (int k2 = 0; k2 < K / 2; ++k2) {
         const int i0 = min(i_base + (2 * k2) * 32, i_hi - 1);
         const int i1 = min(i_base + (2 * k2 + 1) * 32, i_hi - 1);
-        nxi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 0], -a.x_i[3 * (size_t)i1 + 0]);
-        nyi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 1], -a.x_i[3 * (size_t)i1 + 1]);
-        nzi[k2] = pack2(-a.x_i[3 * (size_t)i0 + 2], -a.x_i[3 * (size_t)i1 + 2]);
+        nxi[k2] = pack2(neg_canon(a.x_i[3 * (size_t)i0 + 0]), neg_canon(a.x_i[3 * (size_t)i1 + 0]));
+        nyi[k2] = pack2(neg_canon(a.x_i[3 * (size_t)i0 + 1]), neg_canon(a.x_i[3 * (size_t)i1 + 1]));
+        nzi[k2] = pack2(neg_canon(a.x_i[3 * (size_t)i0 + 2]), neg_canon(a.x_i[3 * (size_t)i1 + 2]));
     }
     const u64 eps2_2 = pack2(a.eps2, a.eps2);
     u64 e2[K / 2];

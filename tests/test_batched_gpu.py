@@ -124,3 +124,45 @@ def test_bench_size_sampled(nb):
         i0, i1, j0, j1 = (int(v) for v in (w.i_offsets[b], w.i_offsets[b + 1], w.j_offsets[b], w.j_offsets[b + 1]))
         ra, rp = oracle.force(w.x_i[i0:i1], w.x_j[j0:j1], w.m_j[j0:j1], w.eps2)
         check(acc[i0:i1], pot[i0:i1], ra, rp, f"group {b}")
+
+
+def test_own_members_scattered_through_the_lists_eps0(nb):
+    """The kernel decides per 64 j (bounding box of the tile's i-particles) between the masked and the untested loop.
+    Here the copies of the i-particles sit at random places of the lists (every part of some lists holds one, many hold
+    none), twice each in one group, next to outsiders placed strictly inside the box, with eps = 0 and signed zeros:
+    a coincident pair that met the untested loop would give inf/NaN."""
+    rng = np.random.default_rng(11)
+    n_batch = 12
+    ni = rng.integers(1, 200, n_batch)
+    ni[0], ni[1], ni[2] = 64, 33, 1
+    xi_all, xj_all, mj_all, io, jo = [], [], [], [0], [0]
+    for b in range(n_batch):
+        centre = rng.normal(size=3) * 3.0
+        xi = (centre + rng.uniform(-0.5, 0.5, (ni[b], 3))).astype(np.float32)
+        if b == 3:
+            xi[:, 0] = np.where(np.arange(ni[b]) % 2 == 0, 0.0, -0.0).astype(np.float32)   # signed zeros, x only
+        far = (centre + rng.normal(size=(rng.integers(300, 1500), 3)) * 4.0).astype(np.float32)
+        inside = (centre + rng.uniform(-0.4, 0.4, (40, 3))).astype(np.float32)           # in the box, not coincident
+        own = xi.copy()
+        if b == 3:
+            own[:, 0] = -own[:, 0]                                                       # +0 meets -0: still coincident
+        parts = [far, inside, own] + ([own] if b == 4 else [])
+        xj = np.concatenate(parts)
+        perm = rng.permutation(xj.shape[0])
+        xj = xj[perm]
+        xi_all.append(xi); xj_all.append(xj)
+        mj_all.append(rng.uniform(0.5, 1.5, xj.shape[0]).astype(np.float32) / 1000.0)
+        io.append(io[-1] + ni[b]); jo.append(jo[-1] + xj.shape[0])
+    w = wl.BatchedWorkload("scattered", np.asarray(io, np.int32), np.asarray(jo, np.int32), np.concatenate(xi_all),
+                           np.concatenate(xj_all), np.concatenate(mj_all), 0.0)
+    acc, pot = gpu_batched(nb, w, fill=float("nan"))
+    assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot))
+    ra, rp = oracle.force_batched(w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j, 0.0)
+    check(acc, pot, ra, rp, "scattered")
+    # with a softening the acceleration-only call (untested loop everywhere) must agree bit for bit
+    w1 = wl.BatchedWorkload("scattered-eps", w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j, 1.0 / 4096)
+    a1, p1 = gpu_batched(nb, w1)
+    a2, _ = gpu_batched(nb, w1, want_pot=False)
+    assert np.array_equal(a1, a2)
+    ra, rp = oracle.force_batched(w1.i_offsets, w1.j_offsets, w1.x_i, w1.x_j, w1.m_j, w1.eps2)
+    check(a1, p1, ra, rp, "scattered-eps")

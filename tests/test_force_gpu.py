@@ -482,3 +482,27 @@ def test_randomised_shapes_plans_and_modes(nb, monkeypatch):
         assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4, (label, e)
         if pot is not None:
             assert e["pot_rms"] <= 1e-5, (label, e)
+
+
+@pytest.mark.parametrize("eps2", [0.0, 1.0 / 4096])
+def test_signed_zero_coordinates_coincide(nb, eps2):
+    """Reading R1 asks for differences that are exactly zero, whatever the signs of the zeros: x_i = +0 against
+    x_j = -0 (and the reverse) is a coincident pair.  The kernels hold -x_i with zeros canonicalised to +0, so the
+    difference is +0 in all four sign combinations and the bitwise test catches it."""
+    rng = np.random.default_rng(21)
+    n = 1500
+    x = rng.normal(size=(n, 3)).astype(np.float32)
+    m = (rng.uniform(0.5, 1.5, n) / n).astype(np.float32)
+    x[10] = (0.0, 0.5, -0.0); x[900] = (-0.0, 0.5, 0.0)          # the same point, opposite zero signs
+    x[11] = (-0.0, -0.0, -0.0); x[901] = (0.0, 0.0, 0.0); x[1400] = (-0.0, 0.0, -0.0)
+    acc, pot = gpu_force(nb, x, x, m, eps2)
+    assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot))
+    ref_acc, ref_pot = oracle.force(x, x, m, eps2)
+    check_parity(acc, pot, ref_acc, ref_pot, "signed zeros")
+    # separate i-set (not aliased), zeros of the other sign
+    xi = x[[10, 11, 900, 901, 1400]].copy() * np.float32(-1.0)
+    xi[:, 1] = x[[10, 11, 900, 901, 1400], 1]
+    acc, pot = gpu_force(nb, xi, x, m, eps2)
+    assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot))
+    ref_acc, ref_pot = oracle.force(xi, x, m, eps2)
+    check_parity(acc, pot, ref_acc, ref_pot, "signed zeros, separate i")
