@@ -302,8 +302,32 @@ struct ForceArgs {
 };
 
 // how the force kernel honours the coincident-pair rule
-enum { MODE_EXACT = 0,     // masked loop everywhere (small calls; eps2 == 0 or tiny)
+enum { MODE_EXACT = 0,     // masked loop everywhere (eps2 == 0 or tiny; per-i softening on small calls)
+       MODE_BLOOM = 1,     // per-warp Bloom filter of the i-positions in shared memory, every 256-j block tested (mid-size calls)
        MODE_LIST = 2 };    // coincidence lists from the pre-pass, no test in the hot loop (large calls; a-only calls)
+
+// MODE_BLOOM: 2^16 filter bits (8 KB) per group of warps that hold the same i-particles, two bits per position.
+// The key is computed on the coordinates as the loop sees them (x + 0 under add.ftz: -0 and subnormals become +0),
+// so two positions the masked loop calls coincident always have the same key: no false negatives.
+constexpr int kBloomWords = 2048;
+__device__ __forceinline__ uint32_t bloom_key(float x, float y, float z) {
+    float cx, cy, cz;
+    asm("add.ftz.f32 %0, %1, 0f00000000;" : "=f"(cx) : "f"(x));
+    asm("add.ftz.f32 %0, %1, 0f00000000;" : "=f"(cy) : "f"(y));
+    asm("add.ftz.f32 %0, %1, 0f00000000;" : "=f"(cz) : "f"(z));
+    uint32_t h = __float_as_uint(cx) * 0x9E3779B1u;
+    h = __float_as_uint(cy) * 0x85EBCA77u + h;
+    h = __float_as_uint(cz) * 0xC2B2AE3Du + (h ^ (h >> 15));
+    h ^= h >> 16;
+    return h * 0x2C1B3C6Du;
+}
+__device__ __forceinline__ void bloom_set(uint32_t* filt, uint32_t h) {
+    atomicOr(filt + (h >> 21), 1u << ((h >> 16) & 31u));
+    atomicOr(filt + ((h >> 5) & 2047u), 1u << (h & 31u));
+}
+__device__ __forceinline__ bool bloom_test(const uint32_t* filt, uint32_t h) {
+    return ((filt[h >> 21] >> ((h >> 16) & 31u)) & (filt[(h >> 5) & 2047u] >> (h & 31u)) & 1u) != 0u;
+}
 
 // ---------------------------------------------------------------- a2..a7: the force kernel
 // CTA = 8 warps = WI (along i) x WJ (along j).  A CTA owns 32*K*WI i-particles (K per thread, in
@@ -315,7 +339,7 @@ template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I = fals
           int SUB = 256>
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
-    static_assert(MODE == MODE_EXACT || MODE == MODE_LIST, "masked everywhere, or coincidence lists");
+    static_assert(MODE == MODE_EXACT || MODE == MODE_BLOOM || MODE == MODE_LIST, "masked everywhere, Bloom filter, or coincidence lists");
     static_assert(SUB == kCoinSeg, "coincidence segments are SUB j-particles");
     extern __shared__ __align__(128) unsigned char smem_raw[];
 
@@ -375,7 +399,21 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
         }
     }
 
-    __syncthreads();                                                   // barriers initialised
+    // MODE_BLOOM: the filter of this warp's i-positions (the WJ warps with the same wi share it)
+    uint32_t* filt = reinterpret_cast<uint32_t*>(smem_raw + WJ * RING_BYTES + 2 * WJ * STAGES * 8) + wi * kBloomWords;
+    if (MODE == MODE_BLOOM) {
+        uint4* z = reinterpret_cast<uint4*>(smem_raw + WJ * RING_BYTES + 2 * WJ * STAGES * 8);
+        for (int q = threadIdx.x; q < WI * kBloomWords / 4; q += 32 * WI * WJ) z[q] = make_uint4(0u, 0u, 0u, 0u);
+        __syncthreads();
+        if (wj == 0) {
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                const int i = min(i_base + k * 32, i_hi - 1);
+                bloom_set(filt, bloom_key(a.x_i[3 * (size_t)i + 0], a.x_i[3 * (size_t)i + 1], a.x_i[3 * (size_t)i + 2]));
+            }
+        }
+    }
+    __syncthreads();                                                   // barriers initialised, filters built
 
     // Small calls (nbody_b200.cu: the whole sub-range fits the ring): rows a1 + a2 in one step -- the WI warps of the
     // group pack their sub-range from x_j / m_j into the ring themselves (Fig. A.1 packing loop);
@@ -430,6 +468,17 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_force_kernel(const ForceAr
                     coin_next = (coin_pos < coin_cnt) ? coin[1 + coin_pos] : 0x7fffffff;
                 }
                 if (coin_cnt < 0 || coin_next <= seg_hi)               // rare: the block holds a coincident pair
+                    tile_sweep<K, MASK_EXACT, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph, e2);
+                else
+                    tile_sweep<K, MASK_NONE, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph, e2);
+            } else if (MODE == MODE_BLOOM) {
+                bool hit = false;                                      // may a j of this block coincide with an i of this warp?
+#pragma unroll
+                for (int q = 0; q < SUB; q += 32) {                    // branch-free: 8 independent chains (a short block tests its last j again)
+                    const float4 J = sp[c + min(q + lane, nc - 1)];
+                    hit |= bloom_test(filt, bloom_key(J.x, J.y, J.z));
+                }
+                if (__any_sync(0xffffffffu, hit))
                     tile_sweep<K, MASK_EXACT, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph, e2);
                 else
                     tile_sweep<K, MASK_NONE, EPS_I, PHI>(sp + c, nc, nxi, nyi, nzi, eps2_2, pax, pay, paz, pph, e2);

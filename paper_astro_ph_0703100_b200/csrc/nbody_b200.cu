@@ -113,19 +113,27 @@ nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count) {
 // the acceleration-only path need eps2 >= 2^-40; below that (and for eps2 == 0) every pair is masked.
 constexpr float kUnmaskedMinEps2 = 9.094947017729282e-13f;
 
-// Calls with at least this many pairs locate their coincident pairs with the hash-join pre-pass
-// (MODE_LIST: three extra O(n) launches, ~35 us, no test in the hot loop); smaller ones mask every pair
-// (MODE_EXACT: a small call is a single wave of CTAs, and 35 us of pre-pass would cost more than the mask).
-constexpr double kListMinPairs = 536870912.0;    // 2^29
+// Where the coincident pairs are found (reading R1), by call size:
+//   >= 2^32 pairs   MODE_LIST: hash-join pre-pass (three extra O(n) launches, ~35 us), no test in the hot loop;
+//   >= 2^25 pairs   MODE_BLOOM: the force kernel tests every 256-j block against a Bloom filter of its warp's
+//                   i-positions (~1 % of the loop), no pre-pass -- and the small-call one-launch path stays possible;
+//   smaller, eps2 < 2^-40, per-i softening below the list size: MODE_EXACT, every pair masked.
+constexpr double kListMinPairs = 4294967296.0;   // 2^32
+constexpr double kListMinPairsNoBloom = 536870912.0;   // 2^29 (per-i softening and the jerk kernel have no Bloom instantiation)
+constexpr double kBloomMinPairs = 33554432.0;    // 2^25
 
-int pick_mode(int64_t n_i, int64_t n_j, float eps2) {
-    // debugging aid: NB_MASK=exact|list forces a mode (list still needs eps2 >= 2^-40 and n_j <= 2^29)
+int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool bloom_ok) {
+    // debugging aid: NB_MASK=exact|bloom|list forces a mode (bloom and list still need eps2 >= 2^-40, list n_j <= 2^29)
     const char* e = std::getenv("NB_MASK");
     if (e && e[0] == 'e') return nb::MODE_EXACT;
     if (eps2 < kUnmaskedMinEps2) return nb::MODE_EXACT;
-    if (n_j > ((int64_t)1 << 29)) return nb::MODE_EXACT;             // the 32-bit hash table holds 2 n_j <= 2^30 slots
-    if (e && e[0] == 'l') return nb::MODE_LIST;
-    return ((double)n_i * (double)n_j >= kListMinPairs) ? nb::MODE_LIST : nb::MODE_EXACT;
+    const bool list_ok = n_j <= ((int64_t)1 << 29);                    // the 32-bit hash table holds 2 n_j <= 2^30 slots
+    const double pairs = (double)n_i * (double)n_j;
+    if (!bloom_ok) return (list_ok && ((e && e[0] == 'l') || pairs >= kListMinPairsNoBloom)) ? nb::MODE_LIST : nb::MODE_EXACT;
+    if (e && e[0] == 'l') return list_ok ? nb::MODE_LIST : nb::MODE_EXACT;
+    if (e && e[0] == 'b') return nb::MODE_BLOOM;
+    if (list_ok && pairs >= kListMinPairs) return nb::MODE_LIST;
+    return pairs >= kBloomMinPairs ? nb::MODE_BLOOM : nb::MODE_EXACT;
 }
 
 // One launch of a dominant kernel: raises the kernel's dynamic shared-memory limit once per device, brackets the
@@ -159,7 +167,8 @@ template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool EPS_I, bool 
 int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     constexpr size_t ring = (size_t)WJ * STAGES * TJ * 16;
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
-    constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
+    constexpr size_t bloom = (MODE == nb::MODE_BLOOM) ? (size_t)WI * nb::kBloomWords * sizeof(uint32_t) : 0;
+    constexpr size_t smem = (ring + bloom > red ? ring + bloom : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
     static bool configured[64] = {};
     return launch_dominant(nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, EPS_I, PHI, DIRECT>, configured,
                            dim3((unsigned)plan.tiles_i, (unsigned)plan.S, 1), 32 * WI * WJ, smem, stream, args);
@@ -267,7 +276,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         }
     }
 
-    const int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2);
+    const int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2, eps2_i == nullptr);
     // Without phi no pair needs a mask when eps2 >= 2^-40: an unmasked coincident pair adds m u^3 * (+-0) = +-0 to a
     // (only phi would get m / eps), so a_i is bit for bit the masked loop's.  The list-mode kernel then runs with an
     // empty list: no pre-pass, the untested loop everywhere (nb_leapfrog_kdk: every evaluation but the last).
@@ -276,7 +285,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     // sub-range itself, one launch fewer (C0: 21 -> 16 us per call).  NB_DIRECT=0 disables it (tests compare).
     const int64_t sub_max = (n_j + (int64_t)plan.S * plan.WJ - 1) / ((int64_t)plan.S * plan.WJ);
     const char* dr = std::getenv("NB_DIRECT");
-    const bool direct = !packed_j && !eps2_i && mode == nb::MODE_EXACT && sub_max <= (int64_t)plan.tile_j * plan.stages &&
+    const bool direct = !packed_j && !eps2_i && mode != nb::MODE_LIST && sub_max <= (int64_t)plan.tile_j * plan.stages &&
                         !(dr && dr[0] == '0');
     const float4* jp = packed_j ? packed_j : reinterpret_cast<const float4*>(ws->jp);
     if (!packed_j && !direct) {   // a1: j-pack
@@ -305,8 +314,9 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.coin_flag = nullptr;
     args.i_off = args.j_off = args.tile_start = args.cta_batch = nullptr;
     args.n_batch = 0;
-    if (direct) {                                                      // small call: one launch (masked loop, packs its own j)
-        rc = launch_force<nb::MODE_EXACT, false, true>(args, plan, stream);
+    if (direct) {                                                      // small call: one launch (packs its own j)
+        rc = (mode == nb::MODE_BLOOM) ? launch_force<nb::MODE_BLOOM, false, true>(args, plan, stream)
+                                      : launch_force<nb::MODE_EXACT, false, true>(args, plan, stream);
     } else if (a_only) {
         rc = (plan.K == 8) ? launch_force_nophi(args, plan, stream) : launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (mode == nb::MODE_LIST) {
@@ -317,6 +327,8 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         else rc = launch_force<nb::MODE_LIST>(args, plan, stream);
     } else if (eps2_i) {
         rc = launch_force<nb::MODE_EXACT, true>(args, plan, stream);
+    } else if (mode == nb::MODE_BLOOM) {
+        rc = launch_force<nb::MODE_BLOOM>(args, plan, stream);
     } else {
         rc = launch_force<nb::MODE_EXACT>(args, plan, stream);
     }
@@ -439,7 +451,7 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     args.S = plan.S;
     args.eps2 = eps2;
     // small calls mask every pair, large ones use the coincidence lists
-    const int mode = pick_mode(n_i, n_j, eps2);
+    const int mode = pick_mode(n_i, n_j, eps2, false);
     if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, args.jp, 2, stream, &args.coin_lists, &args.coin_flag);
         if (rc != NB_OK) return rc;

@@ -118,10 +118,13 @@ def test_masked_list_and_acceleration_only_paths_agree_bitwise(nb, monkeypatch):
 
 def _both_modes(nb, monkeypatch, x_i, x_j, m_j, eps2, alias=False):
     out = {}
-    for mode in ("exact", "list"):
+    for mode in ("exact", "list", "bloom"):
         monkeypatch.setenv("NB_MASK", mode)
         out[mode] = gpu_force(nb, x_i, x_j, m_j, eps2, alias=alias)
     monkeypatch.delenv("NB_MASK")
+    # MODE_BLOOM (filter of the warp's i-positions in shared memory, every 256-j block tested in the kernel) must
+    # store what the always-masked kernel stores, bit for bit, wherever the list mode must
+    assert np.array_equal(out["exact"][0], out["bloom"][0]) and np.array_equal(out["exact"][1], out["bloom"][1])
     return out
 
 
@@ -341,7 +344,7 @@ def test_no_potential_variant_gives_the_same_acceleration_bitwise(nb, monkeypatc
         assert p2 is None and np.array_equal(a1, a2), plan
 
 
-@pytest.mark.parametrize("n,mode", [(2048, ""), (3000, "list"), (3000, "exact")])
+@pytest.mark.parametrize("n,mode", [(2048, ""), (3000, "list"), (3000, "exact"), (3000, "bloom"), (9000, "")])
 def test_cuda_graph_capture_and_replay(nb, n, mode, monkeypatch):
     """include/nbody_b200.h: "once warm the call is CUDA-graph capturable" -- capture nb_force (small-call path with the
     fused second pass; large-call path with the coincidence pre-pass and its memset), replay on new inputs."""
@@ -459,7 +462,7 @@ def test_randomised_shapes_plans_and_modes(nb, monkeypatch):
         alias = bool(rng.integers(0, 2))
         n_i = n_j if alias else int(rng.integers(1, 3000))
         k = int(rng.choice([2, 4, 8])); wj = int(rng.choice([1, 2, 4, 8])); s = int(rng.integers(1, 7))
-        mode = str(rng.choice(["exact", "list", ""]))
+        mode = str(rng.choice(["exact", "list", "bloom", ""]))
         want_pot = bool(rng.integers(0, 4))
         eps2 = float(np.float32(2.0 ** rng.integers(-16, -2)))
         x_j = rng.normal(size=(n_j, 3)).astype(np.float32)
@@ -506,3 +509,32 @@ def test_signed_zero_coordinates_coincide(nb, eps2):
     assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot))
     ref_acc, ref_pot = oracle.force(xi, x, m, eps2)
     check_parity(acc, pot, ref_acc, ref_pot, "signed zeros, separate i")
+
+
+@pytest.mark.parametrize("n", [4096, 9000])
+def test_bloom_mode_lattice_duplicates_and_eps_threshold(nb, n, monkeypatch):
+    """MODE_BLOOM on inputs that stress the filter: a cubic lattice (few mantissa bits set: weak keys would collide),
+    every particle present twice, planar z = +-0, one sub-call direct (one launch) and one through the packed ring;
+    the result is the always-masked one bit for bit and within tolerance of the oracle."""
+    side = int(round((n / 2) ** (1.0 / 3.0))) + 1
+    g = np.stack(np.meshgrid(*[np.arange(side, dtype=np.float32)] * 3, indexing="ij"), -1).reshape(-1, 3)[: n // 2]
+    g = g / np.float32(side) - np.float32(0.5)
+    g[:, 2] = np.where(np.arange(g.shape[0]) % 2 == 0, np.float32(0.0), np.float32(-0.0)) if n == 4096 else g[:, 2]
+    x = np.concatenate([g, g[::-1]]).astype(np.float32)               # every position twice, far apart in j
+    rng = np.random.default_rng(5)
+    m = (rng.uniform(0.5, 1.5, x.shape[0]) / x.shape[0]).astype(np.float32)
+    eps2 = 1.0 / 1024
+    for direct in ("1", "0"):
+        monkeypatch.setenv("NB_DIRECT", direct)
+        out = {}
+        for mode in ("exact", "bloom"):
+            monkeypatch.setenv("NB_MASK", mode)
+            out[mode] = gpu_force(nb, x, x, m, eps2, alias=True)
+        monkeypatch.delenv("NB_MASK")
+        assert np.array_equal(out["exact"][0], out["bloom"][0]) and np.array_equal(out["exact"][1], out["bloom"][1])
+    ref_acc, ref_pot = oracle.force(x, x, m, eps2)
+    e = oracle.error_metrics(out["bloom"][0], ref_acc, out["bloom"][1], ref_pot)
+    assert e["pot_rms"] <= 1e-5, e                                     # a missed duplicate would shift phi by m / eps
+    # lattice forces cancel by symmetry in the interior: compare a absolutely against the typical magnitude
+    scale = np.sqrt((ref_acc.astype(np.float64) ** 2).sum(1)).max()
+    assert np.abs(out["bloom"][0] - ref_acc).max() <= 1e-5 * scale
