@@ -18,7 +18,8 @@
 //       3 FADD (d)  3 FFMA (r2)  3 FMUL (u2, m u, m u^3)  3 FADD (dv)  1 FMUL + 2 FFMA (d.dv)
 //       2 FMUL (u2 (d.dv), m u^5 (d.dv))  3 FFMA (a)  3 FFMA (J1)  3 FFMA (J2)  1 FADD (phi).
 // Coincident pairs (all three POSITION differences exactly zero, reading R1) add nothing:
-// MODE_EXACT masks every pair; MODE_LIST uses the coincidence lists of the pre-pass (nb_kernels.cuh)
+// MODE_EXACT masks every pair; MODE_BLOOM tests every 256-j block against a filter of the warp's i-positions;
+// MODE_LIST uses the coincidence lists of the pre-pass (all three: nb_kernels.cuh)
 // and masks only the listed j-segments.  An unmasked coincident pair would add m dv / eps^3 to the
 // jerk, so unlike the plain force there is no speculative mode here.
 #pragma once
@@ -127,7 +128,7 @@ template <int K, int WI, int WJ, int TJ, int STAGES, int MODE, bool PHI = true, 
 __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const HermiteArgs a) {
     static_assert(K % 2 == 0, "i-particles are held in pairs");
     static_assert(SUB == kCoinSeg, "coincidence segments are SUB j-particles");
-    static_assert(MODE == MODE_EXACT || MODE == MODE_LIST, "no speculative mode for the jerk");
+    static_assert(MODE == MODE_EXACT || MODE == MODE_BLOOM || MODE == MODE_LIST, "masked everywhere, Bloom filter, or coincidence lists");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int REC = 32;
     constexpr int RING_BYTES = STAGES * TJ * REC;
@@ -169,7 +170,21 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
         }
     }
     const u64 eps2_2 = pack2(a.eps2, a.eps2);
-    __syncthreads();
+    // MODE_BLOOM: the filter of this warp's i-positions (nb_kernels.cuh; the WJ warps with the same wi share it)
+    uint32_t* filt = reinterpret_cast<uint32_t*>(smem_raw + WJ * RING_BYTES + 2 * WJ * STAGES * 8) + wi * kBloomWords;
+    if (MODE == MODE_BLOOM) {
+        uint4* z = reinterpret_cast<uint4*>(smem_raw + WJ * RING_BYTES + 2 * WJ * STAGES * 8);
+        for (int q = threadIdx.x; q < WI * kBloomWords / 4; q += 32 * WI * WJ) z[q] = make_uint4(0u, 0u, 0u, 0u);
+        __syncthreads();
+        if (wj == 0) {
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                const int i = min(i_base + k * 32, a.n_i - 1);
+                bloom_set(filt, bloom_key(a.x_i[3 * (size_t)i + 0], a.x_i[3 * (size_t)i + 1], a.x_i[3 * (size_t)i + 2]));
+            }
+        }
+    }
+    __syncthreads();                                                   // barriers initialised, filters built
 
     if (producer) {
         const int pre = n_tiles < STAGES ? n_tiles : STAGES;
@@ -211,6 +226,14 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
                     coin_next = (coin_pos < coin_cnt) ? coin[1 + coin_pos] : 0x7fffffff;
                 }
                 masked = (coin_cnt < 0 || coin_next <= seg_hi);
+            } else if (MODE == MODE_BLOOM) {
+                bool hit = false;                                      // may a j of this block coincide with an i of this warp?
+#pragma unroll
+                for (int q = 0; q < SUB; q += 32) {                    // branch-free: 8 independent chains
+                    const float4 J = sp[2 * (c + min(q + lane, nc - 1))];
+                    hit |= bloom_test(filt, bloom_key(J.x, J.y, J.z));
+                }
+                masked = __any_sync(0xffffffffu, hit);
             }
             if (masked) hermite_sweep<K, true, PHI>(sp + 2 * c, nc, ni, eps2_2, part);
             else hermite_sweep<K, false, PHI>(sp + 2 * c, nc, ni, eps2_2, part);

@@ -119,10 +119,11 @@ constexpr float kUnmaskedMinEps2 = 9.094947017729282e-13f;
 //                   i-positions (~1 % of the loop), no pre-pass -- and the small-call one-launch path stays possible;
 //   smaller, eps2 < 2^-40, per-i softening below the list size: MODE_EXACT, every pair masked.
 constexpr double kListMinPairs = 4294967296.0;   // 2^32
-constexpr double kListMinPairsNoBloom = 536870912.0;   // 2^29 (per-i softening and the jerk kernel have no Bloom instantiation)
+constexpr double kListMinPairsNoBloom = 536870912.0;   // 2^29 (per-i softening has no Bloom instantiation)
 constexpr double kBloomMinPairs = 33554432.0;    // 2^25
+constexpr double kListMinPairsJerk = 1073741824.0;   // 2^30: the jerk kernel's pre-pass pays off earlier (measured tie at N = 32768)
 
-int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool bloom_ok) {
+int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool bloom_ok, double list_min_pairs = kListMinPairs) {
     // debugging aid: NB_MASK=exact|bloom|list forces a mode (bloom and list still need eps2 >= 2^-40, list n_j <= 2^29)
     const char* e = std::getenv("NB_MASK");
     if (e && e[0] == 'e') return nb::MODE_EXACT;
@@ -132,7 +133,7 @@ int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool bloom_ok) {
     if (!bloom_ok) return (list_ok && ((e && e[0] == 'l') || pairs >= kListMinPairsNoBloom)) ? nb::MODE_LIST : nb::MODE_EXACT;
     if (e && e[0] == 'l') return list_ok ? nb::MODE_LIST : nb::MODE_EXACT;
     if (e && e[0] == 'b') return nb::MODE_BLOOM;
-    if (list_ok && pairs >= kListMinPairs) return nb::MODE_LIST;
+    if (list_ok && pairs >= list_min_pairs) return nb::MODE_LIST;
     return pairs >= kBloomMinPairs ? nb::MODE_BLOOM : nb::MODE_EXACT;
 }
 
@@ -359,7 +360,8 @@ int launch_hermite_inst(const nb::HermiteArgs& args, const nb::Plan& plan, cudaS
     constexpr int TJ = 256;
     constexpr size_t ring = (size_t)WJ * STAGES * TJ * 32;
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * nb::kHermiteAcc * (WI * 32) * sizeof(double) : 0;
-    constexpr size_t smem = (ring > red ? ring : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
+    constexpr size_t bloom = (MODE == nb::MODE_BLOOM) ? (size_t)WI * nb::kBloomWords * sizeof(uint32_t) : 0;
+    constexpr size_t smem = (ring + bloom > red ? ring + bloom : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
     static bool configured[64] = {};
     return launch_dominant(nb::nb_hermite_kernel<K, WI, WJ, TJ, STAGES, MODE, PHI>, configured,
                            dim3((unsigned)plan.tiles_i, (unsigned)plan.S, 1), 32 * WI * WJ, smem, stream, args);
@@ -375,13 +377,14 @@ int launch_hermite_k(const nb::HermiteArgs& args, const nb::Plan& plan, cudaStre
     }
 }
 
-// pot_out == NULL on a large call (nb_hermite4: every evaluation but the last): 26 instructions per pair, K = 4 only
+// pot_out == NULL (nb_hermite4: every evaluation but the last): 26 instructions per pair, K = 4, list and Bloom modes
+template <int MODE>
 int launch_hermite_nophi(const nb::HermiteArgs& args, const nb::Plan& plan, cudaStream_t stream) {
     switch (plan.WJ) {
-        case 1: return launch_hermite_inst<4, 8, 1, 4, nb::MODE_LIST, false>(args, plan, stream);
-        case 2: return launch_hermite_inst<4, 4, 2, 4, nb::MODE_LIST, false>(args, plan, stream);
-        case 4: return launch_hermite_inst<4, 2, 4, 3, nb::MODE_LIST, false>(args, plan, stream);
-        default: return launch_hermite_inst<4, 1, 8, 3, nb::MODE_LIST, false>(args, plan, stream);
+        case 1: return launch_hermite_inst<4, 8, 1, 4, MODE, false>(args, plan, stream);
+        case 2: return launch_hermite_inst<4, 4, 2, 4, MODE, false>(args, plan, stream);
+        case 4: return launch_hermite_inst<4, 2, 4, 3, MODE, false>(args, plan, stream);
+        default: return launch_hermite_inst<4, 1, 8, 3, MODE, false>(args, plan, stream);
     }
 }
 
@@ -450,12 +453,14 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     args.n_j = (int)n_j;
     args.S = plan.S;
     args.eps2 = eps2;
-    // small calls mask every pair, large ones use the coincidence lists
-    const int mode = pick_mode(n_i, n_j, eps2, false);
+    // small calls mask every pair, mid-size ones test every block against a Bloom filter, large ones use the coincidence lists
+    const int mode = pick_mode(n_i, n_j, eps2, true, kListMinPairsJerk);
     if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, args.jp, 2, stream, &args.coin_lists, &args.coin_flag);
         if (rc != NB_OK) return rc;
-        rc = (!pot_out && plan.K == 4) ? launch_hermite_nophi(args, plan, stream) : launch_hermite<nb::MODE_LIST>(args, plan, stream);
+        rc = (!pot_out && plan.K == 4) ? launch_hermite_nophi<nb::MODE_LIST>(args, plan, stream) : launch_hermite<nb::MODE_LIST>(args, plan, stream);
+    } else if (mode == nb::MODE_BLOOM) {
+        rc = (!pot_out && plan.K == 4) ? launch_hermite_nophi<nb::MODE_BLOOM>(args, plan, stream) : launch_hermite<nb::MODE_BLOOM>(args, plan, stream);
     } else {
         rc = launch_hermite<nb::MODE_EXACT>(args, plan, stream);
     }

@@ -76,7 +76,7 @@ def test_ragged_shapes_separate_sets(nb, n_i, n_j):
 PLANS = [(k, 8 // wj, wj, s) for k in (2, 4) for wj in (1, 2, 4, 8) for s in (1, 3)]
 
 
-@pytest.mark.parametrize("mode", ["exact", "list"])
+@pytest.mark.parametrize("mode", ["exact", "list", "bloom"])
 @pytest.mark.parametrize("plan", PLANS, ids=lambda p: "K%d_WI%d_WJ%d_S%d" % p)
 def test_every_decomposition_matches_oracle(nb, plan, mode, monkeypatch):
     monkeypatch.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
@@ -96,11 +96,19 @@ def test_list_mode_agrees_bitwise_with_masked_kernel(nb, monkeypatch):
     x[2999] = x[5]; x[1500] = x[5]                 # duplicates in other segments, with their own velocities
     x[700] = (0.0, 0.0, 0.0); x[2100] = (-0.0, 1e-41, 0.0)
     out = {}
-    for mode in ("exact", "list"):
+    for mode in ("exact", "list", "bloom"):
         monkeypatch.setenv("NB_MASK", mode)
         out[mode] = gpu_fj(nb, x, v, x, v, m, eps2, alias=True)
-    for a, b in zip(out["exact"], out["list"]):
-        assert np.array_equal(a, b)
+    for a, b, c in zip(out["exact"], out["list"], out["bloom"]):
+        assert np.array_equal(a, b) and np.array_equal(a, c)
+    monkeypatch.setenv("NB_PLAN", "4,8,1,2")       # K = 4: without the potential the 26-instruction loop runs; same a and jerk
+    monkeypatch.setenv("NB_MASK", "exact")
+    ref = gpu_fj(nb, x, v, x, v, m, eps2, alias=True)
+    for mode in ("list", "bloom"):
+        monkeypatch.setenv("NB_MASK", mode)
+        a, j, p = gpu_fj(nb, x, v, x, v, m, eps2, alias=True, want_pot=False)
+        assert p is None and np.array_equal(a, ref[0]) and np.array_equal(j, ref[1])
+    monkeypatch.delenv("NB_PLAN")
     ra, rj, rp = oracle.force_jerk(x, v, x, v, m, eps2)
     keep = np.ones(3000, bool); keep[[700, 2100]] = False       # the oracle does not flush 1e-41
     check(out["list"][0][keep], out["list"][1][keep], out["list"][2][keep], ra[keep], rj[keep], rp[keep], "list")
