@@ -893,7 +893,39 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
     float* vp = reinterpret_cast<float*>(base + b3);
     float* a1 = reinterpret_cast<float*>(base + 2 * b3);
     float* j1 = reinterpret_cast<float*>(base + 3 * b3);
+    // As in nb_leapfrog_kdk: on small systems the host's enqueueing is the limit, so the identical middle steps
+    // (predict, force + jerk without phi, correct) are captured once into a CUDA graph and replayed.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    NB_CUDA(cudaStreamIsCapturing(stream, &cap));
+    const char* ng = std::getenv("NB_STEP_GRAPH");
+    const bool real_stream = reinterpret_cast<uintptr_t>(stream) > 2;   // the default streams cannot be captured
+    const bool step_graph = real_stream && n_steps >= 16 && n <= 32768 && cap == cudaStreamCaptureStatusNone && !t_profile &&
+                            !(ng && ng[0] == '0');
     for (int64_t s = 0; s < n_steps; ++s) {
+        if (step_graph && s == 2) {                                    // steps 0 and 1 ran eagerly: everything is warm
+            cudaGraph_t graph = nullptr;
+            cudaGraphExec_t exec = nullptr;
+            NB_CUDA(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
+            nb::nb_hermite_predict_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, xp, vp, n3, dt);
+            t_launches = 0;
+            rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, nullptr, stream);
+            const int64_t per_step = t_launches + 2;
+            nb::nb_hermite_correct_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, a1, j1, n3, dt);
+            cudaError_t ce = cudaStreamEndCapture(stream, &graph);
+            if (rc != NB_OK || ce != cudaSuccess) {
+                if (graph) (void)cudaGraphDestroy(graph);
+                if (rc != NB_OK) return rc;
+                t_last_cuda_error = (int)ce;
+                return NB_ERR_CUDA;
+            }
+            NB_CUDA(cudaGraphInstantiate(&exec, graph, 0));
+            const int64_t replays = n_steps - 1 - s;                   // steps s .. n_steps-2
+            for (int64_t r = 0; r < replays; ++r) NB_CUDA(cudaGraphLaunch(exec, stream));
+            (void)cudaGraphExecDestroy(exec);                          // freed by the runtime once the replays have run
+            (void)cudaGraphDestroy(graph);
+            launches += per_step * replays;
+            s += replays;                                              // the last step follows eagerly (it wants phi)
+        }
         nb::nb_hermite_predict_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, xp, vp, n3, dt);
         NB_CUDA(cudaGetLastError());
         t_launches = 0;

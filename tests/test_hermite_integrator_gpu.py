@@ -76,3 +76,25 @@ def test_invalid_arguments(nb):
     L = nb.lib()
     assert L.nb_hermite4(5, None, None, None, 0.1, 0.1, 1, None, None, None, None) == 1
     assert L.nb_hermite4(0, None, None, None, 0.1, 0.1, -1, None, None, None, None) == 1
+
+
+@pytest.mark.parametrize("n", [1500, 9000])
+def test_step_graph_replay_is_bitwise_the_eager_sequence(nb, n, monkeypatch):
+    """Small systems replay their identical middle steps (predict, force + jerk without phi, correct) from a CUDA
+    graph: same launches, same bits as the eager sequence (n = 9000: the Bloom-filter kernel inside the graph)."""
+    import torch
+    w = wl.plummer_workload(n, 1.0 / 64, seed=8, with_velocities=True)
+    out = {}
+    side = torch.cuda.Stream()                     # the default stream cannot be captured: graphs need a real stream
+    for mode in ("1", "0"):
+        monkeypatch.setenv("NB_STEP_GRAPH", mode)
+        x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            acc, jerk, pot = nb.hermite4(x, v, m, w.eps2, 1.0 / 256, 24)
+        torch.cuda.synchronize()
+        out[mode] = (x.cpu().numpy(), v.cpu().numpy(), acc.cpu().numpy(), jerk.cpu().numpy(), pot.cpu().numpy(),
+                     nb.last_launch_count())
+    for a, b in zip(out["1"][:5], out["0"][:5]):
+        assert np.array_equal(a, b)
+    assert out["1"][5] == out["0"][5]
