@@ -58,7 +58,7 @@ inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, i
     const double waves = double((int64_t)((ctas + sm_count - 1) / sm_count));
     const double j_per_cta = double(n_j) / S;
     // fewer i-particles per thread: more shared-memory reads and loop overhead per pair
-    const double k_pen = (K == 8) ? 1.0 : (K == 4 ? 1.03 : 1.12);
+    const double k_pen = (K == 8) ? 1.0 : (K == 4 ? 1.06 : 1.15);
     // measured on B200 at full occupancy (one wave of 148 CTAs, K = 8): WJ = 1 / 2 / 4 / 8 reach
     // 82.8 / 77.9 / 81.7 / 81.6 % of the FP32 roofline
     const double wj_pen = (WJ == 1) ? 1.0 : (WJ == 2 ? 1.06 : 1.014);

@@ -104,6 +104,7 @@ nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count) {
     auto it = g_plans.find(key);
     if (it != g_plans.end() && !std::getenv("NB_PLAN")) return it->second;
     nb::Plan p = nb::make_plan(n_i, n_j, sm_count);
+    if (std::getenv("NB_PLAN")) return p;                              // a forced plan is not remembered
     if (g_plans.size() > 4096) g_plans.clear();
     g_plans[key] = p;
     return p;
