@@ -327,14 +327,26 @@ __global__ void __launch_bounds__(128) nb_hermite_reduce_kernel(const double* __
 
 // ---------------------------------------------------------------- shared-time-step Hermite integrator (O(N) kernels)
 // predict:  xp = x + v dt + a dt^2/2 + j dt^3/6,   vp = v + a dt + j dt^2/2      (Horner form, FP32 FMAs)
-__global__ void __launch_bounds__(256) nb_hermite_predict_kernel(const float* __restrict__ x, const float* __restrict__ v,
-                                                                 const float* __restrict__ a, const float* __restrict__ j,
-                                                                 float* __restrict__ xp, float* __restrict__ vp, int n3, float dt) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n3) return;
-    const float aa = a[k], jj = j[k], vv = v[k];
-    xp[k] = fmaf(fmaf(fmaf(jj, dt * (1.0f / 3.0f), aa), dt * 0.5f, vv), dt, x[k]);
-    vp[k] = fmaf(fmaf(jj, dt * 0.5f, aa), dt, vv);
+// One thread per particle; it also writes the packed (x, y, z, m | vx, vy, vz, 0) records of the predicted state
+// (what nb_pack_jv_kernel would write): a step of nb_hermite4 saves a launch and a pass over the particles.
+__global__ void __launch_bounds__(256) nb_hermite_predict_pack_kernel(const float* __restrict__ x, const float* __restrict__ v,
+                                                                      const float* __restrict__ a, const float* __restrict__ j,
+                                                                      const float* __restrict__ m, float* __restrict__ xp,
+                                                                      float* __restrict__ vp, float4* __restrict__ jp, int n, float dt) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float px[3], pv[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const size_t k = 3 * (size_t)i + c;
+        const float aa = a[k], jj = j[k], vv = v[k];
+        px[c] = fmaf(fmaf(fmaf(jj, dt * (1.0f / 3.0f), aa), dt * 0.5f, vv), dt, x[k]);
+        pv[c] = fmaf(fmaf(jj, dt * 0.5f, aa), dt, vv);
+        xp[k] = px[c];
+        vp[k] = pv[c];
+    }
+    jp[2 * (size_t)i + 0] = make_float4(px[0], px[1], px[2], m[i]);
+    jp[2 * (size_t)i + 1] = make_float4(pv[0], pv[1], pv[2], 0.0f);
 }
 // correct:  v' = v + (a0 + a1) dt/2 + (j0 - j1) dt^2/12,   x' = x + (v + v') dt/2 + (a0 - a1) dt^2/12;   a0, j0 <- a1, j1
 __global__ void __launch_bounds__(256) nb_hermite_correct_kernel(float* __restrict__ x, float* __restrict__ v,

@@ -395,7 +395,8 @@ int launch_hermite(const nb::HermiteArgs& args, const nb::Plan& plan, cudaStream
 }
 
 int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j, const float* x_j, const float* v_j,
-                    const float* m_j, float eps2, float* acc_out, float* jerk_out, float* pot_out, cudaStream_t stream) {
+                    const float* m_j, float eps2, float* acc_out, float* jerk_out, float* pot_out, cudaStream_t stream,
+                    bool prepacked = false) {   // prepacked: the caller has filled the workspace's packed j records
     if (bad_count(n_i) || bad_count(n_j)) return NB_ERR_INVALID_VALUE;
     if (!(eps2 >= 0.0f) || !std::isfinite(eps2)) return NB_ERR_INVALID_VALUE;
     if (n_i > 0 && (!x_i || !v_i || !acc_out || !jerk_out)) return NB_ERR_INVALID_VALUE;
@@ -421,7 +422,7 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
         } else {
             plan = hermite_plan(n_i, n_j, info.sm_count);
             if (g_hplans.size() > 4096) g_hplans.clear();
-            g_hplans[key] = plan;
+            if (!std::getenv("NB_PLAN")) g_hplans[key] = plan;       // a forced plan is not remembered
         }
     }
     Workspace* ws;
@@ -435,10 +436,12 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
         rc = ensure(&ws->hpartial, &ws->hpartial_bytes, (size_t)plan.S * (size_t)n_i * nb::kHermiteAcc * sizeof(double), stream);
         if (rc != NB_OK) return rc;
     }
-    nb::nb_pack_jv_kernel<<<(unsigned)((n_j + 255) / 256), 256, 0, stream>>>(x_j, v_j, m_j, (int)n_j,
-                                                                              reinterpret_cast<float4*>(ws->jp2));
-    NB_CUDA(cudaGetLastError());
-    ++t_launches;
+    if (!prepacked) {
+        nb::nb_pack_jv_kernel<<<(unsigned)((n_j + 255) / 256), 256, 0, stream>>>(x_j, v_j, m_j, (int)n_j,
+                                                                                  reinterpret_cast<float4*>(ws->jp2));
+        NB_CUDA(cudaGetLastError());
+        ++t_launches;
+    }
 
     nb::HermiteArgs args;
     args.x_i = x_i;
@@ -894,6 +897,11 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
     float* vp = reinterpret_cast<float*>(base + b3);
     float* a1 = reinterpret_cast<float*>(base + 2 * b3);
     float* j1 = reinterpret_cast<float*>(base + 3 * b3);
+    // the prediction writes the packed j records of the predicted state itself (one launch fewer per step)
+    rc = ensure(&ws->jp2, &ws->jp2_bytes, (size_t)n * 2 * sizeof(float4), stream);
+    if (rc != NB_OK) return rc;
+    float4* jp2 = reinterpret_cast<float4*>(ws->jp2);
+    const int pblocks = (int)((n + threads - 1) / threads);
     // As in nb_leapfrog_kdk: on small systems the host's enqueueing is the limit, so the identical middle steps
     // (predict, force + jerk without phi, correct) are captured once into a CUDA graph and replayed.
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
@@ -907,9 +915,9 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
             cudaGraph_t graph = nullptr;
             cudaGraphExec_t exec = nullptr;
             NB_CUDA(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
-            nb::nb_hermite_predict_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, xp, vp, n3, dt);
+            nb::nb_hermite_predict_pack_kernel<<<pblocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, m, xp, vp, jp2, (int)n, dt);
             t_launches = 0;
-            rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, nullptr, stream);
+            rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, nullptr, stream, true);
             const int64_t per_step = t_launches + 2;
             nb::nb_hermite_correct_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, a1, j1, n3, dt);
             cudaError_t ce = cudaStreamEndCapture(stream, &graph);
@@ -927,10 +935,10 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
             launches += per_step * replays;
             s += replays;                                              // the last step follows eagerly (it wants phi)
         }
-        nb::nb_hermite_predict_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, xp, vp, n3, dt);
+        nb::nb_hermite_predict_pack_kernel<<<pblocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, m, xp, vp, jp2, (int)n, dt);
         NB_CUDA(cudaGetLastError());
         t_launches = 0;
-        rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, s + 1 == n_steps ? pot_out : nullptr, stream);
+        rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, s + 1 == n_steps ? pot_out : nullptr, stream, true);
         if (rc != NB_OK) return rc;
         launches += t_launches + 2;
         nb::nb_hermite_correct_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, a1, j1, n3, dt);
