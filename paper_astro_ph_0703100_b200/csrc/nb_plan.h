@@ -21,7 +21,9 @@ constexpr int kMaxS = 2048;
 // Second pass over the S chunk partials of an i-tile: done inside the force kernel by the tile's last CTA when
 // the tile's partials are small (one launch fewer: C0 31 -> 24 us, C2 65 -> 38 us per call), else by a separate
 // nb_reduce_kernel launch (a 2048-particle tile with S = 18..30 would keep one CTA busy for ~10 us at the tail).
-constexpr int64_t kFusedReduceBytes = 1048576;
+// Measured per tile: 96 / 144 KB of partials: fused 1.4 / 3.2 us faster; 288 KB: tie; 512 / 576 KB: separate 3 .. 10 us
+// faster; 786 / 917 KB / 1.2 MB: separate 8 .. 15 us faster.
+constexpr int64_t kFusedReduceBytes = 327680;
 inline bool fused_second_pass(int tile_i, int S) { return S > 1 && (int64_t)tile_i * S * 32 <= kFusedReduceBytes; }
 
 struct Plan {
@@ -50,7 +52,7 @@ inline void ring_shape(int WJ, int* tile_j, int* stages) {
 inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, int WJ, int S,
                         double pair_inst = 13.0, double partial_bytes = 32.0) {
     const double c_fixed = 6000.0;                    // CTA start + first TMA round trip + epilogue
-    const double c_reduce_launch = 8000.0;            // second kernel
+    const double c_reduce_launch = 6000.0;            // second kernel
     const double pair_cycles = pair_inst / (128.0 * 0.84);
     const int tile_i = 32 * K * WI;
     const int64_t tiles_i = (n_i + tile_i - 1) / tile_i;
@@ -68,8 +70,9 @@ inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, i
     if (S > 1) {
         if (fused_second_pass(tile_i, S))
             cost += 1500.0 + 200.0 * S;               // the last CTA of a tile walks S partials
-        else {                                        // separate launch: ~5 TB/s at ~2 GHz, or the latency of S loads in a row
-            const double bw = double(n_i) * S * partial_bytes / 2500.0, lat = 200.0 * S;
+        else {                                        // separate launch: the partials are written and read back at ~5 TB/s
+                                                      // (~2 GHz), or the latency of S loads in a row
+            const double bw = double(n_i) * S * partial_bytes / 1250.0, lat = 200.0 * S;
             cost += c_reduce_launch + (bw > lat ? bw : lat);
         }
     }
