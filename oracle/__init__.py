@@ -60,6 +60,8 @@ def _load():
         lib.oracle_force_eps_i_f64.restype = ctypes.c_int
         lib.oracle_hermite4_f64.argtypes = [i64, p, p, p, f64, f64, i64, p, p, p]
         lib.oracle_hermite4_f64.restype = ctypes.c_int
+        lib.oracle_lj_f64.argtypes = [i64, p, i64, p, p]
+        lib.oracle_lj_f64.restype = ctypes.c_int
         lib.oracle_num_threads.restype = ctypes.c_int
         lib.oracle_set_num_threads.argtypes = [ctypes.c_int]
         _lib = lib
@@ -141,6 +143,18 @@ def force_eps_i(x_i: np.ndarray, eps2_i: np.ndarray, x_j: np.ndarray, m_j: np.nd
     if rc != 0:
         raise ValueError(f"oracle_force_eps_i returned {rc}")
     return acc, pot
+
+
+def lennard_jones(p_xi: np.ndarray, p_xj: np.ndarray) -> np.ndarray:
+    """Row f3, reading R19: 12-6 Lennard-Jones with Lorentz-Berthelot mixing, all pairs.  Rows
+    p_xi [n_i, 5] = (x, y, z, sigma_i / 2, sqrt(eps_i)), p_xj [n_j, 5] likewise (float32 or float64, promoted exactly
+    to double).  Returns p_fi [n_i, 4] = (Fx, Fy, Fz, U) in float64: the force ON i and the sum of its pair energies."""
+    xi, xj = _c(p_xi, np.float64).reshape(-1, 5), _c(p_xj, np.float64).reshape(-1, 5)
+    out = np.zeros((xi.shape[0], 4), dtype=np.float64)
+    rc = _load().oracle_lj_f64(xi.shape[0], _ptr(xi), xj.shape[0], _ptr(xj), _ptr(out))
+    if rc != 0:
+        raise ValueError(f"oracle_lj returned {rc}")
+    return out
 
 
 def force_batched(i_offsets: np.ndarray, j_offsets: np.ndarray, x_i: np.ndarray, x_j: np.ndarray, m_j: np.ndarray,

@@ -360,3 +360,49 @@ int oracle_hermite4_f64(int64_t n, double *x, double *v, const double *m, double
     free(xp); free(vp); free(a1); free(j1);
     return rc;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Row f3, a central force other than gravity: the paper lists "van der Waals molecular interactions" among the
+ * interactions its generalised library runs (section 4.5) and gives no formula; reading R19
+ * takes the textbook 12-6 Lennard-Jones pair with Lorentz-Berthelot mixing, all pairs, no cut-off:
+ *
+ *     i-record (x, y, z, sigma_i / 2, sqrt(eps_i))      j-record (x, y, z, sigma_j / 2, sqrt(eps_j))
+ *     sigma = sigma_i / 2 + sigma_j / 2       eps = sqrt(eps_i) sqrt(eps_j)       d = r_j - r_i      r2 = d . d
+ *     s6 = (sigma^2 / r2)^3
+ *     F_i = - sum_j 24 eps (2 s6^2 - s6) / r2 * d            (force ON i: repulsive inside r = 2^(1/6) sigma)
+ *     U_i =   sum_j  4 eps (s6^2 - s6)                       (pair energies seen by i; E_total = 1/2 sum_i U_i)
+ *
+ * A pair with d = 0 contributes nothing (reading R1).  Result record (Fx, Fy, Fz, U), plain double sums in j order.
+ * Pins (tests/test_oracle_pins.py, "lj"): zero force and U = -eps at r = 2^(1/6) sigma; U = 0 and |F| = 24 eps / sigma
+ * at r = sigma; exact rationals at r = 2 sigma; the mixing rule against a single-species pair; Newton's third law;
+ * F = -grad E_total by central differences; a pure-Python double loop.
+ */
+int oracle_lj_f64(int64_t n_i, const double *p_xi, int64_t n_j, const double *p_xj, double *p_fi)
+{
+    if (n_i < 0 || n_j < 0) return 1;
+    if (n_i > 0 && (!p_xi || !p_fi)) return 1;
+    if (n_j > 0 && !p_xj) return 1;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n_i; ++i) {
+        const double *I = &p_xi[5 * i];
+        double fx = 0.0, fy = 0.0, fz = 0.0, u = 0.0;
+        for (int64_t j = 0; j < n_j; ++j) {
+            const double *J = &p_xj[5 * j];
+            const double dx = J[0] - I[0], dy = J[1] - I[1], dz = J[2] - I[2];
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 == 0.0) continue;                                   /* coincident pair: nothing (R1) */
+            const double sigma = I[3] + J[3], eps = I[4] * J[4];
+            const double s2 = sigma * sigma / r2, s6 = s2 * s2 * s2;
+            const double f = 24.0 * eps * (2.0 * s6 * s6 - s6) / r2;
+            fx -= f * dx;
+            fy -= f * dy;
+            fz -= f * dz;
+            u += 4.0 * eps * (s6 * s6 - s6);
+        }
+        p_fi[4 * i + 0] = fx;
+        p_fi[4 * i + 1] = fy;
+        p_fi[4 * i + 2] = fz;
+        p_fi[4 * i + 3] = u;
+    }
+    return 0;
+}

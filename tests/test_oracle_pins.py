@@ -520,3 +520,90 @@ def test_p13_mass_linearity_and_superposition():
     perm = rng.permutation(40)                               # the order of the j-particles does not matter (to rounding)
     a3, p3 = oracle.force(xi, xj[perm], mj[perm], 0.02)
     np.testing.assert_allclose(a3, a, rtol=1e-13, atol=1e-15); np.testing.assert_allclose(p3, p, rtol=1e-13)
+
+
+# ----------------------------------------------------------------------------- lj (row f3, reading R19)
+def _lj_rows(x, sigma, eps):
+    x = np.asarray(x, dtype=np.float64).reshape(-1, 3)
+    n = x.shape[0]
+    return np.concatenate([x, np.broadcast_to(np.asarray(sigma, dtype=np.float64) / 2.0, (n,)).reshape(n, 1),
+                           np.sqrt(np.broadcast_to(np.asarray(eps, dtype=np.float64), (n,))).reshape(n, 1)], axis=1)
+
+
+def test_lj_two_body_closed_forms():
+    """12-6 Lennard-Jones, one pair on the x-axis: zero force and U = -eps at the minimum r = 2^(1/6) sigma; U = 0 and a
+    repulsion of 24 eps / sigma at r = sigma; at r = 2 sigma the exact rationals U = 4 eps (2^-12 - 2^-6) and
+    |F| = 24 eps (2^-6 - 2^-11) / (2 sigma), attractive.  The force is the one ON the i-particle."""
+    sigma, eps = 1.5, 0.7
+    i = _lj_rows([[0.0, 0.0, 0.0]], sigma, eps)
+    for r, f_expect, u_expect in (
+            (2.0 ** (1.0 / 6.0) * sigma, 0.0, -eps),
+            (sigma, -24.0 * eps / sigma, 0.0),                                  # pushed away from j: toward -x
+            (2.0 * sigma, float(Fraction(24) * Fraction(7, 10) * (Fraction(1, 64) - Fraction(2, 4096)) / 3), None)):
+        out = oracle.lennard_jones(i, _lj_rows([[r, 0.0, 0.0]], sigma, eps))
+        assert abs(out[0, 0] - f_expect) <= 1e-13 * max(1.0, abs(f_expect)), (r, out)
+        assert out[0, 1] == 0.0 and out[0, 2] == 0.0
+        if u_expect is not None:
+            assert abs(out[0, 3] - u_expect) <= 1e-14
+    u2 = oracle.lennard_jones(i, _lj_rows([[0.0, 0.0, -2.0 * sigma]], sigma, eps))
+    assert abs(u2[0, 3] - 4 * eps * (2.0 ** -12 - 2.0 ** -6)) <= 1e-16
+    assert u2[0, 2] < 0.0 and u2[0, 0] == 0.0                                   # attracted toward j at -z
+
+
+def test_lj_mixing_rule_third_law_and_coincident_pairs():
+    rng = np.random.default_rng(31)
+    n = 40
+    x = rng.uniform(0.0, 6.0, (n, 3))
+    sig = rng.uniform(0.8, 1.2, n); eps = rng.uniform(0.5, 2.0, n)
+    rows = _lj_rows(x, sig, eps)
+    out = oracle.lennard_jones(rows, rows)                                     # the self pair adds nothing (R1)
+    assert np.all(np.isfinite(out))
+    # Lorentz-Berthelot: the pair (a, b) is a single-species pair with sigma = (sig_a + sig_b) / 2, eps = sqrt(eps_a eps_b)
+    a, b = 3, 17
+    pair = oracle.lennard_jones(rows[a:a + 1], rows[b:b + 1])
+    s, e = 0.5 * (sig[a] + sig[b]), math.sqrt(eps[a] * eps[b])
+    same = oracle.lennard_jones(_lj_rows(x[a], s, e), _lj_rows(x[b], s, e))
+    np.testing.assert_allclose(pair, same, rtol=1e-14)
+    # Newton's third law: the forces of a closed system sum to zero; U is symmetric, so sum_i U_i = 2 E_total
+    scale = np.abs(out[:, :3]).sum()
+    assert np.abs(out[:, :3].sum(axis=0)).max() <= 1e-13 * scale
+    # a duplicate of particle 0 elsewhere in the j-list: skipped for i = 0, felt by everybody else
+    rows2 = np.concatenate([rows, rows[:1]])
+    out2 = oracle.lennard_jones(rows, rows2)
+    np.testing.assert_array_equal(out2[0], out[0])
+    assert np.all(out2[1:, 3] != out[1:, 3])
+
+
+def test_lj_force_is_minus_gradient_of_total_energy_and_python_loop():
+    rng = np.random.default_rng(32)
+    n = 12
+    g = np.stack(np.meshgrid(*[np.arange(3.0)] * 3, indexing="ij"), -1).reshape(-1, 3)[:n] * 1.3
+    x = g + rng.uniform(-0.1, 0.1, (n, 3))
+    sig = rng.uniform(0.9, 1.1, n); eps = rng.uniform(0.5, 1.5, n)
+
+    def energy(xx):
+        r = _lj_rows(xx, sig, eps)
+        return 0.5 * oracle.lennard_jones(r, r)[:, 3].sum()
+
+    out = oracle.lennard_jones(_lj_rows(x, sig, eps), _lj_rows(x, sig, eps))
+    h = 1e-5
+    for i in (0, 5, 11):
+        for c in range(3):
+            xp, xm = x.copy(), x.copy()
+            xp[i, c] += h; xm[i, c] -= h
+            np.testing.assert_allclose(out[i, c], -(energy(xp) - energy(xm)) / (2 * h), rtol=2e-7, atol=1e-8)
+    # the definition written out as a pure-Python double loop (F on i points from j to i when repulsive)
+    for i in range(n):
+        f = [0.0, 0.0, 0.0]; u = 0.0
+        for j in range(n):
+            if j == i:
+                continue
+            d = [x[i][c] - x[j][c] for c in range(3)]
+            r = math.sqrt(sum(v * v for v in d))
+            s = 0.5 * (sig[i] + sig[j]); e = math.sqrt(eps[i] * eps[j])
+            dudr = 4 * e * (-12 * s ** 12 / r ** 13 + 6 * s ** 6 / r ** 7)
+            for c in range(3):
+                f[c] += -dudr * d[c] / r
+            u += 4 * e * ((s / r) ** 12 - (s / r) ** 6)
+        np.testing.assert_allclose(out[i, :3], f, rtol=1e-11, atol=1e-12)
+        assert abs(out[i, 3] - u) <= 1e-12 * max(1.0, abs(u))
