@@ -185,6 +185,22 @@ int nb_cunbody_force(const float *p_xj, const float *p_xi, float *p_fi, int64_t 
 int nb_cunbody_force_jerk_pot(const float *p_xj, const float *p_xi, float *p_fi, int64_t ni, int64_t nj, void *stream);
 
 /*
+ * nb_cunbody_lennard_jones -- the same cunbody_api call for a central force other than gravity: the paper lists
+ * "van der Waals molecular interactions" among the interactions of its generalised library (section 4.5,
+ * PAPER.md:363) without a formula; reading R19 takes the 12-6 Lennard-Jones pair with Lorentz-Berthelot
+ * mixing, all pairs, no cut-off, with d = r_j - r_i, r2 = d.d, sigma = sigma_i/2 + sigma_j/2,
+ * eps = sqrt(eps_i) sqrt(eps_j), s6 = (sigma^2 / r2)^3:
+ *
+ *     F_i = - sum_j 24 eps (2 s6^2 - s6) / r2 * d          U_i = sum_j 4 eps (s6^2 - s6)
+ *
+ *        p_xj [nj][5] = (x, y, z, sigma_j / 2, sqrt(eps_j))       p_xi [ni][5] likewise       p_fi [ni][4] = (Fx, Fy, Fz, U)
+ *
+ * F_i is the force ON particle i; the total energy of a closed system is 1/2 sum_i U_i.  DEVICE float rows, p_fi
+ * overwritten, coincident pairs add nothing, errors as for nb_cunbody_force.
+ */
+int nb_cunbody_lennard_jones(const float *p_xj, const float *p_xi, float *p_fi, int64_t ni, int64_t nj, void *stream);
+
+/*
  * nb_force_batched -- many independent small (i-set, j-set) sub-problems of nb_force in ONE launch:
  * the use the paper shapes its interface for, a host tree code calling the force routine on
  * interaction lists of "several thousands" particles per group (PAPER.md:246 last sentence, section

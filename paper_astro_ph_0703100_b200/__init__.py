@@ -7,6 +7,7 @@ from .binding import (  # noqa: F401
     NBError,
     cunbody_force,
     cunbody_force_jerk_pot,
+    cunbody_lennard_jones,
     force,
     force_batched,
     force_eps_i,

@@ -45,7 +45,7 @@ def lib() -> ctypes.CDLL:
         l.nb_leapfrog_kdk.restype = ci
         l.nb_force_jerk.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p, p]
         l.nb_force_jerk.restype = ci
-        for fn in (l.nb_cunbody_force, l.nb_cunbody_force_jerk_pot):
+        for fn in (l.nb_cunbody_force, l.nb_cunbody_force_jerk_pot, l.nb_cunbody_lennard_jones):
             fn.argtypes = [p, p, p, i64, i64, p]
             fn.restype = ci
         l.nb_pack_j.argtypes = [i64, p, p, p, p]
@@ -167,6 +167,12 @@ def cunbody_force(p_xj, p_xi, p_fi=None, stream=None):
 def cunbody_force_jerk_pot(p_xj, p_xi, p_fi=None, stream=None):
     """nb_cunbody_force_jerk_pot: the Fig. A.4 pipeline.  p_xj [nj,7], p_xi [ni,6] -> p_fi [ni,7]."""
     return _cunbody("nb_cunbody_force_jerk_pot", p_xj, p_xi, 6, 7, 7, p_fi, stream)
+
+
+def cunbody_lennard_jones(p_xj, p_xi, p_fi=None, stream=None):
+    """nb_cunbody_lennard_jones: 12-6 Lennard-Jones with Lorentz-Berthelot mixing.  p_xj [nj,5], p_xi [ni,5] =
+    (x, y, z, sigma/2, sqrt(eps)) -> p_fi [ni,4] = (Fx, Fy, Fz, U)."""
+    return _cunbody("nb_cunbody_lennard_jones", p_xj, p_xi, 5, 5, 4, p_fi, stream)
 
 
 def pack_j(x_j, m_j, xm_out, stream=None):

@@ -1,5 +1,5 @@
-// nb_pipelines.cuh -- the paper's two pipeline descriptions, statement by statement, as pipelines of the
-// generalised kernel (include/nb_pipeline.cuh).  The only addition to the listings is the coincident-pair rule
+// nb_pipelines.cuh -- the paper's two pipeline descriptions, statement by statement, and a Lennard-Jones pipeline, as
+// pipelines of the generalised kernel (include/nb_pipeline.cuh).  The only addition to the listings is the coincident-pair rule
 // (reading R1): a pair whose three position differences are exactly zero adds nothing.
 #pragma once
 #include "../../include/nb_pipeline.cuh"
@@ -55,6 +55,27 @@ struct PipelineForceJerkPotA4 {
         OUTPUT[4] += mf * dv_1 - mf3a * dx_1;
         OUTPUT[5] += mf * dv_2 - mf3a * dx_2;
         OUTPUT[6] -= pot;
+    }
+};
+
+// A central force other than gravity (section 4.5: "van der Waals molecular interactions"; no formula in
+// the paper -- DESIGN.md reading R19): 12-6 Lennard-Jones with Lorentz-Berthelot mixing, all pairs, no cut-off.
+// IDIM 5 = (x, y, z, sigma_i / 2, sqrt(eps_i)), JDIM 5 likewise, FDIM 4 = (Fx, Fy, Fz, U): force ON i, pair energies of i.
+struct PipelineLennardJones {
+    static constexpr int IDIM = 5, JDIM = 5, FDIM = 4;
+    static __device__ __forceinline__ void pair(const float* INPUT_I, const float* INPUT_J, float* OUTPUT) {
+        const float dx = INPUT_J[0] - INPUT_I[0], dy = INPUT_J[1] - INPUT_I[1], dz = INPUT_J[2] - INPUT_I[2];
+        const float r2 = dx * dx + dy * dy + dz * dz;
+        const float r1i = (r2 == 0.0f) ? 0.0f : pipeline_rsqrt(r2);    // reading R1, branch-free: r1i = 0 => the pair adds 0
+        const float r2i = r1i * r1i;
+        const float sigma = INPUT_I[3] + INPUT_J[3], eps = INPUT_I[4] * INPUT_J[4];         // Lorentz-Berthelot
+        const float s2 = sigma * sigma * r2i, s6 = s2 * s2 * s2;
+        const float es6 = eps * s6;
+        const float f = 24.0f * es6 * (2.0f * s6 - 1.0f) * r2i;        // 24 eps (2 s^12 - s^6) / r^2
+        OUTPUT[0] -= f * dx;
+        OUTPUT[1] -= f * dy;
+        OUTPUT[2] -= f * dz;
+        OUTPUT[3] += 4.0f * es6 * (s6 - 1.0f);                         // 4 eps (s^12 - s^6)
     }
 };
 

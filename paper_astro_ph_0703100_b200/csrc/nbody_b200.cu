@@ -715,6 +715,10 @@ int nb_cunbody_force_jerk_pot(const float* p_xj, const float* p_xi, float* p_fi,
     return cunbody_call<nb::PipelineForceJerkPotA4>(p_xj, p_xi, p_fi, ni, nj, reinterpret_cast<cudaStream_t>(stream));
 }
 
+int nb_cunbody_lennard_jones(const float* p_xj, const float* p_xi, float* p_fi, int64_t ni, int64_t nj, void* stream) {
+    return cunbody_call<nb::PipelineLennardJones>(p_xj, p_xi, p_fi, ni, nj, reinterpret_cast<cudaStream_t>(stream));
+}
+
 int nb_pack_j(int64_t n_j, const float* x_j, const float* m_j, float* xm_out, void* stream) {
     t_launches = 0;
     if (bad_count(n_j)) return NB_ERR_INVALID_VALUE;

@@ -248,3 +248,19 @@ def tree_list_workload(n_particles: int, group_min: int, group_max: int, list_mi
                            m_j=_f32(np.concatenate(mj_parts)), eps2=float(np.float32(eps * eps)), seed=seed,
                            meta={"model": "plummer a=1 truncated at 10a, grid-sorted groups with own + near + cell lists",
                                  "eps": eps, "groups": len(sizes)})
+
+
+def lj_fluid_rows(n: int, density: float, jitter: float, seed: int) -> np.ndarray:
+    """Row f3 (Lennard-Jones pipeline): n particles on a jittered simple-cubic lattice of number density ``density``
+    (reduced units, sigma ~ 1) -- a dense fluid without overlaps -- with per-particle sigma in [0.9, 1.1] and eps in
+    [0.5, 1.5].  Returns float32 rows [n, 5] = (x, y, z, sigma / 2, sqrt(eps)), the record format of
+    nb_cunbody_lennard_jones.  ``jitter`` is the maximum displacement in units of the lattice spacing."""
+    rng = _rng(seed)
+    side = int(np.ceil(n ** (1.0 / 3.0)))
+    a = density ** (-1.0 / 3.0)
+    g = np.stack(np.meshgrid(*[np.arange(side, dtype=np.float64)] * 3, indexing="ij"), -1).reshape(-1, 3)
+    pick = rng.permutation(g.shape[0])[:n]
+    x = (g[pick] + rng.uniform(-jitter, jitter, (n, 3))) * a
+    sigma = rng.uniform(0.9, 1.1, n)
+    eps = rng.uniform(0.5, 1.5, n)
+    return _f32(np.concatenate([x, 0.5 * sigma[:, None], np.sqrt(eps)[:, None]], axis=1))

@@ -65,6 +65,8 @@ def test_argument_validation_happens_before_any_cuda_call():
     assert lib.nb_pack_j(1, p, None, p, None) == 1
     assert lib.nb_cunbody_force(p, None, p, 1, 1, None) == 1
     assert lib.nb_cunbody_force_jerk_pot(None, p, p, 1, 1, None) == 1
+    assert lib.nb_cunbody_lennard_jones(None, p, p, 1, 1, None) == 1
+    assert lib.nb_cunbody_lennard_jones(p, p, p, -1, 1, None) == 1
     assert lib.nb_plan_query_jerk(5, -5, 148, out) == 1
 
 

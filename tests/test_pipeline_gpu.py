@@ -83,3 +83,64 @@ def test_agrees_with_the_specialised_kernels_and_edge_sizes(nb):
     assert out.shape == (5000, 3) and not out.any()
     assert nb.cunbody_force(dev(p_xj), z).shape == (0, 3)                       # ni = 0
     assert nb.lib().nb_cunbody_force(None, None, None, 5, 5, None) == 1
+
+
+# ------------------------------------------------------------------ a central force other than gravity (reading R19)
+def _lj_scales(rows_i, rows_j):
+    """sum_j |f_ij| |d| and sum_j |u_ij| per i, in double: what the FP32 rounding errors of the pairs are relative to."""
+    xi, xj = rows_i.astype(np.float64), rows_j.astype(np.float64)
+    fs, us = np.zeros(xi.shape[0]), np.zeros(xi.shape[0])
+    for lo in range(0, xi.shape[0], 256):
+        I = xi[lo:lo + 256]
+        d = xj[None, :, :3] - I[:, None, :3]
+        r2 = (d * d).sum(-1)
+        ok = r2 > 0
+        r2 = np.where(ok, r2, 1.0)
+        s6 = ((I[:, None, 3] + xj[None, :, 3]) ** 2 / r2) ** 3
+        e = I[:, None, 4] * xj[None, :, 4]
+        fs[lo:lo + 256] = np.where(ok, 24 * e * (2 * s6 * s6 + s6) / np.sqrt(r2), 0.0).sum(1)
+        us[lo:lo + 256] = np.where(ok, 4 * e * (s6 * s6 + s6), 0.0).sum(1)
+    return fs, us
+
+
+@pytest.mark.parametrize("n_i,n_j", [(1, 1), (700, 3001), (2500, 2500), (257, 20000)])
+def test_lennard_jones_pipeline_matches_oracle(nb, n_i, n_j):
+    """nb_cunbody_lennard_jones against the double-precision oracle on a dense fluid (jittered lattice, density 0.8,
+    mixed sigma and eps).  Tolerance: every pair carries the rsqrt.approx error (2^-22) six times in s^12 plus ~10 FP32
+    roundings, < 4e-6 of its own magnitude; block partials are FP32 over <= 256 j, totals FP64 -- so
+    |F - F_ref| <= 1e-5 sum_j |f_ij| and |U - U_ref| <= 1e-5 sum_j |u_ij| (measured: 1e-6)."""
+    import torch
+    rows = wl.lj_fluid_rows(max(n_i, n_j), 0.8, 0.1, seed=41)
+    rows_j = rows[:n_j]
+    rows_i = rows[:n_i] if n_i <= n_j else rows
+    if n_i == 257:
+        rows_i = rows[::-1][:n_i].copy()                              # a subset from the other end of the list
+    out = nb.cunbody_lennard_jones(dev(rows_j), dev(rows_i))
+    torch.cuda.synchronize()
+    out = out.cpu().numpy().astype(np.float64)
+    ref = oracle.lennard_jones(rows_i, rows_j)
+    if n_j == 1:
+        assert not out.any() and not ref.any()                        # the only pair is the particle with itself
+        return
+    fs, us = _lj_scales(rows_i, rows_j)
+    assert np.all(np.isfinite(out))
+    assert (np.linalg.norm(out[:, :3] - ref[:, :3], axis=1) / fs).max() <= 1e-5
+    assert (np.abs(out[:, 3] - ref[:, 3]) / us).max() <= 1e-5
+    if n_i == n_j:                                                    # closed system: the forces sum to zero up to the
+        # accumulated rounding of n_i independent results
+        assert np.abs(out[:, :3].sum(0)).max() <= 1e-5 * fs.mean() * np.sqrt(n_i)
+
+
+def test_lennard_jones_pipeline_edge_cases(nb):
+    import torch
+    rows = wl.lj_fluid_rows(100, 0.8, 0.1, seed=42)
+    empty = torch.empty((0, 5), dtype=torch.float32, device="cuda")
+    out = nb.cunbody_lennard_jones(empty, dev(rows))                  # no j-particles: zeros
+    assert out.shape == (100, 4) and not out.cpu().numpy().any()
+    out = nb.cunbody_lennard_jones(dev(rows), empty)                  # no i-particles: nothing to do
+    assert out.shape == (0, 4)
+    # two particles at the potential minimum: no force, U = -eps for both
+    sigma, eps = 1.0, 2.0
+    pair = np.array([[0, 0, 0, sigma / 2, np.sqrt(eps)], [2 ** (1 / 6) * sigma, 0, 0, sigma / 2, np.sqrt(eps)]], np.float32)
+    out = nb.cunbody_lennard_jones(dev(pair), dev(pair)).cpu().numpy()
+    assert np.abs(out[:, :3]).max() <= 2e-5 * 24 * eps / sigma and np.abs(out[:, 3] + eps).max() <= 1e-5 * eps
