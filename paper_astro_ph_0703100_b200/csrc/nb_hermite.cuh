@@ -50,6 +50,7 @@ struct HermiteArgs {
     float* jerk;           // [n_i][3]
     float* pot;            // [n_i] or nullptr
     double* partial;       // [S][n_i][10] when S > 1
+    int* tickets;          // [tiles_i] zeroed counters: the last CTA of an i-tile makes the second pass; nullptr: separate launch
     const int* coin_lists;
     const int* coin_flag;
     int n_i;
@@ -272,22 +273,23 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
 #pragma unroll
             for (int c = 0; c < kHermiteAcc; ++c) red[((wj * K + k) * kHermiteAcc + c) * (WI * 32) + tig] = run[k][c];
         __syncthreads();
-        if (wj != 0) return;
+        if (wj == 0) {
 #pragma unroll
-        for (int k = 0; k < K; ++k)
+            for (int k = 0; k < K; ++k)
 #pragma unroll
-            for (int c = 0; c < kHermiteAcc; ++c) {
-                double s = red[((0 * K + k) * kHermiteAcc + c) * (WI * 32) + tig];
+                for (int c = 0; c < kHermiteAcc; ++c) {
+                    double s = red[((0 * K + k) * kHermiteAcc + c) * (WI * 32) + tig];
 #pragma unroll
-                for (int w = 1; w < WJ; ++w) s += red[((w * K + k) * kHermiteAcc + c) * (WI * 32) + tig];
-                run[k][c] = s;
-            }
+                    for (int w = 1; w < WJ; ++w) s += red[((w * K + k) * kHermiteAcc + c) * (WI * 32) + tig];
+                    run[k][c] = s;
+                }
+        }
     }
 
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const int i = i_base + k * 32;
-        if (i >= a.n_i) continue;
+        if (i >= a.n_i || wj != 0) continue;
         if (a.S == 1) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
@@ -299,6 +301,43 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
             double* dst = a.partial + ((size_t)blockIdx.y * a.n_i + i) * kHermiteAcc;
 #pragma unroll
             for (int c = 0; c < kHermiteAcc; c += 2) *reinterpret_cast<double2*>(dst + c) = make_double2(run[k][c], run[k][c + 1]);
+        }
+    }
+
+    // second pass, fused (as in nb_force_kernel): the CTA that finishes LAST among the S chunks of this i-tile sums the
+    // S partials in the fixed order s = 0 .. S-1 -- the sum nb_hermite_reduce_kernel makes, bit for bit -- and writes
+    // a, jerk and phi; the tile's ticket counter returns to zero for the next call.
+    if (a.S > 1 && a.tickets != nullptr) {
+        __shared__ int s_last;
+        __threadfence();                                               // partials visible device-wide before the ticket
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const int ticket = atomicAdd(a.tickets + blockIdx.x, 1);
+            s_last = (ticket == a.S - 1);
+            if (s_last) a.tickets[blockIdx.x] = 0;
+        }
+        __syncthreads();
+        if (!s_last) return;
+        __threadfence();
+        const int tile0 = blockIdx.x * (32 * K * WI);
+        const int tile_n = min(32 * K * WI, a.n_i - tile0);
+        for (int q = threadIdx.x; q < tile_n; q += 32 * WI * WJ) {
+            const int i = tile0 + q;
+            double s[kHermiteAcc];
+            const double2* p2 = reinterpret_cast<const double2*>(a.partial + (size_t)i * kHermiteAcc);   // L2 reads
+#pragma unroll
+            for (int c = 0; c < kHermiteAcc; c += 2) { const double2 t = __ldcg(p2 + c / 2); s[c] = t.x; s[c + 1] = t.y; }
+            for (int ch = 1; ch < a.S; ++ch) {
+                p2 = reinterpret_cast<const double2*>(a.partial + ((size_t)ch * a.n_i + i) * kHermiteAcc);
+#pragma unroll
+                for (int c = 0; c < kHermiteAcc; c += 2) { const double2 t = __ldcg(p2 + c / 2); s[c] += t.x; s[c + 1] += t.y; }
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                a.acc[3 * (size_t)i + c] = (float)s[c];
+                a.jerk[3 * (size_t)i + c] = (float)(s[3 + c] - 3.0 * s[6 + c]);
+            }
+            if (a.pot) a.pot[i] = -(float)s[9];
         }
     }
 }

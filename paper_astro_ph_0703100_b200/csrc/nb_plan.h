@@ -24,7 +24,9 @@ constexpr int kMaxS = 2048;
 // Measured per tile: 96 / 144 KB of partials: fused 1.4 / 3.2 us faster; 288 KB: tie; 512 / 576 KB: separate 3 .. 10 us
 // faster; 786 / 917 KB / 1.2 MB: separate 8 .. 15 us faster.
 constexpr int64_t kFusedReduceBytes = 327680;
-inline bool fused_second_pass(int tile_i, int S) { return S > 1 && (int64_t)tile_i * S * 32 <= kFusedReduceBytes; }
+inline bool fused_second_pass(int tile_i, int S, double partial_bytes = 32.0) {
+    return S > 1 && (double)tile_i * S * partial_bytes <= (double)kFusedReduceBytes;
+}
 
 struct Plan {
     int K;            // i-particles per thread (2, 4 or 8; held as K/2 packed pairs)
@@ -68,7 +70,7 @@ inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, i
     if (WJ > 1) cta_cycles += 1500.0;                 // cross-warp reduction through shared memory
     double cost = waves * cta_cycles;
     if (S > 1) {
-        if (fused_second_pass(tile_i, S))
+        if (fused_second_pass(tile_i, S, partial_bytes))
             cost += 1500.0 + 200.0 * S;               // the last CTA of a tile walks S partials
         else {                                        // separate launch: the partials are written and read back at ~5 TB/s
                                                       // (~2 GHz), or the latency of S loads in a row

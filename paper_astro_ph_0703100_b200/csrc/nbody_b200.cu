@@ -432,9 +432,17 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     }
     rc = ensure(&ws->jp2, &ws->jp2_bytes, (size_t)n_j * 2 * sizeof(float4), stream);
     if (rc != NB_OK) return rc;
+    // second pass: fused into the kernel (small tiles) or a separate launch, as for nb_force; NB_FUSED_REDUCE=0/1 forces
+    const char* fr = std::getenv("NB_FUSED_REDUCE");
+    const bool fused_reduce = plan.S > 1 && (fr ? (fr[0] != '0') : nb::fused_second_pass(plan.tile_i, plan.S, kHermitePartialBytes));
     if (plan.S > 1) {
         rc = ensure(&ws->hpartial, &ws->hpartial_bytes, (size_t)plan.S * (size_t)n_i * nb::kHermiteAcc * sizeof(double), stream);
         if (rc != NB_OK) return rc;
+        if (fused_reduce && (size_t)plan.tiles_i * sizeof(int) > ws->tickets_bytes) {
+            rc = ensure(&ws->tickets, &ws->tickets_bytes, (size_t)plan.tiles_i * sizeof(int), stream);
+            if (rc != NB_OK) return rc;
+            NB_CUDA(cudaMemsetAsync(ws->tickets, 0, ws->tickets_bytes, stream));   // once per growth; kernels leave zeros
+        }
     }
     if (!prepacked) {
         nb::nb_pack_jv_kernel<<<(unsigned)((n_j + 255) / 256), 256, 0, stream>>>(x_j, v_j, m_j, (int)n_j,
@@ -451,6 +459,7 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     args.jerk = jerk_out;
     args.pot = pot_out;
     args.partial = reinterpret_cast<double*>(ws->hpartial);
+    args.tickets = fused_reduce ? reinterpret_cast<int*>(ws->tickets) : nullptr;
     args.coin_lists = nullptr;
     args.coin_flag = nullptr;
     args.n_i = (int)n_i;
@@ -469,7 +478,7 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
         rc = launch_hermite<nb::MODE_EXACT>(args, plan, stream);
     }
     if (rc != NB_OK) return rc;
-    if (plan.S > 1) {
+    if (plan.S > 1 && !fused_reduce) {
         nb::nb_hermite_reduce_kernel<<<(unsigned)((n_i + 127) / 128), 128, 0, stream>>>(
             reinterpret_cast<const double*>(ws->hpartial), (int)n_i, plan.S, acc_out, jerk_out, pot_out);
         NB_CUDA(cudaGetLastError());

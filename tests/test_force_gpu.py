@@ -538,3 +538,23 @@ def test_bloom_mode_lattice_duplicates_and_eps_threshold(nb, n, monkeypatch):
     # lattice forces cancel by symmetry in the interior: compare a absolutely against the typical magnitude
     scale = np.sqrt((ref_acc.astype(np.float64) ** 2).sum(1)).max()
     assert np.abs(out["bloom"][0] - ref_acc).max() <= 1e-5 * scale
+
+
+@pytest.mark.parametrize("plan", [(8, 8, 1, 5), (4, 2, 4, 3), (2, 1, 8, 7), (8, 4, 2, 2)], ids=lambda p: "K%d_WI%d_WJ%d_S%d" % p)
+def test_fused_second_pass_is_bitwise_the_separate_reduce(nb, plan, monkeypatch):
+    """The sum over the S chunk partials is made in the order s = 0 .. S-1 whoever makes it: the last CTA of an
+    i-tile inside the force kernel (ticket counter) or nb_reduce_kernel.  Same bits; repeated calls find the ticket
+    counters back at zero."""
+    monkeypatch.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
+    w = wl.plummer_workload(5000, 1.0 / 64, seed=17)
+    out = {}
+    for fused in ("1", "0"):
+        monkeypatch.setenv("NB_FUSED_REDUCE", fused)
+        runs = [gpu_force(nb, w.x_j, w.x_j, w.m_j, w.eps2, alias=True) for _ in range(3)]
+        for r in runs[1:]:
+            assert np.array_equal(r[0], runs[0][0]) and np.array_equal(r[1], runs[0][1])
+        out[fused] = runs[0] + (nb.last_launch_count(),)
+    assert np.array_equal(out["1"][0], out["0"][0]) and np.array_equal(out["1"][1], out["0"][1])
+    assert out["0"][2] == out["1"][2] + 1                              # one launch fewer
+    ref_acc, ref_pot = oracle.force(w.x_j, w.x_j, w.m_j, w.eps2)
+    check_parity(out["1"][0], out["1"][1], ref_acc, ref_pot, "fused " + str(plan))

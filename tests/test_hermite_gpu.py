@@ -202,3 +202,22 @@ def test_force_jerk_host_matches_device_path(nb):
     ra, rj, _ = oracle.force_jerk(xi, vi, x, v, m, eps2)
     assert p_h is None
     check(a_h, j_h, None, ra, rj, None, "host subset")
+
+
+@pytest.mark.parametrize("plan", [(4, 8, 1, 5), (4, 2, 4, 3), (2, 1, 8, 7), (2, 4, 2, 2)], ids=lambda p: "K%d_WI%d_WJ%d_S%d" % p)
+def test_fused_second_pass_is_bitwise_the_separate_reduce(nb, plan, monkeypatch):
+    """nb_force_jerk: the last CTA of an i-tile sums the S chunk partials in the order nb_hermite_reduce_kernel does;
+    same bits, one launch fewer, ticket counters back at zero after every call."""
+    monkeypatch.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
+    x, v, m, eps2 = plummer_xv(4000, 1.0 / 64, 19)
+    out = {}
+    for fused in ("1", "0"):
+        monkeypatch.setenv("NB_FUSED_REDUCE", fused)
+        runs = [gpu_fj(nb, x, v, x, v, m, eps2, alias=True) for _ in range(3)]
+        for r in runs[1:]:
+            assert all(np.array_equal(a, b) for a, b in zip(r, runs[0]))
+        out[fused] = runs[0] + (nb.last_launch_count(),)
+    assert all(np.array_equal(a, b) for a, b in zip(out["1"][:3], out["0"][:3]))
+    assert out["0"][3] == out["1"][3] + 1
+    ra, rj, rp = oracle.force_jerk(x, v, x, v, m, eps2)
+    check(out["1"][0], out["1"][1], out["1"][2], ra, rj, rp, "fused " + str(plan))
