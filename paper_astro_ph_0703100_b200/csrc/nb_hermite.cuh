@@ -130,6 +130,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
     static_assert(K % 2 == 0, "i-particles are held in pairs");
     static_assert(SUB == kCoinSeg, "coincidence segments are SUB j-particles");
     static_assert(MODE == MODE_EXACT || MODE == MODE_BLOOM || MODE == MODE_LIST, "masked everywhere, Bloom filter, or coincidence lists");
+    constexpr bool FUSED = (MODE == MODE_EXACT);                       // can make the second pass itself (a.tickets)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int REC = 32;
     constexpr int RING_BYTES = STAGES * TJ * REC;
@@ -273,6 +274,7 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
 #pragma unroll
             for (int c = 0; c < kHermiteAcc; ++c) red[((wj * K + k) * kHermiteAcc + c) * (WI * 32) + tig] = run[k][c];
         __syncthreads();
+        if (!FUSED && wj != 0) return;
         if (wj == 0) {
 #pragma unroll
             for (int k = 0; k < K; ++k)
@@ -304,10 +306,11 @@ __global__ void __launch_bounds__(32 * WI * WJ, 1) nb_hermite_kernel(const Hermi
         }
     }
 
-    // second pass, fused (as in nb_force_kernel): the CTA that finishes LAST among the S chunks of this i-tile sums the
+    // second pass, fused (as in nb_force_kernel; MODE_EXACT instantiations only -- the small calls, where a launch
+    // matters; the large-call kernels carry none of this): the CTA that finishes LAST among the S chunks of this i-tile sums the
     // S partials in the fixed order s = 0 .. S-1 -- the sum nb_hermite_reduce_kernel makes, bit for bit -- and writes
     // a, jerk and phi; the tile's ticket counter returns to zero for the next call.
-    if (a.S > 1 && a.tickets != nullptr) {
+    if (FUSED && a.S > 1 && a.tickets != nullptr) {
         __shared__ int s_last;
         __threadfence();                                               // partials visible device-wide before the ticket
         __syncthreads();

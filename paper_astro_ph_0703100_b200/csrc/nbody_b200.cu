@@ -434,7 +434,9 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     if (rc != NB_OK) return rc;
     // second pass: fused into the kernel (small tiles) or a separate launch, as for nb_force; NB_FUSED_REDUCE=0/1 forces
     const char* fr = std::getenv("NB_FUSED_REDUCE");
-    const bool fused_reduce = plan.S > 1 && (fr ? (fr[0] != '0') : nb::fused_second_pass(plan.tile_i, plan.S, kHermitePartialBytes));
+    const int mode = pick_mode(n_i, n_j, eps2, true, kListMinPairsJerk);
+    const bool fused_reduce = plan.S > 1 && mode == nb::MODE_EXACT &&      // only the masked (small-call) kernels carry the ticket code
+                              (fr ? (fr[0] != '0') : nb::fused_second_pass(plan.tile_i, plan.S, kHermitePartialBytes));
     if (plan.S > 1) {
         rc = ensure(&ws->hpartial, &ws->hpartial_bytes, (size_t)plan.S * (size_t)n_i * nb::kHermiteAcc * sizeof(double), stream);
         if (rc != NB_OK) return rc;
@@ -467,7 +469,6 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     args.S = plan.S;
     args.eps2 = eps2;
     // small calls mask every pair, mid-size ones test every block against a Bloom filter, large ones use the coincidence lists
-    const int mode = pick_mode(n_i, n_j, eps2, true, kListMinPairsJerk);
     if (mode == nb::MODE_LIST) {
         rc = coin_prepass(ws, plan, n_i, x_i, n_j, args.jp, 2, stream, &args.coin_lists, &args.coin_flag);
         if (rc != NB_OK) return rc;
