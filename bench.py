@@ -160,6 +160,9 @@ def reference_arm(args, wl):
     elif args.op == "cunbody":
         w = wl.config(1)
         name = "row f3 (G1): configs[1]'s particles, Fig. A.3 pipeline (oracle force on a sample)"
+    elif args.op == "lj":
+        w = LJ_ROWS(wl)
+        name = "row f3 (L1): Lennard-Jones fluid, 131072 particles (oracle lennard_jones on a sample)"
     elif args.op == "hermite":
         w = wl.plummer_workload(65536, 1.0 / 128, seed=4, name="C4", with_velocities=True)
         name = "C4's particles, force+jerk evaluations of the Hermite integration (oracle force_jerk on a sample)"
@@ -215,7 +218,15 @@ OPS = {
     "cunbody": {"inst": 12, "kernel": "pipeline_kernel<PipelineForceA3> (generalised kernel, row f3)", "flops": (20, 38)},
     "leapfrog": {"inst": 12, "kernel": "nb_force_kernel<PHI=false> inside nb_leapfrog_kdk (row a8)", "flops": (20, 38)},
 }
+# row f3, a central force other than gravity (reading R19): 24 FP32-pipe instructions per pair in the SASS of
+# pipeline_kernel<PipelineLennardJones> (12 FMUL + 7 FFMA + 5 FADD) + 1 MUFU.RSQ; Gflop/s printed at 24 and at 50 per pair
+OPS["lj"] = {"inst": 24, "kernel": "pipeline_kernel<PipelineLennardJones> (generalised kernel, row f3)", "flops": (24, 50)}
 LEAPFROG_KDK_PER_CALL = 100
+
+
+def LJ_ROWS(wl):
+    """row f3 (L1): the Lennard-Jones bench workload -- a dense fluid of 131072 particles (jittered lattice, density 0.8)."""
+    return wl.lj_fluid_rows(131072, 0.8, 0.1, seed=1)
 # (phi is wanted only at the final time: 100 of the 101 evaluations of a call run the 26-instruction loop without it)
 OPS["hermite"] = {"inst": 26, "kernel": "nb_hermite_kernel<PHI=false> inside nb_hermite4 (consumer of row f1)", "flops": (60, 60)}
 
@@ -254,6 +265,13 @@ class Problem:
             p_xj = np.concatenate([w.x_j, w.m_j[:, None]], axis=1).astype(np.float32)
             self.host = [np.ascontiguousarray(p_xj), np.ascontiguousarray(p_xi)]
             self.n_out = w.n_j
+        elif op == "lj":
+            rows = LJ_ROWS(wl)
+            self.w, self.pairs = rows, float(rows.shape[0]) ** 2
+            self.name = (f"row f3 (L1): Lennard-Jones fluid on a jittered simple-cubic lattice, density 0.8, sigma in [0.9, 1.1], eps in "
+                         f"[0.5, 1.5], rows (x,y,z,sigma/2,sqrt(eps)), n={rows.shape[0]}, seed=1; one nb_cunbody_lennard_jones call")
+            self.host = [rows, rows]
+            self.n_out = rows.shape[0]
         elif op == "hermite":
             w = wl.config(4)
             self.w = w
@@ -280,10 +298,10 @@ class Problem:
         self.dev = [torch.from_numpy(a).cuda() for a in self.host]
         self.pinned = [torch.from_numpy(a).pin_memory() for a in self.host]
         n = self.n_out
-        self.outs = [torch.empty((n, 3), dtype=torch.float32, device="cuda")]
+        self.outs = [torch.empty((n, 4 if op == "lj" else 3), dtype=torch.float32, device="cuda")]
         if op in ("jerk", "hermite"):
             self.outs.append(torch.empty((n, 3), dtype=torch.float32, device="cuda"))
-        if op != "cunbody":
+        if op not in ("cunbody", "lj"):
             self.outs.append(torch.empty((n,), dtype=torch.float32, device="cuda"))
         self.h_outs = [torch.empty(o.shape, dtype=torch.float32).pin_memory() for o in self.outs]
         self.h2d = int(sum(a.nbytes for a in self.host))
@@ -298,6 +316,8 @@ class Problem:
             nb.force(xi, xj, mj, w.eps2, acc_out=self.outs[0], pot_out=self.outs[1])
         elif self.op == "cunbody":
             nb.cunbody_force(t[0], t[1], self.outs[0])
+        elif self.op == "lj":
+            nb.cunbody_lennard_jones(t[0], t[1], self.outs[0])
         elif self.op == "leapfrog":
             nb.leapfrog_kdk(t[0], t[1], t[2], w.eps2, w.dt, LEAPFROG_KDK_PER_CALL, acc_io=self.outs[0], pot_out=self.outs[1])
             if t is self.dev:
@@ -339,6 +359,8 @@ class Problem:
             return "nb_force_jerk_host (pinned host buffers)"
         if self.op == "cunbody":
             return "pinned host rows -> cudaMemcpyAsync -> nb_cunbody_force -> cudaMemcpyAsync -> pinned host"
+        if self.op == "lj":
+            return "pinned host rows -> cudaMemcpyAsync -> nb_cunbody_lennard_jones -> cudaMemcpyAsync -> pinned host"
         if self.op == "hermite":
             return "pinned host (x, v, m) -> cudaMemcpyAsync -> nb_hermite4 (100 steps) -> cudaMemcpyAsync of a, j, phi -> pinned host"
         if self.op == "leapfrog":
@@ -348,8 +370,8 @@ class Problem:
     def plan(self, sm_count):
         if self.op == "force":
             return self.nb.plan_query(self.w.n_i, self.w.n_j, sm_count)
-        if self.op == "cunbody":
-            return {"cta": "256 threads x 2 i-records, 128-record j tiles, j-range split over S CTAs + second pass"}
+        if self.op in ("cunbody", "lj"):
+            return {"cta": "256 threads x 2 or 4 i-records, 128-record j tiles, j-range split over S CTAs + second pass"}
         if self.op == "hermite":
             return self.nb.plan_query_jerk(self.w.n_j, self.w.n_j, sm_count)
         if self.op == "leapfrog":
@@ -368,6 +390,21 @@ def oracle_rate_op(op, w, target_seconds, rng_seed=0):
         op = "jerk"
     cores = oracle.num_threads()
     rng = np.random.default_rng(rng_seed)
+    if op == "lj":
+        n = w.shape[0]
+
+        def run_lj(n_i):
+            idx = np.sort(rng.choice(n, n_i, replace=False))
+            rows_i = np.ascontiguousarray(w[idx])
+            t0 = time.perf_counter()
+            oracle.lennard_jones(rows_i, w)
+            return time.perf_counter() - t0
+        run_lj(64)
+        n_probe = max(64, 8 * cores)
+        rate = n_probe * n / run_lj(n_probe)
+        n_i = int(min(n, max(n_probe, target_seconds * rate / n)))
+        t = run_lj(n_i)
+        return n_i * n / t, cores, f"{n_i} of {n} i-particles (seeded) x all {n} j-particles, {t:.2f} s"
     if op == "jerk":
         def run(n_i):
             idx = np.sort(rng.choice(w.n_i, n_i, replace=False))
