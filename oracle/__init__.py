@@ -60,6 +60,8 @@ def _load():
         lib.oracle_force_eps_i_f64.restype = ctypes.c_int
         lib.oracle_hermite4_f64.argtypes = [i64, p, p, p, f64, f64, i64, p, p, p]
         lib.oracle_hermite4_f64.restype = ctypes.c_int
+        lib.oracle_hermite4_block_step_f64.argtypes = [i64, p, p, p, p, p, p, i64, p, f64, f64]
+        lib.oracle_hermite4_block_step_f64.restype = ctypes.c_int
         lib.oracle_lj_f64.argtypes = [i64, p, i64, p, p]
         lib.oracle_lj_f64.restype = ctypes.c_int
         lib.oracle_num_threads.restype = ctypes.c_int
@@ -211,6 +213,30 @@ def hermite4(x: np.ndarray, v: np.ndarray, m: np.ndarray, eps2: float, dt: float
     if rc != 0:
         raise ValueError(f"oracle_hermite4 returned {rc}")
     return xx, vv, acc, jerk, pot
+
+
+def hermite4_block_step(x: np.ndarray, v: np.ndarray, m: np.ndarray, acc: np.ndarray, jerk: np.ndarray, t: np.ndarray,
+                        active: np.ndarray, t_now: float, eps2: float):
+    """One block step of the individual-time-step Hermite scheme in double (reading R20): everybody is
+    predicted to t_now, the particles listed in ``active`` are evaluated against all and corrected.  Returns new
+    (x, v, acc, jerk, t); inputs are not modified."""
+    xx = np.array(x, dtype=np.float64, order="C").reshape(-1, 3)
+    vv = np.array(v, dtype=np.float64, order="C").reshape(-1, 3)
+    aa = np.array(acc, dtype=np.float64, order="C").reshape(-1, 3)
+    jj = np.array(jerk, dtype=np.float64, order="C").reshape(-1, 3)
+    tt = np.array(t, dtype=np.float64, order="C").reshape(-1)
+    mm = _c(m, np.float64).reshape(-1)
+    idx = _c(np.asarray(active), np.int32).reshape(-1)
+    n = xx.shape[0]
+    if not (vv.shape[0] == aa.shape[0] == jj.shape[0] == tt.shape[0] == mm.shape[0] == n):
+        raise ValueError("array lengths differ")
+    if np.unique(idx).size != idx.size:
+        raise ValueError("active indices must be distinct")
+    rc = _load().oracle_hermite4_block_step_f64(n, _ptr(xx), _ptr(vv), _ptr(mm), _ptr(aa), _ptr(jj), _ptr(tt),
+                                                idx.size, _ptr(idx) if idx.size else None, float(t_now), float(eps2))
+    if rc != 0:
+        raise ValueError(f"oracle_hermite4_block_step returned {rc}")
+    return xx, vv, aa, jj, tt
 
 
 def error_metrics(acc_test: np.ndarray, acc_ref: np.ndarray, pot_test: Optional[np.ndarray] = None,

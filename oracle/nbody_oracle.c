@@ -362,6 +362,72 @@ int oracle_hermite4_f64(int64_t n, double *x, double *v, const double *m, double
 }
 
 /* ------------------------------------------------------------------------------------------------
+ * Row f4, second half: one block step of the 4th-order Hermite scheme with individual (block) time steps -- the
+ * "active-subset" use BASELINE.json configs[2] is shaped for (i-set = the particles due now, j-set = everybody).
+ * Not in the paper (it only names the Hermite scheme); reading R20 takes the textbook
+ * form (Makino 1991; Makino & Aarseth 1992).  Every particle k holds (x, v, a, j) at its OWN time t[k] <= t_now.
+ *
+ *     for every particle k:   h = t_now - t[k]                                    (predict everybody to t_now)
+ *         xp = x + v h + a h^2/2 + j h^3/6        vp = v + a h + j h^2/2
+ *     for the active particles i only:
+ *         a1, j1 = force_jerk(i-set = (xp, vp) of the active, j-set = (xp, vp, m) of all)            (evaluate)
+ *         h = t_now - t[i]
+ *         v' = v + (a + a1) h/2 + (j - j1) h^2/12       x' = x + (v + v') h/2 + (a - a1) h^2/12      (correct)
+ *         x, v, a, j, t <- x', v', a1, j1, t_now
+ *     the others are left exactly as they were (their predicted state is discarded).
+ *
+ * Who is active and the next step of each particle are the caller's business (the scheduler is outside this call).
+ * active[] holds n_act distinct indices in [0, n).  With every particle active and all t equal this is one step of
+ * oracle_hermite4_f64.
+ * Pins (tests/test_oracle_hermite_pins.py, "h8"): that reduction; inactive particles bitwise untouched; a two-level
+ * schedule against scipy DOP853 with 4th-order convergence (fails when stale particles are not predicted or are
+ * predicted over the wrong interval); a pure-Python restatement with math.fsum on a tiny case.
+ */
+int oracle_hermite4_block_step_f64(int64_t n, double *x, double *v, const double *m, double *acc, double *jerk, double *t,
+                                   int64_t n_act, const int32_t *active, double t_now, double eps2)
+{
+    if (n < 0 || n_act < 0 || n_act > n || !(eps2 >= 0.0)) return 1;
+    if (n > 0 && (!x || !v || !m || !acc || !jerk || !t)) return 1;
+    if (n_act > 0 && !active) return 1;
+    for (int64_t q = 0; q < n_act; ++q) if (active[q] < 0 || active[q] >= n) return 1;
+    if (n_act == 0) return 0;
+    size_t n3 = 3 * (size_t)n, a3 = 3 * (size_t)n_act;
+    double *xp = (double *)malloc(sizeof(double) * n3), *vp = (double *)malloc(sizeof(double) * n3);
+    double *xi = (double *)malloc(sizeof(double) * a3), *vi = (double *)malloc(sizeof(double) * a3);
+    double *a1 = (double *)malloc(sizeof(double) * a3), *j1 = (double *)malloc(sizeof(double) * a3);
+    if (!xp || !vp || !xi || !vi || !a1 || !j1) { free(xp); free(vp); free(xi); free(vi); free(a1); free(j1); return 2; }
+    for (int64_t k = 0; k < n; ++k) {                                           /* predict everybody */
+        const double h = t_now - t[k], h2 = h * h, h3 = h * h * h;
+        for (int c = 0; c < 3; ++c) {
+            const size_t e = 3 * (size_t)k + c;
+            xp[e] = x[e] + v[e] * h + acc[e] * (h2 / 2.0) + jerk[e] * (h3 / 6.0);
+            vp[e] = v[e] + acc[e] * h + jerk[e] * (h2 / 2.0);
+        }
+    }
+    for (int64_t q = 0; q < n_act; ++q)                                         /* the i-set: the active, predicted */
+        for (int c = 0; c < 3; ++c) {
+            xi[3 * q + c] = xp[3 * (size_t)active[q] + c];
+            vi[3 * q + c] = vp[3 * (size_t)active[q] + c];
+        }
+    int rc = oracle_force_jerk_f64(n_act, xi, vi, n, xp, vp, m, eps2, a1, j1, NULL);   /* evaluate */
+    for (int64_t q = 0; q < n_act && rc == 0; ++q) {                            /* correct the active */
+        const size_t k = (size_t)active[q];
+        const double h = t_now - t[k], h2 = h * h;
+        for (int c = 0; c < 3; ++c) {
+            const size_t e = 3 * k + c;
+            const double vn = v[e] + (acc[e] + a1[3 * q + c]) * (h / 2.0) + (jerk[e] - j1[3 * q + c]) * (h2 / 12.0);
+            x[e] = x[e] + (v[e] + vn) * (h / 2.0) + (acc[e] - a1[3 * q + c]) * (h2 / 12.0);
+            v[e] = vn;
+            acc[e] = a1[3 * q + c];
+            jerk[e] = j1[3 * q + c];
+        }
+        t[k] = t_now;
+    }
+    free(xp); free(vp); free(xi); free(vi); free(a1); free(j1);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------------------
  * Row f3, a central force other than gravity: the paper lists "van der Waals molecular interactions" among the
  * interactions its generalised library runs (section 4.5) and gives no formula; reading R19
  * takes the textbook 12-6 Lennard-Jones pair with Lorentz-Berthelot mixing, all pairs, no cut-off:

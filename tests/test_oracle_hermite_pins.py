@@ -217,3 +217,124 @@ def test_h7_hermite_energy_error_far_below_leapfrog_and_outputs_are_the_carried_
     x, v, a, j, p = oracle.hermite4(x0, v0, m, eps2, dt, 0)
     ra, rj, rp = oracle.force_jerk(x0, v0, x0, v0, m, eps2)
     assert np.array_equal(x, x0) and np.array_equal(a, ra) and np.array_equal(j, rj) and np.array_equal(p, rp)
+
+
+# ----------------------------------------------------------------------------- h8: one block step (individual time steps)
+def _block_run(x0, v0, m, eps2, T, base_steps, slow, ratio):
+    """Two-level block schedule: particles in ``slow`` step with ratio * dt, the others with dt = T / base_steps."""
+    n = len(m)
+    x, v = x0.copy(), v0.copy()
+    a, j, _ = oracle.force_jerk(x, v, x, v, m, eps2)
+    t = np.zeros(n)
+    fast = np.array([k for k in range(n) if k not in slow], dtype=np.int32)
+    everybody = np.arange(n, dtype=np.int32)
+    dt = T / base_steps
+    for s in range(1, base_steps + 1):
+        active = everybody if s % ratio == 0 else fast
+        x, v, a, j, t = oracle.hermite4_block_step(x, v, m, a, j, t, active, s * dt, eps2)
+    assert np.all(t == T)
+    return x, v
+
+
+def test_h8_all_active_at_equal_times_is_one_shared_step():
+    x0, v0, m = _random_system(17, 5)
+    eps2, dt = 0.02, 1.0 / 32
+    a0, j0, _ = oracle.force_jerk(x0, v0, x0, v0, m, eps2)
+    x, v, a, j, t = oracle.hermite4_block_step(x0, v0, m, a0, j0, np.full(17, 0.25), np.arange(17), 0.25 + dt, eps2)
+    xr, vr, ar, jr, _ = oracle.hermite4(x0, v0, m, eps2, dt, 1)                    # pinned by h7
+    for got, ref in ((x, xr), (v, vr), (a, ar), (j, jr)):
+        np.testing.assert_allclose(got, ref, rtol=1e-14, atol=1e-15)
+    assert np.all(t == 0.25 + dt)
+    # the order in which the active particles are listed does not matter
+    perm = np.random.default_rng(0).permutation(17)
+    x2, v2, a2, j2, _ = oracle.hermite4_block_step(x0, v0, m, a0, j0, np.full(17, 0.25), perm, 0.25 + dt, eps2)
+    assert np.array_equal(x2, x) and np.array_equal(v2, v) and np.array_equal(a2, a) and np.array_equal(j2, j)
+
+
+def test_h8_inactive_particles_are_untouched_and_empty_active_set_is_a_no_op():
+    x0, v0, m = _random_system(12, 6)
+    eps2 = 0.01
+    a0, j0, _ = oracle.force_jerk(x0, v0, x0, v0, m, eps2)
+    t0 = np.linspace(0.0, 0.05, 12)
+    active = np.array([7, 2, 9], dtype=np.int32)
+    x, v, a, j, t = oracle.hermite4_block_step(x0, v0, m, a0, j0, t0, active, 0.0625, eps2)
+    rest = np.setdiff1d(np.arange(12), active)
+    for got, ref in ((x, x0), (v, v0), (a, a0), (j, j0), (t, t0)):
+        assert np.array_equal(got[rest], ref[rest])
+        assert not np.array_equal(got[active], ref[active])
+    assert np.all(t[active] == 0.0625)
+    out = oracle.hermite4_block_step(x0, v0, m, a0, j0, t0, np.zeros(0, dtype=np.int32), 0.0625, eps2)
+    for got, ref in zip(out, (x0, v0, a0, j0, t0)):
+        assert np.array_equal(got, ref)
+    with pytest.raises(ValueError):
+        oracle.hermite4_block_step(x0, v0, m, a0, j0, t0, np.array([3, 3]), 0.0625, eps2)
+    with pytest.raises(ValueError):
+        oracle.hermite4_block_step(x0, v0, m, a0, j0, t0, np.array([12]), 0.0625, eps2)
+
+
+def test_h8_pure_python_restatement_of_one_block_step():
+    """Independent evaluator: textbook formulas in Python floats with math.fsum, own pair loop, own indexing."""
+    import math
+    x0, v0, m = _random_system(6, 7)
+    eps2, t_now = 0.03, 0.125
+    a0, j0, _ = oracle.force_jerk(x0, v0, x0, v0, m, eps2)
+    t0 = np.array([0.0, 0.0625, 0.09375, 0.0, 0.0625, 0.109375])
+    active = [4, 0, 5]
+    got = oracle.hermite4_block_step(x0, v0, m, a0, j0, t0, np.array(active), t_now, eps2)
+    xp, vp = [], []
+    for k in range(6):
+        h = t_now - t0[k]
+        xp.append([math.fsum([x0[k][c], v0[k][c] * h, a0[k][c] * h * h / 2, j0[k][c] * h ** 3 / 6]) for c in range(3)])
+        vp.append([math.fsum([v0[k][c], a0[k][c] * h, j0[k][c] * h * h / 2]) for c in range(3)])
+    for i in active:
+        h = t_now - t0[i]
+        a1, j1 = [[], [], []], [[], [], []]
+        for q in range(6):
+            if q == i:
+                continue
+            d = [xp[q][c] - xp[i][c] for c in range(3)]
+            w = [vp[q][c] - vp[i][c] for c in range(3)]
+            r2 = math.fsum([d[0] ** 2, d[1] ** 2, d[2] ** 2, eps2])
+            rv = math.fsum([d[c] * w[c] for c in range(3)])
+            for c in range(3):
+                a1[c].append(m[q] * d[c] / r2 ** 1.5)
+                j1[c].append(m[q] * (w[c] / r2 ** 1.5 - 3 * rv * d[c] / r2 ** 2.5))
+        for c in range(3):
+            an, jn = math.fsum(a1[c]), math.fsum(j1[c])
+            vn = math.fsum([v0[i][c], (a0[i][c] + an) * h / 2, (j0[i][c] - jn) * h * h / 12])
+            xn = math.fsum([x0[i][c], (v0[i][c] + vn) * h / 2, (a0[i][c] - an) * h * h / 12])
+            assert got[0][i][c] == pytest.approx(xn, rel=1e-13, abs=1e-15)
+            assert got[1][i][c] == pytest.approx(vn, rel=1e-13, abs=1e-15)
+            assert got[2][i][c] == pytest.approx(an, rel=1e-13, abs=1e-15)
+            assert got[3][i][c] == pytest.approx(jn, rel=1e-12, abs=1e-14)
+
+
+def test_h8_two_level_schedule_matches_an_adaptive_solver_and_is_fourth_order():
+    """Particle 0 steps with 2 dt, particles 1 and 2 with dt: at every odd sub-step particle 0 enters only through its
+    prediction from a stale state.  A missing or mis-timed prediction leaves a first- or second-order error."""
+    from scipy.integrate import solve_ivp
+    x0, v0, m = _three_body()
+    eps2, T = 0.01, 1.0
+
+    def rhs(t, y):
+        x, v = y[:9].reshape(3, 3), y[9:].reshape(3, 3)
+        a = np.zeros((3, 3))
+        for p in range(3):
+            for q in range(3):
+                if p != q:
+                    d = x[q] - x[p]
+                    a[p] += m[q] * d / (d @ d + eps2) ** 1.5
+        return np.concatenate([v.ravel(), a.ravel()])
+
+    sol = solve_ivp(rhs, (0.0, T), np.concatenate([x0.ravel(), v0.ravel()]), method="DOP853", rtol=1e-13, atol=1e-14)
+    x_ref, v_ref = sol.y[:9, -1].reshape(3, 3), sol.y[9:, -1].reshape(3, 3)
+    errs = []
+    for steps in (64, 128, 256):
+        x, v = _block_run(x0, v0, m, eps2, T, steps, slow={0}, ratio=2)
+        errs.append(max(np.abs(x - x_ref).max(), np.abs(v - v_ref).max()))
+    assert errs[2] < 1e-7
+    assert 10.0 < errs[0] / errs[1] < 24.0 and 10.0 < errs[1] / errs[2] < 24.0       # error ~ dt^4
+    # and the block scheme's result differs from the shared-step one (the schedule really is two-level)
+    xs, _, _, _, _ = oracle.hermite4(x0, v0, m, eps2, T / 64, 64)
+    xb, _ = _block_run(x0, v0, m, eps2, T, 64, slow={0}, ratio=2)
+    assert np.abs(xs - xb).max() > 1e-9
