@@ -252,6 +252,32 @@ int nb_hermite4(int64_t n, float *x, float *v, const float *m,
                 void *stream);
 
 /*
+ * nb_hermite4_block_step -- ONE block step of the 4th-order Hermite scheme with individual (block) time steps: the
+ * active-subset integration that BASELINE.json configs[2] is shaped for (i-set = the particles due now, j-set =
+ * everybody), on top of the separate i- and j-sets of the paper's call.  The paper names the Hermite
+ * scheme as the user of its force + jerk pipeline and does not describe it; this is the textbook
+ * form (reading R20).  Every particle k holds (x, v, a, j) at its OWN time t[k] <= t_now:
+ *
+ *     all k:          h = t_now - t[k];  xp = x + v h + a h^2/2 + j h^3/6;  vp = v + a h + j h^2/2
+ *     active i only:  a1, j1 = force_jerk(i-set = (xp, vp) of the active, j-set = (xp, vp, m) of all n)
+ *                     v' = v + (a + a1) h/2 + (j - j1) h^2/12;   x' = x + (v + v') h/2 + (a - a1) h^2/12
+ *                     x, v, a, j, t <- x', v', a1, j1, t_now
+ *
+ *   x, v, acc_io, jerk_io   device, float [n][3]: state at t[k]; the active rows are updated in place, no other row
+ *             is written          m   device, const, float [n]
+ *   t         device, double [n]: each particle's own time; the active entries become t_now.  h is formed in double
+ *             and rounded to float once (exact for the usual power-of-two step hierarchy)
+ *   active    device, const, int32 [n_act]: DISTINCT indices in [0, n), any order; not validated on the device
+ *             (out-of-range or repeated indices: undefined results).  n_act == 0: success, nothing is touched
+ *   t_now     the block time.  Who is due and each particle's next step are the caller's business.
+ * Asynchronous on `stream`; 3 small launches + those of one nb_force_jerk(n_act, n) without phi.
+ */
+int nb_hermite4_block_step(int64_t n, float *x, float *v, const float *m,
+                           float *acc_io, float *jerk_io, double *t,
+                           int64_t n_act, const int32_t *active, double t_now,
+                           float eps2, void *stream);
+
+/*
  * nb_force_jerk_host -- nb_force_jerk on HOST arrays: the paper's force() of Fig. A.2 with its
  * host->device and device->host copies (steps (a) and (l)) inside the call.  Blocking.
  */

@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     force_jerk_host,
     force_packed,
     hermite4,
+    hermite4_block_step,
     last_launch_count,
     leapfrog_kdk,
     pack_j,

@@ -62,6 +62,8 @@ def lib() -> ctypes.CDLL:
         l.nb_plan_query_jerk.restype = ci
         l.nb_hermite4.argtypes = [i64, p, p, p, f32, f32, i64, p, p, p, p]
         l.nb_hermite4.restype = ci
+        l.nb_hermite4_block_step.argtypes = [i64, p, p, p, p, p, p, i64, p, ctypes.c_double, f32, p]
+        l.nb_hermite4_block_step.restype = ci
         l.nb_plan_query.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
         l.nb_plan_query.restype = ci
         l.nb_last_launch_count.restype = i64
@@ -333,6 +335,28 @@ def hermite4(x, v, m, eps2: float, dt: float, n_steps: int, acc_io=None, jerk_io
                                _stream_ptr(stream))
     _check(st, "nb_hermite4")
     return acc_io, jerk_io, pot_out
+
+
+def hermite4_block_step(x, v, m, acc_io, jerk_io, t, active, t_now: float, eps2: float, stream=None) -> None:
+    """nb_hermite4_block_step: the rows of x, v, acc_io, jerk_io, t listed in ``active`` are updated IN PLACE."""
+    import torch
+    _dev_f32(x, "x", (3,)); _dev_f32(v, "v", (3,)); _dev_f32(m, "m", ())
+    _dev_f32(acc_io, "acc_io", (3,)); _dev_f32(jerk_io, "jerk_io", (3,))
+    n = x.shape[0]
+    if not (v.shape[0] == m.shape[0] == acc_io.shape[0] == jerk_io.shape[0] == n):
+        raise ValueError("x, v, m, acc_io, jerk_io lengths differ")
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == (n,)):
+        raise ValueError("t must be a contiguous CUDA float64 tensor of shape (n,)")
+    if not (active.is_cuda and active.dtype == torch.int32 and active.is_contiguous() and active.dim() == 1):
+        raise ValueError("active must be a contiguous 1-D CUDA int32 tensor")
+    if t.device != x.device or active.device != x.device:
+        raise ValueError("tensors live on different devices")
+    with torch.cuda.device(x.device):
+        st = lib().nb_hermite4_block_step(n, x.data_ptr(), v.data_ptr(), m.data_ptr(), acc_io.data_ptr(),
+                                          jerk_io.data_ptr(), t.data_ptr(), int(active.shape[0]),
+                                          active.data_ptr() if active.shape[0] else None, float(t_now), float(eps2),
+                                          _stream_ptr(stream))
+    _check(st, "nb_hermite4_block_step")
 
 
 def plan_query(n_i: int, n_j: int, sm_count: int = 148) -> dict:

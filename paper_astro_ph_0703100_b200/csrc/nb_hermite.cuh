@@ -406,4 +406,65 @@ __global__ void __launch_bounds__(256) nb_hermite_correct_kernel(float* __restri
     j0[k] = j_new;
 }
 
+// ---------------------------------------------------------------- block (individual) time steps: one block step, row f4
+// Every particle holds (x, v, a, j) at its own time t[k] (FP64; the interval h = t_now - t[k] is rounded to FP32 once).
+// predict everybody to t_now (same Horner form as the shared-step kernel, h per particle) and pack the j records:
+__global__ void __launch_bounds__(256) nb_block_predict_pack_kernel(const float* __restrict__ x, const float* __restrict__ v,
+                                                                    const float* __restrict__ a, const float* __restrict__ j,
+                                                                    const float* __restrict__ m, const double* __restrict__ t,
+                                                                    double t_now, float* __restrict__ xp, float* __restrict__ vp,
+                                                                    float4* __restrict__ jp, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float dt = (float)(t_now - t[i]);
+    float px[3], pv[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const size_t k = 3 * (size_t)i + c;
+        const float aa = a[k], jj = j[k], vv = v[k];
+        px[c] = fmaf(fmaf(fmaf(jj, dt * (1.0f / 3.0f), aa), dt * 0.5f, vv), dt, x[k]);
+        pv[c] = fmaf(fmaf(jj, dt * 0.5f, aa), dt, vv);
+        xp[k] = px[c];
+        vp[k] = pv[c];
+    }
+    jp[2 * (size_t)i + 0] = make_float4(px[0], px[1], px[2], m[i]);
+    jp[2 * (size_t)i + 1] = make_float4(pv[0], pv[1], pv[2], 0.0f);
+}
+// the i-set of the block step: predicted state of the active particles, in the order of active[]
+__global__ void __launch_bounds__(256) nb_block_gather_kernel(const float* __restrict__ xp, const float* __restrict__ vp,
+                                                              const int* __restrict__ active, int n_act,
+                                                              float* __restrict__ xi, float* __restrict__ vi) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n_act) return;
+    const size_t k = 3 * (size_t)active[q];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        xi[3 * (size_t)q + c] = xp[k + c];
+        vi[3 * (size_t)q + c] = vp[k + c];
+    }
+}
+// correct the active particles over their own interval and advance their clocks; nobody else is written
+__global__ void __launch_bounds__(256) nb_block_correct_kernel(float* __restrict__ x, float* __restrict__ v,
+                                                               float* __restrict__ a0, float* __restrict__ j0,
+                                                               double* __restrict__ t, const int* __restrict__ active,
+                                                               const float* __restrict__ a1, const float* __restrict__ j1,
+                                                               double t_now, int n_act) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n_act) return;
+    const int i = active[q];
+    const float dt = (float)(t_now - t[i]);
+    const float h = 0.5f * dt, h2 = dt * dt * (1.0f / 12.0f);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const size_t k = 3 * (size_t)i + c, e = 3 * (size_t)q + c;
+        const float a_old = a0[k], a_new = a1[e], j_old = j0[k], j_new = j1[e], v_old = v[k];
+        const float v_new = fmaf(j_old - j_new, h2, fmaf(a_old + a_new, h, v_old));
+        x[k] = fmaf(a_old - a_new, h2, fmaf(v_old + v_new, h, x[k]));
+        v[k] = v_new;
+        a0[k] = a_new;
+        j0[k] = j_new;
+    }
+    t[i] = t_now;
+}
+
 }  // namespace nb

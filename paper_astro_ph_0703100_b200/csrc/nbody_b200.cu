@@ -962,6 +962,52 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
     return NB_OK;
 }
 
+int nb_hermite4_block_step(int64_t n, float* x, float* v, const float* m, float* acc_io, float* jerk_io, double* t,
+                           int64_t n_act, const int32_t* active, double t_now, float eps2, void* stream_) {
+    t_launches = 0;
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (bad_count(n) || bad_count(n_act) || n_act > n) return NB_ERR_INVALID_VALUE;
+    if (!(eps2 >= 0.0f) || !std::isfinite(eps2) || !std::isfinite(t_now)) return NB_ERR_INVALID_VALUE;
+    if (n > 0 && (!x || !v || !m || !acc_io || !jerk_io || !t)) return NB_ERR_INVALID_VALUE;
+    if (n_act > 0 && !active) return NB_ERR_INVALID_VALUE;
+    if (3 * n > (int64_t)INT32_MAX) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n_act == 0) return NB_OK;                                     // nobody is due: the state stays as it is
+    Workspace* ws;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        ws = &g_ws[std::make_pair(dev, stream)];
+    }
+    const size_t b3 = ((size_t)3 * n * sizeof(float) + 255) / 256 * 256;
+    rc = ensure(&ws->hstate, &ws->hstate_bytes, 6 * b3, stream);      // xp, vp [n]; a1, j1, x_i, v_i [n_act <= n]
+    if (rc != NB_OK) return rc;
+    char* base = reinterpret_cast<char*>(ws->hstate);
+    float* xp = reinterpret_cast<float*>(base);
+    float* vp = reinterpret_cast<float*>(base + b3);
+    float* a1 = reinterpret_cast<float*>(base + 2 * b3);
+    float* j1 = reinterpret_cast<float*>(base + 3 * b3);
+    float* xi = reinterpret_cast<float*>(base + 4 * b3);
+    float* vi = reinterpret_cast<float*>(base + 5 * b3);
+    rc = ensure(&ws->jp2, &ws->jp2_bytes, (size_t)n * 2 * sizeof(float4), stream);
+    if (rc != NB_OK) return rc;
+    const int threads = 256;
+    const unsigned ablocks = (unsigned)((n_act + threads - 1) / threads);
+    nb::nb_block_predict_pack_kernel<<<(unsigned)((n + threads - 1) / threads), threads, 0, stream>>>(
+        x, v, acc_io, jerk_io, m, t, t_now, xp, vp, reinterpret_cast<float4*>(ws->jp2), (int)n);
+    NB_CUDA(cudaGetLastError());
+    nb::nb_block_gather_kernel<<<ablocks, threads, 0, stream>>>(xp, vp, active, (int)n_act, xi, vi);
+    NB_CUDA(cudaGetLastError());
+    rc = force_jerk_impl(n_act, xi, vi, n, xp, vp, m, eps2, a1, j1, nullptr, stream, true);
+    if (rc != NB_OK) return rc;
+    nb::nb_block_correct_kernel<<<ablocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, t, active, a1, j1, t_now, (int)n_act);
+    NB_CUDA(cudaGetLastError());
+    t_launches += 3;
+    return NB_OK;
+}
+
 int nb_plan_query(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]) {
     if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
     const nb::Plan p = nb::make_plan(n_i, n_j, sm_count);

@@ -264,3 +264,14 @@ def lj_fluid_rows(n: int, density: float, jitter: float, seed: int) -> np.ndarra
     sigma = rng.uniform(0.9, 1.1, n)
     eps = rng.uniform(0.5, 1.5, n)
     return _f32(np.concatenate([x, 0.5 * sigma[:, None], np.sqrt(eps)[:, None]], axis=1))
+
+
+def block_levels(n: int, seed: int, n_levels: int = 3) -> np.ndarray:
+    """Seeded block-time-step levels for the active-subset integration (row f4): particle k steps with dt * 2**level[k].
+    Half of the particles sit on the finest level, the rest are spread evenly over the coarser ones (block-step runs
+    of a Plummer sphere keep most particles on few levels).  Holds no arithmetic of the method: who is due at
+    sub-step s is ``s % 2**level == 0``, evaluated by the caller."""
+    rng = _rng(seed)
+    p = np.full(n_levels, 0.5 / max(n_levels - 1, 1))
+    p[0] = 0.5 if n_levels > 1 else 1.0
+    return rng.choice(n_levels, size=n, p=p).astype(np.int32)

@@ -1,0 +1,116 @@
+"""nb_hermite4_block_step (row f4: active-subset integration with block time steps, on top of C2-style force + jerk
+calls) against the FP64 oracle's block step on the same seeded state and the same schedule."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_astro_ph_0703100_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def nb():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    import paper_astro_ph_0703100_b200 as nb_
+    nb_.lib()
+    return nb_
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def start(nb, w):
+    """Device state with a, j of the initial state from nb_force_jerk, oracle state with its own evaluation."""
+    x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
+    acc, jerk, _ = nb.force_jerk(x, v, x, v, m, w.eps2)
+    ra, rj, _ = oracle.force_jerk(w.x_j, w.v, w.x_j, w.v, w.m_j, w.eps2)
+    return (x, v, m, acc, jerk), (w.x_j.astype(np.float64), w.v.astype(np.float64), ra, rj)
+
+
+def host(*ts):
+    import torch
+    torch.cuda.synchronize()
+    return [t.cpu().numpy() for t in ts]
+
+
+@pytest.mark.parametrize("n,n_act,seed", [(1500, 1, 0), (1500, 37, 1), (2049, 513, 2), (700, 700, 3), (5000, 2500, 4)])
+def test_one_block_step_matches_oracle(nb, n, n_act, seed):
+    """Particles sit at different own times (three levels); a ragged, shuffled active set is advanced to t_now."""
+    import torch
+    w = wl.plummer_workload(n, 1.0 / 64, seed=10 + seed, with_velocities=True)
+    (x, v, m, acc, jerk), (xr, vr, ar, jr) = start(nb, w)
+    dt = 1.0 / 256
+    t0 = -dt * wl.block_levels(n, seed).astype(np.float64)             # own times 0, -dt, -2 dt; t_now = dt
+    active = np.random.default_rng(seed).permutation(n)[:n_act].astype(np.int32)
+    t = dev(t0.copy())
+    before = host(x, v, acc, jerk)
+    nb.hermite4_block_step(x, v, m, acc, jerk, t, dev(active), dt, w.eps2)
+    gx, gv, ga, gj, gt = host(x, v, acc, jerk, t)
+    # the oracle starts from the SAME FP32 a, j the device holds (its own a, j differ by FP32 rounding only)
+    ox, ov, oa, oj, ot = oracle.hermite4_block_step(xr, vr, w.m_j, before[2].astype(np.float64),
+                                                    before[3].astype(np.float64), t0, active, dt, w.eps2)
+    assert np.array_equal(gt, ot)                                                   # clocks: exact
+    rest = np.setdiff1d(np.arange(n), active)
+    for g, b in zip((gx, gv, ga, gj), before):
+        assert np.array_equal(g[rest], b[rest])                                     # inactive rows: bitwise untouched
+    assert np.abs(gx - ox).max() < 2e-6 and np.abs(gv - ov).max() < 2e-6
+    e = oracle.error_metrics(ga[active], oa[active])
+    ej = oracle.error_metrics(gj[active], oj[active])
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-4
+
+
+def test_empty_active_set_is_a_no_op(nb):
+    import torch
+    w = wl.plummer_workload(300, 1.0 / 64, seed=20, with_velocities=True)
+    (x, v, m, acc, jerk), _ = start(nb, w)
+    t = dev(np.zeros(300))
+    before = host(x, v, acc, jerk, t)
+    nb.hermite4_block_step(x, v, m, acc, jerk, t, torch.zeros(0, dtype=torch.int32, device="cuda"), 0.125, w.eps2)
+    for g, b in zip(host(x, v, acc, jerk, t), before):
+        assert np.array_equal(g, b)
+    assert nb.last_launch_count() == 0
+
+
+def test_all_active_equals_one_shared_step_bitwise(nb):
+    """Everybody due at the same time: the block step is one step of nb_hermite4 (same arithmetic, same kernels)."""
+    import torch
+    n = 1024
+    w = wl.plummer_workload(n, 1.0 / 64, seed=21, with_velocities=True)
+    dt = 1.0 / 128
+    (x, v, m, acc, jerk), _ = start(nb, w)
+    t = dev(np.full(n, 0.5))
+    nb.hermite4_block_step(x, v, m, acc, jerk, t, torch.arange(n, dtype=torch.int32, device="cuda"), 0.5 + dt, w.eps2)
+    x2, v2 = dev(w.x_j.copy()), dev(w.v.copy())
+    a2, j2, _ = nb.hermite4(x2, v2, m, w.eps2, dt, 1)
+    gx, gv, ga, gj, sx, sv, sa, sj = host(x, v, acc, jerk, x2, v2, a2, j2)
+    assert np.array_equal(gx, sx) and np.array_equal(gv, sv) and np.array_equal(ga, sa) and np.array_equal(gj, sj)
+
+
+@pytest.mark.parametrize("n,sub_steps", [(1200, 8), (4096, 4)])
+def test_three_level_schedule_matches_oracle_and_conserves_energy(nb, n, sub_steps):
+    """A block-step run: level-L particles are due every 2^L sub-steps; device and oracle follow the same schedule."""
+    w = wl.plummer_workload(n, 1.0 / 32, seed=22, with_velocities=True)
+    (x, v, m, acc, jerk), (xr, vr, ar, jr) = start(nb, w)
+    level = wl.block_levels(n, 5)
+    dt = 1.0 / 512
+    t, tr = dev(np.zeros(n)), np.zeros(n)
+    n_due = []
+    for s in range(1, sub_steps + 1):
+        active = np.nonzero(s % (1 << level) == 0)[0].astype(np.int32)
+        n_due.append(active.size)
+        nb.hermite4_block_step(x, v, m, acc, jerk, t, dev(active), s * dt, w.eps2)
+        xr, vr, ar, jr, tr = oracle.hermite4_block_step(xr, vr, w.m_j, ar, jr, tr, active, s * dt, w.eps2)
+    assert len(set(n_due)) >= 3                                                     # the schedule really has three levels
+    gx, gv, ga, gj, gt = host(x, v, acc, jerk, t)
+    assert np.array_equal(gt, tr) and np.all(gt == sub_steps * dt)
+    assert np.abs(gx - xr).max() < 1e-5 and np.abs(gv - vr).max() < 1e-5
+    e = oracle.error_metrics(ga, ar)
+    ej = oracle.error_metrics(gj, jr)
+    assert e["acc_rms"] <= 1e-4 and ej["acc_rms"] <= 1e-3                           # values at the FP32 trajectory's state
+    _, _, e0 = oracle.energy(w.x_j, w.v, w.m_j, w.eps2)
+    _, _, e1 = oracle.energy(gx, gv, w.m_j, w.eps2)
+    assert abs(e1 - e0) / abs(e0) < 1e-5
