@@ -166,6 +166,9 @@ def reference_arm(args, wl):
     elif args.op == "hermite":
         w = wl.plummer_workload(65536, 1.0 / 128, seed=4, name="C4", with_velocities=True)
         name = "C4's particles, force+jerk evaluations of the Hermite integration (oracle force_jerk on a sample)"
+    elif args.op == "block":
+        w = wl.plummer_workload(65536, 1.0 / 128, seed=4, name="C4", with_velocities=True)
+        name = "row f4 (B1): C4's particles, force+jerk evaluations of the block-step integration (oracle force_jerk on a sample)"
     elif args.op == "leapfrog":
         w = wl.config(4)
         name = "BASELINE.json configs[4] (C4): force evaluations of the KDK integration, N=65536 (oracle force on a sample)"
@@ -229,6 +232,11 @@ def LJ_ROWS(wl):
     return wl.lj_fluid_rows(131072, 0.8, 0.1, seed=1)
 # (phi is wanted only at the final time: 100 of the 101 evaluations of a call run the 26-instruction loop without it)
 OPS["hermite"] = {"inst": 26, "kernel": "nb_hermite_kernel<PHI=false> inside nb_hermite4 (consumer of row f1)", "flops": (60, 60)}
+# row f4, active-subset integration: one bench "step" = one cycle of BLOCK_SUB_STEPS nb_hermite4_block_step calls under a
+# three-level block schedule (half of the particles due every sub-step, a quarter every 2nd, a quarter every 4th)
+OPS["block"] = {"inst": 26, "kernel": "nb_hermite_kernel<PHI=false> inside nb_hermite4_block_step (row f4, n_act x n pairs)",
+                "flops": (60, 60)}
+BLOCK_SUB_STEPS = 4
 
 
 class Problem:
@@ -281,6 +289,23 @@ class Problem:
             self.host = [w.x_j, w.v, w.m_j]
             self.n_out = w.n_j
             self.kdk_done = 0
+        elif op == "block":
+            w = wl.config(4)
+            self.w = w
+            level = wl.block_levels(w.n_j, seed=4)
+            self.active = [np.nonzero(s % (1 << level) == 0)[0].astype(np.int32) for s in range(1, BLOCK_SUB_STEPS + 1)]
+            self.pairs = float(sum(a.size for a in self.active)) * float(w.n_j)
+            self.sub_dt = w.dt / BLOCK_SUB_STEPS
+            self.name = (f"row f4 (B1): configs[4]'s particles (C4: N={w.n_j}, eps2={w.eps2:.6g}, seed=4) under block time steps, "
+                         f"three levels (seeded: 1/2 of the particles step with dt/4, 1/4 with dt/2, 1/4 with dt = 1/512); one "
+                         f"step = one cycle of {BLOCK_SUB_STEPS} nb_hermite4_block_step calls, n_act = "
+                         f"{[int(a.size) for a in self.active]} of {w.n_j} against all {w.n_j}")
+            dx, dv, dm = (torch.from_numpy(a).cuda() for a in (w.x_j, w.v, w.m_j))
+            a0, j0, _ = nb.force_jerk(dx, dv, dx, dv, dm, w.eps2, want_pot=False)      # a, j of the start state (set-up)
+            torch.cuda.synchronize()
+            self.host = [w.x_j, w.v, w.m_j, a0.cpu().numpy(), j0.cpu().numpy(), np.zeros(w.n_j, dtype=np.float64)] + self.active
+            self.n_out = w.n_j
+            self.cycles_done = 0
         elif op == "jerk":
             w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
             self.w, self.pairs = w, float(w.n_i) * float(w.n_j)
@@ -299,9 +324,11 @@ class Problem:
         self.pinned = [torch.from_numpy(a).pin_memory() for a in self.host]
         n = self.n_out
         self.outs = [torch.empty((n, 4 if op == "lj" else 3), dtype=torch.float32, device="cuda")]
+        if op == "block":
+            self.outs = [self.dev[k] for k in (0, 1, 3, 4)]            # the state itself is the result: x, v, a, j
         if op in ("jerk", "hermite"):
             self.outs.append(torch.empty((n, 3), dtype=torch.float32, device="cuda"))
-        if op not in ("cunbody", "lj"):
+        if op not in ("cunbody", "lj", "block"):
             self.outs.append(torch.empty((n,), dtype=torch.float32, device="cuda"))
         self.h_outs = [torch.empty(o.shape, dtype=torch.float32).pin_memory() for o in self.outs]
         self.h2d = int(sum(a.nbytes for a in self.host))
@@ -327,6 +354,15 @@ class Problem:
                         pot_out=self.outs[2])
             if t is self.dev:
                 self.kdk_done += LEAPFROG_KDK_PER_CALL
+        elif self.op == "block":
+            base = self.cycles_done * BLOCK_SUB_STEPS if t is self.dev else 0          # staged state starts at time 0
+            launches = 0
+            for s in range(1, BLOCK_SUB_STEPS + 1):
+                nb.hermite4_block_step(t[0], t[1], t[2], t[3], t[4], t[5], t[5 + s], (base + s) * self.sub_dt, w.eps2)
+                launches += nb.last_launch_count()
+            self.launches = launches
+            if t is self.dev:
+                self.cycles_done += 1
         elif self.op == "jerk":
             nb.force_jerk(t[0], t[1], t[0], t[1], t[2], w.eps2, acc_out=self.outs[0], jerk_out=self.outs[1], pot_out=self.outs[2])
         else:
@@ -347,7 +383,8 @@ class Problem:
             return
         staged = [p.cuda(non_blocking=True) for p in self.pinned]
         self.call(staged)
-        for h, d in zip(self.h_outs, self.outs):
+        outs = [staged[k] for k in (0, 1, 3, 4)] if self.op == "block" else self.outs
+        for h, d in zip(self.h_outs, outs):
             h.copy_(d, non_blocking=True)
         self.torch.cuda.synchronize()
 
@@ -361,6 +398,9 @@ class Problem:
             return "pinned host rows -> cudaMemcpyAsync -> nb_cunbody_force -> cudaMemcpyAsync -> pinned host"
         if self.op == "lj":
             return "pinned host rows -> cudaMemcpyAsync -> nb_cunbody_lennard_jones -> cudaMemcpyAsync -> pinned host"
+        if self.op == "block":
+            return ("pinned host (x, v, m, a, j, t, 4 active lists) -> cudaMemcpyAsync -> 4 x nb_hermite4_block_step -> "
+                    "cudaMemcpyAsync of x, v, a, j -> pinned host")
         if self.op == "hermite":
             return "pinned host (x, v, m) -> cudaMemcpyAsync -> nb_hermite4 (100 steps) -> cudaMemcpyAsync of a, j, phi -> pinned host"
         if self.op == "leapfrog":
@@ -378,6 +418,8 @@ class Problem:
             return self.nb.plan_query(self.w.n_j, self.w.n_j, sm_count)
         if self.op == "jerk":
             return self.nb.plan_query_jerk(self.w.n_i, self.w.n_j, sm_count)
+        if self.op == "block":
+            return {str(int(a.size)): self.nb.plan_query_jerk(int(a.size), self.w.n_j, sm_count) for a in self.active[:3]}
         return {"cta": "one row of CTAs, 8 warps split each list (WJ = 8), no split across CTAs"}
 
 
@@ -386,7 +428,7 @@ def oracle_rate_op(op, w, target_seconds, rng_seed=0):
     import oracle
     if op in ("force", "leapfrog", "cunbody"):
         return oracle_rate(w, target_seconds, rng_seed)
-    if op == "hermite":
+    if op in ("hermite", "block"):
         op = "jerk"
     cores = oracle.num_threads()
     rng = np.random.default_rng(rng_seed)
@@ -503,7 +545,7 @@ def main():
         flush.fill_(1)
         prob.call()
     torch.cuda.synchronize()
-    launches_per_step = nb.last_launch_count()
+    launches_per_step = prob.launches if args.op == "block" else nb.last_launch_count()
 
     sampler = ClockSampler(physical_gpu_index(local_rank))
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
@@ -569,6 +611,8 @@ def main():
         peak_inst = sm_count * FP32_LANES_PER_SM_CLK * f_max                 # FP32-pipe lane-instructions / s
         # interactions per launch of the dominant kernel (a leapfrog call launches it once per force evaluation)
         pairs_k = float(prob.w.n_j) ** 2 if args.op in ("leapfrog", "hermite") else pairs   # (sharded: this rank's slice x all j)
+        if args.op == "block":
+            pairs_k = pairs / BLOCK_SUB_STEPS                                # mean over the cycle's launches (n_act varies)
         k_rate = pairs_k * n_k / (k_ms * 1e-3) if n_k else 0.0
         inst = op["inst"]
         achieved = inst * k_rate
@@ -610,6 +654,8 @@ def main():
         if graph_ms is not None:
             out["graph_replay"] = {"ms_per_call": graph_ms, "value": pairs / (graph_ms * 1e-3), "unit": METRIC,
                                    "note": "one captured nb_force call replayed 200x back to back, L2 warm"}
+        if args.op == "block":
+            out["block_steps_per_s"] = BLOCK_SUB_STEPS * args.steps / (total_ms * 1e-3)
         if args.op == "hermite":
             out["hermite_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
         if args.op in ("leapfrog", "hermite") and not args.no_cpu_baseline:
@@ -619,6 +665,15 @@ def main():
             _, _, e_end = oracle.energy(prob.dev[0].cpu().numpy(), prob.dev[1].cpu().numpy(), w.m_j, w.eps2)
             out["energy"] = {"time_steps": prob.kdk_done, "kdk_steps": prob.kdk_done, "E_start": e_start, "E_end": e_end,
                              "rel_drift": abs(e_end - e_start) / abs(e_start), "by": "oracle.energy (FP64) on the GPU's FP32 (x, v)"}
+        if args.op == "block" and not args.no_cpu_baseline:
+            import oracle
+            w = prob.w
+            _, _, e_start = oracle.energy(w.x_j, w.v, w.m_j, w.eps2)
+            _, _, e_end = oracle.energy(prob.dev[0].cpu().numpy(), prob.dev[1].cpu().numpy(), w.m_j, w.eps2)
+            out["energy"] = {"cycles": prob.cycles_done, "block_steps": prob.cycles_done * BLOCK_SUB_STEPS,
+                             "time": prob.cycles_done * w.dt, "E_start": e_start, "E_end": e_end,
+                             "rel_drift": abs(e_end - e_start) / abs(e_start),
+                             "by": "oracle.energy (FP64) on the GPU's FP32 (x, v), all clocks equal at the end of a cycle"}
         if args.op == "leapfrog":
             out["kdk_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
         if args.check and args.op in ("force", "jerk") and not args.shard:
