@@ -114,3 +114,35 @@ def test_three_level_schedule_matches_oracle_and_conserves_energy(nb, n, sub_ste
     _, _, e0 = oracle.energy(w.x_j, w.v, w.m_j, w.eps2)
     _, _, e1 = oracle.energy(gx, gv, w.m_j, w.eps2)
     assert abs(e1 - e0) / abs(e0) < 1e-5
+
+
+def test_bench_size_block_cycle_sampled_against_oracle(nb):
+    """bench.py --op block's own configuration (C4's particles, N = 65536, workloads.block_levels(seed=4), list-mode
+    force + jerk on n_act x n >= 2^31 pairs): each of the cycle's four block steps is checked on 384 sampled due
+    particles -- the oracle advances only the sample (a due particle's update does not depend on who else is due)
+    from the device's own state before the step."""
+    import torch
+    w = wl.config(4)
+    n = w.n_j
+    level = wl.block_levels(n, seed=4)
+    sub_dt = w.dt / 4
+    (x, v, m, acc, jerk), _ = start(nb, w)
+    t = dev(np.zeros(n))
+    rng = np.random.default_rng(0)
+    for s in range(1, 5):
+        active = np.nonzero(s % (1 << level) == 0)[0].astype(np.int32)
+        assert active.size * n >= 2 ** 31 or s % 2 == 1
+        bx, bv, ba, bj, bt = host(x, v, acc, jerk, t)
+        nb.hermite4_block_step(x, v, m, acc, jerk, t, dev(active), s * sub_dt, w.eps2)
+        gx, gv, ga, gj, gt = host(x, v, acc, jerk, t)
+        sample = np.sort(rng.choice(active, 384, replace=False)).astype(np.int32)
+        ox, ov, oa, oj, ot = oracle.hermite4_block_step(bx.astype(np.float64), bv.astype(np.float64), w.m_j,
+                                                        ba.astype(np.float64), bj.astype(np.float64), bt, sample,
+                                                        s * sub_dt, w.eps2)
+        assert np.all(gt[active] == s * sub_dt) and np.array_equal(gt[sample], ot[sample])
+        rest = np.setdiff1d(np.arange(n), active)
+        assert np.array_equal(gx[rest], bx[rest]) and np.array_equal(gj[rest], bj[rest]) and np.array_equal(gt[rest], bt[rest])
+        assert np.abs(gx[sample] - ox[sample]).max() < 2e-6 and np.abs(gv[sample] - ov[sample]).max() < 2e-6
+        e = oracle.error_metrics(ga[sample], oa[sample])
+        ej = oracle.error_metrics(gj[sample], oj[sample])
+        assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-3, (s, e, ej)
