@@ -239,6 +239,22 @@ def hermite4_block_step(x: np.ndarray, v: np.ndarray, m: np.ndarray, acc: np.nda
     return xx, vv, aa, jj, tt
 
 
+def block_schedule(t: np.ndarray, dt: np.ndarray):
+    """The block-step scheduler's definition (reading R20): the next block time is the earliest due time
+    t_next = min_k (t[k] + dt[k]) (one FP64 addition per particle), and the due particles are those whose due time
+    EQUALS it, in ascending index order.  Returns (t_next, active int32 [n_act]); n = 0 gives (+inf, empty).
+    Pins (tests/test_oracle_hermite_pins.py, "h9"): hand-worked cases, ties, a pure-Python loop."""
+    tt = np.asarray(t, dtype=np.float64).reshape(-1)
+    dd = np.asarray(dt, dtype=np.float64).reshape(-1)
+    if tt.shape != dd.shape:
+        raise ValueError("array lengths differ")
+    if tt.size == 0:
+        return float("inf"), np.zeros(0, dtype=np.int32)
+    due = tt + dd
+    t_next = float(due.min())
+    return t_next, np.nonzero(due == t_next)[0].astype(np.int32)
+
+
 def error_metrics(acc_test: np.ndarray, acc_ref: np.ndarray, pot_test: Optional[np.ndarray] = None,
                   pot_ref: Optional[np.ndarray] = None) -> dict:
     """Eq. (3): e_i = |a_test,i - a_ref,i| / |a_ref,i|; max and RMS over i; same for phi."""

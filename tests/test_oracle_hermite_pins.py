@@ -338,3 +338,40 @@ def test_h8_two_level_schedule_matches_an_adaptive_solver_and_is_fourth_order():
     xs, _, _, _, _ = oracle.hermite4(x0, v0, m, eps2, T / 64, 64)
     xb, _ = _block_run(x0, v0, m, eps2, T, 64, slow={0}, ratio=2)
     assert np.abs(xs - xb).max() > 1e-9
+
+
+# ----------------------------------------------------------------------------- h9: the block-step scheduler
+def test_h9_block_schedule_hand_worked_cases():
+    t = np.array([0.0, 0.5, 0.25, 0.0, 0.75])
+    dt = np.array([1.0, 0.25, 0.5, 0.5, 0.125])
+    # due times: 1.0, 0.75, 0.75, 0.5, 0.875  ->  particle 3 alone at 0.5
+    t_next, active = oracle.block_schedule(t, dt)
+    assert t_next == 0.5 and active.dtype == np.int32 and active.tolist() == [3]
+    # after particle 3 has stepped to 0.5 with dt 0.25, three particles tie at 0.75, listed in ascending order
+    t[3] = 0.5; dt[3] = 0.25
+    t_next, active = oracle.block_schedule(t, dt)
+    assert t_next == 0.75 and active.tolist() == [1, 2, 3]
+    # negative times, a single particle, everybody due, nobody there
+    assert oracle.block_schedule(np.array([-2.0, -1.5]), np.array([0.25, 0.5]))[1].tolist() == [0]
+    assert oracle.block_schedule(np.array([3.0]), np.array([0.125])) == (3.125, np.array([0], dtype=np.int32))
+    t_next, active = oracle.block_schedule(np.full(7, 1.0), np.full(7, 0.5))
+    assert t_next == 1.5 and active.tolist() == list(range(7))
+    t_next, active = oracle.block_schedule(np.zeros(0), np.zeros(0))
+    assert t_next == float("inf") and active.size == 0
+
+
+def test_h9_block_schedule_against_a_python_loop():
+    rng = np.random.default_rng(9)
+    for n in (1, 2, 33, 500):
+        level = rng.integers(0, 5, n)
+        dt = 2.0 ** -(3 + level)
+        t = dt * rng.integers(0, 4, n)                                   # clocks on each particle's own dyadic grid
+        t_next, active = oracle.block_schedule(t, dt)
+        best, who = None, []
+        for k in range(n):
+            due = float(t[k]) + float(dt[k])
+            if best is None or due < best:
+                best, who = due, [k]
+            elif due == best:
+                who.append(k)
+        assert t_next == best and active.tolist() == who
