@@ -278,6 +278,22 @@ int nb_hermite4_block_step(int64_t n, float *x, float *v, const float *m,
                            float eps2, void *stream);
 
 /*
+ * nb_block_schedule -- the scheduler's question for nb_hermite4_block_step: when is the next block step and who is due
+ * (reading R20; the paper has no integrator).  With due_k = t[k] + dt[k] (one FP64 addition):
+ *
+ *     t_next = min_k due_k          active = { k : due_k == t_next } in ASCENDING index order
+ *
+ *   t, dt       device, const, double [n]: each particle's own time and its current step
+ *   t_next_out  device, double [1]         active_out  device, int32 [n] (only the first n_act entries are written)
+ *   n_act_out   device, int32 [1]: the caller reads it back (4 bytes) to size the nb_hermite4_block_step call
+ * Index work: exact and deterministic (no floating-point atomics, ordered compaction).  n == 0: t_next = +inf, n_act = 0.
+ * Non-finite due times are never selected (all non-finite: t_next = +inf, n_act = 0).  Asynchronous on `stream`.
+ */
+int nb_block_schedule(int64_t n, const double *t, const double *dt,
+                      double *t_next_out, int32_t *active_out, int32_t *n_act_out,
+                      void *stream);
+
+/*
  * nb_force_jerk_host -- nb_force_jerk on HOST arrays: the paper's force() of Fig. A.2 with its
  * host->device and device->host copies (steps (a) and (l)) inside the call.  Blocking.
  */

@@ -17,6 +17,7 @@ from .binding import (  # noqa: F401
     force_packed,
     hermite4,
     hermite4_block_step,
+    block_schedule,
     last_launch_count,
     leapfrog_kdk,
     pack_j,

@@ -64,6 +64,8 @@ def lib() -> ctypes.CDLL:
         l.nb_hermite4.restype = ci
         l.nb_hermite4_block_step.argtypes = [i64, p, p, p, p, p, p, i64, p, ctypes.c_double, f32, p]
         l.nb_hermite4_block_step.restype = ci
+        l.nb_block_schedule.argtypes = [i64, p, p, p, p, p, p]
+        l.nb_block_schedule.restype = ci
         l.nb_plan_query.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
         l.nb_plan_query.restype = ci
         l.nb_last_launch_count.restype = i64
@@ -357,6 +359,31 @@ def hermite4_block_step(x, v, m, acc_io, jerk_io, t, active, t_now: float, eps2:
                                           active.data_ptr() if active.shape[0] else None, float(t_now), float(eps2),
                                           _stream_ptr(stream))
     _check(st, "nb_hermite4_block_step")
+
+
+def block_schedule(t, dt, t_next_out=None, active_out=None, n_act_out=None, stream=None):
+    """nb_block_schedule on CUDA float64 tensors.  Returns (t_next [1] f64, active [n] int32, n_act [1] int32), all on
+    the device and asynchronous: only active[:n_act] is meaningful."""
+    import torch
+    for a, name in ((t, "t"), (dt, "dt")):
+        if not (isinstance(a, torch.Tensor) and a.is_cuda and a.dtype == torch.float64 and a.is_contiguous() and a.dim() == 1):
+            raise TypeError(f"{name} must be a contiguous 1-D float64 CUDA tensor")
+    n = t.shape[0]
+    if dt.shape[0] != n or dt.device != t.device:
+        raise ValueError("t and dt differ in length or device")
+    if t_next_out is None:
+        t_next_out = torch.empty((1,), dtype=torch.float64, device=t.device)
+    if active_out is None:
+        active_out = torch.empty((n,), dtype=torch.int32, device=t.device)
+    if n_act_out is None:
+        n_act_out = torch.empty((1,), dtype=torch.int32, device=t.device)
+    if active_out.dtype != torch.int32 or active_out.numel() < n or not active_out.is_contiguous():
+        raise ValueError("active_out must be a contiguous int32 tensor with at least n entries")
+    with torch.cuda.device(t.device):
+        st = lib().nb_block_schedule(n, t.data_ptr() if n else None, dt.data_ptr() if n else None, t_next_out.data_ptr(),
+                                     active_out.data_ptr() if n else None, n_act_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_block_schedule")
+    return t_next_out, active_out, n_act_out
 
 
 def plan_query(n_i: int, n_j: int, sm_count: int = 148) -> dict:

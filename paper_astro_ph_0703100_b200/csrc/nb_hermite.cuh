@@ -23,6 +23,7 @@
 // and masks only the listed j-segments.  An unmasked coincident pair would add m dv / eps^3 to the
 // jerk, so unlike the plain force there is no speculative mode here.
 #pragma once
+#include <math_constants.h>
 #include "nb_kernels.cuh"
 
 namespace nb {
@@ -465,6 +466,112 @@ __global__ void __launch_bounds__(256) nb_block_correct_kernel(float* __restrict
         j0[k] = j_new;
     }
     t[i] = t_now;
+}
+
+// ---------------------------------------------------------------- block-step scheduler: who is due next (index work, exact)
+// t_next = min_k (t[k] + dt[k]);  active = ascending { k : t[k] + dt[k] == t_next }.  One FP64 add per particle, the same
+// on both passes, so the equality is exact.  A CTA covers kSchedTile consecutive particles, a thread kSchedItems of them.
+constexpr int kSchedThreads = 256, kSchedItems = 4, kSchedTile = kSchedThreads * kSchedItems;
+
+__global__ void __launch_bounds__(kSchedThreads) nb_sched_min_kernel(const double* __restrict__ t, const double* __restrict__ dt,
+                                                                    int n, double* __restrict__ block_min) {
+    __shared__ double warp_min[kSchedThreads / 32];
+    const size_t base = (size_t)blockIdx.x * kSchedTile + (size_t)threadIdx.x * kSchedItems;
+    double lo = CUDART_INF;
+#pragma unroll
+    for (int e = 0; e < kSchedItems; ++e)
+        if (base + e < (size_t)n) lo = fmin(lo, __dadd_rn(t[base + e], dt[base + e]));
+    for (int o = 16; o > 0; o >>= 1) lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    if ((threadIdx.x & 31) == 0) warp_min[threadIdx.x >> 5] = lo;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < kSchedThreads / 32; ++w) lo = fmin(lo, warp_min[w]);
+        block_min[blockIdx.x] = lo;
+    }
+}
+// one CTA: the minimum of the CTA minima (+inf when there is no particle)
+__global__ void __launch_bounds__(1024) nb_sched_final_min_kernel(const double* __restrict__ block_min, int n_blocks,
+                                                                  double* __restrict__ t_next) {
+    __shared__ double warp_min[32];
+    double lo = CUDART_INF;
+    for (int b = threadIdx.x; b < n_blocks; b += 1024) lo = fmin(lo, block_min[b]);
+    for (int o = 16; o > 0; o >>= 1) lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    if ((threadIdx.x & 31) == 0) warp_min[threadIdx.x >> 5] = lo;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 32; ++w) lo = fmin(lo, warp_min[w]);
+        *t_next = lo;
+    }
+}
+// how many of a CTA's particles are due
+__global__ void __launch_bounds__(kSchedThreads) nb_sched_count_kernel(const double* __restrict__ t, const double* __restrict__ dt,
+                                                                      int n, const double* __restrict__ t_next,
+                                                                      int* __restrict__ counts) {
+    __shared__ int total;
+    if (threadIdx.x == 0) total = 0;
+    __syncthreads();
+    const double due = *t_next;
+    const size_t base = (size_t)blockIdx.x * kSchedTile + (size_t)threadIdx.x * kSchedItems;
+    int c = 0;
+#pragma unroll
+    for (int e = 0; e < kSchedItems; ++e)
+        if (base + e < (size_t)n) c += (__dadd_rn(t[base + e], dt[base + e]) == due);
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(&total, c);          // integer sum: the order does not matter
+    __syncthreads();
+    if (threadIdx.x == 0) counts[blockIdx.x] = total;
+}
+// one CTA: exclusive scan of the CTA counts in place, the grand total to n_act
+__global__ void __launch_bounds__(1024) nb_sched_scan_kernel(int* __restrict__ counts, int n_blocks, int* __restrict__ n_act) {
+    __shared__ int buf[1024];
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int c0 = 0; c0 < n_blocks; c0 += 1024) {
+        const int b = c0 + threadIdx.x;
+        const int mine = b < n_blocks ? counts[b] : 0;
+        buf[threadIdx.x] = mine;
+        __syncthreads();
+        for (int o = 1; o < 1024; o <<= 1) {                          // Hillis-Steele inclusive scan
+            const int add = threadIdx.x >= o ? buf[threadIdx.x - o] : 0;
+            __syncthreads();
+            buf[threadIdx.x] += add;
+            __syncthreads();
+        }
+        const int before = carry;
+        if (b < n_blocks) counts[b] = before + buf[threadIdx.x] - mine;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry = before + buf[1023];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *n_act = carry;
+}
+// the due particles' indices, ascending: CTA offset + position inside the CTA
+__global__ void __launch_bounds__(kSchedThreads) nb_sched_scatter_kernel(const double* __restrict__ t, const double* __restrict__ dt,
+                                                                        int n, const double* __restrict__ t_next,
+                                                                        const int* __restrict__ offsets, int* __restrict__ active) {
+    __shared__ int warp_sum[kSchedThreads / 32];
+    const double due = *t_next;
+    const size_t base = (size_t)blockIdx.x * kSchedTile + (size_t)threadIdx.x * kSchedItems;
+    bool flag[kSchedItems];
+    int c = 0;
+#pragma unroll
+    for (int e = 0; e < kSchedItems; ++e) {
+        flag[e] = base + e < (size_t)n && __dadd_rn(t[base + e], dt[base + e]) == due;
+        c += flag[e];
+    }
+    int incl = c;                                                      // inclusive scan over the warp
+    for (int o = 1; o < 32; o <<= 1) {
+        const int up = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((threadIdx.x & 31) >= o) incl += up;
+    }
+    if ((threadIdx.x & 31) == 31) warp_sum[threadIdx.x >> 5] = incl;
+    __syncthreads();
+    int pos = offsets[blockIdx.x] + incl - c;
+    for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) pos += warp_sum[w];
+#pragma unroll
+    for (int e = 0; e < kSchedItems; ++e)
+        if (flag[e]) active[pos++] = (int)(base + e);
 }
 
 }  // namespace nb

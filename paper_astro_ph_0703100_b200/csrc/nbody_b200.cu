@@ -1008,6 +1008,50 @@ int nb_hermite4_block_step(int64_t n, float* x, float* v, const float* m, float*
     return NB_OK;
 }
 
+int nb_block_schedule(int64_t n, const double* t, const double* dt, double* t_next_out, int32_t* active_out,
+                      int32_t* n_act_out, void* stream_) {
+    t_launches = 0;
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (bad_count(n) || !t_next_out || !n_act_out) return NB_ERR_INVALID_VALUE;
+    if (n > 0 && (!t || !dt || !active_out)) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    Workspace* ws;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        ws = &g_ws[std::make_pair(dev, stream)];
+    }
+    const int n_blocks = (int)((n + nb::kSchedTile - 1) / nb::kSchedTile);
+    // scratch: [n_blocks] double CTA minima | [n_blocks] int CTA counts -> offsets
+    rc = ensure(&ws->tiles, &ws->tiles_bytes, (size_t)(n_blocks + 1) * (sizeof(double) + sizeof(int)), stream);
+    if (rc != NB_OK) return rc;
+    double* block_min = reinterpret_cast<double*>(ws->tiles);
+    int* counts = reinterpret_cast<int*>(block_min + n_blocks + 1);
+    if (n_blocks > 0) {
+        nb::nb_sched_min_kernel<<<n_blocks, nb::kSchedThreads, 0, stream>>>(t, dt, (int)n, block_min);
+        NB_CUDA(cudaGetLastError());
+        ++t_launches;
+    }
+    nb::nb_sched_final_min_kernel<<<1, 1024, 0, stream>>>(block_min, n_blocks, t_next_out);
+    NB_CUDA(cudaGetLastError());
+    if (n_blocks > 0) {
+        nb::nb_sched_count_kernel<<<n_blocks, nb::kSchedThreads, 0, stream>>>(t, dt, (int)n, t_next_out, counts);
+        NB_CUDA(cudaGetLastError());
+        ++t_launches;
+    }
+    nb::nb_sched_scan_kernel<<<1, 1024, 0, stream>>>(counts, n_blocks, n_act_out);
+    NB_CUDA(cudaGetLastError());
+    if (n_blocks > 0) {
+        nb::nb_sched_scatter_kernel<<<n_blocks, nb::kSchedThreads, 0, stream>>>(t, dt, (int)n, t_next_out, counts, active_out);
+        NB_CUDA(cudaGetLastError());
+        ++t_launches;
+    }
+    t_launches += 2;
+    return NB_OK;
+}
+
 int nb_plan_query(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]) {
     if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
     const nb::Plan p = nb::make_plan(n_i, n_j, sm_count);
