@@ -35,7 +35,7 @@ CONFIG_INDEX = {"C0": 0, "C1": 1, "C2": 2, "C3": 3, "C4": 4}
 L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/r01_ncu_full.md); null for configs / ops without a capture
-NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 71.0e6, "jerk": 105.4e6, "batched": 248.5e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 71.0e6, "jerk": 105.4e6, "batched": 248.5e6, "block": 5.0e6}   # block: mean of 2 launches
 
 
 def load_peaks():
