@@ -31,6 +31,15 @@ def start(nb, w):
     return (x, v, m, acc, jerk), (w.x_j.astype(np.float64), w.v.astype(np.float64), ra, rj)
 
 
+def start_shared(w):
+    """One FP32 start state for both sides: a, j come from the oracle, rounded to FP32 and uploaded -- no value computed
+    by the CUDA path enters the oracle."""
+    ra, rj, _ = oracle.force_jerk(w.x_j, w.v, w.x_j, w.v, w.m_j, w.eps2)
+    a32, j32 = ra.astype(np.float32), rj.astype(np.float32)
+    device = (dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j), dev(a32), dev(j32))
+    return device, (w.x_j.astype(np.float64), w.v.astype(np.float64), a32.astype(np.float64), j32.astype(np.float64))
+
+
 def host(*ts):
     import torch
     torch.cuda.synchronize()
@@ -42,7 +51,7 @@ def test_one_block_step_matches_oracle(nb, n, n_act, seed):
     """Particles sit at different own times (three levels); a ragged, shuffled active set is advanced to t_now."""
     import torch
     w = wl.plummer_workload(n, 1.0 / 64, seed=10 + seed, with_velocities=True)
-    (x, v, m, acc, jerk), (xr, vr, ar, jr) = start(nb, w)
+    (x, v, m, acc, jerk), (xr, vr, ar, jr) = start_shared(w)
     dt = 1.0 / 256
     t0 = -dt * wl.block_levels(n, seed).astype(np.float64)             # own times 0, -dt, -2 dt; t_now = dt
     active = np.random.default_rng(seed).permutation(n)[:n_act].astype(np.int32)
@@ -50,9 +59,7 @@ def test_one_block_step_matches_oracle(nb, n, n_act, seed):
     before = host(x, v, acc, jerk)
     nb.hermite4_block_step(x, v, m, acc, jerk, t, dev(active), dt, w.eps2)
     gx, gv, ga, gj, gt = host(x, v, acc, jerk, t)
-    # the oracle starts from the SAME FP32 a, j the device holds (its own a, j differ by FP32 rounding only)
-    ox, ov, oa, oj, ot = oracle.hermite4_block_step(xr, vr, w.m_j, before[2].astype(np.float64),
-                                                    before[3].astype(np.float64), t0, active, dt, w.eps2)
+    ox, ov, oa, oj, ot = oracle.hermite4_block_step(xr, vr, w.m_j, ar, jr, t0, active, dt, w.eps2)
     assert np.array_equal(gt, ot)                                                   # clocks: exact
     rest = np.setdiff1d(np.arange(n), active)
     for g, b in zip((gx, gv, ga, gj), before):
@@ -116,32 +123,31 @@ def test_three_level_schedule_matches_oracle_and_conserves_energy(nb, n, sub_ste
     assert abs(e1 - e0) / abs(e0) < 1e-5
 
 
-def test_bench_size_block_cycle_sampled_against_oracle(nb):
+def test_bench_size_block_steps_sampled_against_oracle(nb):
     """bench.py --op block's own configuration (C4's particles, N = 65536, workloads.block_levels(seed=4), list-mode
-    force + jerk on n_act x n >= 2^31 pairs): each of the cycle's four block steps is checked on 384 sampled due
-    particles -- the oracle advances only the sample (a due particle's update does not depend on who else is due)
-    from the device's own state before the step."""
+    force + jerk on n_act x n >= 2^31 pairs): each of the cycle's four due sets is advanced by one block step from the
+    same oracle-made FP32 start state with staggered clocks, and checked on 384 sampled due particles -- the oracle
+    advances only the sample (a due particle's update does not depend on who else is due)."""
     import torch
     w = wl.config(4)
     n = w.n_j
     level = wl.block_levels(n, seed=4)
     sub_dt = w.dt / 4
-    (x, v, m, acc, jerk), _ = start(nb, w)
-    t = dev(np.zeros(n))
+    t0 = -sub_dt * ((1 << level) - 1).astype(np.float64)                 # own times 0, -dt/4, -3 dt/4; t_now = dt/4
+    (x0, v0, m, a0, j0), (xr, vr, ar, jr) = start_shared(w)
     rng = np.random.default_rng(0)
     for s in range(1, 5):
         active = np.nonzero(s % (1 << level) == 0)[0].astype(np.int32)
-        assert active.size * n >= 2 ** 31 or s % 2 == 1
-        bx, bv, ba, bj, bt = host(x, v, acc, jerk, t)
-        nb.hermite4_block_step(x, v, m, acc, jerk, t, dev(active), s * sub_dt, w.eps2)
+        assert active.size * n >= 2 ** 30
+        x, v, acc, jerk, t = x0.clone(), v0.clone(), a0.clone(), j0.clone(), dev(t0.copy())
+        bx, bv, ba, bj = host(x, v, acc, jerk)
+        nb.hermite4_block_step(x, v, m, acc, jerk, t, dev(active), sub_dt, w.eps2)
         gx, gv, ga, gj, gt = host(x, v, acc, jerk, t)
         sample = np.sort(rng.choice(active, 384, replace=False)).astype(np.int32)
-        ox, ov, oa, oj, ot = oracle.hermite4_block_step(bx.astype(np.float64), bv.astype(np.float64), w.m_j,
-                                                        ba.astype(np.float64), bj.astype(np.float64), bt, sample,
-                                                        s * sub_dt, w.eps2)
-        assert np.all(gt[active] == s * sub_dt) and np.array_equal(gt[sample], ot[sample])
+        ox, ov, oa, oj, ot = oracle.hermite4_block_step(xr, vr, w.m_j, ar, jr, t0, sample, sub_dt, w.eps2)
+        assert np.all(gt[active] == sub_dt) and np.array_equal(gt[sample], ot[sample])
         rest = np.setdiff1d(np.arange(n), active)
-        assert np.array_equal(gx[rest], bx[rest]) and np.array_equal(gj[rest], bj[rest]) and np.array_equal(gt[rest], bt[rest])
+        assert np.array_equal(gx[rest], bx[rest]) and np.array_equal(gj[rest], bj[rest]) and np.array_equal(gt[rest], t0[rest])
         assert np.abs(gx[sample] - ox[sample]).max() < 2e-6 and np.abs(gv[sample] - ov[sample]).max() < 2e-6
         e = oracle.error_metrics(ga[sample], oa[sample])
         ej = oracle.error_metrics(gj[sample], oj[sample])
