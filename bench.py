@@ -656,6 +656,20 @@ def main():
                                    "note": "one captured nb_force call replayed 200x back to back, L2 warm"}
         if args.op == "block":
             out["block_steps_per_s"] = BLOCK_SUB_STEPS * args.steps / (total_ms * 1e-3)
+            # the scheduler's share when the due sets are not precomputed: nb_block_schedule + the 4-byte read-back of n_act
+            level = wl.block_levels(prob.w.n_j, seed=4)
+            dt_k = torch.from_numpy(prob.sub_dt * 2.0 ** level.astype(np.float64)).cuda()
+            for _ in range(3):
+                _, _, n_act = nb.block_schedule(prob.dev[5], dt_k)
+                n_act.item()
+            reps = 50
+            t0 = time.perf_counter()
+            for _ in range(reps):
+                _, _, n_act = nb.block_schedule(prob.dev[5], dt_k)
+                n_due = int(n_act.item())
+            out["scheduler"] = {"us_per_call": 1e6 * (time.perf_counter() - t0) / reps, "n_due": n_due,
+                                "api": "nb_block_schedule (5 launches) + 4-byte read-back of n_act, host wall clock",
+                                "share_of_a_block_step": (time.perf_counter() - t0) / reps / (total_ms * 1e-3 / (BLOCK_SUB_STEPS * args.steps))}
         if args.op == "hermite":
             out["hermite_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
         if args.op in ("leapfrog", "hermite") and not args.no_cpu_baseline:
