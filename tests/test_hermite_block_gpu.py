@@ -152,3 +152,78 @@ def test_bench_size_block_steps_sampled_against_oracle(nb):
         e = oracle.error_metrics(ga[sample], oa[sample])
         ej = oracle.error_metrics(gj[sample], oj[sample])
         assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-3, (s, e, ej)
+
+
+def test_order_of_the_active_list_does_not_matter_bitwise(nb):
+    """A due particle's sum over j runs in a fixed order wherever the particle sits in the i-set (P11 of SURVEY 8.1.3)."""
+    n = 3000
+    w = wl.plummer_workload(n, 1.0 / 64, seed=40, with_velocities=True)
+    rng = np.random.default_rng(1)
+    active = np.sort(rng.permutation(n)[:1111]).astype(np.int32)
+    shuffled = rng.permutation(active).astype(np.int32)
+    t0 = -(1.0 / 256) * wl.block_levels(n, 8).astype(np.float64)
+    outs = []
+    for lst in (active, shuffled):
+        (x, v, m, acc, jerk), _ = start_shared(w)
+        t = dev(t0.copy())
+        nb.hermite4_block_step(x, v, m, acc, jerk, t, dev(lst), 1.0 / 256, w.eps2)
+        outs.append(host(x, v, acc, jerk, t))
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
+
+
+def test_coincident_particles_and_zero_softening(nb):
+    """eps2 = 0 with exact duplicates among the particles (reading R1: a pair at zero distance adds nothing): finite
+    results that match the oracle, for a due particle whose twin is due too and for one whose twin is only predicted."""
+    n = 900
+    w = wl.plummer_workload(n, 1.0 / 64, seed=41, with_velocities=True)
+    x0, v0 = w.x_j.copy(), w.v.copy()
+    x0[500:520], v0[500:520] = x0[0:20], v0[0:20]                       # twins: same position and velocity
+    ra, rj, _ = oracle.force_jerk(x0, v0, x0, v0, w.m_j, 0.0)
+    a32, j32 = ra.astype(np.float32), rj.astype(np.float32)
+    assert np.array_equal(a32[500:520], a32[0:20])                       # so the twins stay together when predicted
+    x, v, m, acc, jerk = dev(x0), dev(v0), dev(w.m_j), dev(a32), dev(j32)
+    t = dev(np.zeros(n))
+    active = np.concatenate([np.arange(0, 20), np.arange(500, 510), np.arange(600, 700)]).astype(np.int32)
+    nb.hermite4_block_step(x, v, m, acc, jerk, t, dev(active), 1.0 / 512, 0.0)
+    gx, gv, ga, gj = host(x, v, acc, jerk)
+    ox, ov, oa, oj, _ = oracle.hermite4_block_step(x0, v0, w.m_j, a32, j32, np.zeros(n), active, 1.0 / 512, 0.0)
+    assert np.isfinite(ga).all() and np.isfinite(gj).all()
+    assert np.abs(gx - ox).max() < 2e-6 and np.abs(gv - ov).max() < 2e-6
+    e = oracle.error_metrics(ga[active], oa[active])
+    ej = oracle.error_metrics(gj[active], oj[active])
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-4
+
+
+def test_runs_on_a_side_stream_and_in_a_cuda_graph(nb):
+    """Asynchronous on the caller's stream; capturable (no synchronisation, no allocation once the workspace is warm)."""
+    import torch
+    n = 2048
+    w = wl.plummer_workload(n, 1.0 / 64, seed=42, with_velocities=True)
+    active = dev(np.arange(0, n, 3, dtype=np.int32))
+    (x, v, m, acc, jerk), _ = start_shared(w)
+    t = dev(np.zeros(n))
+    nb.hermite4_block_step(x, v, m, acc, jerk, t, active, 1.0 / 256, w.eps2)
+    ref = host(x, v, acc, jerk, t)
+    side = torch.cuda.Stream()
+    (x, v, m, acc, jerk), _ = start_shared(w)
+    t = dev(np.zeros(n))
+    keep = [a.clone() for a in (x, v, acc, jerk, t)]
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        nb.hermite4_block_step(x, v, m, acc, jerk, t, active, 1.0 / 256, w.eps2, stream=side)      # warms this stream's workspace
+        side.synchronize()
+        for a, b in zip(host(x, v, acc, jerk, t), ref):
+            assert np.array_equal(a, b)
+        for a, k in zip((x, v, acc, jerk, t), keep):
+            a.copy_(k)
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            nb.hermite4_block_step(x, v, m, acc, jerk, t, active, 1.0 / 256, w.eps2, stream=side)
+        for a, k in zip((x, v, acc, jerk, t), keep):                   # capture does not execute: restore and replay once
+            a.copy_(k)
+        g.replay()
+        side.synchronize()
+    for a, b in zip(host(x, v, acc, jerk, t), ref):
+        assert np.array_equal(a, b)
