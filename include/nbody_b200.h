@@ -270,7 +270,7 @@ int nb_hermite4(int64_t n, float *x, float *v, const float *m,
  *   active    device, const, int32 [n_act]: DISTINCT indices in [0, n), any order; not validated on the device
  *             (out-of-range or repeated indices: undefined results).  n_act == 0: success, nothing is touched
  *   t_now     the block time.  Who is due and each particle's next step are the caller's business.
- * Asynchronous on `stream`; 3 small launches + those of one nb_force_jerk(n_act, n) without phi.
+ * Asynchronous on `stream`; 2 small launches + those of one nb_force_jerk(n_act, n) without phi.
  */
 int nb_hermite4_block_step(int64_t n, float *x, float *v, const float *m,
                            float *acc_io, float *jerk_io, double *t,

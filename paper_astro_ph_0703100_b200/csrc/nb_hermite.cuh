@@ -410,38 +410,50 @@ __global__ void __launch_bounds__(256) nb_hermite_correct_kernel(float* __restri
 // ---------------------------------------------------------------- block (individual) time steps: one block step, row f4
 // Every particle holds (x, v, a, j) at its own time t[k] (FP64; the interval h = t_now - t[k] is rounded to FP32 once).
 // predict everybody to t_now (same Horner form as the shared-step kernel, h per particle) and pack the j records:
-__global__ void __launch_bounds__(256) nb_block_predict_pack_kernel(const float* __restrict__ x, const float* __restrict__ v,
-                                                                    const float* __restrict__ a, const float* __restrict__ j,
-                                                                    const float* __restrict__ m, const double* __restrict__ t,
-                                                                    double t_now, float* __restrict__ xp, float* __restrict__ vp,
-                                                                    float4* __restrict__ jp, int n) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+// Predicted state of particle i at t_now (shared by both halves of the kernel below, so the due particles' i-records
+// are bitwise the j-records of the same particles: the coincidence test sees each particle's own record).
+__device__ __forceinline__ void nb_block_predict(const float* __restrict__ x, const float* __restrict__ v,
+                                                 const float* __restrict__ a, const float* __restrict__ j,
+                                                 const double* __restrict__ t, double t_now, int i, float px[3], float pv[3]) {
     const float dt = (float)(t_now - t[i]);
-    float px[3], pv[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const size_t k = 3 * (size_t)i + c;
         const float aa = a[k], jj = j[k], vv = v[k];
         px[c] = fmaf(fmaf(fmaf(jj, dt * (1.0f / 3.0f), aa), dt * 0.5f, vv), dt, x[k]);
         pv[c] = fmaf(fmaf(jj, dt * 0.5f, aa), dt, vv);
-        xp[k] = px[c];
-        vp[k] = pv[c];
     }
-    jp[2 * (size_t)i + 0] = make_float4(px[0], px[1], px[2], m[i]);
-    jp[2 * (size_t)i + 1] = make_float4(pv[0], pv[1], pv[2], 0.0f);
 }
-// the i-set of the block step: predicted state of the active particles, in the order of active[]
-__global__ void __launch_bounds__(256) nb_block_gather_kernel(const float* __restrict__ xp, const float* __restrict__ vp,
-                                                              const int* __restrict__ active, int n_act,
-                                                              float* __restrict__ xi, float* __restrict__ vi) {
-    const int q = blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= n_act) return;
-    const size_t k = 3 * (size_t)active[q];
+// CTAs [0, j_blocks): everybody's packed j record (and xp, vp); CTAs [j_blocks, ...): the i-set = predicted state of the
+// due particles in the order of active[] (one launch instead of a prediction and a gather)
+__global__ void __launch_bounds__(256) nb_block_predict_pack_kernel(const float* __restrict__ x, const float* __restrict__ v,
+                                                                    const float* __restrict__ a, const float* __restrict__ j,
+                                                                    const float* __restrict__ m, const double* __restrict__ t,
+                                                                    double t_now, float* __restrict__ xp, float* __restrict__ vp,
+                                                                    float4* __restrict__ jp, int n, int j_blocks,
+                                                                    const int* __restrict__ active, int n_act,
+                                                                    float* __restrict__ xi, float* __restrict__ vi) {
+    float px[3], pv[3];
+    if ((int)blockIdx.x < j_blocks) {
+        const int i = blockIdx.x * blockDim.x + threadIdx.x;
+        if (i >= n) return;
+        nb_block_predict(x, v, a, j, t, t_now, i, px, pv);
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        xi[3 * (size_t)q + c] = xp[k + c];
-        vi[3 * (size_t)q + c] = vp[k + c];
+        for (int c = 0; c < 3; ++c) {
+            xp[3 * (size_t)i + c] = px[c];
+            vp[3 * (size_t)i + c] = pv[c];
+        }
+        jp[2 * (size_t)i + 0] = make_float4(px[0], px[1], px[2], m[i]);
+        jp[2 * (size_t)i + 1] = make_float4(pv[0], pv[1], pv[2], 0.0f);
+    } else {
+        const int q = ((int)blockIdx.x - j_blocks) * blockDim.x + threadIdx.x;
+        if (q >= n_act) return;
+        nb_block_predict(x, v, a, j, t, t_now, active[q], px, pv);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            xi[3 * (size_t)q + c] = px[c];
+            vi[3 * (size_t)q + c] = pv[c];
+        }
     }
 }
 // correct the active particles over their own interval and advance their clocks; nobody else is written

@@ -995,16 +995,16 @@ int nb_hermite4_block_step(int64_t n, float* x, float* v, const float* m, float*
     if (rc != NB_OK) return rc;
     const int threads = 256;
     const unsigned ablocks = (unsigned)((n_act + threads - 1) / threads);
-    nb::nb_block_predict_pack_kernel<<<(unsigned)((n + threads - 1) / threads), threads, 0, stream>>>(
-        x, v, acc_io, jerk_io, m, t, t_now, xp, vp, reinterpret_cast<float4*>(ws->jp2), (int)n);
-    NB_CUDA(cudaGetLastError());
-    nb::nb_block_gather_kernel<<<ablocks, threads, 0, stream>>>(xp, vp, active, (int)n_act, xi, vi);
+    const unsigned jblocks = (unsigned)((n + threads - 1) / threads);
+    nb::nb_block_predict_pack_kernel<<<jblocks + ablocks, threads, 0, stream>>>(
+        x, v, acc_io, jerk_io, m, t, t_now, xp, vp, reinterpret_cast<float4*>(ws->jp2), (int)n, (int)jblocks, active,
+        (int)n_act, xi, vi);
     NB_CUDA(cudaGetLastError());
     rc = force_jerk_impl(n_act, xi, vi, n, xp, vp, m, eps2, a1, j1, nullptr, stream, true);
     if (rc != NB_OK) return rc;
     nb::nb_block_correct_kernel<<<ablocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, t, active, a1, j1, t_now, (int)n_act);
     NB_CUDA(cudaGetLastError());
-    t_launches += 3;
+    t_launches += 2;
     return NB_OK;
 }
 
