@@ -227,3 +227,31 @@ def test_runs_on_a_side_stream_and_in_a_cuda_graph(nb):
         side.synchronize()
     for a, b in zip(host(x, v, acc, jerk, t), ref):
         assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("case", range(16))
+def test_randomised_block_steps(nb, case):
+    """Seeded sweep over sizes, due-set sizes, softening (incl. 0), clock staggering and the block time."""
+    rng = np.random.default_rng(1000 + case)
+    n = int(rng.integers(2, 6000))
+    n_act = int(rng.integers(1, n + 1)) if case % 4 else max(1, n // int(rng.integers(20, 200)))
+    eps = [0.0, 1.0 / 1024, 1.0 / 64, 0.5][case % 4]
+    w = wl.plummer_workload(n, 1.0 / 64, seed=2000 + case, with_velocities=True)
+    eps2 = np.float32(eps * eps)
+    ra, rj, _ = oracle.force_jerk(w.x_j, w.v, w.x_j, w.v, w.m_j, float(eps2))
+    a32, j32 = ra.astype(np.float32), rj.astype(np.float32)
+    dt = 2.0 ** -float(rng.integers(7, 11))
+    t_now = dt * float(rng.integers(1, 9))
+    t0 = t_now - dt * (1 << wl.block_levels(n, 3000 + case, n_levels=int(rng.integers(1, 5)))).astype(np.float64)
+    active = rng.permutation(n)[:n_act].astype(np.int32)
+    x, v, m, acc, jerk, t = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j), dev(a32), dev(j32), dev(t0.copy())
+    nb.hermite4_block_step(x, v, m, acc, jerk, t, dev(active), t_now, float(eps2))
+    gx, gv, ga, gj, gt = host(x, v, acc, jerk, t)
+    ox, ov, oa, oj, ot = oracle.hermite4_block_step(w.x_j, w.v, w.m_j, a32, j32, t0, active, t_now, float(eps2))
+    assert np.array_equal(gt, ot)
+    rest = np.setdiff1d(np.arange(n), active)
+    assert np.array_equal(gx[rest], w.x_j[rest]) and np.array_equal(ga[rest], a32[rest]) and np.array_equal(gj[rest], j32[rest])
+    assert np.abs(gx - ox).max() < 4e-6 and np.abs(gv - ov).max() < 4e-6
+    e = oracle.error_metrics(ga[active], oa[active])
+    ej = oracle.error_metrics(gj[active], oj[active])
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-4, (n, n_act, eps, e, ej)
