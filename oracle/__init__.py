@@ -6,7 +6,8 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 
 The arithmetic lives in ``nbody_oracle.c`` (plain C, double precision; see its header for the
 passages of PAPER.md each line follows).  This file only builds that C file with gcc and marshals
-numpy arrays into it through ctypes.
+numpy arrays into it through ctypes -- with one exception, ``block_schedule``, whose definition (a minimum
+and an equality test, index work) is written out in numpy below.  Parity unpinned: nothing in this package.
 """
 from __future__ import annotations
 
