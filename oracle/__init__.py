@@ -6,8 +6,9 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 
 The arithmetic lives in ``nbody_oracle.c`` (plain C, double precision; see its header for the
 passages of PAPER.md each line follows).  This file only builds that C file with gcc and marshals
-numpy arrays into it through ctypes -- with one exception, ``block_schedule``, whose definition (a minimum
-and an equality test, index work) is written out in numpy below.  Parity unpinned: nothing in this package.
+numpy arrays into it through ctypes -- with two exceptions written out in numpy below: ``block_schedule`` (a minimum and
+an equality test, index work) and ``block_step_size`` (a criterion that feeds an integer decision, so it is
+defined in the kernel's precision, FP32, one rounded operation at a time).  Parity unpinned: nothing in this package.
 """
 from __future__ import annotations
 
@@ -254,6 +255,42 @@ def block_schedule(t: np.ndarray, dt: np.ndarray):
     due = tt + dd
     t_next = float(due.min())
     return t_next, np.nonzero(due == t_next)[0].astype(np.int32)
+
+
+def block_step_size(a0: np.ndarray, j0: np.ndarray, a1: np.ndarray, j1: np.ndarray, h: np.ndarray, eta: float) -> np.ndarray:
+    """The Aarseth step-size criterion of the block Hermite scheme (textbook, reading R20; Makino &
+    Aarseth 1992), from the two evaluations (a0, j0) at t and (a1, j1) at t + h of one particle:
+
+        a2 = (-6 (a0 - a1) - h (4 j0 + 2 j1)) / h^2        a3 = (12 (a0 - a1) + 6 h (j0 + j1)) / h^3     (at t)
+        a2' = a2 + h a3                                     (second derivative at t + h; a3 is constant)
+        dt = sqrt( eta (|a1| |a2'| + |j1|^2) / (|j1| |a3| + |a2'|^2) )
+
+    The result feeds an integer decision (the block level), so the definition fixes the precision and the order:
+    every operation below is ONE IEEE FP32 operation (numpy float32 element-wise), in the order written; norms are
+    sqrt((x x + y y) + z z).  Returns dt, float32 [n].  Pins (tests/test_oracle_hermite_pins.py, "h10"): cubic
+    a(t) (the interpolant is exact), the circular orbit's sqrt(eta)/omega with its h^2 convergence."""
+    f = np.float32
+    a0, j0, a1, j1 = (np.ascontiguousarray(z, dtype=f).reshape(-1, 3) for z in (a0, j0, a1, j1))
+    h = np.ascontiguousarray(h, dtype=f).reshape(-1, 1)
+    eta = f(eta)
+    da = a0 - a1
+    s1 = f(4) * j0 + f(2) * j1
+    h2 = h * h
+    a2 = -(f(6) * da + h * s1) / h2
+    s2 = j0 + j1
+    h3 = h2 * h
+    a3 = (f(12) * da + (f(6) * h) * s2) / h3
+    a2 = a2 + h * a3
+
+    def sq(z):
+        return (z[:, 0] * z[:, 0] + z[:, 1] * z[:, 1]) + z[:, 2] * z[:, 2]
+    a1sq, j1sq, a2sq, a3sq = sq(a1), sq(j1), sq(a2), sq(a3)
+    top = np.sqrt(a1sq) * np.sqrt(a2sq) + j1sq
+    bot = np.sqrt(j1sq) * np.sqrt(a3sq) + a2sq
+    with np.errstate(divide="ignore", invalid="ignore"):
+        out = np.sqrt(eta * (top / bot))
+    assert out.dtype == np.float32
+    return out
 
 
 def error_metrics(acc_test: np.ndarray, acc_ref: np.ndarray, pot_test: Optional[np.ndarray] = None,

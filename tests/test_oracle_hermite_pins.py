@@ -375,3 +375,56 @@ def test_h9_block_schedule_against_a_python_loop():
             elif due == best:
                 who.append(k)
         assert t_next == best and active.tolist() == who
+
+
+# ----------------------------------------------------------------------------- h10: the step-size criterion
+def test_h10_cubic_acceleration_is_interpolated_exactly():
+    """a(t) = c0 + c1 t + c2 t^2 + c3 t^3 with small integer coefficients and h = 2: every FP32 operation of the
+    interpolation is exact, so dt must be the criterion evaluated on the true derivatives at t + h."""
+    rng = np.random.default_rng(10)
+    c = rng.integers(-4, 5, size=(4, 50, 3)).astype(np.float64)
+    c[3][c[3] == 0] = 1.0
+    t0, h = 1.0, 2.0
+    def acc(t): return c[0] + c[1] * t + c[2] * t ** 2 + c[3] * t ** 3
+    def jerk(t): return c[1] + 2 * c[2] * t + 3 * c[3] * t ** 2
+    a0, j0, a1, j1 = acc(t0), jerk(t0), acc(t0 + h), jerk(t0 + h)
+    a2 = 2 * c[2] + 6 * c[3] * (t0 + h)
+    a3 = 6 * c[3]
+    nrm = lambda z: np.sqrt((z * z).sum(1))
+    eta = 0.02
+    want = np.sqrt(eta * (nrm(a1) * nrm(a2) + nrm(j1) ** 2) / (nrm(j1) * nrm(a3) + nrm(a2) ** 2))
+    got = oracle.block_step_size(a0, j0, a1, j1, np.full(50, h), eta)
+    assert got.dtype == np.float32
+    np.testing.assert_allclose(got, want, rtol=1e-6)
+
+
+def test_h10_circular_orbit_gives_sqrt_eta_over_omega():
+    """r(t) on a circle of radius R with angular speed w: |a| = R w^2, |j| = R w^3, |a2| = R w^4, |a3| = R w^5, so the
+    criterion is sqrt(eta) / w whatever R; the interpolated derivatives carry an O((w h)^2) error."""
+    eta = 0.01
+    errs = []
+    for h in (0.25, 0.125):
+        w_, R = 1.5, 2.0
+        def state(t):
+            cs, sn = np.cos(w_ * t), np.sin(w_ * t)
+            a = -R * w_ ** 2 * np.array([[cs, sn, 0.0]])
+            j = -R * w_ ** 3 * np.array([[-sn, cs, 0.0]])
+            return a, j
+        a0, j0 = state(0.3)
+        a1, j1 = state(0.3 + h)
+        got = float(oracle.block_step_size(a0, j0, a1, j1, np.array([h]), eta)[0])
+        errs.append(abs(got * w_ / np.sqrt(eta) - 1.0))
+    assert errs[1] < 5e-3 and 3.0 < errs[0] / errs[1] < 5.0
+
+
+def test_h10_scaling_laws():
+    """dt scales with sqrt(eta); rescaling time by s (a -> a/s^2, j -> j/s^3, h -> s h) rescales dt by s."""
+    rng = np.random.default_rng(11)
+    a0, j0 = rng.normal(size=(30, 3)), rng.normal(size=(30, 3))
+    a1, j1 = a0 + 0.1 * rng.normal(size=(30, 3)), j0 + 0.1 * rng.normal(size=(30, 3))
+    h = np.full(30, 0.125)
+    d1 = oracle.block_step_size(a0, j0, a1, j1, h, 0.01)
+    d4 = oracle.block_step_size(a0, j0, a1, j1, h, 0.04)
+    np.testing.assert_allclose(d4, 2 * d1, rtol=1e-6)
+    ds = oracle.block_step_size(a0 / 4, j0 / 8, a1 / 4, j1 / 8, 2 * h, 0.01)        # s = 2: powers of two, exact
+    np.testing.assert_array_equal(ds, 2 * d1)
