@@ -294,6 +294,26 @@ int nb_block_schedule(int64_t n, const double *t, const double *dt,
                       void *stream);
 
 /*
+ * nb_block_step_size -- the Aarseth step-size criterion of the block Hermite scheme (textbook; reading R20),
+ * per particle, from its two evaluations (a0, j0) at t and (a1, j1) at t + h:
+ *
+ *     a2 = (-6 (a0 - a1) - h (4 j0 + 2 j1)) / h^2       a3 = (12 (a0 - a1) + 6 h (j0 + j1)) / h^3
+ *     a2' = a2 + h a3          dt = sqrt( eta (|a1| |a2'| + |j1|^2) / (|j1| |a3| + |a2'|^2) )
+ *
+ * The value feeds an integer decision (the block level = its power-of-two quantisation, the caller's), so the arithmetic
+ * is pinned: FP32, every operation one IEEE round-to-nearest operation in the order written (da = a0 - a1;
+ * s1 = 4 j0 + 2 j1; a2 = -(6 da + h s1) / (h h); s2 = j0 + j1; a3 = (12 da + (6 h) s2) / ((h h) h); a2' = a2 + h a3;
+ * |z|^2 = (x x + y y) + z z; top = sqrt|a1|^2 sqrt|a2'|^2 + |j1|^2; bot = sqrt|j1|^2 sqrt|a3|^2 + |a2'|^2;
+ * dt = sqrt(eta (top / bot))): bit-identical to the oracle's numpy float32 definition.
+ *
+ *   a0, j0, a1, j1   device, const, float [n][3]      h   device, const, float [n] (> 0)
+ *   eta   > 0, finite                                 dt_out   device, float [n]
+ * bot == 0 (a particle with constant acceleration) gives +inf or NaN as IEEE arithmetic says.  Asynchronous on `stream`.
+ */
+int nb_block_step_size(int64_t n, const float *a0, const float *j0, const float *a1, const float *j1,
+                       const float *h, float eta, float *dt_out, void *stream);
+
+/*
  * nb_force_jerk_host -- nb_force_jerk on HOST arrays: the paper's force() of Fig. A.2 with its
  * host->device and device->host copies (steps (a) and (l)) inside the call.  Blocking.
  */

@@ -273,6 +273,7 @@ def block_step_size(a0: np.ndarray, j0: np.ndarray, a1: np.ndarray, j1: np.ndarr
     a0, j0, a1, j1 = (np.ascontiguousarray(z, dtype=f).reshape(-1, 3) for z in (a0, j0, a1, j1))
     h = np.ascontiguousarray(h, dtype=f).reshape(-1, 1)
     eta = f(eta)
+    old = np.seterr(over="ignore", divide="ignore", invalid="ignore")     # IEEE inf / NaN are part of the definition
     da = a0 - a1
     s1 = f(4) * j0 + f(2) * j1
     h2 = h * h
@@ -287,8 +288,8 @@ def block_step_size(a0: np.ndarray, j0: np.ndarray, a1: np.ndarray, j1: np.ndarr
     a1sq, j1sq, a2sq, a3sq = sq(a1), sq(j1), sq(a2), sq(a3)
     top = np.sqrt(a1sq) * np.sqrt(a2sq) + j1sq
     bot = np.sqrt(j1sq) * np.sqrt(a3sq) + a2sq
-    with np.errstate(divide="ignore", invalid="ignore"):
-        out = np.sqrt(eta * (top / bot))
+    out = np.sqrt(eta * (top / bot))
+    np.seterr(**old)
     assert out.dtype == np.float32
     return out
 

@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     hermite4,
     hermite4_block_step,
     block_schedule,
+    block_step_size,
     last_launch_count,
     leapfrog_kdk,
     pack_j,

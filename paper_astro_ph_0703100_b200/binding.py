@@ -66,6 +66,8 @@ def lib() -> ctypes.CDLL:
         l.nb_hermite4_block_step.restype = ci
         l.nb_block_schedule.argtypes = [i64, p, p, p, p, p, p]
         l.nb_block_schedule.restype = ci
+        l.nb_block_step_size.argtypes = [i64, p, p, p, p, p, f32, p, p]
+        l.nb_block_step_size.restype = ci
         l.nb_plan_query.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
         l.nb_plan_query.restype = ci
         l.nb_last_launch_count.restype = i64
@@ -384,6 +386,25 @@ def block_schedule(t, dt, t_next_out=None, active_out=None, n_act_out=None, stre
                                      active_out.data_ptr() if n else None, n_act_out.data_ptr(), _stream_ptr(stream))
     _check(st, "nb_block_schedule")
     return t_next_out, active_out, n_act_out
+
+
+def block_step_size(a0, j0, a1, j1, h, eta: float, dt_out=None, stream=None):
+    """nb_block_step_size on CUDA float32 tensors.  Returns dt [n] float32; asynchronous."""
+    import torch
+    for z, name in ((a0, "a0"), (j0, "j0"), (a1, "a1"), (j1, "j1")):
+        _dev_f32(z, name, (3,))
+    _dev_f32(h, "h", ())
+    n = a0.shape[0]
+    if not (j0.shape[0] == a1.shape[0] == j1.shape[0] == h.shape[0] == n):
+        raise ValueError("array lengths differ")
+    if dt_out is None:
+        dt_out = torch.empty((n,), dtype=torch.float32, device=a0.device)
+    _dev_f32(dt_out, "dt_out", ())
+    with torch.cuda.device(a0.device):
+        st = lib().nb_block_step_size(n, a0.data_ptr(), j0.data_ptr(), a1.data_ptr(), j1.data_ptr(), h.data_ptr(), float(eta),
+                                      dt_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_block_step_size")
+    return dt_out
 
 
 def plan_query(n_i: int, n_j: int, sm_count: int = 148) -> dict:

@@ -586,4 +586,40 @@ __global__ void __launch_bounds__(kSchedThreads) nb_sched_scatter_kernel(const d
         if (flag[e]) active[pos++] = (int)(base + e);
 }
 
+// ---------------------------------------------------------------- block-step size: the Aarseth criterion, FP32, fixed order
+// dt = sqrt(eta (|a1||a2'| + |j1|^2) / (|j1||a3| + |a2'|^2)) from the Hermite interpolant of (a0, j0) -> (a1, j1) over h.
+// The value feeds an integer decision (the block level), so every operation is one explicitly rounded FP32 operation
+// (no FMA contraction, IEEE division and square root), in the order the header states.
+__device__ __forceinline__ float nb_norm2_rn(const float z[3]) {
+    return __fadd_rn(__fadd_rn(__fmul_rn(z[0], z[0]), __fmul_rn(z[1], z[1])), __fmul_rn(z[2], z[2]));
+}
+__global__ void __launch_bounds__(256) nb_block_step_size_kernel(const float* __restrict__ a0, const float* __restrict__ j0,
+                                                                 const float* __restrict__ a1, const float* __restrict__ j1,
+                                                                 const float* __restrict__ h, float eta, float* __restrict__ dt_out,
+                                                                 int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float hh = h[i];
+    const float h2 = __fmul_rn(hh, hh), h3 = __fmul_rn(h2, hh), h6 = __fmul_rn(6.0f, hh);
+    float va1[3], vj1[3], va2[3], va3[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const size_t k = 3 * (size_t)i + c;
+        const float p0 = a0[k], q0 = j0[k], p1 = a1[k], q1 = j1[k];
+        const float da = __fsub_rn(p0, p1);
+        const float s1 = __fadd_rn(__fmul_rn(4.0f, q0), __fmul_rn(2.0f, q1));
+        const float a2 = __fdiv_rn(-__fadd_rn(__fmul_rn(6.0f, da), __fmul_rn(hh, s1)), h2);
+        const float s2 = __fadd_rn(q0, q1);
+        const float a3 = __fdiv_rn(__fadd_rn(__fmul_rn(12.0f, da), __fmul_rn(h6, s2)), h3);
+        va1[c] = p1;
+        vj1[c] = q1;
+        va3[c] = a3;
+        va2[c] = __fadd_rn(a2, __fmul_rn(hh, a3));
+    }
+    const float a1sq = nb_norm2_rn(va1), j1sq = nb_norm2_rn(vj1), a2sq = nb_norm2_rn(va2), a3sq = nb_norm2_rn(va3);
+    const float top = __fadd_rn(__fmul_rn(__fsqrt_rn(a1sq), __fsqrt_rn(a2sq)), j1sq);
+    const float bot = __fadd_rn(__fmul_rn(__fsqrt_rn(j1sq), __fsqrt_rn(a3sq)), a2sq);
+    dt_out[i] = __fsqrt_rn(__fmul_rn(eta, __fdiv_rn(top, bot)));
+}
+
 }  // namespace nb

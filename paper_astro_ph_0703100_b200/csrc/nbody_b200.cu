@@ -1008,6 +1008,24 @@ int nb_hermite4_block_step(int64_t n, float* x, float* v, const float* m, float*
     return NB_OK;
 }
 
+int nb_block_step_size(int64_t n, const float* a0, const float* j0, const float* a1, const float* j1, const float* h, float eta,
+                       float* dt_out, void* stream_) {
+    t_launches = 0;
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (bad_count(n) || !(eta > 0.0f) || !std::isfinite(eta)) return NB_ERR_INVALID_VALUE;
+    if (n > 0 && (!a0 || !j0 || !a1 || !j1 || !h || !dt_out)) return NB_ERR_INVALID_VALUE;
+    if (3 * n > (int64_t)INT32_MAX) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n == 0) return NB_OK;
+    nb::nb_block_step_size_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(a0, j0, a1, j1, h, eta, dt_out, (int)n);
+    NB_CUDA(cudaGetLastError());
+    t_launches = 1;
+    return NB_OK;
+}
+
 int nb_block_schedule(int64_t n, const double* t, const double* dt, double* t_next_out, int32_t* active_out,
                       int32_t* n_act_out, void* stream_) {
     t_launches = 0;

@@ -65,6 +65,8 @@ def test_argument_validation_happens_before_any_cuda_call():
     assert lib.nb_block_schedule(4, p, None, p, p, p, None) == 1
     assert lib.nb_block_schedule(4, p, p, None, p, p, None) == 1
     assert lib.nb_block_schedule(-1, p, p, p, p, p, None) == 1
+    assert lib.nb_block_step_size(4, p, p, p, p, p, 0.0, p, None) == 1                       # eta must be > 0
+    assert lib.nb_block_step_size(4, p, p, None, p, p, 0.01, p, None) == 1
     assert lib.nb_force_batched(-1, p, p, 1, p, 1, p, p, 0.1, p, None, None) == 1
     assert lib.nb_force_batched(2, None, p, 1, p, 1, p, p, 0.1, p, None, None) == 1
     assert lib.nb_force_eps_i(1, p, None, 1, p, p, p, None, None) == 1
@@ -96,6 +98,7 @@ def test_without_a_device_every_compute_entry_reports_an_error():
                lib.nb_hermite4(1, p, p, p, 0.1, 0.1, 1, p, p, None, None),
                lib.nb_hermite4_block_step(1, p, p, p, p, p, p, 1, p, 0.5, 0.1, None),
                lib.nb_block_schedule(1, p, p, p, p, p, None),
+               lib.nb_block_step_size(1, p, p, p, p, p, 0.01, p, None),
                lib.nb_cunbody_force(p, p, p, 1, 1, None)):
         assert st in (2, 4), "without a B200 the library must report an error, not compute on the CPU"
 
