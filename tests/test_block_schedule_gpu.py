@@ -99,3 +99,53 @@ def test_block_step_run_driven_by_the_device_scheduler(nb):
     torch.cuda.synchronize()
     assert len(set(sizes)) == 3 and np.array_equal(t.cpu().numpy(), tr) and np.all(tr == 8.0 / 512)
     assert np.abs(x.cpu().numpy() - xr).max() < 1e-5 and np.abs(v.cpu().numpy() - vr).max() < 1e-5
+
+
+def test_adaptive_block_step_run_with_all_three_calls(nb):
+    """A whole block-time-step integration on the device: nb_block_schedule says who is due, nb_hermite4_block_step
+    advances them, nb_block_step_size proposes each one's next step; the quantisation to the block grid (halve when the
+    criterion asks for less, double only at commensurate times, dt_min <= dt <= dt_max) is the caller's, done here with
+    torch on the device.  Properties: every clock ends exactly at t_end, several levels are in use, energy and momentum
+    are conserved far better than the step sizes alone would suggest."""
+    import torch
+    n, eta = 1024, 0.01
+    dt_min, dt_max, t_end = 2.0 ** -13, 2.0 ** -6, 2.0 ** -4
+    w = wl.plummer_workload(n, 1.0 / 32, seed=31, with_velocities=True)
+    x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
+    acc, jerk, _ = nb.force_jerk(x, v, x, v, m, w.eps2)
+    t = torch.zeros(n, dtype=torch.float64, device="cuda")
+    dt = torch.full((n,), 2.0 ** -10, dtype=torch.float64, device="cuda")
+    steps, evaluated, levels_seen = 0, 0, set()
+    while True:
+        t_next, active, n_act = nb.block_schedule(t, dt)
+        tn, k = float(t_next.item()), int(n_act.item())
+        if tn > t_end:
+            break
+        idx = active[:k].long()
+        a_old, j_old = acc[idx].contiguous(), jerk[idx].contiguous()
+        h = (tn - t[idx]).float()
+        nb.hermite4_block_step(x, v, m, acc, jerk, t, active[:k], tn, w.eps2)
+        crit = nb.block_step_size(a_old, j_old, acc[idx].contiguous(), jerk[idx].contiguous(), h, eta).double()
+        old = dt[idx]
+        new = old.clone()
+        for _ in range(4):                                                  # halve while the criterion asks for less
+            new = torch.where((crit < new) & (new > dt_min), new / 2, new)
+        may_double = (crit >= 2 * old) & (2 * old <= dt_max) & (torch.remainder(torch.full_like(old, tn), 2 * old) == 0)
+        new = torch.where(may_double, 2 * old, new)
+        dt[idx] = new
+        steps += 1
+        evaluated += k
+        levels_seen.update(torch.unique(new).tolist())
+        assert steps < 5000
+    torch.cuda.synchronize()
+    assert torch.all(t == t_end).item()                                     # everybody arrives exactly
+    assert len(levels_seen) >= 3 and evaluated < steps * n                  # a real hierarchy, real savings
+    gx, gv = x.cpu().numpy(), v.cpu().numpy()
+    _, _, e0 = oracle.energy(w.x_j, w.v, w.m_j, w.eps2)
+    _, _, e1 = oracle.energy(gx, gv, w.m_j, w.eps2)
+    assert abs(e1 - e0) / abs(e0) < 2e-6
+    p0 = (w.m_j[:, None] * w.v.astype(np.float64)).sum(0)
+    p1 = (w.m_j[:, None] * gv.astype(np.float64)).sum(0)
+    assert np.abs(p1 - p0).max() < 1e-6
+    print(f"adaptive block run: {steps} block steps, {evaluated} particle evaluations of {steps * n}, "
+          f"levels {sorted(levels_seen)}, dE/E = {abs(e1 - e0) / abs(e0):.2e}")
