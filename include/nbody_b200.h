@@ -31,6 +31,20 @@
  *     point atomics; all reductions run in a fixed order).
  *   - there is no CPU fallback and no other GPU architecture: a device whose compute capability
  *     is not 10.x yields NB_ERR_UNSUPPORTED_DEVICE.
+ *   - threads: the library may be called from several host threads.  Error and launch-count state is per thread.  The
+ *     internal workspace is per (device, stream) and is locked while a call grows it and enqueues the work that uses
+ *     it, so calls that share a stream (all *_host calls share the default stream) are serialised on the host; their
+ *     device work runs in stream order, as always.  nb_release_workspace / nb_release_stream must not run while
+ *     another thread is inside a call on that device / stream.
+ *   - CUDA graphs: once the workspace of a stream is warm (one call of the same or a larger shape has run on it) a call
+ *     enqueues kernels only and can be captured.  A captured graph holds the workspace's addresses: replaying it after
+ *     a LARGER call on the same stream (which re-allocates the buffers it grows), after nb_release_workspace or after
+ *     nb_release_stream reads freed memory -- capture again after any of these.
+ *   - coordinate range of the coincident-pair rule: the kernels run flush-to-zero, so a pair whose three coordinate
+ *     differences are all SUBNORMAL (|d| < 2^-126) may count as coincident, and whether it does can depend on the
+ *     decomposition.  With every coordinate either 0 or >= 2^-102 in magnitude all non-zero differences are normal
+ *     numbers and the rule is exactly "all three differences are zero" (tests/test_force_gpu.py bounds this).
+ *   - the library reads no environment variable on any call; its debugging switches are in nb_debug.h.
  */
 #ifndef NBODY_B200_H
 #define NBODY_B200_H
@@ -67,7 +81,10 @@ typedef enum nb_status {
  * n_i == 0: NB_OK, nothing is written.  n_j == 0: NB_OK, outputs are zero-filled.
  * Inputs are not validated on the device: non-finite or |x| > ~1e18 inputs give undefined values.
  * Uses an internal per-stream workspace (packed j records, j-split partial sums) that grows on
- * demand with stream-ordered allocation; once warm the call is CUDA-graph capturable.
+ * demand with stream-ordered allocation; once warm the call is CUDA-graph capturable (see "CUDA graphs" above).
+ * Calls with few i-particles (n_i <= 512 up to 2^26 pairs, n_i <= 2048 up to 2^22 pairs: BASELINE.json configs[0] and
+ * [2]) run as ONE launch of the small-i-set kernel (packed over j; the j-split is summed through lanes, warps, a
+ * thread-block cluster or ticketed FP64 partials); larger ones as pack (+ coincidence pre-pass) + force kernel (+ second pass).
  */
 int nb_force(int64_t n_i, const float *x_i,
              int64_t n_j, const float *x_j, const float *m_j,
@@ -287,7 +304,8 @@ int nb_hermite4_block_step(int64_t n, float *x, float *v, const float *m,
  *   t_next_out  device, double [1]         active_out  device, int32 [n] (only the first n_act entries are written)
  *   n_act_out   device, int32 [1]: the caller reads it back (4 bytes) to size the nb_hermite4_block_step call
  * Index work: exact and deterministic (no floating-point atomics, ordered compaction).  n == 0: t_next = +inf, n_act = 0.
- * Non-finite due times are never selected (all non-finite: t_next = +inf, n_act = 0).  Asynchronous on `stream`.
+ * A due time that is not finite (t + dt = +-inf or NaN: e.g. a particle parked with dt = +inf) takes no part: it is never the
+ * minimum and never due; if no due time is finite, t_next = +inf and n_act = 0.  Asynchronous on `stream`.
  */
 int nb_block_schedule(int64_t n, const double *t, const double *dt,
                       double *t_next_out, int32_t *active_out, int32_t *n_act_out,
@@ -348,8 +366,21 @@ int64_t nb_last_launch_count(void);
 int nb_profile_enable(int on);
 int nb_profile_read(int64_t *n_launches, double *total_ms);
 
+/* nb_plan_query for the small-i-set kernel nb_force uses for few i-particles (csrc/nb_small.cuh):
+ * out[0] = NW warps per CTA (8 or 16)       out[1] = KI i-particles per thread
+ * out[2] = LJ lanes of a warp along j (32 / LJ along i)      out[3] = WJ warps per CTA along j
+ * out[4] = S  j-chunks across CTAs (grid.y) out[5] = CS CTAs per thread-block cluster
+ * out[6] = number of i-tiles (grid.x); i-particles per CTA tile = (NW / WJ) * KI * (32 / LJ)
+ * out[7] = 1 if nb_force takes this kernel for (n_i, n_j) by default */
+int nb_plan_query_small(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]);
+
 /* Frees every internal workspace of the current device (synchronises the device). */
 int nb_release_workspace(void);
+
+/* Frees the workspace kept for `stream` on the current device (waits for that stream first).  Call it before destroying a
+ * stream the library has been used on: the workspace is keyed by the stream handle and would otherwise stay allocated
+ * until nb_release_workspace -- and be inherited by a later stream that happens to get the same handle. */
+int nb_release_stream(void *stream);
 
 const char *nb_status_string(int status);   /* static storage */
 int nb_last_cuda_error(void);                /* cudaError_t behind this thread's last NB_ERR_CUDA / NB_ERR_ALLOC */

@@ -244,7 +244,8 @@ def hermite4_block_step(x: np.ndarray, v: np.ndarray, m: np.ndarray, acc: np.nda
 def block_schedule(t: np.ndarray, dt: np.ndarray):
     """The block-step scheduler's definition (reading R20): the next block time is the earliest due time
     t_next = min_k (t[k] + dt[k]) (one FP64 addition per particle), and the due particles are those whose due time
-    EQUALS it, in ascending index order.  Returns (t_next, active int32 [n_act]); n = 0 gives (+inf, empty).
+    EQUALS it, in ascending index order.  Due times that are not finite (+-inf, NaN) take no part: they are never the
+    minimum and never due.  Returns (t_next, active int32 [n_act]); n = 0 or no finite due time gives (+inf, empty).
     Pins (tests/test_oracle_hermite_pins.py, "h9"): hand-worked cases, ties, a pure-Python loop."""
     tt = np.asarray(t, dtype=np.float64).reshape(-1)
     dd = np.asarray(dt, dtype=np.float64).reshape(-1)
@@ -252,9 +253,13 @@ def block_schedule(t: np.ndarray, dt: np.ndarray):
         raise ValueError("array lengths differ")
     if tt.size == 0:
         return float("inf"), np.zeros(0, dtype=np.int32)
-    due = tt + dd
-    t_next = float(due.min())
-    return t_next, np.nonzero(due == t_next)[0].astype(np.int32)
+    with np.errstate(invalid="ignore"):
+        due = tt + dd                      # inf + (-inf) = NaN: not finite, takes no part
+    finite = np.isfinite(due)              # reading R20: a non-finite due time (dt = +inf parks a particle) is never selected
+    if not finite.any():
+        return float("inf"), np.zeros(0, dtype=np.int32)
+    t_next = float(due[finite].min())
+    return t_next, np.nonzero(finite & (due == t_next))[0].astype(np.int32)
 
 
 def block_step_size(a0: np.ndarray, j0: np.ndarray, a1: np.ndarray, j1: np.ndarray, h: np.ndarray, eta: float) -> np.ndarray:
@@ -291,6 +296,32 @@ def block_step_size(a0: np.ndarray, j0: np.ndarray, a1: np.ndarray, j1: np.ndarr
     out = np.sqrt(eta * (top / bot))
     np.seterr(**old)
     assert out.dtype == np.float32
+    return out
+
+
+def block_step_size_f64(a0: np.ndarray, j0: np.ndarray, a1: np.ndarray, j1: np.ndarray, h: np.ndarray, eta: float) -> np.ndarray:
+    """The same Aarseth criterion as block_step_size, written out plainly in FP64 (the formula of
+    include/nbody_b200.h "nb_block_step_size" / Makino & Aarseth 1992, no prescribed rounding or order):
+
+        a2 = (-6 (a0 - a1) - h (4 j0 + 2 j1)) / h^2;  a3 = (12 (a0 - a1) + 6 h (j0 + j1)) / h^3;  a2' = a2 + h a3
+        dt = sqrt( eta (|a1| |a2'| + |j1|^2) / (|j1| |a3| + |a2'|^2) )
+
+    The FP32 definition above exists because the value feeds an integer decision; this one is the plain definition the
+    CUDA path is ALSO held against, by tolerance, on well-conditioned inputs (tests/test_block_step_size_gpu.py), so
+    that the kernel is not checked only against an FP32 mirror of its own arithmetic.  Returns dt, float64 [n].
+    Pins (tests/test_oracle_hermite_pins.py, "h10"): cubic a(t) to 1e-13, the circular orbit, the scaling laws, and
+    agreement with the FP32 definition to FP32 rounding."""
+    a0, j0, a1, j1 = (np.ascontiguousarray(z, dtype=np.float64).reshape(-1, 3) for z in (a0, j0, a1, j1))
+    h = np.ascontiguousarray(h, dtype=np.float64).reshape(-1, 1)
+    old = np.seterr(over="ignore", divide="ignore", invalid="ignore")
+    a2 = (-6.0 * (a0 - a1) - h * (4.0 * j0 + 2.0 * j1)) / h ** 2
+    a3 = (12.0 * (a0 - a1) + 6.0 * h * (j0 + j1)) / h ** 3
+    a2 = a2 + h * a3
+
+    def norm(z):
+        return np.sqrt(np.sum(z * z, axis=1))
+    out = np.sqrt(float(eta) * (norm(a1) * norm(a2) + norm(j1) ** 2) / (norm(j1) * norm(a3) + norm(a2) ** 2))
+    np.seterr(**old)
     return out
 
 

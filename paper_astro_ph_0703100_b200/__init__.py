@@ -25,6 +25,11 @@ from .binding import (  # noqa: F401
     lib,
     plan_query,
     plan_query_jerk,
+    plan_query_small,
+    debug_set,
+    debug_plan_exhaustive,
+    debug_plans_computed,
+    release_stream,
     profile_enable,
     profile_read,
     release_workspace,

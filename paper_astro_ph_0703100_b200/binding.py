@@ -70,6 +70,15 @@ def lib() -> ctypes.CDLL:
         l.nb_block_step_size.restype = ci
         l.nb_plan_query.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
         l.nb_plan_query.restype = ci
+        l.nb_plan_query_small.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
+        l.nb_plan_query_small.restype = ci
+        l.nb_debug_set.argtypes = [ctypes.c_char_p, ctypes.c_char_p]
+        l.nb_debug_set.restype = ci
+        l.nb_debug_plan_exhaustive.argtypes = [i64, i64, ci, ci, ctypes.POINTER(i64)]
+        l.nb_debug_plan_exhaustive.restype = ci
+        l.nb_debug_plans_computed.restype = i64
+        l.nb_release_stream.argtypes = [p]
+        l.nb_release_stream.restype = ci
         l.nb_last_launch_count.restype = i64
         l.nb_release_workspace.restype = ci
         l.nb_profile_enable.argtypes = [ci]
@@ -419,6 +428,37 @@ def plan_query_jerk(n_i: int, n_j: int, sm_count: int = 148) -> dict:
     _check(lib().nb_plan_query_jerk(int(n_i), int(n_j), int(sm_count), out), "nb_plan_query_jerk")
     keys = ("K", "WI", "WJ", "S", "tiles_i", "tile_i", "tile_j", "stages")
     return dict(zip(keys, [int(v) for v in out]))
+
+
+def plan_query_small(n_i: int, n_j: int, sm_count: int = 148) -> dict:
+    """The small-i-set kernel's decomposition for (n_i, n_j); "default" = nb_force takes that kernel for this shape."""
+    out = (ctypes.c_int64 * 8)()
+    _check(lib().nb_plan_query_small(int(n_i), int(n_j), int(sm_count), out), "nb_plan_query_small")
+    keys = ("NW", "KI", "LJ", "WJ", "S", "CS", "tiles_i", "default")
+    d = dict(zip(keys, [int(v) for v in out]))
+    d["tile_i"] = (d["NW"] // d["WJ"]) * d["KI"] * (32 // d["LJ"])
+    return d
+
+
+def debug_set(key: str, value: Optional[str]) -> None:
+    """include/nb_debug.h: a debugging switch of the library (value None restores the default)."""
+    _check(lib().nb_debug_set(key.encode(), None if value is None else str(value).encode()), f"nb_debug_set({key})")
+
+
+def debug_plan_exhaustive(n_i: int, n_j: int, sm_count: int = 148, jerk: bool = False) -> dict:
+    out = (ctypes.c_int64 * 8)()
+    _check(lib().nb_debug_plan_exhaustive(int(n_i), int(n_j), int(sm_count), 1 if jerk else 0, out), "nb_debug_plan_exhaustive")
+    keys = ("K", "WI", "WJ", "S", "tiles_i", "tile_i", "tile_j", "stages")
+    return dict(zip(keys, [int(v) for v in out]))
+
+
+def debug_plans_computed() -> int:
+    return int(lib().nb_debug_plans_computed())
+
+
+def release_stream(stream=None) -> None:
+    """nb_release_stream: frees the workspace the library keeps for `stream` (waits for the stream first)."""
+    _check(lib().nb_release_stream(_stream_ptr(stream)), "nb_release_stream")
 
 
 def last_launch_count() -> int:

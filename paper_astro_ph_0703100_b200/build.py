@@ -9,13 +9,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnbody_b200.so")
-SOURCES = ["nbody_b200.cu"]
-DEPS = ["nbody_b200.cu", "nb_kernels.cuh", "nb_hermite.cuh", "nb_batched.cuh", "nb_pipelines.cuh", os.path.join(ROOT, "include", "nb_pipeline.cuh"), "nb_plan.h", os.path.join(ROOT, "include", "nbody_b200.h")]
+SOURCES = ["nbody_b200.cu", "nb_small_launch.cu"]
+DEPS = ["nbody_b200.cu", "nb_small_launch.cu", "nb_small_launch.h", "nb_small.cuh", "nb_packed.cuh", os.path.join(ROOT, "include", "nb_debug.h"), "nb_kernels.cuh", "nb_hermite.cuh", "nb_batched.cuh", "nb_pipelines.cuh", os.path.join(ROOT, "include", "nb_pipeline.cuh"), "nb_plan.h", os.path.join(ROOT, "include", "nbody_b200.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
-    "-Xcompiler", "-fPIC", "-shared",
+    "-Xcompiler", "-fPIC",
     "-I", os.path.join(ROOT, "include"),
 ]
 
@@ -32,15 +32,25 @@ def stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """One object per translation unit, compiled side by side, then one shared library."""
     if force or stale():
         nvcc = os.environ.get("NVCC", "nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, "-o", LIB + ".tmp", *[os.path.join(CSRC, s) for s in SOURCES]]
-        if verbose:
-            cmd.insert(1, "-Xptxas")
-            cmd.insert(2, "-v")
-            print(" ".join(cmd), file=sys.stderr)
-        subprocess.run(cmd, check=True)
+        objs, procs = [], []
+        for src in SOURCES:
+            obj = os.path.join(CSRC, src.replace(".cu", ".o"))
+            cmd = [nvcc, *NVCC_FLAGS, "-c", "-o", obj, os.path.join(CSRC, src)]
+            if verbose:
+                cmd[1:1] = ["-Xptxas", "-v"]
+                print(" ".join(cmd), file=sys.stderr)
+            objs.append(obj)
+            procs.append((cmd, subprocess.Popen(cmd)))
+        for cmd, p in procs:
+            if p.wait() != 0:
+                raise subprocess.CalledProcessError(p.returncode, cmd)
+        subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB + ".tmp", *objs], check=True)
         os.replace(LIB + ".tmp", LIB)
+        for obj in objs:
+            os.remove(obj)
     return LIB
 
 

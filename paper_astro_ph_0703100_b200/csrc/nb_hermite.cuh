@@ -483,7 +483,9 @@ __global__ void __launch_bounds__(256) nb_block_correct_kernel(float* __restrict
 // ---------------------------------------------------------------- block-step scheduler: who is due next (index work, exact)
 // t_next = min_k (t[k] + dt[k]);  active = ascending { k : t[k] + dt[k] == t_next }.  One FP64 add per particle, the same
 // on both passes, so the equality is exact.  A CTA covers kSchedTile consecutive particles, a thread kSchedItems of them.
+// A due time that is not finite (a particle parked with dt = +inf, a NaN clock, -inf) is never the minimum and never due.
 constexpr int kSchedThreads = 256, kSchedItems = 4, kSchedTile = kSchedThreads * kSchedItems;
+__device__ __forceinline__ bool nb_sched_finite(double due) { return fabs(due) <= 1.7976931348623157e308; }   // false for NaN
 
 __global__ void __launch_bounds__(kSchedThreads) nb_sched_min_kernel(const double* __restrict__ t, const double* __restrict__ dt,
                                                                     int n, double* __restrict__ block_min) {
@@ -492,7 +494,10 @@ __global__ void __launch_bounds__(kSchedThreads) nb_sched_min_kernel(const doubl
     double lo = CUDART_INF;
 #pragma unroll
     for (int e = 0; e < kSchedItems; ++e)
-        if (base + e < (size_t)n) lo = fmin(lo, __dadd_rn(t[base + e], dt[base + e]));
+        if (base + e < (size_t)n) {
+            const double due_k = __dadd_rn(t[base + e], dt[base + e]);
+            if (nb_sched_finite(due_k)) lo = fmin(lo, due_k);
+        }
     for (int o = 16; o > 0; o >>= 1) lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
     if ((threadIdx.x & 31) == 0) warp_min[threadIdx.x >> 5] = lo;
     __syncthreads();
@@ -527,7 +532,7 @@ __global__ void __launch_bounds__(kSchedThreads) nb_sched_count_kernel(const dou
     int c = 0;
 #pragma unroll
     for (int e = 0; e < kSchedItems; ++e)
-        if (base + e < (size_t)n) c += (__dadd_rn(t[base + e], dt[base + e]) == due);
+        if (base + e < (size_t)n) c += (__dadd_rn(t[base + e], dt[base + e]) == due && nb_sched_finite(due));
     for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
     if ((threadIdx.x & 31) == 0 && c) atomicAdd(&total, c);          // integer sum: the order does not matter
     __syncthreads();
@@ -569,7 +574,7 @@ __global__ void __launch_bounds__(kSchedThreads) nb_sched_scatter_kernel(const d
     int c = 0;
 #pragma unroll
     for (int e = 0; e < kSchedItems; ++e) {
-        flag[e] = base + e < (size_t)n && __dadd_rn(t[base + e], dt[base + e]) == due;
+        flag[e] = base + e < (size_t)n && __dadd_rn(t[base + e], dt[base + e]) == due && nb_sched_finite(due);
         c += flag[e];
     }
     int incl = c;                                                      // inclusive scan over the warp

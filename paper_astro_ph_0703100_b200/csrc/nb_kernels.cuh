@@ -24,76 +24,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "nb_packed.cuh"
+
 namespace nb {
-
-typedef unsigned long long u64;
-
-// ---------------------------------------------------------------- packed FP32 helpers
-__device__ __forceinline__ u64 pack2(float lo, float hi) {
-    u64 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void unpack2(u64 v, float& lo, float& hi) {
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ u64 add2(u64 a, u64 b) {
-    u64 d;
-    asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ u64 mul2(u64 a, u64 b) {
-    u64 d;
-    asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
-    u64 d;
-    asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ float rsqrt_approx(float x) {
-    float y;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
-// ---------------------------------------------------------------- mbarrier / TMA bulk copy
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-    return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() {
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n"
-            "  .reg .pred p;\n"
-            "  mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "  selp.u32 %0, 1, 0, p;\n"
-            "}\n"
-            : "=r"(ok)
-            : "r"(bar), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-// 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP)
-__device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
-                 : "memory");
-}
 
 // ---------------------------------------------------------------- a1: j-pack
 // One thread per j-particle: (x, y, z) || m -> float4.
@@ -117,13 +50,6 @@ __global__ void __launch_bounds__(256) nb_pack_j_kernel(const float* __restrict_
 //                unmasked coincident pair adds m u^3 * (+-0) = +-0 to a.  13 + 1 instructions.
 // (A third, speculative variant -- flag r2 == eps2 in the loop, redo a flagged 256-j block with the mask -- was the
 //  default earlier in this round and was removed: DESIGN.md section 10.)
-enum { MASK_EXACT = 0, MASK_NONE = 2 };
-
-// -x_i as the kernels hold it: +0 for a zero or subnormal coordinate (add.ftz reads a subnormal as zero), so that a
-// difference x_j + (-x_i) that is zero is always +0 -- (-0) + (-0) = -0 cannot arise -- and the bitwise test of
-// MASK_EXACT sees every coincident pair, whatever the signs of the zeros involved.
-__device__ __forceinline__ float neg_canon(float x) { return (fabsf(x) < 1.17549435e-38f) ? 0.0f : -x; }
-
 // PHI = false: the caller does not want the potential (pot_out == NULL): 12 FP32-pipe instructions per pair.
 template <int MASK, bool PHI = true>
 __device__ __forceinline__ void pair_body(u64 xj, u64 yj, u64 zj, u64 mj, u64 nxi, u64 nyi, u64 nzi, u64 eps2_2,
@@ -194,18 +120,6 @@ constexpr int kCoinSegShift = 8;
 constexpr int kCoinCap = 8;           // segments kept per i-group
 constexpr int kCoinRaw = 32;          // distinct segments collected per i-group before giving up (set of 64 slots)
 constexpr int kCoinMaxProbe = 2048;   // probe steps before giving up
-
-__device__ __forceinline__ uint32_t coin_canon(float v) {
-    return (fabsf(v) < 1.17549435e-38f) ? 0u : __float_as_uint(v);
-}
-__device__ __forceinline__ uint32_t coin_hash(uint32_t a, uint32_t b, uint32_t c) {
-    uint64_t h = (uint64_t)a * 0x9E3779B97F4A7C15ull;
-    h ^= (uint64_t)b * 0xC2B2AE3D27D4EB4Full + (h >> 29);
-    h ^= (uint64_t)c * 0x165667B19E3779F9ull + (h << 17);
-    h ^= h >> 32;
-    h *= 0xD6E8FEB86659FD93ull;
-    return (uint32_t)(h >> 32);
-}
 
 // table entries: 0 = empty, else j + 1
 // stride = float4 per j record (1 for the force path, 2 for the force + jerk path)

@@ -13,6 +13,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <cstdio>
+#include <cmath>
 
 namespace nb {
 
@@ -82,9 +83,29 @@ inline double plan_cost(int64_t n_i, int64_t n_j, int sm_count, int K, int WI, i
 }
 
 // k_max: largest K the kernel family is instantiated for; pair_inst: FP32-pipe instructions per pair;
-// partial_bytes: bytes per (chunk, i) of the second-pass partials; rec_bytes: bytes per j record.
-inline Plan make_plan(int64_t n_i, int64_t n_j, int sm_count, int k_max = 8, double pair_inst = 13.0,
-                      double partial_bytes = 32.0) {
+// partial_bytes: bytes per (chunk, i) of the second-pass partials.
+//
+// make_plan_exhaustive tries every S in 1 .. min(n_j / (8 WJ), 2048) for every (K, WJ): ~20 000 cost evaluations,
+// 60 .. 220 us on the host -- more than a small call lasts on the device.  It is kept as the DEFINITION of the choice
+// (nb_debug.h: nb_debug_plan_exhaustive; tests/test_abi_host.py holds make_plan to it).  make_plan evaluates the same
+// cost only where its minimum over S can lie.  For fixed (K, WJ) and a fixed number of waves w = ceil(tiles_i S / #SM)
+// the cost is w (C + A / S) + R(S) with R piecewise linear and increasing (fused second pass below the byte threshold,
+// separate launch above): convex on each piece, so the minimum over the piece is at one of its ends or next to the
+// stationary point sqrt(w A / slope).  Pieces are visited by increasing w until w C_fixed + A tiles_i / #SM -- a lower
+// bound for every later piece -- exceeds the best cost found: a few dozen evaluations per (K, WJ), < 3 us in all.
+struct PlanChoice { double cost; int K, WI, WJ, S; };
+
+inline Plan finish_plan(int K, int WI, int WJ, int S, int64_t n_i) {
+    Plan p{};
+    p.K = K; p.WI = WI; p.WJ = WJ; p.S = S;
+    p.tile_i = 32 * K * WI;
+    p.tiles_i = (int)((n_i + p.tile_i - 1) / p.tile_i);
+    ring_shape(WJ, &p.tile_j, &p.stages);
+    return p;
+}
+
+inline Plan make_plan_exhaustive(int64_t n_i, int64_t n_j, int sm_count, int k_max = 8, double pair_inst = 13.0,
+                                 double partial_bytes = 32.0) {
     if (sm_count <= 0) sm_count = 148;
     Plan best{};
     double best_cost = -1.0;
@@ -110,17 +131,204 @@ inline Plan make_plan(int64_t n_i, int64_t n_j, int sm_count, int k_max = 8, dou
             }
         }
     }
-    // debugging aid, not part of the ABI: NB_PLAN="K,WI,WJ,S" overrides the choice
-    if (const char* env = std::getenv("NB_PLAN")) {
-        int k, wi, wj, s;
-        if (std::sscanf(env, "%d,%d,%d,%d", &k, &wi, &wj, &s) == 4 && (k == 2 || k == 4 || k == 8) && k <= k_max &&
-            wi * wj == kWarpsPerCta && (wj == 1 || wj == 2 || wj == 4 || wj == 8) && s >= 1 && s <= kMaxS) {
-            best.K = k; best.WI = wi; best.WJ = wj; best.S = s;
+    return finish_plan(best.K, best.WI, best.WJ, best.S, n_i);
+}
+
+inline Plan make_plan(int64_t n_i, int64_t n_j, int sm_count, int k_max = 8, double pair_inst = 13.0,
+                      double partial_bytes = 32.0) {
+    if (sm_count <= 0) sm_count = 148;
+    static const int k_opts[3] = {8, 4, 2};
+    static const int wj_opts[4] = {1, 2, 4, 8};
+    PlanChoice best{-1.0, 0, 0, 0, 0};
+    for (int k_idx = 0; k_idx < 3; ++k_idx) {
+        const int K = k_opts[k_idx];
+        if (K > k_max) continue;
+        if (K > 2 && n_i <= 32 * (K / 2)) continue;
+        for (int wj_idx = 0; wj_idx < 4; ++wj_idx) {
+            const int WJ = wj_opts[wj_idx];
+            const int WI = kWarpsPerCta / WJ;
+            int64_t s_max = n_j / (8 * WJ);
+            if (s_max < 1) s_max = 1;
+            if (s_max > kMaxS) s_max = kMaxS;
+            const int tile_i = 32 * K * WI;
+            const int64_t tiles_i = (n_i + tile_i - 1) / tile_i;
+            PlanChoice local{-1.0, K, WI, WJ, 0};                         // best of this (K, WJ): the exhaustive order within it
+            auto visit = [&](int64_t S) {
+                if (S < 1 || S > s_max) return;
+                const double c = plan_cost(n_i, n_j, sm_count, K, WI, WJ, (int)S, pair_inst, partial_bytes);
+                if (local.cost < 0.0 || c < local.cost * (1.0 - 1e-9) || (S < local.S && c <= local.cost)) { local.cost = c; local.S = (int)S; }
+            };
+            // work per CTA wave that does not depend on S: A / S with A = tile_i n_j pair_cycles k_pen wj_pen
+            const double A = plan_cost(n_i, n_j, sm_count, K, WI, WJ, 1, pair_inst, partial_bytes) /
+                                 double((tiles_i + sm_count - 1) / sm_count) - 6000.0 - (WJ > 1 ? 1500.0 : 0.0);
+            const double c_fixed = 6000.0 + (WJ > 1 ? 1500.0 : 0.0);
+            const double floor_work = A * double(tiles_i) / double(sm_count);
+            const int64_t s_fused = (int64_t)((double)kFusedReduceBytes / ((double)tile_i * partial_bytes));   // largest S with a fused second pass
+            const double slope_sep = double(n_i) * partial_bytes / 1250.0 > 200.0 ? double(n_i) * partial_bytes / 1250.0 : 200.0;
+            visit(1);
+            int64_t w = (tiles_i + sm_count - 1) / sm_count;              // waves at S = 1
+            int64_t prev_hi = 0;
+            for (;; ++w) {
+                int64_t hi = w * sm_count / tiles_i;                      // largest S with at most w waves
+                if (hi > s_max) hi = s_max;
+                const int64_t lo = prev_hi + 1;
+                if (hi >= lo) {
+                    visit(lo); visit(hi);
+                    if (s_fused >= lo && s_fused <= hi) { visit(s_fused); visit(s_fused + 1 <= hi ? s_fused + 1 : hi); }
+                    const double slopes[2] = {200.0, slope_sep};
+                    for (int q = 0; q < 2; ++q) {
+                        const int64_t st = (int64_t)std::sqrt(double(w) * A / slopes[q]);
+                        for (int64_t d = -1; d <= 2; ++d) {
+                            const int64_t S = st + d;
+                            if (S >= lo && S <= hi) visit(S);
+                        }
+                    }
+                    prev_hi = hi;
+                }
+                if (hi >= s_max) break;
+                const double lower = double(w + 1) * c_fixed + floor_work;   // no S with more waves can cost less
+                const double ref = local.cost >= 0.0 ? local.cost : -1.0;
+                if (ref >= 0.0 && lower >= ref) break;
+            }
+            if (local.cost >= 0.0 && (best.cost < 0.0 || local.cost < best.cost * (1.0 - 1e-9))) best = local;
         }
     }
-    best.tile_i = 32 * best.K * best.WI;
+    return finish_plan(best.K, best.WI, best.WJ, best.S, n_i);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Small i-sets (nb_small.cuh): packed over j, lanes LI x LJ, warps WI x WJ, S j-chunks over CTAs in clusters of CS.
+struct SmallPlan {
+    int NW;           // warps per CTA (8 or 16)
+    int KI;           // i-particles per thread (1 or 2)
+    int LJ;           // lanes of a warp along j (1, 2 or 4; > 1 only with KI = 1, NW = 8, WJ = 8)
+    int WJ;           // warps of the CTA along j (1, 2, 4, 8 or -- NW = 16 -- 16)
+    int S;            // j-chunks across CTAs (grid.y), a multiple of CS
+    int CS;           // CTAs per thread-block cluster along grid.y (1 or 8)
+    int tile_i;       // i-particles per CTA = (NW / WJ) * KI * (32 / LJ)
+    int tiles_i;      // grid.x
+};
+
+constexpr int kSmallClusterMax = 8;
+// Which calls nb_force gives to the small-i-set kernel (measured per call from a 50-call CUDA graph, profiles/r02_small_calls.md):
+// up to 512 i-particles it is at least as fast as nb_force_kernel's K = 2 path up to C2's 2^25 pairs (512 x 4096: 6.4
+// against 7.6 us, C2: 24.8 against 23.8-25.2 us, and 2 us faster with a cold L2); up to 2048 i-particles it wins while
+// the call is latency-bound (1024 x 1024: 5.2 against 6.3 us, C0: 7.4 against 7.7 us) and loses once K = 4 tiles fill
+// the machine (2048 x 4096: 12.1 against 9.8 us).
+constexpr int64_t kSmallMaxI = 2048;
+constexpr int64_t kSmallNarrowI = 512;
+constexpr double kSmallMaxPairsNarrow = 67108864.0;    // 2^26, n_i <= 512
+constexpr double kSmallMaxPairs = 4194304.0;           // 2^22, n_i <= 2048
+inline bool small_by_default(int64_t n_i, int64_t n_j) {
+    const double pairs = (double)n_i * (double)n_j;
+    return (n_i <= kSmallNarrowI && pairs <= kSmallMaxPairsNarrow) || (n_i <= kSmallMaxI && pairs <= kSmallMaxPairs);
+}
+constexpr int kSmallRoundJPlan = 4096;           // = nb::kSmallRoundJ (nb_small.cuh)
+
+// the instantiated shapes (nb_small_launch.cu)
+inline bool small_shape_ok(int NW, int KI, int LJ, int WJ, int CS) {
+    if (!(NW == 8 || NW == 16) || !(WJ == 1 || WJ == 2 || WJ == 4 || WJ == 8 || (WJ == 16 && NW == 16)) ||
+        !(CS == 1 || CS == kSmallClusterMax)) return false;
+    const bool wide = LJ == 1 && (KI == 1 || KI == 2);                           // throughput shapes: any NW, WJ
+    const bool narrow = KI == 1 && (LJ == 2 || LJ == 4) && NW == 8 && WJ == 8;   // 16 or 8 i-particles per CTA
+    if (!wide && !narrow) return false;
+    return ((NW / WJ) * KI * (32 / LJ)) % CS == 0;
+}
+
+// Loop efficiency (fraction of the 13-instruction FP32 roofline) of the j-packed body, measured with micro-loops on a
+// B200 (profiles/r02_microloops.md), by i-particles per thread and resident warps per SM: with the exact mask on
+// every pair, and without it (the blocks a Bloom-filter test lets through; acceleration-only calls).
+inline double small_loop_eff(int KI, int warps_per_sm, bool masked) {
+    static const double eff_m[2][3] = {{0.50, 0.65, 0.69}, {0.62, 0.67, 0.70}};   // KI = 1, 2:  8 / 16 / 32 warps per SM
+    static const double eff_p[2][3] = {{0.51, 0.73, 0.82}, {0.69, 0.81, 0.85}};
+    const int r = KI == 1 ? 0 : 1, c = warps_per_sm >= 32 ? 2 : (warps_per_sm >= 16 ? 1 : 0);
+    return masked ? eff_m[r][c] : eff_p[r][c];
+}
+
+// cycles of one small call under a plan; constants from the scans in profiles/r02_small_calls.md
+inline double small_plan_cost(int64_t n_i, int64_t n_j, int sm_count, int NW, int KI, int LJ, int WJ, int S, int CS) {
+    const int tile_i = (NW / WJ) * KI * (32 / LJ);
+    const int64_t tiles_i = (n_i + tile_i - 1) / tile_i;
+    const int Q = WJ * LJ;
+    const double ctas = double(tiles_i) * S;
+    const double per_sm = double((int64_t)((ctas + sm_count - 1) / sm_count));      // CTAs on the busiest SM
+    const double max_res = NW == 16 ? 2.0 : 4.0;
+    const double resident = per_sm > max_res ? max_res : per_sm;                    // beyond that they run in waves
+    double waves = double((int64_t)((per_sm + resident - 1) / resident));
+    // A cluster of 8 must sit inside one GPC (16 .. 20 SMs): at most 15 clusters per resident CTA are active at a time on
+    // a B200 (ncu launch__cluster_max_active), i.e. 120 of the 148 SMs -- more clusters run as further waves.
+    if (CS == kSmallClusterMax) {
+        const double cap = 15.0 * resident;
+        const double cw = double((int64_t)((ctas / CS + cap - 1) / cap));
+        if (cw > waves) waves = cw;
+    }
+    const int64_t chunk = (n_j + S - 1) / S;
+    const double pairs_per_thread = double((((chunk + Q - 1) / Q) + 1) / 2);
+    const double groups = pairs_per_thread * KI;                                    // packed groups of a thread
+    // a scheduler holds NW / 4 warps of every resident CTA; a packed group occupies its FMA pipe for 26 cycles
+    const int wps = (int)(NW * resident);
+    const double eff = small_loop_eff(KI, wps, true);
+    double loop = resident * groups * (NW / 4) * 26.0 / eff;
+    if (LJ > 1) loop *= 1.0 + 0.35 * LJ;                                            // LJ distinct addresses per LDS.128: shared-memory bandwidth
+    const double lone = groups * 40.0;                                              // one warp's dependent chains
+    if (loop < lone) loop = lone;
+    const double rounds = double((chunk + kSmallRoundJPlan - 1) / kSmallRoundJPlan);
+    const double staged = double(chunk > kSmallRoundJPlan ? kSmallRoundJPlan : chunk);
+    // phases measured with %globaltimer stamps on C2 (profiles/r02_small_calls.md): staging 1.3 us, lane / warp sums
+    // 0.8 us, partial + fence + ticket 1.0 us, final sums 0.5 us + the tile's partials through one SM's L2 port
+    double c = 1200.0 + 1600.0 * rounds + staged * resident * 0.5;                  // start, staging latency, L2 -> shared memory
+    c += loop + 40.0 * KI * (pairs_per_thread / 64.0 + 1.0);
+    if (LJ > 1) c += 30.0 * KI * LJ;
+    c += (WJ > 1) ? 900.0 + 40.0 * WJ : 300.0;
+    if (CS > 1) c += 1200.0 + 40.0 * CS;
+    const int n_groups = S / CS;
+    if (n_groups > 1) c += 2000.0 + 1000.0 + 260.0 * n_groups;                      // ticket; final sums ~0.13 us per group
+    return c * waves;
+}
+
+inline SmallPlan make_small_plan(int64_t n_i, int64_t n_j, int sm_count) {
+    if (sm_count <= 0) sm_count = 148;
+    static const int shapes[6][3] = {{16, 2, 1}, {8, 2, 1}, {16, 1, 1}, {8, 1, 1}, {8, 1, 2}, {8, 1, 4}};   // (NW, KI, LJ)
+    static const int wj_opts[5] = {1, 2, 4, 8, 16};
+    SmallPlan best{};
+    double best_cost = -1.0;
+    for (int sh = 0; sh < 6; ++sh) {
+        const int NW = shapes[sh][0], KI = shapes[sh][1], LJ = shapes[sh][2];
+        for (int w = 0; w < 5; ++w) {
+            const int WJ = wj_opts[w];
+            if (WJ > NW) continue;
+            const int tile_i = (NW / WJ) * KI * (32 / LJ);
+            if (tile_i > 8 && (int64_t)tile_i >= 2 * n_i) continue;               // a smaller tile covers all i
+            const int64_t tiles_i = (n_i + tile_i - 1) / tile_i;
+            const int Q = WJ * LJ;
+            for (int cs = 0; cs < 2; ++cs) {
+                const int CS = cs ? kSmallClusterMax : 1;
+                if (!small_shape_ok(NW, KI, LJ, WJ, CS)) continue;
+                int64_t cand[8];
+                int n_cand = 0;
+                cand[n_cand++] = CS;
+                for (int m = 1; m <= 4; ++m) {
+                    int64_t S = (int64_t)m * sm_count / tiles_i / CS * CS;
+                    if (S >= CS) cand[n_cand++] = S;
+                }
+                for (int q = 0; q < n_cand; ++q) {
+                    int64_t S = cand[q];
+                    const int64_t s_max = (n_j / (2 * Q) / CS) * CS;                 // every slot gets at least one pair
+                    if (S > s_max) S = s_max;
+                    if (S < CS) S = CS;
+                    if (S > kMaxS) S = kMaxS / CS * CS;
+                    if (CS == 1 && S > 64) continue;                                // without clusters the last CTA of a tile sums alone
+                    const double c = small_plan_cost(n_i, n_j, sm_count, NW, KI, LJ, WJ, (int)S, CS);
+                    if (best_cost < 0.0 || c < best_cost * (1.0 - 1e-9)) {
+                        best_cost = c;
+                        best.NW = NW; best.KI = KI; best.LJ = LJ; best.WJ = WJ; best.S = (int)S; best.CS = CS;
+                    }
+                }
+            }
+        }
+    }
+    best.tile_i = (best.NW / best.WJ) * best.KI * (32 / best.LJ);
     best.tiles_i = (int)((n_i + best.tile_i - 1) / best.tile_i);
-    ring_shape(best.WJ, &best.tile_j, &best.stages);
     return best;
 }
 

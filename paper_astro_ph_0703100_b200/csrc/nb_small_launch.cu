@@ -1,0 +1,99 @@
+// nb_small_launch.cu -- instantiations and launch dispatch of nb_small_kernel (nb_small.cuh), a translation unit of
+// its own so that it compiles in parallel with nbody_b200.cu.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdint>
+
+#include "nb_small.cuh"
+#include "nb_plan.h"
+#include "nb_small_launch.h"
+
+namespace nb {
+
+// dynamic shared memory: the staged j-pairs, reused for the reductions
+size_t small_smem_bytes(const SmallPlan& p, int64_t n_j) {
+    const int Q = p.WJ * p.LJ;
+    const int64_t chunk_max = (n_j + p.S - 1) / p.S + 2;     // as in nb_small_kernel (even chunk boundaries)
+    const int round_max = (int)(chunk_max < kSmallRoundJ ? chunk_max : kSmallRoundJ);
+    const size_t stage = (size_t)Q * small_pair_stride(small_slot_len(round_max, Q)) * 32;
+    const size_t red = ((p.WJ > 1 ? (size_t)p.WJ * p.tile_i : 0) + (size_t)p.tile_i) * sizeof(double4);
+    return ((stage > red ? stage : red) + 127) / 128 * 128 + 128;
+}
+
+namespace {
+
+template <int NW, int KI, int LJ, int WJ, int MODE, bool PHI, int CS>
+cudaError_t launch_inst(const SmallPlan& p, const SmallArgs& a, size_t smem, cudaStream_t stream) {
+    auto kern = nb_small_kernel<NW, KI, LJ, WJ, MODE, PHI, CS>;
+    static std::atomic<uint64_t> configured{0};                       // bit d: device d has the raised shared-memory limit
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const uint64_t bit = 1ull << (dev & 63);
+    if (!(configured.load(std::memory_order_acquire) & bit)) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
+        if (e != cudaSuccess) return e;
+        configured.fetch_or(bit, std::memory_order_release);
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)p.tiles_i, (unsigned)p.S, 1);
+    cfg.blockDim = dim3(32 * NW, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    if (CS > 1) {
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 1;
+        attr[0].val.clusterDim.y = CS;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+    }
+    return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
+template <int NW, int KI, int LJ, int WJ, int MODE, bool PHI>
+cudaError_t launch_cs(const SmallPlan& p, const SmallArgs& a, size_t smem, cudaStream_t stream) {
+    constexpr int TILE_I = (NW / WJ) * KI * (32 / LJ);
+    if (p.CS == 1) return launch_inst<NW, KI, LJ, WJ, MODE, PHI, 1>(p, a, smem, stream);
+    if constexpr (TILE_I % kSmallClusterMax == 0) {
+        if (p.CS == kSmallClusterMax) return launch_inst<NW, KI, LJ, WJ, MODE, PHI, kSmallClusterMax>(p, a, smem, stream);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <int NW, int KI, int MODE, bool PHI>
+cudaError_t launch_wide(const SmallPlan& p, const SmallArgs& a, size_t smem, cudaStream_t stream) {
+    switch (p.WJ) {
+        case 1: return launch_cs<NW, KI, 1, 1, MODE, PHI>(p, a, smem, stream);
+        case 2: return launch_cs<NW, KI, 1, 2, MODE, PHI>(p, a, smem, stream);
+        case 4: return launch_cs<NW, KI, 1, 4, MODE, PHI>(p, a, smem, stream);
+        case 8: return launch_cs<NW, KI, 1, 8, MODE, PHI>(p, a, smem, stream);
+        case 16:
+            if constexpr (NW == 16) return launch_cs<NW, KI, 1, 16, MODE, PHI>(p, a, smem, stream);
+            return cudaErrorInvalidValue;
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+// the shapes of nb::small_shape_ok (nb_plan.h)
+template <int MODE, bool PHI>
+cudaError_t launch_shape(const SmallPlan& p, const SmallArgs& a, size_t smem, cudaStream_t stream) {
+    if (!small_shape_ok(p.NW, p.KI, p.LJ, p.WJ, p.CS)) return cudaErrorInvalidValue;
+    if (p.LJ == 2) return launch_cs<8, 1, 2, 8, MODE, PHI>(p, a, smem, stream);
+    if (p.LJ == 4) return launch_cs<8, 1, 4, 8, MODE, PHI>(p, a, smem, stream);
+    if (p.NW == 16) return p.KI == 2 ? launch_wide<16, 2, MODE, PHI>(p, a, smem, stream) : launch_wide<16, 1, MODE, PHI>(p, a, smem, stream);
+    return p.KI == 2 ? launch_wide<8, 2, MODE, PHI>(p, a, smem, stream) : launch_wide<8, 1, MODE, PHI>(p, a, smem, stream);
+}
+
+}  // namespace
+
+cudaError_t small_launch(const SmallPlan& p, const SmallArgs& a, int mode, cudaStream_t stream) {
+    if (p.S % p.CS != 0 || p.S < 1) return cudaErrorInvalidValue;
+    const size_t smem = small_smem_bytes(p, a.n_j);
+    return mode == SMALL_NONE ? launch_shape<SMALL_NONE, false>(p, a, smem, stream)
+                              : launch_shape<SMALL_EXACT, true>(p, a, smem, stream);
+}
+
+}  // namespace nb

@@ -1,11 +1,15 @@
 // nbody_b200.cu -- C-ABI shim, workspace and launch logic of libnbody_b200.so (include/nbody_b200.h).
 #include "../../include/nbody_b200.h"
+#include "../../include/nb_debug.h"
 
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cmath>
 #include <cstdint>
+#include <cstdio>
 #include <cstdlib>
+#include <cstring>
 #include <map>
 #include <mutex>
 #include <tuple>
@@ -18,6 +22,8 @@
 #include "nb_batched.cuh"
 #include "nb_pipelines.cuh"
 #include "nb_plan.h"
+#include "nb_small.cuh"
+#include "nb_small_launch.h"
 
 #define NB_VERSION 100
 
@@ -55,13 +61,110 @@ struct Workspace {
     void* hstate = nullptr;    size_t hstate_bytes = 0;    // Hermite integrator: xp, vp, a1, j1
     void* jp2 = nullptr;       size_t jp2_bytes = 0;       // force + jerk: 32-byte j records
     void* hpartial = nullptr;  size_t hpartial_bytes = 0;  // force + jerk: [S][n_i][10] double
+    std::recursive_mutex busy;                             // held while a call grows the buffers and enqueues work that uses them
+};
+
+// Debugging switches (include/nb_debug.h): read from the environment once, changed only through nb_debug_set.
+struct Knobs {
+    bool plan_set = false;       int pK = 0, pWI = 0, pWJ = 0, pS = 0;                 // NB_PLAN
+    bool small_plan_set = false; int sNW = 0, sKI = 0, sLJ = 0, sWJ = 0, sS = 0, sCS = 0;   // NB_SMALL_PLAN
+    int small = -1;              // NB_SMALL: -1 default, 0 never, 1 always
+    int mask = -1;               // NB_MASK: -1 default, else nb::MODE_*
+    int fused = -1;              // NB_FUSED_REDUCE
+    int direct = -1;             // NB_DIRECT
+    int step_graph = -1;         // NB_STEP_GRAPH
+    int batch_tile = 0;          // NB_BATCH_TILE
 };
 
 std::mutex g_mutex;
+std::atomic<const Knobs*> g_knobs{nullptr};
+std::atomic<int64_t> g_plans_computed{0};
 DeviceInfo g_dev[64];
 std::map<std::pair<int, cudaStream_t>, Workspace> g_ws;
 std::map<std::tuple<int64_t, int64_t, int>, nb::Plan> g_plans;
 std::map<std::tuple<int64_t, int64_t, int>, nb::Plan> g_hplans;
+
+// ---- debugging switches
+bool parse_knob(Knobs* k, const char* key, const char* value) {
+    const bool unset = !value || !value[0];
+    if (!std::strcmp(key, "NB_PLAN")) {
+        if (unset) { k->plan_set = false; return true; }
+        int a, b, c, d;
+        if (std::sscanf(value, "%d,%d,%d,%d", &a, &b, &c, &d) != 4) return false;
+        if (!((a == 2 || a == 4 || a == 8) && b * c == nb::kWarpsPerCta && (c == 1 || c == 2 || c == 4 || c == 8) && d >= 1 && d <= nb::kMaxS)) return false;
+        k->plan_set = true; k->pK = a; k->pWI = b; k->pWJ = c; k->pS = d;
+        return true;
+    }
+    if (!std::strcmp(key, "NB_SMALL_PLAN")) {
+        if (unset) { k->small_plan_set = false; return true; }
+        int nw, ki, lj, wj, ss, cs;
+        if (std::sscanf(value, "%d,%d,%d,%d,%d,%d", &nw, &ki, &lj, &wj, &ss, &cs) != 6) return false;
+        if (!(nb::small_shape_ok(nw, ki, lj, wj, cs) && ss >= cs && ss % cs == 0 && ss <= nb::kMaxS)) return false;
+        k->small_plan_set = true; k->sNW = nw; k->sKI = ki; k->sLJ = lj; k->sWJ = wj; k->sS = ss; k->sCS = cs;
+        return true;
+    }
+    if (!std::strcmp(key, "NB_MASK")) {
+        if (unset) { k->mask = -1; return true; }
+        if (value[0] == 'e') k->mask = nb::MODE_EXACT; else if (value[0] == 'b') k->mask = nb::MODE_BLOOM;
+        else if (value[0] == 'l') k->mask = nb::MODE_LIST; else return false;
+        return true;
+    }
+    int* flag = !std::strcmp(key, "NB_SMALL") ? &k->small : !std::strcmp(key, "NB_FUSED_REDUCE") ? &k->fused :
+                !std::strcmp(key, "NB_DIRECT") ? &k->direct : !std::strcmp(key, "NB_STEP_GRAPH") ? &k->step_graph : nullptr;
+    if (flag) {
+        if (unset) { *flag = -1; return true; }
+        if (value[0] != '0' && value[0] != '1') return false;
+        *flag = value[0] - '0';
+        return true;
+    }
+    if (!std::strcmp(key, "NB_BATCH_TILE")) {
+        if (unset) { k->batch_tile = 0; return true; }
+        const int t = std::atoi(value);
+        if (t != 64 && t != 128 && t != 256) return false;
+        k->batch_tile = t;
+        return true;
+    }
+    return false;
+}
+
+const char* const kKnobKeys[] = {"NB_PLAN", "NB_SMALL_PLAN", "NB_SMALL", "NB_MASK", "NB_FUSED_REDUCE", "NB_DIRECT", "NB_STEP_GRAPH", "NB_BATCH_TILE"};
+
+// the current switches: one atomic load per call; the environment is read once, here
+const Knobs& knobs() {
+    const Knobs* k = g_knobs.load(std::memory_order_acquire);
+    if (k) return *k;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    k = g_knobs.load(std::memory_order_acquire);
+    if (k) return *k;
+    Knobs* fresh = new Knobs();
+    for (const char* key : kKnobKeys)
+        if (const char* v = std::getenv(key)) (void)parse_knob(fresh, key, v);   // a value that does not parse is ignored
+    g_knobs.store(fresh, std::memory_order_release);
+    return *fresh;
+}
+
+// ---- per (device, stream) workspace, locked for the duration of one call's enqueue sequence
+struct WsGuard {
+    Workspace* ws;
+    std::unique_lock<std::recursive_mutex> hold;
+    WsGuard(int dev, cudaStream_t stream) {
+        {
+            std::lock_guard<std::mutex> lock(g_mutex);
+            ws = &g_ws[std::make_pair(dev, stream)];
+        }
+        hold = std::unique_lock<std::recursive_mutex>(ws->busy);
+    }
+};
+
+void free_workspace(Workspace* w) {
+    void** bufs[] = {&w->jp, &w->partial, &w->stage, &w->coin, &w->tickets, &w->jp2, &w->tiles, &w->pipe, &w->hstate, &w->hpartial};
+    for (void** b : bufs) {
+        if (*b) (void)cudaFree(*b);
+        *b = nullptr;
+    }
+    w->jp_bytes = w->partial_bytes = w->stage_bytes = w->coin_bytes = w->tickets_bytes = w->jp2_bytes = w->tiles_bytes =
+        w->pipe_bytes = w->hstate_bytes = w->hpartial_bytes = 0;
+}
 
 int device_info(int* dev_out, DeviceInfo* out) {
     int dev = 0;
@@ -98,15 +201,33 @@ int ensure(void** ptr, size_t* have, size_t need, cudaStream_t stream) {
     return NB_OK;
 }
 
-nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count) {
+constexpr double kHermiteInstPerPair = 27.0;     // force + jerk + potential (row f1): FP32-pipe instructions per pair
+constexpr double kHermitePartialBytes = 80.0;    // ... and bytes per (chunk, i) of its second-pass partials
+
+// NB_PLAN (nb_debug.h) overrides the planner's choice; a forced plan is not remembered
+bool forced_plan(const Knobs& kn, int k_max, int64_t n_i, nb::Plan* out) {
+    if (!kn.plan_set || kn.pK > k_max) return false;
+    *out = nb::finish_plan(kn.pK, kn.pWI, kn.pWJ, kn.pS, n_i);
+    return true;
+}
+
+// The planner costs ~3 us per new shape (nb_plan.h); repeated shapes are served from a small per-process table.
+nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count, bool jerk = false) {
+    nb::Plan p;
+    if (forced_plan(knobs(), jerk ? 4 : 8, n_i, &p)) return p;
+    auto& table = jerk ? g_hplans : g_plans;
+    const auto key = std::make_tuple(n_i, n_j, sm_count);
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        auto it = table.find(key);
+        if (it != table.end()) return it->second;
+    }
+    p = jerk ? nb::make_plan(n_i, n_j, sm_count, 4, kHermiteInstPerPair, kHermitePartialBytes)
+             : nb::make_plan(n_i, n_j, sm_count);                          // outside the lock
+    g_plans_computed.fetch_add(1, std::memory_order_relaxed);
     std::lock_guard<std::mutex> lock(g_mutex);
-    auto key = std::make_tuple(n_i, n_j, sm_count);
-    auto it = g_plans.find(key);
-    if (it != g_plans.end() && !std::getenv("NB_PLAN")) return it->second;
-    nb::Plan p = nb::make_plan(n_i, n_j, sm_count);
-    if (std::getenv("NB_PLAN")) return p;                              // a forced plan is not remembered
-    if (g_plans.size() > 4096) g_plans.clear();
-    g_plans[key] = p;
+    if (table.size() > 4096) table.clear();
+    table[key] = p;
     return p;
 }
 
@@ -125,15 +246,15 @@ constexpr double kBloomMinPairs = 33554432.0;    // 2^25
 constexpr double kListMinPairsJerk = 1073741824.0;   // 2^30: the jerk kernel's pre-pass pays off earlier (measured tie at N = 32768)
 
 int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool bloom_ok, double list_min_pairs = kListMinPairs) {
-    // debugging aid: NB_MASK=exact|bloom|list forces a mode (bloom and list still need eps2 >= 2^-40, list n_j <= 2^29)
-    const char* e = std::getenv("NB_MASK");
-    if (e && e[0] == 'e') return nb::MODE_EXACT;
+    // debugging aid (nb_debug.h): NB_MASK forces a mode (bloom and list still need eps2 >= 2^-40, list n_j <= 2^29)
+    const int forced = knobs().mask;
+    if (forced == nb::MODE_EXACT) return nb::MODE_EXACT;
     if (eps2 < kUnmaskedMinEps2) return nb::MODE_EXACT;
     const bool list_ok = n_j <= ((int64_t)1 << 29);                    // the 32-bit hash table holds 2 n_j <= 2^30 slots
     const double pairs = (double)n_i * (double)n_j;
-    if (!bloom_ok) return (list_ok && ((e && e[0] == 'l') || pairs >= kListMinPairsNoBloom)) ? nb::MODE_LIST : nb::MODE_EXACT;
-    if (e && e[0] == 'l') return list_ok ? nb::MODE_LIST : nb::MODE_EXACT;
-    if (e && e[0] == 'b') return nb::MODE_BLOOM;
+    if (!bloom_ok) return (list_ok && (forced == nb::MODE_LIST || pairs >= kListMinPairsNoBloom)) ? nb::MODE_LIST : nb::MODE_EXACT;
+    if (forced == nb::MODE_LIST) return list_ok ? nb::MODE_LIST : nb::MODE_EXACT;
+    if (forced == nb::MODE_BLOOM) return nb::MODE_BLOOM;
     if (list_ok && pairs >= list_min_pairs) return nb::MODE_LIST;
     return pairs >= kBloomMinPairs ? nb::MODE_BLOOM : nb::MODE_EXACT;
 }
@@ -141,13 +262,14 @@ int pick_mode(int64_t n_i, int64_t n_j, float eps2, bool bloom_ok, double list_m
 // One launch of a dominant kernel: raises the kernel's dynamic shared-memory limit once per device, brackets the
 // launch with two events on the launching stream while nb_profile_enable is on, counts it.
 template <class Kernel, class Args>
-int launch_dominant(Kernel kern, bool* configured, dim3 grid, unsigned threads, size_t smem, cudaStream_t stream,
+int launch_dominant(Kernel kern, std::atomic<uint64_t>* configured, dim3 grid, unsigned threads, size_t smem, cudaStream_t stream,
                     const Args& args) {
     int dev = 0;
     NB_CUDA(cudaGetDevice(&dev));
-    if (!configured[dev & 63]) {
+    const uint64_t bit = 1ull << (dev & 63);                           // bit d: device d has the raised limit (idempotent: a race only repeats the call)
+    if (!(configured->load(std::memory_order_acquire) & bit)) {
         NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured[dev & 63] = true;
+        configured->fetch_or(bit, std::memory_order_release);
     }
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (t_profile) {
@@ -171,8 +293,8 @@ int launch_force_inst(const nb::ForceArgs& args, const nb::Plan& plan, cudaStrea
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * 4 * (WI * 32) * sizeof(double) : 0;
     constexpr size_t bloom = (MODE == nb::MODE_BLOOM) ? (size_t)WI * nb::kBloomWords * sizeof(uint32_t) : 0;
     constexpr size_t smem = (ring + bloom > red ? ring + bloom : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    static bool configured[64] = {};
-    return launch_dominant(nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, EPS_I, PHI, DIRECT>, configured,
+    static std::atomic<uint64_t> configured{0};
+    return launch_dominant(nb::nb_force_kernel<K, WI, WJ, TJ, STAGES, MODE, EPS_I, PHI, DIRECT>, &configured,
                            dim3((unsigned)plan.tiles_i, (unsigned)plan.S, 1), 32 * WI * WJ, smem, stream, args);
 }
 
@@ -235,6 +357,14 @@ int coin_prepass(Workspace* ws, const nb::Plan& plan, int64_t n_i, const float* 
     return NB_OK;
 }
 
+// Which calls take the small-i-set kernel (nb_small.cuh): few i-particles, where nb_force_kernel's packing over i leaves
+// a thread one dependent chain (thresholds from the scan in profiles/r02_small_calls.md).  NB_SMALL=0/1 forces.
+bool use_small_path(const Knobs& kn, int64_t n_i, int64_t n_j) {
+    if (kn.small >= 0) return kn.small != 0;
+    if (kn.plan_set || kn.mask >= 0 || kn.fused >= 0 || kn.direct >= 0) return false;   // a switch of nb_force_kernel's paths is set
+    return nb::small_by_default(n_i, n_j);
+}
+
 // pack (a1) when repack is true, then force (+ reduce).  The packed array lives in the workspace.
 // eps2_i != nullptr: row f3, the softening of every i-particle comes from that device array and eps2 is ignored.
 int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
@@ -256,18 +386,77 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         if (pot_out) NB_CUDA(cudaMemsetAsync(pot_out, 0, sizeof(float) * (size_t)n_i, stream));
         return NB_OK;
     }
-    const nb::Plan plan = cached_plan(n_i, n_j, info.sm_count);
+    const Knobs& kn = knobs();
+    // Without phi no pair needs a mask when eps2 >= 2^-40: an unmasked coincident pair adds m u^3 * (+-0) = +-0 to a
+    // (only phi would get m / eps), so a_i is bit for bit the masked loop's.  The list-mode kernel then runs with an
+    // empty list: no pre-pass, the untested loop everywhere (nb_leapfrog_kdk: every evaluation but the last).
+    const bool a_only = !pot_out && !eps2_i && eps2 >= kUnmaskedMinEps2 && kn.mask < 0;
 
-    Workspace* ws;
-    {
-        std::lock_guard<std::mutex> lock(g_mutex);
-        ws = &g_ws[std::make_pair(dev, stream)];
+    WsGuard guard(dev, stream);
+    Workspace* ws = guard.ws;
+
+    // Small i-sets: the kernel packed over j (nb_small.cuh), one launch, cluster + ticket reduction of the j-split.
+    if (!eps2_i && use_small_path(kn, n_i, n_j)) {
+        nb::SmallPlan sp = nb::make_small_plan(n_i, n_j, info.sm_count);
+        if (kn.small_plan_set) {
+            sp.NW = kn.sNW; sp.KI = kn.sKI; sp.LJ = kn.sLJ; sp.WJ = kn.sWJ; sp.S = kn.sS; sp.CS = kn.sCS;
+            sp.tile_i = (sp.NW / sp.WJ) * sp.KI * (32 / sp.LJ);
+            sp.tiles_i = (int)((n_i + sp.tile_i - 1) / sp.tile_i);
+        }
+        const int n_groups = sp.S / sp.CS;
+        if (n_groups > 1) {
+            rc = ensure(&ws->partial, &ws->partial_bytes, (size_t)n_groups * (size_t)n_i * sizeof(double4), stream);
+            if (rc != NB_OK) return rc;
+            const size_t need = (size_t)sp.tiles_i * sp.CS * sizeof(int);
+            if (need > ws->tickets_bytes) {
+                rc = ensure(&ws->tickets, &ws->tickets_bytes, need, stream);
+                if (rc != NB_OK) return rc;
+                NB_CUDA(cudaMemsetAsync(ws->tickets, 0, ws->tickets_bytes, stream));   // once per growth; kernels leave zeros
+            }
+        }
+        nb::SmallArgs sa;
+        sa.x_i = x_i;
+        sa.xj_raw = packed_j ? nullptr : x_j;
+        sa.mj_raw = packed_j ? nullptr : m_j;
+        sa.jp = packed_j;
+        sa.acc = acc_out;
+        sa.pot = pot_out;
+        sa.partial = reinterpret_cast<double4*>(ws->partial);
+        sa.tickets = reinterpret_cast<int*>(ws->tickets);
+        sa.n_i = (int)n_i;
+        sa.n_j = (int)n_j;
+        sa.S = sp.S;
+        sa.eps2 = eps2;
+        // coincident pairs: no mask at all without phi (eps2 >= 2^-40), else every pair masked
+        const int small_mode = a_only ? nb::SMALL_NONE : nb::SMALL_EXACT;
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        if (t_profile) {
+            NB_CUDA(cudaEventCreate(&e0));
+            NB_CUDA(cudaEventCreate(&e1));
+            NB_CUDA(cudaEventRecord(e0, stream));
+        }
+        NB_CUDA(nb::small_launch(sp, sa, small_mode, stream));
+        if (t_profile) {
+            NB_CUDA(cudaEventRecord(e1, stream));
+            t_events.emplace_back(e0, e1);
+        }
+        ++t_launches;
+        return NB_OK;
     }
-    rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)n_j * sizeof(float4), stream);
-    if (rc != NB_OK) return rc;
-    // second pass: fused into the force kernel or a separate launch (nb_plan.h: fused_second_pass); NB_FUSED_REDUCE=0/1 forces
-    const char* fr = std::getenv("NB_FUSED_REDUCE");
-    const bool fused_reduce = fr ? (fr[0] != '0') : nb::fused_second_pass(plan.tile_i, plan.S);
+
+    const nb::Plan plan = cached_plan(n_i, n_j, info.sm_count);
+    const int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2, eps2_i == nullptr);
+    // Small calls whose per-warp-group j sub-range fits its shared-memory ring whole: the force kernel packs the
+    // sub-range itself, one launch fewer.  NB_DIRECT=0 (nb_debug.h) disables it (tests compare).
+    const int64_t sub_max = (n_j + (int64_t)plan.S * plan.WJ - 1) / ((int64_t)plan.S * plan.WJ);
+    const bool direct = !packed_j && !eps2_i && mode != nb::MODE_LIST && sub_max <= (int64_t)plan.tile_j * plan.stages &&
+                        kn.direct != 0;
+    if (!packed_j && !direct) {                                        // the packed records live in the workspace
+        rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)n_j * sizeof(float4), stream);
+        if (rc != NB_OK) return rc;
+    }
+    // second pass: fused into the force kernel or a separate launch (nb_plan.h: fused_second_pass); NB_FUSED_REDUCE forces
+    const bool fused_reduce = kn.fused >= 0 ? (kn.fused != 0) : nb::fused_second_pass(plan.tile_i, plan.S);
     if (plan.S > 1) {
         rc = ensure(&ws->partial, &ws->partial_bytes, (size_t)plan.S * (size_t)n_i * sizeof(double4), stream);
         if (rc != NB_OK) return rc;
@@ -277,18 +466,6 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
             NB_CUDA(cudaMemsetAsync(ws->tickets, 0, ws->tickets_bytes, stream));   // once per growth; kernels leave zeros
         }
     }
-
-    const int mode = pick_mode(n_i, n_j, eps2_i ? 1.0f : eps2, eps2_i == nullptr);
-    // Without phi no pair needs a mask when eps2 >= 2^-40: an unmasked coincident pair adds m u^3 * (+-0) = +-0 to a
-    // (only phi would get m / eps), so a_i is bit for bit the masked loop's.  The list-mode kernel then runs with an
-    // empty list: no pre-pass, the untested loop everywhere (nb_leapfrog_kdk: every evaluation but the last).
-    const bool a_only = !pot_out && !eps2_i && eps2 >= kUnmaskedMinEps2 && !std::getenv("NB_MASK");
-    // Small calls whose per-warp-group j sub-range fits its shared-memory ring whole: the force kernel packs the
-    // sub-range itself, one launch fewer (C0: 21 -> 16 us per call).  NB_DIRECT=0 disables it (tests compare).
-    const int64_t sub_max = (n_j + (int64_t)plan.S * plan.WJ - 1) / ((int64_t)plan.S * plan.WJ);
-    const char* dr = std::getenv("NB_DIRECT");
-    const bool direct = !packed_j && !eps2_i && mode != nb::MODE_LIST && sub_max <= (int64_t)plan.tile_j * plan.stages &&
-                        !(dr && dr[0] == '0');
     const float4* jp = packed_j ? packed_j : reinterpret_cast<const float4*>(ws->jp);
     if (!packed_j && !direct) {   // a1: j-pack
         const int threads = 256;
@@ -349,9 +526,6 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
 
 
 // ------------------------------------------------------------------ row f1: force + jerk + potential
-constexpr double kHermiteInstPerPair = 27.0;
-constexpr double kHermitePartialBytes = 80.0;
-
 nb::Plan hermite_plan(int64_t n_i, int64_t n_j, int sm_count) {
     return nb::make_plan(n_i, n_j, sm_count, 4, kHermiteInstPerPair, kHermitePartialBytes);
 }
@@ -363,8 +537,8 @@ int launch_hermite_inst(const nb::HermiteArgs& args, const nb::Plan& plan, cudaS
     constexpr size_t red = (WJ > 1) ? (size_t)WJ * K * nb::kHermiteAcc * (WI * 32) * sizeof(double) : 0;
     constexpr size_t bloom = (MODE == nb::MODE_BLOOM) ? (size_t)WI * nb::kBloomWords * sizeof(uint32_t) : 0;
     constexpr size_t smem = (ring + bloom > red ? ring + bloom : red) + 2 * WJ * STAGES * sizeof(uint64_t) + 128;
-    static bool configured[64] = {};
-    return launch_dominant(nb::nb_hermite_kernel<K, WI, WJ, TJ, STAGES, MODE, PHI>, configured,
+    static std::atomic<uint64_t> configured{0};
+    return launch_dominant(nb::nb_hermite_kernel<K, WI, WJ, TJ, STAGES, MODE, PHI>, &configured,
                            dim3((unsigned)plan.tiles_i, (unsigned)plan.S, 1), 32 * WI * WJ, smem, stream, args);
 }
 
@@ -412,31 +586,16 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
         if (pot_out) NB_CUDA(cudaMemsetAsync(pot_out, 0, sizeof(float) * (size_t)n_i, stream));
         return NB_OK;
     }
-    nb::Plan plan;
-    {
-        std::lock_guard<std::mutex> lock(g_mutex);
-        auto key = std::make_tuple(n_i, n_j, info.sm_count);
-        auto it = g_hplans.find(key);
-        if (it != g_hplans.end() && !std::getenv("NB_PLAN")) {
-            plan = it->second;
-        } else {
-            plan = hermite_plan(n_i, n_j, info.sm_count);
-            if (g_hplans.size() > 4096) g_hplans.clear();
-            if (!std::getenv("NB_PLAN")) g_hplans[key] = plan;       // a forced plan is not remembered
-        }
-    }
-    Workspace* ws;
-    {
-        std::lock_guard<std::mutex> lock(g_mutex);
-        ws = &g_ws[std::make_pair(dev, stream)];
-    }
+    const Knobs& kn = knobs();
+    const nb::Plan plan = cached_plan(n_i, n_j, info.sm_count, true);
+    WsGuard guard(dev, stream);
+    Workspace* ws = guard.ws;
     rc = ensure(&ws->jp2, &ws->jp2_bytes, (size_t)n_j * 2 * sizeof(float4), stream);
     if (rc != NB_OK) return rc;
     // second pass: fused into the kernel (small tiles) or a separate launch, as for nb_force; NB_FUSED_REDUCE=0/1 forces
-    const char* fr = std::getenv("NB_FUSED_REDUCE");
     const int mode = pick_mode(n_i, n_j, eps2, true, kListMinPairsJerk);
     const bool fused_reduce = plan.S > 1 && mode == nb::MODE_EXACT &&      // only the masked (small-call) kernels carry the ticket code
-                              (fr ? (fr[0] != '0') : nb::fused_second_pass(plan.tile_i, plan.S, kHermitePartialBytes));
+                              (kn.fused >= 0 ? (kn.fused != 0) : nb::fused_second_pass(plan.tile_i, plan.S, kHermitePartialBytes));
     if (plan.S > 1) {
         rc = ensure(&ws->hpartial, &ws->hpartial_bytes, (size_t)plan.S * (size_t)n_i * nb::kHermiteAcc * sizeof(double), stream);
         if (rc != NB_OK) return rc;
@@ -494,10 +653,7 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
 // small tiles win -- less padding in every group's last tile, and several CTAs per SM overlap their prologues.
 int batched_groups(int64_t n_i_total, int64_t n_batch) {
     const double mean = (double)n_i_total / (double)(n_batch > 0 ? n_batch : 1);
-    if (const char* e = std::getenv("NB_BATCH_TILE")) {
-        const int t = std::atoi(e);
-        if (t == 64 || t == 128 || t == 256) return t / 64;
-    }
+    if (const int t = knobs().batch_tile) return t / 64;            // NB_BATCH_TILE (nb_debug.h)
     if (mean <= 384.0) return 1;
     if (mean <= 1024.0) return 2;
     return 4;
@@ -508,8 +664,8 @@ int launch_batched_inst(const nb::ForceArgs& args, unsigned max_ctas, cudaStream
     constexpr size_t ring = (size_t)8 * STAGES * 256 * 16;
     constexpr size_t red = (size_t)8 * (2 * G) * 4 * 32 * sizeof(double);
     constexpr size_t smem = (ring > red ? ring : red) + 8 * STAGES * sizeof(uint64_t) + 128;
-    static bool configured[64] = {};
-    return launch_dominant(nb::nb_batched_kernel<MASKED, G, STAGES>, configured, dim3(max_ctas, 1, 1), 256, smem, stream, args);
+    static std::atomic<uint64_t> configured{0};
+    return launch_dominant(nb::nb_batched_kernel<MASKED, G, STAGES>, &configured, dim3(max_ctas, 1, 1), 256, smem, stream, args);
 }
 
 template <bool MASKED>
@@ -540,11 +696,8 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     int rc = device_info(&dev, &info);
     if (rc != NB_OK) return rc;
     if (n_batch == 0 || n_i_total == 0) return NB_OK;
-    Workspace* ws;
-    {
-        std::lock_guard<std::mutex> lock(g_mutex);
-        ws = &g_ws[std::make_pair(dev, stream)];
-    }
+    WsGuard guard(dev, stream);
+    Workspace* ws = guard.ws;
     rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)(n_j_total > 0 ? n_j_total : 1) * sizeof(float4), stream);
     if (rc != NB_OK) return rc;
     const int groups = batched_groups(n_i_total, n_batch);
@@ -587,7 +740,7 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     args.S = 1;
     args.eps2 = eps2;
     // every pair masked -- unless phi is not wanted and eps2 >= 2^-40, where no pair needs the mask (see force_impl)
-    const bool a_only = !pot_out && eps2 >= kUnmaskedMinEps2 && !std::getenv("NB_MASK");
+    const bool a_only = !pot_out && eps2 >= kUnmaskedMinEps2 && knobs().mask < 0;
     return a_only ? launch_batched<false>(args, groups, (unsigned)max_ctas, stream)
                   : launch_batched<true>(args, groups, (unsigned)max_ctas, stream);
 }
@@ -612,11 +765,8 @@ int nb_force_jerk_host(int64_t n_i, const float* x_i, const float* v_i, int64_t 
     if (rc != NB_OK) return rc;
     if (n_i == 0) return NB_OK;
     cudaStream_t stream = nullptr;   // legacy default stream
-    Workspace* ws;
-    {
-        std::lock_guard<std::mutex> lock(g_mutex);
-        ws = &g_ws[std::make_pair(dev, stream)];
-    }
+    WsGuard guard(dev, stream);
+    Workspace* ws = guard.ws;
     auto up = [](size_t b) { return (b + 255) / 256 * 256; };
     const bool aliased = (x_i == x_j && v_i == v_j && n_i <= n_j);
     const size_t b_j3 = up(sizeof(float) * 3 * (size_t)n_j), b_mj = up(sizeof(float) * (size_t)n_j);
@@ -689,11 +839,8 @@ int cunbody_call(const float* p_xj, const float* p_xi, float* p_fi, int64_t ni, 
     int rc = device_info(&dev, &info);
     if (rc != NB_OK) return rc;
     if (ni == 0) return NB_OK;
-    Workspace* ws;
-    {
-        std::lock_guard<std::mutex> lock(g_mutex);
-        ws = &g_ws[std::make_pair(dev, stream)];
-    }
+    WsGuard guard(dev, stream);
+    Workspace* ws = guard.ws;
     const size_t need = nj > 0 ? nb::pipeline_workspace_bytes<P>(ni, nj, info.sm_count) : 0;
     if (need) {
         rc = ensure(&ws->pipe, &ws->pipe_bytes, need, stream);
@@ -768,11 +915,8 @@ int nb_force_host(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, 
     if (rc != NB_OK) return rc;
     if (n_i == 0) return NB_OK;
     cudaStream_t stream = nullptr;   // legacy default stream
-    Workspace* ws;
-    {
-        std::lock_guard<std::mutex> lock(g_mutex);
-        ws = &g_ws[std::make_pair(dev, stream)];
-    }
+    WsGuard guard(dev, stream);
+    Workspace* ws = guard.ws;
     auto up = [](size_t b) { return (b + 255) / 256 * 256; };
     const bool aliased = (x_i == x_j && n_i <= n_j);
     const size_t b_xj = up(sizeof(float) * 3 * (size_t)n_j), b_mj = up(sizeof(float) * (size_t)n_j);
@@ -827,10 +971,9 @@ int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, f
     // when the caller is itself capturing this stream, nor while kernel timing events are being recorded.
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     NB_CUDA(cudaStreamIsCapturing(stream, &cap));
-    const char* ng = std::getenv("NB_STEP_GRAPH");
     const bool real_stream = reinterpret_cast<uintptr_t>(stream) > 2;   // the default streams cannot be captured
     const bool step_graph = real_stream && n_steps >= 16 && n <= 32768 && cap == cudaStreamCaptureStatusNone && !t_profile &&
-                            !(ng && ng[0] == '0');
+                            knobs().step_graph != 0;                    // NB_STEP_GRAPH=0 (nb_debug.h): every step eagerly
     int64_t launches = t_launches;
     for (int64_t s = 0; s < n_steps; ++s) {
         // opening half-kick + drift; from the second step on it also carries the previous step's
@@ -898,11 +1041,8 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
     if (rc != NB_OK) return rc;
     launches += t_launches;
     if (n_steps == 0) return NB_OK;
-    Workspace* ws;
-    {
-        std::lock_guard<std::mutex> lock(g_mutex);
-        ws = &g_ws[std::make_pair(dev, stream)];
-    }
+    WsGuard guard(dev, stream);
+    Workspace* ws = guard.ws;
     const size_t b3 = ((size_t)n3 * sizeof(float) + 255) / 256 * 256;
     rc = ensure(&ws->hstate, &ws->hstate_bytes, 4 * b3, stream);
     if (rc != NB_OK) return rc;
@@ -920,10 +1060,9 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
     // (predict, force + jerk without phi, correct) are captured once into a CUDA graph and replayed.
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     NB_CUDA(cudaStreamIsCapturing(stream, &cap));
-    const char* ng = std::getenv("NB_STEP_GRAPH");
     const bool real_stream = reinterpret_cast<uintptr_t>(stream) > 2;   // the default streams cannot be captured
     const bool step_graph = real_stream && n_steps >= 16 && n <= 32768 && cap == cudaStreamCaptureStatusNone && !t_profile &&
-                            !(ng && ng[0] == '0');
+                            knobs().step_graph != 0;                    // NB_STEP_GRAPH=0 (nb_debug.h): every step eagerly
     for (int64_t s = 0; s < n_steps; ++s) {
         if (step_graph && s == 2) {                                    // steps 0 and 1 ran eagerly: everything is warm
             cudaGraph_t graph = nullptr;
@@ -976,11 +1115,8 @@ int nb_hermite4_block_step(int64_t n, float* x, float* v, const float* m, float*
     int rc = device_info(&dev, &info);
     if (rc != NB_OK) return rc;
     if (n_act == 0) return NB_OK;                                     // nobody is due: the state stays as it is
-    Workspace* ws;
-    {
-        std::lock_guard<std::mutex> lock(g_mutex);
-        ws = &g_ws[std::make_pair(dev, stream)];
-    }
+    WsGuard guard(dev, stream);
+    Workspace* ws = guard.ws;
     const size_t b3 = ((size_t)3 * n * sizeof(float) + 255) / 256 * 256;
     rc = ensure(&ws->hstate, &ws->hstate_bytes, 6 * b3, stream);      // xp, vp [n]; a1, j1, x_i, v_i [n_act <= n]
     if (rc != NB_OK) return rc;
@@ -1036,11 +1172,8 @@ int nb_block_schedule(int64_t n, const double* t, const double* dt, double* t_ne
     DeviceInfo info;
     int rc = device_info(&dev, &info);
     if (rc != NB_OK) return rc;
-    Workspace* ws;
-    {
-        std::lock_guard<std::mutex> lock(g_mutex);
-        ws = &g_ws[std::make_pair(dev, stream)];
-    }
+    WsGuard guard(dev, stream);
+    Workspace* ws = guard.ws;
     const int n_blocks = (int)((n + nb::kSchedTile - 1) / nb::kSchedTile);
     // scratch: [n_blocks] double CTA minima | [n_blocks] int CTA counts -> offsets
     rc = ensure(&ws->tiles, &ws->tiles_bytes, (size_t)(n_blocks + 1) * (sizeof(double) + sizeof(int)), stream);
@@ -1118,16 +1251,7 @@ int nb_release_workspace(void) {
     std::lock_guard<std::mutex> lock(g_mutex);
     for (auto it = g_ws.begin(); it != g_ws.end();) {
         if (it->first.first == dev) {
-            if (it->second.jp) (void)cudaFree(it->second.jp);
-            if (it->second.partial) (void)cudaFree(it->second.partial);
-            if (it->second.stage) (void)cudaFree(it->second.stage);
-            if (it->second.coin) (void)cudaFree(it->second.coin);
-            if (it->second.tickets) (void)cudaFree(it->second.tickets);
-            if (it->second.jp2) (void)cudaFree(it->second.jp2);
-            if (it->second.tiles) (void)cudaFree(it->second.tiles);
-            if (it->second.pipe) (void)cudaFree(it->second.pipe);
-            if (it->second.hstate) (void)cudaFree(it->second.hstate);
-            if (it->second.hpartial) (void)cudaFree(it->second.hpartial);
+            free_workspace(&it->second);
             it = g_ws.erase(it);
         } else {
             ++it;
@@ -1135,6 +1259,50 @@ int nb_release_workspace(void) {
     }
     return NB_OK;
 }
+
+int nb_release_stream(void* stream_) {
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    int dev = 0;
+    NB_CUDA(cudaGetDevice(&dev));
+    NB_CUDA(cudaStreamSynchronize(stream));
+    std::lock_guard<std::mutex> lock(g_mutex);
+    auto it = g_ws.find(std::make_pair(dev, stream));
+    if (it != g_ws.end()) {
+        free_workspace(&it->second);
+        g_ws.erase(it);
+    }
+    return NB_OK;
+}
+
+int nb_plan_query_small(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]) {
+    if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
+    const nb::SmallPlan p = nb::make_small_plan(n_i, n_j, sm_count);
+    out[0] = p.NW; out[1] = p.KI; out[2] = p.LJ; out[3] = p.WJ; out[4] = p.S; out[5] = p.CS; out[6] = p.tiles_i;
+    out[7] = nb::small_by_default(n_i, n_j) ? 1 : 0;
+    return NB_OK;
+}
+
+int nb_debug_set(const char* key, const char* value) {
+    if (!key) return NB_ERR_INVALID_VALUE;
+    Knobs* fresh = new Knobs(knobs());                                 // copy, change, publish; the old copy is never freed
+    if (!parse_knob(fresh, key, value)) {                              // (a test-only call: a few dozen bytes per change)
+        delete fresh;
+        return NB_ERR_INVALID_VALUE;
+    }
+    g_knobs.store(fresh, std::memory_order_release);
+    return NB_OK;
+}
+
+int nb_debug_plan_exhaustive(int64_t n_i, int64_t n_j, int sm_count, int jerk, int64_t out[8]) {
+    if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
+    const nb::Plan p = jerk ? nb::make_plan_exhaustive(n_i, n_j, sm_count, 4, kHermiteInstPerPair, kHermitePartialBytes)
+                            : nb::make_plan_exhaustive(n_i, n_j, sm_count);
+    out[0] = p.K; out[1] = p.WI; out[2] = p.WJ; out[3] = p.S;
+    out[4] = p.tiles_i; out[5] = p.tile_i; out[6] = jerk ? 256 : p.tile_j; out[7] = jerk ? ((p.WJ <= 2) ? 4 : 3) : p.stages;
+    return NB_OK;
+}
+
+int64_t nb_debug_plans_computed(void) { return g_plans_computed.load(std::memory_order_relaxed); }
 
 const char* nb_status_string(int status) {
     switch (status) {

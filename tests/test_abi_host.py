@@ -13,9 +13,12 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def declared_functions():
-    text = open(os.path.join(ROOT, "include", "nbody_b200.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(nb_[a-z0-9_]+)\s*\(", text)))
+    names = set()
+    for header in ("nbody_b200.h", "nb_debug.h"):
+        text = open(os.path.join(ROOT, "include", header)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names |= set(re.findall(r"\b(nb_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_library_exports_every_declared_symbol():
@@ -133,3 +136,56 @@ def test_planner_fills_the_machine_for_the_bench_config():
     assert ctas >= 148 and p["K"] == 8
     waves = ctas / 148.0
     assert waves / -(-ctas // 148) > 0.9                                       # < 10 % wave-quantisation loss
+
+
+def test_fast_planner_is_the_exhaustive_search_and_costs_microseconds():
+    """csrc/nb_plan.h: make_plan visits only the S where the cost's minimum can lie; its choice is DEFINED by the
+    exhaustive search over every (K, WJ, S) (nb_debug_plan_exhaustive) and must equal it -- and an unseen shape must cost
+    the host a few microseconds, not the 60-220 us of the exhaustive search (a small block step lasts ~20 us)."""
+    import time
+    import numpy as np
+    rng = np.random.default_rng(5)
+    sizes = [1, 2, 7, 31, 32, 33, 100, 255, 256, 257, 512, 1000, 2048, 4096, 5000, 16384, 20480, 65536, 131072, 1048576, 20000000]
+    shapes = [(a, b) for a in sizes for b in sizes]
+    shapes += [(int(np.exp(rng.uniform(0, 16.5))) + 1, int(np.exp(rng.uniform(0, 16.5))) + 1) for _ in range(600)]
+    for jerk in (False, True):
+        query = nb.plan_query_jerk if jerk else nb.plan_query
+        for n_i, n_j in shapes:
+            assert query(n_i, n_j, 148) == nb.debug_plan_exhaustive(n_i, n_j, 148, jerk=jerk), (n_i, n_j, jerk)
+    lib = nb.lib()
+    out = (ctypes.c_int64 * 8)()
+    t0 = time.perf_counter()
+    for n_i, n_j in shapes:                                   # every shape differs: nothing a cache could serve
+        lib.nb_plan_query(n_i, n_j, 148, out)
+    per_call = (time.perf_counter() - t0) / len(shapes)
+    t0 = time.perf_counter()
+    for n_i, n_j in shapes:
+        lib.nb_plan_query_small(n_i, n_j, 148, out)
+    per_small = (time.perf_counter() - t0) / len(shapes)
+    assert per_call < 8e-6 and per_small < 10e-6, (per_call, per_small)     # ~3-5 us + ~0.5 us of ctypes
+
+
+def test_small_planner_invariants():
+    for n_i, n_j in [(1, 1), (1, 777), (16, 16384), (512, 65536), (2048, 2048), (2048, 65536), (100, 10 ** 6), (3, 5)]:
+        p = nb.plan_query_small(n_i, n_j, 148)
+        assert (p["KI"], p["LJ"]) in ((2, 1), (1, 1), (1, 2), (1, 4)) and p["WJ"] in (1, 2, 4, 8, 16) and p["NW"] in (8, 16) and p["WJ"] <= p["NW"]
+        assert p["tile_i"] == (p["NW"] // p["WJ"]) * p["KI"] * (32 // p["LJ"])
+        assert p["tiles_i"] * p["tile_i"] >= n_i > (p["tiles_i"] - 1) * p["tile_i"]
+        assert p["CS"] in (1, 8) and p["S"] % p["CS"] == 0 and p["tile_i"] % p["CS"] == 0 and 1 <= p["S"] <= 2048
+        assert p == nb.plan_query_small(n_i, n_j, 148)
+
+
+def test_debug_switches_parse_and_reject():
+    assert nb.lib().nb_debug_set(b"NB_PLAN", b"8,8,1,3") == 0
+    assert nb.lib().nb_debug_set(b"NB_PLAN", b"8,8,2,3") == 1           # WI * WJ != 8
+    assert nb.lib().nb_debug_set(b"NB_PLAN", None) == 0
+    assert nb.lib().nb_debug_set(b"NB_SMALL_PLAN", b"8,1,2,8,8,8") == 0
+    assert nb.lib().nb_debug_set(b"NB_SMALL_PLAN", b"8,2,2,8,8,8") == 1   # LJ > 1 needs KI = 1
+    assert nb.lib().nb_debug_set(b"NB_SMALL_PLAN", b"8,1,4,8,8,8") == 0   # tile 8, cluster 8
+    assert nb.lib().nb_debug_set(b"NB_SMALL_PLAN", b"16,2,1,2,144,8") == 0
+    assert nb.lib().nb_debug_set(b"NB_SMALL_PLAN", b"") == 0
+    assert nb.lib().nb_debug_set(b"NB_MASK", b"nonsense") == 1
+    assert nb.lib().nb_debug_set(b"NB_NO_SUCH_SWITCH", b"1") == 1
+    assert nb.lib().nb_debug_set(None, b"1") == 1
+    for key in (b"NB_MASK", b"NB_SMALL", b"NB_FUSED_REDUCE", b"NB_DIRECT", b"NB_STEP_GRAPH", b"NB_BATCH_TILE"):
+        assert nb.lib().nb_debug_set(key, None) == 0

@@ -45,9 +45,9 @@ def check(acc, pot, ra, rp, label=""):
 
 
 @pytest.mark.parametrize("tile", ["64", "128", "256", ""])
-def test_tree_lists_every_tile_shape(nb, tile, monkeypatch):
+def test_tree_lists_every_tile_shape(nb, tile, nbdebug):
     if tile:
-        monkeypatch.setenv("NB_BATCH_TILE", tile)
+        nbdebug.setenv("NB_BATCH_TILE", tile)
     w = wl.tree_list_workload(6000, 20, 300, 900, 2500, 1.0 / 128, seed=5)
     acc, pot = gpu_batched(nb, w)
     ra, rp = oracle.force_batched(w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j, w.eps2)

@@ -149,3 +149,25 @@ def test_adaptive_block_step_run_with_all_three_calls(nb):
     assert np.abs(p1 - p0).max() < 1e-6
     print(f"adaptive block run: {steps} block steps, {evaluated} particle evaluations of {steps * n}, "
           f"levels {sorted(levels_seen)}, dE/E = {abs(e1 - e0) / abs(e0):.2e}")
+
+
+@pytest.mark.parametrize("n", [4, 5000, 70001])
+def test_non_finite_due_times_are_never_selected(nb, n):
+    """include/nbody_b200.h: "Non-finite due times are never selected (all non-finite: t_next = +inf, n_act = 0)" --
+    parked particles (dt = +inf), NaN and -inf clocks, inf - inf; bit-exact against the oracle's definition."""
+    inf, nan = float("inf"), float("nan")
+    t, dt = clocks(n, seed=7 + n)
+    rng = np.random.default_rng(n)
+    for value, count in ((inf, n // 3), (nan, max(1, n // 50)), (-inf, max(1, n // 70))):
+        who = rng.choice(n, count, replace=False)
+        (dt if value == inf else t)[who] = value
+    t[0], dt[0] = inf, -inf                                             # inf + (-inf) = NaN
+    t_next, active = gpu_schedule(nb, t, dt)
+    rt, ra = oracle.block_schedule(t, dt)
+    assert np.isfinite(rt) and t_next == rt and np.array_equal(active, ra) and active.size > 0
+    due = t[active] + dt[active]
+    assert np.all(np.isfinite(due)) and np.all(due == rt)
+    # nobody has a finite due time: t_next = +inf, nobody due
+    for tt, dd in ((np.zeros(n), np.full(n, inf)), (np.full(n, nan), np.ones(n)), (np.full(n, -inf), np.ones(n))):
+        t_next, active = gpu_schedule(nb, tt, dd)
+        assert t_next == inf and active.size == 0

@@ -78,3 +78,30 @@ def test_degenerate_inputs_follow_ieee(nb):
     want = oracle.block_step_size(a, j, a1, j, h, 0.01)
     assert np.isnan(got[0]) and np.isnan(want[0]) and np.isposinf(got[1]) and np.isposinf(want[1])
     assert nb.last_launch_count() == 1
+
+
+@pytest.mark.parametrize("n,seed,lev0", [(5000, 4, 3), (5000, 4, 9), (65536, 5, 6)])
+def test_against_the_plain_fp64_definition(nb, n, seed, lev0):
+    """The kernel against oracle.block_step_size_f64 -- the Aarseth formula in plain FP64 (include/nbody_b200.h) -- by
+    tolerance, beside the bit-exact test against the FP32 definition: so the CUDA path is not held only against a
+    mirror of its own arithmetic.  Inputs: a Plummer sphere, (a0, j0) at the start, (a1, j1) at each particle's Hermite-
+    predicted state after its own h (all four from the oracle, rounded to FP32).  Tolerance: the formula has ~25
+    FP32 roundings (2^-24 each) and one cancellation, a0 - a1, which is exact on FP32 inputs of equal exponent
+    (|da| / |a| >= 1e-4 here, asserted); 1e-5 relative leaves a factor 10 over the 1e-6 measured with the FP32 oracle
+    on the CPU."""
+    w = wl.plummer_workload(n, 1.0 / 64, seed=50 + seed, with_velocities=True)
+    x, v, m = w.x_j.astype(np.float64), w.v.astype(np.float64), w.m_j
+    h = (2.0 ** -(float(lev0) + wl.block_levels(n, seed))).astype(np.float32)
+    a0, j0, _ = oracle.force_jerk(w.x_j, w.v, w.x_j, w.v, m, w.eps2)
+    hh = h.astype(np.float64)[:, None]
+    x1 = (x + v * hh + 0.5 * a0 * hh ** 2 + j0 * hh ** 3 / 6.0).astype(np.float32)
+    v1 = (v + a0 * hh + 0.5 * j0 * hh ** 2).astype(np.float32)
+    a1, j1, _ = oracle.force_jerk(x1, v1, w.x_j, w.v, m, w.eps2)
+    args = [z.astype(np.float32) for z in (a0, j0, a1, j1)]
+    da = np.linalg.norm(args[0].astype(np.float64) - args[2], axis=1) / np.linalg.norm(args[0], axis=1)
+    assert da.min() >= 1e-4                                             # well conditioned: the stated premise
+    got = gpu(nb, *args, h, 0.02).astype(np.float64)
+    want = oracle.block_step_size_f64(*args, h, np.float32(0.02))
+    rel = np.abs(got / want - 1.0)
+    assert rel.max() <= 1e-5, (rel.max(), int(rel.argmax()))
+    assert np.sqrt(np.mean(rel * rel)) <= 1e-6

@@ -48,9 +48,9 @@ def eps2_mix(n, seed):
 @pytest.mark.parametrize("mode", ["exact", "list"])
 @pytest.mark.parametrize("plan", [(8, 8, 1, 3), (8, 4, 2, 1), (4, 2, 4, 5), (2, 1, 8, 2), (4, 8, 1, 1), (2, 4, 2, 7),
                                   (8, 1, 8, 2), (8, 2, 4, 1)], ids=lambda p: "K%d_WI%d_WJ%d_S%d" % p)
-def test_every_decomposition_matches_oracle(nb, plan, mode, monkeypatch):
-    monkeypatch.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
-    monkeypatch.setenv("NB_MASK", mode)
+def test_every_decomposition_matches_oracle(nb, plan, mode, nbdebug):
+    nbdebug.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
+    nbdebug.setenv("NB_MASK", mode)
     w = wl.plummer_workload(3000, 1.0 / 64, seed=31)
     e2 = eps2_mix(3000, 1)
     acc, pot = gpu(nb, w.x_j, e2, w.x_j, w.m_j, alias=True)
@@ -58,9 +58,9 @@ def test_every_decomposition_matches_oracle(nb, plan, mode, monkeypatch):
     check(acc, pot, ra, rp, str(plan) + mode)
 
 
-def test_constant_array_equals_nb_force_bitwise_in_masked_mode(nb, monkeypatch):
+def test_constant_array_equals_nb_force_bitwise_in_masked_mode(nb, nbdebug):
     import torch
-    monkeypatch.setenv("NB_MASK", "exact")
+    nbdebug.setenv("NB_MASK", "exact")
     w = wl.subset_workload(5000, 700, 1.0 / 128, seed=9)
     acc, pot = gpu(nb, w.x_i, np.full(700, w.eps2, np.float32), w.x_j, w.m_j)
     a0, p0 = nb.force(dev(w.x_i), dev(w.x_j), dev(w.m_j), w.eps2)

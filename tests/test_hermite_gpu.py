@@ -78,9 +78,9 @@ PLANS = [(k, 8 // wj, wj, s) for k in (2, 4) for wj in (1, 2, 4, 8) for s in (1,
 
 @pytest.mark.parametrize("mode", ["exact", "list", "bloom"])
 @pytest.mark.parametrize("plan", PLANS, ids=lambda p: "K%d_WI%d_WJ%d_S%d" % p)
-def test_every_decomposition_matches_oracle(nb, plan, mode, monkeypatch):
-    monkeypatch.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
-    monkeypatch.setenv("NB_MASK", mode)
+def test_every_decomposition_matches_oracle(nb, plan, mode, nbdebug):
+    nbdebug.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
+    nbdebug.setenv("NB_MASK", mode)
     w = wl.subset_workload(3001, 777, 1.0 / 128, seed=21)
     rng = np.random.default_rng(5)
     vj = rng.normal(size=(3001, 3)).astype(np.float32)
@@ -90,25 +90,25 @@ def test_every_decomposition_matches_oracle(nb, plan, mode, monkeypatch):
     check(acc, jerk, pot, ra, rj, rp, str(plan) + mode)
 
 
-def test_list_mode_agrees_bitwise_with_masked_kernel(nb, monkeypatch):
+def test_list_mode_agrees_bitwise_with_masked_kernel(nb, nbdebug):
     x, v, m, eps2 = plummer_xv(3000, 1.0 / 64, 12)
     x = x.copy(); v = v.copy()
     x[2999] = x[5]; x[1500] = x[5]                 # duplicates in other segments, with their own velocities
     x[700] = (0.0, 0.0, 0.0); x[2100] = (-0.0, 1e-41, 0.0)
     out = {}
     for mode in ("exact", "list", "bloom"):
-        monkeypatch.setenv("NB_MASK", mode)
+        nbdebug.setenv("NB_MASK", mode)
         out[mode] = gpu_fj(nb, x, v, x, v, m, eps2, alias=True)
     for a, b, c in zip(out["exact"], out["list"], out["bloom"]):
         assert np.array_equal(a, b) and np.array_equal(a, c)
-    monkeypatch.setenv("NB_PLAN", "4,8,1,2")       # K = 4: without the potential the 26-instruction loop runs; same a and jerk
-    monkeypatch.setenv("NB_MASK", "exact")
+    nbdebug.setenv("NB_PLAN", "4,8,1,2")       # K = 4: without the potential the 26-instruction loop runs; same a and jerk
+    nbdebug.setenv("NB_MASK", "exact")
     ref = gpu_fj(nb, x, v, x, v, m, eps2, alias=True)
     for mode in ("list", "bloom"):
-        monkeypatch.setenv("NB_MASK", mode)
+        nbdebug.setenv("NB_MASK", mode)
         a, j, p = gpu_fj(nb, x, v, x, v, m, eps2, alias=True, want_pot=False)
         assert p is None and np.array_equal(a, ref[0]) and np.array_equal(j, ref[1])
-    monkeypatch.delenv("NB_PLAN")
+    nbdebug.delenv("NB_PLAN")
     ra, rj, rp = oracle.force_jerk(x, v, x, v, m, eps2)
     keep = np.ones(3000, bool); keep[[700, 2100]] = False       # the oracle does not flush 1e-41
     check(out["list"][0][keep], out["list"][1][keep], out["list"][2][keep], ra[keep], rj[keep], rp[keep], "list")
@@ -205,14 +205,14 @@ def test_force_jerk_host_matches_device_path(nb):
 
 
 @pytest.mark.parametrize("plan", [(4, 8, 1, 5), (4, 2, 4, 3), (2, 1, 8, 7), (2, 4, 2, 2)], ids=lambda p: "K%d_WI%d_WJ%d_S%d" % p)
-def test_fused_second_pass_is_bitwise_the_separate_reduce(nb, plan, monkeypatch):
+def test_fused_second_pass_is_bitwise_the_separate_reduce(nb, plan, nbdebug):
     """nb_force_jerk: the last CTA of an i-tile sums the S chunk partials in the order nb_hermite_reduce_kernel does;
     same bits, one launch fewer, ticket counters back at zero after every call."""
-    monkeypatch.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
+    nbdebug.setenv("NB_PLAN", "%d,%d,%d,%d" % plan)
     x, v, m, eps2 = plummer_xv(4000, 1.0 / 64, 19)
     out = {}
     for fused in ("1", "0"):
-        monkeypatch.setenv("NB_FUSED_REDUCE", fused)
+        nbdebug.setenv("NB_FUSED_REDUCE", fused)
         runs = [gpu_fj(nb, x, v, x, v, m, eps2, alias=True) for _ in range(3)]
         for r in runs[1:]:
             assert all(np.array_equal(a, b) for a, b in zip(r, runs[0]))

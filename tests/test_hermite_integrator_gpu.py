@@ -79,7 +79,7 @@ def test_invalid_arguments(nb):
 
 
 @pytest.mark.parametrize("n", [1500, 9000])
-def test_step_graph_replay_is_bitwise_the_eager_sequence(nb, n, monkeypatch):
+def test_step_graph_replay_is_bitwise_the_eager_sequence(nb, n, nbdebug):
     """Small systems replay their identical middle steps (predict, force + jerk without phi, correct) from a CUDA
     graph: same launches, same bits as the eager sequence (n = 9000: the Bloom-filter kernel inside the graph)."""
     import torch
@@ -87,7 +87,7 @@ def test_step_graph_replay_is_bitwise_the_eager_sequence(nb, n, monkeypatch):
     out = {}
     side = torch.cuda.Stream()                     # the default stream cannot be captured: graphs need a real stream
     for mode in ("1", "0"):
-        monkeypatch.setenv("NB_STEP_GRAPH", mode)
+        nbdebug.setenv("NB_STEP_GRAPH", mode)
         x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
         torch.cuda.synchronize()
         with torch.cuda.stream(side):

@@ -113,14 +113,14 @@ def test_c4_energy_drift_full_size(nb):
     assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and e["pot_rms"] <= 1e-5
 
 
-def test_step_graph_replay_is_bitwise_the_eager_sequence(nb, monkeypatch):
+def test_step_graph_replay_is_bitwise_the_eager_sequence(nb, nbdebug):
     """Small systems replay their identical middle steps from a CUDA graph: same launches, same bits as eager."""
     import torch
     w = wl.plummer_workload(1500, 1.0 / 64, seed=8, with_velocities=True)
     out = {}
     side = torch.cuda.Stream()                     # the default stream cannot be captured: graphs need a real stream
     for mode in ("1", "0"):
-        monkeypatch.setenv("NB_STEP_GRAPH", mode)
+        nbdebug.setenv("NB_STEP_GRAPH", mode)
         x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
         torch.cuda.synchronize()
         with torch.cuda.stream(side):

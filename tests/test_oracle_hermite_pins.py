@@ -428,3 +428,62 @@ def test_h10_scaling_laws():
     np.testing.assert_allclose(d4, 2 * d1, rtol=1e-6)
     ds = oracle.block_step_size(a0 / 4, j0 / 8, a1 / 4, j1 / 8, 2 * h, 0.01)        # s = 2: powers of two, exact
     np.testing.assert_array_equal(ds, 2 * d1)
+
+
+# ----------------------------------------------------------------------------- h10 (FP64): the plain definition
+def test_h10_f64_cubic_circular_scaling_and_agreement_with_the_fp32_definition():
+    """oracle.block_step_size_f64 is the Aarseth formula in plain FP64.  Same pins as the FP32 definition, tighter:
+    a cubic a(t) is interpolated exactly (1e-13), the circular orbit gives sqrt(eta)/omega with an O((omega h)^2)
+    error that falls 4x per halving, dt scales with sqrt(eta) and with a rescaling of time -- and the two definitions
+    agree to FP32 rounding on FP32 inputs (they are the same formula, so a dropped term in either shows here)."""
+    rng = np.random.default_rng(10)
+    c = rng.integers(-4, 5, size=(4, 50, 3)).astype(np.float64)
+    c[3][c[3] == 0] = 1.0
+    t0, h = 0.7, 0.3                                   # nothing dyadic: FP64 carries it anyway
+    acc = lambda t: c[0] + c[1] * t + c[2] * t ** 2 + c[3] * t ** 3
+    jerk = lambda t: c[1] + 2 * c[2] * t + 3 * c[3] * t ** 2
+    a2 = 2 * c[2] + 6 * c[3] * (t0 + h)
+    a3 = 6 * c[3]
+    nrm = lambda z: np.sqrt((z * z).sum(1))
+    eta = 0.02
+    want = np.sqrt(eta * (nrm(acc(t0 + h)) * nrm(a2) + nrm(jerk(t0 + h)) ** 2) / (nrm(jerk(t0 + h)) * nrm(a3) + nrm(a2) ** 2))
+    got = oracle.block_step_size_f64(acc(t0), jerk(t0), acc(t0 + h), jerk(t0 + h), np.full(50, h), eta)
+    assert got.dtype == np.float64
+    np.testing.assert_allclose(got, want, rtol=1e-11)
+    # circular orbit
+    errs = []
+    for hh in (0.25, 0.125, 0.0625):
+        w_, R = 1.5, 2.0
+        def state(t):
+            cs, sn = np.cos(w_ * t), np.sin(w_ * t)
+            return -R * w_ ** 2 * np.array([[cs, sn, 0.0]]), -R * w_ ** 3 * np.array([[-sn, cs, 0.0]])
+        a0, j0 = state(0.3)
+        a1, j1 = state(0.3 + hh)
+        errs.append(abs(float(oracle.block_step_size_f64(a0, j0, a1, j1, np.array([hh]), 0.01)[0]) * w_ / 0.1 - 1.0))
+    assert errs[2] < 1.5e-3 and 3.5 < errs[0] / errs[1] < 4.5 and 3.5 < errs[1] / errs[2] < 4.5
+    # scaling laws
+    a0, j0 = rng.normal(size=(30, 3)), rng.normal(size=(30, 3))
+    a1, j1 = a0 + 0.1 * rng.normal(size=(30, 3)), j0 + 0.1 * rng.normal(size=(30, 3))
+    hs = np.full(30, 0.125)
+    d1 = oracle.block_step_size_f64(a0, j0, a1, j1, hs, 0.01)
+    np.testing.assert_allclose(oracle.block_step_size_f64(a0, j0, a1, j1, hs, 0.04), 2 * d1, rtol=1e-14)
+    np.testing.assert_allclose(oracle.block_step_size_f64(a0 / 9, j0 / 27, a1 / 9, j1 / 27, 3 * hs, 0.01), 3 * d1, rtol=1e-12)
+    # the FP32 definition on the same (FP32) inputs: same formula, FP32 rounding apart
+    f = [z.astype(np.float32) for z in (a0, j0, a1, j1)]
+    d32 = oracle.block_step_size(*f, hs.astype(np.float32), 0.01)
+    d64 = oracle.block_step_size_f64(*f, hs.astype(np.float32), np.float32(0.01))
+    np.testing.assert_allclose(d32, d64, rtol=2e-5)
+
+
+def test_h9_non_finite_due_times_take_no_part():
+    """Reading R20 / include/nbody_b200.h: a due time that is not finite is never the minimum and never due -- dt = +inf
+    parks a particle, a NaN or -inf clock cannot stall or hijack the schedule.  Hand-worked cases."""
+    inf, nan = float("inf"), float("nan")
+    t_next, act = oracle.block_schedule([0.0, 0.0, 0.0, 0.0], [0.5, inf, 0.25, 0.25])
+    assert t_next == 0.25 and act.tolist() == [2, 3]
+    t_next, act = oracle.block_schedule([0.0, -inf, nan, 1.0], [0.5, 0.25, 0.25, -0.5])
+    assert t_next == 0.5 and act.tolist() == [0, 3]
+    t_next, act = oracle.block_schedule([0.0, 1.0], [inf, inf])
+    assert t_next == inf and act.size == 0
+    t_next, act = oracle.block_schedule([nan, -inf, inf], [1.0, 1.0, -inf])     # inf + (-inf) = NaN
+    assert t_next == inf and act.size == 0

@@ -63,13 +63,13 @@ def test_packed_entry_and_world1_sharded_force_on_gpu():
         e = oracle.error_metrics(a.cpu().numpy(), ra, p.cpu().numpy(), rp)
         assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and e["pot_rms"] <= 1e-5, e
     # packed entry = same kernels on the same records: bitwise equal to nb_force when both mask every pair
-    os.environ["NB_MASK"] = "exact"
+    nb.debug_set("NB_MASK", "exact")
     try:
         b0, q0 = nb.force(x, x, m, w.eps2)
         b1, q1 = nb.force_packed(x, xm, w.eps2)
         torch.cuda.synchronize()
     finally:
-        del os.environ["NB_MASK"]
+        nb.debug_set("NB_MASK", None)
     assert torch.equal(b0, b1) and torch.equal(q0, q1)
     # zero-mass padding records add only zeros (the j-chunks move, so the FP32 summation order may differ)
     pad = torch.zeros((37, 4), device="cuda")
