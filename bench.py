@@ -165,6 +165,9 @@ def reference_arm(args, wl):
     elif args.op == "cunbody":
         w = wl.config(1)
         name = "row f3 (G1): configs[1]'s particles, Fig. A.3 pipeline (oracle force on a sample)"
+    elif args.op == "cunbody4":
+        w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
+        name = "row f3 (G2): H1's particles, Fig. A.4 pipeline (oracle force_jerk on a sample)"
     elif args.op == "lj":
         w = LJ_ROWS(wl)
         name = "row f3 (L1): Lennard-Jones fluid, 131072 particles (oracle lennard_jones on a sample)"
@@ -223,7 +226,9 @@ OPS = {
     #  loop without it, so the algorithmic count for the roofline is 12 per interaction here)
     # row f3: the paper's cunbody_api call for its Fig. A.3 pipeline through the generalised kernel (scalar FP32;
     # the listing has no potential: 12 FP32-pipe instructions per interaction)
-    "cunbody": {"inst": 12, "kernel": "pipeline_kernel<PipelineForceA3> (generalised kernel, row f3)", "flops": (20, 38)},
+    "cunbody": {"inst": 12, "kernel": "pipeline_kernel2<PipelineForceA3> (generalised kernel, packed path, row f3)", "flops": (20, 38)},
+    # Fig. A.4 through the generalised kernel: the listing's 27 FP32-pipe instructions per pair (28 in the packed form's SASS)
+    "cunbody4": {"inst": 27, "kernel": "pipeline_kernel2<PipelineForceJerkPotA4> (generalised kernel, packed path, row f3)", "flops": (60, 60)},
     "leapfrog": {"inst": 12, "kernel": "nb_force_kernel<PHI=false> inside nb_leapfrog_kdk (row a8)", "flops": (20, 38)},
 }
 # row f3, a central force other than gravity (reading R19): 24 FP32-pipe instructions per pair in the SASS of
@@ -278,6 +283,15 @@ class Problem:
             p_xj = np.concatenate([w.x_j, w.m_j[:, None]], axis=1).astype(np.float32)
             self.host = [np.ascontiguousarray(p_xj), np.ascontiguousarray(p_xi)]
             self.n_out = w.n_j
+        elif op == "cunbody4":
+            w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
+            self.w, self.pairs = w, float(w.n_j) ** 2
+            self.name = (f"row f3 (G2): H1's particles as the paper's rows p_xi[n][6] = (x, v), p_xj[n][7] = (x, v, m) (Fig. A.2), "
+                         f"n={w.n_j}, eps2 = 1/256^2 (the listing's constant); one nb_cunbody_force_jerk_pot call (Fig. A.4 pipeline)")
+            p_xi = np.concatenate([w.x_j, w.v], axis=1).astype(np.float32)
+            p_xj = np.concatenate([w.x_j, w.v, w.m_j[:, None]], axis=1).astype(np.float32)
+            self.host = [np.ascontiguousarray(p_xj), np.ascontiguousarray(p_xi)]
+            self.n_out = w.n_j
         elif op == "lj":
             rows = LJ_ROWS(wl)
             self.w, self.pairs = rows, float(rows.shape[0]) ** 2
@@ -328,12 +342,12 @@ class Problem:
         self.dev = [torch.from_numpy(a).cuda() for a in self.host]
         self.pinned = [torch.from_numpy(a).pin_memory() for a in self.host]
         n = self.n_out
-        self.outs = [torch.empty((n, 4 if op == "lj" else 3), dtype=torch.float32, device="cuda")]
+        self.outs = [torch.empty((n, 4 if op == "lj" else (7 if op == "cunbody4" else 3)), dtype=torch.float32, device="cuda")]
         if op == "block":
             self.outs = [self.dev[k] for k in (0, 1, 3, 4)]            # the state itself is the result: x, v, a, j
         if op in ("jerk", "hermite"):
             self.outs.append(torch.empty((n, 3), dtype=torch.float32, device="cuda"))
-        if op not in ("cunbody", "lj", "block"):
+        if op not in ("cunbody", "cunbody4", "lj", "block"):
             self.outs.append(torch.empty((n,), dtype=torch.float32, device="cuda"))
         self.h_outs = [torch.empty(o.shape, dtype=torch.float32).pin_memory() for o in self.outs]
         self.h2d = int(sum(a.nbytes for a in self.host))
@@ -348,6 +362,8 @@ class Problem:
             nb.force(xi, xj, mj, w.eps2, acc_out=self.outs[0], pot_out=self.outs[1])
         elif self.op == "cunbody":
             nb.cunbody_force(t[0], t[1], self.outs[0])
+        elif self.op == "cunbody4":
+            nb.cunbody_force_jerk_pot(t[0], t[1], self.outs[0])
         elif self.op == "lj":
             nb.cunbody_lennard_jones(t[0], t[1], self.outs[0])
         elif self.op == "leapfrog":
@@ -401,6 +417,8 @@ class Problem:
             return "nb_force_jerk_host (pinned host buffers)"
         if self.op == "cunbody":
             return "pinned host rows -> cudaMemcpyAsync -> nb_cunbody_force -> cudaMemcpyAsync -> pinned host"
+        if self.op == "cunbody4":
+            return "pinned host rows -> cudaMemcpyAsync -> nb_cunbody_force_jerk_pot -> cudaMemcpyAsync -> pinned host"
         if self.op == "lj":
             return "pinned host rows -> cudaMemcpyAsync -> nb_cunbody_lennard_jones -> cudaMemcpyAsync -> pinned host"
         if self.op == "block":
@@ -415,8 +433,9 @@ class Problem:
     def plan(self, sm_count):
         if self.op == "force":
             return self.nb.plan_query(self.w.n_i, self.w.n_j, sm_count)
-        if self.op in ("cunbody", "lj"):
-            return {"cta": "256 threads x 2 or 4 i-records, 128-record j tiles, j-range split over S CTAs + second pass"}
+        if self.op in ("cunbody", "cunbody4", "lj"):
+            return {"cta": "256 threads x 8 or 4 i-records as packed pairs, double-buffered 128-record j tiles, Bloom test per tile, "
+                           "j-range split over S CTAs in whole waves + second pass"}
         if self.op == "hermite":
             return self.nb.plan_query_jerk(self.w.n_j, self.w.n_j, sm_count)
         if self.op == "leapfrog":
@@ -433,7 +452,7 @@ def oracle_rate_op(op, w, target_seconds, rng_seed=0):
     import oracle
     if op in ("force", "leapfrog", "cunbody"):
         return oracle_rate(w, target_seconds, rng_seed)
-    if op in ("hermite", "block"):
+    if op in ("hermite", "block", "cunbody4"):
         op = "jerk"
     cores = oracle.num_threads()
     rng = np.random.default_rng(rng_seed)

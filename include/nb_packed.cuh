@@ -1,4 +1,4 @@
-// nb_packed.cuh -- inline device helpers shared by the kernels: packed FP32 (f32x2) arithmetic, mbarrier / TMA bulk copy,
+// nb_packed.cuh -- inline device helpers shared by the kernels and by user pipelines (nb_pipeline.cuh): packed FP32 (f32x2) arithmetic, mbarrier / TMA bulk copy,
 // and the coincident-pair conventions (reading R1).  Inline functions only: safe in several translation units.
 #pragma once
 #include <cuda_runtime.h>
@@ -20,6 +20,11 @@ __device__ __forceinline__ void unpack2(u64 v, float& lo, float& hi) {
 __device__ __forceinline__ u64 add2(u64 a, u64 b) {
     u64 d;
     asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) {
+    u64 d;
+    asm("sub.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
     return d;
 }
 __device__ __forceinline__ u64 mul2(u64 a, u64 b) {
@@ -95,6 +100,30 @@ __device__ __forceinline__ uint32_t coin_hash(uint32_t a, uint32_t b, uint32_t c
     h ^= h >> 32;
     h *= 0xD6E8FEB86659FD93ull;
     return (uint32_t)(h >> 32);
+}
+
+// ---------------------------------------------------------------- Bloom filter of a warp's i-positions (block-level coincidence test)
+// MODE_BLOOM: 2^16 filter bits (8 KB) per group of warps that hold the same i-particles, two bits per position.
+// The key is computed on the coordinates as the loop sees them (x + 0 under add.ftz: -0 and subnormals become +0),
+// so two positions the masked loop calls coincident always have the same key: no false negatives.
+constexpr int kBloomWords = 2048;
+__device__ __forceinline__ uint32_t bloom_key(float x, float y, float z) {
+    float cx, cy, cz;
+    asm("add.ftz.f32 %0, %1, 0f00000000;" : "=f"(cx) : "f"(x));
+    asm("add.ftz.f32 %0, %1, 0f00000000;" : "=f"(cy) : "f"(y));
+    asm("add.ftz.f32 %0, %1, 0f00000000;" : "=f"(cz) : "f"(z));
+    uint32_t h = __float_as_uint(cx) * 0x9E3779B1u;
+    h = __float_as_uint(cy) * 0x85EBCA77u + h;
+    h = __float_as_uint(cz) * 0xC2B2AE3Du + (h ^ (h >> 15));
+    h ^= h >> 16;
+    return h * 0x2C1B3C6Du;
+}
+__device__ __forceinline__ void bloom_set(uint32_t* filt, uint32_t h) {
+    atomicOr(filt + (h >> 21), 1u << ((h >> 16) & 31u));
+    atomicOr(filt + ((h >> 5) & 2047u), 1u << (h & 31u));
+}
+__device__ __forceinline__ bool bloom_test(const uint32_t* filt, uint32_t h) {
+    return ((filt[h >> 21] >> ((h >> 16) & 31u)) & (filt[(h >> 5) & 2047u] >> (h & 31u)) & 1u) != 0u;
 }
 
 }  // namespace nb

@@ -127,6 +127,20 @@ int nb_leapfrog_kdk(int64_t n, float *x, float *v, const float *m,
                     void *stream);
 
 /*
+ * nb_kick_drift / nb_kick -- the O(n) updates of the KDK leapfrog on their own (the kernels nb_leapfrog_kdk runs between its
+ * force evaluations), for drivers that own only a SLICE of the particles: the i-sharded multi-GPU integration of
+ * DESIGN.md section 8 calls them on each rank's slice around the all-gather + nb_force_packed of every step.
+ *
+ *     nb_kick_drift:  v += acc * h  (n_kicks = 1)  or  v += acc * h; v += acc * h  (n_kicks = 2: the closing half-kick of one
+ *                     step and the opening half-kick of the next, two separately rounded FMAs);  then  x += v * dt
+ *     nb_kick:        v += acc * h
+ *
+ *   x, v  device, float [n][3], updated in place      acc  device, const, float [n][3]      h, dt finite
+ */
+int nb_kick_drift(int64_t n, float *x, float *v, const float *acc, float h, int n_kicks, float dt, void *stream);
+int nb_kick(int64_t n, float *v, const float *acc, float h, void *stream);
+
+/*
  * nb_force_jerk -- force + jerk + potential for the 4th-order Hermite scheme: the paper's second
  * pipeline description (Fig. A.2, Fig. A.4; used by the authors'
  * Hermite code):
@@ -244,6 +258,20 @@ int nb_force_batched(int64_t n_batch, const int32_t *i_offsets, const int32_t *j
                      float eps2,
                      float *acc_out, float *pot_out,
                      void *stream);
+
+/*
+ * nb_force_batched_packed -- nb_force_batched for a caller that keeps the interaction-list records on the device as packed
+ * 16-byte (x, y, z, m) rows (the batched analogue of nb_force_packed; the paper's own layout, Fig. A.1):
+ * no pack pass -- on tree lists that pass moves 32 B per list entry per call, 5-6 % of a call -- and a host caller ships
+ * 16 B per entry once instead of re-sending (x, y, z) and m.  xm_j: device, const, float [n_j_total][4], 16-byte aligned.
+ * Same results as nb_force_batched on the same records, bit for bit; everything else as there.
+ */
+int nb_force_batched_packed(int64_t n_batch, const int32_t *i_offsets, const int32_t *j_offsets,
+                            int64_t n_i_total, const float *x_i,
+                            int64_t n_j_total, const float *xm_j,
+                            float eps2,
+                            float *acc_out, float *pot_out,
+                            void *stream);
 
 /*
  * nb_hermite4 -- n_steps steps of the 4th-order Hermite scheme with a shared, constant time step, all state on the

@@ -43,6 +43,10 @@ def lib() -> ctypes.CDLL:
         l.nb_force_host.restype = ci
         l.nb_leapfrog_kdk.argtypes = [i64, p, p, p, f32, f32, i64, p, p, p]
         l.nb_leapfrog_kdk.restype = ci
+        l.nb_kick_drift.argtypes = [i64, p, p, p, f32, ci, f32, p]
+        l.nb_kick_drift.restype = ci
+        l.nb_kick.argtypes = [i64, p, p, f32, p]
+        l.nb_kick.restype = ci
         l.nb_force_jerk.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p, p]
         l.nb_force_jerk.restype = ci
         for fn in (l.nb_cunbody_force, l.nb_cunbody_force_jerk_pot, l.nb_cunbody_lennard_jones):
@@ -56,6 +60,8 @@ def lib() -> ctypes.CDLL:
         l.nb_force_eps_i.restype = ci
         l.nb_force_batched.argtypes = [i64, p, p, i64, p, i64, p, p, f32, p, p, p]
         l.nb_force_batched.restype = ci
+        l.nb_force_batched_packed.argtypes = [i64, p, p, i64, p, i64, p, f32, p, p, p]
+        l.nb_force_batched_packed.restype = ci
         l.nb_force_jerk_host.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p]
         l.nb_force_jerk_host.restype = ci
         l.nb_plan_query_jerk.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
@@ -262,6 +268,29 @@ def force_batched(i_offsets, j_offsets, x_i, x_j, m_j, eps2: float, acc_out=None
     return acc_out, pot_out
 
 
+def force_batched_packed(i_offsets, j_offsets, x_i, xm_j, eps2: float, acc_out=None, pot_out=None, want_pot: bool = True,
+                         stream=None):
+    """nb_force_batched_packed on CUDA tensors: the list records as packed (x, y, z, m) rows [n_j_total, 4]."""
+    import torch
+    _dev_f32(x_i, "x_i", (3,)); _dev_f32(xm_j, "xm_j", (4,))
+    for t, name in ((i_offsets, "i_offsets"), (j_offsets, "j_offsets")):
+        if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.int32 or not t.is_contiguous() or t.dim() != 1:
+            raise TypeError(f"{name} must be a contiguous 1-D int32 CUDA tensor")
+    if i_offsets.shape[0] != j_offsets.shape[0] or i_offsets.shape[0] < 1:
+        raise ValueError("i_offsets and j_offsets must both have n_batch + 1 entries")
+    n_batch, n_i, n_j = i_offsets.shape[0] - 1, x_i.shape[0], xm_j.shape[0]
+    if acc_out is None:
+        acc_out = torch.zeros((n_i, 3), dtype=torch.float32, device=x_i.device)
+    if pot_out is None and want_pot:
+        pot_out = torch.zeros((n_i,), dtype=torch.float32, device=x_i.device)
+    with torch.cuda.device(x_i.device):
+        st = lib().nb_force_batched_packed(n_batch, i_offsets.data_ptr(), j_offsets.data_ptr(), n_i, x_i.data_ptr(), n_j,
+                                           xm_j.data_ptr(), float(eps2), acc_out.data_ptr(),
+                                           None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_force_batched_packed")
+    return acc_out, pot_out
+
+
 def force_jerk_host(x_i, v_i, x_j, v_j, m_j, eps2: float, acc_out=None, jerk_out=None, pot_out=None, want_pot: bool = True):
     """nb_force_jerk_host on numpy float32 arrays (or pinned CPU tensors' numpy views).  Blocking."""
     import numpy as np
@@ -414,6 +443,24 @@ def block_step_size(a0, j0, a1, j1, h, eta: float, dt_out=None, stream=None):
                                       dt_out.data_ptr(), _stream_ptr(stream))
     _check(st, "nb_block_step_size")
     return dt_out
+
+
+def kick_drift(x, v, acc, h: float, n_kicks: int, dt: float, stream=None) -> None:
+    """nb_kick_drift on CUDA tensors [n, 3]: v += acc h (once or twice), x += v dt; in place."""
+    import torch
+    _dev_f32(x, "x", (3,)); _dev_f32(v, "v", (3,)); _dev_f32(acc, "acc", (3,))
+    with torch.cuda.device(x.device):
+        st = lib().nb_kick_drift(x.shape[0], x.data_ptr(), v.data_ptr(), acc.data_ptr(), float(h), int(n_kicks), float(dt), _stream_ptr(stream))
+    _check(st, "nb_kick_drift")
+
+
+def kick(v, acc, h: float, stream=None) -> None:
+    """nb_kick on CUDA tensors [n, 3]: v += acc h; in place."""
+    import torch
+    _dev_f32(v, "v", (3,)); _dev_f32(acc, "acc", (3,))
+    with torch.cuda.device(v.device):
+        st = lib().nb_kick(v.shape[0], v.data_ptr(), acc.data_ptr(), float(h), _stream_ptr(stream))
+    _check(st, "nb_kick")
 
 
 def plan_query(n_i: int, n_j: int, sm_count: int = 148) -> dict:

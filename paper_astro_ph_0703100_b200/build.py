@@ -10,7 +10,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnbody_b200.so")
 SOURCES = ["nbody_b200.cu", "nb_small_launch.cu"]
-DEPS = ["nbody_b200.cu", "nb_small_launch.cu", "nb_small_launch.h", "nb_small.cuh", "nb_packed.cuh", os.path.join(ROOT, "include", "nb_debug.h"), "nb_kernels.cuh", "nb_hermite.cuh", "nb_batched.cuh", "nb_pipelines.cuh", os.path.join(ROOT, "include", "nb_pipeline.cuh"), "nb_plan.h", os.path.join(ROOT, "include", "nbody_b200.h")]
+DEPS = ["nbody_b200.cu", "nb_small_launch.cu", "nb_small_launch.h", "nb_small.cuh", os.path.join(ROOT, "include", "nb_packed.cuh"), os.path.join(ROOT, "include", "nb_debug.h"), "nb_kernels.cuh", "nb_hermite.cuh", "nb_batched.cuh", "nb_pipelines.cuh", os.path.join(ROOT, "include", "nb_pipeline.cuh"), "nb_plan.h", os.path.join(ROOT, "include", "nbody_b200.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -54,5 +54,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_microloops() -> str:
+    """The stand-alone micro-benchmarks behind the roofline peak (csrc/nb_microloops.cu) -> nb_microloops (in-tree)."""
+    out = os.path.join(HERE, "nb_microloops")
+    nvcc = os.environ.get("NVCC", "nvcc")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-o", out,
+                    os.path.join(CSRC, "nb_microloops.cu")], check=True)
+    return out
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--microloops" in sys.argv:
+        print(build_microloops())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

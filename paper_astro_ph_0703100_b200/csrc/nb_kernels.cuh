@@ -24,7 +24,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "nb_packed.cuh"
+#include "../../include/nb_packed.cuh"
 
 namespace nb {
 
@@ -219,29 +219,6 @@ struct ForceArgs {
 enum { MODE_EXACT = 0,     // masked loop everywhere (eps2 == 0 or tiny; per-i softening on small calls)
        MODE_BLOOM = 1,     // per-warp Bloom filter of the i-positions in shared memory, every 256-j block tested (mid-size calls)
        MODE_LIST = 2 };    // coincidence lists from the pre-pass, no test in the hot loop (large calls; a-only calls)
-
-// MODE_BLOOM: 2^16 filter bits (8 KB) per group of warps that hold the same i-particles, two bits per position.
-// The key is computed on the coordinates as the loop sees them (x + 0 under add.ftz: -0 and subnormals become +0),
-// so two positions the masked loop calls coincident always have the same key: no false negatives.
-constexpr int kBloomWords = 2048;
-__device__ __forceinline__ uint32_t bloom_key(float x, float y, float z) {
-    float cx, cy, cz;
-    asm("add.ftz.f32 %0, %1, 0f00000000;" : "=f"(cx) : "f"(x));
-    asm("add.ftz.f32 %0, %1, 0f00000000;" : "=f"(cy) : "f"(y));
-    asm("add.ftz.f32 %0, %1, 0f00000000;" : "=f"(cz) : "f"(z));
-    uint32_t h = __float_as_uint(cx) * 0x9E3779B1u;
-    h = __float_as_uint(cy) * 0x85EBCA77u + h;
-    h = __float_as_uint(cz) * 0xC2B2AE3Du + (h ^ (h >> 15));
-    h ^= h >> 16;
-    return h * 0x2C1B3C6Du;
-}
-__device__ __forceinline__ void bloom_set(uint32_t* filt, uint32_t h) {
-    atomicOr(filt + (h >> 21), 1u << ((h >> 16) & 31u));
-    atomicOr(filt + ((h >> 5) & 2047u), 1u << (h & 31u));
-}
-__device__ __forceinline__ bool bloom_test(const uint32_t* filt, uint32_t h) {
-    return ((filt[h >> 21] >> ((h >> 16) & 31u)) & (filt[(h >> 5) & 2047u] >> (h & 31u)) & 1u) != 0u;
-}
 
 // ---------------------------------------------------------------- a2..a7: the force kernel
 // CTA = 8 warps = WI (along i) x WJ (along j).  A CTA owns 32*K*WI i-particles (K per thread, in

@@ -31,6 +31,39 @@ struct PipelineForceA3 {
         OUTPUT[1] += mr3i * dy;
         OUTPUT[2] += mr3i * dz;
     }
+    // The same statements for two i-records at once (nb_pipeline.cuh, packed path): I2[c] = (rec0[c], rec1[c]).
+    static constexpr bool kPacked = true, kCoincidentRule = true;
+    static __device__ __forceinline__ void prep_i(float* rec) {        // positions are held as -x, zeros canonicalised (reading R1)
+        rec[0] = neg_canon(rec[0]); rec[1] = neg_canon(rec[1]); rec[2] = neg_canon(rec[2]);
+    }
+    template <bool MASKED>
+    static __device__ __forceinline__ void pair2(const u64* I2, const float* INPUT_J, u64* OUT2) {
+        const float xj = INPUT_J[0], yj = INPUT_J[1], zj = INPUT_J[2], mj = INPUT_J[3];
+        const u64 dx = add2(pack2(xj, xj), I2[0]), dy = add2(pack2(yj, yj), I2[1]), dz = add2(pack2(zj, zj), I2[2]);
+        u64 r2 = fma2(dx, dx, I2[3]);                                                      // PAPER.md:461-464 (any order: reading R6)
+        r2 = fma2(dy, dy, r2);
+        r2 = fma2(dz, dz, r2);
+        float ra, rb;
+        unpack2(r2, ra, rb);
+        if (MASKED) {
+            float a0, a1, b0, b1, c0, c1;
+            unpack2(dx, a0, a1); unpack2(dy, b0, b1); unpack2(dz, c0, c1);
+            const uint32_t ta = __float_as_uint(a0) | __float_as_uint(b0) | __float_as_uint(c0);
+            const uint32_t tb = __float_as_uint(a1) | __float_as_uint(b1) | __float_as_uint(c1);
+            ra = (ta == 0u) ? __int_as_float(0x7f800000) : ra;         // rsqrt(+inf) = +0: the pair adds 0
+            rb = (tb == 0u) ? __int_as_float(0x7f800000) : rb;
+        }
+        const u64 r1i = pack2(pipeline_rsqrt(ra), pipeline_rsqrt(rb));
+        const u64 r2i = mul2(r1i, r1i);
+        const u64 mr1i = mul2(pack2(mj, mj), r1i);
+        const u64 mr3i = mul2(mr1i, r2i);
+        OUT2[0] = fma2(mr3i, dx, OUT2[0]);
+        OUT2[1] = fma2(mr3i, dy, OUT2[1]);
+        OUT2[2] = fma2(mr3i, dz, OUT2[2]);
+    }
+    static __device__ __forceinline__ void finish(const double* sum, float* OUTPUT) {
+        OUTPUT[0] = (float)sum[0]; OUTPUT[1] = (float)sum[1]; OUTPUT[2] = (float)sum[2];
+    }
 };
 
 // Fig. A.2 / A.4: IDIM 6 = (x, v), JDIM 7 = (x, v, m), FDIM 7 = (a, jerk, pot);
@@ -56,6 +89,54 @@ struct PipelineForceJerkPotA4 {
         OUTPUT[5] += mf * dv_2 - mf3a * dx_2;
         OUTPUT[6] -= pot;
     }
+    // Packed form: the listing's statements for two i-records at once; d = x_j - x_i and dv = v_j - v_i are formed through
+    // -x_i (canonicalised, reading R1) and -v_i; pot is summed with its sign applied at the end.
+    static constexpr bool kPacked = true, kCoincidentRule = true;
+    static __device__ __forceinline__ void prep_i(float* rec) {        // -x canonicalised, -v
+        rec[0] = neg_canon(rec[0]); rec[1] = neg_canon(rec[1]); rec[2] = neg_canon(rec[2]);
+        rec[3] = -rec[3]; rec[4] = -rec[4]; rec[5] = -rec[5];
+    }
+    template <bool MASKED>
+    static __device__ __forceinline__ void pair2(const u64* I2, const float* INPUT_J, u64* OUT2) {
+        const float e2 = 1.0f / (256.0f * 256.0f);
+        const u64 dx0 = add2(pack2(INPUT_J[0], INPUT_J[0]), I2[0]), dx1 = add2(pack2(INPUT_J[1], INPUT_J[1]), I2[1]),
+                  dx2 = add2(pack2(INPUT_J[2], INPUT_J[2]), I2[2]);
+        u64 r2 = fma2(dx0, dx0, pack2(e2, e2));
+        r2 = fma2(dx1, dx1, r2);
+        r2 = fma2(dx2, dx2, r2);
+        float ra, rb;
+        unpack2(r2, ra, rb);
+        if (MASKED) {
+            float a0, a1, b0, b1, c0, c1;
+            unpack2(dx0, a0, a1); unpack2(dx1, b0, b1); unpack2(dx2, c0, c1);
+            const uint32_t ta = __float_as_uint(a0) | __float_as_uint(b0) | __float_as_uint(c0);
+            const uint32_t tb = __float_as_uint(a1) | __float_as_uint(b1) | __float_as_uint(c1);
+            ra = (ta == 0u) ? __int_as_float(0x7f800000) : ra;         // r1i = +0: the pair adds 0
+            rb = (tb == 0u) ? __int_as_float(0x7f800000) : rb;
+        }
+        const u64 r1i = pack2(pipeline_rsqrt(ra), pipeline_rsqrt(rb));
+        const u64 r2i = mul2(r1i, r1i);
+        const u64 pot = mul2(pack2(INPUT_J[6], INPUT_J[6]), r1i);                           // pot = mj r1i
+        const u64 mf = mul2(pot, r2i);                                                      // mf = mj r3i
+        const u64 dv0 = add2(pack2(INPUT_J[3], INPUT_J[3]), I2[3]), dv1 = add2(pack2(INPUT_J[4], INPUT_J[4]), I2[4]),
+                  dv2 = add2(pack2(INPUT_J[5], INPUT_J[5]), I2[5]);
+        u64 xv = mul2(dx0, dv0);
+        xv = fma2(dx1, dv1, xv);
+        xv = fma2(dx2, dv2, xv);
+        const u64 nmf3a = mul2(mul2(mf, r2i), mul2(xv, pack2(-3.0f, -3.0f)));               // -3 mr5i (dx.dv)
+        OUT2[0] = fma2(mf, dx0, OUT2[0]);
+        OUT2[1] = fma2(mf, dx1, OUT2[1]);
+        OUT2[2] = fma2(mf, dx2, OUT2[2]);
+        OUT2[3] = fma2(nmf3a, dx0, fma2(mf, dv0, OUT2[3]));
+        OUT2[4] = fma2(nmf3a, dx1, fma2(mf, dv1, OUT2[4]));
+        OUT2[5] = fma2(nmf3a, dx2, fma2(mf, dv2, OUT2[5]));
+        OUT2[6] = add2(OUT2[6], pot);                                                       // sign at the end
+    }
+    static __device__ __forceinline__ void finish(const double* sum, float* OUTPUT) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) OUTPUT[c] = (float)sum[c];
+        OUTPUT[6] = -(float)sum[6];
+    }
 };
 
 // A central force other than gravity (section 4.5: "van der Waals molecular interactions"; no formula in
@@ -76,6 +157,40 @@ struct PipelineLennardJones {
         OUTPUT[1] -= f * dy;
         OUTPUT[2] -= f * dz;
         OUTPUT[3] += 4.0f * es6 * (s6 - 1.0f);                         // 4 eps (s^12 - s^6)
+    }
+    // Packed form.  d = r_j - r_i is held through -r_i; the force on i is -f d: accumulate +f d and flip the sign at the end.
+    static constexpr bool kPacked = true, kCoincidentRule = true;
+    static __device__ __forceinline__ void prep_i(float* rec) {
+        rec[0] = neg_canon(rec[0]); rec[1] = neg_canon(rec[1]); rec[2] = neg_canon(rec[2]);
+    }
+    template <bool MASKED>
+    static __device__ __forceinline__ void pair2(const u64* I2, const float* INPUT_J, u64* OUT2) {
+        const u64 dx = add2(pack2(INPUT_J[0], INPUT_J[0]), I2[0]), dy = add2(pack2(INPUT_J[1], INPUT_J[1]), I2[1]),
+                  dz = add2(pack2(INPUT_J[2], INPUT_J[2]), I2[2]);
+        u64 r2 = mul2(dx, dx);
+        r2 = fma2(dy, dy, r2);
+        r2 = fma2(dz, dz, r2);
+        float ra, rb;
+        unpack2(r2, ra, rb);
+        if (MASKED) {                                                  // r2 == 0 (coincident, or closer than 1e-19): r1i = 0
+            ra = (ra == 0.0f) ? __int_as_float(0x7f800000) : ra;
+            rb = (rb == 0.0f) ? __int_as_float(0x7f800000) : rb;
+        }
+        const u64 r1i = pack2(pipeline_rsqrt(ra), pipeline_rsqrt(rb));
+        const u64 r2i = mul2(r1i, r1i);
+        const u64 sigma = add2(pack2(INPUT_J[3], INPUT_J[3]), I2[3]);                       // Lorentz-Berthelot
+        const u64 eps = mul2(pack2(INPUT_J[4], INPUT_J[4]), I2[4]);
+        const u64 s2 = mul2(mul2(sigma, sigma), r2i);
+        const u64 s6 = mul2(mul2(s2, s2), s2);
+        const u64 es6 = mul2(eps, s6);
+        const u64 f = mul2(mul2(es6, pack2(24.0f, 24.0f)), mul2(fma2(s6, pack2(2.0f, 2.0f), pack2(-1.0f, -1.0f)), r2i));
+        OUT2[0] = fma2(f, dx, OUT2[0]);
+        OUT2[1] = fma2(f, dy, OUT2[1]);
+        OUT2[2] = fma2(f, dz, OUT2[2]);
+        OUT2[3] = fma2(mul2(es6, pack2(4.0f, 4.0f)), add2(s6, pack2(-1.0f, -1.0f)), OUT2[3]);
+    }
+    static __device__ __forceinline__ void finish(const double* sum, float* OUTPUT) {
+        OUTPUT[0] = -(float)sum[0]; OUTPUT[1] = -(float)sum[1]; OUTPUT[2] = -(float)sum[2]; OUTPUT[3] = (float)sum[3];
     }
 };
 

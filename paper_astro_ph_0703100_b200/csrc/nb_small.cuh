@@ -28,7 +28,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "nb_packed.cuh"
+#include "../../include/nb_packed.cuh"
 
 namespace nb {
 

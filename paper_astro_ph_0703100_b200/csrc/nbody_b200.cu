@@ -681,16 +681,21 @@ int launch_batched(const nb::ForceArgs& args, int groups, unsigned max_ctas, cud
 
 extern "C" {
 
-int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j_offsets, int64_t n_i_total,
-                     const float* x_i, int64_t n_j_total, const float* x_j, const float* m_j, float eps2,
-                     float* acc_out, float* pot_out, void* stream_) {
+}  // extern "C"
+
+namespace {
+// packed_j != nullptr: the caller holds the list records as 16-byte (x, y, z, m) rows already (nb_force_batched_packed)
+int force_batched_impl(int64_t n_batch, const int32_t* i_offsets, const int32_t* j_offsets, int64_t n_i_total,
+                       const float* x_i, int64_t n_j_total, const float* x_j, const float* m_j, const float4* packed_j,
+                       float eps2, float* acc_out, float* pot_out, void* stream_) {
     t_launches = 0;
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
     if (bad_count(n_batch) || bad_count(n_i_total) || bad_count(n_j_total)) return NB_ERR_INVALID_VALUE;
     if (!(eps2 >= 0.0f) || !std::isfinite(eps2)) return NB_ERR_INVALID_VALUE;
     if (n_batch > 0 && (!i_offsets || !j_offsets)) return NB_ERR_INVALID_VALUE;
     if (n_i_total > 0 && (!x_i || !acc_out)) return NB_ERR_INVALID_VALUE;
-    if (n_j_total > 0 && (!x_j || !m_j)) return NB_ERR_INVALID_VALUE;
+    if (n_j_total > 0 && !packed_j && (!x_j || !m_j)) return NB_ERR_INVALID_VALUE;
+    if (packed_j && (reinterpret_cast<uintptr_t>(packed_j) & 15u)) return NB_ERR_INVALID_VALUE;
     int dev = 0;
     DeviceInfo info;
     int rc = device_info(&dev, &info);
@@ -698,8 +703,10 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     if (n_batch == 0 || n_i_total == 0) return NB_OK;
     WsGuard guard(dev, stream);
     Workspace* ws = guard.ws;
-    rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)(n_j_total > 0 ? n_j_total : 1) * sizeof(float4), stream);
-    if (rc != NB_OK) return rc;
+    if (!packed_j) {
+        rc = ensure(&ws->jp, &ws->jp_bytes, (size_t)(n_j_total > 0 ? n_j_total : 1) * sizeof(float4), stream);
+        if (rc != NB_OK) return rc;
+    }
     const int groups = batched_groups(n_i_total, n_batch);
     const int tile = 64 * groups;
     // sum_b ceil(n_i(b) / tile) <= n_i_total / tile + n_batch
@@ -707,7 +714,7 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     if (max_ctas > (int64_t)INT32_MAX) return NB_ERR_INVALID_VALUE;
     rc = ensure(&ws->tiles, &ws->tiles_bytes, (size_t)(n_batch + 1 + max_ctas) * sizeof(int), stream);
     if (rc != NB_OK) return rc;
-    if (n_j_total > 0) {
+    if (n_j_total > 0 && !packed_j) {
         nb::nb_pack_j_kernel<<<(unsigned)((n_j_total + 255) / 256), 256, 0, stream>>>(x_j, m_j, (int)n_j_total,
                                                                                       reinterpret_cast<float4*>(ws->jp));
         NB_CUDA(cudaGetLastError());
@@ -722,7 +729,7 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     nb::ForceArgs args;
     args.x_i = x_i;
     args.eps2_i = nullptr;
-    args.jp = reinterpret_cast<const float4*>(ws->jp);
+    args.jp = packed_j ? packed_j : reinterpret_cast<const float4*>(ws->jp);
     args.xj_raw = args.mj_raw = nullptr;
     args.acc = acc_out;
     args.pot = pot_out;
@@ -743,6 +750,24 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
     const bool a_only = !pot_out && eps2 >= kUnmaskedMinEps2 && knobs().mask < 0;
     return a_only ? launch_batched<false>(args, groups, (unsigned)max_ctas, stream)
                   : launch_batched<true>(args, groups, (unsigned)max_ctas, stream);
+}
+}  // namespace
+
+extern "C" {
+
+int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j_offsets, int64_t n_i_total,
+                     const float* x_i, int64_t n_j_total, const float* x_j, const float* m_j, float eps2,
+                     float* acc_out, float* pot_out, void* stream) {
+    return force_batched_impl(n_batch, i_offsets, j_offsets, n_i_total, x_i, n_j_total, x_j, m_j, nullptr, eps2, acc_out, pot_out, stream);
+}
+
+int nb_force_batched_packed(int64_t n_batch, const int32_t* i_offsets, const int32_t* j_offsets, int64_t n_i_total,
+                            const float* x_i, int64_t n_j_total, const float* xm_j, float eps2,
+                            float* acc_out, float* pot_out, void* stream) {
+    if (n_j_total > 0 && !xm_j) return NB_ERR_INVALID_VALUE;
+    static const float4 dummy = {0.f, 0.f, 0.f, 0.f};
+    return force_batched_impl(n_batch, i_offsets, j_offsets, n_i_total, x_i, n_j_total, nullptr, nullptr,
+                              xm_j ? reinterpret_cast<const float4*>(xm_j) : &dummy, eps2, acc_out, pot_out, stream);
 }
 
 int nb_force_jerk(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j, const float* x_j, const float* v_j,
@@ -1017,6 +1042,42 @@ int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, f
         NB_CUDA(cudaGetLastError());
         ++t_launches;
     }
+    return NB_OK;
+}
+
+int nb_kick_drift(int64_t n, float* x, float* v, const float* acc, float h, int n_kicks, float dt, void* stream_) {
+    t_launches = 0;
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (bad_count(n) || 3 * n > (int64_t)INT32_MAX || (n_kicks != 1 && n_kicks != 2)) return NB_ERR_INVALID_VALUE;
+    if (!std::isfinite(h) || !std::isfinite(dt)) return NB_ERR_INVALID_VALUE;
+    if (n > 0 && (!x || !v || !acc)) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n == 0) return NB_OK;
+    const int n3 = (int)(3 * n), threads = 256, blocks = (n3 + threads - 1) / threads;
+    if (n_kicks == 2) nb::nb_kick_drift_kernel<true><<<blocks, threads, 0, stream>>>(x, v, acc, n3, h, dt);
+    else nb::nb_kick_drift_kernel<false><<<blocks, threads, 0, stream>>>(x, v, acc, n3, h, dt);
+    NB_CUDA(cudaGetLastError());
+    t_launches = 1;
+    return NB_OK;
+}
+
+int nb_kick(int64_t n, float* v, const float* acc, float h, void* stream_) {
+    t_launches = 0;
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (bad_count(n) || 3 * n > (int64_t)INT32_MAX || !std::isfinite(h)) return NB_ERR_INVALID_VALUE;
+    if (n > 0 && (!v || !acc)) return NB_ERR_INVALID_VALUE;
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n == 0) return NB_OK;
+    const int n3 = (int)(3 * n), threads = 256, blocks = (n3 + threads - 1) / threads;
+    nb::nb_kick_kernel<<<blocks, threads, 0, stream>>>(v, acc, n3, h);
+    NB_CUDA(cudaGetLastError());
+    t_launches = 1;
     return NB_OK;
 }
 

@@ -166,3 +166,25 @@ def test_own_members_scattered_through_the_lists_eps0(nb):
     assert np.array_equal(a1, a2)
     ra, rp = oracle.force_batched(w1.i_offsets, w1.j_offsets, w1.x_i, w1.x_j, w1.m_j, w1.eps2)
     check(a1, p1, ra, rp, "scattered-eps")
+
+
+def test_packed_entry_is_bitwise_the_unpacked_call(nb):
+    """nb_force_batched_packed on (x, y, z, m) rows: no pack pass, one launch fewer, the same bits -- with and without phi;
+    argument validation as for the unpacked call."""
+    import torch
+    w = wl.tree_list_workload(5000, 30, 200, 700, 2000, 1.0 / 128, seed=6)
+    io, jo, xi, xj, mj = (dev(a) for a in (w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j))
+    xm = torch.cat([xj, mj[:, None]], dim=1).contiguous()
+    for want_pot in (True, False):
+        a0, p0 = nb.force_batched(io, jo, xi, xj, mj, w.eps2, want_pot=want_pot)
+        l0 = nb.last_launch_count()
+        a1, p1 = nb.force_batched_packed(io, jo, xi, xm, w.eps2, want_pot=want_pot)
+        l1 = nb.last_launch_count()
+        torch.cuda.synchronize()
+        assert l1 == l0 - 1
+        assert torch.equal(a0, a1) and (p0 is None or torch.equal(p0, p1))
+    ra, rp = oracle.force_batched(w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j, w.eps2)
+    check(a1.cpu().numpy(), None, ra, None, "packed")
+    lib = nb.lib()
+    assert lib.nb_force_batched_packed(1, io.data_ptr(), jo.data_ptr(), 5, xi.data_ptr(), 5, None, 0.1, a1.data_ptr(), None, None) == 1
+    assert lib.nb_force_batched_packed(1, io.data_ptr(), jo.data_ptr(), 5, xi.data_ptr(), 5, xm.data_ptr() + 4, 0.1, a1.data_ptr(), None, None) == 1

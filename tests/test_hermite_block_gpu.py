@@ -67,7 +67,8 @@ def test_one_block_step_matches_oracle(nb, n, n_act, seed):
     assert np.abs(gx - ox).max() < 2e-6 and np.abs(gv - ov).max() < 2e-6
     e = oracle.error_metrics(ga[active], oa[active])
     ej = oracle.error_metrics(gj[active], oj[active])
-    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-4
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4
+    assert ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-4               # DESIGN.md R16 (measured: 2.6e-6 / 3e-5 at worst)
 
 
 def test_empty_active_set_is_a_no_op(nb):
@@ -117,7 +118,8 @@ def test_three_level_schedule_matches_oracle_and_conserves_energy(nb, n, sub_ste
     assert np.abs(gx - xr).max() < 1e-5 and np.abs(gv - vr).max() < 1e-5
     e = oracle.error_metrics(ga, ar)
     ej = oracle.error_metrics(gj, jr)
-    assert e["acc_rms"] <= 1e-4 and ej["acc_rms"] <= 1e-3                           # values at the FP32 trajectory's state
+    # a, j sit at the FP32 trajectory's own state after up to 8 sub-steps; still inside DESIGN.md R16 (measured 2.5e-6 / 1.5e-5)
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-4
     _, _, e0 = oracle.energy(w.x_j, w.v, w.m_j, w.eps2)
     _, _, e1 = oracle.energy(gx, gv, w.m_j, w.eps2)
     assert abs(e1 - e0) / abs(e0) < 1e-5
@@ -151,7 +153,7 @@ def test_bench_size_block_steps_sampled_against_oracle(nb):
         assert np.abs(gx[sample] - ox[sample]).max() < 2e-6 and np.abs(gv[sample] - ov[sample]).max() < 2e-6
         e = oracle.error_metrics(ga[sample], oa[sample])
         ej = oracle.error_metrics(gj[sample], oj[sample])
-        assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-3, (s, e, ej)
+        assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-4, (s, e, ej)
 
 
 def test_order_of_the_active_list_does_not_matter_bitwise(nb):
@@ -192,7 +194,8 @@ def test_coincident_particles_and_zero_softening(nb):
     assert np.abs(gx - ox).max() < 2e-6 and np.abs(gv - ov).max() < 2e-6
     e = oracle.error_metrics(ga[active], oa[active])
     ej = oracle.error_metrics(gj[active], oj[active])
-    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-4
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4
+    assert ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-4               # DESIGN.md R16 (measured: 2.6e-6 / 3e-5 at worst)
 
 
 def test_runs_on_a_side_stream_and_in_a_cuda_graph(nb):
@@ -254,4 +257,4 @@ def test_randomised_block_steps(nb, case):
     assert np.abs(gx - ox).max() < 4e-6 and np.abs(gv - ov).max() < 4e-6
     e = oracle.error_metrics(ga[active], oa[active])
     ej = oracle.error_metrics(gj[active], oj[active])
-    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-4, (n, n_act, eps, e, ej)
+    assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-4, (n, n_act, eps, e, ej)

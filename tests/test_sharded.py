@@ -1,5 +1,6 @@
-"""Row f4: i-sharded force evaluation.  CPU: slice arithmetic and the world-size-2 gloo path (gather order, ragged
-padding with zero-mass records) with the oracle as the injected force; GPU: world size 1 through nb_force_packed."""
+"""Row f4: i-sharded force evaluation and leapfrog.  CPU: slice arithmetic and the world-size-2/3 gloo paths (gather order,
+ragged padding with zero-mass records, step sequence) with CPU stand-ins injected for the kernels; GPU: world size 2 on one
+device (records exchanged through host memory) and world size 1 through nb_force_packed."""
 import json
 import os
 import socket
@@ -32,19 +33,49 @@ def _free_port():
     return port
 
 
-@pytest.mark.parametrize("n,nproc", [(1001, 2), (600, 3)])
-def test_sharded_force_world_gloo_matches_unsharded_oracle(n, nproc):
+def _run_worker(nproc, *args, timeout=300):
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={nproc}",
            "--master-addr", "127.0.0.1", "--master-port", str(_free_port()),
-           os.path.join(ROOT, "tests", "_gloo_shard_worker.py"), str(n)]
-    r = subprocess.run(cmd, cwd=ROOT, env=dict(os.environ, OMP_NUM_THREADS="2"), capture_output=True, text=True, timeout=300)
+           os.path.join(ROOT, "tests", "_gloo_shard_worker.py"), *[str(a) for a in args]]
+    r = subprocess.run(cmd, cwd=ROOT, env=dict(os.environ, OMP_NUM_THREADS="2"), capture_output=True, text=True, timeout=timeout)
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
     assert len(lines) == 1, r.stdout
-    d = json.loads(lines[0])
+    return json.loads(lines[0])
+
+
+@pytest.mark.parametrize("n,nproc", [(1001, 2), (600, 3)])
+def test_sharded_force_world_gloo_matches_unsharded_oracle(n, nproc):
+    """Host logic at world size 2 and 3 on CPU ranks: the pack, the force (= the oracle) and nothing else injected."""
+    d = _run_worker(nproc, "force", "cpu", n)
     assert d["world"] == nproc and d["slices"][-1][1] == n
     # same double-precision sums, only the zero-mass padding records differ: exact agreement
     assert d["acc_max_abs_diff"] == 0.0 and d["pot_max_abs_diff"] == 0.0
+
+
+@pytest.mark.parametrize("n,nproc,steps", [(601, 2, 5), (300, 3, 4)])
+def test_sharded_leapfrog_world_gloo_matches_oracle_integrator(n, nproc, steps):
+    """every rank owns its slice of (x, v), one all-gather of the packed records per step.  CPU ranks
+    with float64 stand-ins for the kernels: the step sequence (fused double kick, phi only at the end, ragged slices) must
+    reproduce the oracle's textbook KDK on the whole system."""
+    d = _run_worker(nproc, "leapfrog", "cpu", n, steps)
+    assert d["world"] == nproc and d["slices"][-1][1] == n
+    # float64 stand-ins, float64 records: the same arithmetic as the oracle's integrator up to the order of a few additions
+    assert d["x_max_abs_diff"] <= 1e-12 and d["v_max_abs_diff"] <= 1e-12 and d["acc_rel"] <= 1e-12 and d["pot_rel"] <= 1e-12
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("mode,n,steps", [("force", 5001, 0), ("leapfrog", 3001, 6)])
+def test_sharded_world2_on_the_device(mode, n, steps):
+    """Two ranks, both on cuda:0 (one GPU on the box; NCCL refuses two ranks on one device, so the records travel through
+    host memory over gloo): nb_pack_j -> gather -> nb_force_packed (-> nb_kick_drift / nb_kick) on ragged slices with
+    zero-mass padding, against the oracle on the whole system."""
+    d = _run_worker(2, mode, "cuda", n, steps, timeout=600)
+    assert d["world"] == 2 and d["slices"] == [[0, (n + 1) // 2], [(n + 1) // 2, n]]
+    if mode == "force":
+        assert d["acc_rms"] <= 1e-5 and d["acc_max"] <= 1e-4 and d["pot_rms"] <= 1e-5, d
+    else:
+        assert d["x_max_abs_diff"] <= 1e-5 and d["v_max_abs_diff"] <= 1e-5 and d["acc_rel"] <= 1e-4 and d["pot_rel"] <= 1e-5, d
 
 
 @pytest.mark.gpu
