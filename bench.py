@@ -33,9 +33,25 @@ FP32_INST_PER_PAIR = 13          # FMA-pipe instructions per interaction (acc + 
 FP32_LANES_PER_SM_CLK = 128
 CONFIG_INDEX = {"C0": 0, "C1": 1, "C2": 2, "C3": 3, "C4": 4}
 L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/r01_ncu_full.md); null for configs / ops without a capture
-NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 71.0e6, "jerk": 105.4e6, "batched": 248.5e6, "block": 5.0e6}   # block: mean of 2 launches
+
+
+def modelled_traffic(args, prob, nb, sm_count):
+    """DRAM bytes one launch of the dominant kernel moves, MODELLED from the live plan (not pasted from an old capture):
+    first touch of the inputs it reads + its outputs + the j-split partials (written, then read by the second pass; they
+    fit L2, so this is an upper bound for them).  The ncu measurements it is checked against are in profiles/."""
+    if args.op != "force":
+        return None, "not modelled for this op (ncu captures: profiles/)"
+    w = prob.w
+    base = 16.0 * w.n_j + 12.0 * w.n_i + 16.0 * w.n_i              # packed j (or x_j + m_j), x_i, a + phi
+    sp = nb.plan_query_small(w.n_i, w.n_j, sm_count)
+    if sp["default"]:
+        groups = sp["S"] // sp["CS"]
+        partial = 2.0 * 32.0 * w.n_i * groups if groups > 1 else 0.0
+        return base + partial, f"modelled from the live plan (small-i-set kernel, {groups} partial group(s) of 32 B per i)"
+    p = nb.plan_query(w.n_i, w.n_j, sm_count)
+    partial = 2.0 * 32.0 * w.n_i * p["S"] if p["S"] > 1 else 0.0
+    return base + partial, (f"modelled from the live plan (S = {p['S']} j-chunks x n_i x 32 B of FP64 partials, written and read "
+                            "back; ncu on C1: 71 MB, profiles/r01_ncu_full.md)")
 
 
 def load_peaks():
@@ -432,7 +448,8 @@ class Problem:
 
     def plan(self, sm_count):
         if self.op == "force":
-            return self.nb.plan_query(self.w.n_i, self.w.n_j, sm_count)
+            sp = self.nb.plan_query_small(self.w.n_i, self.w.n_j, sm_count)
+            return dict(sp, kernel="nb_small_kernel") if sp["default"] else self.nb.plan_query(self.w.n_i, self.w.n_j, sm_count)
         if self.op in ("cunbody", "cunbody4", "lj"):
             return {"cta": "256 threads x 8 or 4 i-records as packed pairs, double-buffered 128-record j tiles, Bloom test per tile, "
                            "j-range split over S CTAs in whole waves + second pass"}
@@ -591,8 +608,11 @@ def main():
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
 
-    # small calls are launch-bound: also report the same call replayed from a CUDA graph (no L2 flush between replays)
+    # small calls are launch-bound: also report the same call replayed from a CUDA graph (no L2 flush between replays).
+    # GRAPH_CALLS calls are captured into ONE graph: a graph of a single 5-us kernel replayed in a Python loop measures the
+    # host's cudaGraphLaunch rate (~8 us per replay), not the device
     graph_ms = None
+    GRAPH_CALLS, GRAPH_REPLAYS = 50, 8
     if args.op == "force" and not args.shard and prob.pairs < 2.0 ** 30:
         gs = torch.cuda.Stream()
         with torch.cuda.stream(gs):
@@ -601,17 +621,17 @@ def main():
             gs.synchronize()
             g = torch.cuda.CUDAGraph()
             with torch.cuda.graph(g, stream=gs):
-                prob.call()
+                for _ in range(GRAPH_CALLS):
+                    prob.call()
             g.replay()
             gs.synchronize()
-            reps = 200
             g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             g0.record(gs)
-            for _ in range(reps):
+            for _ in range(GRAPH_REPLAYS):
                 g.replay()
             g1.record(gs)
             gs.synchronize()
-        graph_ms = g0.elapsed_time(g1) / reps
+        graph_ms = g0.elapsed_time(g1) / (GRAPH_CALLS * GRAPH_REPLAYS)
 
     # end to end with HOST buffers (pinned), copies inside the timed region
     e2e_steps = max(3, min(args.steps, 10))
@@ -641,13 +661,15 @@ def main():
         k_rate = pairs_k * n_k / (k_ms * 1e-3) if n_k else 0.0
         inst = op["inst"]
         achieved = inst * k_rate
-        traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(args.op) if args.op != "force" else (
-            None if args.n > 0 else NCU_DRAM_BYTES_PER_LAUNCH.get(args.config))
+        traffic, traffic_kind = modelled_traffic(args, prob, nb, sm_count)
         roofline = {
-            "bound": "alu", "kernel": op["kernel"],
+            "bound": "alu",
+            "kernel": ("nb_small_kernel (small-i-set kernel: pair interaction packed over j, rows a1-a7 in one launch)"
+                       if args.op == "force" and nb.plan_query_small(prob.w.n_i, prob.w.n_j, sm_count)["default"] else op["kernel"]),
             "achieved": achieved / 1e12, "peak": peak_inst / 1e12, "unit": "FP32-pipe Tinst/s",
             "frac": achieved / peak_inst, "traffic": traffic,
-            "traffic_unit": "DRAM bytes per launch (ncu --set full, profiles/)",
+            "traffic_unit": "DRAM bytes per launch of the dominant kernel",
+            "traffic_kind": traffic_kind,
             "kernel_ms": k_ms / max(1, n_k), "kernel_launches_timed": n_k,
             "kernel_interactions_per_s": k_rate, "roofline_interactions_per_s": peak_inst / inst,
             "peak_source": f"{sm_count} SMs x {FP32_LANES_PER_SM_CLK} FP32 lanes x sm_max_mhz {f_max / 1e6:.0f} MHz "
@@ -678,7 +700,9 @@ def main():
         }
         if graph_ms is not None:
             out["graph_replay"] = {"ms_per_call": graph_ms, "value": pairs / (graph_ms * 1e-3), "unit": METRIC,
-                                   "note": "one captured nb_force call replayed 200x back to back, L2 warm"}
+                                   "note": f"{GRAPH_CALLS} nb_force calls captured into one CUDA graph, replayed {GRAPH_REPLAYS}x back to "
+                                           "back, per call; L2 warm (device time per call: a one-call graph replayed from Python "
+                                           "measures the host's launch rate instead)"}
         if args.op == "block":
             out["block_steps_per_s"] = BLOCK_SUB_STEPS * args.steps / (total_ms * 1e-3)
             # the scheduler's share when the due sets are not precomputed: nb_block_schedule + the 4-byte read-back of n_act
@@ -695,6 +719,34 @@ def main():
             out["scheduler"] = {"us_per_call": 1e6 * (time.perf_counter() - t0) / reps, "n_due": n_due,
                                 "api": "nb_block_schedule (5 launches) + 4-byte read-back of n_act, host wall clock",
                                 "share_of_a_block_step": (time.perf_counter() - t0) / reps / (total_ms * 1e-3 / (BLOCK_SUB_STEPS * args.steps))}
+        if args.op == "block":
+            # An ADAPTIVE run never repeats a shape: n_act differs at every block step, so every call plans a new
+            # decomposition.  64 block steps with 64 distinct n_act on a copy of the state, timed on the HOST wall clock
+            # (enqueue + planning + device), with the planner's cache misses counted (nb_debug_plans_computed).
+            rng = np.random.default_rng(11)
+            order = rng.permutation(prob.w.n_j)
+            sizes = [int(v) for v in np.unique(rng.integers(8, 4096, 96))[:64]]
+            acts = [torch.from_numpy(np.sort(order[:k]).astype(np.int32)).cuda() for k in sizes]
+            st = [t.clone() for t in prob.dev[:6]]
+            t_now = float(st[5].max().item())
+            for a in acts[:4]:                                           # warm the workspace, not the plan cache (sizes differ)
+                t_now += 1e-9
+                nb.hermite4_block_step(st[0], st[1], st[2], st[3], st[4], st[5], a, t_now, prob.w.eps2)
+            torch.cuda.synchronize()
+            plans0 = nb.debug_plans_computed()
+            t0 = time.perf_counter()
+            for a in acts[4:]:
+                t_now += 1e-9
+                nb.hermite4_block_step(st[0], st[1], st[2], st[3], st[4], st[5], a, t_now, prob.w.eps2)
+            t_enq = time.perf_counter() - t0
+            torch.cuda.synchronize()
+            t_all = time.perf_counter() - t0
+            n_steps = len(acts) - 4
+            out["adaptive"] = {"block_steps": n_steps, "n_act_range": [sizes[4], sizes[-1]], "distinct_shapes": n_steps,
+                               "plans_computed": nb.debug_plans_computed() - plans0,
+                               "host_enqueue_us_per_step": 1e6 * t_enq / n_steps, "wall_us_per_step": 1e6 * t_all / n_steps,
+                               "block_steps_per_s": n_steps / t_all,
+                               "note": "every step a new (n_act, n): no plan-cache hit; host wall clock including the planner"}
         if args.op == "hermite":
             out["hermite_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
         if args.op in ("leapfrog", "hermite") and not args.no_cpu_baseline:

@@ -6,12 +6,18 @@
 //     over j (nb_small.cuh), with and without the exact coincidence mask, by warps per SM -- as a fraction of the
 //     13-instruction FP32 roofline (128 lanes / 13 instructions per clock per SM).
 // Build and run:  python -m paper_astro_ph_0703100_b200.build --microloops && ./paper_astro_ph_0703100_b200/nb_microloops
-// Output of the round-2 run: profiles/r02_microloops.md.
+//   * `nb_microloops --phases`: nb_small_kernel on a C2-shaped call (512 x 65536) with a time stamp after every phase
+//     (staging, loop, lane / warp sums, ticket, final sums), per CTA: where a small call spends its time.
+// Output of the round-2 runs: profiles/r02_microloops.md, profiles/r02_small_calls.md.
+#define NB_SMALL_STAMPS   // this program only: nb_small_kernel writes %globaltimer / clock64 stamps of its phases
 #include <cuda_runtime.h>
 #include <cstdio>
 #include <cstdlib>
 #include <cstdint>
 #include <vector>
+#include <algorithm>
+#include <random>
+#include <cstring>
 #include "../../include/nb_packed.cuh"
 #include "nb_small.cuh"
 using namespace nb;
@@ -105,6 +111,58 @@ __global__ void jpacked_kernel(const float4* jp2, int n_pairs, float* out, float
 
 static int g_sm = 148; static double g_hz = 1.965e9;
 
+// ---------------- phases of nb_small_kernel (--phases)
+template <int NW, int KI, int LJ, int WJ, int MODE, bool PHI>
+void phase_run(const char* name, int n_i, int n_j, int S, float* xi, float* xj, float* mj, float* acc, float* pot, double4* partial, int* tickets, long long* stamps) {
+    constexpr int TILE = (NW / WJ) * KI * (32 / LJ);
+    const int tiles = (n_i + TILE - 1) / TILE, Q = WJ * LJ;
+    const int chunk_max = (n_j + S - 1) / S + 2, round_max = chunk_max < kSmallRoundJ ? chunk_max : kSmallRoundJ;
+    size_t stage = (size_t)Q * small_pair_stride(small_slot_len(round_max, Q)) * 32, red = ((WJ > 1 ? (size_t)WJ * TILE : 0) + TILE) * 32;
+    size_t smem = ((stage > red ? stage : red) + 127) / 128 * 128;
+    SmallArgs a{}; a.x_i = xi; a.xj_raw = xj; a.mj_raw = mj; a.jp = nullptr; a.acc = acc; a.pot = PHI ? pot : nullptr; a.partial = partial; a.tickets = tickets;
+    a.n_i = n_i; a.n_j = n_j; a.S = S; a.eps2 = 1.f / 16384; a.stamps = nullptr;
+    smem += 128;
+    auto kern = nb_small_kernel<NW, KI, LJ, WJ, MODE, PHI, 1>;
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024));
+    const int n_ctas = tiles * S;
+    for (int r = 0; r < 5; ++r) kern<<<dim3(tiles, S), 32 * NW, smem>>>(a);
+    CK(cudaDeviceSynchronize());
+    cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    CK(cudaEventRecord(e0)); for (int r = 0; r < 20; ++r) kern<<<dim3(tiles, S), 32 * NW, smem>>>(a); CK(cudaEventRecord(e1)); CK(cudaEventSynchronize(e1));
+    float ms; CK(cudaEventElapsedTime(&ms, e0, e1));
+    a.stamps = stamps; CK(cudaMemset(stamps, 0, n_ctas * 16 * 8));
+    kern<<<dim3(tiles, S), 32 * NW, smem>>>(a); CK(cudaDeviceSynchronize());
+    std::vector<long long> h(n_ctas * 16); CK(cudaMemcpy(h.data(), stamps, h.size() * 8, cudaMemcpyDeviceToHost));
+    long long t0 = h[0]; for (int c = 0; c < n_ctas; ++c) t0 = std::min(t0, h[c * 16]);
+    printf("%s: grid %d x %d, %d threads, smem %zu: %.2f us per back-to-back launch\n", name, tiles, S, 32 * NW, smem, ms * 1e3 / 20);
+    const char* ph[7] = {"start", "staged", "loop done", "tile sums out", "ticket taken", "final sums done", "after sleep"};
+    for (int k = 0; k < 7; ++k) {
+        std::vector<double> g, c;
+        for (int q = 0; q < n_ctas; ++q) if (h[q * 16 + k]) { g.push_back((h[q * 16 + k] - t0) * 1e-3); c.push_back((h[q * 16 + 8 + k] - h[q * 16 + 8]) / 1.965e3); }
+        if (g.empty()) continue;
+        std::sort(g.begin(), g.end()); std::sort(c.begin(), c.end());
+        printf("   %-16s (%3zu CTAs)  since first CTA start [us]: min %.2f med %.2f max %.2f | since own start (clock64 at 1.965 GHz) [us]: min %.2f med %.2f max %.2f\n",
+               ph[k], g.size(), g.front(), g[g.size() / 2], g.back(), c.front(), c[c.size() / 2], c.back());
+    }
+}
+
+static int phases_main() {
+    const int n_i = 512, n_j = 65536;
+    std::mt19937 rng(1); std::normal_distribution<float> nd;
+    std::vector<float> hx(3 * n_j), hm(n_j, 1.f / n_j), hi(3 * n_i);
+    for (auto& v : hx) v = nd(rng);
+    for (int i = 0; i < n_i; ++i) for (int c = 0; c < 3; ++c) hi[3 * i + c] = hx[3 * (i * 97) + c];
+    float *xi, *xj, *mj, *acc, *pot; double4* partial; int* tickets; long long* stamps;
+    CK(cudaMalloc(&xi, hi.size() * 4)); CK(cudaMalloc(&xj, hx.size() * 4)); CK(cudaMalloc(&mj, hm.size() * 4)); CK(cudaMalloc(&acc, n_i * 12)); CK(cudaMalloc(&pot, n_i * 4));
+    CK(cudaMalloc(&partial, (size_t)512 * n_i * 32)); CK(cudaMalloc(&tickets, 4096)); CK(cudaMemset(tickets, 0, 4096)); CK(cudaMalloc(&stamps, 4096 * 16 * 8));
+    CK(cudaMemcpy(xi, hi.data(), hi.size() * 4, cudaMemcpyHostToDevice)); CK(cudaMemcpy(xj, hx.data(), hx.size() * 4, cudaMemcpyHostToDevice)); CK(cudaMemcpy(mj, hm.data(), hm.size() * 4, cudaMemcpyHostToDevice));
+    phase_run<16, 2, 1, 8, SMALL_EXACT, true>("NW16 KI2 WJ8 exact S37", n_i, n_j, 37, xi, xj, mj, acc, pot, partial, tickets, stamps);
+    phase_run<16, 2, 1, 16, SMALL_EXACT, true>("NW16 KI2 WJ16 exact S18", n_i, n_j, 18, xi, xj, mj, acc, pot, partial, tickets, stamps);
+    phase_run<16, 1, 1, 8, SMALL_EXACT, true>("NW16 KI1 WJ8 exact S18", n_i, n_j, 18, xi, xj, mj, acc, pot, partial, tickets, stamps);
+    phase_run<16, 2, 1, 16, SMALL_NONE, false>("NW16 KI2 WJ16 no mask, no phi S18", n_i, n_j, 18, xi, xj, mj, acc, pot, partial, tickets, stamps);
+        return 0;
+}
+
 template <class F> static double run(F f, int reps = 20) {
     cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     for (int r = 0; r < 3; ++r) f();
@@ -116,7 +174,8 @@ template <class F> static double run(F f, int reps = 20) {
     return ms / reps * 1e-3;
 }
 
-int main() {
+int main(int argc, char** argv) {
+    if (argc > 1 && !std::strcmp(argv[1], "--phases")) return phases_main();
     cudaDeviceProp prop; CK(cudaGetDeviceProperties(&prop, 0)); g_sm = prop.multiProcessorCount;
     int khz = 0; CK(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, 0)); g_hz = khz * 1e3;
     printf("# %s, %d SMs, clock attribute %.0f MHz (rates below are per SM per clock at that clock)\n", prop.name, g_sm, g_hz / 1e6);

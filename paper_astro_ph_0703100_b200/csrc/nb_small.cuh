@@ -351,8 +351,9 @@ __global__ void __launch_bounds__(32 * NW) nb_small_kernel(const SmallArgs a) {
         NB_STAMP(4);
         if (!s_last) return;
         // One thread per (i, half): half = (ax, ay) or (az, phi); the loads run ahead, the adds keep the order g = 0 .. n-1.
-        // (The tile's partials come through one SM's L2 port at ~0.1-0.15 us per group, measured: the planner keeps the
-        // number of groups small.)
+        // (One SM pulls the other CTAs' partials at only ~25-40 GB/s, whatever the number of loads in flight -- 1.5 us for
+        // 18 groups of a 64-particle tile, 3.9 us for 37 groups of 128, against 0.8-1.0 us when every load hits the SM's own
+        // row; waiting 3 us first changes nothing (measured with %globaltimer stamps).  The planner keeps groups x tile small.)
         for (int t = threadIdx.x; t < 2 * SLICE; t += kSmallThreads) {
             const int i = tile0 + (int)rank * SLICE + (t >> 1), half = t & 1;
             if (i >= a.n_i) continue;
