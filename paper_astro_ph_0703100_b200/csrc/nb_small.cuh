@@ -28,6 +28,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "../../include/nb_packed.cuh"
 
 namespace nb {
@@ -44,6 +46,7 @@ struct SmallArgs {
     int n_i;
     int n_j;
     int S;                 // j-chunks across CTAs (grid.y), a multiple of CS
+    int flag_offset;       // SMALL_FLAG: byte offset of the tile's Bloom filter + the slot bitmaps in dynamic shared memory
 #ifdef NB_SMALL_STAMPS
     long long* stamps;     // working builds only: [n_ctas][16] %globaltimer and clock64 stamps of the kernel's phases
 #endif
@@ -53,8 +56,8 @@ struct SmallArgs {
 constexpr int kSmallThreadsMax = 512;
 constexpr int kSmallRoundJ = 4096;     // j-particles staged in shared memory at a time (64 KB + padding)
 constexpr int kSmallLoadBatch = 4;     // j-pairs a thread loads before it stores them to shared memory
-constexpr int kSmallBlockPairs = 64;   // Eq. (2): FP32 partial sums run over at most 64 j-pairs = 128 j of a slot (also the
-                                       // granularity of the Bloom test: a block with a hit runs the masked loop)
+constexpr int kSmallBlockPairs = 64;   // Eq. (2): FP32 partial sums run over at most 64 j-pairs = 128 j of a slot (= one 64-bit
+                                       // word of the SMALL_FLAG bitmap of marked pairs)
 
 // ---------------------------------------------------------------- thread-block cluster helpers
 __device__ __forceinline__ uint32_t cluster_ctarank() {
@@ -125,19 +128,28 @@ __host__ __device__ inline int small_pair_stride(int slot_len) { return (slot_le
 // Coincident pairs (reading R1), MODE:
 //   SMALL_EXACT  every pair masked (LOP3 + FSEL per pair on the ALU pipe): the loop reaches 62-70 % of the FP32 roofline
 //                where the unmasked loop reaches 69-85 % (profiles/r02_microloops.md);
-//   SMALL_NONE   no mask: valid without phi for eps2 >= 2^-40 (an unmasked coincident pair adds m u^3 (+-0) to a).
+//   SMALL_NONE   no mask: valid without phi for eps2 >= 2^-40 (an unmasked coincident pair adds m u^3 (+-0) to a);
+//   SMALL_FLAG   (LJ = 1, eps2 >= 2^-40) the j-PAIRS that may hold a coincident particle are marked while they are staged:
+//                the CTA builds a Bloom filter of its tile's i-positions (nb_packed.cuh; no false negatives), every staged
+//                j is tested once, and a hit sets the pair's bit in a per-slot bitmap.  All lanes of a warp sweep the same
+//                pair, so the loop branches warp-uniformly: runs of unmarked pairs go through the unmasked body, a marked
+//                pair through the masked one.  Same pairs, same order, and the two bodies give the same bits for a pair
+//                that is not coincident: the result is the always-masked one bit for bit (a false positive only costs
+//                the mask), whatever the tile holds -- invariant under permutation of the i-set.
 // Two cheaper ways to honour the rule were built and measured on C2 and dropped: a per-warp Bloom
 // filter tested per Eq. (2) block (the CTA lasts as long as its slowest warp, and with one or two blocks per warp the
 // masked ones set the pace: 26.3 against 25.7 us), and a hash join of the staged j-particles against the CTA's i-tile
 // with the coincident ones swept separately (the probe made staging 4x slower, and a sum order that depends on which
 // particles share a tile is not invariant under permutation of the i-set).
-enum { SMALL_EXACT = 0, SMALL_NONE = 2 };
+enum { SMALL_EXACT = 0, SMALL_FLAG = 1, SMALL_NONE = 2 };
+__host__ __device__ inline int small_flag_words(int pstride) { return (pstride + 63) >> 6; }   // 64-bit words per slot bitmap
 
 template <int NW, int KI, int LJ, int WJ, int MODE, bool PHI, int CS>
 __global__ void __launch_bounds__(32 * NW) nb_small_kernel(const SmallArgs a) {
     constexpr int WI = NW / WJ, LI = 32 / LJ, Q = WJ * LJ, TILE_I = WI * KI * LI, kSmallThreads = 32 * NW;
     static_assert(WI * WJ == NW && LI * LJ == 32, "NW warps of 32 lanes");
-    static_assert(MODE == SMALL_EXACT || MODE == SMALL_NONE, "masked everywhere or no mask");
+    static_assert(MODE == SMALL_EXACT || MODE == SMALL_FLAG || MODE == SMALL_NONE, "masked everywhere, marked pairs only, or no mask");
+    static_assert(MODE != SMALL_FLAG || LJ == 1, "the marked-pair branch must be warp-uniform");
     static_assert(TILE_I % CS == 0, "every CTA of a cluster sums a whole slice of the i-tile");
     extern __shared__ __align__(128) unsigned char smem_raw[];
 #ifdef NB_SMALL_STAMPS
@@ -182,6 +194,21 @@ __global__ void __launch_bounds__(32 * NW) nb_small_kernel(const SmallArgs a) {
     // 8-byte loads of two consecutive particles need 8-byte aligned arrays (c_lo and every pair index are even)
     const bool wide = a.jp == nullptr && ((reinterpret_cast<uintptr_t>(a.xj_raw) | reinterpret_cast<uintptr_t>(a.mj_raw)) & 7u) == 0;
 
+    // SMALL_FLAG: Bloom filter of the tile's i-positions, then one bitmap of marked pairs per j-slot
+    uint32_t* filt = reinterpret_cast<uint32_t*>(smem_raw + a.flag_offset);
+    unsigned long long* sbits = reinterpret_cast<unsigned long long*>(filt + kBloomWords);
+    const int sw = small_flag_words(pstride);
+    if (MODE == SMALL_FLAG) {
+        for (int w = threadIdx.x; w < kBloomWords; w += kSmallThreads) filt[w] = 0u;
+        for (int w = threadIdx.x; w < Q * sw; w += kSmallThreads) sbits[w] = 0ull;
+        __syncthreads();
+        for (int il = threadIdx.x; il < TILE_I; il += kSmallThreads) {
+            const int i = tile0 + il;
+            if (i < a.n_i) bloom_set(filt, bloom_key(a.x_i[3 * (size_t)i + 0], a.x_i[3 * (size_t)i + 1], a.x_i[3 * (size_t)i + 2]));
+        }
+        __syncthreads();
+    }
+
     // a1 + a2: the CTA packs a round into the interleaved pair layout (Fig. A.1 packing loop).  One thread
     // per j-pair; the loads of kSmallLoadBatch pairs are in flight together (one memory latency per batch).
     auto stage_round = [&](int r_lo, int nr) {
@@ -217,16 +244,25 @@ __global__ void __launch_bounds__(32 * NW) nb_small_kernel(const SmallArgs a) {
                 const int jj = 2 * pp, sq = jj / slot_len, pos = jj - sq * slot_len;
                 float4* d = sj + ((size_t)sq * pstride + (pos >> 1)) * 2;
                 d[0] = A[u]; d[1] = B[u];
+                if (MODE == SMALL_FLAG) {                              // may one of the two coincide with an i-particle of the tile?
+                    const bool hit = bloom_test(filt, bloom_key(A[u].x, A[u].z, B[u].x)) | bloom_test(filt, bloom_key(A[u].y, A[u].w, B[u].y));
+                    if (hit) atomicOr(&sbits[sq * sw + (pos >> 7)], 1ull << ((pos >> 1) & 63));
+                }
             }
         }
     };
 
     for (int r_lo = c_lo; r_lo < c_hi; r_lo += kSmallRoundJ) {
         const int nr = min(kSmallRoundJ, c_hi - r_lo);
-        if (r_lo != c_lo) __syncthreads();                             // the previous round has been consumed
+        if (r_lo != c_lo) {
+            __syncthreads();                                           // the previous round has been consumed
+            if (MODE == SMALL_FLAG) {
+                for (int w = threadIdx.x; w < Q * sw; w += kSmallThreads) sbits[w] = 0ull;
+                __syncthreads();
+            }
+        }
         stage_round(r_lo, nr);
         __syncthreads();
-        constexpr bool masked = (MODE == SMALL_EXACT);
         NB_STAMP(1);
 
         const int len_q = max(0, min(slot_len, nr - q * slot_len));
@@ -238,13 +274,34 @@ __global__ void __launch_bounds__(32 * NW) nb_small_kernel(const SmallArgs a) {
             u64 pax[KI], pay[KI], paz[KI], pph[KI];
 #pragma unroll
             for (int k = 0; k < KI; ++k) { pax[k] = 0ull; pay[k] = 0ull; paz[k] = 0ull; pph[k] = 0ull; }
+            auto sweep = [&](auto mask_tag, int p_lo, int p_hi) {
+                constexpr int MASK = decltype(mask_tag)::value;
 #pragma unroll(KI == 2 ? 4 : 8)
-            for (int p = 0; p < nb_; ++p) {
-                const float4 A = sp[2 * (b + p)], B = sp[2 * (b + p) + 1];   // two LDS.128: (x0 x1 y0 y1) (z0 z1 m0 m1)
-                const u64 xj2 = pack2(A.x, A.y), yj2 = pack2(A.z, A.w), zj2 = pack2(B.x, B.y), mj2 = pack2(B.z, B.w);
+                for (int p = p_lo; p < p_hi; ++p) {
+                    const float4 A = sp[2 * (b + p)], B = sp[2 * (b + p) + 1];   // two LDS.128: (x0 x1 y0 y1) (z0 z1 m0 m1)
+                    const u64 xj2 = pack2(A.x, A.y), yj2 = pack2(A.z, A.w), zj2 = pack2(B.x, B.y), mj2 = pack2(B.z, B.w);
 #pragma unroll
-                for (int k = 0; k < KI; ++k)
-                    pair_body_j2<masked ? MASK_EXACT : MASK_NONE, PHI>(xj2, yj2, zj2, mj2, nxi[k], nyi[k], nzi[k], eps2_2, pax[k], pay[k], paz[k], pph[k]);
+                    for (int k = 0; k < KI; ++k)
+                        pair_body_j2<MASK, PHI>(xj2, yj2, zj2, mj2, nxi[k], nyi[k], nzi[k], eps2_2, pax[k], pay[k], paz[k], pph[k]);
+                }
+            };
+            if (MODE == SMALL_FLAG) {
+                const unsigned long long word = sbits[q * sw + (b >> 6)];      // warp-uniform (LJ = 1): kSmallBlockPairs = 64 pairs per word
+                int p = 0;
+                while (p < nb_) {                                      // alternate runs of unmarked and of marked pairs
+                    const unsigned long long rest = word >> p;
+                    const int stop = rest ? min(nb_, p + __ffsll((long long)rest) - 1) : nb_;
+                    sweep(std::integral_constant<int, MASK_NONE>{}, p, stop);
+                    if (stop >= nb_) break;
+                    const unsigned long long clear = ~(word >> stop);  // first unmarked pair at or after stop
+                    const int stop2 = clear ? min(nb_, stop + __ffsll((long long)clear) - 1) : nb_;
+                    sweep(std::integral_constant<int, MASK_EXACT>{}, stop, stop2);
+                    p = stop2;
+                }
+            } else if (MODE == SMALL_EXACT) {
+                sweep(std::integral_constant<int, MASK_EXACT>{}, 0, nb_);
+            } else {
+                sweep(std::integral_constant<int, MASK_NONE>{}, 0, nb_);
             }
 #pragma unroll
             for (int k = 0; k < KI; ++k) {                             // a5: even-j half first, then odd-j half

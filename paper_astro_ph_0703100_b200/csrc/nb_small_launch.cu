@@ -11,14 +11,19 @@
 
 namespace nb {
 
-// dynamic shared memory: the staged j-pairs, reused for the reductions
-size_t small_smem_bytes(const SmallPlan& p, int64_t n_j) {
+// dynamic shared memory: the staged j-pairs (reused for the reductions), then -- SMALL_FLAG -- the tile's Bloom filter and
+// the slot bitmaps of marked pairs
+size_t small_smem_bytes(const SmallPlan& p, int64_t n_j, bool flag, int* flag_offset) {
     const int Q = p.WJ * p.LJ;
     const int64_t chunk_max = (n_j + p.S - 1) / p.S + 2;     // as in nb_small_kernel (even chunk boundaries)
     const int round_max = (int)(chunk_max < kSmallRoundJ ? chunk_max : kSmallRoundJ);
-    const size_t stage = (size_t)Q * small_pair_stride(small_slot_len(round_max, Q)) * 32;
+    const int pstride = small_pair_stride(small_slot_len(round_max, Q));
+    const size_t stage = (size_t)Q * pstride * 32;
     const size_t red = ((p.WJ > 1 ? (size_t)p.WJ * p.tile_i : 0) + (size_t)p.tile_i) * sizeof(double4);
-    return ((stage > red ? stage : red) + 127) / 128 * 128 + 128;
+    size_t bytes = ((stage > red ? stage : red) + 127) / 128 * 128;
+    *flag_offset = (int)bytes;
+    if (flag) bytes += (size_t)kBloomWords * sizeof(uint32_t) + (size_t)Q * small_flag_words(pstride) * sizeof(unsigned long long);
+    return bytes + 128;
 }
 
 namespace {
@@ -87,13 +92,23 @@ cudaError_t launch_shape(const SmallPlan& p, const SmallArgs& a, size_t smem, cu
     return p.KI == 2 ? launch_wide<8, 2, MODE, PHI>(p, a, smem, stream) : launch_wide<8, 1, MODE, PHI>(p, a, smem, stream);
 }
 
+cudaError_t launch_flag(const SmallPlan& p, const SmallArgs& a, size_t smem, cudaStream_t stream) {
+    if (!small_shape_ok(p.NW, p.KI, p.LJ, p.WJ, p.CS) || p.LJ != 1) return cudaErrorInvalidValue;
+    if (p.NW == 16) return p.KI == 2 ? launch_wide<16, 2, SMALL_FLAG, true>(p, a, smem, stream) : launch_wide<16, 1, SMALL_FLAG, true>(p, a, smem, stream);
+    return p.KI == 2 ? launch_wide<8, 2, SMALL_FLAG, true>(p, a, smem, stream) : launch_wide<8, 1, SMALL_FLAG, true>(p, a, smem, stream);
+}
+
 }  // namespace
 
-cudaError_t small_launch(const SmallPlan& p, const SmallArgs& a, int mode, cudaStream_t stream) {
+cudaError_t small_launch(const SmallPlan& p, SmallArgs a, int mode, cudaStream_t stream) {
     if (p.S % p.CS != 0 || p.S < 1) return cudaErrorInvalidValue;
-    const size_t smem = small_smem_bytes(p, a.n_j);
-    return mode == SMALL_NONE ? launch_shape<SMALL_NONE, false>(p, a, smem, stream)
-                              : launch_shape<SMALL_EXACT, true>(p, a, smem, stream);
+    if (mode == SMALL_FLAG && p.LJ != 1) mode = SMALL_EXACT;           // the marked-pair branch needs a warp-uniform j-slot
+    const size_t smem = small_smem_bytes(p, a.n_j, mode == SMALL_FLAG, &a.flag_offset);
+    switch (mode) {
+        case SMALL_NONE: return launch_shape<SMALL_NONE, false>(p, a, smem, stream);
+        case SMALL_FLAG: return launch_flag(p, a, smem, stream);
+        default: return launch_shape<SMALL_EXACT, true>(p, a, smem, stream);
+    }
 }
 
 }  // namespace nb

@@ -8,7 +8,8 @@
 namespace nb {
 struct SmallArgs;
 struct SmallPlan;
-// One launch of nb_small_kernel under plan p.  mode = SMALL_EXACT (every pair masked) or SMALL_NONE (no mask, no
+// One launch of nb_small_kernel under plan p.  mode = SMALL_EXACT (every pair masked), SMALL_FLAG (pairs marked while
+// staged, only those masked; needs eps2 >= 2^-40; falls back to SMALL_EXACT for LJ > 1) or SMALL_NONE (no mask, no
 // potential: valid when pot == nullptr and eps2 >= 2^-40) -- nb_small.cuh.
-cudaError_t small_launch(const SmallPlan& p, const SmallArgs& a, int mode, cudaStream_t stream);
+cudaError_t small_launch(const SmallPlan& p, SmallArgs a, int mode, cudaStream_t stream);
 }  // namespace nb

@@ -69,6 +69,7 @@ struct Knobs {
     bool plan_set = false;       int pK = 0, pWI = 0, pWJ = 0, pS = 0;                 // NB_PLAN
     bool small_plan_set = false; int sNW = 0, sKI = 0, sLJ = 0, sWJ = 0, sS = 0, sCS = 0;   // NB_SMALL_PLAN
     int small = -1;              // NB_SMALL: -1 default, 0 never, 1 always
+    int small_mask = -1;         // NB_SMALL_MASK: -1 default (marked pairs), nb::SMALL_EXACT = every pair masked
     int mask = -1;               // NB_MASK: -1 default, else nb::MODE_*
     int fused = -1;              // NB_FUSED_REDUCE
     int direct = -1;             // NB_DIRECT
@@ -103,6 +104,11 @@ bool parse_knob(Knobs* k, const char* key, const char* value) {
         k->small_plan_set = true; k->sNW = nw; k->sKI = ki; k->sLJ = lj; k->sWJ = wj; k->sS = ss; k->sCS = cs;
         return true;
     }
+    if (!std::strcmp(key, "NB_SMALL_MASK")) {
+        if (unset) { k->small_mask = -1; return true; }
+        if (value[0] == 'e') k->small_mask = nb::SMALL_EXACT; else if (value[0] == 'f') k->small_mask = nb::SMALL_FLAG; else return false;
+        return true;
+    }
     if (!std::strcmp(key, "NB_MASK")) {
         if (unset) { k->mask = -1; return true; }
         if (value[0] == 'e') k->mask = nb::MODE_EXACT; else if (value[0] == 'b') k->mask = nb::MODE_BLOOM;
@@ -127,7 +133,7 @@ bool parse_knob(Knobs* k, const char* key, const char* value) {
     return false;
 }
 
-const char* const kKnobKeys[] = {"NB_PLAN", "NB_SMALL_PLAN", "NB_SMALL", "NB_MASK", "NB_FUSED_REDUCE", "NB_DIRECT", "NB_STEP_GRAPH", "NB_BATCH_TILE"};
+const char* const kKnobKeys[] = {"NB_PLAN", "NB_SMALL_PLAN", "NB_SMALL", "NB_SMALL_MASK", "NB_MASK", "NB_FUSED_REDUCE", "NB_DIRECT", "NB_STEP_GRAPH", "NB_BATCH_TILE"};
 
 // the current switches: one atomic load per call; the environment is read once, here
 const Knobs& knobs() {
@@ -427,8 +433,15 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         sa.n_j = (int)n_j;
         sa.S = sp.S;
         sa.eps2 = eps2;
-        // coincident pairs: no mask at all without phi (eps2 >= 2^-40), else every pair masked
-        const int small_mode = a_only ? nb::SMALL_NONE : nb::SMALL_EXACT;
+        sa.flag_offset = 0;
+        // coincident pairs: no mask at all without phi (eps2 >= 2^-40); else only the pairs marked while staged are masked
+        // -- or every pair: eps2 < 2^-40 (an unmasked coincident pair would overflow), NB_SMALL_MASK=exact
+        // (marking pays when a CTA stages many j per i-tile: filter + tests cost ~1 us, the unmasked loop runs 15 % faster;
+        //  measured on C2 24.65 -> 23.64 us per call, on C0 -- 512 j per CTA -- nothing: profiles/r02_small_calls.md)
+        const bool flag_pays = (n_j + sp.S - 1) / sp.S >= 1024;
+        const int small_mode = a_only ? nb::SMALL_NONE
+                               : (eps2 >= kUnmaskedMinEps2 && kn.small_mask != nb::SMALL_EXACT && (flag_pays || kn.small_mask == nb::SMALL_FLAG))
+                                     ? nb::SMALL_FLAG : nb::SMALL_EXACT;
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (t_profile) {
             NB_CUDA(cudaEventCreate(&e0));

@@ -60,6 +60,14 @@ def test_every_small_decomposition_matches_oracle(nb, plan, nbdebug):
     assert nb.last_launch_count() == 1
     ref_acc, ref_pot = oracle.force(w.x_i, w.x_j, w.m_j, w.eps2)
     check_parity(acc, pot, ref_acc, ref_pot, str(plan))
+    # masking only the j-pairs marked while staged (Bloom filter of the tile's i-positions; LJ = 1 shapes, the default for
+    # large j-chunks) and masking every pair store the same bits
+    nbdebug.setenv("NB_SMALL_MASK", "flag")
+    acc, pot = gpu_force(nb, w.x_i, w.x_j, w.m_j, w.eps2)
+    nbdebug.setenv("NB_SMALL_MASK", "exact")
+    acc_e, pot_e = gpu_force(nb, w.x_i, w.x_j, w.m_j, w.eps2)
+    nbdebug.delenv("NB_SMALL_MASK")
+    assert np.array_equal(acc, acc_e) and np.array_equal(pot, pot_e)
     # acceleration only: the unmasked 12-instruction loop (a coincident pair adds m u^3 (+-0) = +-0); the same sum as the
     # masked loop's bit for bit
     acc2, pot2 = gpu_force(nb, w.x_i, w.x_j, w.m_j, w.eps2, want_pot=False)
@@ -203,7 +211,12 @@ def test_degenerate_positions(nb, nbdebug):
     x[:900] = (1.0, 2.0, 3.0)
     for plan in ("16,2,1,2,1,1", "8,1,1,8,3,1", None):
         nbdebug.setenv("NB_SMALL_PLAN", plan) if plan else nbdebug.delenv("NB_SMALL_PLAN")
+        nbdebug.setenv("NB_SMALL_MASK", "flag")
         acc, pot = gpu_force(nb, x, x, m, 1e-3, alias=True)
+        nbdebug.setenv("NB_SMALL_MASK", "exact")
+        acc_e, pot_e = gpu_force(nb, x, x, m, 1e-3, alias=True)
+        nbdebug.delenv("NB_SMALL_MASK")
+        assert np.array_equal(acc, acc_e) and np.array_equal(pot, pot_e)       # every pair marked: same bits as masked everywhere
         ref_acc, ref_pot = oracle.force(x, x, m, 1e-3)
         sel = slice(900, n)                                       # the coincident ones have a ~ 0: compare the others relatively
         check_parity(acc[sel], pot[sel], ref_acc[sel], ref_pot[sel], f"degenerate {plan}")
