@@ -249,6 +249,9 @@ OPS = {
 }
 # row f3, a central force other than gravity (reading R19): 24 FP32-pipe instructions per pair in the SASS of
 # pipeline_kernel<PipelineLennardJones> (12 FMUL + 7 FFMA + 5 FADD) + 1 MUFU.RSQ; Gflop/s printed at 24 and at 50 per pair
+# row f2 with the lists as int32 indices into ONE packed particle array (nb_force_batched_indexed): same kernel arithmetic,
+# the ring filled by gathered cp.async copies; 4 B per list entry + 16 B per distinct particle cross PCIe in the e2e leg
+OPS["batched_indexed"] = {"inst": 13, "kernel": "nb_batched_kernel<INDEXED> (row f2, lists as indices)", "flops": (20, 38)}
 OPS["lj"] = {"inst": 24, "kernel": "pipeline_kernel<PipelineLennardJones> (generalised kernel, row f3)", "flops": (24, 50)}
 LEAPFROG_KDK_PER_CALL = 100
 
@@ -348,6 +351,21 @@ class Problem:
                          f"eps2={w.eps2:.6g}, seed=1, one nb_force_jerk call with phi (configs[1]'s particles)")
             self.host = [w.x_j, w.v, w.m_j]
             self.n_out = w.n_i
+        elif op == "batched_indexed":
+            w = wl.tree_list_workload(524288, 32, 256, 2000, 6000, 1.0 / 128, seed=7, name="T1")
+            self.w, self.pairs = w, float(w.pairs)
+            # the distinct list records are the tree code's particle array (particles + cell pseudo-particles), the lists
+            # become indices into it: pure re-indexing of the seeded workload, no arithmetic
+            rec = np.ascontiguousarray(np.concatenate([w.x_j, w.m_j[:, None]], axis=1).astype(np.float32))
+            key = rec.view(np.uint64).reshape(-1, 2)
+            _, first, inv = np.unique(key[:, 0] ^ (key[:, 1] * np.uint64(0x9E3779B97F4A7C15)), return_index=True, return_inverse=True)
+            xm_p = np.ascontiguousarray(rec[first])
+            assert np.array_equal(xm_p[inv], rec)
+            self.name = (f"row f2 (T1 indexed): {w.meta.get('model', '')}; 524288 particles in {w.n_batch} groups of 32..256, lists "
+                         f"of 2000..6000 as int32 indices ({inv.size} entries) into {xm_p.shape[0]} distinct packed records, "
+                         f"eps2={w.eps2:.6g}, seed=7, one nb_force_batched_indexed call with phi")
+            self.host = [w.i_offsets, w.j_offsets, w.x_i, inv.astype(np.int32), xm_p]
+            self.n_out = w.x_i.shape[0]
         else:
             w = wl.tree_list_workload(524288, 32, 256, 2000, 6000, 1.0 / 128, seed=7, name="T1")
             self.w, self.pairs = w, float(w.pairs)
@@ -400,6 +418,8 @@ class Problem:
             self.launches = launches
             if t is self.dev:
                 self.cycles_done += 1
+        elif self.op == "batched_indexed":
+            nb.force_batched_indexed(t[0], t[1], t[2], t[3], t[4], w.eps2, acc_out=self.outs[0], pot_out=self.outs[1])
         elif self.op == "jerk":
             nb.force_jerk(t[0], t[1], t[0], t[1], t[2], w.eps2, acc_out=self.outs[0], jerk_out=self.outs[1], pot_out=self.outs[2])
         else:
@@ -444,7 +464,8 @@ class Problem:
             return "pinned host (x, v, m) -> cudaMemcpyAsync -> nb_hermite4 (100 steps) -> cudaMemcpyAsync of a, j, phi -> pinned host"
         if self.op == "leapfrog":
             return "pinned host (x, v, m) -> cudaMemcpyAsync -> nb_leapfrog_kdk (100 KDK steps) -> cudaMemcpyAsync of a, phi -> pinned host"
-        return f"pinned host tensors -> cudaMemcpyAsync -> nb_{'force_jerk' if self.op == 'jerk' else 'force_batched'} -> cudaMemcpyAsync -> pinned host"
+        name = {"jerk": "force_jerk", "batched_indexed": "force_batched_indexed"}.get(self.op, "force_batched")
+        return f"pinned host tensors -> cudaMemcpyAsync -> nb_{name} -> cudaMemcpyAsync -> pinned host"
 
     def plan(self, sm_count):
         if self.op == "force":
@@ -471,6 +492,8 @@ def oracle_rate_op(op, w, target_seconds, rng_seed=0):
         return oracle_rate(w, target_seconds, rng_seed)
     if op in ("hermite", "block", "cunbody4"):
         op = "jerk"
+    if op == "batched_indexed":
+        op = "batched"
     cores = oracle.num_threads()
     rng = np.random.default_rng(rng_seed)
     if op == "lj":

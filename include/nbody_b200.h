@@ -274,6 +274,24 @@ int nb_force_batched_packed(int64_t n_batch, const int32_t *i_offsets, const int
                             void *stream);
 
 /*
+ * nb_force_batched_indexed -- nb_force_batched with the interaction lists given as INDICES into one array of packed particle
+ * records: what a tree code holds (its particles and cell pseudo-particles once, a list of integers per group).  Sub-problem
+ * b: i-particles as in nb_force_batched; j-list = xm_p[j_index[k]] for k in [j_offsets[b], j_offsets[b+1]).  4 bytes per list
+ * entry instead of 16 cross PCIe / HBM; the kernel fills its shared-memory rings with gathered 16-byte asynchronous copies.
+ *
+ *   j_index   device, const, int32 [n_list_total], every value in [0, n_p) (not validated: device data)
+ *   xm_p      device, const, float [n_p][4] = (x, y, z, m), 16-byte aligned
+ * Same results as nb_force_batched on the expanded lists, bit for bit; everything else as there.
+ */
+int nb_force_batched_indexed(int64_t n_batch, const int32_t *i_offsets, const int32_t *j_offsets,
+                             int64_t n_i_total, const float *x_i,
+                             int64_t n_list_total, const int32_t *j_index,
+                             int64_t n_p, const float *xm_p,
+                             float eps2,
+                             float *acc_out, float *pot_out,
+                             void *stream);
+
+/*
  * nb_hermite4 -- n_steps steps of the 4th-order Hermite scheme with a shared, constant time step, all state on the
  * device: the scheme the paper names as the user of its force + jerk pipeline; the paper does
  * not describe it, this is the textbook predict - evaluate - correct form with one nb_force_jerk per step:

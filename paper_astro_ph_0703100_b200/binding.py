@@ -62,6 +62,8 @@ def lib() -> ctypes.CDLL:
         l.nb_force_batched.restype = ci
         l.nb_force_batched_packed.argtypes = [i64, p, p, i64, p, i64, p, f32, p, p, p]
         l.nb_force_batched_packed.restype = ci
+        l.nb_force_batched_indexed.argtypes = [i64, p, p, i64, p, i64, p, i64, p, f32, p, p, p]
+        l.nb_force_batched_indexed.restype = ci
         l.nb_force_jerk_host.argtypes = [i64, p, p, i64, p, p, p, f32, p, p, p]
         l.nb_force_jerk_host.restype = ci
         l.nb_plan_query_jerk.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
@@ -288,6 +290,29 @@ def force_batched_packed(i_offsets, j_offsets, x_i, xm_j, eps2: float, acc_out=N
                                            xm_j.data_ptr(), float(eps2), acc_out.data_ptr(),
                                            None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
     _check(st, "nb_force_batched_packed")
+    return acc_out, pot_out
+
+
+def force_batched_indexed(i_offsets, j_offsets, x_i, j_index, xm_p, eps2: float, acc_out=None, pot_out=None,
+                          want_pot: bool = True, stream=None):
+    """nb_force_batched_indexed on CUDA tensors: lists as int32 indices [n_list_total] into packed records xm_p [n_p, 4]."""
+    import torch
+    _dev_f32(x_i, "x_i", (3,)); _dev_f32(xm_p, "xm_p", (4,))
+    for t, name in ((i_offsets, "i_offsets"), (j_offsets, "j_offsets"), (j_index, "j_index")):
+        if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.int32 or not t.is_contiguous() or t.dim() != 1:
+            raise TypeError(f"{name} must be a contiguous 1-D int32 CUDA tensor")
+    if i_offsets.shape[0] != j_offsets.shape[0] or i_offsets.shape[0] < 1:
+        raise ValueError("i_offsets and j_offsets must both have n_batch + 1 entries")
+    n_batch, n_i = i_offsets.shape[0] - 1, x_i.shape[0]
+    if acc_out is None:
+        acc_out = torch.zeros((n_i, 3), dtype=torch.float32, device=x_i.device)
+    if pot_out is None and want_pot:
+        pot_out = torch.zeros((n_i,), dtype=torch.float32, device=x_i.device)
+    with torch.cuda.device(x_i.device):
+        st = lib().nb_force_batched_indexed(n_batch, i_offsets.data_ptr(), j_offsets.data_ptr(), n_i, x_i.data_ptr(),
+                                            j_index.shape[0], j_index.data_ptr(), xm_p.shape[0], xm_p.data_ptr(), float(eps2),
+                                            acc_out.data_ptr(), None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_force_batched_indexed")
     return acc_out, pot_out
 
 

@@ -86,8 +86,20 @@ __device__ __forceinline__ void half_sweep(const float4* __restrict__ sp, int np
     }
 }
 
+// 16-byte asynchronous copy global -> shared (LDGSTS) and its group bookkeeping: the gathered ring fill of INDEXED lists
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 // G = packed groups of 64 i-particles a CTA can hold (tile = 64 G); STAGES = ring depth per warp.
-template <bool MASKED, int G, int STAGES>
+// INDEXED: the lists are int32 indices (a.j_index) into ONE array of packed particle records (a.jp) -- what a tree code
+// holds: 4 bytes per list entry instead of 16.  A ring slot is then filled by 256 gathered 16-byte cp.async copies (8 per
+// lane, the indices of the tile after next already in registers) instead of one bulk copy; completion is tracked per lane
+// with cp.async groups (one group per tile, empty ones included, so the count is uniform) + __syncwarp.
+template <bool MASKED, int G, int STAGES, bool INDEXED = false>
 __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const ForceArgs a) {
     static_assert(G >= 1 && G <= 4, "1 .. 4 packed groups");
     constexpr int K = 2 * G, WJ = 8, TJ = 256, kBatchTile = 64 * G;
@@ -115,7 +127,23 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
     const int j_end = jr_lo + (int)((long long)jr_n * (wj + 1) / WJ);
     const int n_sub = j_end - j_begin;
     const int n_tiles = (n_sub + TJ - 1) / TJ;
-    const unsigned char* src = reinterpret_cast<const unsigned char*>(a.jp + j_begin);
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(a.jp + (INDEXED ? 0 : j_begin));
+    // INDEXED: indices of the tile that will be issued next (8 per lane), and the issue of one tile's gathers
+    int nxt[8];
+    auto load_indices = [&](int t) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int e = t * TJ + q * 32 + lane;
+            nxt[q] = (t < n_tiles && e < n_sub) ? a.j_index[j_begin + e] : -1;
+        }
+    };
+    auto issue_gather = [&](int t) {                                   // tile t into slot t % STAGES, from the indices in nxt[]
+        const uint32_t dst = ring + (t % STAGES) * TJ * 16;
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+            if (nxt[q] >= 0) cp_async_16(dst + (q * 32 + lane) * 16, a.jp + nxt[q]);
+        cp_async_commit();
+    };
 
     const int i_base = i_lo + lane;
     u64 nxi[G], nyi[G], nzi[G];
@@ -159,8 +187,15 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
     }
     __syncthreads();                                                   // barriers initialised
 
+    if (INDEXED) {
+        load_indices(0);
+        for (int t = 0; t < STAGES; ++t) {                             // STAGES groups in flight, empty beyond the list
+            issue_gather(t);
+            load_indices(t + 1);
+        }
+    }
     // each warp is its own producer; a ring slot is refilled by the warp that has just finished reading it
-    if (lane == 0) {
+    if (!INDEXED && lane == 0) {
         const int pre = n_tiles < STAGES ? n_tiles : STAGES;
         for (int t = 0; t < pre; ++t) {
             const uint32_t bytes = (uint32_t)min(TJ, n_sub - t * TJ) * 16u;
@@ -175,7 +210,12 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
 
     for (int t = 0; t < n_tiles; ++t) {
         const int slot = t % STAGES;
-        mbar_wait(full0 + 8 * slot, (uint32_t)(t / STAGES) & 1u);
+        if (INDEXED) {
+            cp_async_wait<STAGES - 1>();                               // this lane's copies of tile t have landed ...
+            __syncwarp();                                              // ... and so have the other lanes'
+        } else {
+            mbar_wait(full0 + 8 * slot, (uint32_t)(t / STAGES) & 1u);
+        }
         const int nc = min(TJ, n_sub - t * TJ);                        // TJ == SUB: one Eq. (2) block per tile
         const float4* sp = reinterpret_cast<const float4*>(rings + wj * RING_BYTES + slot * TJ * 16);
         u64 pax[G], pay[G], paz[G], pph[G];
@@ -216,7 +256,11 @@ __global__ void __launch_bounds__(256, (G == 1 ? 2 : 1)) nb_batched_kernel(const
             add_partials<G>(run, pax, pay, paz, pph);
         }
         __syncwarp();                                                  // every lane is done with the slot
-        if (lane == 0 && t + STAGES < n_tiles) {
+        if (INDEXED) {
+            issue_gather(t + STAGES);                                  // nxt[] holds tile t + STAGES (or nothing: an empty group)
+            load_indices(t + STAGES + 1);
+        }
+        if (!INDEXED && lane == 0 && t + STAGES < n_tiles) {
             const int tn = t + STAGES;
             const uint32_t bytes = (uint32_t)min(TJ, n_sub - tn * TJ) * 16u;
             mbar_expect_tx(full0 + 8 * slot, bytes);

@@ -208,6 +208,7 @@ struct ForceArgs {
     const int* j_off;      // nb_batched_kernel: [n_batch + 1] first j of every sub-problem
     const int* tile_start; // nb_batched_kernel: [n_batch + 1] first CTA of every sub-problem (exclusive scan of its i-tiles)
     const int* cta_batch;  // nb_batched_kernel: [number of CTAs] sub-problem of every CTA
+    const int* j_index;    // nb_batched_kernel<INDEXED>: [n_list_total] indices into jp (the packed particle array)
     int n_batch;
     int n_i;
     int n_j;

@@ -504,7 +504,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
     args.eps2 = eps2;
     args.coin_lists = nullptr;
     args.coin_flag = nullptr;
-    args.i_off = args.j_off = args.tile_start = args.cta_batch = nullptr;
+    args.i_off = args.j_off = args.tile_start = args.cta_batch = args.j_index = nullptr;
     args.n_batch = 0;
     if (direct) {                                                      // small call: one launch (packs its own j)
         rc = (mode == nb::MODE_BLOOM) ? launch_force<nb::MODE_BLOOM, false, true>(args, plan, stream)
@@ -672,21 +672,21 @@ int batched_groups(int64_t n_i_total, int64_t n_batch) {
     return 4;
 }
 
-template <bool MASKED, int G, int STAGES>
+template <bool MASKED, int G, int STAGES, bool INDEXED>
 int launch_batched_inst(const nb::ForceArgs& args, unsigned max_ctas, cudaStream_t stream) {
     constexpr size_t ring = (size_t)8 * STAGES * 256 * 16;
     constexpr size_t red = (size_t)8 * (2 * G) * 4 * 32 * sizeof(double);
     constexpr size_t smem = (ring > red ? ring : red) + 8 * STAGES * sizeof(uint64_t) + 128;
     static std::atomic<uint64_t> configured{0};
-    return launch_dominant(nb::nb_batched_kernel<MASKED, G, STAGES>, &configured, dim3(max_ctas, 1, 1), 256, smem, stream, args);
+    return launch_dominant(nb::nb_batched_kernel<MASKED, G, STAGES, INDEXED>, &configured, dim3(max_ctas, 1, 1), 256, smem, stream, args);
 }
 
-template <bool MASKED>
+template <bool MASKED, bool INDEXED>
 int launch_batched(const nb::ForceArgs& args, int groups, unsigned max_ctas, cudaStream_t stream) {
     switch (groups) {
-        case 1: return launch_batched_inst<MASKED, 1, 2>(args, max_ctas, stream);  // 64 KB of rings, 2 CTAs per SM
-        case 2: return launch_batched_inst<MASKED, 2, 3>(args, max_ctas, stream);
-        default: return launch_batched_inst<MASKED, 4, 3>(args, max_ctas, stream);
+        case 1: return launch_batched_inst<MASKED, 1, 2, INDEXED>(args, max_ctas, stream);  // 64 KB of rings, 2 CTAs per SM
+        case 2: return launch_batched_inst<MASKED, 2, 3, INDEXED>(args, max_ctas, stream);
+        default: return launch_batched_inst<MASKED, 4, 3, INDEXED>(args, max_ctas, stream);
     }
 }
 
@@ -698,9 +698,11 @@ extern "C" {
 
 namespace {
 // packed_j != nullptr: the caller holds the list records as 16-byte (x, y, z, m) rows already (nb_force_batched_packed)
+// j_index != nullptr: the lists are indices into the packed particle array packed_j [n_p] (nb_force_batched_indexed);
+// n_j_total is then the number of list entries
 int force_batched_impl(int64_t n_batch, const int32_t* i_offsets, const int32_t* j_offsets, int64_t n_i_total,
                        const float* x_i, int64_t n_j_total, const float* x_j, const float* m_j, const float4* packed_j,
-                       float eps2, float* acc_out, float* pot_out, void* stream_) {
+                       float eps2, float* acc_out, float* pot_out, void* stream_, const int32_t* j_index = nullptr) {
     t_launches = 0;
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
     if (bad_count(n_batch) || bad_count(n_i_total) || bad_count(n_j_total)) return NB_ERR_INVALID_VALUE;
@@ -750,6 +752,7 @@ int force_batched_impl(int64_t n_batch, const int32_t* i_offsets, const int32_t*
     args.tickets = nullptr;
     args.coin_lists = nullptr;
     args.coin_flag = nullptr;
+    args.j_index = j_index;
     args.i_off = i_offsets;
     args.j_off = j_offsets;
     args.tile_start = tile_start;
@@ -761,8 +764,11 @@ int force_batched_impl(int64_t n_batch, const int32_t* i_offsets, const int32_t*
     args.eps2 = eps2;
     // every pair masked -- unless phi is not wanted and eps2 >= 2^-40, where no pair needs the mask (see force_impl)
     const bool a_only = !pot_out && eps2 >= kUnmaskedMinEps2 && knobs().mask < 0;
-    return a_only ? launch_batched<false>(args, groups, (unsigned)max_ctas, stream)
-                  : launch_batched<true>(args, groups, (unsigned)max_ctas, stream);
+    if (j_index)
+        return a_only ? launch_batched<false, true>(args, groups, (unsigned)max_ctas, stream)
+                      : launch_batched<true, true>(args, groups, (unsigned)max_ctas, stream);
+    return a_only ? launch_batched<false, false>(args, groups, (unsigned)max_ctas, stream)
+                  : launch_batched<true, false>(args, groups, (unsigned)max_ctas, stream);
 }
 }  // namespace
 
@@ -772,6 +778,17 @@ int nb_force_batched(int64_t n_batch, const int32_t* i_offsets, const int32_t* j
                      const float* x_i, int64_t n_j_total, const float* x_j, const float* m_j, float eps2,
                      float* acc_out, float* pot_out, void* stream) {
     return force_batched_impl(n_batch, i_offsets, j_offsets, n_i_total, x_i, n_j_total, x_j, m_j, nullptr, eps2, acc_out, pot_out, stream);
+}
+
+int nb_force_batched_indexed(int64_t n_batch, const int32_t* i_offsets, const int32_t* j_offsets, int64_t n_i_total,
+                             const float* x_i, int64_t n_list_total, const int32_t* j_index, int64_t n_p, const float* xm_p,
+                             float eps2, float* acc_out, float* pot_out, void* stream) {
+    if (bad_count(n_p) || (n_list_total > 0 && (!j_index || !xm_p || n_p < 1))) return NB_ERR_INVALID_VALUE;
+    static const float4 dummy = {0.f, 0.f, 0.f, 0.f};
+    static const int32_t dummy_index = 0;
+    return force_batched_impl(n_batch, i_offsets, j_offsets, n_i_total, x_i, n_list_total, nullptr, nullptr,
+                              xm_p ? reinterpret_cast<const float4*>(xm_p) : &dummy, eps2, acc_out, pot_out, stream,
+                              j_index ? j_index : &dummy_index);
 }
 
 int nb_force_batched_packed(int64_t n_batch, const int32_t* i_offsets, const int32_t* j_offsets, int64_t n_i_total,

@@ -188,3 +188,43 @@ def test_packed_entry_is_bitwise_the_unpacked_call(nb):
     lib = nb.lib()
     assert lib.nb_force_batched_packed(1, io.data_ptr(), jo.data_ptr(), 5, xi.data_ptr(), 5, None, 0.1, a1.data_ptr(), None, None) == 1
     assert lib.nb_force_batched_packed(1, io.data_ptr(), jo.data_ptr(), 5, xi.data_ptr(), 5, xm.data_ptr() + 4, 0.1, a1.data_ptr(), None, None) == 1
+
+
+def test_indexed_entry_is_bitwise_the_expanded_lists(nb):
+    """nb_force_batched_indexed: lists as int32 indices into ONE array of packed particle records (what a tree code holds).
+    The particle array is the de-duplicated, shuffled set of list records; the result must be bit for bit the one of
+    nb_force_batched_packed on the expanded lists (same records, same order, gathered instead of bulk-copied) -- with and
+    without phi, for every tile shape -- and within tolerance of the oracle."""
+    import torch
+    w = wl.tree_list_workload(5000, 30, 200, 700, 2000, 1.0 / 128, seed=6)
+    rec = np.concatenate([w.x_j, w.m_j[:, None]], axis=1).astype(np.float32)
+    uniq, inverse = np.unique(np.ascontiguousarray(rec).view([("", np.float32)] * 4).ravel(), return_inverse=True)
+    perm = np.random.default_rng(1).permutation(uniq.size)
+    xm_p = np.ascontiguousarray(uniq.view(np.float32).reshape(-1, 4)[perm])
+    where = np.empty(uniq.size, dtype=np.int64); where[perm] = np.arange(uniq.size)
+    j_index = where[inverse.ravel()].astype(np.int32)
+    assert np.array_equal(xm_p[j_index], rec) and xm_p.shape[0] < rec.shape[0]          # lists share particles
+    io, jo, xi = dev(w.i_offsets), dev(w.j_offsets), dev(w.x_i)
+    for want_pot in (True, False):
+        a0, p0 = nb.force_batched_packed(io, jo, xi, dev(rec), w.eps2, want_pot=want_pot)
+        a1, p1 = nb.force_batched_indexed(io, jo, xi, dev(j_index), dev(xm_p), w.eps2, want_pot=want_pot)
+        torch.cuda.synchronize()
+        assert nb.last_launch_count() == 2
+        assert torch.equal(a0, a1) and (p0 is None or torch.equal(p0, p1))
+    ra, rp = oracle.force_batched(w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j, w.eps2)
+    a1, p1 = nb.force_batched_indexed(io, jo, xi, dev(j_index), dev(xm_p), w.eps2)
+    check(a1.cpu().numpy(), p1.cpu().numpy(), ra, rp, "indexed")
+    lib = nb.lib()
+    assert lib.nb_force_batched_indexed(1, io.data_ptr(), jo.data_ptr(), 5, xi.data_ptr(), 5, None, 5, dev(xm_p).data_ptr(), 0.1, a1.data_ptr(), None, None) == 1
+    # ragged: lists of 1 .. 9 entries, tiles of 1 .. 70 particles
+    rng = np.random.default_rng(2)
+    n_b = 40
+    ni = rng.integers(1, 71, n_b); nj = rng.integers(1, 10, n_b)
+    io2 = np.concatenate([[0], np.cumsum(ni)]).astype(np.int32); jo2 = np.concatenate([[0], np.cumsum(nj)]).astype(np.int32)
+    xp = rng.normal(size=(50, 3)).astype(np.float32); mp = rng.uniform(0.5, 1.5, 50).astype(np.float32)
+    idx2 = rng.integers(0, 50, jo2[-1]).astype(np.int32)
+    xi2 = rng.normal(size=(io2[-1], 3)).astype(np.float32)
+    a2, p2 = nb.force_batched_indexed(dev(io2), dev(jo2), dev(xi2), dev(idx2), dev(np.concatenate([xp, mp[:, None]], 1)), 0.01)
+    torch.cuda.synchronize()
+    ra, rp = oracle.force_batched(io2, jo2, xi2, xp[idx2], mp[idx2], 0.01)
+    check(a2.cpu().numpy(), p2.cpu().numpy(), ra, rp, "indexed ragged")

@@ -35,7 +35,7 @@ def test_contract_line_small_force_call_with_parity():
     assert "workload" in d["config"] and "sm_mhz" in d["clocks"]
 
 
-@pytest.mark.parametrize("op", ["jerk", "batched", "leapfrog", "hermite", "block", "cunbody", "cunbody4", "lj"])
+@pytest.mark.parametrize("op", ["jerk", "batched", "batched_indexed", "leapfrog", "hermite", "block", "cunbody", "cunbody4", "lj"])
 def test_every_op_prints_a_line(op):
     d = _run("--op", op, "--steps", "1", "--warmup", "3", "--no-cpu-baseline")
     assert d["config"]["op"] == op and d["value"] > 0 and d["gpu_launches"] > 0

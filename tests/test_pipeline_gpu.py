@@ -144,3 +144,49 @@ def test_lennard_jones_pipeline_edge_cases(nb):
     pair = np.array([[0, 0, 0, sigma / 2, np.sqrt(eps)], [2 ** (1 / 6) * sigma, 0, 0, sigma / 2, np.sqrt(eps)]], np.float32)
     out = nb.cunbody_lennard_jones(dev(pair), dev(pair)).cpu().numpy()
     assert np.abs(out[:, :3]).max() <= 2e-5 * 24 * eps / sigma and np.abs(out[:, 3] + eps).max() <= 1e-5 * eps
+
+
+@pytest.mark.parametrize("which", ["a3", "a4", "lj"])
+def test_bench_size_in_the_launch_configuration_bench_times(nb, which):
+    """N = 131072, the calls `bench.py --op cunbody | cunbody4 | lj` time (packed path, S j-chunks in whole waves, second
+    pass): 2048 seeded i-records of the full-size output against the oracle, plus finiteness of everything."""
+    import torch
+    n = 131072
+    idx = np.sort(np.random.default_rng(3).choice(n, 2048, replace=False))
+    if which == "lj":
+        rows = wl.lj_fluid_rows(n, 0.8, 0.1, seed=1)
+        out = nb.cunbody_lennard_jones(dev(rows), dev(rows))
+        torch.cuda.synchronize()
+        out = out.cpu().numpy().astype(np.float64)
+        assert np.all(np.isfinite(out))
+        ref = oracle.lennard_jones(np.ascontiguousarray(rows[idx]), rows)
+        sub = idx[::16]                                               # the error scales need an [i][j][3] array: 128 records
+        fs, us = np.concatenate([_lj_scales(np.ascontiguousarray(rows[sub[k:k + 32]]), rows) for k in range(0, sub.size, 32)], axis=1)
+        assert (np.linalg.norm(out[sub, :3] - ref[::16, :3], axis=1) / fs).max() <= 1e-5
+        assert (np.abs(out[sub, 3] - ref[::16, 3]) / us).max() <= 1e-5
+        # all 2048: relative to the largest force / energy scale of the sample (the fluid is homogeneous)
+        assert np.abs(out[idx, :3] - ref[:, :3]).max() <= 1e-5 * fs.max() and np.abs(out[idx, 3] - ref[:, 3]).max() <= 1e-5 * us.max()
+        return
+    w = wl.plummer_workload(n, 1.0 / 256, seed=1, with_velocities=True)
+    if which == "a3":
+        e2 = np.full(n, w.eps2, np.float32)
+        p_xi, p_xj = rows_a3(w.x_j, e2, w.x_j, w.m_j)
+        p_fi = nb.cunbody_force(dev(p_xj), dev(p_xi))
+        torch.cuda.synchronize()
+        p_fi = p_fi.cpu().numpy()
+        assert np.all(np.isfinite(p_fi))
+        ra, _ = oracle.force(np.ascontiguousarray(w.x_j[idx]), w.x_j, w.m_j, w.eps2)
+        e = oracle.error_metrics(p_fi[idx], ra)
+        assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4, e
+    else:
+        p_xi, p_xj = rows_a4(w.x_j, w.v, w.x_j, w.v, w.m_j)
+        p_fi = nb.cunbody_force_jerk_pot(dev(p_xj), dev(p_xi))
+        torch.cuda.synchronize()
+        p_fi = p_fi.cpu().numpy()
+        assert np.all(np.isfinite(p_fi))
+        ra, rj, rp = oracle.force_jerk(np.ascontiguousarray(w.x_j[idx]), np.ascontiguousarray(w.v[idx]), w.x_j, w.v, w.m_j,
+                                       np.float32(1.0 / 65536.0))
+        e = oracle.error_metrics(p_fi[idx, 0:3], ra, p_fi[idx, 6], rp)
+        ej = oracle.error_metrics(p_fi[idx, 3:6], rj)
+        assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and e["pot_rms"] <= 1e-5, e
+        assert ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-4, ej
