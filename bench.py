@@ -51,7 +51,7 @@ def modelled_traffic(args, prob, nb, sm_count):
     p = nb.plan_query(w.n_i, w.n_j, sm_count)
     partial = 2.0 * 32.0 * w.n_i * p["S"] if p["S"] > 1 else 0.0
     return base + partial, (f"modelled from the live plan (S = {p['S']} j-chunks x n_i x 32 B of FP64 partials, written and read "
-                            "back; ncu on C1: 71 MB, profiles/r01_ncu_full.md)")
+                            "back; ncu on C1: 72.0 MB, profiles/r02_ncu_c1.md)")
 
 
 def load_peaks():

@@ -597,3 +597,48 @@ def test_ftz_deviation_is_confined_to_subnormal_differences(nb, mode, nbdebug):
     acc, pot = gpu_force(nb, xi, x, w.m_j, w.eps2)
     ref_acc, ref_pot = oracle.force(xi, x, w.m_j, w.eps2)
     assert np.abs(pot / ref_pot - 1.0).max() < 1e-5
+
+
+def test_concurrent_host_threads_share_the_default_stream_safely(nb):
+    """include/nbody_b200.h "threads": the workspace of a (device, stream) is locked while a call grows it and enqueues
+    the work that uses it.  Two host threads hammer nb_force_host (both on the default stream, different sizes, so the
+    shared staging buffer is re-grown and re-filled all the time) and a third one nb_force on its own stream; every result
+    must be the one the same call gives alone, bit for bit."""
+    import threading
+    import torch
+    ws = [wl.subset_workload(3000 + 517 * k, 300 + 91 * k, 1.0 / 128, seed=60 + k) for k in range(4)]
+    alone = [nb.force_host(w.x_i, w.x_j, w.m_j, w.eps2) for w in ws]
+    errors = []
+
+    def host_worker(offset):
+        try:
+            for r in range(12):
+                k = (r + offset) % 4
+                a, p = nb.force_host(ws[k].x_i, ws[k].x_j, ws[k].m_j, ws[k].eps2)
+                if not (np.array_equal(a, alone[k][0]) and np.array_equal(p, alone[k][1])):
+                    errors.append(("host", offset, r, k))
+        except Exception as exc:                                       # pragma: no cover
+            errors.append(repr(exc))
+
+    def device_worker():
+        try:
+            torch.cuda.set_device(0)
+            s = torch.cuda.Stream()
+            with torch.cuda.stream(s):
+                for r in range(12):
+                    k = r % 4
+                    a, p = nb.force(dev(ws[k].x_i), dev(ws[k].x_j), dev(ws[k].m_j), ws[k].eps2)
+                    s.synchronize()
+                    if not (np.array_equal(a.cpu().numpy(), alone[k][0]) and np.array_equal(p.cpu().numpy(), alone[k][1])):
+                        errors.append(("device", r, k))
+            nb.release_stream(s)                                       # the stream's workspace goes with it
+        except Exception as exc:                                       # pragma: no cover
+            errors.append(repr(exc))
+
+    threads = [threading.Thread(target=host_worker, args=(0,)), threading.Thread(target=host_worker, args=(2,)),
+               threading.Thread(target=device_worker)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors[:5]
