@@ -159,6 +159,9 @@ __global__ void __launch_bounds__(32 * NW) nb_small_kernel(const SmallArgs a) {
 #else
 #define NB_STAMP(k) do { } while (0)
 #endif
+    // Programmatic dependent launch (nb_small_launch.cu sets the attribute): this grid may be scheduled while the previous
+    // kernel of the stream is still draining; nothing of its output -- nor the ticket counters -- is touched before this wait.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     NB_STAMP(0);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -315,6 +318,7 @@ __global__ void __launch_bounds__(32 * NW) nb_small_kernel(const SmallArgs a) {
     }
 
     NB_STAMP(2);
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");    // the pair loop is done: the next launch may start scheduling
     // a7, level 1: the LJ lanes that hold the same i-particle, in the order lj = 0 .. LJ-1 (every lane forms the same sum)
     if (LJ > 1) {
 #pragma unroll
