@@ -325,11 +325,15 @@ inline cudaError_t pipeline_run(const float* p_xj, const float* p_xi, float* p_f
     if constexpr (pipe_is_packed<P>::value) {
         constexpr int K = PipeK2<P>::value;
         const size_t smem = pipeline_smem2<P>();
-        static std::atomic<bool> configured{false};                    // idempotent: a race only repeats the call
-        if (!configured.load(std::memory_order_acquire)) {
-            cudaError_t ce = cudaFuncSetAttribute(pipeline_kernel2<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        static std::atomic<uint64_t> configured{0};                    // bit d: device d has the raised shared-memory limit
+        int dev = 0;                                                   // (idempotent: a race only repeats the call)
+        cudaError_t ce = cudaGetDevice(&dev);
+        if (ce != cudaSuccess) return ce;
+        const uint64_t bit = 1ull << (dev & 63);
+        if (!(configured.load(std::memory_order_acquire) & bit)) {
+            ce = cudaFuncSetAttribute(pipeline_kernel2<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (ce != cudaSuccess) return ce;
-            configured.store(true, std::memory_order_release);
+            configured.fetch_or(bit, std::memory_order_release);
         }
         const unsigned tiles = (unsigned)((n_i + kPipeThreads * K - 1) / (kPipeThreads * K));
         pipeline_kernel2<P><<<dim3(tiles, (unsigned)S, 1), kPipeThreads, smem, stream>>>(p_xj, p_xi, p_fi, reinterpret_cast<double*>(workspace),
