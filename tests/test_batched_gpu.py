@@ -228,3 +228,28 @@ def test_indexed_entry_is_bitwise_the_expanded_lists(nb):
     torch.cuda.synchronize()
     ra, rp = oracle.force_batched(io2, jo2, xi2, xp[idx2], mp[idx2], 0.01)
     check(a2.cpu().numpy(), p2.cpu().numpy(), ra, rp, "indexed ragged")
+
+
+def test_batched_entries_write_inside_their_bounds_only(nb):
+    """Guard bands around acc_out / pot_out for the three batched entries (compute-sanitizer is closed on this pool)."""
+    import torch
+    w = wl.tree_list_workload(3000, 20, 150, 500, 1500, 1.0 / 128, seed=9)
+    io, jo, xi, xj, mj = (dev(a) for a in (w.i_offsets, w.j_offsets, w.x_i, w.x_j, w.m_j))
+    xm = torch.cat([xj, mj[:, None]], dim=1).contiguous()
+    idx = torch.arange(xm.shape[0], dtype=torch.int32, device="cuda")
+    n_i, pad, sentinel = xi.shape[0], 300, -777.0
+    calls = (lambda a, p: nb.force_batched(io, jo, xi, xj, mj, w.eps2, acc_out=a, pot_out=p),
+             lambda a, p: nb.force_batched_packed(io, jo, xi, xm, w.eps2, acc_out=a, pot_out=p),
+             lambda a, p: nb.force_batched_indexed(io, jo, xi, idx, xm, w.eps2, acc_out=a, pot_out=p))
+    results = []
+    for call in calls:
+        big_a = torch.full((n_i + 2 * pad, 3), sentinel, device="cuda")
+        big_p = torch.full((n_i + 2 * pad,), sentinel, device="cuda")
+        call(big_a[pad:pad + n_i], big_p[pad:pad + n_i])
+        torch.cuda.synchronize()
+        assert torch.all(big_a[:pad] == sentinel) and torch.all(big_a[pad + n_i:] == sentinel)
+        assert torch.all(big_p[:pad] == sentinel) and torch.all(big_p[pad + n_i:] == sentinel)
+        assert not torch.any(big_a[pad:pad + n_i] == sentinel) and not torch.any(big_p[pad:pad + n_i] == sentinel)
+        results.append((big_a[pad:pad + n_i].clone(), big_p[pad:pad + n_i].clone()))
+    for a, p in results[1:]:
+        assert torch.equal(a, results[0][0]) and torch.equal(p, results[0][1])

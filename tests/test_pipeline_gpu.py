@@ -190,3 +190,21 @@ def test_bench_size_in_the_launch_configuration_bench_times(nb, which):
         ej = oracle.error_metrics(p_fi[idx, 3:6], rj)
         assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and e["pot_rms"] <= 1e-5, e
         assert ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-4, ej
+
+
+def test_generalised_kernel_writes_inside_its_bounds_only(nb):
+    """Guard bands around p_fi for the three pipelines on the packed path, ragged sizes (compute-sanitizer is closed here)."""
+    import torch
+    n_i, n_j, pad, sentinel = 2500, 3001, 200, -999.0
+    w = wl.plummer_workload(n_j, 1.0 / 256, seed=43, with_velocities=True)
+    rows = wl.lj_fluid_rows(n_j, 0.8, 0.1, seed=43)
+    e2 = np.full(n_i, w.eps2, np.float32)
+    a3 = rows_a3(w.x_j[:n_i], e2, w.x_j, w.m_j)
+    a4 = rows_a4(w.x_j[:n_i], w.v[:n_i], w.x_j, w.v, w.m_j)
+    for fn, p_xi, p_xj, fdim in ((nb.cunbody_force, a3[0], a3[1], 3), (nb.cunbody_force_jerk_pot, a4[0], a4[1], 7),
+                                 (nb.cunbody_lennard_jones, rows[:n_i], rows, 4)):
+        big = torch.full((n_i + 2 * pad, fdim), sentinel, device="cuda")
+        fn(dev(p_xj), dev(p_xi), big[pad:pad + n_i])
+        torch.cuda.synchronize()
+        assert torch.all(big[:pad] == sentinel) and torch.all(big[pad + n_i:] == sentinel)
+        assert not torch.any(big[pad:pad + n_i] == sentinel) and torch.all(torch.isfinite(big[pad:pad + n_i]))

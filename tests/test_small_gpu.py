@@ -221,3 +221,26 @@ def test_degenerate_positions(nb, nbdebug):
         sel = slice(900, n)                                       # the coincident ones have a ~ 0: compare the others relatively
         check_parity(acc[sel], pot[sel], ref_acc[sel], ref_pot[sel], f"degenerate {plan}")
         assert np.abs(pot[:900] - ref_pot[:900]).max() <= 1e-5 * np.abs(ref_pot[:900]).max()
+
+
+@pytest.mark.parametrize("n_i,n_j", [(1, 1), (33, 777), (513, 4097), (2048, 2048), (512, 65536), (70, 9001)])
+def test_outputs_are_written_inside_their_bounds_only(nb, n_i, n_j, nbdebug):
+    """Guard bands (compute-sanitizer is closed on this pool): acc_out / pot_out are slices of larger buffers filled with a
+    sentinel; the kernel (default plan and mode, with and without phi) must write every element of the slices and nothing
+    around them; the workspace is re-grown from scratch for each shape."""
+    import torch
+    nbdebug.setenv("NB_SMALL", "1")
+    nb.release_workspace()
+    w = wl.plummer_workload(max(n_i, n_j), 1.0 / 64, seed=77)
+    x_j, m_j, x_i = dev(w.x_j[:n_j]), dev(w.m_j[:n_j]), dev(w.x_j[:n_i] if n_i <= n_j else w.x_j[:n_i])
+    pad, sentinel = 257, -12345.0
+    for want_pot in (True, False):
+        big_a = torch.full((n_i + 2 * pad, 3), sentinel, device="cuda")
+        big_p = torch.full((n_i + 2 * pad,), sentinel, device="cuda")
+        acc, pot = big_a[pad:pad + n_i], (big_p[pad:pad + n_i] if want_pot else None)
+        nb.force(x_i, x_j, m_j, w.eps2, acc_out=acc, pot_out=pot, want_pot=want_pot)
+        torch.cuda.synchronize()
+        assert torch.all(big_a[:pad] == sentinel) and torch.all(big_a[pad + n_i:] == sentinel)
+        assert torch.all(big_p[:pad] == sentinel) and torch.all(big_p[pad + n_i:] == sentinel)
+        assert not torch.any(acc == sentinel)
+        assert torch.all(big_p[pad:pad + n_i] != sentinel) if want_pot else torch.all(big_p == sentinel)
