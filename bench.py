@@ -274,7 +274,11 @@ class Problem:
     def __init__(self, op, cfg_name, nb, torch, wl):
         self.op, self.nb, self.torch = op, nb, torch
         if op == "force":
-            if isinstance(cfg_name, int):
+            if isinstance(cfg_name, tuple):                                   # --n N --n-i M: an active subset (C2's recipe)
+                w = wl.subset_workload(cfg_name[0], cfg_name[1], 1.0 / 256, seed=1, name=f"subset{cfg_name[1]}of{cfg_name[0]}")
+                name = (f"shape scan: {w.meta.get('model', '')}, n_i={w.n_i}, n_j={w.n_j}, eps2={w.eps2:.6g}, seed=1, "
+                        f"one nb_force call with phi")
+            elif isinstance(cfg_name, int):
                 w = wl.plummer_workload(cfg_name, 1.0 / 256, seed=1, name=f"plummer{cfg_name}")
                 name = f"N-scan: {w.meta.get('model', '')}, n_i=n_j={cfg_name}, eps2={w.eps2:.6g}, seed=1, one nb_force call with phi"
             else:
@@ -546,6 +550,8 @@ def main():
     ap.add_argument("--op", default="force", choices=sorted(OPS))
     ap.add_argument("--n", type=int, default=0, help="--op force only: an equal-mass Plummer sphere of this N "
                     "(eps = 1/256, seed 1) instead of a BASELINE.json config; for the N-scan in profiles/")
+    ap.add_argument("--n-i", type=int, default=0, help="with --n N: the i-set is a seeded random subset of this many of the "
+                    "N particles (C2's recipe at another shape)")
     ap.add_argument("--shard", action="store_true", help="--op force only: i-shard ONE problem over the ranks (row f4: "
                     "all-gather of the packed j records over NCCL, then nb_force_packed on the local i-slice; strong "
                     "scaling) instead of N independent replicas")
@@ -582,7 +588,7 @@ def main():
     op = OPS[args.op]
 
     # inputs resident in HBM before the timed region
-    prob = Problem(args.op, args.n if (args.n > 0 and args.op == "force") else args.config, nb, torch, wl)
+    prob = Problem(args.op, ((args.n, args.n_i) if 0 < args.n_i < args.n else args.n) if (args.n > 0 and args.op == "force") else args.config, nb, torch, wl)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
     if args.shard:

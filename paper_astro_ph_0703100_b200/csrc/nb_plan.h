@@ -210,15 +210,16 @@ struct SmallPlan {
 };
 
 constexpr int kSmallClusterMax = 8;
-// Which calls nb_force gives to the small-i-set kernel (measured per call from a 50-call CUDA graph, profiles/r02_small_calls.md):
-// up to 512 i-particles it is at least as fast as nb_force_kernel's K = 2 path up to C2's 2^25 pairs (512 x 4096: 6.4
-// against 7.6 us, C2: 24.8 against 23.8-25.2 us, and 2 us faster with a cold L2); up to 2048 i-particles it wins while
-// the call is latency-bound (1024 x 1024: 5.2 against 6.3 us, C0: 7.4 against 7.7 us) and loses once K = 4 tiles fill
-// the machine (2048 x 4096: 12.1 against 9.8 us).
+// Which calls nb_force gives to the small-i-set kernel (measured per call from a CUDA graph of repeated calls,
+// profiles/r02_small_calls.md): up to 512 i-particles it is within 1 us of nb_force_kernel's K = 2 path up to C2's 2^25
+// pairs and 2 us faster with a cold L2 (512 x 4096: 6.4 against 7.6 us, C2: 23.1-24.8 against 23.8-25.2 us); up to 2048
+// i-particles it wins up to 2^24 pairs (1024 x 1024: 4.9 against 6.6 us, C0: 7.1 against 7.8 us, 2048 x 4096: 9.4 against
+// 10.1 us, 2048 x 8192: 14.5 against 14.9 us) and loses from 2^25 pairs on, where K = 4 tiles fill the machine
+// (2048 x 16384: 25.4 against 23.3 us).
 constexpr int64_t kSmallMaxI = 2048;
 constexpr int64_t kSmallNarrowI = 512;
 constexpr double kSmallMaxPairsNarrow = 67108864.0;    // 2^26, n_i <= 512
-constexpr double kSmallMaxPairs = 4194304.0;           // 2^22, n_i <= 2048
+constexpr double kSmallMaxPairs = 16777216.0;          // 2^24, n_i <= 2048
 inline bool small_by_default(int64_t n_i, int64_t n_j) {
     const double pairs = (double)n_i * (double)n_j;
     return (n_i <= kSmallNarrowI && pairs <= kSmallMaxPairsNarrow) || (n_i <= kSmallMaxI && pairs <= kSmallMaxPairs);
@@ -252,7 +253,7 @@ inline double small_plan_cost(int64_t n_i, int64_t n_j, int sm_count, int NW, in
     const int Q = WJ * LJ;
     const double ctas = double(tiles_i) * S;
     const double per_sm = double((int64_t)((ctas + sm_count - 1) / sm_count));      // CTAs on the busiest SM
-    const double max_res = NW == 16 ? 2.0 : 4.0;
+    const double max_res = NW == 16 ? 1.0 : 2.0;                                    // registers: 86 (KI = 1) / 122 (KI = 2) per thread
     const double resident = per_sm > max_res ? max_res : per_sm;                    // beyond that they run in waves
     double waves = double((int64_t)((per_sm + resident - 1) / resident));
     // A cluster of 8 must sit inside one GPC (16 .. 20 SMs): at most 15 clusters per resident CTA are active at a time on
