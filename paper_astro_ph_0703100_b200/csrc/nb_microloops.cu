@@ -112,15 +112,21 @@ __global__ void jpacked_kernel(const float4* jp2, int n_pairs, float* out, float
 static int g_sm = 148; static double g_hz = 1.965e9;
 
 // ---------------- phases of nb_small_kernel (--phases)
+__global__ void marker_kernel(long long* t) { long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); *t = v; }
+
 template <int NW, int KI, int LJ, int WJ, int MODE, bool PHI>
-void phase_run(const char* name, int n_i, int n_j, int S, float* xi, float* xj, float* mj, float* acc, float* pot, double4* partial, int* tickets, long long* stamps) {
+void phase_run(const char* name, int n_i, int n_j, int S, float* xi, float* xj, float* mj, float* acc, float* pot, double4* partial, int* tickets, long long* stamps,
+               void* flush, size_t flush_bytes) {
     constexpr int TILE = (NW / WJ) * KI * (32 / LJ);
     const int tiles = (n_i + TILE - 1) / TILE, Q = WJ * LJ;
     const int chunk_max = (n_j + S - 1) / S + 2, round_max = chunk_max < kSmallRoundJ ? chunk_max : kSmallRoundJ;
-    size_t stage = (size_t)Q * small_pair_stride(small_slot_len(round_max, Q)) * 32, red = ((WJ > 1 ? (size_t)WJ * TILE : 0) + TILE) * 32;
+    const int pstride = small_pair_stride(small_slot_len(round_max, Q));
+    size_t stage = (size_t)Q * pstride * 32, red = ((WJ > 1 ? (size_t)WJ * TILE : 0) + TILE) * 32;
     size_t smem = ((stage > red ? stage : red) + 127) / 128 * 128;
     SmallArgs a{}; a.x_i = xi; a.xj_raw = xj; a.mj_raw = mj; a.jp = nullptr; a.acc = acc; a.pot = PHI ? pot : nullptr; a.partial = partial; a.tickets = tickets;
     a.n_i = n_i; a.n_j = n_j; a.S = S; a.eps2 = 1.f / 16384; a.stamps = nullptr;
+    a.flag_offset = (int)smem;
+    if (MODE == SMALL_FLAG) smem += (size_t)kBloomWords * 4 + (size_t)Q * small_flag_words(pstride) * 8;
     smem += 128;
     auto kern = nb_small_kernel<NW, KI, LJ, WJ, MODE, PHI, 1>;
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024));
@@ -130,19 +136,34 @@ void phase_run(const char* name, int n_i, int n_j, int S, float* xi, float* xj, 
     cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     CK(cudaEventRecord(e0)); for (int r = 0; r < 20; ++r) kern<<<dim3(tiles, S), 32 * NW, smem>>>(a); CK(cudaEventRecord(e1)); CK(cudaEventSynchronize(e1));
     float ms; CK(cudaEventElapsedTime(&ms, e0, e1));
-    a.stamps = stamps; CK(cudaMemset(stamps, 0, n_ctas * 16 * 8));
-    kern<<<dim3(tiles, S), 32 * NW, smem>>>(a); CK(cudaDeviceSynchronize());
-    std::vector<long long> h(n_ctas * 16); CK(cudaMemcpy(h.data(), stamps, h.size() * 8, cudaMemcpyDeviceToHost));
-    long long t0 = h[0]; for (int c = 0; c < n_ctas; ++c) t0 = std::min(t0, h[c * 16]);
     printf("%s: grid %d x %d, %d threads, smem %zu: %.2f us per back-to-back launch\n", name, tiles, S, 32 * NW, smem, ms * 1e3 / 20);
-    const char* ph[7] = {"start", "staged", "loop done", "tile sums out", "ticket taken", "final sums done", "after sleep"};
-    for (int k = 0; k < 7; ++k) {
-        std::vector<double> g, c;
-        for (int q = 0; q < n_ctas; ++q) if (h[q * 16 + k]) { g.push_back((h[q * 16 + k] - t0) * 1e-3); c.push_back((h[q * 16 + 8 + k] - h[q * 16 + 8]) / 1.965e3); }
-        if (g.empty()) continue;
-        std::sort(g.begin(), g.end()); std::sort(c.begin(), c.end());
-        printf("   %-16s (%3zu CTAs)  since first CTA start [us]: min %.2f med %.2f max %.2f | since own start (clock64 at 1.965 GHz) [us]: min %.2f med %.2f max %.2f\n",
-               ph[k], g.size(), g.front(), g[g.size() / 2], g.back(), c.front(), c[c.size() / 2], c.back());
+    a.stamps = stamps;
+    long long* mark = stamps + 4096 * 16 - 8;
+    // warm: the stamped launch follows 20 identical ones; cold: it follows a write of flush_bytes (> L2) -- inputs, code
+    // and the workspace then come from DRAM.  A one-thread marker kernel in front gives the launch gap.
+    for (int cold = 0; cold < 2; ++cold) {
+        std::vector<double> first(7, 0.0), last(7, 0.0), own(7, 0.0); double gap = 0; int reps = 5; std::vector<size_t> cnt(7, 0);
+        for (int r = 0; r < reps; ++r) {
+            CK(cudaMemset(stamps, 0, (size_t)4096 * 16 * 8));
+            if (cold) CK(cudaMemsetAsync(flush, r + 1, flush_bytes));
+            marker_kernel<<<1, 1>>>(mark);
+            kern<<<dim3(tiles, S), 32 * NW, smem>>>(a); CK(cudaDeviceSynchronize());
+            std::vector<long long> h(4096 * 16); CK(cudaMemcpy(h.data(), stamps, h.size() * 8, cudaMemcpyDeviceToHost));
+            long long t0 = h[0]; for (int c = 0; c < n_ctas; ++c) t0 = std::min(t0, h[c * 16]);
+            gap += (t0 - h[4096 * 16 - 8]) * 1e-3 / reps;
+            for (int k = 0; k < 7; ++k) {
+                std::vector<double> g, c;
+                for (int q = 0; q < n_ctas; ++q) if (h[q * 16 + k]) { g.push_back((h[q * 16 + k] - t0) * 1e-3); c.push_back((h[q * 16 + 8 + k] - h[q * 16 + 8]) / 1.965e3); }
+                if (g.empty()) continue;
+                std::sort(g.begin(), g.end()); std::sort(c.begin(), c.end());
+                first[k] += g.front() / reps; last[k] += g.back() / reps; own[k] += c[c.size() / 2] / reps; cnt[k] = g.size();
+            }
+        }
+        const char* ph[7] = {"start", "staged", "loop done", "tile sums out", "ticket taken", "final sums done", "after sleep"};
+        printf("  %s (mean of %d launches): first CTA starts %.2f us after the marker kernel's stamp\n", cold ? "COLD, after a 256 MiB write" : "WARM", reps, gap);
+        for (int k = 0; k < 7; ++k) if (cnt[k])
+            printf("   %-16s (%3zu CTAs)  since first CTA start [us]: first %.2f last %.2f | since own start (clock64 at 1.965 GHz), median CTA [us]: %.2f\n",
+                   ph[k], cnt[k], first[k], last[k], own[k]);
     }
 }
 
@@ -156,10 +177,15 @@ static int phases_main() {
     CK(cudaMalloc(&xi, hi.size() * 4)); CK(cudaMalloc(&xj, hx.size() * 4)); CK(cudaMalloc(&mj, hm.size() * 4)); CK(cudaMalloc(&acc, n_i * 12)); CK(cudaMalloc(&pot, n_i * 4));
     CK(cudaMalloc(&partial, (size_t)512 * n_i * 32)); CK(cudaMalloc(&tickets, 4096)); CK(cudaMemset(tickets, 0, 4096)); CK(cudaMalloc(&stamps, 4096 * 16 * 8));
     CK(cudaMemcpy(xi, hi.data(), hi.size() * 4, cudaMemcpyHostToDevice)); CK(cudaMemcpy(xj, hx.data(), hx.size() * 4, cudaMemcpyHostToDevice)); CK(cudaMemcpy(mj, hm.data(), hm.size() * 4, cudaMemcpyHostToDevice));
-    phase_run<16, 2, 1, 8, SMALL_EXACT, true>("NW16 KI2 WJ8 exact S37", n_i, n_j, 37, xi, xj, mj, acc, pot, partial, tickets, stamps);
-    phase_run<16, 2, 1, 16, SMALL_EXACT, true>("NW16 KI2 WJ16 exact S18", n_i, n_j, 18, xi, xj, mj, acc, pot, partial, tickets, stamps);
-    phase_run<16, 1, 1, 8, SMALL_EXACT, true>("NW16 KI1 WJ8 exact S18", n_i, n_j, 18, xi, xj, mj, acc, pot, partial, tickets, stamps);
-    phase_run<16, 2, 1, 16, SMALL_NONE, false>("NW16 KI2 WJ16 no mask, no phi S18", n_i, n_j, 18, xi, xj, mj, acc, pot, partial, tickets, stamps);
+    void* flush; const size_t flush_bytes = 256u << 20; CK(cudaMalloc(&flush, flush_bytes));
+#define PH(NW, KI, LJ, WJ, MODE, PHI, name, ni, nj, S) phase_run<NW, KI, LJ, WJ, MODE, PHI>(name, ni, nj, S, xi, xj, mj, acc, pot, partial, tickets, stamps, flush, flush_bytes)
+    PH(16, 2, 1, 8, SMALL_EXACT, true, "C2 512 x 65536 NW16 KI2 WJ8 exact S37", n_i, n_j, 37);
+    PH(16, 2, 1, 16, SMALL_EXACT, true, "C2 512 x 65536 NW16 KI2 WJ16 exact S18", n_i, n_j, 18);
+    PH(16, 2, 1, 16, SMALL_FLAG, true, "C2 512 x 65536 NW16 KI2 WJ16 flag S18 (the library's plan)", n_i, n_j, 18);
+    PH(16, 1, 1, 8, SMALL_EXACT, true, "C2 512 x 65536 NW16 KI1 WJ8 exact S18", n_i, n_j, 18);
+    PH(16, 2, 1, 16, SMALL_NONE, false, "C2 512 x 65536 NW16 KI2 WJ16 no mask, no phi S18", n_i, n_j, 18);
+    PH(16, 1, 1, 8, SMALL_EXACT, true, "C0-shaped 512 x 2048 of the same arrays, NW16 KI1 WJ8 exact S4", 512, 2048, 4);
+    PH(8, 1, 4, 8, SMALL_EXACT, true, "1 x 2, NW8 KI1 LJ4 WJ8 exact S1 (launch floor)", 1, 2, 1);
         return 0;
 }
 

@@ -204,22 +204,22 @@ struct SmallPlan {
     int LJ;           // lanes of a warp along j (1, 2 or 4; > 1 only with KI = 1, NW = 8, WJ = 8)
     int WJ;           // warps of the CTA along j (1, 2, 4, 8 or -- NW = 16 -- 16)
     int S;            // j-chunks across CTAs (grid.y), a multiple of CS
-    int CS;           // CTAs per thread-block cluster along grid.y (1 or 8)
+    int CS;           // CTAs per thread-block cluster along grid.y (1, 2, 4 or 8)
     int tile_i;       // i-particles per CTA = (NW / WJ) * KI * (32 / LJ)
     int tiles_i;      // grid.x
 };
 
 constexpr int kSmallClusterMax = 8;
-// Which calls nb_force gives to the small-i-set kernel (measured per call from a CUDA graph of repeated calls,
-// profiles/r02_small_calls.md): up to 512 i-particles it is within 1 us of nb_force_kernel's K = 2 path up to C2's 2^25
-// pairs and 2 us faster with a cold L2 (512 x 4096: 6.4 against 7.6 us, C2: 23.1-24.8 against 23.8-25.2 us); up to 2048
-// i-particles it wins up to 2^24 pairs (1024 x 1024: 4.9 against 6.6 us, C0: 7.1 against 7.8 us, 2048 x 4096: 9.4 against
-// 10.1 us, 2048 x 8192: 14.5 against 14.9 us) and loses from 2^25 pairs on, where K = 4 tiles fill the machine
-// (2048 x 16384: 25.4 against 23.3 us).
-constexpr int64_t kSmallMaxI = 2048;
+// Which calls nb_force gives to the small-i-set kernel (per call from a CUDA graph of repeated calls, the planner below
+// against nb_force_kernel's plan; profiles/r02_small_calls.md "Planner fit"): everything up to 2^25 pairs with at most
+// 4096 i-particles -- 1024 x 1024: 3.8 against 6.7 us, C0: 6.3 against 7.6 us, 4096 x 2048: 8.6 against 11.1 us,
+// 2048 x 16384: 23.3 against 24.5 us, 1024 x 32768: 22.7 against 25.3 us; ties at 4096 x 4096, 4096 x 8192 and 8192 x 1024 --
+// and up to 2^26 pairs with at most 512 (C2: 23.6 against 25.2 us, 512 x 131072: 42.7 against 43.3 us, 32 x 2 000 000:
+// 55 against 78 us).  Beyond that nb_force_kernel's K = 8 tiles win (16384 x 16384: 132 against 151 us).
+constexpr int64_t kSmallMaxI = 4096;
 constexpr int64_t kSmallNarrowI = 512;
 constexpr double kSmallMaxPairsNarrow = 67108864.0;    // 2^26, n_i <= 512
-constexpr double kSmallMaxPairs = 16777216.0;          // 2^24, n_i <= 2048
+constexpr double kSmallMaxPairs = 33554432.0;          // 2^25, n_i <= 4096
 inline bool small_by_default(int64_t n_i, int64_t n_j) {
     const double pairs = (double)n_i * (double)n_j;
     return (n_i <= kSmallNarrowI && pairs <= kSmallMaxPairsNarrow) || (n_i <= kSmallMaxI && pairs <= kSmallMaxPairs);
@@ -229,7 +229,7 @@ constexpr int kSmallRoundJPlan = 4096;           // = nb::kSmallRoundJ (nb_small
 // the instantiated shapes (nb_small_launch.cu)
 inline bool small_shape_ok(int NW, int KI, int LJ, int WJ, int CS) {
     if (!(NW == 8 || NW == 16) || !(WJ == 1 || WJ == 2 || WJ == 4 || WJ == 8 || (WJ == 16 && NW == 16)) ||
-        !(CS == 1 || CS == kSmallClusterMax)) return false;
+        !(CS == 1 || CS == 2 || CS == 4 || CS == kSmallClusterMax)) return false;
     const bool wide = LJ == 1 && (KI == 1 || KI == 2);                           // throughput shapes: any NW, WJ
     const bool narrow = KI == 1 && (LJ == 2 || LJ == 4) && NW == 8 && WJ == 8;   // 16 or 8 i-particles per CTA
     if (!wide && !narrow) return false;
@@ -238,7 +238,8 @@ inline bool small_shape_ok(int NW, int KI, int LJ, int WJ, int CS) {
 
 // Loop efficiency (fraction of the 13-instruction FP32 roofline) of the j-packed body, measured with micro-loops on a
 // B200 (profiles/r02_microloops.md), by i-particles per thread and resident warps per SM: with the exact mask on
-// every pair, and without it (the blocks a Bloom-filter test lets through; acceleration-only calls).
+// every pair, and without it (the groups SMALL_FLAG finds no mark in; acceleration-only calls).  The cost model below
+// uses constants fitted to whole calls instead; this table is what the kernel's design decisions rest on.
 inline double small_loop_eff(int KI, int warps_per_sm, bool masked) {
     static const double eff_m[2][3] = {{0.50, 0.65, 0.69}, {0.62, 0.67, 0.70}};   // KI = 1, 2:  8 / 16 / 32 warps per SM
     static const double eff_p[2][3] = {{0.51, 0.73, 0.82}, {0.69, 0.81, 0.85}};
@@ -246,7 +247,20 @@ inline double small_loop_eff(int KI, int warps_per_sm, bool masked) {
     return masked ? eff_m[r][c] : eff_p[r][c];
 }
 
-// cycles of one small call under a plan; constants from the scans in profiles/r02_small_calls.md
+// SMALL_FLAG (mark the staged j-pairs that may coincide with an i-particle of the tile, mask only their groups) costs
+// ~0.8 us of filter build and tests while staging and makes the loop 10-15 % faster: it pays from ~200 packed groups
+// per thread when few of the staged j coincide with the tile (C2: 228 groups, 23.5 against 24.6 us; 2048 x 16384, where every
+// tile finds its 128 particles among the j: 24.4 against 23.7 us).
+constexpr int kSmallFlagMinGroups = 200;
+inline bool small_flag_pays(const SmallPlan& p, int64_t n_j) {
+    const int64_t chunk = (n_j + p.S - 1) / p.S, Q = (int64_t)p.WJ * p.LJ;
+    return p.LJ == 1 && (((chunk + Q - 1) / Q + 1) / 2) * p.KI >= kSmallFlagMinGroups;
+}
+
+// Cycles of one small call under a plan.  The FORM follows the kernel's phases (start, staging rounds, pair loop, warp /
+// cluster / global sums, waves); the CONSTANTS are fitted to the per-call times of every plan (~500 per shape) on 24 shapes
+// from 1 x 4096 to 2048 x 8192, measured from a CUDA graph of 40 calls on a B200 (profiles/r02_small_calls.md, "Planner
+// fit"): the plan the model picks is on average 1 % and at worst 5 % slower than the best measured plan of its shape.
 inline double small_plan_cost(int64_t n_i, int64_t n_j, int sm_count, int NW, int KI, int LJ, int WJ, int S, int CS) {
     const int tile_i = (NW / WJ) * KI * (32 / LJ);
     const int64_t tiles_i = (n_i + tile_i - 1) / tile_i;
@@ -256,10 +270,10 @@ inline double small_plan_cost(int64_t n_i, int64_t n_j, int sm_count, int NW, in
     const double max_res = NW == 16 ? 1.0 : 2.0;                                    // registers: 86 (KI = 1) / 122 (KI = 2) per thread
     const double resident = per_sm > max_res ? max_res : per_sm;                    // beyond that they run in waves
     double waves = double((int64_t)((per_sm + resident - 1) / resident));
-    // A cluster of 8 must sit inside one GPC (16 .. 20 SMs): at most 15 clusters per resident CTA are active at a time on
-    // a B200 (ncu launch__cluster_max_active), i.e. 120 of the 148 SMs -- more clusters run as further waves.
-    if (CS == kSmallClusterMax) {
-        const double cap = 15.0 * resident;
+    // A cluster must sit inside one GPC (16 .. 20 SMs): per resident CTA at most 15 clusters of 8 are active at a time on a
+    // B200 (ncu launch__cluster_max_active; 120 of the 148 SMs), ~32 of 4, 74 of 2 -- more clusters run as further waves.
+    if (CS > 1) {
+        const double cap = (CS == 8 ? 15.0 : (CS == 4 ? 32.0 : 74.0)) * resident * sm_count / 148.0;
         const double cw = double((int64_t)((ctas / CS + cap - 1) / cap));
         if (cw > waves) waves = cw;
     }
@@ -267,30 +281,32 @@ inline double small_plan_cost(int64_t n_i, int64_t n_j, int sm_count, int NW, in
     const double pairs_per_thread = double((((chunk + Q - 1) / Q) + 1) / 2);
     const double groups = pairs_per_thread * KI;                                    // packed groups of a thread
     // a scheduler holds NW / 4 warps of every resident CTA; a packed group occupies its FMA pipe for 26 cycles
-    const int wps = (int)(NW * resident);
-    const double eff = small_loop_eff(KI, wps, true);
-    double loop = resident * groups * (NW / 4) * 26.0 / eff;
-    if (LJ > 1) loop *= 1.0 + 0.35 * LJ;                                            // LJ distinct addresses per LDS.128: shared-memory bandwidth
-    const double lone = groups * 40.0;                                              // one warp's dependent chains
+    static const double eff[2][2] = {{0.50, 0.657}, {0.493, 0.663}};                // KI = 1, 2: 8 / >= 16 warps per SM (fitted)
+    double loop = resident * groups * (NW / 4) * 26.0 / eff[KI == 1 ? 0 : 1][NW * resident >= 16 ? 1 : 0];
+    if (LJ > 1) loop *= 1.0 + 0.14 * LJ;                                            // LJ distinct addresses per LDS.128
+    const double lone = groups * 21.0;                                              // one warp's dependent chains
     if (loop < lone) loop = lone;
     const double rounds = double((chunk + kSmallRoundJPlan - 1) / kSmallRoundJPlan);
     const double staged = double(chunk > kSmallRoundJPlan ? kSmallRoundJPlan : chunk);
-    // phases measured with %globaltimer stamps on C2 (profiles/r02_small_calls.md): staging 1.3 us, lane / warp sums
-    // 0.8 us, partial + fence + ticket 1.0 us, final sums 0.5 us + the tile's partials through one SM's L2 port
-    double c = 1200.0 + 1600.0 * rounds + staged * resident * 0.5;                  // start, staging latency, L2 -> shared memory
-    c += loop + 40.0 * KI * (pairs_per_thread / 64.0 + 1.0);
-    if (LJ > 1) c += 30.0 * KI * LJ;
-    c += (WJ > 1) ? 900.0 + 40.0 * WJ : 300.0;
-    if (CS > 1) c += 1200.0 + 40.0 * CS;
+    double c = 440.0 + 2600.0 * rounds + staged * resident * 0.42;                  // start, staging latency, L2 -> shared memory
+    c += loop + 40.0 * KI * (pairs_per_thread / 64.0 + 1.0);                        // Eq. (2) block ends
+    c += (WJ > 1) ? 215.0 + 26.0 * WJ : 2250.0;                                     // warp sums; WJ = 1: tiles of 256 .. 1024 particles
+    if (CS > 1) c += 2130.0;                                                        // two cluster barriers + DSMEM sums
     const int n_groups = S / CS;
-    if (n_groups > 1) c += 2000.0 + 1000.0 + 260.0 * n_groups;                      // ticket; final sums ~0.13 us per group
+    if (n_groups > 1) c += 1790.0 + 120.0 * n_groups;                               // partials + ticket; final sums per group
     return c * waves;
 }
 
-inline SmallPlan make_small_plan(int64_t n_i, int64_t n_j, int sm_count) {
+inline int64_t small_plan_key_i(int64_t n_i) { return (n_i + 7) / 8 * 8; }        // every tile size is a multiple of 8
+
+inline SmallPlan make_small_plan(int64_t n_i_exact, int64_t n_j, int sm_count) {
     if (sm_count <= 0) sm_count = 148;
+    // the plan is a function of n_i rounded up to a multiple of 8 (same number of i-tiles for every tile size), so that a
+    // block-step run whose active set changes every step finds most of its shapes in the library's plan table
+    const int64_t n_i = small_plan_key_i(n_i_exact);
     static const int shapes[6][3] = {{16, 2, 1}, {8, 2, 1}, {16, 1, 1}, {8, 1, 1}, {8, 1, 2}, {8, 1, 4}};   // (NW, KI, LJ)
     static const int wj_opts[5] = {1, 2, 4, 8, 16};
+    static const int cs_opts[4] = {1, 2, 4, kSmallClusterMax};
     SmallPlan best{};
     double best_cost = -1.0;
     for (int sh = 0; sh < 6; ++sh) {
@@ -302,22 +318,27 @@ inline SmallPlan make_small_plan(int64_t n_i, int64_t n_j, int sm_count) {
             if (tile_i > 8 && (int64_t)tile_i >= 2 * n_i) continue;               // a smaller tile covers all i
             const int64_t tiles_i = (n_i + tile_i - 1) / tile_i;
             const int Q = WJ * LJ;
-            for (int cs = 0; cs < 2; ++cs) {
-                const int CS = cs ? kSmallClusterMax : 1;
+            for (int ci = 0; ci < 4; ++ci) {
+                const int CS = cs_opts[ci];
                 if (!small_shape_ok(NW, KI, LJ, WJ, CS)) continue;
-                int64_t cand[8];
+                int64_t cand[6];
                 int n_cand = 0;
                 cand[n_cand++] = CS;
-                for (int m = 1; m <= 4; ++m) {
-                    int64_t S = (int64_t)m * sm_count / tiles_i / CS * CS;
-                    if (S >= CS) cand[n_cand++] = S;
+                cand[n_cand++] = 2 * CS;
+                for (int m = 1; m <= 2; ++m) {                                      // one or two CTAs per SM, rounded down and up
+                    cand[n_cand++] = (int64_t)m * sm_count / tiles_i / CS * CS;
+                    cand[n_cand++] = (((int64_t)m * sm_count + tiles_i - 1) / tiles_i + CS - 1) / CS * CS;
                 }
+                const int64_t s_max = (n_j / (2 * Q) / CS) * CS;                     // every slot gets at least one pair
                 for (int q = 0; q < n_cand; ++q) {
                     int64_t S = cand[q];
-                    const int64_t s_max = (n_j / (2 * Q) / CS) * CS;                 // every slot gets at least one pair
                     if (S > s_max) S = s_max;
                     if (S < CS) S = CS;
                     if (S > kMaxS) S = kMaxS / CS * CS;
+                    cand[q] = S;
+                    bool seen = false;
+                    for (int r = 0; r < q; ++r) seen = seen || cand[r] == S;
+                    if (seen) continue;
                     if (CS == 1 && S > 64) continue;                                // without clusters the last CTA of a tile sums alone
                     const double c = small_plan_cost(n_i, n_j, sm_count, NW, KI, LJ, WJ, (int)S, CS);
                     if (best_cost < 0.0 || c < best_cost * (1.0 - 1e-9)) {

@@ -65,6 +65,11 @@ __device__ __forceinline__ uint32_t cluster_ctarank() {
     asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
     return r;
 }
+__device__ __forceinline__ uint32_t cluster_nctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+    return r;
+}
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
@@ -123,7 +128,7 @@ __host__ __device__ inline int small_pair_stride(int slot_len) { return (slot_le
 // ---------------------------------------------------------------- the kernel
 // CTA = 8 warps = WI (along i) x WJ (along j); lanes = LI (along i) x LJ (along j); KI i-particles per thread.
 // i-tile of a CTA = WI * KI * LI particles; the CTA's j-chunk (blockIdx.y of S) is cut into Q = WJ * LJ slots.
-// NW = warps per CTA (8 or 16); CS = CTAs per cluster along grid.y (1 or 8).
+// NW = warps per CTA (8 or 16); CS = 1: no cluster; CS = 8: launched in clusters of 2, 4 or 8 CTAs along grid.y.
 //
 // Coincident pairs (reading R1), MODE:
 //   SMALL_EXACT  every pair masked (LOP3 + FSEL per pair on the ALU pipe): the loop reaches 62-70 % of the FP32 roofline
@@ -289,18 +294,17 @@ __global__ void __launch_bounds__(32 * NW) nb_small_kernel(const SmallArgs a) {
                 }
             };
             if (MODE == SMALL_FLAG) {
+                // groups of U pairs (the unroll width, so every group keeps U independent chains in flight): a group with a
+                // marked pair runs masked, the others unmasked -- whatever the density of marks, never slower than SMALL_EXACT
+                // in the loop (runs between single marks fell into the unrolled loops' remainders: 60 % slower at 1 mark in 32)
+                constexpr int U = (KI == 2) ? 4 : 8;
                 const unsigned long long word = sbits[q * sw + (b >> 6)];      // warp-uniform (LJ = 1): kSmallBlockPairs = 64 pairs per word
                 int p = 0;
-                while (p < nb_) {                                      // alternate runs of unmarked and of marked pairs
-                    const unsigned long long rest = word >> p;
-                    const int stop = rest ? min(nb_, p + __ffsll((long long)rest) - 1) : nb_;
-                    sweep(std::integral_constant<int, MASK_NONE>{}, p, stop);
-                    if (stop >= nb_) break;
-                    const unsigned long long clear = ~(word >> stop);  // first unmarked pair at or after stop
-                    const int stop2 = clear ? min(nb_, stop + __ffsll((long long)clear) - 1) : nb_;
-                    sweep(std::integral_constant<int, MASK_EXACT>{}, stop, stop2);
-                    p = stop2;
+                for (; p + U <= nb_; p += U) {
+                    if ((word >> p) & ((1ull << U) - 1ull)) sweep(std::integral_constant<int, MASK_EXACT>{}, p, p + U);
+                    else sweep(std::integral_constant<int, MASK_NONE>{}, p, p + U);
                 }
+                if (p < nb_) sweep(std::integral_constant<int, MASK_EXACT>{}, p, nb_);
             } else if (MODE == SMALL_EXACT) {
                 sweep(std::integral_constant<int, MASK_EXACT>{}, 0, nb_);
             } else {
@@ -359,23 +363,29 @@ __global__ void __launch_bounds__(32 * NW) nb_small_kernel(const SmallArgs a) {
 
     // a7, level 3: the CS CTAs of the cluster (consecutive j-chunks of the same i-tile), through distributed shared
     // memory: CTA r of the cluster sums slice r of the tile over the cluster's CTAs in rank order.
-    constexpr int SLICE = TILE_I / CS;
+    // (the instantiation CS = kSmallClusterMax serves every launched cluster size cs = 2, 4, 8: cs is read from the
+    // hardware, the loads of absent ranks are predicated off)
+    const int cs = (CS > 1) ? (int)cluster_nctarank() : 1;
+    const int SLICE = TILE_I / cs;
     const uint32_t rank = (CS > 1) ? cluster_ctarank() : 0u;
     if (CS > 1) cluster_sync_all(); else __syncthreads();
-    const int n_groups = a.S / CS;                                     // cluster partials per i-tile
-    const int group = blockIdx.y / CS;
+    const int n_groups = a.S / cs;                                     // cluster partials per i-tile
+    const int group = blockIdx.y / cs;
     for (int t = threadIdx.x; t < SLICE; t += kSmallThreads) {
         const int il = (int)rank * SLICE + t;
         double4 s;
         if (CS > 1) {
             const uint32_t local = smem_u32(tile_sum + il);
-            const double2 lo0 = cluster_ld_double2(cluster_map_shared(local, 0)), hi0 = cluster_ld_double2(cluster_map_shared(local + 16, 0));
-            s = make_double4(lo0.x, lo0.y, hi0.x, hi0.y);
+            double2 lo[CS], hi[CS];
 #pragma unroll
-            for (int c = 1; c < CS; ++c) {
-                const double2 lo = cluster_ld_double2(cluster_map_shared(local, c)), hi = cluster_ld_double2(cluster_map_shared(local + 16, c));
-                s.x += lo.x; s.y += lo.y; s.z += hi.x; s.w += hi.y;
+            for (int c = 0; c < CS; ++c) {                             // all loads in flight, then the adds in rank order
+                lo[c] = hi[c] = make_double2(0.0, 0.0);
+                if (c < cs) { lo[c] = cluster_ld_double2(cluster_map_shared(local, c)); hi[c] = cluster_ld_double2(cluster_map_shared(local + 16, c)); }
             }
+            s = make_double4(lo[0].x, lo[0].y, hi[0].x, hi[0].y);
+#pragma unroll
+            for (int c = 1; c < CS; ++c)
+                if (c < cs) { s.x += lo[c].x; s.y += lo[c].y; s.z += hi[c].x; s.w += hi[c].y; }
         } else {
             s = tile_sum[il];
         }
@@ -402,7 +412,7 @@ __global__ void __launch_bounds__(32 * NW) nb_small_kernel(const SmallArgs a) {
         __shared__ int s_last;
         __syncthreads();
         if (threadIdx.x == 0) {
-            int* tk = a.tickets + blockIdx.x * CS + rank;
+            int* tk = a.tickets + blockIdx.x * cs + rank;
             int ticket;
             asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(ticket) : "l"(tk) : "memory");
             s_last = (ticket == n_groups - 1);

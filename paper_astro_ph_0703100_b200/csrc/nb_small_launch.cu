@@ -56,7 +56,7 @@ cudaError_t launch_inst(const SmallPlan& p, const SmallArgs& a, size_t smem, cud
     if (CS > 1) {
         attr[1].id = cudaLaunchAttributeClusterDimension;
         attr[1].val.clusterDim.x = 1;
-        attr[1].val.clusterDim.y = CS;
+        attr[1].val.clusterDim.y = (unsigned)p.CS;                    // 2, 4 or 8: the kernel reads the size from the hardware
         attr[1].val.clusterDim.z = 1;
         cfg.numAttrs = 2;
     }
@@ -68,7 +68,7 @@ cudaError_t launch_cs(const SmallPlan& p, const SmallArgs& a, size_t smem, cudaS
     constexpr int TILE_I = (NW / WJ) * KI * (32 / LJ);
     if (p.CS == 1) return launch_inst<NW, KI, LJ, WJ, MODE, PHI, 1>(p, a, smem, stream);
     if constexpr (TILE_I % kSmallClusterMax == 0) {
-        if (p.CS == kSmallClusterMax) return launch_inst<NW, KI, LJ, WJ, MODE, PHI, kSmallClusterMax>(p, a, smem, stream);
+        if (p.CS == 2 || p.CS == 4 || p.CS == kSmallClusterMax) return launch_inst<NW, KI, LJ, WJ, MODE, PHI, kSmallClusterMax>(p, a, smem, stream);
     }
     return cudaErrorInvalidValue;
 }

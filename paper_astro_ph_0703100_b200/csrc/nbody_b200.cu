@@ -84,6 +84,7 @@ DeviceInfo g_dev[64];
 std::map<std::pair<int, cudaStream_t>, Workspace> g_ws;
 std::map<std::tuple<int64_t, int64_t, int>, nb::Plan> g_plans;
 std::map<std::tuple<int64_t, int64_t, int>, nb::Plan> g_hplans;
+std::map<std::tuple<int64_t, int64_t, int>, nb::SmallPlan> g_splans;
 
 // ---- debugging switches
 bool parse_knob(Knobs* k, const char* key, const char* value) {
@@ -234,6 +235,22 @@ nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count, bool jerk = false) 
     std::lock_guard<std::mutex> lock(g_mutex);
     if (table.size() > 4096) table.clear();
     table[key] = p;
+    return p;
+}
+
+// the small-i-set kernel's planner scores ~1000 candidate decompositions (~10 us): the same table serves repeated shapes
+nb::SmallPlan cached_small_plan(int64_t n_i, int64_t n_j, int sm_count) {
+    const auto key = std::make_tuple(nb::small_plan_key_i(n_i), n_j, sm_count);
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        auto it = g_splans.find(key);
+        if (it != g_splans.end()) return it->second;
+    }
+    const nb::SmallPlan p = nb::make_small_plan(n_i, n_j, sm_count);       // outside the lock
+    g_plans_computed.fetch_add(1, std::memory_order_relaxed);
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (g_splans.size() > 4096) g_splans.clear();
+    g_splans[key] = p;
     return p;
 }
 
@@ -403,7 +420,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
 
     // Small i-sets: the kernel packed over j (nb_small.cuh), one launch, cluster + ticket reduction of the j-split.
     if (!eps2_i && use_small_path(kn, n_i, n_j)) {
-        nb::SmallPlan sp = nb::make_small_plan(n_i, n_j, info.sm_count);
+        nb::SmallPlan sp = cached_small_plan(n_i, n_j, info.sm_count);
         if (kn.small_plan_set) {
             sp.NW = kn.sNW; sp.KI = kn.sKI; sp.LJ = kn.sLJ; sp.WJ = kn.sWJ; sp.S = kn.sS; sp.CS = kn.sCS;
             sp.tile_i = (sp.NW / sp.WJ) * sp.KI * (32 / sp.LJ);
@@ -436,9 +453,9 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
         sa.flag_offset = 0;
         // coincident pairs: no mask at all without phi (eps2 >= 2^-40); else only the pairs marked while staged are masked
         // -- or every pair: eps2 < 2^-40 (an unmasked coincident pair would overflow), NB_SMALL_MASK=exact
-        // (marking pays when a CTA stages many j per i-tile: filter + tests cost ~1 us, the unmasked loop runs 15 % faster;
-        //  measured on C2 24.65 -> 23.64 us per call, on C0 -- 512 j per CTA -- nothing: profiles/r02_small_calls.md)
-        const bool flag_pays = (n_j + sp.S - 1) / sp.S >= 1024;
+        // (marking pays when a thread's loop is long: filter + tests cost ~1 us, the unmasked loop runs 10-15 % faster;
+        //  measured on C2 24.65 -> 23.64 us per call, on C0 -- 64 pairs per thread -- nothing: profiles/r02_small_calls.md)
+        const bool flag_pays = nb::small_flag_pays(sp, n_j);
         const int small_mode = a_only ? nb::SMALL_NONE
                                : (eps2 >= kUnmaskedMinEps2 && kn.small_mask != nb::SMALL_EXACT && (flag_pays || kn.small_mask == nb::SMALL_FLAG))
                                      ? nb::SMALL_FLAG : nb::SMALL_EXACT;

@@ -163,7 +163,9 @@ def test_fast_planner_is_the_exhaustive_search_and_costs_microseconds():
             best = min(best, (time.perf_counter() - t0) / len(shapes))
         return best
     per_call, per_small = per_shape(lib.nb_plan_query), per_shape(lib.nb_plan_query_small)
-    assert per_call < 8e-6 and per_small < 10e-6, (per_call, per_small)     # ~3-5 us + ~0.5 us of ctypes
+    # ~3-5 us + ~0.5 us of ctypes; the small-i-set planner scores ~600 decompositions (~10 us), and its table is keyed by
+    # n_i rounded up to a multiple of 8
+    assert per_call < 8e-6 and per_small < 20e-6, (per_call, per_small)
 
 
 def test_small_planner_invariants():
@@ -172,8 +174,10 @@ def test_small_planner_invariants():
         assert (p["KI"], p["LJ"]) in ((2, 1), (1, 1), (1, 2), (1, 4)) and p["WJ"] in (1, 2, 4, 8, 16) and p["NW"] in (8, 16) and p["WJ"] <= p["NW"]
         assert p["tile_i"] == (p["NW"] // p["WJ"]) * p["KI"] * (32 // p["LJ"])
         assert p["tiles_i"] * p["tile_i"] >= n_i > (p["tiles_i"] - 1) * p["tile_i"]
-        assert p["CS"] in (1, 8) and p["S"] % p["CS"] == 0 and p["tile_i"] % p["CS"] == 0 and 1 <= p["S"] <= 2048
+        assert p["CS"] in (1, 2, 4, 8) and p["S"] % p["CS"] == 0 and p["tile_i"] % p["CS"] == 0 and 1 <= p["S"] <= 2048
         assert p == nb.plan_query_small(n_i, n_j, 148)
+        q = nb.plan_query_small((n_i + 7) // 8 * 8, n_j, 148)               # the plan depends on n_i through ceil(n_i / 8) only
+        assert {k: v for k, v in p.items() if k != "default"} == {k: v for k, v in q.items() if k != "default"}
 
 
 def test_debug_switches_parse_and_reject():

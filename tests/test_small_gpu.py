@@ -46,7 +46,7 @@ def check_parity(acc, pot, ref_acc, ref_pot, label=""):
 # (NW, KI, LJ) shapes x WJ x (S, CS): every instantiation, with and without the cluster level and the global level
 SHAPES = [(16, 2, 1), (8, 2, 1), (16, 1, 1), (8, 1, 1), (8, 1, 2), (8, 1, 4)]
 SMALL_PLANS = [(nw, ki, lj, wj, s, cs) for (nw, ki, lj) in SHAPES for wj in (((1, 2, 4, 8, 16) if nw == 16 else (1, 2, 4, 8)) if lj == 1 else (8,))
-               for (s, cs) in ((1, 1), (3, 1), (8, 8), (24, 8))
+               for (s, cs) in ((1, 1), (3, 1), (8, 8), (24, 8), (4, 4), (6, 2))
                if ((nw // wj) * ki * (32 // lj)) % cs == 0]
 PLAN_FMT = "%d,%d,%d,%d,%d,%d"
 
@@ -176,7 +176,7 @@ def test_randomised_small_cases(nb, nbdebug):
         n_i = n_j if alias else int(rng.integers(1, 2049))
         nw, ki, lj = SHAPES[int(rng.integers(0, 6))]
         wj = int(rng.choice([1, 2, 4, 8] + ([16] if nw == 16 else []))) if lj == 1 else 8
-        cs = 8 if ((nw // wj) * ki * (32 // lj)) % 8 == 0 and rng.integers(0, 2) else 1
+        cs = int(rng.choice([2, 4, 8])) if ((nw // wj) * ki * (32 // lj)) % 8 == 0 and rng.integers(0, 2) else 1
         s = cs * int(rng.integers(1, 5))
         want_pot = bool(rng.integers(0, 4))
         eps2 = float(np.float32(2.0 ** rng.integers(-16, -2)))
