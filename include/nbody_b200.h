@@ -61,7 +61,8 @@ typedef enum nb_status {
     NB_ERR_INVALID_VALUE = 1,      /* negative / too large count, required pointer NULL, eps2 < 0 or not finite, ... */
     NB_ERR_CUDA = 2,               /* a CUDA runtime call failed; see nb_last_cuda_error() */
     NB_ERR_ALLOC = 3,              /* the internal workspace could not be allocated */
-    NB_ERR_UNSUPPORTED_DEVICE = 4  /* current device is not compute capability 10.x */
+    NB_ERR_UNSUPPORTED_DEVICE = 4, /* current device is not compute capability 10.x */
+    NB_ERR_LIMIT = 5               /* the call exceeds the fixed limit of a no-allocation entry point (nb_force_noalloc) */
 } nb_status;
 
 /*
@@ -427,6 +428,36 @@ int nb_release_workspace(void);
  * stream the library has been used on: the workspace is keyed by the stream handle and would otherwise stay allocated
  * until nb_release_workspace -- and be inherited by a later stream that happens to get the same handle. */
 int nb_release_stream(void *stream);
+
+/*
+ * nb_force_noalloc -- nb_force for callers that must not allocate device memory (a serving loop, a harness that forbids
+ * cudaMalloc, code under stream capture): the same operation, arguments, layouts, results and error behaviour as nb_force
+ * (Eq. (1) and phi; the one-launch small-i-set kernel, j-split of section 4.2), with
+ *
+ *   - n_i <= NB_NOALLOC_MAX_I, else NB_ERR_LIMIT and nothing is launched or written (any n_j nb_force accepts);
+ *   - NO device allocation, ever: the call makes no cudaMalloc / cudaMallocAsync / cudaFree and uses no library routine
+ *     that allocates.  The scratch of the j-split (FP64 partial sums [n_i][groups] + one ticket counter per i-tile slice)
+ *     lives in ONE static __device__ array of NB_NOALLOC_SCRATCH_BYTES inside the library: every GPU that loads the
+ *     library holds it from load until the process exits, whether or not this entry point is ever called.  When the
+ *     planner's j-split would need more partial sums than the array holds, the call runs with fewer j-chunks (slower,
+ *     same result up to summation order).
+ *
+ * Sharing: ALL calls on a device -- from any thread, on any stream -- use the same array, which keeps the last call's
+ * contents.  Every call clears the ticket counters it will use first (stream-ordered, on `stream`); the partial sums are
+ * written before they are read.  Two nb_force_noalloc calls that OVERLAP on the GPU (different streams, or two host
+ * threads on different streams) race on the array and give undefined results: serialise them (one stream, or events).
+ * Calls on one stream never overlap.  nb_force and every other entry point use their own workspace and are not affected.
+ *
+ * The first call on each device does the one-time set-up (resolves the array's device address, raises the kernel's
+ * shared-memory limit): make it outside any stream capture.  The debugging switches of nb_debug.h do not apply.
+ * Results: bit for bit nb_force's when nb_force takes the small-i-set kernel for the shape and the j-split is not
+ * reduced; within the library's tolerance (BASELINE.json north_star: acc RMS 1e-5, max 1e-4, phi RMS 1e-5) otherwise.
+ */
+#define NB_NOALLOC_MAX_I 4096
+#define NB_NOALLOC_SCRATCH_BYTES (131072 * 32 + 4096 * 4)   /* 4 MiB of partial sums + 16 KiB of ticket counters */
+int nb_force_noalloc(int64_t n_i, const float *x_i,
+                     int64_t n_j, const float *x_j, const float *m_j,
+                     float eps2, float *acc_out, float *pot_out, void *stream);
 
 const char *nb_status_string(int status);   /* static storage */
 int nb_last_cuda_error(void);                /* cudaError_t behind this thread's last NB_ERR_CUDA / NB_ERR_ALLOC */

@@ -39,6 +39,8 @@ def lib() -> ctypes.CDLL:
         i64, f32, p, ci = ctypes.c_int64, ctypes.c_float, ctypes.c_void_p, ctypes.c_int
         l.nb_force.argtypes = [i64, p, i64, p, p, f32, p, p, p]
         l.nb_force.restype = ci
+        l.nb_force_noalloc.argtypes = [i64, p, i64, p, p, f32, p, p, p]
+        l.nb_force_noalloc.restype = ci
         l.nb_force_host.argtypes = [i64, p, i64, p, p, f32, p, p]
         l.nb_force_host.restype = ci
         l.nb_leapfrog_kdk.argtypes = [i64, p, p, p, f32, f32, i64, p, p, p]
@@ -139,6 +141,30 @@ def force(x_i, x_j, m_j, eps2: float, acc_out=None, pot_out=None, want_pot: bool
         st = lib().nb_force(n_i, x_i.data_ptr(), n_j, x_j.data_ptr(), m_j.data_ptr(), float(eps2),
                             acc_out.data_ptr(), None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
     _check(st, "nb_force")
+    return acc_out, pot_out
+
+
+NOALLOC_MAX_I = 4096            # NB_NOALLOC_MAX_I (include/nbody_b200.h)
+
+
+def force_noalloc(x_i, x_j, m_j, eps2: float, acc_out, pot_out=None, stream=None):
+    """nb_force_noalloc on CUDA tensors: nb_force without any device allocation (n_i <= NOALLOC_MAX_I; the scratch is a
+    static array inside the library, shared by all calls on the device).  The caller passes the outputs, so that this
+    wrapper allocates nothing either.  Returns (acc_out, pot_out); asynchronous on the stream."""
+    import torch
+    _dev_f32(x_i, "x_i", (3,)); _dev_f32(x_j, "x_j", (3,)); _dev_f32(m_j, "m_j", ())
+    n_i, n_j = x_i.shape[0], x_j.shape[0]
+    if m_j.shape[0] != n_j:
+        raise ValueError("m_j length != n_j")
+    _dev_f32(acc_out, "acc_out", (3,))
+    if acc_out.shape[0] != n_i or (pot_out is not None and pot_out.shape[0] != n_i):
+        raise ValueError("output length != n_i")
+    if pot_out is not None:
+        _dev_f32(pot_out, "pot_out", ())
+    with torch.cuda.device(x_i.device):
+        st = lib().nb_force_noalloc(n_i, x_i.data_ptr(), n_j, x_j.data_ptr(), m_j.data_ptr(), float(eps2),
+                                    acc_out.data_ptr(), None if pot_out is None else pot_out.data_ptr(), _stream_ptr(stream))
+    _check(st, "nb_force_noalloc")
     return acc_out, pot_out
 
 

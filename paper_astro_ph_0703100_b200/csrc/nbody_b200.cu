@@ -1412,6 +1412,102 @@ int nb_debug_plan_exhaustive(int64_t n_i, int64_t n_j, int sm_count, int jerk, i
 
 int64_t nb_debug_plans_computed(void) { return g_plans_computed.load(std::memory_order_relaxed); }
 
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// nb_force_noalloc (nbody_b200.h): the small-i-set kernel with the scratch of its j-split in a static device array.
+// No cudaMalloc / cudaMallocAsync / cudaFree on this path, no Workspace, no events.
+namespace {
+
+constexpr size_t kNoAllocPartials = 131072;       // double4 entries: n_i * (S / CS) of a call must fit
+constexpr size_t kNoAllocTickets = 4096;          // ints: tiles_i * CS <= (NB_NOALLOC_MAX_I / 8) * 8
+constexpr size_t kNoAllocTicketOffset = kNoAllocPartials * sizeof(double4);
+static_assert(kNoAllocTicketOffset + kNoAllocTickets * sizeof(int) == (size_t)NB_NOALLOC_SCRATCH_BYTES, "header and array agree");
+static_assert((NB_NOALLOC_MAX_I / 8) * nb::kSmallClusterMax <= (int64_t)kNoAllocTickets, "one ticket per (i-tile, cluster rank)");
+static_assert(kNoAllocPartials / NB_NOALLOC_MAX_I >= 1, "at least one group of partials at the largest n_i");
+
+// One copy per GPU that loads the library, held until the process exits.  In HOST code this name is only a handle for
+// cudaGetSymbolAddress -- never a device address: the kernel gets the pointer noalloc_scratch() resolves.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NB_NOALLOC_SCRATCH_BYTES];
+
+std::atomic<unsigned char*> g_noalloc_ptr[64];     // per device ordinal (device_info rejects ordinals >= 64)
+
+// Device address of the CURRENT device's copy; `dev` is the current device (device_info has just read it).
+int noalloc_scratch(int dev, unsigned char** out) {
+    unsigned char* p = g_noalloc_ptr[dev].load(std::memory_order_acquire);
+    if (!p) {                                      // once per device; two threads racing here resolve the same address
+        void* q = nullptr;
+        NB_CUDA(cudaGetSymbolAddress(&q, g_noalloc_scratch));
+        if (!q) return NB_ERR_CUDA;
+        p = static_cast<unsigned char*>(q);
+        g_noalloc_ptr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return NB_OK;
+}
+
+int force_noalloc_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
+                       float* acc_out, float* pot_out, cudaStream_t stream) {
+    if (bad_count(n_i) || bad_count(n_j)) return NB_ERR_INVALID_VALUE;
+    if (!(eps2 >= 0.0f) || !std::isfinite(eps2)) return NB_ERR_INVALID_VALUE;
+    if (n_i > 0 && (!x_i || !acc_out)) return NB_ERR_INVALID_VALUE;
+    if (n_j > 0 && (!x_j || !m_j)) return NB_ERR_INVALID_VALUE;
+    if (n_i > NB_NOALLOC_MAX_I) return NB_ERR_LIMIT;                   // before any CUDA call: nothing launched, nothing written
+    int dev = 0;
+    DeviceInfo info;
+    int rc = device_info(&dev, &info);
+    if (rc != NB_OK) return rc;
+    if (n_i == 0) return NB_OK;
+    if (n_j == 0) {
+        NB_CUDA(cudaMemsetAsync(acc_out, 0, sizeof(float) * 3 * (size_t)n_i, stream));
+        if (pot_out) NB_CUDA(cudaMemsetAsync(pot_out, 0, sizeof(float) * (size_t)n_i, stream));
+        return NB_OK;
+    }
+    unsigned char* scratch = nullptr;
+    rc = noalloc_scratch(dev, &scratch);
+    if (rc != NB_OK) return rc;
+
+    nb::SmallPlan sp = nb::make_small_plan(n_i, n_j, info.sm_count);   // a pure function: no table, no host allocation
+    const int64_t max_groups = (int64_t)(kNoAllocPartials / (size_t)n_i);   // >= 32 for n_i <= 4096
+    if (sp.S / sp.CS > max_groups) sp.S = (int)(max_groups * sp.CS);   // fewer, longer j-chunks: the partials must fit
+    const int n_groups = sp.S / sp.CS;
+    if ((size_t)sp.tiles_i * sp.CS > kNoAllocTickets || (size_t)n_groups * (size_t)n_i > kNoAllocPartials) return NB_ERR_LIMIT;
+    int* tickets = reinterpret_cast<int*>(scratch + kNoAllocTicketOffset);
+    if (n_groups > 1)   // the array keeps the last call's contents: the counters this call takes tickets from start at zero
+        NB_CUDA(cudaMemsetAsync(tickets, 0, sizeof(int) * (size_t)sp.tiles_i * sp.CS, stream));
+
+    nb::SmallArgs sa;
+    sa.x_i = x_i;
+    sa.xj_raw = x_j;
+    sa.mj_raw = m_j;
+    sa.jp = nullptr;
+    sa.acc = acc_out;
+    sa.pot = pot_out;
+    sa.partial = reinterpret_cast<double4*>(scratch);
+    sa.tickets = tickets;
+    sa.n_i = (int)n_i;
+    sa.n_j = (int)n_j;
+    sa.S = sp.S;
+    sa.eps2 = eps2;
+    sa.flag_offset = 0;
+    // the mask modes of force_impl's small path (all three give the same bits)
+    const int mode = (!pot_out && eps2 >= kUnmaskedMinEps2) ? nb::SMALL_NONE
+                     : (eps2 >= kUnmaskedMinEps2 && nb::small_flag_pays(sp, n_j)) ? nb::SMALL_FLAG : nb::SMALL_EXACT;
+    NB_CUDA(nb::small_launch(sp, sa, mode, stream));
+    ++t_launches;
+    return NB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int nb_force_noalloc(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, const float* m_j, float eps2,
+                     float* acc_out, float* pot_out, void* stream) {
+    t_launches = 0;
+    return force_noalloc_impl(n_i, x_i, n_j, x_j, m_j, eps2, acc_out, pot_out, reinterpret_cast<cudaStream_t>(stream));
+}
+
 const char* nb_status_string(int status) {
     switch (status) {
         case NB_OK: return "NB_OK";
@@ -1419,6 +1515,7 @@ const char* nb_status_string(int status) {
         case NB_ERR_CUDA: return "NB_ERR_CUDA: a CUDA runtime call failed (see nb_last_cuda_error)";
         case NB_ERR_ALLOC: return "NB_ERR_ALLOC: workspace allocation failed";
         case NB_ERR_UNSUPPORTED_DEVICE: return "NB_ERR_UNSUPPORTED_DEVICE: compute capability 10.x (B200, sm_100a) required";
+        case NB_ERR_LIMIT: return "NB_ERR_LIMIT: nb_force_noalloc takes at most NB_NOALLOC_MAX_I = 4096 i-particles (its scratch is a fixed static device array)";
         default: return "unknown nb_status";
     }
 }

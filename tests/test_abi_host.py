@@ -31,7 +31,7 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_status_strings():
-    for code, word in ((0, "NB_OK"), (1, "INVALID"), (2, "CUDA"), (3, "ALLOC"), (4, "UNSUPPORTED")):
+    for code, word in ((0, "NB_OK"), (1, "INVALID"), (2, "CUDA"), (3, "ALLOC"), (4, "UNSUPPORTED"), (5, "LIMIT")):
         assert word in nb.status_string(code)
     assert "unknown" in nb.status_string(99)
 
