@@ -205,6 +205,7 @@ struct SmallPlan {
     int WJ;           // warps of the CTA along j (1, 2, 4, 8 or -- NW = 16 -- 16)
     int S;            // j-chunks across CTAs (grid.y), a multiple of CS
     int CS;           // CTAs per thread-block cluster along grid.y (1, 2, 4 or 8)
+    int pdl = 1;      // launch with programmatic stream serialisation (NB_SMALL_PDL=0 switches it off: nb_debug.h)
     int tile_i;       // i-particles per CTA = (NW / WJ) * KI * (32 / LJ)
     int tiles_i;      // grid.x
 };

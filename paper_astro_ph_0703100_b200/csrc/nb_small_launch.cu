@@ -50,7 +50,7 @@ cudaError_t launch_inst(const SmallPlan& p, const SmallArgs& a, size_t smem, cud
     // kernel's first instruction is griddepcontrol.wait (a small call is ~2.4 us of launch around a few us of work)
     cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    attr[0].val.programmaticStreamSerializationAllowed = p.pdl ? 1 : 0;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     if (CS > 1) {

@@ -69,6 +69,7 @@ struct Knobs {
     bool plan_set = false;       int pK = 0, pWI = 0, pWJ = 0, pS = 0;                 // NB_PLAN
     bool small_plan_set = false; int sNW = 0, sKI = 0, sLJ = 0, sWJ = 0, sS = 0, sCS = 0;   // NB_SMALL_PLAN
     int small = -1;              // NB_SMALL: -1 default, 0 never, 1 always
+    int small_pdl = -1;          // NB_SMALL_PDL: -1 / 1 programmatic dependent launch of nb_small_kernel, 0 plain launch
     int small_mask = -1;         // NB_SMALL_MASK: -1 default (marked pairs), nb::SMALL_EXACT = every pair masked
     int mask = -1;               // NB_MASK: -1 default, else nb::MODE_*
     int fused = -1;              // NB_FUSED_REDUCE
@@ -105,6 +106,12 @@ bool parse_knob(Knobs* k, const char* key, const char* value) {
         k->small_plan_set = true; k->sNW = nw; k->sKI = ki; k->sLJ = lj; k->sWJ = wj; k->sS = ss; k->sCS = cs;
         return true;
     }
+    if (!std::strcmp(key, "NB_SMALL_PDL")) {
+        if (unset) { k->small_pdl = -1; return true; }
+        if (std::strcmp(value, "0") && std::strcmp(value, "1")) return false;
+        k->small_pdl = value[0] - '0';
+        return true;
+    }
     if (!std::strcmp(key, "NB_SMALL_MASK")) {
         if (unset) { k->small_mask = -1; return true; }
         if (value[0] == 'e') k->small_mask = nb::SMALL_EXACT; else if (value[0] == 'f') k->small_mask = nb::SMALL_FLAG; else return false;
@@ -134,7 +141,7 @@ bool parse_knob(Knobs* k, const char* key, const char* value) {
     return false;
 }
 
-const char* const kKnobKeys[] = {"NB_PLAN", "NB_SMALL_PLAN", "NB_SMALL", "NB_SMALL_MASK", "NB_MASK", "NB_FUSED_REDUCE", "NB_DIRECT", "NB_STEP_GRAPH", "NB_BATCH_TILE"};
+const char* const kKnobKeys[] = {"NB_PLAN", "NB_SMALL_PLAN", "NB_SMALL", "NB_SMALL_MASK", "NB_SMALL_PDL", "NB_MASK", "NB_FUSED_REDUCE", "NB_DIRECT", "NB_STEP_GRAPH", "NB_BATCH_TILE"};
 
 // the current switches: one atomic load per call; the environment is read once, here
 const Knobs& knobs() {
@@ -426,6 +433,7 @@ int force_impl(int64_t n_i, const float* x_i, int64_t n_j, const float* x_j, con
             sp.tile_i = (sp.NW / sp.WJ) * sp.KI * (32 / sp.LJ);
             sp.tiles_i = (int)((n_i + sp.tile_i - 1) / sp.tile_i);
         }
+        if (kn.small_pdl == 0) sp.pdl = 0;
         const int n_groups = sp.S / sp.CS;
         if (n_groups > 1) {
             rc = ensure(&ws->partial, &ws->partial_bytes, (size_t)n_groups * (size_t)n_i * sizeof(double4), stream);
