@@ -88,6 +88,28 @@ def test_c0_and_c2_take_the_small_kernel_by_default(nb):
         assert e["acc_max"] < 2e-5                                   # paper's blocked sums: ~1e-6 (Table 2)
 
 
+@pytest.mark.parametrize("n_i,n_j,small", [(4096, 8192, 1), (4097, 8191, 0), (4096, 8193, 0), (512, 131072, 1), (513, 131072, 0),
+                                           (3000, 3000, 1), (4096, 2048, 1), (40, 1600000, 1)])
+def test_the_edges_of_the_default_choice(nb, n_i, n_j, small):
+    """`small_by_default` (nb_plan.h): n_i <= 512 up to 2^26 pairs, n_i <= 4096 up to 2^25 pairs.  On both sides of every
+    edge nb_force -- no switch set -- matches the oracle on a sample of the i-particles, all of which coincide with a j."""
+    assert nb.plan_query_small(n_i, n_j)["default"] == small
+    if n_i <= n_j:
+        w = wl.subset_workload(n_j, n_i, 1.0 / 256, seed=n_i + n_j)
+        x_i = w.x_i
+    else:                                                    # more i than j: every j is an i, the rest lie elsewhere
+        w = wl.plummer_workload(n_j, 1.0 / 256, seed=n_i + n_j)
+        extra = np.random.default_rng(n_i).normal(size=(n_i - n_j, 3)).astype(np.float32)
+        x_i = np.ascontiguousarray(np.concatenate([w.x_j, extra]))
+    acc, pot = gpu_force(nb, x_i, w.x_j, w.m_j, w.eps2)
+    if small:
+        assert nb.last_launch_count() == 1
+    idx = np.unique(np.concatenate([np.arange(0, n_i, max(1, n_i // 64)), [n_i - 1]]))
+    ref_acc, ref_pot = oracle.force(x_i[idx], w.x_j, w.m_j, w.eps2)
+    check_parity(acc[idx], pot[idx], ref_acc, ref_pot, f"{n_i}x{n_j}")
+    assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot))
+
+
 @pytest.mark.parametrize("n_i,n_j", [(1, 1), (1, 777), (3, 200000), (129, 8), (31, 1000), (2048, 3), (1500, 4999),
                                      (17, 4097), (2048, 9000), (64, 70001), (5, 2)])
 def test_ragged_shapes_default_plan(nb, n_i, n_j, nbdebug):
