@@ -82,6 +82,8 @@ def lib() -> ctypes.CDLL:
         l.nb_plan_query.restype = ci
         l.nb_plan_query_small.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
         l.nb_plan_query_small.restype = ci
+        l.nb_plan_query_small_jerk.argtypes = [i64, i64, ci, ctypes.POINTER(i64)]
+        l.nb_plan_query_small_jerk.restype = ci
         l.nb_debug_set.argtypes = [ctypes.c_char_p, ctypes.c_char_p]
         l.nb_debug_set.restype = ci
         l.nb_debug_plan_exhaustive.argtypes = [i64, i64, ci, ci, ctypes.POINTER(i64)]
@@ -532,6 +534,16 @@ def plan_query_small(n_i: int, n_j: int, sm_count: int = 148) -> dict:
     """The small-i-set kernel's decomposition for (n_i, n_j); "default" = nb_force takes that kernel for this shape."""
     out = (ctypes.c_int64 * 8)()
     _check(lib().nb_plan_query_small(int(n_i), int(n_j), int(sm_count), out), "nb_plan_query_small")
+    keys = ("NW", "KI", "LJ", "WJ", "S", "CS", "tiles_i", "default")
+    d = dict(zip(keys, [int(v) for v in out]))
+    d["tile_i"] = (d["NW"] // d["WJ"]) * d["KI"] * (32 // d["LJ"])
+    return d
+
+
+def plan_query_small_jerk(n_i: int, n_j: int, sm_count: int = 148) -> dict:
+    """The small-i-set force + jerk kernel's decomposition; "default" = nb_force_jerk takes that kernel for this shape."""
+    out = (ctypes.c_int64 * 8)()
+    _check(lib().nb_plan_query_small_jerk(int(n_i), int(n_j), int(sm_count), out), "nb_plan_query_small_jerk")
     keys = ("NW", "KI", "LJ", "WJ", "S", "CS", "tiles_i", "default")
     d = dict(zip(keys, [int(v) for v in out]))
     d["tile_i"] = (d["NW"] // d["WJ"]) * d["KI"] * (32 // d["LJ"])

@@ -9,8 +9,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnbody_b200.so")
-SOURCES = ["nbody_b200.cu", "nb_small_launch.cu"]
-DEPS = ["nbody_b200.cu", "nb_small_launch.cu", "nb_small_launch.h", "nb_small.cuh", os.path.join(ROOT, "include", "nb_packed.cuh"), os.path.join(ROOT, "include", "nb_debug.h"), "nb_kernels.cuh", "nb_hermite.cuh", "nb_batched.cuh", "nb_pipelines.cuh", os.path.join(ROOT, "include", "nb_pipeline.cuh"), "nb_plan.h", os.path.join(ROOT, "include", "nbody_b200.h")]
+SOURCES = ["nbody_b200.cu", "nb_small_launch.cu", "nb_small_hermite_launch.cu"]
+DEPS = ["nbody_b200.cu", "nb_small_launch.cu", "nb_small_launch.h", "nb_small.cuh", "nb_small_hermite_launch.cu", "nb_small_hermite_launch.h", "nb_small_hermite.cuh", "nb_hermite_pair.cuh", os.path.join(ROOT, "include", "nb_packed.cuh"), os.path.join(ROOT, "include", "nb_debug.h"), "nb_kernels.cuh", "nb_hermite.cuh", "nb_batched.cuh", "nb_pipelines.cuh", os.path.join(ROOT, "include", "nb_pipeline.cuh"), "nb_plan.h", os.path.join(ROOT, "include", "nbody_b200.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

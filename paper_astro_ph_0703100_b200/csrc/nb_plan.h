@@ -355,4 +355,110 @@ inline SmallPlan make_small_plan(int64_t n_i_exact, int64_t n_j, int sm_count) {
     return best;
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// The small-i-set force + jerk kernel (nb_small_hermite.cuh): one i-particle per thread, 27 instructions per pair, ten sums.
+constexpr int kSmallJerkRoundJPlan = 2048;       // = nb::kSmallHRoundJ (nb_small_hermite.cuh)
+
+// the instantiated shapes (nb_small_hermite_launch.cu)
+inline bool small_jerk_shape_ok(int NW, int LJ, int WJ, int CS) {
+    if (!(CS == 1 || CS == 2 || CS == 4 || CS == kSmallClusterMax)) return false;
+    const bool wide = NW == 16 && LJ == 1 && (WJ == 2 || WJ == 4 || WJ == 8 || WJ == 16);
+    const bool narrow = NW == 8 && (LJ == 2 || LJ == 4) && WJ == 8;
+    if (!wide && !narrow) return false;
+    return ((NW / WJ) * (32 / LJ)) % CS == 0;
+}
+
+// Cycles of one call: the form of small_plan_cost with the Hermite body (54 FMA-pipe cycles per packed group), 32-byte
+// records and ten FP64 sums per particle; the constants are fitted, as there, to the per-call times of every plan on 24
+// shapes (3 100 plans; profiles/r02_small_jerk.md): the pick is 1.3 % on average and 7 % at worst behind the best plan.
+inline double small_jerk_plan_cost(int64_t n_i, int64_t n_j, int sm_count, int NW, int LJ, int WJ, int S, int CS) {
+    const int tile_i = (NW / WJ) * (32 / LJ);
+    const int64_t tiles_i = (n_i + tile_i - 1) / tile_i;
+    const int Q = WJ * LJ;
+    const double ctas = double(tiles_i) * S;
+    const double per_sm = double((int64_t)((ctas + sm_count - 1) / sm_count));
+    const double max_res = NW == 16 ? 1.0 : 2.0;                                    // registers: 100 .. 122 per thread
+    const double resident = per_sm > max_res ? max_res : per_sm;
+    double waves = double((int64_t)((per_sm + resident - 1) / resident));
+    if (CS > 1) {                                                                   // clusters active at a time (nb_small.cuh)
+        const double cap = (CS == 8 ? 15.0 : (CS == 4 ? 31.5 : 74.0)) * resident * sm_count / 148.0;
+        const double cw = double((int64_t)((ctas / CS + cap - 1) / cap));
+        if (cw > waves) waves = cw;
+    }
+    const int64_t chunk = (n_j + S - 1) / S;
+    const double groups = double((((chunk + Q - 1) / Q) + 1) / 2);                  // packed groups of a thread
+    double loop = resident * groups * (NW / 4) * 54.0 / (NW * resident >= 16 ? 0.657 : 0.606);
+    if (LJ > 1) loop *= 1.0 + 0.07 * LJ;
+    const double lone = groups * 86.5;                                              // one warp's dependent chains
+    if (loop < lone) loop = lone;
+    const double rounds = double((chunk + kSmallJerkRoundJPlan - 1) / kSmallJerkRoundJPlan);
+    const double staged = double(chunk > kSmallJerkRoundJPlan ? kSmallJerkRoundJPlan : chunk);
+    double c = 1970.0 * rounds + staged * resident * 0.685;                         // staging latency, L2 -> shared memory
+    c += loop + 400.0 * (groups / 32.0 + 1.0);                                      // Eq. (2) block ends: 20 conversions + 20 DADD
+    c += 50.0 + 47.6 * WJ * tile_i / 32.0;                                          // warp sums: ten doubles per particle
+    if (CS > 1) c += 2220.0;                                                        // two cluster barriers + DSMEM sums
+    const int n_groups = S / CS;
+    if (n_groups > 1) c += 3200.0 + n_groups * (25.0 + 2.0 * tile_i / CS);          // partials + ticket; final sums of a slice
+    return c * waves;
+}
+
+inline SmallPlan make_small_jerk_plan(int64_t n_i_exact, int64_t n_j, int sm_count) {
+    if (sm_count <= 0) sm_count = 148;
+    static const int shapes[6][3] = {{16, 1, 2}, {16, 1, 4}, {16, 1, 8}, {16, 1, 16}, {8, 2, 8}, {8, 4, 8}};   // (NW, LJ, WJ)
+    static const int cs_opts[4] = {1, 2, 4, kSmallClusterMax};
+    const int64_t n_i = small_plan_key_i(n_i_exact);
+    SmallPlan best{};
+    double best_cost = -1.0;
+    for (int sh = 0; sh < 6; ++sh) {
+        const int NW = shapes[sh][0], LJ = shapes[sh][1], WJ = shapes[sh][2];
+        const int tile_i = (NW / WJ) * (32 / LJ);
+        if (tile_i > 8 && (int64_t)tile_i >= 2 * n_i) continue;
+        const int64_t tiles_i = (n_i + tile_i - 1) / tile_i;
+        const int Q = WJ * LJ;
+        for (int ci = 0; ci < 4; ++ci) {
+            const int CS = cs_opts[ci];
+            if (!small_jerk_shape_ok(NW, LJ, WJ, CS)) continue;
+            int64_t cand[6];
+            int n_cand = 0;
+            cand[n_cand++] = CS;
+            cand[n_cand++] = 2 * CS;
+            for (int m = 1; m <= 2; ++m) {
+                cand[n_cand++] = (int64_t)m * sm_count / tiles_i / CS * CS;
+                cand[n_cand++] = (((int64_t)m * sm_count + tiles_i - 1) / tiles_i + CS - 1) / CS * CS;
+            }
+            const int64_t s_max = (n_j / (2 * Q) / CS) * CS;
+            for (int q = 0; q < n_cand; ++q) {
+                int64_t S = cand[q];
+                if (S > s_max) S = s_max;
+                if (S < CS) S = CS;
+                if (S > kMaxS) S = kMaxS / CS * CS;
+                cand[q] = S;
+                bool seen = false;
+                for (int r = 0; r < q; ++r) seen = seen || cand[r] == S;
+                if (seen) continue;
+                if (CS == 1 && S > 64) continue;
+                const double c = small_jerk_plan_cost(n_i, n_j, sm_count, NW, LJ, WJ, (int)S, CS);
+                if (best_cost < 0.0 || c < best_cost * (1.0 - 1e-9)) {
+                    best_cost = c;
+                    best.NW = NW; best.KI = 1; best.LJ = LJ; best.WJ = WJ; best.S = (int)S; best.CS = CS;
+                }
+            }
+        }
+    }
+    best.tile_i = (best.NW / best.WJ) * (32 / best.LJ);
+    best.tiles_i = (int)((n_i + best.tile_i - 1) / best.tile_i);
+    return best;
+}
+
+// Which nb_force_jerk / Hermite-step evaluations take it (per call from a CUDA graph, pack launch included, best plan of
+// this kernel against nb_hermite_kernel's; profiles/r02_small_jerk.md): it wins up to 2^22 pairs -- 256 x 256: 5.3 against
+// 7.8 us, 1024 x 1024: 7.3 against 9.0, 100 x 10000: 9.2 against 14.5, 64 x 65536: 15.6 against 26.1, 2048 x 2048: 12.5
+// against 13.4 -- ties at 1024 x 4096 and loses beyond (2048 x 8192: 28.9 against 26.2, 256 x 65536: 31.6 against 30.0):
+// with ONE i-particle per thread the loop has no more independent chains than the i-packed K = 2 / 4 body.
+constexpr double kSmallJerkMaxPairs = 4194304.0;       // 2^22
+constexpr int64_t kSmallJerkMaxI = 4096;
+inline bool small_jerk_by_default(int64_t n_i, int64_t n_j) {
+    return n_i <= kSmallJerkMaxI && (double)n_i * (double)n_j <= kSmallJerkMaxPairs;
+}
+
 }  // namespace nb

@@ -24,6 +24,8 @@
 #include "nb_plan.h"
 #include "nb_small.cuh"
 #include "nb_small_launch.h"
+#include "nb_small_hermite.cuh"
+#include "nb_small_hermite_launch.h"
 
 #define NB_VERSION 100
 
@@ -69,6 +71,8 @@ struct Knobs {
     bool plan_set = false;       int pK = 0, pWI = 0, pWJ = 0, pS = 0;                 // NB_PLAN
     bool small_plan_set = false; int sNW = 0, sKI = 0, sLJ = 0, sWJ = 0, sS = 0, sCS = 0;   // NB_SMALL_PLAN
     int small = -1;              // NB_SMALL: -1 default, 0 never, 1 always
+    int small_jerk = -1;         // NB_SMALL_JERK: -1 default, 0 never, 1 always (nb_force_jerk and the block step)
+    bool small_jerk_plan_set = false; int jNW = 0, jLJ = 0, jWJ = 0, jS = 0, jCS = 0;   // NB_SMALL_JERK_PLAN
     int small_pdl = -1;          // NB_SMALL_PDL: -1 / 1 programmatic dependent launch of nb_small_kernel, 0 plain launch
     int small_mask = -1;         // NB_SMALL_MASK: -1 default (marked pairs), nb::SMALL_EXACT = every pair masked
     int mask = -1;               // NB_MASK: -1 default, else nb::MODE_*
@@ -86,6 +90,7 @@ std::map<std::pair<int, cudaStream_t>, Workspace> g_ws;
 std::map<std::tuple<int64_t, int64_t, int>, nb::Plan> g_plans;
 std::map<std::tuple<int64_t, int64_t, int>, nb::Plan> g_hplans;
 std::map<std::tuple<int64_t, int64_t, int>, nb::SmallPlan> g_splans;
+std::map<std::tuple<int64_t, int64_t, int>, nb::SmallPlan> g_sjplans;
 
 // ---- debugging switches
 bool parse_knob(Knobs* k, const char* key, const char* value) {
@@ -104,6 +109,20 @@ bool parse_knob(Knobs* k, const char* key, const char* value) {
         if (std::sscanf(value, "%d,%d,%d,%d,%d,%d", &nw, &ki, &lj, &wj, &ss, &cs) != 6) return false;
         if (!(nb::small_shape_ok(nw, ki, lj, wj, cs) && ss >= cs && ss % cs == 0 && ss <= nb::kMaxS)) return false;
         k->small_plan_set = true; k->sNW = nw; k->sKI = ki; k->sLJ = lj; k->sWJ = wj; k->sS = ss; k->sCS = cs;
+        return true;
+    }
+    if (!std::strcmp(key, "NB_SMALL_JERK")) {
+        if (unset) { k->small_jerk = -1; return true; }
+        if (std::strcmp(value, "0") && std::strcmp(value, "1")) return false;
+        k->small_jerk = value[0] - '0';
+        return true;
+    }
+    if (!std::strcmp(key, "NB_SMALL_JERK_PLAN")) {
+        if (unset) { k->small_jerk_plan_set = false; return true; }
+        int nw, lj, wj, ss, cs;
+        if (std::sscanf(value, "%d,%d,%d,%d,%d", &nw, &lj, &wj, &ss, &cs) != 5) return false;
+        if (!(nb::small_jerk_shape_ok(nw, lj, wj, cs) && ss >= cs && ss % cs == 0 && ss <= nb::kMaxS)) return false;
+        k->small_jerk_plan_set = true; k->jNW = nw; k->jLJ = lj; k->jWJ = wj; k->jS = ss; k->jCS = cs;
         return true;
     }
     if (!std::strcmp(key, "NB_SMALL_PDL")) {
@@ -141,7 +160,7 @@ bool parse_knob(Knobs* k, const char* key, const char* value) {
     return false;
 }
 
-const char* const kKnobKeys[] = {"NB_PLAN", "NB_SMALL_PLAN", "NB_SMALL", "NB_SMALL_MASK", "NB_SMALL_PDL", "NB_MASK", "NB_FUSED_REDUCE", "NB_DIRECT", "NB_STEP_GRAPH", "NB_BATCH_TILE"};
+const char* const kKnobKeys[] = {"NB_PLAN", "NB_SMALL_PLAN", "NB_SMALL", "NB_SMALL_MASK", "NB_SMALL_PDL", "NB_SMALL_JERK", "NB_SMALL_JERK_PLAN", "NB_MASK", "NB_FUSED_REDUCE", "NB_DIRECT", "NB_STEP_GRAPH", "NB_BATCH_TILE"};
 
 // the current switches: one atomic load per call; the environment is read once, here
 const Knobs& knobs() {
@@ -258,6 +277,21 @@ nb::SmallPlan cached_small_plan(int64_t n_i, int64_t n_j, int sm_count) {
     std::lock_guard<std::mutex> lock(g_mutex);
     if (g_splans.size() > 4096) g_splans.clear();
     g_splans[key] = p;
+    return p;
+}
+
+nb::SmallPlan cached_small_jerk_plan(int64_t n_i, int64_t n_j, int sm_count) {
+    const auto key = std::make_tuple(nb::small_plan_key_i(n_i), n_j, sm_count);
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        auto it = g_sjplans.find(key);
+        if (it != g_sjplans.end()) return it->second;
+    }
+    const nb::SmallPlan p = nb::make_small_jerk_plan(n_i, n_j, sm_count);  // outside the lock
+    g_plans_computed.fetch_add(1, std::memory_order_relaxed);
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (g_sjplans.size() > 4096) g_sjplans.clear();
+    g_sjplans[key] = p;
     return p;
 }
 
@@ -630,6 +664,60 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     Workspace* ws = guard.ws;
     rc = ensure(&ws->jp2, &ws->jp2_bytes, (size_t)n_j * 2 * sizeof(float4), stream);
     if (rc != NB_OK) return rc;
+    // Small i-sets: the kernel packed over j (nb_small_hermite.cuh), one launch after the records are packed
+    if (kn.small_jerk >= 0 ? (kn.small_jerk != 0)
+                           : (!kn.plan_set && kn.mask < 0 && kn.fused < 0 && nb::small_jerk_by_default(n_i, n_j))) {
+        nb::SmallPlan sp = cached_small_jerk_plan(n_i, n_j, info.sm_count);
+        if (kn.small_jerk_plan_set) {
+            sp.NW = kn.jNW; sp.KI = 1; sp.LJ = kn.jLJ; sp.WJ = kn.jWJ; sp.S = kn.jS; sp.CS = kn.jCS;
+            sp.tile_i = (sp.NW / sp.WJ) * (32 / sp.LJ);
+            sp.tiles_i = (int)((n_i + sp.tile_i - 1) / sp.tile_i);
+        }
+        if (kn.small_pdl == 0) sp.pdl = 0;
+        const int n_groups = sp.S / sp.CS;
+        if (n_groups > 1) {
+            rc = ensure(&ws->hpartial, &ws->hpartial_bytes, (size_t)n_groups * (size_t)n_i * nb::kHermiteAcc * sizeof(double), stream);
+            if (rc != NB_OK) return rc;
+            const size_t need = (size_t)sp.tiles_i * sp.CS * sizeof(int);
+            if (need > ws->tickets_bytes) {
+                rc = ensure(&ws->tickets, &ws->tickets_bytes, need, stream);
+                if (rc != NB_OK) return rc;
+                NB_CUDA(cudaMemsetAsync(ws->tickets, 0, ws->tickets_bytes, stream));   // once per growth; kernels leave zeros
+            }
+        }
+        if (!prepacked) {
+            nb::nb_pack_jv_kernel<<<(unsigned)((n_j + 255) / 256), 256, 0, stream>>>(x_j, v_j, m_j, (int)n_j,
+                                                                                      reinterpret_cast<float4*>(ws->jp2));
+            NB_CUDA(cudaGetLastError());
+            ++t_launches;
+        }
+        nb::SmallHermiteArgs sa;
+        sa.x_i = x_i;
+        sa.v_i = v_i;
+        sa.jp = reinterpret_cast<const float4*>(ws->jp2);
+        sa.acc = acc_out;
+        sa.jerk = jerk_out;
+        sa.pot = pot_out;
+        sa.partial = reinterpret_cast<double*>(ws->hpartial);
+        sa.tickets = reinterpret_cast<int*>(ws->tickets);
+        sa.n_i = (int)n_i;
+        sa.n_j = (int)n_j;
+        sa.S = sp.S;
+        sa.eps2 = eps2;
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        if (t_profile) {
+            NB_CUDA(cudaEventCreate(&e0));
+            NB_CUDA(cudaEventCreate(&e1));
+            NB_CUDA(cudaEventRecord(e0, stream));
+        }
+        NB_CUDA(nb::small_hermite_launch(sp, sa, stream));
+        if (t_profile) {
+            NB_CUDA(cudaEventRecord(e1, stream));
+            t_events.emplace_back(e0, e1);
+        }
+        ++t_launches;
+        return NB_OK;
+    }
     // second pass: fused into the kernel (small tiles) or a separate launch, as for nb_force; NB_FUSED_REDUCE=0/1 forces
     const int mode = pick_mode(n_i, n_j, eps2, true, kListMinPairsJerk);
     const bool fused_reduce = plan.S > 1 && mode == nb::MODE_EXACT &&      // only the masked (small-call) kernels carry the ticket code
@@ -1395,6 +1483,14 @@ int nb_plan_query_small(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]) 
     const nb::SmallPlan p = nb::make_small_plan(n_i, n_j, sm_count);
     out[0] = p.NW; out[1] = p.KI; out[2] = p.LJ; out[3] = p.WJ; out[4] = p.S; out[5] = p.CS; out[6] = p.tiles_i;
     out[7] = nb::small_by_default(n_i, n_j) ? 1 : 0;
+    return NB_OK;
+}
+
+int nb_plan_query_small_jerk(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]) {
+    if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
+    const nb::SmallPlan p = nb::make_small_jerk_plan(n_i, n_j, sm_count);
+    out[0] = p.NW; out[1] = p.KI; out[2] = p.LJ; out[3] = p.WJ; out[4] = p.S; out[5] = p.CS; out[6] = p.tiles_i;
+    out[7] = nb::small_jerk_by_default(n_i, n_j) ? 1 : 0;
     return NB_OK;
 }
 
