@@ -44,6 +44,10 @@ struct SmallHermiteArgs {
 constexpr int kSmallHRoundJ = 2048;      // j-particles staged in shared memory at a time (64 KB + padding)
 constexpr int kSmallHBlockPairs = 32;    // Eq. (2): FP32 partial sums over at most 32 j-pairs = 64 j of a slot
 constexpr int kSmallHLoadBatch = 2;      // j-pairs (64 B each) a thread loads before it stores them to shared memory
+#ifndef NB_SMALL_H_UNROLL
+#define NB_SMALL_H_UNROLL 4
+#endif
+constexpr int kSmallHUnroll = NB_SMALL_H_UNROLL;   // j-pairs per loop iteration (512 x 65536: 54.7 / 50.6 / 52.0 / 49.4 us with 1 / 2 / 3 / 4)
 
 // float4 per j-slot: four per pair, plus one so that the LJ lane groups of a warp (same pair index, LJ different slots)
 // read different banks
@@ -138,7 +142,7 @@ __global__ void __launch_bounds__(32 * NW) nb_small_hermite_kernel(const SmallHe
             u64 part[NA];
 #pragma unroll
             for (int c = 0; c < NA; ++c) part[c] = 0ull;
-#pragma unroll 2
+#pragma unroll kSmallHUnroll
             for (int p = 0; p < nb_; ++p) {
                 const float4 A = sp[4 * (b + p)], B = sp[4 * (b + p) + 1], C = sp[4 * (b + p) + 2], D = sp[4 * (b + p) + 3];
                 hermite_pair<true, PHI>(pack2(A.x, A.y), pack2(A.z, A.w), pack2(B.x, B.y), pack2(B.z, B.w),

@@ -180,6 +180,17 @@ def test_small_planner_invariants():
         assert {k: v for k, v in p.items() if k != "default"} == {k: v for k, v in q.items() if k != "default"}
 
 
+def test_small_jerk_planner_invariants():
+    for n_i, n_j in [(1, 1), (1, 777), (16, 16384), (512, 65536), (2048, 2048), (2048, 65536), (100, 10 ** 6), (3, 5), (4096, 1024)]:
+        p = nb.plan_query_small_jerk(n_i, n_j, 148)
+        assert (p["NW"], p["LJ"], p["WJ"]) in ((16, 1, 2), (16, 1, 4), (16, 1, 8), (16, 1, 16), (8, 2, 8), (8, 4, 8)) and p["KI"] == 1
+        assert p["tile_i"] == (p["NW"] // p["WJ"]) * (32 // p["LJ"])
+        assert p["tiles_i"] * p["tile_i"] >= n_i > (p["tiles_i"] - 1) * p["tile_i"]
+        assert p["CS"] in (1, 2, 4, 8) and p["S"] % p["CS"] == 0 and p["tile_i"] % p["CS"] == 0 and 1 <= p["S"] <= 2048
+        assert p["default"] == int(n_i <= 4096 and n_i * n_j <= 2 ** 22)
+        assert p == nb.plan_query_small_jerk(n_i, n_j, 148)
+
+
 def test_debug_switches_parse_and_reject():
     assert nb.lib().nb_debug_set(b"NB_PLAN", b"8,8,1,3") == 0
     assert nb.lib().nb_debug_set(b"NB_PLAN", b"8,8,2,3") == 1           # WI * WJ != 8
@@ -189,8 +200,15 @@ def test_debug_switches_parse_and_reject():
     assert nb.lib().nb_debug_set(b"NB_SMALL_PLAN", b"8,1,4,8,8,8") == 0   # tile 8, cluster 8
     assert nb.lib().nb_debug_set(b"NB_SMALL_PLAN", b"16,2,1,2,144,8") == 0
     assert nb.lib().nb_debug_set(b"NB_SMALL_PLAN", b"") == 0
+    assert nb.lib().nb_debug_set(b"NB_SMALL_JERK_PLAN", b"16,1,8,18,2") == 0
+    assert nb.lib().nb_debug_set(b"NB_SMALL_JERK_PLAN", b"16,1,1,18,2") == 1   # WJ = 1 is not instantiated for force + jerk
+    assert nb.lib().nb_debug_set(b"NB_SMALL_JERK_PLAN", b"8,4,8,8,4") == 0
+    assert nb.lib().nb_debug_set(b"NB_SMALL_JERK_PLAN", b"8,4,8,6,8") == 1     # S is not a multiple of the cluster size
+    assert nb.lib().nb_debug_set(b"NB_SMALL_JERK_PLAN", None) == 0
+    assert nb.lib().nb_debug_set(b"NB_SMALL_JERK", b"2") == 1
+    assert nb.lib().nb_debug_set(b"NB_SMALL_PDL", b"0") == 0
     assert nb.lib().nb_debug_set(b"NB_MASK", b"nonsense") == 1
     assert nb.lib().nb_debug_set(b"NB_NO_SUCH_SWITCH", b"1") == 1
     assert nb.lib().nb_debug_set(None, b"1") == 1
-    for key in (b"NB_MASK", b"NB_SMALL", b"NB_SMALL_MASK", b"NB_FUSED_REDUCE", b"NB_DIRECT", b"NB_STEP_GRAPH", b"NB_BATCH_TILE"):
+    for key in (b"NB_MASK", b"NB_SMALL", b"NB_SMALL_MASK", b"NB_SMALL_PDL", b"NB_SMALL_JERK", b"NB_SMALL_JERK_PLAN", b"NB_FUSED_REDUCE", b"NB_DIRECT", b"NB_STEP_GRAPH", b"NB_BATCH_TILE"):
         assert nb.lib().nb_debug_set(key, None) == 0
