@@ -22,6 +22,7 @@
  *   NB_FUSED_REDUCE    "0" | "1"                  second pass of the j-split as a separate launch / inside the force kernel
  *   NB_DIRECT          "0"                        small calls go through nb_pack_j_kernel + TMA instead of packing in-kernel
  *   NB_STEP_GRAPH      "0"                        nb_leapfrog_kdk / nb_hermite4 enqueue every step eagerly (no CUDA graph)
+ *   NB_HERMITE_FUSE    "0"                        nb_hermite4 corrects a step and predicts the next in two launches instead of one
  *   NB_BATCH_TILE      "64" | "128" | "256"       i-tile of nb_force_batched
  *
  * value == NULL or "" restores the default.  Returns NB_OK, or NB_ERR_INVALID_VALUE for an unknown key or a value that

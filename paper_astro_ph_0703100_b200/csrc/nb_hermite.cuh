@@ -361,6 +361,37 @@ __global__ void __launch_bounds__(256) nb_hermite_correct_kernel(float* __restri
     j0[k] = j_new;
 }
 
+// correct of step s and predict + pack of step s + 1 in one launch (one thread per particle; the same operations in the same
+// order as the two kernels above, so the same bits): a step of nb_hermite4 is then two launches, which is what counts while
+// the integration of a small system is launch-bound.
+__global__ void __launch_bounds__(256) nb_hermite_correct_predict_pack_kernel(float* __restrict__ x, float* __restrict__ v,
+                                                                              float* __restrict__ a0, float* __restrict__ j0,
+                                                                              const float* __restrict__ a1, const float* __restrict__ j1,
+                                                                              const float* __restrict__ m, float* __restrict__ xp,
+                                                                              float* __restrict__ vp, float4* __restrict__ jp, int n, float dt) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float h = 0.5f * dt, h2 = dt * dt * (1.0f / 12.0f);
+    float px[3], pv[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const size_t k = 3 * (size_t)i + c;
+        const float a_old = a0[k], a_new = a1[k], j_old = j0[k], j_new = j1[k], v_old = v[k];
+        const float v_new = fmaf(j_old - j_new, h2, fmaf(a_old + a_new, h, v_old));
+        const float x_new = fmaf(a_old - a_new, h2, fmaf(v_old + v_new, h, x[k]));
+        x[k] = x_new;
+        v[k] = v_new;
+        a0[k] = a_new;
+        j0[k] = j_new;
+        px[c] = fmaf(fmaf(fmaf(j_new, dt * (1.0f / 3.0f), a_new), dt * 0.5f, v_new), dt, x_new);
+        pv[c] = fmaf(fmaf(j_new, dt * 0.5f, a_new), dt, v_new);
+        xp[k] = px[c];
+        vp[k] = pv[c];
+    }
+    jp[2 * (size_t)i + 0] = make_float4(px[0], px[1], px[2], m[i]);
+    jp[2 * (size_t)i + 1] = make_float4(pv[0], pv[1], pv[2], 0.0f);
+}
+
 // ---------------------------------------------------------------- block (individual) time steps: one block step, row f4
 // Every particle holds (x, v, a, j) at its own time t[k] (FP64; the interval h = t_now - t[k] is rounded to FP32 once).
 // predict everybody to t_now (same Horner form as the shared-step kernel, h per particle) and pack the j records:

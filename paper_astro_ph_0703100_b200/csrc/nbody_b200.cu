@@ -79,6 +79,7 @@ struct Knobs {
     int fused = -1;              // NB_FUSED_REDUCE
     int direct = -1;             // NB_DIRECT
     int step_graph = -1;         // NB_STEP_GRAPH
+    int hermite_fuse = -1;       // NB_HERMITE_FUSE: 0 = correct and predict as separate launches
     int batch_tile = 0;          // NB_BATCH_TILE
 };
 
@@ -125,6 +126,12 @@ bool parse_knob(Knobs* k, const char* key, const char* value) {
         k->small_jerk_plan_set = true; k->jNW = nw; k->jLJ = lj; k->jWJ = wj; k->jS = ss; k->jCS = cs;
         return true;
     }
+    if (!std::strcmp(key, "NB_HERMITE_FUSE")) {
+        if (unset) { k->hermite_fuse = -1; return true; }
+        if (std::strcmp(value, "0") && std::strcmp(value, "1")) return false;
+        k->hermite_fuse = value[0] - '0';
+        return true;
+    }
     if (!std::strcmp(key, "NB_SMALL_PDL")) {
         if (unset) { k->small_pdl = -1; return true; }
         if (std::strcmp(value, "0") && std::strcmp(value, "1")) return false;
@@ -160,7 +167,7 @@ bool parse_knob(Knobs* k, const char* key, const char* value) {
     return false;
 }
 
-const char* const kKnobKeys[] = {"NB_PLAN", "NB_SMALL_PLAN", "NB_SMALL", "NB_SMALL_MASK", "NB_SMALL_PDL", "NB_SMALL_JERK", "NB_SMALL_JERK_PLAN", "NB_MASK", "NB_FUSED_REDUCE", "NB_DIRECT", "NB_STEP_GRAPH", "NB_BATCH_TILE"};
+const char* const kKnobKeys[] = {"NB_PLAN", "NB_SMALL_PLAN", "NB_SMALL", "NB_SMALL_MASK", "NB_SMALL_PDL", "NB_SMALL_JERK", "NB_SMALL_JERK_PLAN", "NB_MASK", "NB_FUSED_REDUCE", "NB_DIRECT", "NB_STEP_GRAPH", "NB_HERMITE_FUSE", "NB_BATCH_TILE"};
 
 // the current switches: one atomic load per call; the environment is read once, here
 const Knobs& knobs() {
@@ -1267,16 +1274,40 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
     const bool real_stream = reinterpret_cast<uintptr_t>(stream) > 2;   // the default streams cannot be captured
     const bool step_graph = real_stream && n_steps >= 16 && n <= 32768 && cap == cudaStreamCaptureStatusNone && !t_profile &&
                             knobs().step_graph != 0;                    // NB_STEP_GRAPH=0 (nb_debug.h): every step eagerly
+    // A step is two launches: force + jerk on the predicted state, then ONE kernel that corrects the step and predicts + packs
+    // the next one (NB_HERMITE_FUSE=0, nb_debug.h: correct and predict as separate launches -- the same bits).
+    const bool fuse = knobs().hermite_fuse != 0;
+    nb::nb_hermite_predict_pack_kernel<<<pblocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, m, xp, vp, jp2, (int)n, dt);
+    NB_CUDA(cudaGetLastError());
+    ++launches;
+    auto launched = [&]() -> bool {                                    // NB_CUDA returns from the enclosing FUNCTION: not inside a lambda
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) t_last_cuda_error = (int)e;
+        return e == cudaSuccess;
+    };
+    auto close_step = [&](bool last) -> int {                          // correct step s; unless it is the last, predict s + 1.  Launches, or -1
+        if (!last && fuse) {
+            nb::nb_hermite_correct_predict_pack_kernel<<<pblocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, a1, j1, m, xp, vp, jp2, (int)n, dt);
+            return launched() ? 1 : -1;
+        }
+        nb::nb_hermite_correct_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, a1, j1, n3, dt);
+        if (!launched()) return -1;
+        if (last) return 1;
+        nb::nb_hermite_predict_pack_kernel<<<pblocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, m, xp, vp, jp2, (int)n, dt);
+        return launched() ? 2 : -1;
+    };
     for (int64_t s = 0; s < n_steps; ++s) {
-        if (step_graph && s == 2) {                                    // steps 0 and 1 ran eagerly: everything is warm
+        if (step_graph && s == 2 && n_steps - 1 - s > 0) {             // steps 0 and 1 ran eagerly: everything is warm
             cudaGraph_t graph = nullptr;
             cudaGraphExec_t exec = nullptr;
             NB_CUDA(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
-            nb::nb_hermite_predict_pack_kernel<<<pblocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, m, xp, vp, jp2, (int)n, dt);
             t_launches = 0;
             rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, nullptr, stream, true);
-            const int64_t per_step = t_launches + 2;
-            nb::nb_hermite_correct_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, a1, j1, n3, dt);
+            int64_t per_step = t_launches;
+            if (rc == NB_OK) {
+                const int k = close_step(false);
+                if (k < 0) rc = NB_ERR_CUDA; else per_step += k;
+            }
             cudaError_t ce = cudaStreamEndCapture(stream, &graph);
             if (rc != NB_OK || ce != cudaSuccess) {
                 if (graph) (void)cudaGraphDestroy(graph);
@@ -1292,14 +1323,14 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
             launches += per_step * replays;
             s += replays;                                              // the last step follows eagerly (it wants phi)
         }
-        nb::nb_hermite_predict_pack_kernel<<<pblocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, m, xp, vp, jp2, (int)n, dt);
-        NB_CUDA(cudaGetLastError());
+        const bool last = s + 1 == n_steps;
         t_launches = 0;
-        rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, s + 1 == n_steps ? pot_out : nullptr, stream, true);
+        rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, last ? pot_out : nullptr, stream, true);
         if (rc != NB_OK) return rc;
-        launches += t_launches + 2;
-        nb::nb_hermite_correct_kernel<<<blocks, threads, 0, stream>>>(x, v, acc_io, jerk_io, a1, j1, n3, dt);
-        NB_CUDA(cudaGetLastError());
+        launches += t_launches;
+        const int k = close_step(last);
+        if (k < 0) return NB_ERR_CUDA;
+        launches += k;
     }
     t_launches = launches;
     return NB_OK;

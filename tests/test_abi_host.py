@@ -210,5 +210,5 @@ def test_debug_switches_parse_and_reject():
     assert nb.lib().nb_debug_set(b"NB_MASK", b"nonsense") == 1
     assert nb.lib().nb_debug_set(b"NB_NO_SUCH_SWITCH", b"1") == 1
     assert nb.lib().nb_debug_set(None, b"1") == 1
-    for key in (b"NB_MASK", b"NB_SMALL", b"NB_SMALL_MASK", b"NB_SMALL_PDL", b"NB_SMALL_JERK", b"NB_SMALL_JERK_PLAN", b"NB_FUSED_REDUCE", b"NB_DIRECT", b"NB_STEP_GRAPH", b"NB_BATCH_TILE"):
+    for key in (b"NB_MASK", b"NB_SMALL", b"NB_SMALL_MASK", b"NB_SMALL_PDL", b"NB_SMALL_JERK", b"NB_SMALL_JERK_PLAN", b"NB_FUSED_REDUCE", b"NB_DIRECT", b"NB_STEP_GRAPH", b"NB_HERMITE_FUSE", b"NB_BATCH_TILE"):
         assert nb.lib().nb_debug_set(key, None) == 0

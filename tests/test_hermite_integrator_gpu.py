@@ -98,3 +98,22 @@ def test_step_graph_replay_is_bitwise_the_eager_sequence(nb, n, nbdebug):
     for a, b in zip(out["1"][:5], out["0"][:5]):
         assert np.array_equal(a, b)
     assert out["1"][5] == out["0"][5]
+
+
+@pytest.mark.parametrize("n", [700, 1500, 9000])
+def test_fused_correct_predict_is_bitwise_the_two_launches(nb, n, nbdebug):
+    """A step closes with ONE kernel that corrects it and predicts + packs the next (two launches per step); with
+    NB_HERMITE_FUSE=0 the correction and the prediction are separate launches: the same bits, one launch more per step."""
+    import torch
+    w = wl.plummer_workload(n, 1.0 / 64, seed=9, with_velocities=True)
+    out = {}
+    for mode in ("1", "0"):
+        nbdebug.setenv("NB_HERMITE_FUSE", mode)
+        x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
+        acc, jerk, pot = nb.hermite4(x, v, m, w.eps2, 1.0 / 256, 7)
+        torch.cuda.synchronize()
+        out[mode] = (x.cpu().numpy(), v.cpu().numpy(), acc.cpu().numpy(), jerk.cpu().numpy(), pot.cpu().numpy(),
+                     nb.last_launch_count())
+    for a, b in zip(out["1"][:5], out["0"][:5]):
+        assert np.array_equal(a, b)
+    assert out["0"][5] == out["1"][5] + 6          # steps 0 .. 5 close with two launches instead of one
