@@ -541,11 +541,14 @@ def plan_query_small(n_i: int, n_j: int, sm_count: int = 148) -> dict:
 
 
 def plan_query_small_jerk(n_i: int, n_j: int, sm_count: int = 148) -> dict:
-    """The small-i-set force + jerk kernel's decomposition; "default" = nb_force_jerk takes that kernel for this shape."""
+    """The small-i-set force + jerk kernel's decomposition; "default" = nb_force_jerk takes that kernel for this shape,
+    "default_steps" = the Hermite steps do."""
     out = (ctypes.c_int64 * 8)()
     _check(lib().nb_plan_query_small_jerk(int(n_i), int(n_j), int(sm_count), out), "nb_plan_query_small_jerk")
     keys = ("NW", "KI", "LJ", "WJ", "S", "CS", "tiles_i", "default")
     d = dict(zip(keys, [int(v) for v in out]))
+    d["default_steps"] = (d["default"] >> 1) & 1        # nb_hermite4 / nb_hermite4_block_step (records already packed)
+    d["default"] &= 1                                   # nb_force_jerk
     d["tile_i"] = (d["NW"] // d["WJ"]) * d["KI"] * (32 // d["LJ"])
     return d
 

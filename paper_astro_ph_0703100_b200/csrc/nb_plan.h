@@ -450,15 +450,26 @@ inline SmallPlan make_small_jerk_plan(int64_t n_i_exact, int64_t n_j, int sm_cou
     return best;
 }
 
-// Which nb_force_jerk / Hermite-step evaluations take it (per call from a CUDA graph, pack launch included, best plan of
-// this kernel against nb_hermite_kernel's; profiles/r02_small_jerk.md): it wins up to 2^22 pairs -- 256 x 256: 5.3 against
-// 7.8 us, 1024 x 1024: 7.3 against 9.0, 100 x 10000: 9.2 against 14.5, 64 x 65536: 15.6 against 26.1, 2048 x 2048: 12.5
-// against 13.4 -- ties at 1024 x 4096 and loses beyond (2048 x 8192: 28.9 against 26.2, 256 x 65536: 31.6 against 30.0):
-// with ONE i-particle per thread the loop has no more independent chains than the i-packed K = 2 / 4 body.
-constexpr double kSmallJerkMaxPairs = 4194304.0;       // 2^22
+// Which evaluations take it (per call from a CUDA graph, best plan of this kernel against nb_hermite_kernel's;
+// profiles/r02_small_jerk.md).
+//  * Hermite steps (nb_hermite4, nb_hermite4_block_step), whose predictor has packed the j-records: up to 2^22 pairs --
+//    256 x 256: 5.3 against 7.8 us, 100 x 10000: 9.2 against 14.5, 64 x 65536: 15.6 against 26.1, 2048 x 2048: 12.5 against
+//    13.4; a tie at 1024 x 4096, and beyond nb_hermite_kernel wins (2048 x 8192: 28.9 against 26.2, 256 x 65536: 31.6 against
+//    30.0): ONE i-particle per thread gives the loop no more independent chains than the i-packed K = 2 / 4 body.
+//  * nb_force_jerk on x_j, v_j, m_j: this kernel packs while it stages, nb_hermite_kernel needs nb_pack_jv_kernel first, so
+//    it stays ahead up to 2^25 pairs (4096 i-particles) and 2^26 pairs (1024): 256 x 256: 3.3 against 7.5 us, 2048 x 2048:
+//    9.9 against 13.7, 4096 x 4096: 25.6 against 28.0, 2048 x 16384: 44.1 against 46.7, 1024 x 65536: 82.7 against 87.0;
+//    2048 x 65536: 157 against 148.
 constexpr int64_t kSmallJerkMaxI = 4096;
-inline bool small_jerk_by_default(int64_t n_i, int64_t n_j) {
-    return n_i <= kSmallJerkMaxI && (double)n_i * (double)n_j <= kSmallJerkMaxPairs;
+constexpr double kSmallJerkMaxPairs = 4194304.0;           // 2^22: records already packed
+constexpr double kSmallJerkMaxPairsRaw = 33554432.0;       // 2^25: nb_force_jerk
+constexpr int64_t kSmallJerkNarrowI = 1024;
+constexpr double kSmallJerkMaxPairsRawNarrow = 67108864.0; // 2^26: nb_force_jerk, n_i <= 1024
+inline bool small_jerk_by_default(int64_t n_i, int64_t n_j, bool prepacked) {
+    const double pairs = (double)n_i * (double)n_j;
+    if (n_i > kSmallJerkMaxI) return false;
+    if (prepacked) return pairs <= kSmallJerkMaxPairs;
+    return pairs <= kSmallJerkMaxPairsRaw || (n_i <= kSmallJerkNarrowI && pairs <= kSmallJerkMaxPairsRawNarrow);
 }
 
 }  // namespace nb

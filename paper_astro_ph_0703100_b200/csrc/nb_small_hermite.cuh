@@ -7,7 +7,8 @@
 //     is the broadcast operand; ONE i-particle per thread, 10 packed accumulators (a, J1, J2, phi);
 //   * the CTA interleaves its j-chunk into shared memory as pairs -- (x0 x1 y0 y1) (z0 z1 m0 m1) (vx0 vx1 vy0 vy1)
 //     (vz0 vz1 - -): four LDS.128 per j-pair, no register shuffling in the loop -- from the packed 32-byte records
-//     (x y z m | vx vy vz 0) that nb_pack_jv_kernel or the predictor of a block step has written;
+//     (x y z m | vx vy vz 0) that the predictor of a Hermite step has written, or from x_j, v_j, m_j directly (nb_force_jerk:
+//     no pack launch);
 //   * lanes LI x LJ, warps WI x WJ, S j-chunks over CTAs; the partial sums are combined in a FIXED order at every level:
 //     shuffles (LJ), shared memory (WJ), distributed shared memory inside a cluster of 2, 4 or 8 CTAs, and -- when S > the
 //     cluster size -- FP64 partials in global memory summed by the last-arriving CTA of every (i-tile, slice).  No
@@ -29,7 +30,10 @@ namespace nb {
 struct SmallHermiteArgs {
     const float* x_i;      // [n_i][3]
     const float* v_i;      // [n_i][3]
-    const float4* jp;      // [n_j][2] packed records (x y z m | vx vy vz 0)
+    const float4* jp;      // [n_j][2] packed records (x y z m | vx vy vz 0), or nullptr: the three arrays below
+    const float* xj_raw;   // [n_j][3]
+    const float* vj_raw;   // [n_j][3]
+    const float* mj_raw;   // [n_j]
     float* acc;            // [n_i][3]
     float* jerk;           // [n_i][3]
     float* pot;            // [n_i] or nullptr
@@ -114,10 +118,19 @@ __global__ void __launch_bounds__(32 * NW) nb_small_hermite_kernel(const SmallHe
                 if (pp >= n_pairs_round) break;
                 const size_t j = (size_t)r_lo + 2 * (size_t)pp;
                 const bool two = 2 * pp + 1 < nr;                      // false: the round's last pair holds one particle
-                P0[u] = a.jp[2 * j]; V0[u] = a.jp[2 * j + 1];
-                // an odd count: the second half is a copy with zero mass (adds nothing)
-                P1[u] = two ? a.jp[2 * j + 2] : make_float4(P0[u].x, P0[u].y, P0[u].z, 0.0f);
-                V1[u] = two ? a.jp[2 * j + 3] : V0[u];
+                if (a.jp) {
+                    P0[u] = a.jp[2 * j]; V0[u] = a.jp[2 * j + 1];
+                    // an odd count: the second half is a copy with zero mass (adds nothing)
+                    P1[u] = two ? a.jp[2 * j + 2] : make_float4(P0[u].x, P0[u].y, P0[u].z, 0.0f);
+                    V1[u] = two ? a.jp[2 * j + 3] : V0[u];
+                } else {                                               // rows a1 + a2 in one step: no pack launch (nb_force_jerk)
+                    const float* xr = a.xj_raw + 3 * j;
+                    const float* vr = a.vj_raw + 3 * j;
+                    P0[u] = make_float4(xr[0], xr[1], xr[2], a.mj_raw[j]);
+                    V0[u] = make_float4(vr[0], vr[1], vr[2], 0.0f);
+                    P1[u] = two ? make_float4(xr[3], xr[4], xr[5], a.mj_raw[j + 1]) : make_float4(P0[u].x, P0[u].y, P0[u].z, 0.0f);
+                    V1[u] = two ? make_float4(vr[3], vr[4], vr[5], 0.0f) : V0[u];
+                }
             }
 #pragma unroll
             for (int u = 0; u < kSmallHLoadBatch; ++u) {

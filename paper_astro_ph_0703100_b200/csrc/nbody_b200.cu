@@ -669,11 +669,10 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
     const nb::Plan plan = cached_plan(n_i, n_j, info.sm_count, true);
     WsGuard guard(dev, stream);
     Workspace* ws = guard.ws;
-    rc = ensure(&ws->jp2, &ws->jp2_bytes, (size_t)n_j * 2 * sizeof(float4), stream);
-    if (rc != NB_OK) return rc;
-    // Small i-sets: the kernel packed over j (nb_small_hermite.cuh), one launch after the records are packed
+    // Small i-sets: the kernel packed over j (nb_small_hermite.cuh), one launch (it packs the j-records itself unless the
+    // caller -- a Hermite step's predictor -- already has)
     if (kn.small_jerk >= 0 ? (kn.small_jerk != 0)
-                           : (!kn.plan_set && kn.mask < 0 && kn.fused < 0 && nb::small_jerk_by_default(n_i, n_j))) {
+                           : (!kn.plan_set && kn.mask < 0 && kn.fused < 0 && nb::small_jerk_by_default(n_i, n_j, prepacked))) {
         nb::SmallPlan sp = cached_small_jerk_plan(n_i, n_j, info.sm_count);
         if (kn.small_jerk_plan_set) {
             sp.NW = kn.jNW; sp.KI = 1; sp.LJ = kn.jLJ; sp.WJ = kn.jWJ; sp.S = kn.jS; sp.CS = kn.jCS;
@@ -692,16 +691,13 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
                 NB_CUDA(cudaMemsetAsync(ws->tickets, 0, ws->tickets_bytes, stream));   // once per growth; kernels leave zeros
             }
         }
-        if (!prepacked) {
-            nb::nb_pack_jv_kernel<<<(unsigned)((n_j + 255) / 256), 256, 0, stream>>>(x_j, v_j, m_j, (int)n_j,
-                                                                                      reinterpret_cast<float4*>(ws->jp2));
-            NB_CUDA(cudaGetLastError());
-            ++t_launches;
-        }
         nb::SmallHermiteArgs sa;
         sa.x_i = x_i;
         sa.v_i = v_i;
-        sa.jp = reinterpret_cast<const float4*>(ws->jp2);
+        sa.jp = prepacked ? reinterpret_cast<const float4*>(ws->jp2) : nullptr;   // not packed yet: the kernel reads the three arrays
+        sa.xj_raw = x_j;
+        sa.vj_raw = v_j;
+        sa.mj_raw = m_j;
         sa.acc = acc_out;
         sa.jerk = jerk_out;
         sa.pot = pot_out;
@@ -725,6 +721,8 @@ int force_jerk_impl(int64_t n_i, const float* x_i, const float* v_i, int64_t n_j
         ++t_launches;
         return NB_OK;
     }
+    rc = ensure(&ws->jp2, &ws->jp2_bytes, (size_t)n_j * 2 * sizeof(float4), stream);
+    if (rc != NB_OK) return rc;
     // second pass: fused into the kernel (small tiles) or a separate launch, as for nb_force; NB_FUSED_REDUCE=0/1 forces
     const int mode = pick_mode(n_i, n_j, eps2, true, kListMinPairsJerk);
     const bool fused_reduce = plan.S > 1 && mode == nb::MODE_EXACT &&      // only the masked (small-call) kernels carry the ticket code
@@ -1521,7 +1519,7 @@ int nb_plan_query_small_jerk(int64_t n_i, int64_t n_j, int sm_count, int64_t out
     if (!out || bad_count(n_i) || bad_count(n_j) || n_i < 1 || n_j < 1) return NB_ERR_INVALID_VALUE;
     const nb::SmallPlan p = nb::make_small_jerk_plan(n_i, n_j, sm_count);
     out[0] = p.NW; out[1] = p.KI; out[2] = p.LJ; out[3] = p.WJ; out[4] = p.S; out[5] = p.CS; out[6] = p.tiles_i;
-    out[7] = nb::small_jerk_by_default(n_i, n_j) ? 1 : 0;
+    out[7] = (nb::small_jerk_by_default(n_i, n_j, false) ? 1 : 0) | (nb::small_jerk_by_default(n_i, n_j, true) ? 2 : 0);
     return NB_OK;
 }
 

@@ -18,6 +18,14 @@ def nb():
     return nb_
 
 
+@pytest.fixture(params=["default-kernel", "nb_hermite_kernel"])
+def both_kernels(request, nbdebug):
+    """Small shapes take the small-i-set force + jerk kernel (csrc/nb_small_hermite.cuh) by default: the tests that carry this
+    fixture run a second time with NB_SMALL_JERK=0, on nb_hermite_kernel."""
+    if request.param == "nb_hermite_kernel":
+        nbdebug.setenv("NB_SMALL_JERK", "0")
+
+
 def dev(a):
     import torch
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
@@ -46,6 +54,7 @@ def host(*ts):
     return [t.cpu().numpy() for t in ts]
 
 
+@pytest.mark.usefixtures("both_kernels")
 @pytest.mark.parametrize("n,n_act,seed", [(1500, 1, 0), (1500, 37, 1), (2049, 513, 2), (700, 700, 3), (5000, 2500, 4)])
 def test_one_block_step_matches_oracle(nb, n, n_act, seed):
     """Particles sit at different own times (three levels); a ragged, shuffled active set is advanced to t_now."""
@@ -83,6 +92,7 @@ def test_empty_active_set_is_a_no_op(nb):
     assert nb.last_launch_count() == 0
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_all_active_equals_one_shared_step_bitwise(nb):
     """Everybody due at the same time: the block step is one step of nb_hermite4 (same arithmetic, same kernels)."""
     import torch
@@ -98,6 +108,7 @@ def test_all_active_equals_one_shared_step_bitwise(nb):
     assert np.array_equal(gx, sx) and np.array_equal(gv, sv) and np.array_equal(ga, sa) and np.array_equal(gj, sj)
 
 
+@pytest.mark.usefixtures("both_kernels")
 @pytest.mark.parametrize("n,sub_steps", [(1200, 8), (4096, 4)])
 def test_three_level_schedule_matches_oracle_and_conserves_energy(nb, n, sub_steps):
     """A block-step run: level-L particles are due every 2^L sub-steps; device and oracle follow the same schedule."""
@@ -156,6 +167,7 @@ def test_bench_size_block_steps_sampled_against_oracle(nb):
         assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and ej["acc_rms"] <= 1e-5 and ej["acc_max"] <= 1e-4, (s, e, ej)
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_order_of_the_active_list_does_not_matter_bitwise(nb):
     """A due particle's sum over j runs in a fixed order wherever the particle sits in the i-set (P11 of SURVEY 8.1.3)."""
     n = 3000
@@ -174,6 +186,7 @@ def test_order_of_the_active_list_does_not_matter_bitwise(nb):
         assert np.array_equal(a, b)
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_coincident_particles_and_zero_softening(nb):
     """eps2 = 0 with exact duplicates among the particles (reading R1: a pair at zero distance adds nothing): finite
     results that match the oracle, for a due particle whose twin is due too and for one whose twin is only predicted."""
@@ -232,6 +245,7 @@ def test_runs_on_a_side_stream_and_in_a_cuda_graph(nb):
         assert np.array_equal(a, b)
 
 
+@pytest.mark.usefixtures("both_kernels")
 @pytest.mark.parametrize("case", range(16))
 def test_randomised_block_steps(nb, case):
     """Seeded sweep over sizes, due-set sizes, softening (incl. 0), clock staggering and the block time."""

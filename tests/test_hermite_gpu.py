@@ -26,6 +26,14 @@ def nb():
     return nb_
 
 
+@pytest.fixture(params=["default-kernel", "nb_hermite_kernel"])
+def both_kernels(request, nbdebug):
+    """Small shapes take the small-i-set force + jerk kernel (csrc/nb_small_hermite.cuh) by default: the tests that carry this
+    fixture run a second time with NB_SMALL_JERK=0, on nb_hermite_kernel."""
+    if request.param == "nb_hermite_kernel":
+        nbdebug.setenv("NB_SMALL_JERK", "0")
+
+
 def dev(a):
     import torch
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
@@ -55,6 +63,7 @@ def plummer_xv(n, eps, seed):
     return w.x_j, w.v, w.m_j, w.eps2
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_c0_shape_full_parity(nb):
     x, v, m, eps2 = plummer_xv(2048, 1.0 / 64, 0)
     acc, jerk, pot = gpu_fj(nb, x, v, x, v, m, eps2, alias=True)
@@ -63,6 +72,7 @@ def test_c0_shape_full_parity(nb):
     assert ej["acc_max"] < 2e-5
 
 
+@pytest.mark.usefixtures("both_kernels")
 @pytest.mark.parametrize("n_i,n_j", [(1500, 4999), (31, 1000), (1, 777), (129, 8), (1025, 2051), (4096, 513)])
 def test_ragged_shapes_separate_sets(nb, n_i, n_j):
     xj, vj, mj, eps2 = plummer_xv(n_j, 1.0 / 32, 11)
@@ -114,6 +124,7 @@ def test_list_mode_agrees_bitwise_with_masked_kernel(nb, nbdebug):
     check(out["list"][0][keep], out["list"][1][keep], out["list"][2][keep], ra[keep], rj[keep], rp[keep], "list")
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_coincident_positions_with_other_velocities_add_nothing(nb):
     one = np.array([[1.0, 2.0, 3.0]], dtype=np.float32)
     for eps2 in (0.0, 1e-4):
@@ -122,6 +133,7 @@ def test_coincident_positions_with_other_velocities_add_nothing(nb):
         assert not acc.any() and not jerk.any() and pot[0] == 0.0
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_two_body_exact_cases(nb):
     path = os.path.join(os.path.dirname(__file__), "golden", "hermite_two_body_exact.txt")
     for line in open(path):
@@ -141,6 +153,7 @@ def test_two_body_exact_cases(nb):
         assert pot[0] == pytest.approx(float(-m / s), rel=1e-6)
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_empty_sets_null_pot_and_invalid_arguments(nb):
     import torch
     x, v, m, eps2 = plummer_xv(100, 1.0 / 16, 3)
@@ -160,6 +173,7 @@ def test_empty_sets_null_pot_and_invalid_arguments(nb):
     assert L.nb_force_jerk(5, None, None, 5, None, None, None, 0.1, None, None, None, None) == 1
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_bitwise_reproducible_and_i_permutation_invariant(nb):
     x, v, m, eps2 = plummer_xv(5000, 1.0 / 64, 8)
     a1 = gpu_fj(nb, x, v, x, v, m, eps2, alias=True)
@@ -172,6 +186,7 @@ def test_bitwise_reproducible_and_i_permutation_invariant(nb):
         assert np.array_equal(p[perm], q)
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_jerk_momentum_antisymmetry_fp32(nb):
     x, v, m, eps2 = plummer_xv(4096, 1.0 / 64, 9)
     acc, jerk, _ = gpu_fj(nb, x, v, x, v, m, eps2, alias=True)
@@ -192,6 +207,7 @@ def test_h1_full_size_all_elements(nb):
     assert tot <= 1e-5 * (m[:, None] * np.linalg.norm(jerk, axis=1)[:, None]).sum()
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_force_jerk_host_matches_device_path(nb):
     x, v, m, eps2 = plummer_xv(3000, 1.0 / 64, 15)
     a_d, j_d, p_d = gpu_fj(nb, x, v, x, v, m, eps2, alias=True)

@@ -18,6 +18,14 @@ def nb():
     return nb_
 
 
+@pytest.fixture(params=["default-kernel", "nb_hermite_kernel"])
+def both_kernels(request, nbdebug):
+    """Small shapes take the small-i-set force + jerk kernel (csrc/nb_small_hermite.cuh) by default: the tests that carry this
+    fixture run a second time with NB_SMALL_JERK=0, on nb_hermite_kernel."""
+    if request.param == "nb_hermite_kernel":
+        nbdebug.setenv("NB_SMALL_JERK", "0")
+
+
 def dev(a):
     import torch
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
@@ -31,6 +39,7 @@ def run_gpu(nb, w, dt, steps):
     return x.cpu().numpy(), v.cpu().numpy(), acc.cpu().numpy(), jerk.cpu().numpy(), pot.cpu().numpy()
 
 
+@pytest.mark.usefixtures("both_kernels")
 @pytest.mark.parametrize("n,steps", [(300, 20), (1024, 8), (2049, 3)])
 def test_matches_oracle_integrator(nb, n, steps):
     w = wl.plummer_workload(n, 1.0 / 64, seed=4, with_velocities=True)
@@ -43,6 +52,7 @@ def test_matches_oracle_integrator(nb, n, steps):
     assert e["acc_rms"] <= 1e-4 and e["pot_rms"] <= 1e-5 and ej["acc_rms"] <= 1e-3      # values at the FP32 trajectory's state
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_zero_steps_is_a_force_jerk_evaluation(nb):
     w = wl.plummer_workload(700, 1.0 / 64, seed=5, with_velocities=True)
     x, v, acc, jerk, pot = run_gpu(nb, w, 1.0 / 128, 0)
@@ -53,6 +63,7 @@ def test_zero_steps_is_a_force_jerk_evaluation(nb):
     assert e["acc_rms"] <= 1e-5 and e["acc_max"] <= 1e-4 and e["pot_rms"] <= 1e-5 and ej["acc_rms"] <= 1e-5
 
 
+@pytest.mark.usefixtures("both_kernels")
 def test_energy_error_below_leapfrog_and_momentum(nb):
     import torch
     w = wl.plummer_workload(4096, 1.0 / 32, seed=6, with_velocities=True)
