@@ -271,6 +271,13 @@ nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count, bool jerk = false) 
     return p;
 }
 
+// Steps captured into ONE graph by nb_leapfrog_kdk / nb_hermite4 (at most 8; fewer for short runs so that the graph is replayed
+// at least four times)
+int64_t graph_steps(int64_t remaining) {
+    const int64_t u = remaining / 4;
+    return u < 1 ? 1 : (u > 8 ? 8 : u);
+}
+
 // the small-i-set kernel's planner scores ~1000 candidate decompositions (~10 us): the same table serves repeated shapes
 nb::SmallPlan cached_small_plan(int64_t n_i, int64_t n_j, int sm_count) {
     const auto key = std::make_tuple(nb::small_plan_key_i(n_i), n_j, sm_count);
@@ -1154,11 +1161,16 @@ int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, f
         if (step_graph && s == 2) {                                    // steps 0 and 1 ran eagerly: everything is warm
             cudaGraph_t graph = nullptr;
             cudaGraphExec_t exec = nullptr;
+            // several steps per graph: one cudaGraphLaunch costs the host ~2 us, as much as a step of a small system
+            const int64_t unroll = graph_steps(n_steps - 1 - s);
             NB_CUDA(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
-            nb::nb_kick_drift_kernel<true><<<blocks, threads, 0, stream>>>(x, v, acc_io, n3, h, dt);
-            t_launches = 0;
-            rc = force_impl(n, x, n, x, m, eps2, acc_io, nullptr, stream);
-            const int64_t per_step = t_launches + 1;
+            int64_t per_step = 0;
+            for (int64_t u = 0; u < unroll && rc == NB_OK; ++u) {
+                nb::nb_kick_drift_kernel<true><<<blocks, threads, 0, stream>>>(x, v, acc_io, n3, h, dt);
+                t_launches = 0;
+                rc = force_impl(n, x, n, x, m, eps2, acc_io, nullptr, stream);
+                per_step = t_launches + 1;
+            }
             cudaError_t ce = cudaStreamEndCapture(stream, &graph);
             if (rc != NB_OK || ce != cudaSuccess) {
                 if (graph) (void)cudaGraphDestroy(graph);
@@ -1167,12 +1179,12 @@ int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, f
                 return NB_ERR_CUDA;
             }
             NB_CUDA(cudaGraphInstantiate(&exec, graph, 0));
-            const int64_t replays = n_steps - 1 - s;                   // steps s .. n_steps-2
+            const int64_t replays = (n_steps - 1 - s) / unroll;        // steps s .. n_steps-2, `unroll` at a time
             for (int64_t r = 0; r < replays; ++r) NB_CUDA(cudaGraphLaunch(exec, stream));
             (void)cudaGraphExecDestroy(exec);                          // freed by the runtime once the replays have run
             (void)cudaGraphDestroy(graph);
-            launches += per_step * replays;
-            s += replays;                                              // the last step follows eagerly (it wants phi)
+            launches += per_step * replays * unroll;
+            s += replays * unroll;                                     // what is left (< unroll steps, and the last, which wants phi) runs eagerly
         }
         if (s == 0)
             nb::nb_kick_drift_kernel<false><<<blocks, threads, 0, stream>>>(x, v, acc_io, n3, h, dt);
@@ -1298,13 +1310,17 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
         if (step_graph && s == 2 && n_steps - 1 - s > 0) {             // steps 0 and 1 ran eagerly: everything is warm
             cudaGraph_t graph = nullptr;
             cudaGraphExec_t exec = nullptr;
+            const int64_t unroll = graph_steps(n_steps - 1 - s);       // several steps per graph, as nb_leapfrog_kdk
             NB_CUDA(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
-            t_launches = 0;
-            rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, nullptr, stream, true);
-            int64_t per_step = t_launches;
-            if (rc == NB_OK) {
-                const int k = close_step(false);
-                if (k < 0) rc = NB_ERR_CUDA; else per_step += k;
+            int64_t per_step = 0;
+            for (int64_t u = 0; u < unroll && rc == NB_OK; ++u) {
+                t_launches = 0;
+                rc = force_jerk_impl(n, xp, vp, n, xp, vp, m, eps2, a1, j1, nullptr, stream, true);
+                per_step = t_launches;
+                if (rc == NB_OK) {
+                    const int k = close_step(false);
+                    if (k < 0) rc = NB_ERR_CUDA; else per_step += k;
+                }
             }
             cudaError_t ce = cudaStreamEndCapture(stream, &graph);
             if (rc != NB_OK || ce != cudaSuccess) {
@@ -1314,12 +1330,12 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
                 return NB_ERR_CUDA;
             }
             NB_CUDA(cudaGraphInstantiate(&exec, graph, 0));
-            const int64_t replays = n_steps - 1 - s;                   // steps s .. n_steps-2
+            const int64_t replays = (n_steps - 1 - s) / unroll;        // steps s .. n_steps-2, `unroll` at a time
             for (int64_t r = 0; r < replays; ++r) NB_CUDA(cudaGraphLaunch(exec, stream));
             (void)cudaGraphExecDestroy(exec);                          // freed by the runtime once the replays have run
             (void)cudaGraphDestroy(graph);
-            launches += per_step * replays;
-            s += replays;                                              // the last step follows eagerly (it wants phi)
+            launches += per_step * replays * unroll;
+            s += replays * unroll;                                     // what is left (< unroll steps, and the last, which wants phi) runs eagerly
         }
         const bool last = s + 1 == n_steps;
         t_launches = 0;
