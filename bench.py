@@ -349,10 +349,11 @@ class Problem:
             self.n_out = w.n_j
             self.cycles_done = 0
         elif op == "jerk":
-            w = wl.plummer_workload(131072, 1.0 / 256, seed=1, name="H1", with_velocities=True)
+            n_h = cfg_name if isinstance(cfg_name, int) else 131072       # --n N: the N-scan of row f1
+            w = wl.plummer_workload(n_h, 1.0 / 256, seed=1, name="H1" if n_h == 131072 else f"plummer{n_h}", with_velocities=True)
             self.w, self.pairs = w, float(w.n_i) * float(w.n_j)
-            self.name = (f"row f1 (H1): {w.meta.get('model', '')} with Aarseth velocities, n_i=n_j={w.n_j}, "
-                         f"eps2={w.eps2:.6g}, seed=1, one nb_force_jerk call with phi (configs[1]'s particles)")
+            self.name = (f"row f1 ({'H1' if n_h == 131072 else 'N-scan'}): {w.meta.get('model', '')} with Aarseth velocities, n_i=n_j={w.n_j}, "
+                         f"eps2={w.eps2:.6g}, seed=1, one nb_force_jerk call with phi" + (" (configs[1]'s particles)" if n_h == 131072 else ""))
             self.host = [w.x_j, w.v, w.m_j]
             self.n_out = w.n_i
         elif op == "batched_indexed":
@@ -483,7 +484,8 @@ class Problem:
         if self.op == "leapfrog":
             return self.nb.plan_query(self.w.n_j, self.w.n_j, sm_count)
         if self.op == "jerk":
-            return self.nb.plan_query_jerk(self.w.n_i, self.w.n_j, sm_count)
+            sp = self.nb.plan_query_small_jerk(self.w.n_i, self.w.n_j, sm_count)
+            return dict(sp, kernel="nb_small_hermite_kernel") if sp["default"] else self.nb.plan_query_jerk(self.w.n_i, self.w.n_j, sm_count)
         if self.op == "block":
             return {str(int(a.size)): self.nb.plan_query_jerk(int(a.size), self.w.n_j, sm_count) for a in self.active[:3]}
         return {"cta": "one row of CTAs, 8 warps split each list (WJ = 8), no split across CTAs"}
@@ -548,7 +550,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
     ap.add_argument("--op", default="force", choices=sorted(OPS))
-    ap.add_argument("--n", type=int, default=0, help="--op force only: an equal-mass Plummer sphere of this N "
+    ap.add_argument("--n", type=int, default=0, help="--op force / jerk: an equal-mass Plummer sphere of this N "
                     "(eps = 1/256, seed 1) instead of a BASELINE.json config; for the N-scan in profiles/")
     ap.add_argument("--n-i", type=int, default=0, help="with --n N: the i-set is a seeded random subset of this many of the "
                     "N particles (C2's recipe at another shape)")
@@ -588,7 +590,7 @@ def main():
     op = OPS[args.op]
 
     # inputs resident in HBM before the timed region
-    prob = Problem(args.op, ((args.n, args.n_i) if 0 < args.n_i < args.n else args.n) if (args.n > 0 and args.op == "force") else args.config, nb, torch, wl)
+    prob = Problem(args.op, ((args.n, args.n_i) if 0 < args.n_i < args.n else args.n) if (args.n > 0 and args.op in ("force", "jerk")) else args.config, nb, torch, wl)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
     if args.shard:
@@ -642,7 +644,7 @@ def main():
     # host's cudaGraphLaunch rate (~8 us per replay), not the device
     graph_ms = None
     GRAPH_CALLS, GRAPH_REPLAYS = 50, 8
-    if args.op == "force" and not args.shard and prob.pairs < 2.0 ** 30:
+    if args.op in ("force", "jerk") and not args.shard and prob.pairs < 2.0 ** 30:
         gs = torch.cuda.Stream()
         with torch.cuda.stream(gs):
             for _ in range(3):
@@ -694,7 +696,9 @@ def main():
         roofline = {
             "bound": "alu",
             "kernel": ("nb_small_kernel (small-i-set kernel: pair interaction packed over j, rows a1-a7 in one launch)"
-                       if args.op == "force" and nb.plan_query_small(prob.w.n_i, prob.w.n_j, sm_count)["default"] else op["kernel"]),
+                       if args.op == "force" and nb.plan_query_small(prob.w.n_i, prob.w.n_j, sm_count)["default"] else
+                       "nb_small_hermite_kernel (small-i-set force + jerk kernel, packed over j, one launch)"
+                       if args.op == "jerk" and nb.plan_query_small_jerk(prob.w.n_i, prob.w.n_j, sm_count)["default"] else op["kernel"]),
             "achieved": achieved / 1e12, "peak": peak_inst / 1e12, "unit": "FP32-pipe Tinst/s",
             "frac": achieved / peak_inst, "traffic": traffic,
             "traffic_unit": "DRAM bytes per launch of the dominant kernel",
@@ -729,7 +733,7 @@ def main():
         }
         if graph_ms is not None:
             out["graph_replay"] = {"ms_per_call": graph_ms, "value": pairs / (graph_ms * 1e-3), "unit": METRIC,
-                                   "note": f"{GRAPH_CALLS} nb_force calls captured into one CUDA graph, replayed {GRAPH_REPLAYS}x back to "
+                                   "note": f"{GRAPH_CALLS} calls captured into one CUDA graph, replayed {GRAPH_REPLAYS}x back to "
                                            "back, per call; L2 warm (device time per call: a one-call graph replayed from Python "
                                            "measures the host's launch rate instead)"}
         if args.op == "block":
