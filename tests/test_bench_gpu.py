@@ -40,3 +40,12 @@ def test_every_op_prints_a_line(op):
     d = _run("--op", op, "--steps", "1", "--warmup", "3", "--no-cpu-baseline")
     assert d["config"]["op"] == op and d["value"] > 0 and d["gpu_launches"] > 0
     assert 0.0 < d["roofline"]["frac"] < 1.0 and d["e2e"]["value"] > 0
+
+
+def test_small_force_jerk_line_with_parity_and_graph_replay():
+    d = _run("--op", "jerk", "--n", "1024", "--steps", "5", "--warmup", "3", "--check", "--no-cpu-baseline")
+    assert d["config"]["plan"]["kernel"] == "nb_small_hermite_kernel" and "nb_small_hermite_kernel" in d["roofline"]["kernel"]
+    assert d["gpu_launches"] == 5                      # one launch per call: the kernel packs the j-records itself
+    p = d["parity"]
+    assert p["acc_rms"] <= 1e-5 and p["acc_max"] <= 1e-4 and p["jerk_rms"] <= 1e-5 and p["jerk_max"] <= 1e-4 and p["pot_rms"] <= 1e-5
+    assert 0.0 < d["graph_replay"]["ms_per_call"] < d["ms_per_step"]
