@@ -16,7 +16,7 @@
  *   NB_SMALL_JERK      "0" | "1"                  never / always route nb_force_jerk (and the Hermite steps) through the
  *                                                 small-i-set force + jerk kernel
  *   NB_SMALL_JERK_PLAN "NW,LJ,WJ,S,CS"            its decomposition (nb_plan_query_small_jerk's out[0], out[2..5])
- *   NB_SMALL_PDL       "0" | "1"                  small-i-set kernel: plain launch / programmatic stream serialisation (default)
+ *   NB_SMALL_PDL       "0" | "1"                  small-i-set kernels (force, force + jerk): plain launch / programmatic stream serialisation (default)
  *   NB_MASK            "exact" | "bloom" | "list" where coincident pairs are found; also switches
  *                                                 the acceleration-only shortcut off
  *   NB_FUSED_REDUCE    "0" | "1"                  second pass of the j-split as a separate launch / inside the force kernel
