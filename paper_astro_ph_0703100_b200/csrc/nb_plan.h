@@ -452,7 +452,8 @@ inline SmallPlan make_small_jerk_plan(int64_t n_i_exact, int64_t n_j, int sm_cou
 
 // Which evaluations take it (per call from a CUDA graph, best plan of this kernel against nb_hermite_kernel's;
 // profiles/r02_small_jerk.md).
-//  * Hermite steps (nb_hermite4, nb_hermite4_block_step), whose predictor has packed the j-records: up to 2^22 pairs --
+//  * Hermite steps (nb_hermite4, nb_hermite4_block_step), whose predictor has packed the j-records: up to 2^22 pairs (2^23
+//    for at most 512 i-particles) --
 //    256 x 256: 5.3 against 7.8 us, 100 x 10000: 9.2 against 14.5, 64 x 65536: 15.6 against 26.1, 2048 x 2048: 12.5 against
 //    13.4; a tie at 1024 x 4096, and beyond nb_hermite_kernel wins (2048 x 8192: 28.9 against 26.2, 256 x 65536: 31.6 against
 //    30.0): ONE i-particle per thread gives the loop no more independent chains than the i-packed K = 2 / 4 body.
@@ -462,13 +463,16 @@ inline SmallPlan make_small_jerk_plan(int64_t n_i_exact, int64_t n_j, int sm_cou
 //    2048 x 65536: 157 against 148.
 constexpr int64_t kSmallJerkMaxI = 4096;
 constexpr double kSmallJerkMaxPairs = 4194304.0;           // 2^22: records already packed
+constexpr int64_t kSmallJerkStepsNarrowI = 512;
+constexpr double kSmallJerkMaxPairsNarrow = 8388608.0;     // 2^23: records already packed, n_i <= 512 (block steps: 128 of
+                                                           // 65536 active 25.9 against 31.3 us, 512 of 16384 26.0 against 27.1)
 constexpr double kSmallJerkMaxPairsRaw = 33554432.0;       // 2^25: nb_force_jerk
 constexpr int64_t kSmallJerkNarrowI = 1024;
 constexpr double kSmallJerkMaxPairsRawNarrow = 67108864.0; // 2^26: nb_force_jerk, n_i <= 1024
 inline bool small_jerk_by_default(int64_t n_i, int64_t n_j, bool prepacked) {
     const double pairs = (double)n_i * (double)n_j;
     if (n_i > kSmallJerkMaxI) return false;
-    if (prepacked) return pairs <= kSmallJerkMaxPairs;
+    if (prepacked) return pairs <= kSmallJerkMaxPairs || (n_i <= kSmallJerkStepsNarrowI && pairs <= kSmallJerkMaxPairsNarrow);
     return pairs <= kSmallJerkMaxPairsRaw || (n_i <= kSmallJerkNarrowI && pairs <= kSmallJerkMaxPairsRawNarrow);
 }
 

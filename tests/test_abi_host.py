@@ -187,7 +187,7 @@ def test_small_jerk_planner_invariants():
         assert p["tile_i"] == (p["NW"] // p["WJ"]) * (32 // p["LJ"])
         assert p["tiles_i"] * p["tile_i"] >= n_i > (p["tiles_i"] - 1) * p["tile_i"]
         assert p["CS"] in (1, 2, 4, 8) and p["S"] % p["CS"] == 0 and p["tile_i"] % p["CS"] == 0 and 1 <= p["S"] <= 2048
-        assert p["default_steps"] == int(n_i <= 4096 and n_i * n_j <= 2 ** 22)
+        assert p["default_steps"] == int(n_i <= 4096 and (n_i * n_j <= 2 ** 22 or (n_i <= 512 and n_i * n_j <= 2 ** 23)))
         assert p["default"] == int(n_i <= 4096 and (n_i * n_j <= 2 ** 25 or (n_i <= 1024 and n_i * n_j <= 2 ** 26)))
         assert p == nb.plan_query_small_jerk(n_i, n_j, 148)
 
