@@ -421,7 +421,7 @@ int nb_profile_read(int64_t *n_launches, double *total_ms);
  * out[7] = 1 if nb_force takes this kernel for (n_i, n_j) by default */
 int nb_plan_query_small(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]);
 /* The same for the small-i-set force + jerk kernel (csrc/nb_small_hermite.cuh; KI = 1): out[7] bit 0 = nb_force_jerk takes
- * it for (n_i, n_j) by default (up to 2^25 pairs; the kernel packs the j-records itself), bit 1 = nb_hermite4 and
+ * it for (n_i, n_j) by default (up to 2^25 pairs, more for narrow i-sets; the kernel packs the j-records itself), bit 1 = nb_hermite4 and
  * nb_hermite4_block_step do (up to 2^22 pairs, 2^23 for at most 512 active particles; their predictor has packed the records). */
 int nb_plan_query_small_jerk(int64_t n_i, int64_t n_j, int sm_count, int64_t out[8]);
 

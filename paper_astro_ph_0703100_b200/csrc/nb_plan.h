@@ -469,11 +469,14 @@ constexpr double kSmallJerkMaxPairsNarrow = 8388608.0;     // 2^23: records alre
 constexpr double kSmallJerkMaxPairsRaw = 33554432.0;       // 2^25: nb_force_jerk
 constexpr int64_t kSmallJerkNarrowI = 1024;
 constexpr double kSmallJerkMaxPairsRawNarrow = 67108864.0; // 2^26: nb_force_jerk, n_i <= 1024
+constexpr int64_t kSmallJerkVeryNarrowI = 256;             // ... and 2^28 for n_i <= 256: nb_pack_jv_kernel over a long j-set costs
+constexpr double kSmallJerkMaxPairsRawVeryNarrow = 268435456.0;   // more than the loop gains (128 x 2^20: 166 against 202 us)
 inline bool small_jerk_by_default(int64_t n_i, int64_t n_j, bool prepacked) {
     const double pairs = (double)n_i * (double)n_j;
     if (n_i > kSmallJerkMaxI) return false;
     if (prepacked) return pairs <= kSmallJerkMaxPairs || (n_i <= kSmallJerkStepsNarrowI && pairs <= kSmallJerkMaxPairsNarrow);
-    return pairs <= kSmallJerkMaxPairsRaw || (n_i <= kSmallJerkNarrowI && pairs <= kSmallJerkMaxPairsRawNarrow);
+    return pairs <= kSmallJerkMaxPairsRaw || (n_i <= kSmallJerkNarrowI && pairs <= kSmallJerkMaxPairsRawNarrow) ||
+           (n_i <= kSmallJerkVeryNarrowI && pairs <= kSmallJerkMaxPairsRawVeryNarrow);
 }
 
 }  // namespace nb

@@ -89,7 +89,7 @@ def test_ragged_shapes_default_plan(nb, n_i, n_j, nbdebug):
 
 def test_default_choice_and_its_edges(nb):
     for n_i, n_j, small in [(2048, 2048, 1), (4096, 8192, 1), (4096, 8193, 0), (1024, 65536, 1), (1025, 65536, 0), (300, 300, 1),
-                            (4097, 1023, 0)]:
+                            (4097, 1023, 0), (256, 1048576, 1), (257, 1048576, 0)]:
         assert nb.plan_query_small_jerk(n_i, n_j)["default"] == small
         xi, vi, xj, vj, mj, eps2 = subset_case(max(n_j, n_i), n_i, 1.0 / 128, n_i + n_j)
         xj, vj, mj = xj[:n_j], vj[:n_j], mj[:n_j]
