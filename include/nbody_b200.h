@@ -83,7 +83,7 @@ typedef enum nb_status {
  * Inputs are not validated on the device: non-finite or |x| > ~1e18 inputs give undefined values.
  * Uses an internal per-stream workspace (packed j records, j-split partial sums) that grows on
  * demand with stream-ordered allocation; once warm the call is CUDA-graph capturable (see "CUDA graphs" above).
- * Calls with few i-particles (n_i <= 512 up to 2^26 pairs, n_i <= 4096 up to 2^25 pairs: BASELINE.json configs[0] and
+ * Calls with few i-particles (n_i <= 512 up to 2^26 pairs, n_i <= 4096 up to 2^25 pairs, n_i <= 32 up to 2^29 pairs: BASELINE.json configs[0] and
  * [2]) run as ONE launch of the small-i-set kernel (packed over j; the j-split is summed through lanes, warps, a
  * thread-block cluster or ticketed FP64 partials); larger ones as pack (+ coincidence pre-pass) + force kernel (+ second pass).
  */

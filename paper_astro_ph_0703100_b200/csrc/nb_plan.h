@@ -221,9 +221,12 @@ constexpr int64_t kSmallMaxI = 4096;
 constexpr int64_t kSmallNarrowI = 512;
 constexpr double kSmallMaxPairsNarrow = 67108864.0;    // 2^26, n_i <= 512
 constexpr double kSmallMaxPairs = 33554432.0;          // 2^25, n_i <= 4096
+constexpr int64_t kSmallVeryNarrowI = 32;              // a handful of i-particles against a long j-set: nb_force_kernel's pack pass over
+constexpr double kSmallMaxPairsVeryNarrow = 536870912.0;   // the j-set costs more than the loop (2^29; 32 x 2^23: 177 against 299 us)
 inline bool small_by_default(int64_t n_i, int64_t n_j) {
     const double pairs = (double)n_i * (double)n_j;
-    return (n_i <= kSmallNarrowI && pairs <= kSmallMaxPairsNarrow) || (n_i <= kSmallMaxI && pairs <= kSmallMaxPairs);
+    return (n_i <= kSmallNarrowI && pairs <= kSmallMaxPairsNarrow) || (n_i <= kSmallMaxI && pairs <= kSmallMaxPairs) ||
+           (n_i <= kSmallVeryNarrowI && pairs <= kSmallMaxPairsVeryNarrow);
 }
 constexpr int kSmallRoundJPlan = 4096;           // = nb::kSmallRoundJ (nb_small.cuh)
 
@@ -471,12 +474,14 @@ constexpr int64_t kSmallJerkNarrowI = 1024;
 constexpr double kSmallJerkMaxPairsRawNarrow = 67108864.0; // 2^26: nb_force_jerk, n_i <= 1024
 constexpr int64_t kSmallJerkVeryNarrowI = 256;             // ... and 2^28 for n_i <= 256: nb_pack_jv_kernel over a long j-set costs
 constexpr double kSmallJerkMaxPairsRawVeryNarrow = 268435456.0;   // more than the loop gains (128 x 2^20: 166 against 202 us)
+constexpr double kSmallJerkMaxPairsRawHandful = 536870912.0;      // 2^29 for n_i <= 32 (32 x 2^23: 369 against 653 us)
 inline bool small_jerk_by_default(int64_t n_i, int64_t n_j, bool prepacked) {
     const double pairs = (double)n_i * (double)n_j;
     if (n_i > kSmallJerkMaxI) return false;
     if (prepacked) return pairs <= kSmallJerkMaxPairs || (n_i <= kSmallJerkStepsNarrowI && pairs <= kSmallJerkMaxPairsNarrow);
     return pairs <= kSmallJerkMaxPairsRaw || (n_i <= kSmallJerkNarrowI && pairs <= kSmallJerkMaxPairsRawNarrow) ||
-           (n_i <= kSmallJerkVeryNarrowI && pairs <= kSmallJerkMaxPairsRawVeryNarrow);
+           (n_i <= kSmallJerkVeryNarrowI && pairs <= kSmallJerkMaxPairsRawVeryNarrow) ||
+           (n_i <= kSmallVeryNarrowI && pairs <= kSmallJerkMaxPairsRawHandful);
 }
 
 }  // namespace nb

@@ -189,7 +189,7 @@ def test_small_jerk_planner_invariants():
         assert p["CS"] in (1, 2, 4, 8) and p["S"] % p["CS"] == 0 and p["tile_i"] % p["CS"] == 0 and 1 <= p["S"] <= 2048
         assert p["default_steps"] == int(n_i <= 4096 and (n_i * n_j <= 2 ** 22 or (n_i <= 512 and n_i * n_j <= 2 ** 23)))
         assert p["default"] == int(n_i <= 4096 and (n_i * n_j <= 2 ** 25 or (n_i <= 1024 and n_i * n_j <= 2 ** 26) or
-                                                    (n_i <= 256 and n_i * n_j <= 2 ** 28)))
+                                                    (n_i <= 256 and n_i * n_j <= 2 ** 28) or (n_i <= 32 and n_i * n_j <= 2 ** 29)))
         assert p == nb.plan_query_small_jerk(n_i, n_j, 148)
 
 

@@ -89,9 +89,9 @@ def test_c0_and_c2_take_the_small_kernel_by_default(nb):
 
 
 @pytest.mark.parametrize("n_i,n_j,small", [(4096, 8192, 1), (4097, 8191, 0), (4096, 8193, 0), (512, 131072, 1), (513, 131072, 0),
-                                           (3000, 3000, 1), (4096, 2048, 1), (40, 1600000, 1)])
+                                           (3000, 3000, 1), (4096, 2048, 1), (40, 1600000, 1), (32, 4194304, 1), (33, 4194304, 0)])
 def test_the_edges_of_the_default_choice(nb, n_i, n_j, small):
-    """`small_by_default` (nb_plan.h): n_i <= 512 up to 2^26 pairs, n_i <= 4096 up to 2^25 pairs.  On both sides of every
+    """`small_by_default` (nb_plan.h): n_i <= 512 up to 2^26 pairs, n_i <= 4096 up to 2^25 pairs, n_i <= 32 up to 2^29 pairs.  On both sides of every
     edge nb_force -- no switch set -- matches the oracle on a sample of the i-particles, all of which coincide with a j."""
     assert nb.plan_query_small(n_i, n_j)["default"] == small
     if n_i <= n_j:
