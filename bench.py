@@ -349,12 +349,18 @@ class Problem:
             self.n_out = w.n_j
             self.cycles_done = 0
         elif op == "jerk":
-            n_h = cfg_name if isinstance(cfg_name, int) else 131072       # --n N: the N-scan of row f1
+            n_sub = cfg_name[1] if isinstance(cfg_name, tuple) else 0     # --n N --n-i M: an active subset (C2's recipe)
+            n_h = cfg_name[0] if isinstance(cfg_name, tuple) else (cfg_name if isinstance(cfg_name, int) else 131072)   # --n N: the N-scan of row f1
             w = wl.plummer_workload(n_h, 1.0 / 256, seed=1, name="H1" if n_h == 131072 else f"plummer{n_h}", with_velocities=True)
+            if n_sub:
+                import dataclasses
+                idx = np.sort(np.random.default_rng(1).choice(n_h, n_sub, replace=False))
+                w = dataclasses.replace(w, x_i=np.ascontiguousarray(w.x_j[idx]), i_index=idx.astype(np.int64), name=f"subset{n_sub}of{n_h}")
             self.w, self.pairs = w, float(w.n_i) * float(w.n_j)
-            self.name = (f"row f1 ({'H1' if n_h == 131072 else 'N-scan'}): {w.meta.get('model', '')} with Aarseth velocities, n_i=n_j={w.n_j}, "
-                         f"eps2={w.eps2:.6g}, seed=1, one nb_force_jerk call with phi" + (" (configs[1]'s particles)" if n_h == 131072 else ""))
-            self.host = [w.x_j, w.v, w.m_j]
+            self.name = (f"row f1 ({'H1' if n_h == 131072 and not n_sub else 'shape scan'}): {w.meta.get('model', '')} with Aarseth velocities, "
+                         f"n_i={w.n_i}, n_j={w.n_j}, eps2={w.eps2:.6g}, seed=1, one nb_force_jerk call with phi"
+                         + (" (configs[1]'s particles)" if n_h == 131072 and not n_sub else ""))
+            self.host = [w.x_j, w.v, w.m_j] + ([w.x_i, np.ascontiguousarray(w.v[w.i_index])] if n_sub else [])
             self.n_out = w.n_i
         elif op == "batched_indexed":
             w = wl.tree_list_workload(524288, 32, 256, 2000, 6000, 1.0 / 128, seed=7, name="T1")
@@ -426,7 +432,8 @@ class Problem:
         elif self.op == "batched_indexed":
             nb.force_batched_indexed(t[0], t[1], t[2], t[3], t[4], w.eps2, acc_out=self.outs[0], pot_out=self.outs[1])
         elif self.op == "jerk":
-            nb.force_jerk(t[0], t[1], t[0], t[1], t[2], w.eps2, acc_out=self.outs[0], jerk_out=self.outs[1], pot_out=self.outs[2])
+            xi, vi = (t[3], t[4]) if len(t) > 3 else (t[0], t[1])
+            nb.force_jerk(xi, vi, t[0], t[1], t[2], w.eps2, acc_out=self.outs[0], jerk_out=self.outs[1], pot_out=self.outs[2])
         else:
             nb.force_batched(t[0], t[1], t[2], t[3], t[4], w.eps2, acc_out=self.outs[0], pot_out=self.outs[1])
 
@@ -440,7 +447,7 @@ class Problem:
             return
         if self.op == "jerk":
             h = [p.numpy() for p in self.pinned]
-            nb.force_jerk_host(h[0], h[1], h[0], h[1], h[2], w.eps2, acc_out=self.h_outs[0].numpy(),
+            nb.force_jerk_host(h[3] if len(h) > 3 else h[0], h[4] if len(h) > 3 else h[1], h[0], h[1], h[2], w.eps2, acc_out=self.h_outs[0].numpy(),
                                jerk_out=self.h_outs[1].numpy(), pot_out=self.h_outs[2].numpy())
             return
         staged = [p.cuda(non_blocking=True) for p in self.pinned]
@@ -520,7 +527,8 @@ def oracle_rate_op(op, w, target_seconds, rng_seed=0):
     if op == "jerk":
         def run(n_i):
             idx = np.sort(rng.choice(w.n_i, n_i, replace=False))
-            xi, vi = np.ascontiguousarray(w.x_j[idx]), np.ascontiguousarray(w.v[idx])
+            v_all = w.v if w.i_index is None else w.v[w.i_index]
+            xi, vi = np.ascontiguousarray(w.xi[idx]), np.ascontiguousarray(v_all[idx])
             t0 = time.perf_counter()
             oracle.force_jerk(xi, vi, w.x_j, w.v, w.m_j, w.eps2)
             return time.perf_counter() - t0
@@ -552,7 +560,7 @@ def main():
     ap.add_argument("--op", default="force", choices=sorted(OPS))
     ap.add_argument("--n", type=int, default=0, help="--op force / jerk: an equal-mass Plummer sphere of this N "
                     "(eps = 1/256, seed 1) instead of a BASELINE.json config; for the N-scan in profiles/")
-    ap.add_argument("--n-i", type=int, default=0, help="with --n N: the i-set is a seeded random subset of this many of the "
+    ap.add_argument("--n-i", type=int, default=0, help="with --n N (--op force / jerk): the i-set is a seeded random subset of this many of the "
                     "N particles (C2's recipe at another shape)")
     ap.add_argument("--shard", action="store_true", help="--op force only: i-shard ONE problem over the ranks (row f4: "
                     "all-gather of the packed j records over NCCL, then nb_force_packed on the local i-slice; strong "
@@ -590,7 +598,8 @@ def main():
     op = OPS[args.op]
 
     # inputs resident in HBM before the timed region
-    prob = Problem(args.op, ((args.n, args.n_i) if 0 < args.n_i < args.n else args.n) if (args.n > 0 and args.op in ("force", "jerk")) else args.config, nb, torch, wl)
+    prob = Problem(args.op, ((args.n, args.n_i) if 0 < args.n_i < args.n else args.n) if (args.n > 0 and args.op in ("force", "jerk")) else args.config,
+                   nb, torch, wl)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
     if args.shard:
@@ -820,7 +829,8 @@ def main():
                     ra, rp = oracle.force(w.xi[idx], w.x_j, w.m_j, w.eps2)
                     par = oracle.error_metrics(got[0], ra, got[1], rp)
                 else:
-                    ra, rj, rp = oracle.force_jerk(w.x_j[idx], w.v[idx], w.x_j, w.v, w.m_j, w.eps2)
+                    v_all = w.v if w.i_index is None else w.v[w.i_index]
+                    ra, rj, rp = oracle.force_jerk(w.xi[idx], v_all[idx], w.x_j, w.v, w.m_j, w.eps2)
                     par = oracle.error_metrics(got[0], ra, got[2], rp)
                     ej = oracle.error_metrics(got[1], rj)
                     par["jerk_max"], par["jerk_rms"] = ej["acc_max"], ej["acc_rms"]

@@ -49,3 +49,11 @@ def test_small_force_jerk_line_with_parity_and_graph_replay():
     p = d["parity"]
     assert p["acc_rms"] <= 1e-5 and p["acc_max"] <= 1e-4 and p["jerk_rms"] <= 1e-5 and p["jerk_max"] <= 1e-4 and p["pot_rms"] <= 1e-5
     assert 0.0 < d["graph_replay"]["ms_per_call"] < d["ms_per_step"]
+
+
+def test_force_jerk_active_subset_line():
+    d = _run("--op", "jerk", "--n", "16384", "--n-i", "256", "--steps", "3", "--warmup", "3", "--check", "--no-cpu-baseline")
+    assert "n_i=256, n_j=16384" in d["config"]["workload"] and d["config"]["plan"]["kernel"] == "nb_small_hermite_kernel"
+    p = d["parity"]
+    assert p["acc_rms"] <= 1e-5 and p["acc_max"] <= 1e-4 and p["jerk_rms"] <= 1e-5 and p["jerk_max"] <= 1e-4 and p["pot_rms"] <= 1e-5
+    assert d["e2e"]["h2d_bytes_per_step"] == 16384 * 28 + 256 * 24 and d["e2e"]["value"] > 0
