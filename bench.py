@@ -288,10 +288,11 @@ class Problem:
             self.host = [w.x_j, w.m_j] + ([] if w.x_i is None else [w.x_i])
             self.n_out = w.n_i
         elif op == "leapfrog":
-            w = wl.config(4)
+            w = self.integrator_workload(cfg_name, wl)
             self.w = w
             self.pairs = float(w.n_j) ** 2 * (LEAPFROG_KDK_PER_CALL + 1)     # force evaluations per call x N^2
-            self.name = (f"BASELINE.json configs[4] (C4): {w.meta.get('model', '')} with Aarseth velocities, N={w.n_j}, "
+            self.name = ((f"BASELINE.json configs[4] (C4)" if w.name == "C4" else "small system (C4's recipe at another N)") +
+                         f": {w.meta.get('model', '')} with Aarseth velocities, N={w.n_j}, "
                          f"eps2={w.eps2:.6g}, dt=1/512, seed=4; one step = one nb_leapfrog_kdk call of "
                          f"{LEAPFROG_KDK_PER_CALL} KDK steps (the config's 1000 steps = 10 such calls)")
             self.host = [w.x_j, w.v, w.m_j]
@@ -323,7 +324,7 @@ class Problem:
             self.host = [rows, rows]
             self.n_out = rows.shape[0]
         elif op == "hermite":
-            w = wl.config(4)
+            w = self.integrator_workload(cfg_name, wl)
             self.w = w
             self.pairs = float(w.n_j) ** 2 * (LEAPFROG_KDK_PER_CALL + 1)
             self.name = (f"configs[4]'s particles (C4: N={w.n_j}, eps2={w.eps2:.6g}, dt=1/512, seed=4) under the 4th-order Hermite "
@@ -397,6 +398,13 @@ class Problem:
         self.h_outs = [torch.empty(o.shape, dtype=torch.float32).pin_memory() for o in self.outs]
         self.h2d = int(sum(a.nbytes for a in self.host))
         self.d2h = int(sum(o.numel() * 4 for o in self.outs))
+
+    @staticmethod
+    def integrator_workload(cfg_name, wl):
+        """C4, or -- with --n N -- C4's recipe (Plummer sphere with Aarseth velocities, eps = 1/128, dt = 1/512, seed 4) at another N."""
+        if isinstance(cfg_name, int):
+            return wl.plummer_workload(cfg_name, 1.0 / 128, seed=4, name=f"plummer{cfg_name}", with_velocities=True, dt=1.0 / 512, n_steps=1000)
+        return wl.config(4)
 
     def call(self, t=None):
         t = self.dev if t is None else t
@@ -558,7 +566,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
     ap.add_argument("--op", default="force", choices=sorted(OPS))
-    ap.add_argument("--n", type=int, default=0, help="--op force / jerk: an equal-mass Plummer sphere of this N "
+    ap.add_argument("--n", type=int, default=0, help="--op force / jerk (leapfrog / hermite: C4's recipe at this N): an equal-mass Plummer sphere of this N "
                     "(eps = 1/256, seed 1) instead of a BASELINE.json config; for the N-scan in profiles/")
     ap.add_argument("--n-i", type=int, default=0, help="with --n N (--op force / jerk): the i-set is a seeded random subset of this many of the "
                     "N particles (C2's recipe at another shape)")
@@ -596,9 +604,13 @@ def main():
     nb.lib()
     peaks, peaks_kind = load_peaks()
     op = OPS[args.op]
+    if args.op in ("leapfrog", "hermite") and args.n > 0:
+        # small systems replay their steps from a CUDA graph inside the library, which needs a capturable stream: the whole
+        # run (flushes, events, calls) goes to a side stream instead of the default one
+        torch.cuda.set_stream(torch.cuda.Stream())
 
     # inputs resident in HBM before the timed region
-    prob = Problem(args.op, ((args.n, args.n_i) if 0 < args.n_i < args.n else args.n) if (args.n > 0 and args.op in ("force", "jerk")) else args.config,
+    prob = Problem(args.op, ((args.n, args.n_i) if 0 < args.n_i < args.n else args.n) if (args.n > 0 and args.op in ("force", "jerk", "leapfrog", "hermite")) else args.config,
                    nb, torch, wl)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
@@ -631,7 +643,10 @@ def main():
 
     sampler = ClockSampler(physical_gpu_index(local_rank))
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    nb.profile_enable(True)
+    # the library's per-kernel events make every launch of a launch-bound small-system run slower and switch its step graph
+    # off: those lines (--op leapfrog / hermite --n N) are timed without them, their roofline comes from the whole call
+    kernel_events = not (args.op in ("leapfrog", "hermite") and args.n > 0)
+    nb.profile_enable(kernel_events)
     barrier()
     sampler.start()
     t_wall0 = time.perf_counter()
@@ -699,6 +714,9 @@ def main():
         if args.op == "block":
             pairs_k = pairs / BLOCK_SUB_STEPS                                # mean over the cycle's launches (n_act varies)
         k_rate = pairs_k * n_k / (k_ms * 1e-3) if n_k else 0.0
+        if not kernel_events:                                                # whole calls instead of kernels: evaluations / call time
+            n_k, k_ms = args.steps * (LEAPFROG_KDK_PER_CALL + 1), total_ms
+            k_rate = pairs_k * n_k / (k_ms * 1e-3)
         inst = op["inst"]
         achieved = inst * k_rate
         traffic, traffic_kind = modelled_traffic(args, prob, nb, sm_count)
@@ -791,6 +809,8 @@ def main():
                                "note": "every step a new (n_act, n): no plan-cache hit; host wall clock including the planner"}
         if args.op == "hermite":
             out["hermite_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
+        if args.op == "leapfrog":
+            out["kdk_steps_per_s"] = LEAPFROG_KDK_PER_CALL * args.steps / (total_ms * 1e-3)
         if args.op in ("leapfrog", "hermite") and not args.no_cpu_baseline:
             import oracle
             w = prob.w

@@ -271,6 +271,10 @@ nb::Plan cached_plan(int64_t n_i, int64_t n_j, int sm_count, bool jerk = false) 
     return p;
 }
 
+// Capturing and instantiating the step graph costs ~140 us, a replayed step saves ~2 us: from 64 steps on it pays
+// (N = 256 leapfrog: 32 steps 8.7 against 8.2 us per step eagerly, 100 steps 5.7 against 7.3; profiles/r02_small_jerk.md)
+constexpr int64_t kStepGraphMinSteps = 64;
+
 // Steps captured into ONE graph by nb_leapfrog_kdk / nb_hermite4 (at most 8; fewer for short runs so that the graph is replayed
 // at least four times)
 int64_t graph_steps(int64_t remaining) {
@@ -1152,7 +1156,7 @@ int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, f
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     NB_CUDA(cudaStreamIsCapturing(stream, &cap));
     const bool real_stream = reinterpret_cast<uintptr_t>(stream) > 2;   // the default streams cannot be captured
-    const bool step_graph = real_stream && n_steps >= 16 && n <= 32768 && cap == cudaStreamCaptureStatusNone && !t_profile &&
+    const bool step_graph = real_stream && n_steps >= kStepGraphMinSteps && n <= 32768 && cap == cudaStreamCaptureStatusNone && !t_profile &&
                             knobs().step_graph != 0;                    // NB_STEP_GRAPH=0 (nb_debug.h): every step eagerly
     int64_t launches = t_launches;
     for (int64_t s = 0; s < n_steps; ++s) {
@@ -1282,7 +1286,7 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     NB_CUDA(cudaStreamIsCapturing(stream, &cap));
     const bool real_stream = reinterpret_cast<uintptr_t>(stream) > 2;   // the default streams cannot be captured
-    const bool step_graph = real_stream && n_steps >= 16 && n <= 32768 && cap == cudaStreamCaptureStatusNone && !t_profile &&
+    const bool step_graph = real_stream && n_steps >= kStepGraphMinSteps && n <= 32768 && cap == cudaStreamCaptureStatusNone && !t_profile &&
                             knobs().step_graph != 0;                    // NB_STEP_GRAPH=0 (nb_debug.h): every step eagerly
     // A step is two launches: force + jerk on the predicted state, then ONE kernel that corrects the step and predicts + packs
     // the next one (NB_HERMITE_FUSE=0, nb_debug.h: correct and predict as separate launches -- the same bits).

@@ -57,3 +57,11 @@ def test_force_jerk_active_subset_line():
     p = d["parity"]
     assert p["acc_rms"] <= 1e-5 and p["acc_max"] <= 1e-4 and p["jerk_rms"] <= 1e-5 and p["jerk_max"] <= 1e-4 and p["pot_rms"] <= 1e-5
     assert d["e2e"]["h2d_bytes_per_step"] == 16384 * 28 + 256 * 24 and d["e2e"]["value"] > 0
+
+
+@pytest.mark.parametrize("op", ["leapfrog", "hermite"])
+def test_small_system_integrator_line(op):
+    d = _run("--op", op, "--n", "1024", "--steps", "2", "--warmup", "3", "--cpu-seconds", "1")
+    assert "N=1024" in d["config"]["workload"] and d["value"] > 0
+    assert d["energy"]["rel_drift"] < 1e-5 and d["energy"]["time_steps"] == 500
+    assert d["kdk_steps_per_s" if op == "leapfrog" else "hermite_steps_per_s"] > 2e4      # graph-replayed steps: > 20 k steps/s
