@@ -121,6 +121,11 @@ int nb_force_host(int64_t n_i, const float *x_i,
  *   pot_out  device, float [n]: receives phi at the final time; may be NULL
  *
  * n_steps == 0 only evaluates a and phi of the given state.
+ * Small systems (n <= 32768) with n_steps >= 64: the identical middle steps are captured into a CUDA graph (eight steps per
+ * graph) and replayed -- the same launches, the same bits (nb_debug.h: NB_STEP_GRAPH=0 switches it off).  A default stream
+ * (NULL / legacy or per-thread) cannot be captured: the run is then enqueued on a private non-blocking stream of the device
+ * that first waits for the work already enqueued on the caller's stream, and the caller's stream waits for the run before
+ * anything enqueued after the call -- the stream order the caller sees is unchanged.  nb_hermite4 does the same.
  */
 int nb_leapfrog_kdk(int64_t n, float *x, float *v, const float *m,
                     float eps2, float dt, int64_t n_steps,

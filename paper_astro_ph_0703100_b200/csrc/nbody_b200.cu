@@ -282,6 +282,43 @@ int64_t graph_steps(int64_t remaining) {
     return u < 1 ? 1 : (u > 8 ? 8 : u);
 }
 
+// The default streams (NULL / legacy and per-thread) cannot be captured, and they are what most callers pass.  A long run on a
+// small system is then moved to a private non-blocking stream of the device for the duration of the call: the private stream
+// first waits for everything enqueued on the caller's stream so far, the caller's stream then waits for the run -- stream order
+// as the caller sees it is unchanged, and the step graph becomes possible.  Host threads that detour on the same device are
+// serialised for the duration of the enqueue (their work would be serialised on the device anyway).
+struct StreamDetour {
+    struct PerDevice { cudaStream_t stream = nullptr; cudaEvent_t ev_in = nullptr, ev_out = nullptr; std::mutex busy; };
+    static PerDevice& slot(int dev) { static PerDevice table[64]; return table[dev & 63]; }
+    PerDevice* pd = nullptr;
+    cudaStream_t user = nullptr;
+    std::unique_lock<std::mutex> lock;
+    // on success *stream is the private stream
+    int begin(int dev, cudaStream_t user_stream, cudaStream_t* stream) {
+        PerDevice& d = slot(dev);
+        lock = std::unique_lock<std::mutex>(d.busy);
+        if (!d.stream) {
+            NB_CUDA(cudaStreamCreateWithFlags(&d.stream, cudaStreamNonBlocking));
+            NB_CUDA(cudaEventCreateWithFlags(&d.ev_in, cudaEventDisableTiming));
+            NB_CUDA(cudaEventCreateWithFlags(&d.ev_out, cudaEventDisableTiming));
+        }
+        NB_CUDA(cudaEventRecord(d.ev_in, user_stream));
+        NB_CUDA(cudaStreamWaitEvent(d.stream, d.ev_in, 0));
+        pd = &d;
+        user = user_stream;
+        *stream = d.stream;
+        return NB_OK;
+    }
+    ~StreamDetour() {                                                  // on every way out of the call, errors included
+        if (!pd) return;
+        if (cudaEventRecord(pd->ev_out, pd->stream) == cudaSuccess) (void)cudaStreamWaitEvent(user, pd->ev_out, 0);
+    }
+};
+// whether nb_leapfrog_kdk / nb_hermite4 would replay their steps from a graph if the stream allowed it
+bool wants_step_graph(int64_t n, int64_t n_steps) {
+    return n_steps >= kStepGraphMinSteps && n <= 32768 && !t_profile && knobs().step_graph != 0;
+}
+
 // the small-i-set kernel's planner scores ~1000 candidate decompositions (~10 us): the same table serves repeated shapes
 nb::SmallPlan cached_small_plan(int64_t n_i, int64_t n_j, int sm_count) {
     const auto key = std::make_tuple(nb::small_plan_key_i(n_i), n_j, sm_count);
@@ -1142,6 +1179,11 @@ int nb_leapfrog_kdk(int64_t n, float* x, float* v, const float* m, float eps2, f
     int rc = device_info(&dev, &info);
     if (rc != NB_OK) return rc;
     if (n == 0) return NB_OK;
+    StreamDetour detour;                                               // a default stream: run on the device's private stream
+    if (reinterpret_cast<uintptr_t>(stream) <= 2 && wants_step_graph(n, n_steps)) {
+        rc = detour.begin(dev, stream, &stream);
+        if (rc != NB_OK) return rc;
+    }
     const int n3 = (int)(3 * n);
     const int threads = 256, blocks = (n3 + threads - 1) / threads;
     const float h = 0.5f * dt;
@@ -1258,6 +1300,11 @@ int nb_hermite4(int64_t n, float* x, float* v, const float* m, float eps2, float
     int rc = device_info(&dev, &info);
     if (rc != NB_OK) return rc;
     if (n == 0) return NB_OK;
+    StreamDetour detour;                                               // a default stream: run on the device's private stream
+    if (reinterpret_cast<uintptr_t>(stream) <= 2 && wants_step_graph(n, n_steps)) {
+        rc = detour.begin(dev, stream, &stream);
+        if (rc != NB_OK) return rc;
+    }
     const int n3 = (int)(3 * n);
     const int threads = 256, blocks = (n3 + threads - 1) / threads;
     int64_t launches = 0;

@@ -128,3 +128,31 @@ def test_fused_correct_predict_is_bitwise_the_two_launches(nb, n, nbdebug):
     for a, b in zip(out["1"][:5], out["0"][:5]):
         assert np.array_equal(a, b)
     assert out["0"][5] == out["1"][5] + 6          # steps 0 .. 5 close with two launches instead of one
+
+
+def test_default_stream_runs_take_the_step_graph_too(nb):
+    """As for nb_leapfrog_kdk (test_leapfrog_gpu.py): a long nb_hermite4 run on a default stream is moved to a private stream of
+    the device for the call; same bits and launches as on a side stream, and later default-stream work sees the result."""
+    import torch
+    w = wl.plummer_workload(1500, 1.0 / 64, seed=8, with_velocities=True)
+    out = {}
+    side = torch.cuda.Stream()
+    for where in ("default", "side"):
+        x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
+        x.mul_(1.0)
+        if where == "side":
+            torch.cuda.synchronize()
+            with torch.cuda.stream(side):
+                acc, jerk, pot = nb.hermite4(x, v, m, w.eps2, 1.0 / 256, 85)
+            torch.cuda.synchronize()
+            x_after = x.clone()
+        else:
+            acc, jerk, pot = nb.hermite4(x, v, m, w.eps2, 1.0 / 256, 85)
+            x_after = x.clone()
+            torch.cuda.synchronize()
+        out[where] = (x.cpu().numpy(), v.cpu().numpy(), acc.cpu().numpy(), jerk.cpu().numpy(), pot.cpu().numpy(), x_after.cpu().numpy(),
+                      nb.last_launch_count())
+    for a, b in zip(out["default"][:6], out["side"][:6]):
+        assert np.array_equal(a, b)
+    assert np.array_equal(out["default"][0], out["default"][5])
+    assert out["default"][6] == out["side"][6]

@@ -130,3 +130,31 @@ def test_step_graph_replay_is_bitwise_the_eager_sequence(nb, nbdebug):
     for a, b in zip(out["1"][:4], out["0"][:4]):
         assert np.array_equal(a, b)
     assert out["1"][4] == out["0"][4]
+
+
+def test_default_stream_runs_take_the_step_graph_too(nb):
+    """The default streams cannot be captured: a long run on one is moved to a private stream of the device for the call, with
+    the caller's stream order kept (it waits for what was enqueued before, the caller's later work waits for it).  Same bits
+    and the same launches as on a side stream; work enqueued on the default stream right after the call sees the result."""
+    import torch
+    w = wl.plummer_workload(1500, 1.0 / 64, seed=8, with_velocities=True)
+    out = {}
+    side = torch.cuda.Stream()
+    for where in ("default", "side"):
+        x, v, m = dev(w.x_j.copy()), dev(w.v.copy()), dev(w.m_j)
+        x.mul_(1.0)                                         # work on the default stream just before the call: the run must wait for it
+        if where == "side":
+            torch.cuda.synchronize()
+            with torch.cuda.stream(side):
+                acc, pot = nb.leapfrog_kdk(x, v, m, w.eps2, 1.0 / 256, 85)
+            torch.cuda.synchronize()
+            x_after = x.clone()
+        else:
+            acc, pot = nb.leapfrog_kdk(x, v, m, w.eps2, 1.0 / 256, 85)
+            x_after = x.clone()                             # enqueued on the default stream, no synchronize in between
+            torch.cuda.synchronize()
+        out[where] = (x.cpu().numpy(), v.cpu().numpy(), acc.cpu().numpy(), pot.cpu().numpy(), x_after.cpu().numpy(), nb.last_launch_count())
+    for a, b in zip(out["default"][:5], out["side"][:5]):
+        assert np.array_equal(a, b)
+    assert np.array_equal(out["default"][0], out["default"][4])
+    assert out["default"][5] == out["side"][5]
